@@ -1,0 +1,213 @@
+/* sdbg_oracle.c — TEST INFRASTRUCTURE ONLY. The plain, slow, single-threaded CPU definition of what
+ * the SdBG-construction hot path computes. Only tests/, __graft_entry__.smoke() and bench.py's
+ * cpu_baseline / --impl reference legs may build, link or call this file. It shares no code with the
+ * CUDA library (paper_1409_7208_b200/csrc): no headers, helpers, tables or pre/post-processing.
+ *
+ * The method reaches an exactly defined result (a sort + group-by), so this is that definition written
+ * out on strings, in the order of SURVEY.md §8(c) steps 1-6:
+ *
+ *  1. E <- []. For each read r, for i = 0 .. L_r-k-1: e <- r[i : i+k+1]; append e and rc(e) to E.
+ *     ("all (k+1)-mers from the input reads", §2 ¶3; both strands and the literal multiset
+ *     reading for palindromes: DESIGN.md readings A4, A5.)  Reads with L_r <= k add nothing (A6).
+ *  2. Sort E: compare a[k-1] vs b[k-1], a[k-2] vs b[k-2], ..., a[0] vs b[0] (A<C<G<T); if all equal,
+ *     a[k] vs b[k].  ("sorting a set of (k+1)-mers ... in reverse lexicographical order of their length-k
+ *     prefixes", §2 ¶2; colex-ascending reading A2, tie-break A3.)
+ *  3. Group equal strings; cnt(e) = group size.  ("sorted and counted".)
+ *  4. S <- groups with cnt >= d, in sorted order.  ("appear at least d (2 by default) times".)
+ *  5. For e = S[i]:  W[i] = e[k];  last[i] = (i == |S|-1) or S[i+1][0:k] != e[0:k];
+ *     minus[i] = exists j < i with S[j][1:k] == e[1:k] and S[j][k] == e[k];  mult[i] = cnt(e).
+ *     (SdBG / BOSS arrays, §2 ¶1, Bowe et al. 2012 PAPER.md:106; flag rules per
+ *     BASELINE.json north_star.)  Because S is sorted by (e[k-1],...,e[0],e[k]), all j with
+ *     S[j][1:k] == e[1:k] are contiguous and directly before i, so the scan over j stops at the first
+ *     j whose S[j][1:k] differs; the O(|S|^2) literal form is checked against this in the tests.
+ *  6. Encodings, only for comparison with the CUDA library: key(e) = symbols (e[k-1],...,e[0],e[k]) at
+ *     2 bits each (A0 C1 G2 T3), first symbol in the top bits of word 0, zero-padded low, w = ceil(2(k+1)/64)
+ *     words per key; W byte = 1 + code(e[k]), + 4 if minus; last packed LSB-first into u64 words.
+ *
+ * Optional restriction (large configs, SURVEY.md §8(c) "Large configs"): keep in step 1 only records whose
+ * key string (e[k-1],...,e[0],e[k]) begins with a given 8 symbols (one l=8 partition). Requires
+ * k >= 9, for which no `last`/minus dependency crosses a partition.
+ *
+ * Pins (tests/test_oracle_pins.py): hand-worked example T0 (tests/golden/t0_handworked.txt), complete
+ * de Bruijn closed form, independent Python brute force, count/closure invariants, numpy sort/unique.
+ * Parity unpinned: nothing.
+ */
+#define _GNU_SOURCE
+#include <stdint.h>
+#include <stdlib.h>
+#include <string.h>
+
+typedef struct orc {
+    uint32_t k, d;
+    int has_prefix;
+    char prefix[8];
+    /* step 1 */
+    char *E; uint64_t nE, capE;       /* records, (k+1) chars each */
+    uint64_t n_seen;                  /* records before the optional prefix restriction */
+    /* steps 3-5 */
+    uint64_t n_distinct, n_solid, sum_solid_mult;
+    char *D; uint32_t *Dcnt;          /* distinct edges + counts */
+    char *S; uint32_t *mult;          /* solid edges */
+    uint8_t *W, *last, *minus;
+} orc;
+
+enum { ORC_OK = 0, ORC_E_BADBASE = -2, ORC_E_NOMEM = -7, ORC_E_INVAL = -1 };
+
+orc *orc_new(uint32_t k, uint32_t d, const char *prefix8 /* NULL or 8 chars */) {
+    if (k < 1 || d < 1) return NULL;
+    if (prefix8 && k < 9) return NULL;
+    orc *o = (orc *)calloc(1, sizeof(orc));
+    if (!o) return NULL;
+    o->k = k; o->d = d;
+    if (prefix8) { o->has_prefix = 1; memcpy(o->prefix, prefix8, 8); }
+    return o;
+}
+
+void orc_free(orc *o) {
+    if (!o) return;
+    free(o->E); free(o->D); free(o->Dcnt); free(o->S); free(o->mult); free(o->W); free(o->last); free(o->minus);
+    free(o);
+}
+
+static char comp(char c) { return c == 'A' ? 'T' : c == 'C' ? 'G' : c == 'G' ? 'C' : 'A'; }
+
+static int push(orc *o, const char *e) {
+    const uint32_t k = o->k;
+    o->n_seen++;
+    if (o->has_prefix)               /* key string symbol t is e[k-1-t] for t < k */
+        for (uint32_t t = 0; t < 8; ++t) if (e[k - 1 - t] != o->prefix[t]) return ORC_OK;
+    if (o->nE == o->capE) {
+        uint64_t nc = o->capE ? o->capE * 2 : 1024;
+        char *p = (char *)realloc(o->E, nc * (k + 1));
+        if (!p) return ORC_E_NOMEM;
+        o->E = p; o->capE = nc;
+    }
+    memcpy(o->E + o->nE * (k + 1), e, k + 1);
+    o->nE++;
+    return ORC_OK;
+}
+
+/* Step 1 over n reads: read r is bases[offsets[r] .. offsets[r+1]). Lower-case acgt is folded to upper case;
+ * any other character fails with ORC_E_BADBASE (reading A7). May be called repeatedly (reads are a multiset). */
+int orc_add_reads(orc *o, const char *bases, const uint64_t *offsets, uint64_t n) {
+    const uint32_t k = o->k;
+    char *e = (char *)malloc(k + 1), *rc = (char *)malloc(k + 1);
+    char *rd = NULL; uint64_t rdcap = 0;
+    int st = ORC_OK;
+    if (!e || !rc) { free(e); free(rc); return ORC_E_NOMEM; }
+    for (uint64_t r = 0; r < n && st == ORC_OK; ++r) {
+        uint64_t L = offsets[r + 1] - offsets[r];
+        if (L > rdcap) { free(rd); rd = (char *)malloc(L); rdcap = L; if (!rd) { st = ORC_E_NOMEM; break; } }
+        for (uint64_t j = 0; j < L; ++j) {
+            char c = bases[offsets[r] + j];
+            if (c >= 'a' && c <= 'z') c = (char)(c - 'a' + 'A');
+            if (c != 'A' && c != 'C' && c != 'G' && c != 'T') { st = ORC_E_BADBASE; break; }
+            rd[j] = c;
+        }
+        if (st != ORC_OK) break;
+        for (uint64_t i = 0; i + k + 1 <= L && st == ORC_OK; ++i) {
+            memcpy(e, rd + i, k + 1);
+            for (uint32_t t = 0; t <= k; ++t) rc[t] = comp(e[k - t]);
+            st = push(o, e);
+            if (st == ORC_OK) st = push(o, rc);
+        }
+    }
+    free(e); free(rc); free(rd);
+    return st;
+}
+
+/* Step 2 comparator. */
+static int cmp_edges(const void *pa, const void *pb, void *ctx) {
+    const char *a = (const char *)pa, *b = (const char *)pb;
+    const uint32_t k = *(const uint32_t *)ctx;
+    for (uint32_t t = k; t-- > 0;) if (a[t] != b[t]) return a[t] < b[t] ? -1 : 1;
+    if (a[k] != b[k]) return a[k] < b[k] ? -1 : 1;
+    return 0;
+}
+
+int orc_finish(orc *o) {
+    const uint32_t k = o->k, R = k + 1;
+    /* 2 */
+    if (o->nE) qsort_r(o->E, o->nE, R, cmp_edges, &o->k);
+    /* 3: count groups */
+    uint64_t nd = 0;
+    for (uint64_t i = 0; i < o->nE; ++i) if (i == 0 || memcmp(o->E + i * R, o->E + (i - 1) * R, R) != 0) nd++;
+    o->n_distinct = nd;
+    o->D = (char *)malloc(nd * R + 1); o->Dcnt = (uint32_t *)malloc(nd * 4 + 4);
+    if (!o->D || !o->Dcnt) return ORC_E_NOMEM;
+    uint64_t g = 0;
+    for (uint64_t i = 0; i < o->nE;) {
+        uint64_t j = i + 1;
+        while (j < o->nE && memcmp(o->E + j * R, o->E + i * R, R) == 0) ++j;
+        memcpy(o->D + g * R, o->E + i * R, R);
+        uint64_t c = j - i;
+        o->Dcnt[g] = c > 0xffffffffull ? 0xffffffffu : (uint32_t)c;   /* A9: saturate */
+        ++g; i = j;
+    }
+    /* 4 */
+    uint64_t ns = 0;
+    for (uint64_t i = 0; i < nd; ++i) if (o->Dcnt[i] >= o->d) ns++;
+    o->n_solid = ns;
+    o->S = (char *)malloc(ns * R + 1); o->mult = (uint32_t *)malloc(ns * 4 + 4);
+    o->W = (uint8_t *)malloc(ns + 1); o->last = (uint8_t *)malloc(ns + 1); o->minus = (uint8_t *)malloc(ns + 1);
+    if (!o->S || !o->mult || !o->W || !o->last || !o->minus) return ORC_E_NOMEM;
+    uint64_t s = 0;
+    o->sum_solid_mult = 0;
+    for (uint64_t i = 0; i < nd; ++i) if (o->Dcnt[i] >= o->d) {
+        memcpy(o->S + s * R, o->D + i * R, R); o->mult[s] = o->Dcnt[i]; o->sum_solid_mult += o->Dcnt[i]; ++s;
+    }
+    /* 5 */
+    for (uint64_t i = 0; i < ns; ++i) {
+        const char *e = o->S + i * R;
+        o->W[i] = (uint8_t)e[k];
+        o->last[i] = (i == ns - 1) || memcmp(o->S + (i + 1) * R, e, k) != 0;
+        uint8_t m = 0;
+        for (uint64_t j = i; j-- > 0;) {
+            const char *f = o->S + j * R;
+            if (memcmp(f + 1, e + 1, k - 1) != 0) break;   /* S[j][1:k] != e[1:k]: no earlier j can match */
+            if (f[k] == e[k]) { m = 1; break; }
+        }
+        o->minus[i] = m;
+    }
+    return ORC_OK;
+}
+
+uint64_t orc_n_raw(const orc *o) { return o->nE; }
+uint64_t orc_n_seen(const orc *o) { return o->n_seen; }
+uint64_t orc_n_distinct(const orc *o) { return o->n_distinct; }
+uint64_t orc_n_solid(const orc *o) { return o->n_solid; }
+uint64_t orc_sum_solid_mult(const orc *o) { return o->sum_solid_mult; }
+const char *orc_sorted_raw(const orc *o) { return o->E; }
+const char *orc_distinct(const orc *o) { return o->D; }
+const uint32_t *orc_distinct_cnt(const orc *o) { return o->Dcnt; }
+const char *orc_solid(const orc *o) { return o->S; }
+const uint32_t *orc_mult(const orc *o) { return o->mult; }
+const uint8_t *orc_W(const orc *o) { return o->W; }
+const uint8_t *orc_last(const orc *o) { return o->last; }
+const uint8_t *orc_minus(const orc *o) { return o->minus; }
+
+static uint64_t code(char c) { return c == 'A' ? 0 : c == 'C' ? 1 : c == 'G' ? 2 : 3; }
+
+/* Step 6, key of one edge string: w words, symbol t of (e[k-1],...,e[0],e[k]) at bits [62-2(t%32), 63-2(t%32)] of word t/32. */
+void orc_encode_keys(const orc *o, const char *edges, uint64_t n, uint64_t *keys) {
+    const uint32_t k = o->k, R = k + 1, w = (2 * R + 63) / 64;
+    for (uint64_t i = 0; i < n; ++i) {
+        const char *e = edges + i * R;
+        uint64_t *kw = keys + i * w;
+        for (uint32_t j = 0; j < w; ++j) kw[j] = 0;
+        for (uint32_t t = 0; t <= k; ++t) {
+            char sym = t < k ? e[k - 1 - t] : e[k];
+            kw[t / 32] |= code(sym) << (62 - 2 * (t % 32));
+        }
+    }
+}
+
+/* Step 6, SdBG arrays of the solid edges. Wbyte[n_solid], last_bits[ceil(n_solid/64)]. */
+void orc_encode_graph(const orc *o, uint8_t *Wbyte, uint64_t *last_bits) {
+    uint64_t ns = o->n_solid;
+    for (uint64_t j = 0; j < (ns + 63) / 64; ++j) last_bits[j] = 0;
+    for (uint64_t i = 0; i < ns; ++i) {
+        Wbyte[i] = (uint8_t)(1 + code((char)o->W[i]) + (o->minus[i] ? 4 : 0));
+        if (o->last[i]) last_bits[i / 64] |= 1ull << (i % 64);
+    }
+}

@@ -1,0 +1,159 @@
+"""ctypes front-end of oracle/sdbg_oracle.c (the plain CPU definition; see that file's header for the
+step-by-step citation of PAPER.md). TEST INFRASTRUCTURE ONLY — never imported by the product path."""
+from __future__ import annotations
+
+import ctypes
+import os
+import subprocess
+from dataclasses import dataclass
+
+import numpy as np
+
+_DIR = os.path.dirname(os.path.abspath(__file__))
+_SRC = os.path.join(_DIR, "sdbg_oracle.c")
+_SO = os.path.join(_DIR, "libsdbg_oracle.so")
+_lib = None
+
+
+def build_oracle_lib(force: bool = False) -> str:
+    if force or not os.path.exists(_SO) or os.path.getmtime(_SRC) > os.path.getmtime(_SO):
+        subprocess.check_call(["gcc", "-O2", "-std=c11", "-shared", "-fPIC", "-o", _SO, _SRC])
+    return _SO
+
+
+def _load():
+    global _lib
+    if _lib is None:
+        L = ctypes.CDLL(build_oracle_lib())
+        vp, u64, u32 = ctypes.c_void_p, ctypes.c_uint64, ctypes.c_uint32
+        L.orc_new.argtypes = [u32, u32, ctypes.c_char_p]; L.orc_new.restype = vp
+        L.orc_free.argtypes = [vp]; L.orc_free.restype = None
+        L.orc_add_reads.argtypes = [vp, vp, vp, u64]; L.orc_add_reads.restype = ctypes.c_int
+        L.orc_finish.argtypes = [vp]; L.orc_finish.restype = ctypes.c_int
+        for f in ("n_raw", "n_seen", "n_distinct", "n_solid", "sum_solid_mult"):
+            getattr(L, "orc_" + f).argtypes = [vp]; getattr(L, "orc_" + f).restype = u64
+        for f in ("sorted_raw", "distinct", "distinct_cnt", "solid", "mult", "W", "last", "minus"):
+            getattr(L, "orc_" + f).argtypes = [vp]; getattr(L, "orc_" + f).restype = vp
+        L.orc_encode_keys.argtypes = [vp, vp, u64, vp]; L.orc_encode_keys.restype = None
+        L.orc_encode_graph.argtypes = [vp, vp, vp]; L.orc_encode_graph.restype = None
+        _lib = L
+    return _lib
+
+
+def _copy(ptr, n, dtype):
+    if n == 0 or not ptr:
+        return np.zeros(0, dtype=dtype)
+    nbytes = n * np.dtype(dtype).itemsize
+    return np.frombuffer(ctypes.string_at(ptr, nbytes), dtype=dtype).copy()
+
+
+@dataclass
+class OracleResult:
+    k: int
+    d: int
+    n_raw: int             # records kept in step 1 (after the optional partition restriction)
+    n_seen: int            # records of step 1 before that restriction (= N = 2*sum max(0, L_r-k))
+    n_distinct: int
+    n_solid: int
+    sum_solid_mult: int
+    distinct: np.ndarray       # (n_distinct, k+1) uint8 letters, sorted
+    distinct_cnt: np.ndarray   # u32
+    solid: np.ndarray          # (n_solid, k+1) uint8 letters, sorted
+    mult: np.ndarray           # u32
+    W: np.ndarray              # uint8 letters
+    last: np.ndarray           # uint8 0/1
+    minus: np.ndarray          # uint8 0/1
+    # step-6 encodings
+    keys: np.ndarray           # u64 (n_solid, w)
+    distinct_keys: np.ndarray  # u64 (n_distinct, w)
+    Wbyte: np.ndarray          # u8
+    last_bits: np.ndarray      # u64 ceil(n_solid/64)
+
+    @property
+    def w(self) -> int:
+        return (2 * (self.k + 1) + 63) // 64
+
+    def solid_strings(self):
+        return [bytes(r).decode() for r in self.solid]
+
+    def distinct_strings(self):
+        return [bytes(r).decode() for r in self.distinct]
+
+
+class Oracle:
+    """Steps 1-6 of sdbg_oracle.c. ``prefix``: optional 8-letter key-string prefix (one l=8 partition)."""
+
+    def __init__(self, k: int, d: int = 2, prefix: str | None = None):
+        L = _load()
+        self.k, self.d = int(k), int(d)
+        self._h = L.orc_new(self.k, self.d, prefix.encode() if prefix else None)
+        if not self._h:
+            raise ValueError("oracle: invalid k/d/prefix")
+
+    def add_reads(self, bases, offsets) -> None:
+        """bases: bytes / uint8 array of the concatenated reads; offsets: n+1 uint64 starts."""
+        b = np.frombuffer(bases, dtype=np.uint8) if isinstance(bases, (bytes, bytearray)) else np.ascontiguousarray(bases, dtype=np.uint8)
+        o = np.ascontiguousarray(offsets, dtype=np.uint64)
+        rc = _load().orc_add_reads(self._h, b.ctypes.data if b.size else None, o.ctypes.data, len(o) - 1)
+        if rc == -2:
+            raise ValueError("oracle: non-ACGT base")
+        if rc != 0:
+            raise MemoryError(f"oracle: error {rc}")
+
+    def finish(self, want_distinct: bool = True) -> OracleResult:
+        L = _load()
+        rc = L.orc_finish(self._h)
+        if rc != 0:
+            raise MemoryError(f"oracle: error {rc}")
+        h, k = self._h, self.k
+        R, w = k + 1, (2 * (k + 1) + 63) // 64
+        nd, ns = L.orc_n_distinct(h), L.orc_n_solid(h)
+        keys = np.zeros(ns * w, dtype=np.uint64)
+        L.orc_encode_keys(h, L.orc_solid(h), ns, keys.ctypes.data)
+        dkeys = np.zeros(nd * w if want_distinct else 0, dtype=np.uint64)
+        if want_distinct:
+            L.orc_encode_keys(h, L.orc_distinct(h), nd, dkeys.ctypes.data)
+        Wb = np.zeros(ns, dtype=np.uint8)
+        lb = np.zeros((ns + 63) // 64, dtype=np.uint64)
+        L.orc_encode_graph(h, Wb.ctypes.data, lb.ctypes.data)
+        return OracleResult(
+            k=k, d=self.d, n_raw=L.orc_n_raw(h), n_seen=L.orc_n_seen(h), n_distinct=nd, n_solid=ns,
+            sum_solid_mult=L.orc_sum_solid_mult(h),
+            distinct=_copy(L.orc_distinct(h), nd * R if want_distinct else 0, np.uint8).reshape(-1, R),
+            distinct_cnt=_copy(L.orc_distinct_cnt(h), nd, np.uint32),
+            solid=_copy(L.orc_solid(h), ns * R, np.uint8).reshape(-1, R),
+            mult=_copy(L.orc_mult(h), ns, np.uint32), W=_copy(L.orc_W(h), ns, np.uint8),
+            last=_copy(L.orc_last(h), ns, np.uint8), minus=_copy(L.orc_minus(h), ns, np.uint8),
+            keys=keys.reshape(-1, w), distinct_keys=dkeys.reshape(-1, w), Wbyte=Wb, last_bits=lb)
+
+    def close(self):
+        if self._h:
+            _load().orc_free(self._h)
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+
+def reads_to_arrays(reads):
+    """list of str -> (uint8 bases, uint64 offsets) — plain concatenation."""
+    offs = np.zeros(len(reads) + 1, dtype=np.uint64)
+    for i, r in enumerate(reads):
+        offs[i + 1] = offs[i] + np.uint64(len(r))
+    return np.frombuffer("".join(reads).encode(), dtype=np.uint8), offs
+
+
+def run_oracle(reads, k: int, d: int = 2, prefix: str | None = None) -> OracleResult:
+    """reads: list of str, or a (bases, offsets) pair."""
+    o = Oracle(k, d, prefix)
+    try:
+        if isinstance(reads, tuple):
+            o.add_reads(*reads)
+        else:
+            o.add_reads(*reads_to_arrays(list(reads)))
+        return o.finish()
+    finally:
+        o.close()

@@ -1,0 +1,97 @@
+"""Independent test-side restatements (brute force, de Bruijn sequences, checksum definition).
+These share no code with oracle/ or the CUDA library; they exist to pin both."""
+import numpy as np
+
+CODE = {"A": 0, "C": 1, "G": 2, "T": 3}
+COMP = {"A": "T", "C": "G", "G": "C", "T": "A"}
+
+
+def rc(s):
+    return "".join(COMP[c] for c in reversed(s))
+
+
+def brute_force(reads, k, d):
+    """Dict count + sorted() with the colex key + literal O(S^2) minus scan (pin P2)."""
+    cnt = {}
+    n = 0
+    for r in reads:
+        r = r.upper()
+        for i in range(len(r) - k):
+            e = r[i:i + k + 1]
+            for x in (e, rc(e)):
+                cnt[x] = cnt.get(x, 0) + 1
+                n += 1
+    distinct = sorted(cnt, key=lambda e: (e[:k][::-1], e[k]))
+    S = [e for e in distinct if cnt[e] >= d]
+    W = [e[k] for e in S]
+    last = [1 if (i == len(S) - 1 or S[i + 1][:k] != S[i][:k]) else 0 for i in range(len(S))]
+    minus = [1 if any(S[j][1:k] == S[i][1:k] and S[j][k] == S[i][k] for j in range(i)) else 0 for i in range(len(S))]
+    return dict(n_raw=n, distinct=distinct, cnt=[cnt[e] for e in distinct], solid=S, mult=[cnt[e] for e in S],
+                W=W, last=last, minus=minus)
+
+
+def key_words(e, k):
+    """Step-6 key of edge string e as a list of w python ints."""
+    w = (2 * (k + 1) + 63) // 64
+    sym = e[:k][::-1] + e[k]
+    v = 0
+    for c in sym:
+        v = (v << 2) | CODE[c]
+    v <<= 64 * w - 2 * (k + 1)
+    return [(v >> (64 * (w - 1 - j))) & (2 ** 64 - 1) for j in range(w)]
+
+
+def de_bruijn(alphabet, n):
+    """Linearised de Bruijn sequence B(|alphabet|, n) by the Lyndon-word (FKM) construction, plus the
+    n-1 wrap-around symbols, so that every n-mer occurs exactly once."""
+    q = len(alphabet)
+    a = [0] * (q * n)
+    seq = []
+
+    def db(t, p):
+        if t > n:
+            if n % p == 0:
+                seq.extend(a[1:p + 1])
+        else:
+            a[t] = a[t - p]
+            db(t + 1, p)
+            for j in range(a[t - p] + 1, q):
+                a[t] = j
+                db(t + 1, t)
+
+    db(1, 1)
+    s = "".join(alphabet[i] for i in seq)
+    return s + s[:n - 1]
+
+
+_M1 = 0xBF58476D1CE4E5B9
+_M2 = 0x94D049BB133111EB
+_MASK = 2 ** 64 - 1
+
+
+def mix64(z):
+    z &= _MASK
+    z = ((z ^ (z >> 30)) * _M1) & _MASK
+    z = ((z ^ (z >> 27)) * _M2) & _MASK
+    return z ^ (z >> 31)
+
+
+def key_mix(words):
+    """include/sdbg.h 'checksum of a key': h = 0; for each word, most significant first: h = mix64(h ^ word)."""
+    h = 0
+    for x in words:
+        h = mix64(h ^ int(x))
+    return h
+
+
+def key_mix_np(keys):
+    """vectorised key_mix over an (n, w) uint64 array."""
+    keys = np.ascontiguousarray(keys, dtype=np.uint64).reshape(len(keys), -1)
+    h = np.zeros(len(keys), dtype=np.uint64)
+    with np.errstate(over="ignore"):
+        for j in range(keys.shape[1]):
+            z = h ^ keys[:, j]
+            z = (z ^ (z >> np.uint64(30))) * np.uint64(_M1)
+            z = (z ^ (z >> np.uint64(27))) * np.uint64(_M2)
+            h = z ^ (z >> np.uint64(31))
+    return h

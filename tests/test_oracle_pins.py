@@ -1,0 +1,214 @@
+"""Pins of the CPU oracle against things other than itself (SURVEY.md §8(c) pins P0-P10). CPU only."""
+import os
+import random
+
+import numpy as np
+import pytest
+
+from oracle import run_oracle
+from tests.helpers import brute_force, de_bruijn, key_words, rc
+
+GOLDEN = os.path.join(os.path.dirname(__file__), "golden")
+T0_READS = ["ACGTTGCA", "CGTTGCAT", "TTGCATGA"]
+
+
+def _t0_rows():
+    rows = []
+    for line in open(os.path.join(GOLDEN, "t0_handworked.txt")):
+        if line.startswith("#") or not line.strip():
+            continue
+        rows.append(line.split())
+    return rows
+
+
+def test_P0_handworked_example():
+    """Every column of the hand-worked table: order, keys, counts, solid set, W, last, minus, bytes."""
+    rows = _t0_rows()
+    r = run_oracle(T0_READS, 3, 2)
+    assert (r.n_raw, r.n_seen, r.n_distinct, r.n_solid, r.sum_solid_mult) == (30, 30, 13, 11, 28)
+    assert r.distinct_strings() == [x[0] for x in rows]
+    assert list(r.distinct_cnt) == [int(x[3]) for x in rows]
+    assert [int(k) >> 56 for k in r.distinct_keys[:, 0]] == [int(x[2], 16) for x in rows]
+    solid = [x for x in rows if x[4] == "y"]
+    assert r.solid_strings() == [x[0] for x in solid]
+    assert list(r.mult) == [int(x[3]) for x in solid]
+    assert [chr(c) for c in r.W] == [x[5] for x in solid]
+    assert list(r.last) == [int(x[6]) for x in solid]
+    assert list(r.minus) == [int(x[7]) for x in solid]
+    assert list(r.Wbyte) == [int(x[8]) for x in solid]
+    assert int(r.last_bits[0]) == 0x7FD
+    # the key string column is the colex key: reversed node then outgoing base
+    for x in rows:
+        assert x[0][:3][::-1] + x[0][3] == x[1]
+
+
+@pytest.mark.parametrize("k", [1, 2, 3, 4, 5])
+def test_P1_complete_de_bruijn_closed_form(k):
+    """One read = linearised B(4, k+1): every (k+1)-mer has cnt exactly 2 (forward + its rc partner;
+    palindromes 1 occurrence x 2 under reading A5), so at d=2: S = 4^(k+1), W = ACGT repeating,
+    last = 0001 repeating, and in each 16-edge group the first 4 have minus=0, the other 12 minus=1."""
+    s = de_bruijn("ACGT", k + 1)
+    assert len(s) == 4 ** (k + 1) + k
+    r = run_oracle([s], k, 2)
+    S = 4 ** (k + 1)
+    assert r.n_raw == 2 * S and r.n_distinct == S and r.n_solid == S
+    assert np.all(r.distinct_cnt == 2)
+    assert bytes(r.W).decode() == "ACGT" * (S // 4)
+    assert list(r.last) == [0, 0, 0, 1] * (S // 4)
+    assert list(r.minus) == ([0] * 4 + [1] * 12) * (S // 16)
+    assert int(r.minus.sum()) == 3 * S // 4
+    # at d=3 nothing survives; at d=1 the same S edges
+    assert run_oracle([s], k, 3).n_solid == 0
+    assert run_oracle([s], k, 1).n_solid == S
+    # keys enumerate 0 .. 4^(k+1)-1 in order (every key string exactly once, ascending)
+    shift = 64 - 2 * (k + 1)
+    assert [int(x) >> shift for x in r.keys[:, 0]] == list(range(S))
+
+
+def _random_reads(rng, n, lo, hi, lower=False):
+    reads = ["".join(rng.choice("ACGT") for _ in range(rng.randint(lo, hi))) for _ in range(n)]
+    if lower:
+        reads = [r.lower() if i % 3 == 0 else r for i, r in enumerate(reads)]
+    return reads
+
+
+@pytest.mark.parametrize("k", list(range(1, 13)) + [15, 31, 32, 40])
+def test_P2_bruteforce_tiny(k):
+    """Independent Python brute force (dict count, sorted() on the colex key, literal O(S^2) minus)."""
+    rng = random.Random(1000 + k)
+    for trial in range(6):
+        # few distinct source strings so that counts >= 2 and branching nodes occur
+        base = _random_reads(rng, 3, k + 1, k + 30)
+        reads = []
+        for _ in range(rng.randint(0, 20)):
+            b = rng.choice(base)
+            i = rng.randint(0, len(b))
+            j = rng.randint(i, len(b))
+            x = b[i:j]
+            if rng.random() < 0.3:
+                x = rc(x)
+            if rng.random() < 0.3 and x:
+                p = rng.randrange(len(x))
+                x = x[:p] + rng.choice("ACGT") + x[p + 1:]
+            reads.append(x)
+        for d in (1, 2, 3):
+            bf = brute_force(reads, k, d)
+            r = run_oracle(reads, k, d)
+            assert r.n_raw == bf["n_raw"] == 2 * sum(max(0, len(x) - k) for x in reads)   # P3 closed form
+            assert r.distinct_strings() == bf["distinct"]
+            assert list(r.distinct_cnt) == bf["cnt"]
+            assert r.solid_strings() == bf["solid"]
+            assert list(r.mult) == bf["mult"]
+            assert [chr(c) for c in r.W] == bf["W"]
+            assert list(r.last) == bf["last"]
+            assert list(r.minus) == bf["minus"]
+            assert [list(map(int, row)) for row in r.keys] == [key_words(e, k) for e in bf["solid"]]
+            assert list(r.Wbyte) == [1 + "ACGT".index(w) + 4 * m for w, m in zip(bf["W"], bf["minus"])]
+            bits = 0
+            for i, l in enumerate(bf["last"]):
+                bits |= l << i
+            got = 0
+            for j, wd in enumerate(r.last_bits):
+                got |= int(wd) << (64 * j)
+            assert got == bits
+
+
+def _small_workload():
+    from workloads import ReadGenerator, get_config
+    g = ReadGenerator(get_config(1, scale=0.05))
+    return g.host()
+
+
+@pytest.mark.parametrize("k,d", [(21, 2), (11, 2), (31, 1), (33, 2), (63, 2)])
+def test_P3_P5_P6_P7_P9_invariants_on_synthetic(k, d):
+    bases, offs = _small_workload()
+    r = run_oracle((bases, offs), k, d)
+    L = np.diff(offs).astype(np.int64)
+    # P3: sum of counts = N = 2 * sum max(0, L-k)
+    N = 2 * int(np.maximum(L - k, 0).sum())
+    assert r.n_raw == N == int(r.distinct_cnt.astype(np.int64).sum())
+    assert r.sum_solid_mult + int(r.distinct_cnt[r.distinct_cnt < d].astype(np.int64).sum()) == N
+    # P5: keys strictly increasing as multiword integers; integer order == string comparator order
+    ints = [int.from_bytes(b"".join(int(x).to_bytes(8, "big") for x in row), "big") for row in r.distinct_keys]
+    assert all(a < b for a, b in zip(ints, ints[1:]))
+    ds = r.distinct_strings()
+    assert ds == sorted(ds, key=lambda e: (e[:k][::-1], e[k]))
+    assert [list(map(int, row)) for row in r.keys[:50]] == [key_words(e, k) for e in r.solid_strings()[:50]]
+    # P6: sum(last) = number of distinct k-prefixes among solid edges
+    S = r.solid_strings()
+    assert int(r.last.sum()) == len({e[:k] for e in S})
+    # P7: #(minus == 0) = number of distinct target k-mers e[1:k+1]
+    assert int((r.minus == 0).sum()) == len({e[1:] for e in S})
+    # P9: reverse-complement closure of the counts
+    cnt = dict(zip(ds, map(int, r.distinct_cnt)))
+    assert all(cnt.get(rc(e)) == c for e, c in cnt.items())
+    assert {rc(e) for e in S} == set(S)
+
+
+def test_P10_reduces_to_numpy_sort_and_unique():
+    """1-word keys: sorted distinct keys + counts == np.unique on the encoded raw keys."""
+    k = 21
+    bases, offs = _small_workload()
+    r = run_oracle((bases, offs), k, 1)
+    s = bytes(bases).decode()
+    code = np.array([{"A": 0, "C": 1, "G": 2, "T": 3}[c] for c in s], dtype=np.uint64)
+    raw = []
+    L = int(offs[1] - offs[0])
+    pw = [np.uint64(4) ** np.uint64(i) for i in range(k + 1)]
+    for r0 in offs[:-1].astype(np.int64):
+        c = code[r0:r0 + L]
+        for i in range(L - k):
+            e = c[i:i + k + 1]
+            # key value: symbols e[k-1..0] then e[k]
+            v = sum(int(e[k - 1 - t]) << (2 * (k - t)) for t in range(k)) + int(e[k])
+            raw.append(v)
+            f = (3 - e)[::-1]
+            raw.append(sum(int(f[k - 1 - t]) << (2 * (k - t)) for t in range(k)) + int(f[k]))
+    u, c = np.unique(np.array(raw, dtype=np.uint64), return_counts=True)
+    assert np.array_equal(u << np.uint64(64 - 2 * (k + 1)), r.distinct_keys[:, 0])
+    assert np.array_equal(c.astype(np.uint32), r.distinct_cnt)
+
+
+def test_error_free_tiling_gives_all_genome_edges():
+    """P10b: d=1 and error-free reads tiling a genome end to end => solid set = all (k+1)-mers of genome U rc."""
+    rng = random.Random(7)
+    G = "".join(rng.choice("ACGT") for _ in range(500))
+    k = 9
+    reads = [G[i:i + 60] for i in range(0, len(G) - 59, 10)] + [G[-60:]]
+    want = set()
+    for i in range(len(G) - k):
+        want.add(G[i:i + k + 1])
+        want.add(rc(G[i:i + k + 1]))
+    assert set(run_oracle(reads, k, 1).solid_strings()) == want
+
+
+def test_edge_cases():
+    assert run_oracle([], 5, 2).n_solid == 0
+    assert run_oracle(["ACG", "", "AC"], 5, 1).n_raw == 0                     # all reads shorter than k+1
+    r = run_oracle(["ACGTAC"], 5, 1)                                           # length exactly k+1
+    assert r.n_raw == 2 and sorted(r.solid_strings()) == sorted(["ACGTAC", "GTACGT"])
+    assert run_oracle(["ACGTAC"], 5, 2).n_solid == 0                           # d above every count
+    a = run_oracle(["acgttgca", "CGTTGCAT", "ttgcatga"], 3, 2)                 # case folding
+    b = run_oracle(T0_READS, 3, 2)
+    assert a.solid_strings() == b.solid_strings() and list(a.mult) == list(b.mult)
+    with pytest.raises(ValueError):
+        run_oracle(["ACGNACGT"], 3, 1)
+    r = run_oracle(["ACGT"] * 5, 3, 2)                                         # palindrome doubles (A5)
+    assert r.solid_strings() == ["ACGT"] and list(r.mult) == [10]
+
+
+def test_partition_restriction_matches_slice_of_full_run():
+    """The l=8 partition restriction yields exactly the slice of the full result (k >= 9)."""
+    bases, offs = _small_workload()
+    k = 21
+    full = run_oracle((bases, offs), k, 2)
+    S = full.solid_strings()
+    prefixes = sorted({e[:k][::-1][:8] for e in S})
+    for p in [prefixes[0], prefixes[len(prefixes) // 2], prefixes[-1]]:
+        part = run_oracle((bases, offs), k, 2, prefix=p)
+        idx = [i for i, e in enumerate(S) if e[:k][::-1][:8] == p]
+        assert part.solid_strings() == [S[i] for i in idx]
+        assert list(part.mult) == [int(full.mult[i]) for i in idx]
+        assert list(part.Wbyte) == [int(full.Wbyte[i]) for i in idx]
+        assert list(part.last) == [int(full.last[i]) for i in idx]
+        assert part.n_seen == full.n_raw
