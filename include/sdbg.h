@@ -1,0 +1,187 @@
+/* sdbg.h — C ABI of libsdbg: the data-parallel hot path of MEGAHIT's succinct de Bruijn graph (SdBG)
+ * construction (arxiv 1409.7208), as hand-written sm_100a CUDA kernels for one B200.
+ *
+ *   reads --sdbg_pack_reads--> 2-bit reads in HBM --sdbg_count_edges(k, d)--> sorted solid (k+1)-mers + counts
+ *         --sdbg_build--> SdBG arrays W (+minus flag), last, multiplicity
+ *
+ * What is computed (PAPER.md = /root/reference/PAPER.md; readings A1..A17 = DESIGN.md "Readings"):
+ *   - every (k+1)-mer ("edge") e = e[0..k] of every read, and its reverse complement, is a record
+ *     (§2 ¶3 "all (k+1)-mers from the input reads are sorted and counted"; both strands: A4, A5);
+ *   - records are sorted "in reverse lexicographical order of their length-k prefixes" (§2 ¶2):
+ *     ascending colex order of the node e[0..k), ties broken by the outgoing base e[k], with A<C<G<T (A1-A3);
+ *   - equal records are counted; "only (k+1)-mers that appear at least d (2 by default) times are kept"
+ *     (PAPER.md:35);
+ *   - the kept ("solid") edges, in sorted order, are the edge list of the SdBG (Bowe et al. 2012, PAPER.md:27-31,
+ *     :106): W[i] = outgoing base (+ minus flag), last[i] = 1 iff edge i is the last edge of its node,
+ *     mult[i] = multiplicity;
+ *   - when the records exceed the workspace, they are processed "block-wise": partitioned "according to their
+ *     length-l prefix (l=8 ...)", "consecutive partitions that fit within the GPU memory are sorted together"
+ *     (PAPER.md:33). The length-8 prefix is the prefix of the SORT KEY (A11): 4^8 = 65,536 partitions.
+ *
+ * Key encoding (what `sdbg_edges.keys` holds): w = ceil(2(k+1)/64) u64 words per edge, word 0 most significant.
+ * The k+1 symbols (e[k-1], e[k-2], ..., e[0], e[k]) are written at 2 bits each (A=0 C=1 G=2 T=3), first symbol
+ * in the top bits of word 0; the low 64w-2(k+1) bits of the last word are zero. Unsigned multi-word ascending
+ * order of keys == the sort order above. Partition ("bucket") of a key = top 16 bits of word 0.
+ *
+ * Memory: every pointer inside the structs below is a DEVICE pointer to memory owned by the caller; the library
+ * never allocates or frees device memory and uses only the workspace given to sdbg_ctx_create. `bases`/`offsets`
+ * of sdbg_pack_reads may be host or device pointers (detected). All work is enqueued on the context's stream.
+ * No exception crosses the ABI; every call returns SDBG_OK (0) or a negative sdbg_status. Not thread-safe per ctx.
+ * There is no CPU fallback: without a CUDA device every compute entry point fails with SDBG_E_CUDA.
+ */
+#ifndef SDBG_H
+#define SDBG_H
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum {
+    SDBG_OK = 0,
+    SDBG_E_INVAL = -1,       /* bad argument (null pointer, d == 0, n mismatch, misaligned buffer) */
+    SDBG_E_BADBASE = -2,     /* a read holds a character outside ACGTacgt (A7); sdbg_last_error names its index */
+    SDBG_E_CAPACITY = -3,    /* an output array is too small; the needed count is written to out->n */
+    SDBG_E_WORKSPACE = -4,   /* workspace too small (even one l=8 partition does not fit) */
+    SDBG_E_CUDA = -5,        /* CUDA runtime error; sdbg_last_error holds its text */
+    SDBG_E_UNSUPPORTED = -6  /* k outside [1, 127] */
+} sdbg_status;
+
+#define SDBG_MAX_K 127u
+#define SDBG_NUM_BUCKETS 65536u      /* 4^l, l = 8 */
+#define SDBG_READ_GUARD_SLOTS 256u   /* slack slots the packed-read buffers need after the last base */
+
+typedef struct sdbg_ctx sdbg_ctx;
+
+/* ---- context -------------------------------------------------------------------------------------------- */
+
+/* Binds a device, a CUDA stream (cudaStream_t passed as void*, NULL = legacy default stream) and a caller-owned
+ * device workspace. The workspace plays the role of MEGAHIT's "-m" memory budget: the sorter
+ * sizes its block-wise passes to it. workspace must be 256-byte aligned. */
+int sdbg_ctx_create(sdbg_ctx **ctx, int device, void *cuda_stream, void *workspace, uint64_t workspace_bytes);
+void sdbg_ctx_destroy(sdbg_ctx *ctx);
+const char *sdbg_strerror(int status);           /* static string */
+const char *sdbg_last_error(const sdbg_ctx *ctx); /* detail of the last failure on this ctx ("" if none) */
+
+/* ---- a1: pack reads ------------------------------------------------------------------------------------- */
+
+/* 2-bit packed reads, layout private to the library. `words` holds slots_cap/32 u64, `ends` slots_cap/64 u64.
+ * Zero-initialise the struct fields n_reads, n_bases, n_slots before the first sdbg_pack_reads call. */
+typedef struct {
+    uint64_t *words;     /* 2-bit bases, 32 per u64 */
+    uint64_t *ends;      /* 1 bit per base slot: read boundary / padding marks */
+    uint64_t slots_cap;  /* capacity in base slots; multiple of 64; see sdbg_read_slots */
+    uint64_t n_reads;    /* reads packed so far */
+    uint64_t n_bases;    /* bases packed so far */
+    uint64_t n_slots;    /* slots used so far (multiple of 64) */
+} sdbg_reads;
+
+/* slots_cap needed to pack n_bases bases with n_calls calls of sdbg_pack_reads (each call pads to 64 slots). */
+uint64_t sdbg_read_slots(uint64_t n_bases, uint64_t n_calls);
+
+/* a1: APPENDS n reads to `out`. Read r is bases[offsets[r] .. offsets[r+1]) — ASCII, one byte
+ * per base, upper or lower case; offsets has n+1 non-decreasing entries; bases and offsets are both host or both
+ * device pointers. Host input is staged through the workspace in chunks (H2D on the ctx stream). Encoding
+ * A=0 C=1 G=2 T=3 (A1); the 2-bit packing is what PAPER.md:31 implies ("2kt bits" for t k-mers).
+ * Synchronises the stream. Errors (the struct `out` is left unchanged by all of them): SDBG_E_BADBASE,
+ * SDBG_E_CAPACITY (slots_cap too small; sdbg_last_error states the needed value), SDBG_E_INVAL,
+ * SDBG_E_WORKSPACE (host input and no room to stage it). */
+int sdbg_pack_reads(sdbg_ctx *ctx, const char *bases, const uint64_t *offsets, uint64_t n, sdbg_reads *out);
+
+/* ---- a2-a4, a6: extract, sort, count, solid filter ------------------------------------------------------- */
+
+typedef struct {
+    uint64_t *keys;   /* n*w u64, record i at keys[i*w .. i*w+w), word 0 most significant */
+    uint32_t *mult;   /* n multiplicities (saturating at 2^32-1, A9) */
+    uint64_t cap;     /* capacity in edges of keys/mult */
+    uint64_t n;       /* out: number of edges */
+    uint32_t k;       /* out (count_edges) / in (build) */
+    uint32_t w;       /* out (count_edges) / in (build): ceil(2(k+1)/64) */
+} sdbg_edges;
+
+typedef struct {
+    uint64_t n_raw;            /* N = 2 * sum_r max(0, L_r - k) records extracted */
+    uint64_t n_distinct;       /* distinct records */
+    uint64_t n_solid;          /* distinct records with count >= d */
+    uint64_t sum_solid_mult;   /* sum of their (unsaturated) counts */
+    uint64_t n_ranges;         /* block-wise passes run (1 when everything fits) */
+    uint64_t max_range_records;/* records of the largest block-wise pass */
+    /* Order-independent checksums, computed only when want_checksums != 0 (they cost ALU time):
+     *   mixk(key) = fold h = mix64(h ^ word) over the key's words, most significant first, h0 = 0,
+     *   mix64 = the splitmix64 finaliser (z^=z>>30; z*=0xBF58476D1CE4E5B9; z^=z>>27; z*=0x94D049BB133111EB; z^=z>>31).
+     *   csum_raw      = sum over all N extracted records of mixk(key)            (mod 2^64), taken before sorting
+     *   csum_distinct = sum over distinct records of count * mixk(key)           (mod 2^64), taken after counting
+     * The sort/count lost or duplicated nothing iff the two agree (pin P4). */
+    uint64_t csum_raw, csum_distinct;
+    uint32_t want_checksums;   /* in */
+    uint32_t reserved;
+    uint64_t *bucket_hist;     /* in, optional device u64[65536]: raw records per l=8 partition (A11) */
+} sdbg_stats;
+
+/* Records per key and workspace sizing. sdbg_full_workspace: bytes with which sdbg_count_edges runs as ONE range
+ * (no block-wise passes) for reads with n_bases bases; sdbg_min_workspace: the fixed state plus room for a
+ * 64 Ki-record range of 4-word keys — sdbg_ctx_create refuses less with SDBG_E_WORKSPACE. */
+uint32_t sdbg_key_words(uint32_t k);
+uint64_t sdbg_full_workspace(uint64_t n_bases, uint32_t k);
+uint64_t sdbg_min_workspace(void);
+
+/* a2 extract + a3 sort + a4 count/filter (+ a6 block-wise planner).
+ * n must equal reads->n_reads. k in [1,127] else SDBG_E_UNSUPPORTED; d >= 1 else SDBG_E_INVAL (A8).
+ * Output: out->keys/mult hold the solid edges in sorted order, strictly increasing keys; out->n, out->k, out->w
+ * set. If out->cap < number of solid edges: SDBG_E_CAPACITY, out->n = needed count, contents unspecified.
+ * If the records do not fit the workspace they are processed in ranges of consecutive l=8 partitions chosen
+ * greedily from the 65,536-bin histogram (A12); the output does not depend on the plan. A single partition
+ * larger than the workspace gives SDBG_E_WORKSPACE. Synchronises the stream before returning. */
+int sdbg_count_edges(sdbg_ctx *ctx, const sdbg_reads *reads, uint64_t n, uint32_t k, uint32_t d,
+                     sdbg_edges *out, sdbg_stats *stats /* nullable */);
+
+/* a6 host logic, exposed for testing: greedy maximal runs of consecutive partitions whose record sum is
+ * <= capacity (A12). hist: HOST u64[65536]. Writes up to max_ranges triples (lo, hi, records) into
+ * ranges[3*i..3*i+3) with hi exclusive, skipping nothing (empty partitions join the current run).
+ * Returns the number of ranges, or SDBG_E_WORKSPACE if one partition exceeds capacity, or SDBG_E_CAPACITY if
+ * max_ranges is too small. */
+int64_t sdbg_plan_ranges(const uint64_t *hist, uint64_t capacity, uint64_t *ranges, uint64_t max_ranges);
+
+/* ---- a5: SdBG arrays ------------------------------------------------------------------------------------ */
+
+#define SDBG_SORTED 1u   /* edges->keys are strictly increasing (the output of sdbg_count_edges) */
+
+typedef struct {
+    uint8_t *W;           /* n bytes: 1..4 = outgoing base A,C,G,T; +4 when the minus flag is set; 0 reserved for '$' (A10) */
+    uint64_t *last_bits;  /* ceil(cap/64) u64, bit i%64 of word i/64 (LSB first) = last[i]; tail bits of the final word zero */
+    uint32_t *mult;       /* n multiplicities */
+    uint64_t cap;         /* capacity in edges */
+    uint64_t n;           /* out */
+} sdbg_graph;
+
+/* a5; SdBG definition, Bowe et al. 2012:
+ *   W[i]     = e[k] of edge i;
+ *   last[i]  = (i == n-1) or node(i+1) != node(i)                                   (A14)
+ *   minus[i] = exists j < i with e_j[1..k) == e_i[1..k) and e_j[k] == e_i[k]        (minus[0] = 0)
+ *   mult[i]  = edges->mult[i].
+ * With SDBG_SORTED the input is used as is (one streaming kernel; does not synchronise). Without it, edges may be
+ * in any order with repeats: they are sorted with the same radix sorter and equal keys are merged by summing mult
+ * (saturating at 2^32-1), so count_edges == build over raw records with mult 1 followed by the d filter. In that
+ * case edges->keys/mult are overwritten with the sorted, merged edges, edges->n is updated, and the call
+ * synchronises. Errors: SDBG_E_CAPACITY (out->n = needed), SDBG_E_WORKSPACE, SDBG_E_INVAL. */
+int sdbg_build(sdbg_ctx *ctx, sdbg_edges *edges, uint32_t flags, sdbg_graph *out);
+
+/* ---- measurement hooks ---------------------------------------------------------------------------------- */
+
+enum { SDBG_T_PACK = 0, SDBG_T_EXTRACT = 1, SDBG_T_RADIX = 2, SDBG_T_COUNT = 3, SDBG_T_EMIT = 4, SDBG_T_OTHER = 5, SDBG_T_NUM = 6 };
+
+typedef struct {
+    double ms[SDBG_T_NUM];          /* device time per kernel class, CUDA events on the ctx stream */
+    uint64_t launches[SDBG_T_NUM];  /* kernel launches per class */
+    uint64_t bytes[SDBG_T_NUM];     /* algorithmic bytes per class */
+} sdbg_timing;
+
+/* on != 0: bracket every kernel class with CUDA events (a few microseconds each). Launch counters always run. */
+int sdbg_ctx_set_timing(sdbg_ctx *ctx, int on);
+/* Synchronises the stream, adds up the event pairs recorded since the last call, writes and resets the totals. */
+int sdbg_ctx_get_timing(sdbg_ctx *ctx, sdbg_timing *out);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* SDBG_H */

@@ -1,0 +1,221 @@
+// api.cu — the C ABI of include/sdbg.h: context, workspace layout, block-wise pass planner (step a6) and the
+// sequencing of the kernels of pack.cu / extract.cu / radix.cu / count.cu / emit.cu. No device allocation happens
+// here: everything lives in the caller's workspace. There is no CPU fallback.
+#include "../../include/sdbg.h"
+#include "kernels.cuh"
+
+#include <algorithm>
+#include <cstdio>
+#include <cstring>
+#include <string>
+#include <vector>
+
+using namespace sdbg;
+
+namespace {
+
+constexpr u64 kAlign = 256;
+inline u64 align_up(u64 x, u64 a = kAlign) { return (x + a - 1) / a * a; }
+inline u64 *U64(uint64_t *p) { return reinterpret_cast<u64 *>(p); }
+inline const u64 *U64C(const uint64_t *p) { return reinterpret_cast<const u64 *>(p); }
+
+// fixed region at the start of the workspace
+constexpr u64 kOffState = 0;
+constexpr u64 kOffDigitHist = 1024;                                         // u64[kMaxPasses][256]
+constexpr u64 kOffBucketHist = kOffDigitHist + (u64)kMaxPasses * kRadix * 8;  // u64[65536]
+constexpr u64 kFixedBytes = (kOffBucketHist + (u64)SDBG_NUM_BUCKETS * 8 + 4095) / 4096 * 4096;
+static_assert(sizeof(DevState) <= 1024, "DevState must fit its slot");
+
+struct EventPair { int cls; cudaEvent_t a, b; };
+
+}  // namespace
+
+struct sdbg_ctx {
+    int device = 0;
+    cudaStream_t stream = nullptr;
+    char *ws = nullptr;
+    u64 ws_bytes = 0;
+    std::string err;
+    bool timing = false;
+    std::vector<EventPair> pending;
+    std::vector<cudaEvent_t> free_events;
+    sdbg_timing acc{};
+
+    DevState *st() const { return reinterpret_cast<DevState *>(ws + kOffState); }
+    u64 *digit_hist() const { return reinterpret_cast<u64 *>(ws + kOffDigitHist); }
+    u64 *bucket_hist() const { return reinterpret_cast<u64 *>(ws + kOffBucketHist); }
+    char *dyn() const { return ws + kFixedBytes; }
+    u64 dyn_bytes() const { return ws_bytes > kFixedBytes ? ws_bytes - kFixedBytes : 0; }
+
+    int fail(int code, const std::string &msg) { err = msg; return code; }
+    int cuda_fail(cudaError_t e, const char *what) {
+        err = std::string(what) + ": " + cudaGetErrorString(e);
+        return SDBG_E_CUDA;
+    }
+    cudaEvent_t get_event() {
+        if (!free_events.empty()) { cudaEvent_t e = free_events.back(); free_events.pop_back(); return e; }
+        cudaEvent_t e = nullptr;
+        cudaEventCreate(&e);
+        return e;
+    }
+};
+
+namespace {
+
+// RAII bracket of one kernel class: counts launches/bytes always, records events when timing is on.
+struct Timed {
+    sdbg_ctx *c; int cls; EventPair ep{};
+    Timed(sdbg_ctx *c_, int cls_, u64 launches, u64 bytes) : c(c_), cls(cls_) {
+        c->acc.launches[cls] += launches;
+        c->acc.bytes[cls] += bytes;
+        if (c->timing) { ep.cls = cls; ep.a = c->get_event(); ep.b = c->get_event(); cudaEventRecord(ep.a, c->stream); }
+    }
+    ~Timed() {
+        if (c->timing) { cudaEventRecord(ep.b, c->stream); c->pending.push_back(ep); }
+    }
+};
+
+#define CU(call)                                                        \
+    do {                                                                \
+        cudaError_t e__ = (call);                                       \
+        if (e__ != cudaSuccess) return ctx->cuda_fail(e__, #call);      \
+    } while (0)
+
+PassTable make_passes(u32 k) {
+    PassTable pt{};
+    const u32 W = (2 * (k + 1) + 63) / 64;
+    const u32 pad = 64 * W - 2 * (k + 1);
+    for (int w = (int)W - 1; w >= 0; --w) {
+        u32 lo = (w == (int)W - 1) ? pad : 0;
+        while (lo < 64) {
+            u32 bits = std::min<u32>(kRadixBits, 64 - lo);
+            pt.p[pt.n++] = PassDesc{(uint8_t)w, (uint8_t)lo, (uint8_t)bits, 0};
+            lo += bits;
+        }
+    }
+    return pt;
+}
+
+bool is_device_ptr(const void *p) {
+    cudaPointerAttributes at{};
+    if (cudaPointerGetAttributes(&at, p) != cudaSuccess) { cudaGetLastError(); return false; }
+    return at.type == cudaMemoryTypeDevice || at.type == cudaMemoryTypeManaged;
+}
+
+// bytes of dynamic workspace a sort+count of n records needs (keys only)
+u64 range_need(u64 n, u32 W) {
+    const u64 K = 8ull * W;
+    const u64 rt = radix_tile_records(W, false), ct = count_tile_records(W);
+    return 2 * align_up(n * K) + align_up(((n + rt - 1) / rt + 1) * kRadix * 8) + align_up(((n + ct - 1) / ct + 1) * 2 * 8);
+}
+// largest n with range_need(n) <= avail
+u64 range_capacity(u64 avail, u32 W) {
+    u64 lo = 0, hi = avail / (16ull * W) + 1;
+    while (lo < hi) {
+        u64 mid = lo + (hi - lo + 1) / 2;
+        if (range_need(mid, W) <= avail) lo = mid; else hi = mid - 1;
+    }
+    return lo;
+}
+
+}  // namespace
+
+extern "C" {
+
+const char *sdbg_strerror(int status) {
+    switch (status) {
+        case SDBG_OK: return "ok";
+        case SDBG_E_INVAL: return "invalid argument";
+        case SDBG_E_BADBASE: return "read contains a character outside ACGTacgt";
+        case SDBG_E_CAPACITY: return "output capacity too small";
+        case SDBG_E_WORKSPACE: return "workspace too small";
+        case SDBG_E_CUDA: return "CUDA error";
+        case SDBG_E_UNSUPPORTED: return "unsupported k (must be in [1, 127])";
+    }
+    return "unknown status";
+}
+
+const char *sdbg_last_error(const sdbg_ctx *ctx) { return ctx ? ctx->err.c_str() : ""; }
+
+int sdbg_ctx_create(sdbg_ctx **out, int device, void *cuda_stream, void *workspace, uint64_t workspace_bytes) {
+    if (!out) return SDBG_E_INVAL;
+    *out = nullptr;
+    if (!workspace || (reinterpret_cast<uintptr_t>(workspace) & (kAlign - 1))) return SDBG_E_INVAL;
+    if (workspace_bytes < sdbg_min_workspace()) return SDBG_E_WORKSPACE;
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || device < 0 || device >= ndev) { cudaGetLastError(); return SDBG_E_CUDA; }
+    if (cudaSetDevice(device) != cudaSuccess) return SDBG_E_CUDA;
+    if (radix_setup() != 0) { cudaGetLastError(); return SDBG_E_CUDA; }
+    sdbg_ctx *c = new sdbg_ctx();
+    c->device = device;
+    c->stream = (cudaStream_t)cuda_stream;
+    c->ws = (char *)workspace;
+    c->ws_bytes = workspace_bytes;
+    *out = c;
+    return SDBG_OK;
+}
+
+void sdbg_ctx_destroy(sdbg_ctx *ctx) {
+    if (!ctx) return;
+    for (auto &p : ctx->pending) { cudaEventDestroy(p.a); cudaEventDestroy(p.b); }
+    for (auto e : ctx->free_events) cudaEventDestroy(e);
+    delete ctx;
+}
+
+int sdbg_ctx_set_timing(sdbg_ctx *ctx, int on) {
+    if (!ctx) return SDBG_E_INVAL;
+    ctx->timing = on != 0;
+    return SDBG_OK;
+}
+
+int sdbg_ctx_get_timing(sdbg_ctx *ctx, sdbg_timing *out) {
+    if (!ctx || !out) return SDBG_E_INVAL;
+    CU(cudaStreamSynchronize(ctx->stream));
+    for (auto &p : ctx->pending) {
+        float ms = 0.f;
+        if (cudaEventElapsedTime(&ms, p.a, p.b) == cudaSuccess) ctx->acc.ms[p.cls] += ms;
+        ctx->free_events.push_back(p.a);
+        ctx->free_events.push_back(p.b);
+    }
+    ctx->pending.clear();
+    *out = ctx->acc;
+    ctx->acc = sdbg_timing{};
+    return SDBG_OK;
+}
+
+uint32_t sdbg_key_words(uint32_t k) { return (2 * (k + 1) + 63) / 64; }
+
+uint64_t sdbg_read_slots(uint64_t n_bases, uint64_t n_calls) {
+    return (n_bases + 64 * std::max<u64>(n_calls, 1) + 63) / 64 * 64 + SDBG_READ_GUARD_SLOTS;
+}
+
+uint64_t sdbg_min_workspace(void) { return kFixedBytes + range_need(1ull << 16, 4); }
+
+uint64_t sdbg_full_workspace(uint64_t n_bases, uint32_t k) {
+    if (k < 1 || k > SDBG_MAX_K) return 0;
+    const u64 need = kFixedBytes + range_need(2 * n_bases, sdbg_key_words(k)) + 4096;
+    return std::max<u64>(need, sdbg_min_workspace());
+}
+
+int64_t sdbg_plan_ranges(const uint64_t *hist, uint64_t capacity, uint64_t *ranges, uint64_t max_ranges) {
+    if (!hist || !ranges) return SDBG_E_INVAL;
+    u64 nr = 0, lo = 0, sum = 0;
+    for (u64 b = 0; b < SDBG_NUM_BUCKETS; ++b) {
+        if (hist[b] > capacity) return SDBG_E_WORKSPACE;
+        if (sum + hist[b] > capacity) {   // close [lo, b)
+            if (nr == max_ranges) return SDBG_E_CAPACITY;
+            ranges[3 * nr] = lo; ranges[3 * nr + 1] = b; ranges[3 * nr + 2] = sum; ++nr;
+            lo = b; sum = 0;
+        }
+        sum += hist[b];
+    }
+    if (nr == max_ranges) return SDBG_E_CAPACITY;
+    ranges[3 * nr] = lo; ranges[3 * nr + 1] = SDBG_NUM_BUCKETS; ranges[3 * nr + 2] = sum; ++nr;
+    return (int64_t)nr;
+}
+
+}  // extern "C"
+
+#include "api_pack.inc"
+#include "api_count.inc"
+#include "api_build.inc"

@@ -1,0 +1,200 @@
+// extract.cu — step a2: every (k+1)-window of the packed reads -> two sort keys (forward edge and
+// its reverse complement; "all (k+1)-mers from the input reads", both strands per reading A4/A5),
+// with the digit histograms of all LSD passes and the 65,536-bin l=8 partition histogram fused in.
+//
+// Key of edge e = symbols (e[k-1],...,e[0],e[k]) MSB-first (include/sdbg.h). For the window e at slot p:
+//   forward key : reversed node ++ e[k]          = rot(Y),  Y = (e[k], e[k-1], ..., e[0]) taken from the
+//                                                  2-bit-group-reversed word stream;
+//   rc key      : (c(e[1]),...,c(e[k]),c(e[0]))  = rot(~win), win = (e[0],...,e[k]) taken from the forward stream;
+// where rot moves the first symbol of a (k+1)-symbol string to its end (identity checked in the tests against
+// the string oracle). One thread owns 32 consecutive slots, one warp 1024; keys leave the warp in coalesced
+// runs at a position reserved with one atomicAdd per warp (the order of raw records is irrelevant: they are sorted).
+#include "kernels.cuh"
+
+namespace sdbg {
+
+__device__ __forceinline__ u64 rev2(u64 x) {   // reverse the order of the 32 2-bit groups
+    u32 lo = (u32)x, hi = (u32)(x >> 32);
+    u64 y = ((u64)__brev(lo) << 32) | (u64)__brev(hi);
+    return ((y >> 1) & 0x5555555555555555ull) | ((y & 0x5555555555555555ull) << 1);
+}
+// top 64 bits of the 128-bit value (hi:lo) << s, s in [0, 63]
+__device__ __forceinline__ u64 funnel(u64 hi, u64 lo, u32 s) { return s ? ((hi << s) | (lo >> (64 - s))) : hi; }
+
+template <int W>
+struct KeyMaker {
+    u64 B[W + 1];    // forward stream: slots 32g .. 32g+32(W+1)
+    u64 R[W + 1];    // reversed stream, pre-shifted so that Y_i starts at symbol 31-i
+    u32 k;
+    u64 lastmask;
+
+    __device__ __forceinline__ void load(const u64 *__restrict__ words, u64 g, u32 k_) {
+        k = k_;
+        lastmask = ~0ull << (64 * W - 2 * (k + 1));
+#pragma unroll
+        for (int j = 0; j <= W; ++j) B[j] = __ldg(words + g + j);
+        u64 T[W + 2];
+#pragma unroll
+        for (int j = 0; j <= W; ++j) T[j] = rev2(B[W - j]);
+        T[W + 1] = 0;
+        const u32 q0 = 32 * (W + 1) - k - 32;   // 1..32 symbols
+        if (q0 == 32) {
+#pragma unroll
+            for (int j = 0; j <= W; ++j) R[j] = T[j + 1];
+        } else {
+#pragma unroll
+            for (int j = 0; j <= W; ++j) R[j] = funnel(T[j], T[j + 1], 2 * q0);
+        }
+    }
+    // rot: first symbol of the (k+1)-symbol string to its end
+    __device__ __forceinline__ void rot(const u64 (&V)[W], u64 (&out)[W]) const {
+        const u64 top = V[0] >> 62;
+#pragma unroll
+        for (int j = 0; j < W; ++j) out[j] = (V[j] << 2) | (j + 1 < W ? (V[j + 1] >> 62) : 0ull);
+        out[W - 1] |= top << (62 - 2 * (k & 31));
+    }
+    __device__ __forceinline__ void keys(u32 i, u64 (&fwd)[W], u64 (&rc)[W]) const {
+        u64 win[W], Y[W];
+        const u32 s = 2 * i, t = 2 * (31 - i);
+#pragma unroll
+        for (int j = 0; j < W; ++j) {
+            win[j] = ~funnel(B[j], B[j + 1], s);
+            Y[j] = funnel(R[j], R[j + 1], t);
+        }
+        win[W - 1] &= lastmask;
+        Y[W - 1] &= lastmask;
+        rot(Y, fwd);
+        rot(win, rc);
+    }
+};
+
+template <int W>
+__device__ __forceinline__ void store_key(u64 *__restrict__ out, u64 pos, const u64 (&key)[W]) {
+    if constexpr (W == 1) {
+        out[pos] = key[0];
+    } else if constexpr (W == 2) {
+        *reinterpret_cast<ulonglong2 *>(out + pos * 2) = make_ulonglong2(key[0], key[1]);
+    } else if constexpr (W == 4) {
+        *reinterpret_cast<ulonglong2 *>(out + pos * 4) = make_ulonglong2(key[0], key[1]);
+        *reinterpret_cast<ulonglong2 *>(out + pos * 4 + 2) = make_ulonglong2(key[2], key[3]);
+    } else {
+#pragma unroll
+        for (int j = 0; j < W; ++j) out[pos * W + j] = key[j];
+    }
+}
+
+template <int W, bool FILTER>
+__global__ void __launch_bounds__(256) extract_kernel(ExtractArgs a, DevState *st) {
+    extern __shared__ u32 s_hist[];   // [n_passes][256] when digit_hist != nullptr
+    const int np = a.passes.n;
+    const bool do_hist = a.digit_hist != nullptr;
+    if (do_hist) {
+        for (int i = threadIdx.x; i < np * kRadix; i += blockDim.x) s_hist[i] = 0;
+        __syncthreads();
+    }
+    const u64 ngroups = a.n_slots / 32;
+    const u32 lane = lane_id();
+    const u32 lt = lanemask_lt();
+    u64 csum = 0;
+
+    // warp-granular grid-stride loop: warp handles groups [32*wg, 32*wg+32)
+    const u64 nwarp_groups = (ngroups + 31) / 32;
+    const u64 warps_total = (u64)gridDim.x * (blockDim.x >> 5);
+    for (u64 wg = (u64)blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5); wg < nwarp_groups; wg += warps_total) {
+        const u64 g = wg * 32 + lane;
+        u32 valid = (g < ngroups) ? valid_mask32(a.ends, g, a.k) : 0u;
+        if (__ballot_sync(0xffffffffu, valid != 0) == 0) continue;
+        KeyMaker<W> km;
+        km.load(a.words, g < ngroups ? g : 0, a.k);
+
+        u32 vf = valid, vr = valid;   // per-strand keep masks
+        if (FILTER) {
+            vf = 0; vr = 0;
+            for (u32 i = 0; i < 32; ++i) {
+                if (!((valid >> i) & 1)) continue;
+                u64 f[W], r[W];
+                km.keys(i, f, r);
+                u32 bf = (u32)(f[0] >> 48), br = (u32)(r[0] >> 48);
+                if (bf >= a.bucket_lo && bf < a.bucket_hi) vf |= 1u << i;
+                if (br >= a.bucket_lo && br < a.bucket_hi) vr |= 1u << i;
+            }
+        }
+        u64 base = 0;
+        if (a.keys_out) {
+            u32 cnt = __popc(vf) + __popc(vr);
+            u32 incl = warp_incl_scan_add(cnt);
+            u32 total = __shfl_sync(0xffffffffu, incl, 31);
+            if (lane == 0 && total) base = atomicAdd(&st->extract_cursor, (u64)total);
+            base = __shfl_sync(0xffffffffu, base, 0);
+            if (base + total > a.out_cap) continue;   // cannot happen when the caller sized out_cap from the histogram
+        }
+        const u32 any_mask = __reduce_or_sync(0xffffffffu, valid);
+        for (u32 i = 0; i < 32; ++i) {
+            if (!((any_mask >> i) & 1)) continue;     // warp-uniform
+            const bool kf = (vf >> i) & 1, kr = (vr >> i) & 1;
+            u64 f[W], r[W];
+            km.keys(i, f, r);
+            if (a.keys_out) {
+                const u32 mf = __ballot_sync(0xffffffffu, kf), mr = __ballot_sync(0xffffffffu, kr);
+                if (kf) store_key<W>(a.keys_out, base + __popc(mf & lt), f);
+                base += __popc(mf);
+                if (kr) store_key<W>(a.keys_out, base + __popc(mr & lt), r);
+                base += __popc(mr);
+            }
+            if (do_hist) {
+#pragma unroll 1
+                for (int p = 0; p < np; ++p) {
+                    const PassDesc pd = a.passes.p[p];
+                    const u32 m = (1u << pd.bits) - 1u;
+                    if (kf) atomicAdd(&s_hist[p * kRadix + ((u32)(f[pd.word] >> pd.shift) & m)], 1u);
+                    if (kr) atomicAdd(&s_hist[p * kRadix + ((u32)(r[pd.word] >> pd.shift) & m)], 1u);
+                }
+            }
+            if (a.bucket_hist && ((valid >> i) & 1)) {
+                atomicAdd(&a.bucket_hist[f[0] >> 48], 1ull);
+                atomicAdd(&a.bucket_hist[r[0] >> 48], 1ull);
+            }
+            if (a.want_csum) {
+                if (kf) csum += mix_key<W>(f);
+                if (kr) csum += mix_key<W>(r);
+            }
+        }
+    }
+    if (a.want_csum) {
+        csum = warp_reduce_add64(csum);
+        if (lane == 0 && csum) atomicAdd(&st->csum_raw, csum);
+    }
+    if (do_hist) {
+        __syncthreads();
+        for (int i = threadIdx.x; i < np * kRadix; i += blockDim.x) {
+            u32 v = s_hist[i];
+            if (v) atomicAdd(&a.digit_hist[i], (u64)v);
+        }
+    }
+}
+
+template <int W>
+static int launch_extract_w(const ExtractArgs &a, DevState *st, cudaStream_t s) {
+    const u64 ngroups = a.n_slots / 32;
+    if (ngroups == 0) return 0;
+    const bool filter = !(a.bucket_lo == 0 && a.bucket_hi >= 65536);
+    u64 blocks = (ngroups + 255) / 256;
+    const u64 maxb = (u64)kNumSMs * 8;
+    if (blocks > maxb) blocks = maxb;
+    size_t smem = a.digit_hist ? (size_t)a.passes.n * kRadix * sizeof(u32) : 0;
+    if (filter) extract_kernel<W, true><<<(unsigned)blocks, 256, smem, s>>>(a, st);
+    else        extract_kernel<W, false><<<(unsigned)blocks, 256, smem, s>>>(a, st);
+    return (int)cudaGetLastError();
+}
+
+int launch_extract(const ExtractArgs &a, DevState *st, cudaStream_t s) {
+    switch (a.W) {
+        case 1: return launch_extract_w<1>(a, st, s);
+        case 2: return launch_extract_w<2>(a, st, s);
+        case 3: return launch_extract_w<3>(a, st, s);
+        case 4: return launch_extract_w<4>(a, st, s);
+    }
+    return (int)cudaErrorInvalidValue;
+}
+
+}  // namespace sdbg

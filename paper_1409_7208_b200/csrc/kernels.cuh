@@ -1,0 +1,101 @@
+// kernels.cuh — launch prototypes of the libsdbg kernels and the device helpers several of them share.
+#pragma once
+#include "common.cuh"
+
+namespace sdbg {
+
+// Valid-window mask of slots [32g, 32g+32): bit b set iff no end mark lies in [32g+b, 32g+b+k), i.e. the (k+1)-window
+// starting there lies inside one read. Reads ends words up to (32g+32+k)/64 (the guard slots keep that in bounds).
+__device__ __forceinline__ u32 valid_mask32(const u64 *__restrict__ ends, u64 g, u32 k) {
+    const u64 wi = g >> 1;
+    const u32 sh = (u32)(g & 1) * 32;
+    u64 e0 = __ldg(ends + wi), e1 = __ldg(ends + wi + 1), e2 = 0, e3 = 0;
+    if (sh + 31 + k > 128) { e2 = __ldg(ends + wi + 2); }
+    if (sh + 31 + k > 192) { e3 = __ldg(ends + wi + 3); }
+    u64 v0, v1, v2;
+    if (sh) {
+        v0 = (e0 >> 32) | (e1 << 32); v1 = (e1 >> 32) | (e2 << 32); v2 = (e2 >> 32) | (e3 << 32);
+    } else {
+        v0 = e0; v1 = e1; v2 = e2;
+    }
+    // smear: bit b of v0 becomes OR of original bits b .. b+k-1
+    u32 cover = 1;
+    while (cover * 2 <= k) {
+        v0 |= (v0 >> cover) | (v1 << (64 - cover));
+        v1 |= (v1 >> cover) | (v2 << (64 - cover));
+        v2 |= (v2 >> cover);
+        cover *= 2;
+    }
+    if (cover < k) {
+        const u32 m = k - cover;   // 1..63
+        v0 |= (v0 >> m) | (v1 << (64 - m));
+    }
+    return ~(u32)v0;
+}
+
+// ---- launchers (host) ----------------------------------------------------------------------------------
+void launch_pack(const unsigned char *d_ascii, u64 nb, u64 *words, u64 slot0, u64 err_index_base, DevState *st, cudaStream_t s);
+void launch_mark_ends(const u64 *d_offsets, u64 n, u64 off0, u64 nb, u64 *ends, u64 slot0, DevState *st, cudaStream_t s);
+void launch_count_windows(const u64 *ends, u64 n_slots, u32 k, DevState *st, cudaStream_t s);
+
+struct ExtractArgs {
+    const u64 *words, *ends;
+    u64 n_slots;
+    u32 k, W;
+    u32 bucket_lo, bucket_hi;     // keep keys with bucket in [lo, hi); full range = [0, 65536)
+    u64 *keys_out;                // nullptr: histogram-only
+    u64 out_cap;                  // records keys_out can hold
+    u64 *digit_hist;              // nullptr or u64[n_passes][256], accumulated
+    u64 *bucket_hist;             // nullptr or u64[65536], accumulated (all buckets, ignores lo/hi)
+    int want_csum;
+    PassTable passes;
+};
+int launch_extract(const ExtractArgs &a, DevState *st, cudaStream_t s);
+
+// exclusive scan of each pass's 256-bin histogram, in place (u64)
+void launch_scan_hist(u64 *digit_hist, int n_passes, cudaStream_t s);
+
+struct RadixArgs {
+    const u64 *keys_in; u64 *keys_out;
+    const u32 *vals_in; u32 *vals_out;   // nullptr: keys only
+    u64 n; u32 W;
+    const u64 *bin_base;                 // u64[256] exclusive bases of this pass
+    u64 *lookback;                       // u64[tiles*256], zeroed once per sort; epoch-tagged per pass
+    u32 *ticket;                         // zeroed
+    PassDesc pass; u32 epoch;
+};
+u64 radix_tile_records(u32 W, bool has_vals);
+int launch_radix_pass(const RadixArgs &a, cudaStream_t s);
+int radix_setup();   // sets max dynamic shared memory attributes; once per process
+
+// keys-only digit histograms over an existing key array (sdbg_build unsorted path)
+void launch_key_hist(const u64 *keys, u64 n, u32 W, const PassTable &pt, u64 *digit_hist, cudaStream_t s);
+
+struct CountArgs {
+    const u64 *keys; u64 n; u32 W, d;
+    u64 *out_keys; u32 *out_mult; u64 out_cap;
+    u64 *lookback;           // u64[2*tiles], zeroed
+    u32 *ticket;             // zeroed
+    int want_csum;
+    int range_parity;        // reads st->out_cursor[parity], writes st->out_cursor[parity^1]
+};
+u64 count_tile_records(u32 W);
+int launch_count_filter(const CountArgs &a, DevState *st, cudaStream_t s);
+
+struct EmitArgs {
+    const u64 *keys; const u32 *mult_in; u64 n; u32 k, W;
+    uint8_t *Wout; u32 *last_bits32; u32 *mult_out;
+};
+void launch_emit(const EmitArgs &a, cudaStream_t s);
+
+// sdbg_build unsorted path: merge equal adjacent keys of a sorted (key, mult) list, summing mult (saturating).
+struct MergeArgs {
+    const u64 *keys; const u32 *mult; u64 n; u32 W;
+    u64 *out_keys; u32 *out_mult;        // capacity n
+    u64 *lookback; u32 *ticket;          // u64[tiles], zeroed
+    u64 *acc;                            // u64[n] scratch accumulators, zeroed
+};
+u64 merge_tile_records();
+void launch_merge(const MergeArgs &a, DevState *st, cudaStream_t s);
+
+}  // namespace sdbg

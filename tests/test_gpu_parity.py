@@ -1,0 +1,179 @@
+"""-m gpu: the CUDA path (through the C ABI binding) against the CPU oracle, element by element, bit-exact."""
+import random
+
+import numpy as np
+import pytest
+
+from oracle import run_oracle
+from tests.gpu_util import assert_matches_oracle, run_gpu, to_arrays
+from tests.helpers import de_bruijn, key_mix_np, rc
+
+pytestmark = pytest.mark.gpu
+
+T0_READS = ["ACGTTGCA", "CGTTGCAT", "TTGCATGA"]
+ALL_K = [1, 2, 3, 5, 8, 9, 12, 15, 16, 21, 30, 31, 32, 33, 47, 62, 63, 64, 65, 95, 96, 99, 126, 127]
+
+
+def _ragged_reads(rng, k, n_src=4, n_reads=60):
+    """Reads cut from a few source strings (so counts >= 2 and branching occur), some reverse-complemented, some with
+    a substitution, some shorter than k+1 or empty, some lower case."""
+    src = ["".join(rng.choice("ACGT") for _ in range(rng.randint(k + 1, k + 90))) for _ in range(n_src)]
+    reads = []
+    for i in range(n_reads):
+        b = rng.choice(src)
+        a = rng.randint(0, len(b))
+        e = rng.randint(a, len(b))
+        x = b[a:e]
+        if rng.random() < 0.4:
+            x = rc(x)
+        if x and rng.random() < 0.3:
+            p = rng.randrange(len(x))
+            x = x[:p] + rng.choice("ACGT") + x[p + 1:]
+        if i % 5 == 0:
+            x = x.lower()
+        reads.append(x)
+    return reads
+
+
+def test_T0_handworked():
+    res = run_gpu(T0_READS, 3, 2)
+    orc = run_oracle(T0_READS, 3, 2)
+    assert_matches_oracle(res, orc)
+    assert res.n == 11 and int(res.last_bits[0]) == 0x7FD and list(res.W) == [2, 1, 4, 3, 1, 4, 2, 6, 3, 4, 3]
+
+
+@pytest.mark.parametrize("k", ALL_K)
+def test_ragged_tiny_all_k(k):
+    rng = random.Random(4242 + k)
+    for trial in range(3):
+        reads = _ragged_reads(rng, k)
+        for d in (1, 2, 3):
+            assert_matches_oracle(run_gpu(reads, k, d), run_oracle(reads, k, d))
+
+
+@pytest.mark.parametrize("k", [1, 2, 3, 4, 5, 6])
+def test_complete_de_bruijn(k):
+    s = de_bruijn("ACGT", k + 1)
+    res = run_gpu([s], k, 2)
+    S = 4 ** (k + 1)
+    assert res.n == S and np.all(res.mult == 2)
+    assert list(res.W & 3) == [1, 2, 3, 0] * (S // 4)            # bytes 1..4 (+4): A,C,G,T repeating
+    assert_matches_oracle(res, run_oracle([s], k, 2))
+
+
+@pytest.mark.parametrize("k,d", [(21, 2), (31, 2), (31, 1), (32, 2), (63, 2), (99, 2), (127, 2), (11, 3)])
+def test_synthetic_medium(k, d):
+    """A few hundred thousand records: many radix tiles and a ragged last tile, for every key width."""
+    from workloads import ReadGenerator, get_config
+    bases, offs = ReadGenerator(get_config(1, scale=0.08)).host()
+    res = run_gpu((bases, offs), k, d)
+    orc = run_oracle((bases, offs), k, d)
+    assert_matches_oracle(res, orc)
+    # P4: the order-independent checksums agree and equal the definition evaluated on the oracle's output
+    want = int((key_mix_np(orc.distinct_keys) * orc.distinct_cnt.astype(np.uint64)).sum(dtype=np.uint64))
+    assert res.stats.csum_raw == res.stats.csum_distinct == want
+
+
+def test_config1_full_and_host_input():
+    from workloads import ReadGenerator, get_config
+    w = get_config(1)
+    bases, offs = ReadGenerator(w).host()
+    orc = run_oracle((bases, offs), w.k, w.d)
+    res = run_gpu((bases, offs), w.k, w.d, bucket_hist=True)
+    assert res.stats.n_raw == w.n_raw_edges and res.stats.n_ranges == 1
+    assert_matches_oracle(res, orc)
+    # bucket histogram (A11) against the oracle's raw records
+    o1 = run_oracle((bases, offs), w.k, 1)
+    want = np.bincount((o1.distinct_keys[:, 0] >> np.uint64(48)).astype(np.int64), weights=o1.distinct_cnt, minlength=65536)
+    assert np.array_equal(res.stats.bucket_hist.cpu().numpy(), want.astype(np.int64))
+    # the same through HOST buffers (H2D staged by the library), packed by 3 appending calls
+    res2 = run_gpu((bases, offs), w.k, w.d, host_input=True, n_calls=3)
+    assert_matches_oracle(res2, orc)
+
+
+@pytest.mark.parametrize("k", [21, 40, 99])
+def test_P8_plan_independence_blockwise(k):
+    """Forcing a tiny workspace (many block-wise ranges of l=8 partitions) gives identical output."""
+    import paper_1409_7208_b200 as sd
+    from workloads import ReadGenerator, get_config
+    bases, offs = ReadGenerator(get_config(1, scale=0.3)).host()
+    orc = run_oracle((bases, offs), k, 2)
+    res = run_gpu((bases, offs), k, 2, workspace_bytes=sd.sdbg_min_workspace())
+    assert res.stats.n_ranges >= 3, res.stats.n_ranges
+    assert_matches_oracle(res, orc)
+
+
+def test_edge_cases():
+    import paper_1409_7208_b200 as sd
+    # n = 0
+    res = run_gpu([], 5, 2)
+    assert res.n == 0 and res.stats.n_raw == 0
+    # all reads shorter than k+1 / empty
+    res = run_gpu(["ACG", "", "AC", "ACGTA"], 5, 1)
+    assert res.n == 0 and res.stats.n_raw == 0
+    # a read of length exactly k+1
+    assert_matches_oracle(run_gpu(["ACGTAC"], 5, 1), run_oracle(["ACGTAC"], 5, 1))
+    # d above every count
+    assert run_gpu(["ACGTAC", "ACGTAC"], 5, 5).n == 0
+    # palindromes double (A5)
+    res = run_gpu(["ACGT"] * 5, 3, 2)
+    assert res.n == 1 and list(res.mult) == [10]
+    # lower case == upper case
+    a, b = run_gpu([r.lower() for r in T0_READS], 3, 2), run_gpu(T0_READS, 3, 2)
+    assert np.array_equal(a.keys, b.keys) and np.array_equal(a.mult, b.mult)
+    # bad base
+    with pytest.raises(sd.SdbgError) as ei:
+        run_gpu(["ACGTACGT", "ACGNACGT"], 3, 1)
+    assert ei.value.name == "SDBG_E_BADBASE" and "index 11" in str(ei.value)
+    with pytest.raises(sd.SdbgError) as ei:
+        run_gpu(["ACGTACGT", "ACGNACGT"], 3, 1, host_input=True)
+    assert ei.value.name == "SDBG_E_BADBASE"
+    # capacity one short -> SDBG_E_CAPACITY and out->n = needed
+    with pytest.raises(sd.SdbgError) as ei:
+        run_gpu(T0_READS, 3, 2, cap=10)
+    assert ei.value.name == "SDBG_E_CAPACITY"
+    # bad k / d
+    for k, d, name in ((0, 2, "SDBG_E_UNSUPPORTED"), (128, 2, "SDBG_E_UNSUPPORTED"), (5, 0, "SDBG_E_INVAL")):
+        with pytest.raises(sd.SdbgError) as ei:
+            run_gpu(T0_READS, k, d)
+        assert ei.value.name == name
+
+
+def test_capacity_reports_needed_count():
+    import paper_1409_7208_b200 as sd
+    bases, offs = to_arrays(T0_READS)
+    import torch
+    ctx = sd.Context(sd.sdbg_min_workspace())
+    rd = sd.Reads(len(bases))
+    sd.sdbg_pack_reads(ctx, torch.from_numpy(bases).cuda(), torch.from_numpy(offs.view(np.int64)).cuda(), 3, rd)
+    ed = sd.Edges(10, 3)
+    with pytest.raises(sd.SdbgError):
+        sd.sdbg_count_edges(ctx, rd, 3, 3, 2, ed)
+    assert ed.n == 11
+
+
+@pytest.mark.parametrize("k", [5, 31, 33, 99])
+def test_build_unsorted_equals_count(k):
+    """sdbg_build over raw records with mult 1 (unsorted, with repeats) == sdbg_count_edges at d=1 (one semantics)."""
+    import torch
+    import paper_1409_7208_b200 as sd
+    rng = random.Random(99 + k)
+    reads = _ragged_reads(rng, k, n_reads=80)
+    orc = run_oracle(reads, k, 1)
+    # raw records = the oracle's distinct keys repeated by their counts, shuffled
+    keys = np.repeat(orc.distinct_keys, orc.distinct_cnt.astype(np.int64), axis=0)
+    perm = np.random.default_rng(k).permutation(len(keys))
+    keys = np.ascontiguousarray(keys[perm])
+    n, w = len(keys), orc.w
+    ctx = sd.Context(sd.sdbg_min_workspace() + 64 * n * w)
+    ed = sd.Edges(n, k)
+    ed.keys[: n * w] = torch.from_numpy(keys.reshape(-1).view(np.int64)).cuda()
+    ed.mult[:n] = 1
+    ed.c.n = n
+    g = sd.Graph(n)
+    sd.sdbg_build(ctx, ed, 0, g)
+    torch.cuda.synchronize()
+    assert ed.n == orc.n_distinct == g.n
+    assert np.array_equal(ed.keys_np(), orc.distinct_keys)
+    assert np.array_equal(ed.mult_np(), orc.distinct_cnt)
+    assert np.array_equal(g.W_np(), orc.Wbyte) and np.array_equal(g.last_bits_np(), orc.last_bits)
