@@ -1,0 +1,268 @@
+#!/usr/bin/env python
+"""bench.py — (k+1)-mers sorted+counted per second on one B200 (BASELINE.json metric), through the C ABI.
+
+A "step" is one pass of the whole hot path over one batch of synthetic reads:
+sdbg_pack_reads -> sdbg_count_edges (extract, radix sort, count, solid filter) -> sdbg_build(SDBG_SORTED).
+Default workload: BASELINE.json configs[1] (single bacterium, 5 Mbp, 150 bp reads at 50x, k=31, d=2).
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--config 1..4] [--impl reference]
+
+`--impl reference` times the CPU oracle (oracle/, as it stands) on a bounded sample of the same workload.
+With N>1 (torchrun) every rank runs an independent replica on its own GPU ("replicas only": the path does not
+shard); value = records of all ranks / max-over-ranks time.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "(k+1)-mers sorted+counted/sec"
+UNIT = "edges/s"
+
+
+def _peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        try:
+            return float(json.load(open(p))["hbm_gbs"]), "measured (MEASURED_PEAKS.json)"
+        except Exception:
+            pass
+    return 6650.0, "fallback (B200_PROFILING.md)"
+
+
+def _traffic(workload_name):
+    """DRAM bytes per launch of the dominant kernel from the committed ncu --set full capture, if any."""
+    p = os.path.join(ROOT, "profiles", "traffic.json")
+    if os.path.exists(p):
+        try:
+            return json.load(open(p)).get(workload_name)
+        except Exception:
+            return None
+    return None
+
+
+class ClockSampler(threading.Thread):
+    """Samples nvidia-smi clocks / throttle reasons while the timed region runs."""
+    Q = ("clocks.sm,clocks.max.sm,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, gpu_index):
+        super().__init__(daemon=True)
+        self.gpu, self.stop_flag, self.rows = gpu_index, threading.Event(), []
+
+    def run(self):
+        while not self.stop_flag.is_set():
+            try:
+                out = subprocess.run(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits", "-i", str(self.gpu)],
+                                     capture_output=True, text=True, timeout=5).stdout.strip()
+                if out:
+                    self.rows.append([x.strip() for x in out.split(",")])
+            except Exception:
+                pass
+            self.stop_flag.wait(0.1)
+
+    def summary(self):
+        self.stop_flag.set()
+        self.join(timeout=6)
+        sm = sorted(float(r[0]) for r in self.rows if r and r[0].replace(".", "").isdigit())
+        mx = [float(r[1]) for r in self.rows if len(r) > 1 and r[1].replace(".", "").isdigit()]
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        reasons = sorted({n for r in self.rows if len(r) >= 6 for n, v in zip(names, r[2:6]) if v.lower().startswith("active")})
+        return {"sm_mhz": sm[len(sm) // 2] if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "reasons": reasons, "samples": len(self.rows)}
+
+
+def run_reference(args, w):
+    """The oracle, as it stands, on the host cores: each step = steps 1-6 on a bounded sample of the workload."""
+    from oracle import run_oracle
+    from workloads import ReadGenerator
+    n_reads = min(w.n_reads, args.ref_reads)
+    bases, offs = ReadGenerator(w).host(0, n_reads)
+    n_rec = 2 * n_reads * max(0, w.read_len - w.k)
+    for _ in range(args.warmup if args.warmup < 2 else 1):
+        run_oracle((bases, offs), w.k, w.d)
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        run_oracle((bases, offs), w.k, w.d)
+    dt = (time.perf_counter() - t0) / args.steps
+    val = n_rec / dt
+    sample = f"first {n_reads} reads of {w.name} ({n_rec} records) per step"
+    line = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": dt * 1e3, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "u64", "data": "synthetic",
+            "config": {"workload": w.name, "k": w.k, "d": w.d, "read_len": w.read_len, "sample": sample},
+            "cpu_baseline": {"value": val, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample},
+            "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
+    print(json.dumps(line), flush=True)
+
+
+def cpu_baseline(w, n_reads):
+    """Oracle timed once on a bounded sample (rank 0, N=1 only): about 10-30 s of single-core CPU work."""
+    from oracle import run_oracle
+    from workloads import ReadGenerator
+    n_reads = min(w.n_reads, n_reads)
+    bases, offs = ReadGenerator(w).host(0, n_reads)
+    n_rec = 2 * n_reads * max(0, w.read_len - w.k)
+    t0 = time.perf_counter()
+    run_oracle((bases, offs), w.k, w.d)
+    dt = time.perf_counter() - t0
+    return {"value": n_rec / dt, "unit": UNIT, "cores": 1, "kind": "oracle",
+            "sample": f"first {n_reads} reads of {w.name} ({n_rec} records), {dt:.1f} s, single thread"}
+
+
+def run_gpu(args, w):
+    import torch
+    import torch.distributed as dist
+    import paper_1409_7208_b200 as sd
+    from workloads import ReadGenerator
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+
+    # ---- inputs resident in HBM: every rank an independent replica (own seed) ------------------------------
+    from dataclasses import replace
+    wl = replace(w, seed=w.seed + 1000003 * rank) if rank else w
+    gen = ReadGenerator(wl)
+    bases_d, offs_d = gen.device()
+    torch.cuda.synchronize()
+    n_bases, n_reads = wl.n_bases, wl.n_reads
+    N = wl.n_raw_edges
+    K = 8 * wl.words_per_key
+
+    ctx = sd.Context(sd.sdbg_full_workspace(n_bases, wl.k))
+    reads = sd.Reads(n_bases)
+    edges = sd.Edges(N // wl.d, wl.k)
+    graph = sd.Graph(N // wl.d)
+
+    def step(src_b, src_o):
+        reads.c.n_reads = reads.c.n_bases = reads.c.n_slots = 0
+        sd.sdbg_pack_reads(ctx, src_b, src_o, n_reads, reads)
+        sd.sdbg_count_edges(ctx, reads, n_reads, wl.k, wl.d, edges, None)
+        sd.sdbg_build(ctx, edges, sd.SDBG_SORTED, graph)
+        return edges.n
+
+    def barrier():
+        torch.cuda.synchronize()
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for _ in range(max(args.warmup, 3)):
+        S = step(bases_d, offs_d)
+    ctx.get_timing()
+    ctx.set_timing(True)
+    sampler = ClockSampler(local)
+    sampler.start()
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    ev0.record()
+    for _ in range(args.steps):
+        step(bases_d, offs_d)
+    ev1.record()
+    barrier()
+    ms_total = ev0.elapsed_time(ev1)
+    tim = ctx.get_timing()
+    clocks = sampler.summary()
+    ctx.set_timing(False)
+
+    # ---- end to end: HOST pinned buffers in, SdBG arrays out, copies inside the timed region ---------------------
+    bases_h = torch.empty(n_bases, dtype=torch.uint8, pin_memory=True)
+    offs_h = torch.empty(n_reads + 1, dtype=torch.int64, pin_memory=True)
+    bases_h.copy_(bases_d); offs_h.copy_(offs_d)
+    out_W = torch.empty(S, dtype=torch.uint8, pin_memory=True)
+    out_last = torch.empty((S + 63) // 64, dtype=torch.int64, pin_memory=True)
+    out_mult = torch.empty(S, dtype=torch.int32, pin_memory=True)
+    out_keys = torch.empty(S * wl.words_per_key, dtype=torch.int64, pin_memory=True)
+
+    def e2e_step():
+        s = step(bases_h, offs_h)
+        out_W.copy_(graph.W[:s], non_blocking=True)
+        out_last.copy_(graph.last_bits[:(s + 63) // 64], non_blocking=True)
+        out_mult.copy_(graph.mult[:s], non_blocking=True)
+        out_keys.copy_(edges.keys[:s * wl.words_per_key], non_blocking=True)
+
+    e2e_step()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    e0.record()
+    for _ in range(args.steps):
+        e2e_step()
+    e1.record()
+    barrier()
+    ms_e2e = e0.elapsed_time(e1)
+    h2d = n_bases + 8 * (n_reads + 1)
+    d2h = S * (1 + 4 + K) + 8 * ((S + 63) // 64)
+
+    t = torch.tensor([ms_total, ms_e2e], dtype=torch.float64, device="cuda")
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    ms_total, ms_e2e = float(t[0]), float(t[1])
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return
+
+    peak, peak_src = _peaks()
+    radix_launches = tim.launches["radix"]
+    radix_ms = tim.ms["radix"] / max(radix_launches, 1)
+    algo_bytes = 2 * N * K                       # one pass reads and writes every key once
+    achieved = algo_bytes / (radix_ms * 1e-3) / 1e9 if radix_ms > 0 else 0.0
+    line = {
+        "metric": METRIC, "value": world * N * args.steps / (ms_total * 1e-3), "unit": UNIT, "n_gpus": world,
+        "steps": args.steps, "warmup": max(args.warmup, 3), "ms_per_step": ms_total / args.steps,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "u64", "data": "synthetic",
+        "config": {"workload": wl.name, "k": wl.k, "d": wl.d, "reads": n_reads, "read_len": wl.read_len, "bases": n_bases,
+                   "raw_edges": N, "solid_edges": int(S), "key_bytes": K, "parallelism": "replicas only" if world > 1 else "1 gpu",
+                   "l2": "inputs larger than L2 (keys %.2f GB, reads %.0f MB ASCII)" % (N * K / 1e9, n_bases / 1e6)},
+        "read_bases_per_s": world * n_bases * args.steps / (ms_total * 1e-3),
+        "clocks": clocks,
+        "e2e": {"value": world * N * args.steps / (ms_e2e * 1e-3), "unit": UNIT, "h2d_bytes_per_step": h2d,
+                "d2h_bytes_per_step": d2h, "ms_per_step": ms_e2e / args.steps},
+        "gpu_launches": int(tim.total_launches),
+        "roofline": {"kernel": "onesweep_kernel (one LSD radix pass)", "bound": "hbm", "achieved": achieved, "peak": peak,
+                     "unit": "GB/s", "frac": achieved / peak, "traffic": _traffic(wl.name), "peak_source": peak_src,
+                     "launches": int(radix_launches), "avg_launch_ms": radix_ms, "algorithmic_bytes_per_launch": algo_bytes},
+        "kernel_ms_per_step": {c: tim.ms[c] / args.steps for c in tim.ms},
+        "kernel_launches_per_step": {c: tim.launches[c] / args.steps for c in tim.launches},
+    }
+    if world == 1 and not args.no_cpu_baseline:
+        line["cpu_baseline"] = cpu_baseline(wl, args.ref_reads)
+    print(json.dumps(line), flush=True)
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--config", type=int, default=2, help="BASELINE.json config number (1-4); default 2 = configs[1]")
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--ref-reads", type=int, default=40000, help="reads in the oracle's bounded sample")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    from workloads import get_config
+    w = get_config(args.config)
+    if args.impl == "reference":
+        if int(os.environ.get("RANK", "0")) == 0:
+            run_reference(args, w)
+        return
+    run_gpu(args, w)
+
+
+if __name__ == "__main__":
+    main()

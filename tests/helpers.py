@@ -86,7 +86,8 @@ def key_mix(words):
 
 def key_mix_np(keys):
     """vectorised key_mix over an (n, w) uint64 array."""
-    keys = np.ascontiguousarray(keys, dtype=np.uint64).reshape(len(keys), -1)
+    keys = np.ascontiguousarray(keys, dtype=np.uint64)
+    keys = keys.reshape(len(keys), keys.shape[1] if keys.ndim == 2 else 1)
     h = np.zeros(len(keys), dtype=np.uint64)
     with np.errstate(over="ignore"):
         for j in range(keys.shape[1]):
