@@ -194,15 +194,17 @@ def run_gpu(args, w):
         out_mult.copy_(graph.mult[:s], non_blocking=True)
         out_keys.copy_(edges.keys[:s * wl.words_per_key], non_blocking=True)
 
-    e2e_step()
-    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    barrier()
-    e0.record()
-    for _ in range(args.steps):
+    ms_e2e = float("nan")
+    if not args.no_e2e:
         e2e_step()
-    e1.record()
-    barrier()
-    ms_e2e = e0.elapsed_time(e1)
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        barrier()
+        e0.record()
+        for _ in range(args.steps):
+            e2e_step()
+        e1.record()
+        barrier()
+        ms_e2e = e0.elapsed_time(e1)
     h2d = n_bases + 8 * (n_reads + 1)
     d2h = S * (1 + 4 + K) + 8 * ((S + 63) // 64)
 
@@ -254,6 +256,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--ref-reads", type=int, default=40000, help="reads in the oracle's bounded sample")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true", help="development runs: skip the host-buffer end-to-end leg")
     args = ap.parse_args()
     from workloads import get_config
     w = get_config(args.config)

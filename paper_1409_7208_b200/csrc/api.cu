@@ -81,18 +81,16 @@ struct Timed {
         if (e__ != cudaSuccess) return ctx->cuda_fail(e__, #call);      \
     } while (0)
 
+// LSD passes over the significant bits only, least significant first. Every digit is one whole byte of a key
+// word (the sorter extracts it with a single byte-permute): the lowest pass starts at the byte that holds the first
+// significant bit, and the zero padding bits below it simply leave some of its 256 bins empty.
 PassTable make_passes(u32 k) {
     PassTable pt{};
     const u32 W = (2 * (k + 1) + 63) / 64;
     const u32 pad = 64 * W - 2 * (k + 1);
-    for (int w = (int)W - 1; w >= 0; --w) {
-        u32 lo = (w == (int)W - 1) ? pad : 0;
-        while (lo < 64) {
-            u32 bits = std::min<u32>(kRadixBits, 64 - lo);
-            pt.p[pt.n++] = PassDesc{(uint8_t)w, (uint8_t)lo, (uint8_t)bits, 0};
-            lo += bits;
-        }
-    }
+    for (int w = (int)W - 1; w >= 0; --w)
+        for (u32 lo = (w == (int)W - 1) ? pad / 8 * 8 : 0; lo < 64; lo += kRadixBits)
+            pt.p[pt.n++] = PassDesc{(uint8_t)w, (uint8_t)lo, (uint8_t)kRadixBits, 0};
     return pt;
 }
 
@@ -108,9 +106,11 @@ u64 range_need(u64 n, u32 W) {
     const u64 rt = radix_tile_records(W, false), ct = count_tile_records(W);
     return 2 * align_up(n * K) + align_up(((n + rt - 1) / rt + 1) * kRadix * 8) + align_up(((n + ct - 1) / ct + 1) * 2 * 8);
 }
-// largest n with range_need(n) <= avail
+// largest n with range_need(n) <= avail; one sort range holds fewer than 2^32 records (the look-back words of the
+// radix passes carry 32-bit counts), larger inputs are split into block-wise ranges like any input that does not fit
+constexpr u64 kMaxRangeRecords = 0xffffffffull;
 u64 range_capacity(u64 avail, u32 W) {
-    u64 lo = 0, hi = avail / (16ull * W) + 1;
+    u64 lo = 0, hi = std::min<u64>(avail / (16ull * W) + 1, kMaxRangeRecords);
     while (lo < hi) {
         u64 mid = lo + (hi - lo + 1) / 2;
         if (range_need(mid, W) <= avail) lo = mid; else hi = mid - 1;

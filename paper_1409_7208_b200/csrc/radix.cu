@@ -17,20 +17,21 @@
 
 namespace sdbg {
 
-#ifndef SDBG_LB_SKIP
-#define SDBG_LB_SKIP 0   // timing experiments only: wrong results
+// How step j of a warp finds the lanes holding the same digit ("match"), one letter per step, repeated cyclically:
+//   B  8 ballots (VOTE + predicated NOT + AND per bit): ~29 ALU-pipe instructions, no shared memory;
+//   A  atomicOr of the lane bit into a warp-private mask word, read back, leader clears: 5 shared-memory
+//      operations, ~3 ALU instructions;
+//   M  the hardware match.any (one instruction, ~61 SM-cycles per warp on sm_100: only worth a small share).
+// The kernel is bound by instruction issue and shared-memory wavefronts at the same time,
+// so the steps are split between B and A to load both pipes equally.
+#ifndef SDBG_LB_EVERY
+#define SDBG_LB_EVERY 4      // rank steps between two look-back polls (power of two)
 #endif
-#ifndef SDBG_LB_DEPTH
-#define SDBG_LB_DEPTH 4  // independent look-back loads in flight per bin
+#ifndef SDBG_PERSISTENT
+#define SDBG_PERSISTENT 1    // 1: persistent CTAs holding the ticket of their next tile; 0: one tile per CTA
 #endif
-#ifndef SDBG_MERGE_BINSTART
-#define SDBG_MERGE_BINSTART 1
-#endif
-#ifndef SDBG_FULL_SPEC
-#define SDBG_FULL_SPEC 0   // duplicating the load/store loops for full tiles overflows the instruction cache: slower
-#endif
-#ifndef SDBG_VSPLIT
-#define SDBG_VSPLIT 1    // independent ranking chains ("virtual warps") per warp
+#ifndef SDBG_RANK_METHODS
+#define SDBG_RANK_METHODS "B"
 #endif
 
 template <int W, bool HAS_VAL> struct RadixCfg;
@@ -49,9 +50,24 @@ template <> struct RadixCfg<2, true>  { static constexpr int THREADS = 512, KPT 
 template <> struct RadixCfg<3, true>  { static constexpr int THREADS = 512, KPT = 4,  MINB = 2; };
 template <> struct RadixCfg<4, true>  { static constexpr int THREADS = 512, KPT = 3,  MINB = 2; };
 
-constexpr u64 kValMask = (1ull << 54) - 1;
-constexpr int kVSplit = SDBG_VSPLIT;
+constexpr char kRankMethods[] = SDBG_RANK_METHODS;
+constexpr int kNumRankMethods = (int)sizeof(kRankMethods) - 1;
+static_assert(kNumRankMethods >= 1 && kNumRankMethods <= 32, "SDBG_RANK_METHODS: 1..32 letters");
+constexpr u64 pack_rank_methods() {   // 2 bits per step: 0 = B, 1 = A, 2 = M
+    u64 v = 0;
+    for (int j = 0; j < kNumRankMethods; ++j)
+        v |= (u64)(kRankMethods[j] == 'A' ? 1 : kRankMethods[j] == 'M' ? 2 : 0) << (2 * j);
+    return v;
+}
+constexpr u64 kRankMethodBits = pack_rank_methods();
+constexpr int kMethodA = 1, kMethodM = 2;   // 0 = B
+__host__ __device__ constexpr int rank_method(int j) { return (int)((kRankMethodBits >> (2 * (j % kNumRankMethods))) & 3u); }
+constexpr bool uses_method(int c, int kpt) {
+    for (int j = 0; j < kpt; ++j) if (rank_method(j) == c) return true;
+    return false;
+}
 
+// generic digit of a pass (histogram helpers; the sort kernel uses digit8)
 template <int W>
 __device__ __forceinline__ u32 digit_of(const u64 (&key)[W], const PassDesc pd) {
     u64 kw = key[0];
@@ -60,9 +76,18 @@ __device__ __forceinline__ u32 digit_of(const u64 (&key)[W], const PassDesc pd) 
     return (u32)(kw >> pd.shift) & ((1u << pd.bits) - 1u);
 }
 
-// lanes of the warp whose 8-bit digit equals mine: 8 ballots, 4 SASS instructions per bit
-// (LOP3 -> predicate, VOTE, predicated NOT, AND) — the hardware match.any is ~3x slower on sm_100.
-__device__ __forceinline__ u32 match_digit(u32 d) {
+// Digit of a byte-aligned 8-bit pass: byte (psel & 3) of the high (HI) or low half of key word `word`; one PRMT.
+template <int W, bool HI>
+__device__ __forceinline__ u32 digit8(const u64 (&key)[W], u32 word, u32 psel) {
+    u64 kw = key[0];
+#pragma unroll
+    for (int j = 1; j < W; ++j) if (word == (u32)j) kw = key[j];
+    return __byte_perm(HI ? (u32)(kw >> 32) : (u32)kw, 0u, psel);
+}
+
+// lanes of the warp whose 8-bit digit equals mine: 8 ballots, 3-4 SASS instructions per bit
+// (R2P/LOP3 -> predicates, VOTE, predicated NOT, AND).
+__device__ __forceinline__ u32 match_ballot(u32 d) {
     u32 m = 0xffffffffu;
 #pragma unroll
     for (int b = 0; b < kRadixBits; ++b) {
@@ -105,45 +130,61 @@ __device__ __forceinline__ void store_rec(u64 *__restrict__ o, const u64 (&k)[W]
     }
 }
 
-template <int W, bool HAS_VAL>
-__global__ void __launch_bounds__(RadixCfg<W, HAS_VAL>::THREADS, RadixCfg<W, HAS_VAL>::MINB)
-onesweep_kernel(RadixArgs a) {
-    using Cfg = RadixCfg<W, HAS_VAL>;
-    constexpr int THREADS = Cfg::THREADS, KPT = Cfg::KPT, WARPS = THREADS / 32, TILE = THREADS * KPT;
-    constexpr int VS = (KPT >= 2 * kVSplit) ? kVSplit : 1;      // ranking chains per warp
-    constexpr int VW = WARPS * VS;                              // virtual warps
-    constexpr int H = (KPT + VS - 1) / VS;                      // steps per chain
-    static_assert(THREADS >= kRadix, "one thread per bin");
+// One non-blocking step of the decoupled look-back of one bin (see phase 3 of onesweep_kernel): consume the entry
+// requested earlier if it has been published for this pass, then request the next predecessor (or the same one
+// again); on reaching an inclusive (GLOBAL) entry publish this tile's inclusive prefix. Entry = tag (status, epoch)
+// in bits 63..54, 32-bit count in bits 31..0: one sort range holds fewer than 2^32 records (api.cu range_capacity).
+__device__ __forceinline__ void lookback_poll(u64 *lb, u32 tile, u32 &t, u64 &pend, u32 &excl, bool &done, u32 real_cnt,
+                                              u32 tagL, u32 tagG) {
+    if (done) return;
+    const u32 tag = (u32)(pend >> 54);
+    if (tag == tagL || tag == tagG) {
+        excl += (u32)pend;
+        if (tag == tagG) {
+            done = true;
+            st_relaxed(lb + (u64)tile * kRadix, ((u64)tagG << 54) | (u64)(excl + real_cnt));
+            return;
+        }
+        --t;   // tile 0 always publishes GLOBAL, so t never passes it
+    }
+    pend = ld_relaxed(lb + (u64)t * kRadix);
+}
 
-    extern __shared__ __align__(16) unsigned char smem_raw[];
-    u64 *s_keys = reinterpret_cast<u64 *>(smem_raw);                 // W planes of TILE
-    u64 *s_binout = s_keys + (size_t)TILE * W;                       // [256] global base - tile bin start
-    u32 *s_whist = reinterpret_cast<u32 *>(s_binout + kRadix);       // [VW][256]: count, then tile position of the group
-    u32 *s_vals = s_whist + VW * kRadix;                             // [TILE] if HAS_VAL
-    __shared__ u32 s_tile;
-    __shared__ u32 s_wtot[kRadix / 32];
-#if !SDBG_MERGE_BINSTART
-    __shared__ u32 s_binstart[kRadix];
-#endif
-
-    const u32 tid = threadIdx.x, lane = tid & 31u, warp = tid >> 5;
-    const u32 lt = lanemask_lt();
-    const PassDesc pd = a.pass;
-
-    if (tid == 0) s_tile = atomicAdd(a.ticket, 1u);
+// digit8 that the compiler may not merge with an earlier evaluation (recomputing one PRMT is cheaper than keeping
+// 16 digits alive across the phases, which spills)
+__device__ __forceinline__ u32 prmt_opaque(u32 x, u32 psel) {
+    u32 d;
+    asm volatile("prmt.b32 %0, %1, 0, %2;" : "=r"(d) : "r"(x), "r"(psel));
+    return d;
+}
+template <int W, bool HI>
+__device__ __forceinline__ u32 digit8_again(const u64 (&key)[W], u32 word, u32 psel) {
+    u64 kw = key[0];
 #pragma unroll
-    for (int i = tid; i < VW * kRadix; i += THREADS) s_whist[i] = 0;
-    __syncthreads();
-    const u32 tile = s_tile;
-    const u64 tile_base = (u64)tile * TILE;
-    const u32 cnt = (a.n - tile_base < (u64)TILE) ? (u32)(a.n - tile_base) : (u32)TILE;
-    const bool full = SDBG_FULL_SPEC && cnt == (u32)TILE;
+    for (int j = 1; j < W; ++j) if (word == (u32)j) kw = key[j];
+    return prmt_opaque(HI ? (u32)(kw >> 32) : (u32)kw, psel);
+}
 
-    // ---- load (warp-striped: lane l, step j -> tile index warp*32*KPT + j*32 + l) --------------------
-    u64 key[KPT][W];
-    u32 val[HAS_VAL ? KPT : 1];
-    const u32 wbase = warp * 32u * KPT + lane;
-    if (full) {
+template <int W, bool HAS_VAL>
+struct RadixSmem {
+    using Cfg = RadixCfg<W, HAS_VAL>;
+    static constexpr int THREADS = Cfg::THREADS, KPT = Cfg::KPT, WARPS = THREADS / 32, TILE = THREADS * KPT;
+    static constexpr bool USE_A = uses_method(kMethodA, KPT);
+    static constexpr size_t kKeys = 0;                                             // u64[W][TILE]
+    static constexpr size_t kBinAddr = kKeys + (size_t)TILE * W * 8;              // u64[256] byte address of bin run - tile start
+    static constexpr size_t kValAddr = kBinAddr + kRadix * 8;                       // u64[256] (HAS_VAL)
+    static constexpr size_t kPos = kValAddr + (HAS_VAL ? kRadix * 8 : 0);           // u32[WARPS][256] counts, then tile positions
+    static constexpr size_t kMask = kPos + (size_t)WARPS * kRadix * 4;              // u32[WARPS][256] match masks (method A)
+    static constexpr size_t kVals = kMask + (USE_A ? (size_t)WARPS * kRadix * 4 : 0);  // u32[TILE] (HAS_VAL)
+    static constexpr size_t kBytes = kVals + (HAS_VAL ? (size_t)TILE * 4 : 0);
+};
+
+// Loads one tile into registers (lane l, step j -> tile index warp*32*KPT + j*32 + l: coalesced 256-byte rows).
+// Slots past the end of the data become all-ones pads: digit 255, last in tile order, so they take the last places.
+template <int W, bool HAS_VAL, int KPT>
+__device__ __forceinline__ void load_tile(const RadixArgs &a, u64 tile_base, u32 cnt, u32 wbase, u64 (&key)[KPT][W],
+                                          u32 (&val)[HAS_VAL ? KPT : 1]) {
+    if (cnt == (u32)(KPT * RadixCfg<W, HAS_VAL>::THREADS)) {
 #pragma unroll
         for (int j = 0; j < KPT; ++j) {
             load_rec<W>(a.keys_in + (tile_base + wbase + j * 32u) * W, key[j]);
@@ -158,165 +199,251 @@ onesweep_kernel(RadixArgs a) {
                 if constexpr (HAS_VAL) val[j] = a.vals_in[tile_base + ti];
             } else {
 #pragma unroll
-                for (int q = 0; q < W; ++q) key[j][q] = ~0ull;   // pads rank last in the last bin
+                for (int q = 0; q < W; ++q) key[j][q] = ~0ull;
                 if constexpr (HAS_VAL) val[j] = 0;
             }
         }
     }
+}
 
-    // ---- rank within the (virtual) warp, stable in tile order ---------------------------------------------
-    // Chain c of the warp owns steps [c*H, (c+1)*H): VS independent smem dependency chains per warp.
-    u32 rank2[(KPT + 1) / 2];   // two 16-bit ranks per register
+// L2 prefetch of a contiguous range by the TMA unit (one instruction; bytes a multiple of 16, p 16-byte aligned).
+__device__ __forceinline__ void prefetch_l2_bulk(const void *p, u32 bytes) {
+    if (bytes) asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(p), "r"(bytes) : "memory");
+}
+
+// One LSD pass over an 8-bit, byte-aligned digit. Persistent CTAs; tiles are handed out by an atomic ticket, one
+// tile AHEAD: while a CTA works on a tile it already holds the ticket of its next one, has asked the TMA unit to
+// prefetch that tile into L2, and loads it into the (then free) key registers before the write-out of the current
+// tile, so that DRAM reads are in flight during the whole life of a tile and not only at its start.
+// Per tile:
+//   1 count digits of the keys in registers into warp-private histograms (shared atomics);
+//   2 one thread per bin: tile count -> look-back state (LOCAL), exclusive scan over bins and warps turns the
+//     histograms into the tile position of the first key of (warp, digit);
+//   3 per step: match the lanes with my digit, position = running (warp, digit) position + rank among them,
+//     key goes to its bin-sorted place in shared memory; the decoupled look-back of the bins advances one
+//     predecessor per step in the shadow of the match arithmetic;
+//   4 the next tile is loaded into the key registers; bin addresses from the look-back result;
+//   5 write-out: place p of the tile goes to bin_address[digit] + p, coalesced per digit run.
+// Forward progress: a CTA's current tile is always older than the ticket it holds in reserve, so the oldest
+// unfinished tile is always being worked on by a resident CTA.
+template <int W, bool HAS_VAL, bool HI>
+__global__ void __launch_bounds__(RadixCfg<W, HAS_VAL>::THREADS, RadixCfg<W, HAS_VAL>::MINB)
+onesweep_kernel(RadixArgs a) {
+    using L = RadixSmem<W, HAS_VAL>;
+    constexpr int THREADS = L::THREADS, KPT = L::KPT, WARPS = L::WARPS, TILE = L::TILE;
+    constexpr bool USE_A = L::USE_A;
+    static_assert(THREADS >= kRadix, "one thread per bin");
+
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    u64 *s_keys = reinterpret_cast<u64 *>(smem_raw + L::kKeys);
+    u64 *s_binaddr = reinterpret_cast<u64 *>(smem_raw + L::kBinAddr);
+    u64 *s_valaddr = reinterpret_cast<u64 *>(smem_raw + L::kValAddr);
+    u32 *s_pos = reinterpret_cast<u32 *>(smem_raw + L::kPos);
+    u32 *s_mask = reinterpret_cast<u32 *>(smem_raw + L::kMask);
+    u32 *s_vals = reinterpret_cast<u32 *>(smem_raw + L::kVals);
+    __shared__ u32 s_tick[2];
+    __shared__ u32 s_wtot[kRadix / 32];
+
+    const u32 tid = threadIdx.x, lane = tid & 31u, warp = tid >> 5;
+    const u32 lt = lanemask_lt();
+    const u32 word = a.pass.word;
+    const u32 psel = 0x4440u | ((a.pass.shift >> 3) & 3u);
+    const u32 ntiles = (u32)((a.n + TILE - 1) / TILE);
+    const u32 wbase = warp * 32u * KPT + lane;
+    u32 *wp = s_pos + warp * kRadix;
+    u32 *wm = s_mask + warp * kRadix;
+    const u32 tagL = ((u32)kStLocal << 8) | a.epoch, tagG = ((u32)kStGlobal << 8) | a.epoch;
+    u64 *lb = a.lookback + tid;
+
+    // warp-private histogram rows start at zero (and are zeroed again by their warp after every rank phase)
+    auto zero_rows = [&]() {
 #pragma unroll
-    for (int i = 0; i < (KPT + 1) / 2; ++i) rank2[i] = 0;
-#pragma unroll
-    for (int jj = 0; jj < H; ++jj) {
-#pragma unroll
-        for (int c = 0; c < VS; ++c) {
-            const int j = c * H + jj;
-            if (j < KPT) {
-                u32 *wh = s_whist + (warp * VS + c) * kRadix;
-                const u32 d = digit_of<W>(key[j], pd);
-                const u32 m = match_digit(d);
-                const u32 prev = wh[d];                            // same address within the group: broadcast read
-                __syncwarp();
-                if ((m >> lane) <= 1u) wh[d] = prev + __popc(m);   // highest lane of the group updates the count
-                const u32 r = prev + __popc(m & lt);
-                rank2[j >> 1] |= (j & 1) ? (r << 16) : r;
-            }
+        for (int i = 0; i < kRadix / 32; ++i) {
+            wp[i * 32 + lane] = 0;
+            if (USE_A) wm[i * 32 + lane] = 0;
         }
         __syncwarp();
-    }
-    __syncthreads();
-
-    // ---- per bin: totals over the virtual warps, publish the tile's count (LOCAL) as early as possible ------------
-    u32 my_cnt = 0, incl = 0, real_cnt = 0;
-    const u64 tagL = ((kStLocal << 8) | a.epoch), tagG = ((kStGlobal << 8) | a.epoch);
-    u64 *lb = a.lookback + tid;
-    if (tid < kRadix) {
-#if SDBG_MERGE_BINSTART
-#pragma unroll
-        for (int v = 0; v < VW; ++v) my_cnt += s_whist[v * kRadix + tid];
-#else
-#pragma unroll
-        for (int v = 0; v < VW; ++v) {
-            const u32 t = s_whist[v * kRadix + tid];
-            s_whist[v * kRadix + tid] = my_cnt;
-            my_cnt += t;
+    };
+    // ---- pieces of the per-tile pipeline ----------------------------------------------------------------------
+    u64 key[KPT][W];
+    u32 val[HAS_VAL ? KPT : 1];
+    u32 it = 0;
+    // ticket of the tile after `the one being loaded`, and its L2 prefetch (thread 0)
+    auto reserve_next = [&]() {
+        if (SDBG_PERSISTENT && tid == 0) {
+            const u32 nx = atomicAdd(a.ticket, 1u);
+            s_tick[(it + 1) & 1] = nx;
+            if (nx < ntiles) {
+                const u64 nb = (u64)nx * TILE;
+                const u64 nc = (a.n - nb < (u64)TILE) ? a.n - nb : (u64)TILE;
+                prefetch_l2_bulk(a.keys_in + nb * W, (u32)(nc * 8u * W) & ~15u);
+                if constexpr (HAS_VAL) prefetch_l2_bulk(a.vals_in + nb, (u32)(nc * 4u) & ~15u);
+            }
         }
-#endif
-        real_cnt = my_cnt;                                            // my_cnt includes the pads (last bin of the pass)
-        if (tid == (1u << pd.bits) - 1u) real_cnt -= (u32)TILE - cnt;
-        st_relaxed(lb + (u64)tile * kRadix, ((tile == 0 ? tagG : tagL) << 54) | real_cnt);
+    };
+    auto tile_count = [&](u32 t) { return (a.n - (u64)t * TILE < (u64)TILE) ? (u32)(a.n - (u64)t * TILE) : (u32)TILE; };
+    // phase 1: digits of the keys in registers -> warp-private histogram
+    auto count_keys = [&]() {
+#pragma unroll
+        for (int j = 0; j < KPT; ++j) atomicAdd(&wp[digit8<W, HI>(key[j], word, psel)], 1u);
+    };
+    // phase 2a (one thread per bin, after a block barrier): tile count, published LOCAL at once; scan over the bins
+    u32 my_cnt = 0, incl = 0;
+    auto scan_bins = [&](u32 t, u32 tcnt) -> u32 {
+        my_cnt = 0;
+#pragma unroll
+        for (int v = 0; v < WARPS; ++v) my_cnt += s_pos[v * kRadix + tid];
+        u32 rc = my_cnt;                                                  // my_cnt includes the pads (bin 255)
+        if (tid == kRadix - 1) rc -= (u32)TILE - tcnt;
+        st_relaxed(lb + (u64)t * kRadix, ((u64)(t == 0 ? tagG : tagL) << 54) | rc);
         incl = warp_incl_scan_add(my_cnt);
         if (lane == 31) s_wtot[warp] = incl;
-    }
-    __syncthreads();
-    u32 bin_start = 0;
-    if (tid < kRadix) {
+        return rc;
+    };
+    // phase 2b (after another barrier): entry (v, bin) becomes the tile position of the first key of digit `bin`
+    // held by warp v; returns the tile position of the bin's first key
+    auto scan_warps = [&]() -> u32 {
         u32 off = 0;
 #pragma unroll
         for (int w = 0; w < kRadix / 32; ++w) off += (w < (int)warp) ? s_wtot[w] : 0u;
-        bin_start = off + incl - my_cnt;
-#if SDBG_MERGE_BINSTART
-        // entry (v, bin) becomes the tile position of the first key of digit `bin` held by virtual warp v
-        u32 run = bin_start;
+        const u32 bs = off + incl - my_cnt;
+        u32 run = bs;
 #pragma unroll
-        for (int v = 0; v < VW; ++v) {
-            const u32 t = s_whist[v * kRadix + tid];
-            s_whist[v * kRadix + tid] = run;
+        for (int v = 0; v < WARPS; ++v) {
+            const u32 t = s_pos[v * kRadix + tid];
+            s_pos[v * kRadix + tid] = run;
             run += t;
         }
-#else
-        s_binstart[tid] = bin_start;
+        return bs;
+    };
+
+    // Decoupled look-back state of the CURRENT tile, one thread per bin. It advances during the rank steps of the
+    // tile and, in the shadow of the next tile's count and scan, until the write-out needs it. lb_t = predecessor
+    // tile being examined; lb_pend = its entry as last read.
+    u64 lb_pend = 0;
+    u32 lb_excl = 0, lb_t = 0, real_cnt = 0, bin_start = 0;
+    bool lb_done = true;
+    auto lookback_begin = [&](u32 t) {
+        lb_excl = 0;
+        lb_done = true;
+#ifndef SDBG_EXP_LBSKIP
+        if (t != 0) {
+            lb_done = false;
+            lb_t = t - 1;
+            lb_pend = ld_relaxed(lb + (u64)lb_t * kRadix);
+        }
 #endif
-    }
+    };
+
+    // ---- prologue: first tile up to the point where its (warp, digit) positions are known ---------------------------
+    if (tid == 0) s_tick[0] = atomicAdd(a.ticket, 1u);
+    zero_rows();
+    __syncthreads();
+    u32 tile = s_tick[0];
+    if (tile >= ntiles) return;
+    u32 cnt = tile_count(tile);
+    load_tile<W, HAS_VAL, KPT>(a, (u64)tile * TILE, cnt, wbase, key, val);
+    reserve_next();
+    count_keys();
+    __syncthreads();
+    if (tid < kRadix) real_cnt = scan_bins(tile, cnt);
+    __syncthreads();
+    if (tid < kRadix) { bin_start = scan_warps(); lookback_begin(tile); }
     __syncthreads();
 
-    // ---- scatter to shared memory in bin-sorted order ------------------------------------------------------
+    for (;; ++it) {
+        const u32 next = SDBG_PERSISTENT ? s_tick[(it + 1) & 1] : ntiles;
+        // ---- 3: rank within the warp (stable in tile order), scatter to shared memory in bin-sorted order ------
 #pragma unroll
-    for (int j = 0; j < KPT; ++j) {
-        const u32 d = digit_of<W>(key[j], pd);
-        const u32 r = (j & 1) ? (rank2[j >> 1] >> 16) : (rank2[j >> 1] & 0xffffu);
-#if SDBG_MERGE_BINSTART
-        const u32 pos = s_whist[(warp * VS + j / H) * kRadix + d] + r;
-#else
-        const u32 pos = s_binstart[d] + s_whist[(warp * VS + j / H) * kRadix + d] + r;
+        for (int j = 0; j < KPT; ++j) {
+            const u32 d = digit8_again<W, HI>(key[j], word, psel);
+            const int method = rank_method(j);                        // constant after unrolling
+            u32 m;
+#ifdef SDBG_EXP_NORANK
+            m = 1u << lane;
+            if (true) {
+            } else
 #endif
-#pragma unroll
-        for (int q = 0; q < W; ++q) s_keys[q * TILE + pos] = key[j][q];
-        if constexpr (HAS_VAL) s_vals[pos] = val[j];
-    }
-
-    // ---- decoupled look-back (one thread per bin), after the scatter so that predecessors had time to finish ---
-    if (tid < kRadix) {
-        u64 excl = 0;
-        if (tile != 0 && !SDBG_LB_SKIP) {
-            // walk back in batches of SDBG_LB_DEPTH independent loads (the chain of dependent L2 round trips is
-            // the cost of the look-back); entries not ready yet are re-polled one by one
-            long long t = (long long)tile - 1;
-            bool done = false;
-            while (!done) {
-                u64 v[SDBG_LB_DEPTH];
-#pragma unroll
-                for (int q = 0; q < SDBG_LB_DEPTH; ++q) v[q] = (t - q >= 0) ? ld_relaxed(lb + (u64)(t - q) * kRadix) : (tagG << 54);
-#pragma unroll
-                for (int q = 0; q < SDBG_LB_DEPTH; ++q) {
-                    if (!done) {
-                        u64 x = v[q];
-                        while ((x >> 54) != tagL && (x >> 54) != tagG) x = ld_relaxed(lb + (u64)(t - q) * kRadix);
-                        excl += x & kValMask;
-                        done = (x >> 54) == tagG;
-                    }
-                }
-                t -= SDBG_LB_DEPTH;
+            if (method == kMethodA) {
+                atomicOr(&wm[d], 1u << lane);
+                __syncwarp();
+                m = wm[d];
+            } else if (method == kMethodM) {
+                m = __match_any_sync(0xffffffffu, d);
+            } else {
+                m = match_ballot(d);
             }
-            st_relaxed(lb + (u64)tile * kRadix, (tagG << 54) | (excl + real_cnt));
+            const u32 prev = wp[d];                                   // same address within the group: broadcast read
+            __syncwarp();
+            if ((m >> lane) <= 1u) {                                  // highest lane of the group
+                wp[d] = prev + __popc(m);
+                if (method == kMethodA) wm[d] = 0;
+            }
+            const u32 pos = prev + __popc(m & lt);
+#pragma unroll
+            for (int q = 0; q < W; ++q) s_keys[q * TILE + pos] = key[j][q];
+            if constexpr (HAS_VAL) s_vals[pos] = val[j];
+            __syncwarp();
+            if ((j & (SDBG_LB_EVERY - 1)) == SDBG_LB_EVERY - 1 && warp < kRadix / 32)
+                lookback_poll(lb, tile, lb_t, lb_pend, lb_excl, lb_done, real_cnt, tagL, tagG);
         }
-        s_binout[tid] = a.bin_base[tid] + excl - bin_start;
-    }
-    __syncthreads();
+        zero_rows();   // own rows only; their last readers were the scan threads, two barriers ago
 
-    // ---- coalesced write-out: position p of the tile goes to bin_out[digit] + p --------------------------------
-    if (full) {
-#pragma unroll
-        for (int i = 0; i < KPT; ++i) {
-            const u32 p = i * THREADS + tid;
-            u64 kk[W];
-#pragma unroll
-            for (int q = 0; q < W; ++q) kk[q] = s_keys[q * TILE + p];
-            const u64 dst = s_binout[digit_of<W>(kk, pd)] + p;
-            store_rec<W>(a.keys_out + dst * W, kk);
-            if constexpr (HAS_VAL) a.vals_out[dst] = s_vals[p];
+        // ---- 1', 2' of the NEXT tile, with the look-back of the current one advancing behind them ------------------
+        const u32 cur_cnt = cnt;
+        u32 next_real = 0;
+        if (next < ntiles) {
+            cnt = tile_count(next);
+            load_tile<W, HAS_VAL, KPT>(a, (u64)next * TILE, cnt, wbase, key, val);
+            ++it; reserve_next(); --it;
+            count_keys();
         }
-    } else {
+        __syncthreads();
+        if (tid < kRadix) {
+            if (next < ntiles) next_real = scan_bins(next, cnt);
+            lookback_poll(lb, tile, lb_t, lb_pend, lb_excl, lb_done, real_cnt, tagL, tagG);
+        }
+        __syncthreads();
+        if (tid < kRadix) {
+            u32 next_start = 0;
+            if (next < ntiles) next_start = scan_warps();
+            // ---- 4: the look-back result is needed now -------------------------------------------------------------
+            while (!lb_done) lookback_poll(lb, tile, lb_t, lb_pend, lb_excl, lb_done, real_cnt, tagL, tagG);
+            const u64 first = a.bin_base[tid] + lb_excl - bin_start;   // output index of tile place 0 if it were in this bin
+            s_binaddr[tid] = reinterpret_cast<u64>(a.keys_out) + first * (8ull * W);
+            if constexpr (HAS_VAL) s_valaddr[tid] = reinterpret_cast<u64>(a.vals_out) + first * 4ull;
+            if (next < ntiles) { real_cnt = next_real; bin_start = next_start; lookback_begin(next); }
+        }
+        __syncthreads();
+
+        // ---- 5: coalesced write-out: place p of the tile goes to bin address[digit] + p ----------------------------
 #pragma unroll
         for (int i = 0; i < KPT; ++i) {
             const u32 p = i * THREADS + tid;
-            if (p < cnt) {
+            if (p < cur_cnt) {
                 u64 kk[W];
 #pragma unroll
                 for (int q = 0; q < W; ++q) kk[q] = s_keys[q * TILE + p];
-                const u64 dst = s_binout[digit_of<W>(kk, pd)] + p;
-                store_rec<W>(a.keys_out + dst * W, kk);
-                if constexpr (HAS_VAL) a.vals_out[dst] = s_vals[p];
+                const u32 d = digit8<W, HI>(kk, word, psel);
+#ifdef SDBG_EXP_NOSTORE
+                if (kk[0] == 0x123456789abcdefull)
+#endif
+                store_rec<W>(reinterpret_cast<u64 *>(s_binaddr[d] + (u64)p * (8u * W)), kk);
+                if constexpr (HAS_VAL) *reinterpret_cast<u32 *>(s_valaddr[d] + (u64)p * 4u) = s_vals[p];
             }
         }
+        if (next >= ntiles) break;
+        tile = next;
+        __syncthreads();   // s_keys is rewritten by the rank steps that follow
     }
-}
-
-template <int W, bool HAS_VAL>
-static constexpr size_t radix_smem_bytes() {
-    using Cfg = RadixCfg<W, HAS_VAL>;
-    constexpr size_t TILE = (size_t)Cfg::THREADS * Cfg::KPT, WARPS = Cfg::THREADS / 32;
-    constexpr size_t VW = WARPS * ((Cfg::KPT >= 2 * kVSplit) ? kVSplit : 1);
-    return TILE * W * 8 + kRadix * 8 + VW * kRadix * 4 + (HAS_VAL ? TILE * 4 : 0);
 }
 
 template <int W, bool HAS_VAL>
 static int setup_one() {
-    return (int)cudaFuncSetAttribute(onesweep_kernel<W, HAS_VAL>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                     (int)radix_smem_bytes<W, HAS_VAL>());
+    const int bytes = (int)RadixSmem<W, HAS_VAL>::kBytes;
+    int e = (int)cudaFuncSetAttribute(onesweep_kernel<W, HAS_VAL, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
+    if (e) return e;
+    return (int)cudaFuncSetAttribute(onesweep_kernel<W, HAS_VAL, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
 }
 
 int radix_setup() {
@@ -350,7 +477,13 @@ static int launch_one(const RadixArgs &a, cudaStream_t s) {
     const u64 tiles = (a.n + tile_of<W, HAS_VAL>() - 1) / tile_of<W, HAS_VAL>();
     if (tiles == 0) return 0;
     if (tiles > 0x7fffffffull) return (int)cudaErrorInvalidValue;
-    onesweep_kernel<W, HAS_VAL><<<(unsigned)tiles, RadixCfg<W, HAS_VAL>::THREADS, radix_smem_bytes<W, HAS_VAL>(), s>>>(a);
+    if (a.pass.bits != kRadixBits || (a.pass.shift & 7u)) return (int)cudaErrorInvalidValue;   // byte-aligned digits only
+    // persistent CTAs: every SM filled to the occupancy the kernel was built for
+    const u64 resident = SDBG_PERSISTENT ? (u64)kNumSMs * RadixCfg<W, HAS_VAL>::MINB : tiles;
+    const unsigned g = (unsigned)(tiles < resident ? tiles : resident), t = RadixCfg<W, HAS_VAL>::THREADS;
+    const size_t sm = RadixSmem<W, HAS_VAL>::kBytes;
+    if (a.pass.shift >= 32) onesweep_kernel<W, HAS_VAL, true><<<g, t, sm, s>>>(a);
+    else                    onesweep_kernel<W, HAS_VAL, false><<<g, t, sm, s>>>(a);
     return (int)cudaGetLastError();
 }
 
