@@ -14,6 +14,7 @@
 // HBM traffic per pass: read n*K + write n*K bytes (K = 8w) — the algorithmic 2nK of DESIGN.md "Byte model" — plus
 // 2 KiB of look-back state per tile.
 #include "kernels.cuh"
+#include <cstdio>
 
 namespace sdbg {
 
@@ -130,10 +131,16 @@ __device__ __forceinline__ void store_rec(u64 *__restrict__ o, const u64 (&k)[W]
     }
 }
 
-// One non-blocking step of the decoupled look-back of one bin (see phase 3 of onesweep_kernel): consume the entry
-// requested earlier if it has been published for this pass, then request the next predecessor (or the same one
-// again); on reaching an inclusive (GLOBAL) entry publish this tile's inclusive prefix. Entry = tag (status, epoch)
-// in bits 63..54, 32-bit count in bits 31..0: one sort range holds fewer than 2^32 records (api.cu range_capacity).
+// One non-blocking step of the decoupled look-back of one bin (see phase 3 of onesweep_kernel).
+// Entry of (tile u, bin) = tag (status, epoch) in bits 63..54, span s in bits 53..32, 32-bit count v in bits 31..0:
+//   LOCAL : v = keys of this bin in tiles (u-s, u]   (s = 1 when first published: the tile's own count)
+//   GLOBAL: v = keys of this bin in tiles [0, u]
+// A walker consumes the entry it requested earlier if it has been published for this pass, jumps over the whole
+// span it covers, RE-PUBLISHES its own entry with the span it has covered so far (so later tiles jump over it in
+// one step: pointer doubling, the walk is logarithmic in the distance to the nearest GLOBAL entry instead of
+// linear), and requests the next entry. On reaching a GLOBAL entry it publishes its inclusive prefix.
+// One sort range holds fewer than 2^32 records (api.cu range_capacity), so counts fit 32 bits.
+constexpr u32 kSpanMask = (1u << 22) - 1u;
 __device__ __forceinline__ void lookback_poll(u64 *lb, u32 tile, u32 &t, u64 &pend, u32 &excl, bool &done, u32 real_cnt,
                                               u32 tagL, u32 tagG) {
     if (done) return;
@@ -145,7 +152,8 @@ __device__ __forceinline__ void lookback_poll(u64 *lb, u32 tile, u32 &t, u64 &pe
             st_relaxed(lb + (u64)tile * kRadix, ((u64)tagG << 54) | (u64)(excl + real_cnt));
             return;
         }
-        --t;   // tile 0 always publishes GLOBAL, so t never passes it
+        t -= (u32)(pend >> 32) & kSpanMask;   // tile 0 always publishes GLOBAL, so t never passes it
+        st_relaxed(lb + (u64)tile * kRadix, ((u64)tagL << 54) | ((u64)(tile - t) << 32) | (u64)(excl + real_cnt));
     }
     pend = ld_relaxed(lb + (u64)t * kRadix);
 }
@@ -295,7 +303,7 @@ onesweep_kernel(RadixArgs a) {
         for (int v = 0; v < WARPS; ++v) my_cnt += s_pos[v * kRadix + tid];
         u32 rc = my_cnt;                                                  // my_cnt includes the pads (bin 255)
         if (tid == kRadix - 1) rc -= (u32)TILE - tcnt;
-        st_relaxed(lb + (u64)t * kRadix, ((u64)(t == 0 ? tagG : tagL) << 54) | rc);
+        st_relaxed(lb + (u64)t * kRadix, ((u64)(t == 0 ? tagG : tagL) << 54) | (t == 0 ? 0ull : 1ull << 32) | rc);
         incl = warp_incl_scan_add(my_cnt);
         if (lane == 31) s_wtot[warp] = incl;
         return rc;
@@ -335,6 +343,10 @@ onesweep_kernel(RadixArgs a) {
 #endif
     };
 
+#ifdef SDBG_EXP_TRACE
+    long long tr_block = 0, tr_start = clock64();
+    u32 tr_polls = 0, tr_depth = 0, tr_pre = 0, tr_tiles = 0;
+#endif
     // ---- prologue: first tile up to the point where its (warp, digit) positions are known ---------------------------
     if (tid == 0) s_tick[0] = atomicAdd(a.ticket, 1u);
     zero_rows();
@@ -408,7 +420,15 @@ onesweep_kernel(RadixArgs a) {
             u32 next_start = 0;
             if (next < ntiles) next_start = scan_warps();
             // ---- 4: the look-back result is needed now -------------------------------------------------------------
+#ifdef SDBG_EXP_TRACE
+            const long long tr0 = clock64();
+            const u32 trd = tile - lb_t;
+            u32 trn = 0;
+            while (!lb_done) { lookback_poll(lb, tile, lb_t, lb_pend, lb_excl, lb_done, real_cnt, tagL, tagG); ++trn; }
+            if (tid == 0) { tr_block += clock64() - tr0; tr_polls += trn; tr_depth += tile - lb_t; tr_pre += trd; ++tr_tiles; }
+#else
             while (!lb_done) lookback_poll(lb, tile, lb_t, lb_pend, lb_excl, lb_done, real_cnt, tagL, tagG);
+#endif
             const u64 first = a.bin_base[tid] + lb_excl - bin_start;   // output index of tile place 0 if it were in this bin
             s_binaddr[tid] = reinterpret_cast<u64>(a.keys_out) + first * (8ull * W);
             if constexpr (HAS_VAL) s_valaddr[tid] = reinterpret_cast<u64>(a.vals_out) + first * 4ull;
@@ -432,6 +452,11 @@ onesweep_kernel(RadixArgs a) {
                 if constexpr (HAS_VAL) *reinterpret_cast<u32 *>(s_valaddr[d] + (u64)p * 4u) = s_vals[p];
             }
         }
+#ifdef SDBG_EXP_TRACE
+        if (next >= ntiles && tid == 0 && a.epoch == 4 && blockIdx.x % 29 == 0)
+            printf("TRACE cta %u tiles %u total_cyc %lld blocked_cyc %lld blocking_polls/tile %.2f depth_before_block %.2f final_depth %.2f\n", blockIdx.x, tr_tiles,
+                   clock64() - tr_start, tr_block, (double)tr_polls / tr_tiles, (double)tr_pre / tr_tiles, (double)tr_depth / tr_tiles);
+#endif
         if (next >= ntiles) break;
         tile = next;
         __syncthreads();   // s_keys is rewritten by the rank steps that follow
