@@ -26,7 +26,7 @@ namespace sdbg {
 // The kernel is bound by instruction issue and shared-memory wavefronts at the same time,
 // so the steps are split between B and A to load both pipes equally.
 #ifndef SDBG_LB_EVERY
-#define SDBG_LB_EVERY 4      // rank steps between two look-back polls (power of two)
+#define SDBG_LB_EVERY 2      // rank steps between two look-back polls (power of two)
 #endif
 #ifndef SDBG_PERSISTENT
 #define SDBG_PERSISTENT 1    // 1: persistent CTAs holding the ticket of their next tile; 0: one tile per CTA
@@ -86,19 +86,22 @@ __device__ __forceinline__ u32 digit8(const u64 (&key)[W], u32 word, u32 psel) {
     return __byte_perm(HI ? (u32)(kw >> 32) : (u32)kw, 0u, psel);
 }
 
-// lanes of the warp whose 8-bit digit equals mine: 8 ballots, 3-4 SASS instructions per bit
-// (R2P/LOP3 -> predicates, VOTE, predicated NOT, AND).
+// lanes of the warp whose 8-bit digit equals mine: per bit one ballot, inverted by the lanes whose bit is clear,
+// and the eight masks ANDed three at a time (R2P/LOP3 -> predicates, 8 VOTE, 8 predicated NOT, 4 LOP3).
 __device__ __forceinline__ u32 match_ballot(u32 d) {
-    u32 m = 0xffffffffu;
+    u32 b[kRadixBits];
 #pragma unroll
-    for (int b = 0; b < kRadixBits; ++b) {
-        asm("{\n\t.reg .pred p;\n\t.reg .b32 t, bal;\n\t"
+    for (int i = 0; i < kRadixBits; ++i) {
+        asm("{\n\t.reg .pred p;\n\t.reg .b32 t;\n\t"
             "and.b32 t, %1, %2;\n\tsetp.ne.u32 p, t, 0;\n\t"
-            "vote.sync.ballot.b32 bal, p, 0xffffffff;\n\t"
-            "@!p not.b32 bal, bal;\n\t"
-            "and.b32 %0, %0, bal;\n\t}" : "+r"(m) : "r"(d), "r"(1u << b));
+            "vote.sync.ballot.b32 %0, p, 0xffffffff;\n\t"
+            "@!p not.b32 %0, %0;\n\t}" : "=r"(b[i]) : "r"(d), "r"(1u << i));
     }
-    return m;
+    u32 m0, m1, m2;
+    asm("lop3.b32 %0, %1, %2, %3, 0x80;" : "=r"(m0) : "r"(b[0]), "r"(b[1]), "r"(b[2]));
+    asm("lop3.b32 %0, %1, %2, %3, 0x80;" : "=r"(m1) : "r"(b[3]), "r"(b[4]), "r"(b[5]));
+    asm("lop3.b32 %0, %1, %2, %3, 0x80;" : "=r"(m2) : "r"(b[6]), "r"(b[7]), "r"(m0));
+    return m1 & m2;
 }
 
 template <int W>
@@ -437,20 +440,23 @@ onesweep_kernel(RadixArgs a) {
         __syncthreads();
 
         // ---- 5: coalesced write-out: place p of the tile goes to bin address[digit] + p ----------------------------
+        auto write_place = [&](u32 p) {
+            u64 kk[W];
 #pragma unroll
-        for (int i = 0; i < KPT; ++i) {
-            const u32 p = i * THREADS + tid;
-            if (p < cur_cnt) {
-                u64 kk[W];
-#pragma unroll
-                for (int q = 0; q < W; ++q) kk[q] = s_keys[q * TILE + p];
-                const u32 d = digit8<W, HI>(kk, word, psel);
+            for (int q = 0; q < W; ++q) kk[q] = s_keys[q * TILE + p];
+            const u32 d = digit8<W, HI>(kk, word, psel);
 #ifdef SDBG_EXP_NOSTORE
-                if (kk[0] == 0x123456789abcdefull)
+            if (kk[0] == 0x123456789abcdefull)
 #endif
-                store_rec<W>(reinterpret_cast<u64 *>(s_binaddr[d] + (u64)p * (8u * W)), kk);
-                if constexpr (HAS_VAL) *reinterpret_cast<u32 *>(s_valaddr[d] + (u64)p * 4u) = s_vals[p];
-            }
+            store_rec<W>(reinterpret_cast<u64 *>(s_binaddr[d] + (u64)p * (8u * W)), kk);
+            if constexpr (HAS_VAL) *reinterpret_cast<u32 *>(s_valaddr[d] + (u64)p * 4u) = s_vals[p];
+        };
+        if (cur_cnt == (u32)TILE) {
+#pragma unroll
+            for (int i = 0; i < KPT; ++i) write_place(i * THREADS + tid);
+        } else {
+#pragma unroll 1
+            for (u32 p = tid; p < cur_cnt; p += THREADS) write_place(p);
         }
 #ifdef SDBG_EXP_TRACE
         if (next >= ntiles && tid == 0 && a.epoch == 4 && blockIdx.x % 29 == 0)
