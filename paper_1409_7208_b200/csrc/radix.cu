@@ -32,7 +32,7 @@ namespace sdbg {
 #define SDBG_PERSISTENT 1    // 1: persistent CTAs holding the ticket of their next tile; 0: one tile per CTA
 #endif
 #ifndef SDBG_RANK_METHODS
-#define SDBG_RANK_METHODS "B"
+#define SDBG_RANK_METHODS "BBBBBM"
 #endif
 
 template <int W, bool HAS_VAL> struct RadixCfg;
@@ -184,7 +184,8 @@ struct RadixSmem {
     static constexpr size_t kKeys = 0;                                             // u64[W][TILE]
     static constexpr size_t kBinAddr = kKeys + (size_t)TILE * W * 8;              // u64[256] byte address of bin run - tile start
     static constexpr size_t kValAddr = kBinAddr + kRadix * 8;                       // u64[256] (HAS_VAL)
-    static constexpr size_t kPos = kValAddr + (HAS_VAL ? kRadix * 8 : 0);           // u32[WARPS][256] counts, then tile positions
+    static constexpr size_t kBinInfo = kValAddr + (HAS_VAL ? kRadix * 8 : 0);       // u32[2][256] tile count and tile start of the bins
+    static constexpr size_t kPos = kBinInfo + 2 * kRadix * 4;                       // u32[WARPS][256] counts, then tile positions
     static constexpr size_t kMask = kPos + (size_t)WARPS * kRadix * 4;              // u32[WARPS][256] match masks (method A)
     static constexpr size_t kVals = kMask + (USE_A ? (size_t)WARPS * kRadix * 4 : 0);  // u32[TILE] (HAS_VAL)
     static constexpr size_t kBytes = kVals + (HAS_VAL ? (size_t)TILE * 4 : 0);
@@ -249,6 +250,7 @@ onesweep_kernel(RadixArgs a) {
     u64 *s_keys = reinterpret_cast<u64 *>(smem_raw + L::kKeys);
     u64 *s_binaddr = reinterpret_cast<u64 *>(smem_raw + L::kBinAddr);
     u64 *s_valaddr = reinterpret_cast<u64 *>(smem_raw + L::kValAddr);
+    u32 *s_real = reinterpret_cast<u32 *>(smem_raw + L::kBinInfo), *s_bstart = s_real + kRadix;
     u32 *s_pos = reinterpret_cast<u32 *>(smem_raw + L::kPos);
     u32 *s_mask = reinterpret_cast<u32 *>(smem_raw + L::kMask);
     u32 *s_vals = reinterpret_cast<u32 *>(smem_raw + L::kVals);
@@ -264,7 +266,11 @@ onesweep_kernel(RadixArgs a) {
     u32 *wp = s_pos + warp * kRadix;
     u32 *wm = s_mask + warp * kRadix;
     const u32 tagL = ((u32)kStLocal << 8) | a.epoch, tagG = ((u32)kStGlobal << 8) | a.epoch;
-    u64 *lb = a.lookback + tid;
+    // two roles of one thread per bin: the first 256 threads scan the histograms, the LAST 256 run the look-back,
+    // so that the two chains of dependent shared / L2 round trips proceed side by side
+    const bool scanner = tid < kRadix, walker = tid >= THREADS - kRadix;
+    u64 *lb = a.lookback + (walker ? tid - (THREADS - kRadix) : tid);   // scanners publish LOCAL of their own bin
+    const u32 wbin = tid - (THREADS - kRadix);
 
     // warp-private histogram rows start at zero (and are zeroed again by their warp after every rank phase)
     auto zero_rows = [&]() {
@@ -300,20 +306,20 @@ onesweep_kernel(RadixArgs a) {
     };
     // phase 2a (one thread per bin, after a block barrier): tile count, published LOCAL at once; scan over the bins
     u32 my_cnt = 0, incl = 0;
-    auto scan_bins = [&](u32 t, u32 tcnt) -> u32 {
+    auto scan_bins = [&](u32 t, u32 tcnt) {
         my_cnt = 0;
 #pragma unroll
         for (int v = 0; v < WARPS; ++v) my_cnt += s_pos[v * kRadix + tid];
         u32 rc = my_cnt;                                                  // my_cnt includes the pads (bin 255)
         if (tid == kRadix - 1) rc -= (u32)TILE - tcnt;
-        st_relaxed(lb + (u64)t * kRadix, ((u64)(t == 0 ? tagG : tagL) << 54) | (t == 0 ? 0ull : 1ull << 32) | rc);
+        st_relaxed(a.lookback + tid + (u64)t * kRadix, ((u64)(t == 0 ? tagG : tagL) << 54) | (t == 0 ? 0ull : 1ull << 32) | rc);
+        s_real[tid] = rc;
         incl = warp_incl_scan_add(my_cnt);
         if (lane == 31) s_wtot[warp] = incl;
-        return rc;
     };
     // phase 2b (after another barrier): entry (v, bin) becomes the tile position of the first key of digit `bin`
     // held by warp v; returns the tile position of the bin's first key
-    auto scan_warps = [&]() -> u32 {
+    auto scan_warps = [&]() {
         u32 off = 0;
 #pragma unroll
         for (int w = 0; w < kRadix / 32; ++w) off += (w < (int)warp) ? s_wtot[w] : 0u;
@@ -325,7 +331,7 @@ onesweep_kernel(RadixArgs a) {
             s_pos[v * kRadix + tid] = run;
             run += t;
         }
-        return bs;
+        s_bstart[tid] = bs;
     };
 
     // Decoupled look-back state of the CURRENT tile, one thread per bin. It advances during the rank steps of the
@@ -334,7 +340,9 @@ onesweep_kernel(RadixArgs a) {
     u64 lb_pend = 0;
     u32 lb_excl = 0, lb_t = 0, real_cnt = 0, bin_start = 0;
     bool lb_done = true;
-    auto lookback_begin = [&](u32 t) {
+    auto lookback_begin = [&](u32 t) {   // after the barrier that follows scan_warps of tile t
+        real_cnt = s_real[wbin];
+        bin_start = s_bstart[wbin];
         lb_excl = 0;
         lb_done = true;
 #ifndef SDBG_EXP_LBSKIP
@@ -361,10 +369,11 @@ onesweep_kernel(RadixArgs a) {
     reserve_next();
     count_keys();
     __syncthreads();
-    if (tid < kRadix) real_cnt = scan_bins(tile, cnt);
+    if (scanner) scan_bins(tile, cnt);
     __syncthreads();
-    if (tid < kRadix) { bin_start = scan_warps(); lookback_begin(tile); }
+    if (scanner) scan_warps();
     __syncthreads();
+    if (walker) lookback_begin(tile);
 
     for (;; ++it) {
         const u32 next = SDBG_PERSISTENT ? s_tick[(it + 1) & 1] : ntiles;
@@ -399,14 +408,13 @@ onesweep_kernel(RadixArgs a) {
             for (int q = 0; q < W; ++q) s_keys[q * TILE + pos] = key[j][q];
             if constexpr (HAS_VAL) s_vals[pos] = val[j];
             __syncwarp();
-            if ((j & (SDBG_LB_EVERY - 1)) == SDBG_LB_EVERY - 1 && warp < kRadix / 32)
+            if ((j & (SDBG_LB_EVERY - 1)) == SDBG_LB_EVERY - 1 && walker)
                 lookback_poll(lb, tile, lb_t, lb_pend, lb_excl, lb_done, real_cnt, tagL, tagG);
         }
         zero_rows();   // own rows only; their last readers were the scan threads, two barriers ago
 
         // ---- 1', 2' of the NEXT tile, with the look-back of the current one advancing behind them ------------------
         const u32 cur_cnt = cnt;
-        u32 next_real = 0;
         if (next < ntiles) {
             cnt = tile_count(next);
             load_tile<W, HAS_VAL, KPT>(a, (u64)next * TILE, cnt, wbase, key, val);
@@ -414,30 +422,19 @@ onesweep_kernel(RadixArgs a) {
             count_keys();
         }
         __syncthreads();
-        if (tid < kRadix) {
-            if (next < ntiles) next_real = scan_bins(next, cnt);
-            lookback_poll(lb, tile, lb_t, lb_pend, lb_excl, lb_done, real_cnt, tagL, tagG);
-        }
+        if (scanner && next < ntiles) scan_bins(next, cnt);
+        if (walker) lookback_poll(lb, tile, lb_t, lb_pend, lb_excl, lb_done, real_cnt, tagL, tagG);
         __syncthreads();
-        if (tid < kRadix) {
-            u32 next_start = 0;
-            if (next < ntiles) next_start = scan_warps();
+        if (scanner && next < ntiles) scan_warps();
+        if (walker) {
             // ---- 4: the look-back result is needed now -------------------------------------------------------------
-#ifdef SDBG_EXP_TRACE
-            const long long tr0 = clock64();
-            const u32 trd = tile - lb_t;
-            u32 trn = 0;
-            while (!lb_done) { lookback_poll(lb, tile, lb_t, lb_pend, lb_excl, lb_done, real_cnt, tagL, tagG); ++trn; }
-            if (tid == 0) { tr_block += clock64() - tr0; tr_polls += trn; tr_depth += tile - lb_t; tr_pre += trd; ++tr_tiles; }
-#else
             while (!lb_done) lookback_poll(lb, tile, lb_t, lb_pend, lb_excl, lb_done, real_cnt, tagL, tagG);
-#endif
-            const u64 first = a.bin_base[tid] + lb_excl - bin_start;   // output index of tile place 0 if it were in this bin
-            s_binaddr[tid] = reinterpret_cast<u64>(a.keys_out) + first * (8ull * W);
-            if constexpr (HAS_VAL) s_valaddr[tid] = reinterpret_cast<u64>(a.vals_out) + first * 4ull;
-            if (next < ntiles) { real_cnt = next_real; bin_start = next_start; lookback_begin(next); }
+            const u64 first = a.bin_base[wbin] + lb_excl - bin_start;   // output index of tile place 0 if it were in this bin
+            s_binaddr[wbin] = reinterpret_cast<u64>(a.keys_out) + first * (8ull * W);
+            if constexpr (HAS_VAL) s_valaddr[wbin] = reinterpret_cast<u64>(a.vals_out) + first * 4ull;
         }
         __syncthreads();
+        if (walker && next < ntiles) lookback_begin(next);
 
         // ---- 5: coalesced write-out: place p of the tile goes to bin address[digit] + p ----------------------------
         auto write_place = [&](u32 p) {
