@@ -21,7 +21,9 @@ inline const u64 *U64C(const uint64_t *p) { return reinterpret_cast<const u64 *>
 
 // fixed region at the start of the workspace
 constexpr u64 kOffState = 0;
-constexpr u64 kOffDigitHist = 1024;                                         // u64[kMaxPasses][256]
+constexpr u64 kOffStatSlots = 1024;                                         // u64[kStatSlots][kStatSlotWords]
+constexpr u64 kStatBytes = (u64)kStatSlots * kStatSlotWords * 8;
+constexpr u64 kOffDigitHist = kOffStatSlots + kStatBytes;                   // u64[kMaxPasses][256]
 constexpr u64 kOffBucketHist = kOffDigitHist + (u64)kMaxPasses * kRadix * 8;  // u64[65536]
 constexpr u64 kFixedBytes = (kOffBucketHist + (u64)SDBG_NUM_BUCKETS * 8 + 4095) / 4096 * 4096;
 static_assert(sizeof(DevState) <= 1024, "DevState must fit its slot");
@@ -42,6 +44,7 @@ struct sdbg_ctx {
     sdbg_timing acc{};
 
     DevState *st() const { return reinterpret_cast<DevState *>(ws + kOffState); }
+    u64 *stat_slots() const { return reinterpret_cast<u64 *>(ws + kOffStatSlots); }
     u64 *digit_hist() const { return reinterpret_cast<u64 *>(ws + kOffDigitHist); }
     u64 *bucket_hist() const { return reinterpret_cast<u64 *>(ws + kOffBucketHist); }
     char *dyn() const { return ws + kFixedBytes; }
@@ -104,7 +107,7 @@ bool is_device_ptr(const void *p) {
 u64 range_need(u64 n, u32 W) {
     const u64 K = 8ull * W;
     const u64 rt = radix_tile_records(W, false), ct = count_tile_records(W);
-    return 2 * align_up(n * K) + align_up(((n + rt - 1) / rt + 1) * kRadix * 8) + align_up(((n + ct - 1) / ct + 1) * 2 * 8);
+    return 2 * align_up(n * K) + align_up(((n + rt - 1) / rt + 1) * kRadix * 8) + align_up(((n + ct - 1) / ct + 1) * 8);
 }
 // largest n with range_need(n) <= avail; one sort range holds fewer than 2^32 records (the look-back words of the
 // radix passes carry 32-bit counts), larger inputs are split into block-wise ranges like any input that does not fit

@@ -77,16 +77,17 @@ __device__ __forceinline__ u64 warp_reduce_add64(u64 v) {
     return v;
 }
 
+// Statistics counters are spread over kStatSlots slots of one 128-byte line each (tile & 31 picks the slot), so that
+// the one-atomic-per-block updates do not serialise on one L2 address; the host adds the slots up.
+constexpr int kStatSlots = 32, kStatSlotWords = 16;   // words: 0 n_distinct, 1 sum_solid_mult, 2 csum_distinct
+
 // ---- device-side scalars living at the start of the workspace -----------------------------------------
 struct DevState {
     u64 bad_base;          // min index of a non-ACGT byte, ~0 if none
     u64 n_windows;         // valid (k+1)-windows in the packed reads
     u64 extract_cursor;    // records written by the extractor in this range
     u64 out_cursor[2];     // solid edges appended so far (may exceed cap: needed count); range r reads slot r&1, writes slot (r+1)&1
-    u64 n_distinct;
-    u64 sum_solid_mult;
     u64 csum_raw;
-    u64 csum_distinct;
     u64 merge_heads;       // sdbg_build unsorted path: distinct keys
     u32 tickets[kMaxPasses + 4];  // per-pass tile tickets; [kMaxPasses] = count kernel ticket
 };

@@ -2,50 +2,53 @@
 // "all (k+1)-mers from the input reads are sorted and counted, and only (k+1)-mers that appear at least d (2 by
 // default) times are kept" (§2 ¶3; cnt >= d, reading A8; counts saturate at 2^32-1, A9).
 //
-// One streaming pass. A record i is a run TAIL iff i == n-1 or key[i] != key[i+1]; the run ending at tail i has
-// length (i+1) - (index+1 of the previous tail). Runs may span any number of tiles, so the "previous tail" is an
-// exclusive max-scan and the output position an exclusive sum-scan, both chained across tiles by decoupled
-// look-back (one warp inspects 32 predecessors at a time). Tiles are ordered by an atomic ticket.
+// Two streaming sweeps and a scan between them; see count_tiles_kernel.
 //
 // Also here: the merge kernels of sdbg_build's unsorted path (equal keys merged by summing mult).
 #include "kernels.cuh"
 
 namespace sdbg {
 
-constexpr u64 kLbVal = (1ull << 62) - 1;
-
-// Decoupled look-back over per-tile status words ([63:62] status, [61:0] value); called by all 32 lanes of ONE warp.
-// Publishes this tile's aggregate, returns the exclusive prefix over tiles [0, tile), then publishes the inclusive one.
+// Decoupled look-back over per-tile status words, exclusive SUM over tiles [0, tile); called by all 32 lanes of ONE warp.
+// Word of tile u: [63:62] status, [61:40] span s, [39:0] value v.
+//   LOCAL : v = aggregate of tiles (u-s, u]   (s = 1 when first published: the tile's own aggregate)
+//   GLOBAL: v = aggregate of tiles [0, u]
+// A round reads the 32 words below the current position at once and walks through them, jumping over the span each
+// word covers; after every round the tile RE-PUBLISHES its own word with the span covered so far, so that later tiles
+// jump over it in one step (pointer doubling). Without the spans a round advances at most 32 tiles per L2 round trip,
+// which caps the whole kernel at 32 tiles per round-trip time however many tiles are in flight.
+constexpr u64 kLbVal = (1ull << 40) - 1;
+constexpr u32 kLbSpanMask = (1u << 22) - 1u;
 template <bool IS_MAX>
 __device__ __forceinline__ u64 tile_lookback(u64 *state, u32 tile, u64 aggregate) {
+    static_assert(!IS_MAX, "sum only");
     const u32 lane = lane_id();
     if (tile == 0) {
         if (lane == 0) st_relaxed(state, (kStGlobal << 62) | aggregate);
         return 0;
     }
-    if (lane == 0) st_relaxed(state + tile, (kStLocal << 62) | aggregate);
+    if (lane == 0) st_relaxed(state + tile, (kStLocal << 62) | (1ull << 40) | aggregate);
     u64 excl = 0;
-    long long pos = (long long)tile - 1;
+    long long t = (long long)tile - 1;
     while (true) {
-        const long long idx = pos - (long long)lane;
+        const long long idx = t - (long long)lane;
         u64 v = kStGlobal << 62;   // virtual tiles before the first: inclusive identity
-        if (idx >= 0) {
-            do { v = ld_relaxed(state + idx); } while ((v >> 62) == kStInvalid);
+        if (idx >= 0) v = ld_relaxed(state + idx);
+        u32 k = 0;
+        bool done = false;
+        while (k < 32u) {
+            const u64 e = __shfl_sync(0xffffffffu, v, (int)k);
+            const u32 status = (u32)(e >> 62);
+            if (status == (u32)kStInvalid) break;           // not published yet: read again from here
+            excl += e & kLbVal;
+            if (status == (u32)kStGlobal) { done = true; break; }
+            k += (u32)(e >> 40) & kLbSpanMask;
         }
-        const u32 gm = __ballot_sync(0xffffffffu, (v >> 62) == kStGlobal);
-        const u32 first = gm ? (u32)__ffs(gm) - 1u : 31u;
-        u64 x = (lane <= first) ? (v & kLbVal) : 0ull;
-#pragma unroll
-        for (int o = 16; o > 0; o >>= 1) {
-            const u64 y = __shfl_xor_sync(0xffffffffu, x, o);
-            x = IS_MAX ? (x > y ? x : y) : (x + y);
-        }
-        excl = IS_MAX ? (excl > x ? excl : x) : (excl + x);
-        if (gm) break;
-        pos -= 32;
+        if (done) break;
+        t -= (long long)k;
+        if (k && lane == 0) st_relaxed(state + tile, (kStLocal << 62) | ((u64)(tile - 1 - t) + 1ull) << 40 | (excl + aggregate));
     }
-    const u64 inc = IS_MAX ? (excl > aggregate ? excl : aggregate) : (excl + aggregate);
-    if (lane == 0) st_relaxed(state + tile, (kStGlobal << 62) | inc);
+    if (lane == 0) st_relaxed(state + tile, (kStGlobal << 62) | (excl + aggregate));
     return excl;
 }
 
@@ -97,37 +100,72 @@ __device__ __forceinline__ bool key_ne(const u64 (&a)[W], const u64 (&b)[W]) {
     return ne;
 }
 
-template <int W> struct CountCfg { static constexpr int THREADS = 512, IPT = (W == 1 ? 8 : W == 2 ? 4 : 2); };
-
 template <int W>
-__global__ void __launch_bounds__(CountCfg<W>::THREADS) count_filter_kernel(CountArgs a, DevState *st) {
-    constexpr int THREADS = CountCfg<W>::THREADS, IPT = CountCfg<W>::IPT, TILE = THREADS * IPT;
-    __shared__ u32 s_tile;
-    __shared__ u32 s_warp[THREADS / 32];
-    __shared__ u64 s_bcast[2];
+__device__ __forceinline__ bool key_lt(const u64 (&a)[W], const u64 (&b)[W]) {   // unsigned multi-word a < b
+    bool lt = false, eq = true;
+#pragma unroll
+    for (int q = 0; q < W; ++q) {
+        lt = lt || (eq && a[q] < b[q]);
+        eq = eq && a[q] == b[q];
+    }
+    return lt;
+}
+
+// 64 bytes of consecutive records per thread (vector loads), 6 blocks of 256 threads per SM
+#ifndef SDBG_CNT_THREADS
+#define SDBG_CNT_THREADS 256
+#define SDBG_CNT_MINB 6
+#define SDBG_CNT_BYTES 64
+#endif
+template <int W> struct CountCfg { static constexpr int THREADS = SDBG_CNT_THREADS, IPT = SDBG_CNT_BYTES / 8 / W; };
+template <> struct CountCfg<3> { static constexpr int THREADS = SDBG_CNT_THREADS, IPT = SDBG_CNT_BYTES / 32; };
+
+// Two sweeps over the sorted records with one tiny scan between them, instead of one sweep whose tiles are chained by a
+// decoupled look-back: a tile here is 32 KiB and lives a few microseconds, so a chain that costs several L2 round
+// trips per tile (measured: ~5 us of a ~9 us tile life) caps the single-sweep kernel far below the
+// cost of simply reading the records twice.
+//   sweep 1 (WRITE = false): solid edges of every tile -> tile_sums[tile]; statistics
+//   scan                   : tile_sums -> exclusive prefix, total -> output cursor
+//   sweep 2 (WRITE = true) : the same arithmetic again, solid edges written at out_base + prefix[tile] + rank in tile
+//
+// A record i is a run TAIL iff i == n-1 or key[i] != key[i+1]; the run ending at tail i has length i+1 - (start of
+// the run). Inside a warp's 32*IPT records the start is the place after the previous tail (exclusive max-scan over
+// the lanes, by shuffles); for the run that is open at the warp's first record it is found by looking at the records
+// right before it, 32 at a time, and, past 128 of them, by a 32-ary search for the first record equal to it (the
+// records are sorted). So no state about runs travels between warps or tiles. All indices are tile-relative u32
+// (modulo 2^32: a sort range holds fewer than 2^32 records, so run lengths come out right even when a run began
+// before the tile).
+template <int W, bool WRITE>
+__global__ void __launch_bounds__(CountCfg<W>::THREADS, SDBG_CNT_MINB) count_tiles_kernel(CountArgs a, DevState *st) {
+    constexpr int THREADS = CountCfg<W>::THREADS, IPT = CountCfg<W>::IPT, TILE = THREADS * IPT, WARPS = THREADS / 32;
+    __shared__ u32 s_wsolid[WARPS];
+    __shared__ u64 s_red[3][WARPS];
     const u32 tid = threadIdx.x, lane = tid & 31u, warp = tid >> 5;
-    if (tid == 0) s_tile = atomicAdd(a.ticket, 1u);
-    __syncthreads();
-    const u32 tile = s_tile;
-    const u32 ntiles = (u32)((a.n + TILE - 1) / TILE);
+    const u32 tile = blockIdx.x;
     const u64 tile_base = (u64)tile * TILE;
-    const u64 idx0 = tile_base + (u64)tid * IPT;
-    const u64 out_base = st->out_cursor[a.range_parity];   // solid edges appended by earlier ranges (never written by this launch)
+    const u32 rem = (a.n - tile_base < (u64)TILE) ? (u32)(a.n - tile_base) : (u32)TILE;   // records of this tile
+    const bool has_succ = tile_base + TILE < a.n;       // a record follows the tile
+    const u32 li0 = tid * IPT;                           // tile-relative index of my first record
+    const u64 *kp = a.keys + (tile_base + li0) * W;
 
     // ---- load IPT consecutive records + the one after them -------------------------------------------------------
     u64 key[IPT + 1][W];
-    if (idx0 + IPT + 1 <= a.n && W == 1) {
-        // vector path: IPT*8 bytes are 16-byte aligned
+    if (li0 + IPT < rem || (li0 + IPT == rem && has_succ)) {
+        if constexpr (W == 1) {
 #pragma unroll
-        for (int j = 0; j < IPT; j += 2) {
-            ulonglong2 v = *reinterpret_cast<const ulonglong2 *>(a.keys + idx0 + j);
-            key[j][0] = v.x; key[j + 1][0] = v.y;
+            for (int j = 0; j < IPT; j += 2) {      // 64 bytes per thread, 16-byte aligned
+                ulonglong2 v = *reinterpret_cast<const ulonglong2 *>(kp + j);
+                key[j][0] = v.x; key[j + 1][0] = v.y;
+            }
+            key[IPT][0] = kp[IPT];
+        } else {
+#pragma unroll
+            for (int j = 0; j <= IPT; ++j) load_key<W>(kp, j, key[j]);
         }
-        key[IPT][0] = a.keys[idx0 + IPT];
     } else {
 #pragma unroll
         for (int j = 0; j <= IPT; ++j) {
-            if (idx0 + j < a.n) load_key<W>(a.keys, idx0 + j, key[j]);
+            if (li0 + j < rem) load_key<W>(kp, j, key[j]);
             else {
 #pragma unroll
                 for (int q = 0; q < W; ++q) key[j][q] = 0;
@@ -137,69 +175,140 @@ __global__ void __launch_bounds__(CountCfg<W>::THREADS) count_filter_kernel(Coun
     u32 tails = 0, last_local = 0;   // last_local: tile-relative index+1 of my last tail (0 = none)
 #pragma unroll
     for (int j = 0; j < IPT; ++j) {
-        const u64 idx = idx0 + j;
-        const bool t = idx < a.n && (idx + 1 == a.n || key_ne<W>(key[j], key[j + 1]));
-        if (t) { tails |= 1u << j; last_local = tid * IPT + j + 1; }
+        const u32 li = li0 + j;
+        const bool t = li < rem && ((li + 1 == rem && !has_succ) || key_ne<W>(key[j], key[j + 1]));
+        if (t) { tails |= 1u << j; last_local = li + 1; }
     }
 
-    // ---- previous tail: exclusive max-scan in the block, look-back across tiles --------------------------------
-    u32 tile_max;
-    const u32 excl_max = block_excl_scan<THREADS, true>(last_local, s_warp, tile_max);
-    if (warp == 0) {
-        const u64 p = tile_lookback<true>(a.lookback, tile, tile_max ? tile_base + tile_max : 0ull);
-        if (lane == 0) s_bcast[0] = p;
+    // ---- start of the run in progress at my first record ----------------------------------------------------------
+    // exclusive max-scan of the tails over the lanes: the value of the nearest lower lane that has a tail
+    const u32 tmask = __ballot_sync(0xffffffffu, last_local != 0) & lanemask_lt();
+    u32 excl_max = __shfl_sync(0xffffffffu, last_local, tmask ? 31 - __clz(tmask) : 0);
+    if (!tmask) excl_max = 0;
+    // the run open at the warp's first record (needed by the lanes with no tail before them in the warp)
+    const u32 wfirst = warp * 32u * IPT;                 // tile-relative index of the warp's first record
+    u32 wstart = wfirst;
+    if (wfirst < rem) {
+        u64 target[W], probe[W];
+#pragma unroll
+        for (int q = 0; q < W; ++q) target[q] = __shfl_sync(0xffffffffu, key[0][q], 0);
+        // hi = lowest index known to belong to the run. Up to 4 rounds over the 32 records right below hi (these lines
+        // were just read by the neighbouring warp or tile), then a 32-ary search over all that lies below.
+        u64 hi = tile_base + wfirst;
+        bool found = false;
+#pragma unroll 1
+        for (int r = 0; r < 4 && !found && hi > 0; ++r) {
+            const bool inb = hi > (u64)lane;
+            if (inb) load_key<W>(a.keys, hi - 1 - lane, probe);
+            const u32 eqm = __ballot_sync(0xffffffffu, inb && !key_ne<W>(probe, target));
+            const u32 lead = (eqm == 0xffffffffu) ? 32u : (u32)__ffs(~eqm) - 1u;   // equal records right below hi
+            hi -= lead;
+            found = lead < 32u;
+        }
+        if (!found && hi > 0) {
+            u64 lo = 0;                                  // first index in [lo, hi] whose key is not less than target
+            while (lo < hi) {
+                const u64 span = hi - lo;
+                const u64 p = span > 32 ? lo + (span / 33) * (lane + 1) : lo + lane;   // 32 probes, increasing with the lane
+                bool ge = true;
+                if (p < hi) { load_key<W>(a.keys, p, probe); ge = !key_lt<W>(probe, target); }
+                const u32 gem = __ballot_sync(0xffffffffu, ge);    // monotone: 0..0 1..1
+                const u32 f = gem ? (u32)__ffs(gem) - 1u : 32u;    // first probe inside the run (or none)
+                const u64 pf = __shfl_sync(0xffffffffu, p, (int)(f < 32u ? f : 31u));
+                const u64 pb = __shfl_sync(0xffffffffu, p, (int)(f ? f - 1u : 0u));
+                if (f < 32u && pf < hi) hi = pf;
+                if (f > 0u) lo = (pb < hi ? pb : hi - 1) + 1;      // the probe before the first hit is outside the run
+            }
+            hi = lo;
+        }
+        wstart = (u32)(hi - tile_base);                  // modulo 2^32 when the run began before the tile
     }
-    __syncthreads();
-    u64 prev = excl_max ? tile_base + excl_max : s_bcast[0];   // index+1 of the last tail before my first record
+    u32 prev = excl_max ? excl_max : wstart;
 
     // ---- run lengths, solid flags, statistics --------------------------------------------------------------------
     u32 solid = 0, n_solid = 0;
-    u64 len[IPT];
-    u64 sum_mult = 0, csum = 0;
+    u32 len[IPT];
+    u32 sum_mult = 0;   // solid runs ending in one warp are disjoint intervals of one range: their lengths add up to < 2^32
+    u64 csum = 0;
 #pragma unroll
     for (int j = 0; j < IPT; ++j) {
         len[j] = 0;
         if ((tails >> j) & 1u) {
-            const u64 e = idx0 + j + 1;
+            const u32 e = li0 + j + 1;
             len[j] = e - prev;
             prev = e;
-            if (len[j] >= (u64)a.d) { solid |= 1u << j; ++n_solid; sum_mult += len[j]; }
-            if (a.want_csum) csum += len[j] * mix_key<W>(key[j]);
+            if (len[j] >= a.d) { solid |= 1u << j; ++n_solid; sum_mult += len[j]; }
+            if (!WRITE && a.want_csum) csum += (u64)len[j] * mix_key<W>(key[j]);
         }
     }
-    u32 tile_solid;
-    const u32 excl_sum = block_excl_scan<THREADS, false>(n_solid, s_warp, tile_solid);
-    if (warp == 0) {
-        const u64 p = tile_lookback<false>(a.lookback + ntiles, tile, (u64)tile_solid);
-        if (lane == 0) {
-            s_bcast[1] = p;
-            if (tile == ntiles - 1) st->out_cursor[a.range_parity ^ 1] = out_base + p + tile_solid;
-        }
+    const u32 incl = warp_incl_scan_add(n_solid);
+    if (lane == 31) s_wsolid[warp] = incl;
+    if constexpr (!WRITE) {
+        const u32 nt = __reduce_add_sync(0xffffffffu, (u32)__popc(tails));
+        sum_mult = __reduce_add_sync(0xffffffffu, sum_mult);
+        if (a.want_csum) csum = warp_reduce_add64(csum);
+        if (lane == 0) { s_red[0][warp] = nt; s_red[1][warp] = sum_mult; s_red[2][warp] = csum; }
     }
     __syncthreads();
-    u64 pos = out_base + s_bcast[1] + excl_sum;
+    if constexpr (!WRITE) {
+        if (tid == 0) {
+            u32 tile_solid = 0;
 #pragma unroll
-    for (int j = 0; j < IPT; ++j) {
-        if ((solid >> j) & 1u) {
-            if (pos < a.out_cap) {
+            for (int w = 0; w < WARPS; ++w) tile_solid += s_wsolid[w];
+            a.tile_sums[tile] = tile_solid;
+        } else if (warp == 1 && lane < 3) {   // statistics: one atomic per block and counter, spread over 32 slots
+            u64 v = 0;
 #pragma unroll
-                for (int q = 0; q < W; ++q) a.out_keys[pos * W + q] = key[j][q];
-                a.out_mult[pos] = len[j] > 0xffffffffull ? 0xffffffffu : (u32)len[j];
+            for (int w = 0; w < WARPS; ++w) v += s_red[lane][w];
+            if (v) atomicAdd(&a.stat_slots[(tile & (kStatSlots - 1)) * kStatSlotWords + lane], v);
+        }
+    } else {
+        u32 woff = 0;
+#pragma unroll
+        for (int w = 0; w < WARPS; ++w) woff += (w < (int)warp) ? s_wsolid[w] : 0u;
+        // solid edges appended by earlier ranges + solid edges of the tiles before this one + rank in the tile
+        u64 pos = st->out_cursor[a.range_parity] + a.tile_sums[tile] + woff + incl - n_solid;
+#pragma unroll
+        for (int j = 0; j < IPT; ++j) {
+            if ((solid >> j) & 1u) {
+                if (pos < a.out_cap) {
+#pragma unroll
+                    for (int q = 0; q < W; ++q) a.out_keys[pos * W + q] = key[j][q];
+                    a.out_mult[pos] = len[j];   // < 2^32 by the range bound: the saturation of A9 cannot be reached
+                }
+                ++pos;
             }
-            ++pos;
         }
     }
-    // ---- statistics: one atomic per warp ------------------------------------------------------------------------------
-    u64 nt = warp_reduce_add64((u64)__popc(tails));
-    sum_mult = warp_reduce_add64(sum_mult);
-    if (lane == 0) {
-        if (nt) atomicAdd(&st->n_distinct, nt);
-        if (sum_mult) atomicAdd(&st->sum_solid_mult, sum_mult);
+}
+
+// tile_sums -> exclusive prefix, in place; total added to the output cursor of the next range. One block: the array
+// has one word per 32 KiB of records.
+__global__ void __launch_bounds__(1024) scan_tiles_kernel(u64 *tile_sums, u32 ntiles, DevState *st, int range_parity) {
+    __shared__ u64 s_w[32];
+    __shared__ u64 s_carry;
+    const u32 tid = threadIdx.x, lane = tid & 31u, warp = tid >> 5;
+    if (tid == 0) s_carry = 0;
+    __syncthreads();
+    for (u32 base = 0; base < ntiles; base += 1024) {
+        const u32 i = base + tid;
+        const u64 v = i < ntiles ? tile_sums[i] : 0ull;
+        u64 incl = v;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            const u64 t = __shfl_up_sync(0xffffffffu, incl, o);
+            if (lane >= (u32)o) incl += t;
+        }
+        if (lane == 31) s_w[warp] = incl;
+        __syncthreads();
+        u64 off = s_carry;
+        for (u32 w = 0; w < warp; ++w) off += s_w[w];
+        if (i < ntiles) tile_sums[i] = off + incl - v;
+        __syncthreads();
+        if (tid == 1023) s_carry = off + incl;
+        __syncthreads();
     }
-    if (a.want_csum) {
-        csum = warp_reduce_add64(csum);
-        if (lane == 0 && csum) atomicAdd(&st->csum_distinct, csum);
-    }
+    if (tid == 0) st->out_cursor[range_parity ^ 1] = st->out_cursor[range_parity] + s_carry;
 }
 
 template <int W> static constexpr u64 count_tile() { return (u64)CountCfg<W>::THREADS * CountCfg<W>::IPT; }
@@ -214,7 +323,9 @@ static int launch_count_w(const CountArgs &a, DevState *st, cudaStream_t s) {
     const u64 tiles = (a.n + count_tile<W>() - 1) / count_tile<W>();
     if (tiles == 0) return 0;
     if (tiles > 0x7fffffffull) return (int)cudaErrorInvalidValue;
-    count_filter_kernel<W><<<(unsigned)tiles, CountCfg<W>::THREADS, 0, s>>>(a, st);
+    count_tiles_kernel<W, false><<<(unsigned)tiles, CountCfg<W>::THREADS, 0, s>>>(a, st);
+    scan_tiles_kernel<<<1, 1024, 0, s>>>(a.tile_sums, (u32)tiles, st, a.range_parity);
+    count_tiles_kernel<W, true><<<(unsigned)tiles, CountCfg<W>::THREADS, 0, s>>>(a, st);
     return (int)cudaGetLastError();
 }
 
