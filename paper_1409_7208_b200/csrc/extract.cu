@@ -92,6 +92,9 @@ __global__ void __launch_bounds__(256) extract_kernel(ExtractArgs a, DevState *s
         for (int i = threadIdx.x; i < np * kRadix; i += blockDim.x) s_hist[i] = 0;
         __syncthreads();
     }
+    // s_hist row of byte 0 of the last key word if it were a pass (rows of the padding bytes are never touched)
+    const u32 b0 = a.passes.n ? (u32)a.passes.p[0].shift >> 3 : 0u;
+    u32 *h_last = s_hist - b0 * kRadix;
     const u64 ngroups = a.n_slots / 32;
     const u32 lane = lane_id();
     const u32 lt = lanemask_lt();
@@ -142,12 +145,19 @@ __global__ void __launch_bounds__(256) extract_kernel(ExtractArgs a, DevState *s
                 base += __popc(mr);
             }
             if (do_hist) {
-#pragma unroll 1
-                for (int p = 0; p < np; ++p) {
-                    const PassDesc pd = a.passes.p[p];
-                    const u32 m = (1u << pd.bits) - 1u;
-                    if (kf) atomicAdd(&s_hist[p * kRadix + ((u32)(f[pd.word] >> pd.shift) & m)], 1u);
-                    if (kr) atomicAdd(&s_hist[p * kRadix + ((u32)(r[pd.word] >> pd.shift) & m)], 1u);
+                // every pass is one whole byte of a key word (api.cu make_passes): byte b of word q is pass
+                // (b - b0) for the last word and (8 - b0) + 8 (W-2-q) + b for the others, b0 = first significant byte
+#pragma unroll
+                for (int q = W - 1; q >= 0; --q) {
+                    u32 *hq = (q == W - 1) ? h_last : h_last + ((8 - b0) + 8 * (W - 2 - q) + b0) * kRadix;
+                    const u32 flo = (u32)f[q], fhi = (u32)(f[q] >> 32), rlo = (u32)r[q], rhi = (u32)(r[q] >> 32);
+#pragma unroll
+                    for (int b = 0; b < 8; ++b) {
+                        if (q == W - 1 && b < (int)b0) continue;     // padding bytes of the last word: no pass
+                        u32 *h = hq + b * kRadix;
+                        if (kf) atomicAdd(&h[__byte_perm(b < 4 ? flo : fhi, 0u, 0x4440u | (b & 3))], 1u);
+                        if (kr) atomicAdd(&h[__byte_perm(b < 4 ? rlo : rhi, 0u, 0x4440u | (b & 3))], 1u);
+                    }
                 }
             }
             if (a.bucket_hist && ((valid >> i) & 1)) {
