@@ -123,6 +123,9 @@ typedef struct {
  * 64 Ki-record range of 4-word keys — sdbg_ctx_create refuses less with SDBG_E_WORKSPACE. */
 uint32_t sdbg_key_words(uint32_t k);
 uint64_t sdbg_full_workspace(uint64_t n_bases, uint32_t k);
+/* The same for a known number of records N = 2 * sum_r max(0, L_r - k) (sdbg_full_workspace assumes the bound
+ * N <= 2 * n_bases, which is loose for long keys: 150-base reads give 51 windows at k = 99). 0 if k is out of range. */
+uint64_t sdbg_workspace_for_records(uint64_t n_records, uint32_t k);
 uint64_t sdbg_min_workspace(void);
 
 /* a2 extract + a3 sort + a4 count/filter (+ a6 block-wise planner).

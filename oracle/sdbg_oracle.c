@@ -25,8 +25,12 @@
  *     words per key; W byte = 1 + code(e[k]), + 4 if minus; last packed LSB-first into u64 words.
  *
  * Optional restriction (large configs, SURVEY.md §8(c) "Large configs"): keep in step 1 only records whose
- * key string (e[k-1],...,e[0],e[k]) begins with a given 8 symbols (one l=8 partition). Requires
- * k >= 9, for which no `last`/minus dependency crosses a partition.
+ * key string (e[k-1],...,e[0],e[k]) begins with one of a given set of 8-symbol strings (l=8 partitions,
+ * PAPER.md:33). Requires k >= 9, for which no `last`/minus dependency crosses a partition, so the result is the
+ * concatenation of those partitions' slices of the full result. For the same purpose step 1 can also be fed
+ * records that were extracted earlier (orc_add_edges): several oracle instances may scan disjoint parts of the
+ * reads (the kept raw records of each are read back with orc_raw) and one instance then runs steps 2-5 on
+ * the union.
  *
  * Pins (tests/test_oracle_pins.py): hand-worked example T0 (tests/golden/t0_handworked.txt), complete
  * de Bruijn closed form, independent Python brute force, count/closure invariants, numpy sort/unique.
@@ -39,8 +43,8 @@
 
 typedef struct orc {
     uint32_t k, d;
-    int has_prefix;
-    char prefix[8];
+    uint32_t n_prefix;
+    char *prefix;                     /* n_prefix * 8 chars */
     /* step 1 */
     char *E; uint64_t nE, capE;       /* records, (k+1) chars each */
     uint64_t n_seen;                  /* records before the optional prefix restriction */
@@ -53,18 +57,24 @@ typedef struct orc {
 
 enum { ORC_OK = 0, ORC_E_BADBASE = -2, ORC_E_NOMEM = -7, ORC_E_INVAL = -1 };
 
-orc *orc_new(uint32_t k, uint32_t d, const char *prefix8 /* NULL or 8 chars */) {
+orc *orc_new(uint32_t k, uint32_t d, const char *prefixes /* NULL or n_prefix * 8 chars */, uint32_t n_prefix) {
     if (k < 1 || d < 1) return NULL;
-    if (prefix8 && k < 9) return NULL;
+    if (prefixes && n_prefix && k < 9) return NULL;
     orc *o = (orc *)calloc(1, sizeof(orc));
     if (!o) return NULL;
     o->k = k; o->d = d;
-    if (prefix8) { o->has_prefix = 1; memcpy(o->prefix, prefix8, 8); }
+    if (prefixes && n_prefix) {
+        o->prefix = (char *)malloc((size_t)n_prefix * 8);
+        if (!o->prefix) { free(o); return NULL; }
+        memcpy(o->prefix, prefixes, (size_t)n_prefix * 8);
+        o->n_prefix = n_prefix;
+    }
     return o;
 }
 
 void orc_free(orc *o) {
     if (!o) return;
+    free(o->prefix);
     free(o->E); free(o->D); free(o->Dcnt); free(o->S); free(o->mult); free(o->W); free(o->last); free(o->minus);
     free(o);
 }
@@ -74,8 +84,14 @@ static char comp(char c) { return c == 'A' ? 'T' : c == 'C' ? 'G' : c == 'G' ? '
 static int push(orc *o, const char *e) {
     const uint32_t k = o->k;
     o->n_seen++;
-    if (o->has_prefix)               /* key string symbol t is e[k-1-t] for t < k */
-        for (uint32_t t = 0; t < 8; ++t) if (e[k - 1 - t] != o->prefix[t]) return ORC_OK;
+    if (o->n_prefix) {               /* key string symbol t is e[k-1-t] for t < k */
+        int keep = 0;
+        for (uint32_t p = 0; p < o->n_prefix && !keep; ++p) {
+            keep = 1;
+            for (uint32_t t = 0; t < 8; ++t) if (e[k - 1 - t] != o->prefix[p * 8 + t]) { keep = 0; break; }
+        }
+        if (!keep) return ORC_OK;
+    }
     if (o->nE == o->capE) {
         uint64_t nc = o->capE ? o->capE * 2 : 1024;
         char *p = (char *)realloc(o->E, nc * (k + 1));
@@ -115,6 +131,15 @@ int orc_add_reads(orc *o, const char *bases, const uint64_t *offsets, uint64_t n
     free(e); free(rc); free(rd);
     return st;
 }
+
+/* Step 1 fed with n records extracted earlier ((k+1) chars each, upper case ACGT): see the header. */
+int orc_add_edges(orc *o, const char *edges, uint64_t n) {
+    int st = ORC_OK;
+    for (uint64_t i = 0; i < n && st == ORC_OK; ++i) st = push(o, edges + i * (o->k + 1));
+    return st;
+}
+/* The records kept by step 1 so far, in the order they were met (before orc_finish sorts them in place). */
+const char *orc_raw(const orc *o) { return o->E; }
 
 /* Step 2 comparator. */
 static int cmp_edges(const void *pa, const void *pb, void *ctx) {

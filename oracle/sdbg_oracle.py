@@ -26,7 +26,9 @@ def _load():
     if _lib is None:
         L = ctypes.CDLL(build_oracle_lib())
         vp, u64, u32 = ctypes.c_void_p, ctypes.c_uint64, ctypes.c_uint32
-        L.orc_new.argtypes = [u32, u32, ctypes.c_char_p]; L.orc_new.restype = vp
+        L.orc_new.argtypes = [u32, u32, ctypes.c_char_p, u32]; L.orc_new.restype = vp
+        L.orc_add_edges.argtypes = [vp, vp, u64]; L.orc_add_edges.restype = ctypes.c_int
+        L.orc_raw.argtypes = [vp]; L.orc_raw.restype = vp
         L.orc_free.argtypes = [vp]; L.orc_free.restype = None
         L.orc_add_reads.argtypes = [vp, vp, vp, u64]; L.orc_add_reads.restype = ctypes.c_int
         L.orc_finish.argtypes = [vp]; L.orc_finish.restype = ctypes.c_int
@@ -81,12 +83,15 @@ class OracleResult:
 
 
 class Oracle:
-    """Steps 1-6 of sdbg_oracle.c. ``prefix``: optional 8-letter key-string prefix (one l=8 partition)."""
+    """Steps 1-6 of sdbg_oracle.c. ``prefix``: optional 8-letter key-string prefix (one l=8 partition) or a list
+    of them."""
 
-    def __init__(self, k: int, d: int = 2, prefix: str | None = None):
+    def __init__(self, k: int, d: int = 2, prefix=None):
         L = _load()
         self.k, self.d = int(k), int(d)
-        self._h = L.orc_new(self.k, self.d, prefix.encode() if prefix else None)
+        plist = [prefix] if isinstance(prefix, str) else list(prefix or [])
+        assert all(len(p) == 8 for p in plist)
+        self._h = L.orc_new(self.k, self.d, "".join(plist).encode() if plist else None, len(plist))
         if not self._h:
             raise ValueError("oracle: invalid k/d/prefix")
 
@@ -99,6 +104,18 @@ class Oracle:
             raise ValueError("oracle: non-ACGT base")
         if rc != 0:
             raise MemoryError(f"oracle: error {rc}")
+
+    def add_edges(self, edges: np.ndarray) -> None:
+        """edges: (n, k+1) uint8 letters extracted earlier (see sdbg_oracle.c header)."""
+        e = np.ascontiguousarray(edges, dtype=np.uint8).reshape(-1, self.k + 1)
+        rc = _load().orc_add_edges(self._h, e.ctypes.data if e.size else None, len(e))
+        if rc != 0:
+            raise MemoryError(f"oracle: error {rc}")
+
+    def raw_edges(self) -> np.ndarray:
+        """The records step 1 has kept so far, (n, k+1) uint8 letters (call before finish)."""
+        L = _load()
+        return _copy(L.orc_raw(self._h), L.orc_n_raw(self._h) * (self.k + 1), np.uint8).reshape(-1, self.k + 1)
 
     def finish(self, want_distinct: bool = True) -> OracleResult:
         L = _load()
@@ -146,7 +163,7 @@ def reads_to_arrays(reads):
     return np.frombuffer("".join(reads).encode(), dtype=np.uint8), offs
 
 
-def run_oracle(reads, k: int, d: int = 2, prefix: str | None = None) -> OracleResult:
+def run_oracle(reads, k: int, d: int = 2, prefix=None) -> OracleResult:
     """reads: list of str, or a (bases, offsets) pair."""
     o = Oracle(k, d, prefix)
     try:

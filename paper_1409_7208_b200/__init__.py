@@ -4,6 +4,6 @@ There is no CPU fallback: without the built library or without a CUDA device the
 from .binding import (  # noqa: F401
     SdbgError, Context, Reads, Edges, Graph, Stats, Timing, lib, lib_path,
     sdbg_pack_reads, sdbg_count_edges, sdbg_build, sdbg_plan_ranges,
-    sdbg_key_words, sdbg_read_slots, sdbg_full_workspace, sdbg_min_workspace, sdbg_strerror,
+    sdbg_key_words, sdbg_read_slots, sdbg_full_workspace, sdbg_workspace_for_records, sdbg_min_workspace, sdbg_strerror,
     SDBG_SORTED, STATUS,
 )

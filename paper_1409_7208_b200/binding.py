@@ -76,6 +76,7 @@ def lib():
         L.sdbg_key_words.argtypes = [u32]; L.sdbg_key_words.restype = u32
         L.sdbg_full_workspace.argtypes = [u64, u32]; L.sdbg_full_workspace.restype = u64
         L.sdbg_min_workspace.argtypes = []; L.sdbg_min_workspace.restype = u64
+        L.sdbg_workspace_for_records.argtypes = [u64, u32]; L.sdbg_workspace_for_records.restype = u64
         L.sdbg_count_edges.argtypes = [vp, C.POINTER(_Reads), u64, u32, u32, C.POINTER(_Edges), C.POINTER(_Stats)]
         L.sdbg_count_edges.restype = i32
         L.sdbg_plan_ranges.argtypes = [vp, u64, vp, u64]; L.sdbg_plan_ranges.restype = C.c_int64
@@ -102,6 +103,10 @@ def sdbg_read_slots(n_bases: int, n_calls: int = 1) -> int:
 
 def sdbg_full_workspace(n_bases: int, k: int) -> int:
     return lib().sdbg_full_workspace(n_bases, k)
+
+
+def sdbg_workspace_for_records(n_records: int, k: int) -> int:
+    return lib().sdbg_workspace_for_records(n_records, k)
 
 
 def sdbg_min_workspace() -> int:

@@ -200,6 +200,12 @@ uint64_t sdbg_full_workspace(uint64_t n_bases, uint32_t k) {
     return std::max<u64>(need, sdbg_min_workspace());
 }
 
+uint64_t sdbg_workspace_for_records(uint64_t n_records, uint32_t k) {
+    if (k < 1 || k > SDBG_MAX_K) return 0;
+    const u64 need = kFixedBytes + range_need(n_records, sdbg_key_words(k)) + 4096;
+    return std::max<u64>(need, sdbg_min_workspace());
+}
+
 int64_t sdbg_plan_ranges(const uint64_t *hist, uint64_t capacity, uint64_t *ranges, uint64_t max_ranges) {
     if (!hist || !ranges) return SDBG_E_INVAL;
     u64 nr = 0, lo = 0, sum = 0;

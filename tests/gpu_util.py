@@ -82,3 +82,171 @@ def assert_matches_oracle(res, orc, check_stats=True):
         s = res.stats
         assert s.n_raw == orc.n_seen and s.n_distinct == orc.n_distinct and s.n_solid == orc.n_solid
         assert s.sum_solid_mult == orc.sum_solid_mult
+
+
+# ---- full-size configs: oracle-verified sampled l=8 partitions + global invariants (BASELINE.json north_star) ----------
+
+SYM = "ACGT"
+
+
+def bucket_prefix(b: int) -> str:
+    """l=8 partition number (top 16 key bits) -> its 8 key-string symbols."""
+    return "".join(SYM[(b >> (14 - 2 * t)) & 3] for t in range(8))
+
+
+_PAR = {}
+
+
+def _scan_part(args):
+    from oracle import Oracle
+    a, b = args
+    bases, offs, k, prefixes = _PAR["bases"], _PAR["offs"], _PAR["k"], _PAR["prefixes"]
+    o = Oracle(k, 1, prefixes)
+    o.add_reads(bases[int(offs[a]):int(offs[b])], offs[a:b + 1] - offs[a])
+    e = o.raw_edges()
+    o.close()
+    return e
+
+
+def oracle_partitions(bases, offs, k, d, buckets, nproc=None):
+    """The oracle restricted to the given l=8 partitions. Step 1 (the scan of the reads) runs in `nproc` forked
+    processes over disjoint parts of the reads; steps 2-5 run in one oracle instance on the union of the kept records
+    (oracle/sdbg_oracle.c header). Returns the OracleResult of the union (partitions concatenated in sorted order)."""
+    import multiprocessing as mp
+    import os
+    from oracle import Oracle
+    prefixes = [bucket_prefix(b) for b in sorted(buckets)]
+    n = len(offs) - 1
+    nproc = nproc or min(os.cpu_count() or 1, 16)
+    parts = max(1, min(n, nproc * 4))
+    cuts = [n * i // parts for i in range(parts + 1)]
+    _PAR.update(bases=bases, offs=offs, k=k, prefixes=prefixes)
+    parent = Oracle(k, d, prefixes)
+    if nproc == 1:
+        for ab in zip(cuts, cuts[1:]):
+            parent.add_edges(_scan_part(ab))
+    else:
+        with mp.get_context("fork").Pool(nproc) as pool:
+            for e in pool.imap(_scan_part, list(zip(cuts, cuts[1:]))):
+                parent.add_edges(e)
+    _PAR.clear()
+    res = parent.finish(want_distinct=False)
+    parent.close()
+    return res
+
+
+def run_gpu_workload(w, workspace_bytes=None, chunk_bases=1 << 30, keep_ascii=False):
+    """Config-sized run through the C ABI: reads generated in HBM chunk by chunk and packed by appending calls,
+    sdbg_count_edges (twice when the number of solid edges is not known: first with capacity 0), sdbg_build."""
+    import torch
+    from workloads import ReadGenerator
+    gen = ReadGenerator(w)
+    reads_per_chunk = max(1, chunk_bases // w.read_len)
+    n_calls = (w.n_reads + reads_per_chunk - 1) // reads_per_chunk
+    ws = workspace_bytes if workspace_bytes is not None else sd.sdbg_workspace_for_records(w.n_raw_edges, w.k)
+    ctx = sd.Context(ws)
+    rd = sd.Reads(w.n_bases, n_calls)
+    buf = torch.empty(min(w.n_reads, reads_per_chunk) * w.read_len, dtype=torch.uint8, device="cuda")
+    host = np.empty(w.n_bases, dtype=np.uint8) if keep_ascii else None
+    for c in range(n_calls):
+        r0, r1 = c * reads_per_chunk, min(w.n_reads, (c + 1) * reads_per_chunk)
+        b, o = gen.device(r0, r1, out=buf)
+        sd.sdbg_pack_reads(ctx, b, o, r1 - r0, rd)
+        if keep_ascii:
+            host[r0 * w.read_len:r1 * w.read_len] = b.cpu().numpy()
+    del buf
+    torch.cuda.empty_cache()
+    st = sd.Stats(want_checksums=True, want_bucket_hist=True)
+    probe = sd.Edges(0, w.k)
+    try:
+        sd.sdbg_count_edges(ctx, rd, rd.n_reads, w.k, w.d, probe, st)
+    except sd.SdbgError as e:
+        assert e.name == "SDBG_E_CAPACITY", e
+    S = probe.n
+    ed = sd.Edges(S, w.k)
+    st = sd.Stats(want_checksums=True, want_bucket_hist=True)
+    sd.sdbg_count_edges(ctx, rd, rd.n_reads, w.k, w.d, ed, st)
+    assert ed.n == S
+    g = sd.Graph(S)
+    sd.sdbg_build(ctx, ed, sd.SDBG_SORTED, g)
+    torch.cuda.synchronize()
+    res = GpuResult()
+    res.ctx, res.reads, res.edges, res.graph, res.stats, res.n, res.host_ascii = ctx, rd, ed, g, st, S, host
+    return res
+
+
+def _u64_sorted_view(t):
+    """int64 tensor holding u64 bit patterns -> int64 tensor with the same order as the unsigned values."""
+    return t ^ (-(2 ** 63))
+
+
+def check_global_invariants(res, w):
+    """Properties that hold at any size, evaluated on the device."""
+    import torch
+    st, ed, g, S, W = res.stats, res.edges, res.graph, res.n, res.edges.w
+    assert st.n_raw == w.n_raw_edges                                   # P3: N = 2 sum max(0, L - k)
+    assert st.csum_raw == st.csum_distinct                             # P4: the sort/count lost or duplicated nothing
+    assert st.n_solid == S and S <= st.n_distinct <= st.n_raw
+    mult = ed.mult[:S]
+    assert int(mult.to(torch.int64).sum()) == st.sum_solid_mult and int(mult.min()) >= w.d
+    assert torch.equal(g.mult[:S], mult)
+    keys = ed.keys[:S * W].view(S, W)
+    # P5: strictly increasing multi-word keys; and nodes (top 2k bits) for P6
+    gt = torch.zeros(S - 1, dtype=torch.bool, device="cuda")
+    eq = torch.ones(S - 1, dtype=torch.bool, device="cuda")
+    node_eq = torch.ones(S - 1, dtype=torch.bool, device="cuda")
+    for q in range(W):
+        col = _u64_sorted_view(keys[:, q].contiguous())
+        a, b = col[:-1], col[1:]
+        gt |= eq & (b > a)
+        eq &= (b == a)
+        nb = min(64, max(0, 2 * w.k - 64 * q))                        # bits of this word that belong to the node
+        if nb == 64:
+            node_eq &= (b == a)
+        elif nb > 0:
+            node_eq &= ((keys[1:, q] ^ keys[:-1, q]) >> (64 - nb)) == 0   # arithmetic shift: zero iff the top nb bits agree
+        del col, a, b
+    assert bool(gt.all()), "keys not strictly increasing"
+    n_nodes = int((~node_eq).sum()) + 1
+    lb = g.last_bits[:(S + 63) // 64]
+    bits = ((lb.unsqueeze(1) >> torch.arange(64, device="cuda")) & 1).reshape(-1)[:S]
+    assert int(bits.sum()) == n_nodes                                  # P6: one `last` per distinct node
+    assert torch.equal(bits[:-1].bool(), ~node_eq) and int(bits[-1]) == 1
+    Wb = g.W[:S]
+    assert int(Wb.min()) >= 1 and int(Wb.max()) <= 8
+    sym = (keys[:, W - 1] >> (64 * W - 2 * (w.k + 1))) & 3            # outgoing base = last symbol of the key
+    assert torch.equal(((Wb - 1) & 3).to(torch.int64), sym)
+    return n_nodes
+
+
+def compare_partitions(res, w, orc, buckets):
+    """Bit-exact comparison of the GPU output slices of the given l=8 partitions with the oracle's result for them."""
+    import torch
+    ed, g, S, W = res.edges, res.graph, res.n, res.edges.w
+    word0 = _u64_sorted_view(ed.keys[:S * W].view(S, W)[:, 0].contiguous())
+    okeys = orc.keys
+    ob = (okeys[:, 0] >> np.uint64(48)).astype(np.int64) if len(okeys) else np.zeros(0, np.int64)
+    total = 0
+    for b in sorted(buckets):
+        lo_v = torch.tensor([(b << 48) - 2 ** 63], dtype=torch.int64, device="cuda")
+        lo = int(torch.searchsorted(word0, lo_v)[0])
+        hi = S if b == 65535 else int(torch.searchsorted(word0, torch.tensor([((b + 1) << 48) - 2 ** 63], dtype=torch.int64, device="cuda"))[0])
+        sel = np.nonzero(ob == b)[0]
+        assert hi - lo == len(sel), (b, hi - lo, len(sel))
+        total += len(sel)
+        if hi == lo:
+            continue
+        o0, o1 = int(sel[0]), int(sel[-1]) + 1
+        assert o1 - o0 == len(sel)
+        gk = ed.keys[lo * W:hi * W].cpu().numpy().view(np.uint64).reshape(-1, W)
+        assert np.array_equal(gk, okeys[o0:o1]), f"partition {b}: keys differ"
+        assert np.array_equal(ed.mult[lo:hi].cpu().numpy().view(np.uint32), orc.mult[o0:o1]), f"partition {b}: mult differs"
+        assert np.array_equal(g.W[lo:hi].cpu().numpy(), orc.Wbyte[o0:o1]), f"partition {b}: W differs"
+        words = g.last_bits[lo // 64:(hi + 63) // 64].cpu().numpy().view(np.uint64)
+        bits = np.unpackbits(words.view(np.uint8), bitorder="little")[lo % 64:lo % 64 + (hi - lo)]
+        want = orc.last[o0:o1].copy()
+        if hi < S:
+            want[-1] = 1      # the partition's last edge: its successor lies in another partition = another node (k >= 9)
+        assert np.array_equal(bits, want), f"partition {b}: last differs"
+    assert total == orc.n_solid
+    return total

@@ -34,7 +34,7 @@ def test_library_exports_every_declared_symbol():
 
 def test_python_binding_has_the_same_names():
     for n in ("sdbg_pack_reads", "sdbg_count_edges", "sdbg_build", "sdbg_plan_ranges", "sdbg_key_words",
-              "sdbg_read_slots", "sdbg_full_workspace", "sdbg_min_workspace", "sdbg_strerror"):
+              "sdbg_read_slots", "sdbg_full_workspace", "sdbg_workspace_for_records", "sdbg_min_workspace", "sdbg_strerror"):
         assert callable(getattr(sd, n))
 
 
@@ -46,6 +46,7 @@ def test_host_helpers():
     w31, w99 = sd.sdbg_full_workspace(10 ** 6, 31), sd.sdbg_full_workspace(10 ** 6, 99)
     assert w31 >= 2 * 8 * 2 * 10 ** 6 and w99 >= 4 * (w31 - sd.sdbg_min_workspace())
     assert sd.sdbg_full_workspace(10 ** 6, 0) == 0 and sd.sdbg_full_workspace(10 ** 6, 128) == 0
+    assert sd.sdbg_workspace_for_records(2 * 10 ** 6, 31) == w31 and sd.sdbg_workspace_for_records(10 ** 6, 31) < w31
 
 
 def test_plan_ranges_greedy_consecutive():

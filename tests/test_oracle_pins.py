@@ -212,3 +212,33 @@ def test_partition_restriction_matches_slice_of_full_run():
         assert list(part.Wbyte) == [int(full.Wbyte[i]) for i in idx]
         assert list(part.last) == [int(full.last[i]) for i in idx]
         assert part.n_seen == full.n_raw
+
+
+def test_several_partitions_and_split_scans_match_the_full_run():
+    """A set of l=8 partitions gives the concatenation of their slices, and scanning the reads in parts (the kept raw
+    records of each part fed to one instance through add_edges) gives the same as one scan (sdbg_oracle.c header)."""
+    from oracle import Oracle
+    bases, offs = _small_workload()
+    k = 21
+    full = run_oracle((bases, offs), k, 2)
+    S = full.solid_strings()
+    prefixes = sorted({e[:k][::-1][:8] for e in S})
+    pick = [prefixes[0], prefixes[3], prefixes[len(prefixes) // 2], prefixes[-1]]
+    idx = [i for i, e in enumerate(S) if e[:k][::-1][:8] in pick]
+    multi = run_oracle((bases, offs), k, 2, prefix=pick)
+    assert multi.solid_strings() == [S[i] for i in idx]
+    assert list(multi.mult) == [int(full.mult[i]) for i in idx]
+    assert list(multi.Wbyte) == [int(full.Wbyte[i]) for i in idx]
+    assert list(multi.last) == [int(full.last[i]) for i in idx]
+    # the same from three partial scans
+    n = len(offs) - 1
+    cuts = [0, n // 3, 2 * n // 3, n]
+    parent = Oracle(k, 2, pick)
+    for a, b in zip(cuts, cuts[1:]):
+        child = Oracle(k, 1, pick)
+        child.add_reads(bases[int(offs[a]):int(offs[b])], offs[a:b + 1] - offs[a])
+        parent.add_edges(child.raw_edges())
+        child.close()
+    res = parent.finish()
+    assert res.solid_strings() == multi.solid_strings() and np.array_equal(res.mult, multi.mult)
+    assert np.array_equal(res.keys, multi.keys) and np.array_equal(res.last_bits, multi.last_bits)
