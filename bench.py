@@ -40,14 +40,19 @@ def _peaks():
 
 
 def _traffic(workload_name):
-    """DRAM bytes per launch of the dominant kernel from the committed ncu --set full capture, if any."""
-    p = os.path.join(ROOT, "profiles", "traffic.json")
-    if os.path.exists(p):
+    """DRAM bytes (read + write) per launch of the dominant kernel, from the committed ncu --set full capture of this
+    workload (profiles/*_traffic.csv, newest round last), or None."""
+    import csv
+    import glob
+    val = None
+    for p in sorted(glob.glob(os.path.join(ROOT, "profiles", "*_traffic.csv"))):
         try:
-            return json.load(open(p)).get(workload_name)
+            for row in csv.DictReader(open(p)):
+                if row.get("workload") == workload_name:
+                    val = int(row["dram_bytes_per_launch"])
         except Exception:
-            return None
-    return None
+            pass
+    return val
 
 
 class ClockSampler(threading.Thread):
@@ -142,7 +147,7 @@ def run_gpu(args, w):
     N = wl.n_raw_edges
     K = 8 * wl.words_per_key
 
-    ctx = sd.Context(sd.sdbg_full_workspace(n_bases, wl.k))
+    ctx = sd.Context(sd.sdbg_workspace_for_records(N, wl.k))
     reads = sd.Reads(n_bases)
     edges = sd.Edges(N // wl.d, wl.k)
     graph = sd.Graph(N // wl.d)
