@@ -282,18 +282,21 @@ __global__ void __launch_bounds__(CountCfg<W>::THREADS, SDBG_CNT_MINB) count_til
     }
 }
 
-// tile_sums -> exclusive prefix, in place; total added to the output cursor of the next range. One block: the array
-// has one word per 32 KiB of records.
+// tile_sums -> exclusive prefix, in place; total added to the output cursor of the next range. One block (the array
+// has one word per 16 KiB of records), 16 words per thread and round.
 __global__ void __launch_bounds__(1024) scan_tiles_kernel(u64 *tile_sums, u32 ntiles, DevState *st, int range_parity) {
+    constexpr u32 PER = 16, ROUND = 1024 * PER;
     __shared__ u64 s_w[32];
     __shared__ u64 s_carry;
     const u32 tid = threadIdx.x, lane = tid & 31u, warp = tid >> 5;
     if (tid == 0) s_carry = 0;
     __syncthreads();
-    for (u32 base = 0; base < ntiles; base += 1024) {
-        const u32 i = base + tid;
-        const u64 v = i < ntiles ? tile_sums[i] : 0ull;
-        u64 incl = v;
+    for (u32 base = 0; base < ntiles; base += ROUND) {
+        const u32 i0 = base + tid * PER;
+        u64 v[PER], sum = 0;
+#pragma unroll
+        for (u32 j = 0; j < PER; ++j) { v[j] = (i0 + j < ntiles) ? tile_sums[i0 + j] : 0ull; sum += v[j]; }
+        u64 incl = sum;
 #pragma unroll
         for (int o = 1; o < 32; o <<= 1) {
             const u64 t = __shfl_up_sync(0xffffffffu, incl, o);
@@ -301,11 +304,12 @@ __global__ void __launch_bounds__(1024) scan_tiles_kernel(u64 *tile_sums, u32 nt
         }
         if (lane == 31) s_w[warp] = incl;
         __syncthreads();
-        u64 off = s_carry;
-        for (u32 w = 0; w < warp; ++w) off += s_w[w];
-        if (i < ntiles) tile_sums[i] = off + incl - v;
+        u64 run = s_carry + incl - sum;
+        for (u32 w = 0; w < warp; ++w) run += s_w[w];
+#pragma unroll
+        for (u32 j = 0; j < PER; ++j) { if (i0 + j < ntiles) tile_sums[i0 + j] = run; run += v[j]; }
         __syncthreads();
-        if (tid == 1023) s_carry = off + incl;
+        if (tid == 1023) s_carry = run;
         __syncthreads();
     }
     if (tid == 0) st->out_cursor[range_parity ^ 1] = st->out_cursor[range_parity] + s_carry;

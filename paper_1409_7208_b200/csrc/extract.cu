@@ -53,6 +53,28 @@ struct KeyMaker {
         for (int j = 0; j < W; ++j) out[j] = (V[j] << 2) | (j + 1 < W ? (V[j + 1] >> 62) : 0ull);
         out[W - 1] |= top << (62 - 2 * (k & 31));
     }
+    // The same for window i = 16 HALF + ii with 32-bit funnel shifts: the word pairs are fixed by HALF, only the
+    // shift amount (< 32) is a run-time value, so a 64-bit window costs two SHF instead of a dozen instructions.
+    template <int HALF>
+    __device__ __forceinline__ void keys_h(u32 ii, u64 (&fwd)[W], u64 (&rc)[W]) const {
+        u64 win[W], Y[W];
+        const u32 s = 2 * ii, t = 30 - 2 * ii;    // bit offsets 32 HALF + s (forward) and 32 (1 - HALF) + t (reversed)
+#pragma unroll
+        for (int j = 0; j < W; ++j) {
+            const u32 wh = __funnelshift_l(w32(B, 2 * j + HALF + 1), w32(B, 2 * j + HALF), s);
+            const u32 wl = __funnelshift_l(w32(B, 2 * j + HALF + 2), w32(B, 2 * j + HALF + 1), s);
+            const u32 yh = __funnelshift_l(w32(R, 2 * j + 2 - HALF), w32(R, 2 * j + 1 - HALF), t);
+            const u32 yl = __funnelshift_l(w32(R, 2 * j + 3 - HALF), w32(R, 2 * j + 2 - HALF), t);
+            win[j] = ~(((u64)wh << 32) | wl);
+            Y[j] = ((u64)yh << 32) | yl;
+        }
+        win[W - 1] &= lastmask;
+        Y[W - 1] &= lastmask;
+        rot(Y, fwd);
+        rot(win, rc);
+    }
+    // 32-bit word m of a stream of u64 words, most significant first
+    static __device__ __forceinline__ u32 w32(const u64 (&S)[W + 1], int m) { return (m & 1) ? (u32)S[m >> 1] : (u32)(S[m >> 1] >> 32); }
     __device__ __forceinline__ void keys(u32 i, u64 (&fwd)[W], u64 (&rc)[W]) const {
         u64 win[W], Y[W];
         const u32 s = 2 * i, t = 2 * (31 - i);
@@ -132,11 +154,8 @@ __global__ void __launch_bounds__(256) extract_kernel(ExtractArgs a, DevState *s
             if (base + total > a.out_cap) continue;   // cannot happen when the caller sized out_cap from the histogram
         }
         const u32 any_mask = __reduce_or_sync(0xffffffffu, valid);
-        for (u32 i = 0; i < 32; ++i) {
-            if (!((any_mask >> i) & 1)) continue;     // warp-uniform
+        auto emit_window = [&](u32 i, const u64 (&f)[W], const u64 (&r)[W]) {
             const bool kf = (vf >> i) & 1, kr = (vr >> i) & 1;
-            u64 f[W], r[W];
-            km.keys(i, f, r);
             if (a.keys_out) {
                 const u32 mf = __ballot_sync(0xffffffffu, kf), mr = __ballot_sync(0xffffffffu, kr);
                 if (kf) store_key<W>(a.keys_out, base + __popc(mf & lt), f);
@@ -147,18 +166,20 @@ __global__ void __launch_bounds__(256) extract_kernel(ExtractArgs a, DevState *s
             if (do_hist) {
                 // every pass is one whole byte of a key word (api.cu make_passes): byte b of word q is pass
                 // (b - b0) for the last word and (8 - b0) + 8 (W-2-q) + b for the others, b0 = first significant byte
+                auto add_key = [&](const u64 (&key)[W]) {
 #pragma unroll
-                for (int q = W - 1; q >= 0; --q) {
-                    u32 *hq = (q == W - 1) ? h_last : h_last + ((8 - b0) + 8 * (W - 2 - q) + b0) * kRadix;
-                    const u32 flo = (u32)f[q], fhi = (u32)(f[q] >> 32), rlo = (u32)r[q], rhi = (u32)(r[q] >> 32);
+                    for (int q = W - 1; q >= 0; --q) {
+                        u32 *hq = (q == W - 1) ? h_last : h_last + ((8 - b0) + 8 * (W - 2 - q) + b0) * kRadix;
+                        const u32 lo = (u32)key[q], hi = (u32)(key[q] >> 32);
 #pragma unroll
-                    for (int b = 0; b < 8; ++b) {
-                        if (q == W - 1 && b < (int)b0) continue;     // padding bytes of the last word: no pass
-                        u32 *h = hq + b * kRadix;
-                        if (kf) atomicAdd(&h[__byte_perm(b < 4 ? flo : fhi, 0u, 0x4440u | (b & 3))], 1u);
-                        if (kr) atomicAdd(&h[__byte_perm(b < 4 ? rlo : rhi, 0u, 0x4440u | (b & 3))], 1u);
+                        for (int b = 0; b < 8; ++b) {
+                            if (q == W - 1 && b < (int)b0) continue;     // padding bytes of the last word: no pass
+                            atomicAdd(&hq[b * kRadix + __byte_perm(b < 4 ? lo : hi, 0u, 0x4440u | (b & 3))], 1u);
+                        }
                     }
-                }
+                };
+                if (kf) add_key(f);
+                if (kr) add_key(r);
             }
             if (a.bucket_hist && ((valid >> i) & 1)) {
                 atomicAdd(&a.bucket_hist[f[0] >> 48], 1ull);
@@ -168,6 +189,20 @@ __global__ void __launch_bounds__(256) extract_kernel(ExtractArgs a, DevState *s
                 if (kf) csum += mix_key<W>(f);
                 if (kr) csum += mix_key<W>(r);
             }
+        };
+#pragma unroll 1
+        for (u32 ii = 0; ii < 16; ++ii) {
+            if (!((any_mask >> ii) & 1)) continue;     // warp-uniform
+            u64 f[W], r[W];
+            km.template keys_h<0>(ii, f, r);
+            emit_window(ii, f, r);
+        }
+#pragma unroll 1
+        for (u32 ii = 0; ii < 16; ++ii) {
+            if (!((any_mask >> (16 + ii)) & 1)) continue;
+            u64 f[W], r[W];
+            km.template keys_h<1>(ii, f, r);
+            emit_window(16 + ii, f, r);
         }
     }
     if (a.want_csum) {
