@@ -2,10 +2,11 @@
 // "all (k+1)-mers from the input reads are sorted and counted, and only (k+1)-mers that appear at least d (2 by
 // default) times are kept" (§2 ¶3; cnt >= d, reading A8; counts saturate at 2^32-1, A9).
 //
-// Two streaming sweeps and a scan between them; see count_tiles_kernel.
+// Two streaming sweeps and a scan between them; see count_chunks_kernel.
 //
 // Also here: the merge kernels of sdbg_build's unsorted path (equal keys merged by summing mult).
 #include "kernels.cuh"
+#include <type_traits>
 
 namespace sdbg {
 
@@ -111,181 +112,186 @@ __device__ __forceinline__ bool key_lt(const u64 (&a)[W], const u64 (&b)[W]) {  
     return lt;
 }
 
-// 64 bytes of consecutive records per thread (vector loads), 6 blocks of 256 threads per SM
-#ifndef SDBG_CNT_THREADS
-#define SDBG_CNT_THREADS 256
-#define SDBG_CNT_MINB 6
-#define SDBG_CNT_BYTES 64
-#endif
-template <int W> struct CountCfg { static constexpr int THREADS = SDBG_CNT_THREADS, IPT = SDBG_CNT_BYTES / 8 / W; };
-template <> struct CountCfg<3> { static constexpr int THREADS = SDBG_CNT_THREADS, IPT = SDBG_CNT_BYTES / 32; };
-
-// Two sweeps over the sorted records with one tiny scan between them, instead of one sweep whose tiles are chained by a
-// decoupled look-back: a tile here is 32 KiB and lives a few microseconds, so a chain that costs several L2 round
-// trips per tile (measured: ~5 us of a ~9 us tile life) caps the single-sweep kernel far below the
-// cost of simply reading the records twice.
-//   sweep 1 (WRITE = false): solid edges of every tile -> tile_sums[tile]; statistics
-//   scan                   : tile_sums -> exclusive prefix, total -> output cursor
-//   sweep 2 (WRITE = true) : the same arithmetic again, solid edges written at out_base + prefix[tile] + rank in tile
+// Two sweeps over the sorted records with one small scan between them, instead of one sweep whose tiles are chained by
+// a decoupled look-back: a tile lives a few microseconds, and a chain that costs several L2 round trips per tile
+// (measured: ~5 us of a ~9 us tile life) caps the single-sweep kernel far below the cost of simply
+// reading the records twice.
+//   sweep 1 (WRITE = false): solid edges of every chunk -> chunk_sums[chunk]; statistics
+//   scan                   : chunk_sums -> exclusive prefix, total -> output cursor
+//   sweep 2 (WRITE = true) : the same arithmetic again, solid edges written at out_base + prefix[chunk] + rank in chunk
 //
-// A record i is a run TAIL iff i == n-1 or key[i] != key[i+1]; the run ending at tail i has length i+1 - (start of
-// the run). Inside a warp's 32*IPT records the start is the place after the previous tail (exclusive max-scan over
-// the lanes, by shuffles); for the run that is open at the warp's first record it is found by looking at the records
-// right before it, 32 at a time, and, past 128 of them, by a 32-ary search for the first record equal to it (the
-// records are sorted). So no state about runs travels between warps or tiles. All indices are tile-relative u32
-// (modulo 2^32: a sort range holds fewer than 2^32 records, so run lengths come out right even when a run began
-// before the tile).
-template <int W, bool WRITE>
-__global__ void __launch_bounds__(CountCfg<W>::THREADS, SDBG_CNT_MINB) count_tiles_kernel(CountArgs a, DevState *st) {
-    constexpr int THREADS = CountCfg<W>::THREADS, IPT = CountCfg<W>::IPT, TILE = THREADS * IPT, WARPS = THREADS / 32;
-    __shared__ u32 s_wsolid[WARPS];
-    __shared__ u64 s_red[3][WARPS];
-    const u32 tid = threadIdx.x, lane = tid & 31u, warp = tid >> 5;
-    const u32 tile = blockIdx.x;
-    const u64 tile_base = (u64)tile * TILE;
-    const u32 rem = (a.n - tile_base < (u64)TILE) ? (u32)(a.n - tile_base) : (u32)TILE;   // records of this tile
-    const bool has_succ = tile_base + TILE < a.n;       // a record follows the tile
-    const u32 li0 = tid * IPT;                           // tile-relative index of my first record
-    const u64 *kp = a.keys + (tile_base + li0) * W;
+// A chunk is kCountChunk consecutive records and belongs to ONE WARP, which walks it in rounds of 32 records, lane l
+// holding record 32 r + l (coalesced loads, several rounds in flight). A record i is a run TAIL iff i == n-1 or
+// key[i] != key[i+1] (the next key comes from the next lane by shuffle); the run ending at tail i has length
+// i+1 - (start of the run), and the start is the place after the previous tail: the nearest lower tail of the round
+// (one ballot, one find-leading-one) or the warp-uniform carry from the rounds before. For the run that is open at
+// the chunk's first record the start is found by looking at the records right before it, 32 at a time, and, past
+// 128 of them, by a 32-ary search for the first record equal to it (the records are sorted). So no state about runs
+// travels between warps. Indices are chunk-relative u32 (modulo 2^32: a sort range holds fewer than 2^32 records, so
+// run lengths come out right even when a run began long before the chunk).
+constexpr u32 kCountChunk = 1024;        // records per warp
+constexpr int kCountWarps = 8;           // warps per block
+constexpr int kCountGroup = 4;           // rounds loaded ahead
 
-    // ---- load IPT consecutive records + the one after them -------------------------------------------------------
-    u64 key[IPT + 1][W];
-    if (li0 + IPT < rem || (li0 + IPT == rem && has_succ)) {
-        if constexpr (W == 1) {
+template <int W>
+__device__ __forceinline__ void shfl_key(u64 (&dst)[W], const u64 (&src)[W], int src_lane) {
 #pragma unroll
-            for (int j = 0; j < IPT; j += 2) {      // 64 bytes per thread, 16-byte aligned
-                ulonglong2 v = *reinterpret_cast<const ulonglong2 *>(kp + j);
-                key[j][0] = v.x; key[j + 1][0] = v.y;
-            }
-            key[IPT][0] = kp[IPT];
-        } else {
-#pragma unroll
-            for (int j = 0; j <= IPT; ++j) load_key<W>(kp, j, key[j]);
-        }
-    } else {
-#pragma unroll
-        for (int j = 0; j <= IPT; ++j) {
-            if (li0 + j < rem) load_key<W>(kp, j, key[j]);
+    for (int q = 0; q < W; ++q) dst[q] = __shfl_sync(0xffffffffu, src[q], src_lane);
+}
+
+template <int W, bool WRITE>
+__global__ void __launch_bounds__(kCountWarps * 32, W == 1 ? 6 : W == 2 ? 4 : 2) count_chunks_kernel(CountArgs a, DevState *st) {
+    constexpr int G = kCountGroup;
+    __shared__ u64 s_red[3][kCountWarps];
+    const u32 tid = threadIdx.x, lane = tid & 31u, warp = tid >> 5;
+    const u32 lt = lanemask_lt();
+    const u64 chunk = (u64)blockIdx.x * kCountWarps + warp;
+    const u64 c0 = chunk * kCountChunk;                     // global index of the chunk's first record
+    u32 n_tails = 0, n_solid = 0, sum_mult = 0;             // lengths of the runs ending in one chunk add up to < 2^32
+    u64 csum = 0;
+    if (c0 < a.n) {
+        const u32 rem = (a.n - c0 < (u64)kCountChunk) ? (u32)(a.n - c0) : kCountChunk;   // records of this chunk
+        const bool has_succ = c0 + kCountChunk < a.n;                                    // a record follows the chunk
+        const u64 *kp = a.keys + c0 * W;
+        auto load_round = [&](u32 r, u64 (&k)[W]) {         // record 32 r + lane, or zeros past the end of the data
+            const u32 i = r * 32u + lane;
+            if (i < rem || (i == rem && has_succ)) load_key<W>(kp, i, k);
             else {
 #pragma unroll
-                for (int q = 0; q < W; ++q) key[j][q] = 0;
+                for (int q = 0; q < W; ++q) k[q] = 0;
             }
-        }
-    }
-    u32 tails = 0, last_local = 0;   // last_local: tile-relative index+1 of my last tail (0 = none)
-#pragma unroll
-    for (int j = 0; j < IPT; ++j) {
-        const u32 li = li0 + j;
-        const bool t = li < rem && ((li + 1 == rem && !has_succ) || key_ne<W>(key[j], key[j + 1]));
-        if (t) { tails |= 1u << j; last_local = li + 1; }
-    }
+        };
+        u64 key[G + 1][W];
+        load_round(0, key[0]);
 
-    // ---- start of the run in progress at my first record ----------------------------------------------------------
-    // exclusive max-scan of the tails over the lanes: the value of the nearest lower lane that has a tail
-    const u32 tmask = __ballot_sync(0xffffffffu, last_local != 0) & lanemask_lt();
-    u32 excl_max = __shfl_sync(0xffffffffu, last_local, tmask ? 31 - __clz(tmask) : 0);
-    if (!tmask) excl_max = 0;
-    // the run open at the warp's first record (needed by the lanes with no tail before them in the warp)
-    const u32 wfirst = warp * 32u * IPT;                 // tile-relative index of the warp's first record
-    u32 wstart = wfirst;
-    if (wfirst < rem) {
-        u64 target[W], probe[W];
-#pragma unroll
-        for (int q = 0; q < W; ++q) target[q] = __shfl_sync(0xffffffffu, key[0][q], 0);
-        // hi = lowest index known to belong to the run. Up to 4 rounds over the 32 records right below hi (these lines
-        // were just read by the neighbouring warp or tile), then a 32-ary search over all that lies below.
-        u64 hi = tile_base + wfirst;
-        bool found = false;
+        // ---- start of the run that is open at the chunk's first record ----------------------------------------
+        u32 carry;                                           // chunk-relative start of the run in progress
+        {
+            u64 target[W], probe[W];
+            shfl_key<W>(target, key[0], 0);
+            // hi = lowest index known to belong to the run. Up to 4 rounds over the 32 records right below hi (these
+            // lines were just read by the neighbouring warp), then a 32-ary search over all that lies below.
+            u64 hi = c0;
+            bool found = false;
 #pragma unroll 1
-        for (int r = 0; r < 4 && !found && hi > 0; ++r) {
-            const bool inb = hi > (u64)lane;
-            if (inb) load_key<W>(a.keys, hi - 1 - lane, probe);
-            const u32 eqm = __ballot_sync(0xffffffffu, inb && !key_ne<W>(probe, target));
-            const u32 lead = (eqm == 0xffffffffu) ? 32u : (u32)__ffs(~eqm) - 1u;   // equal records right below hi
-            hi -= lead;
-            found = lead < 32u;
-        }
-        if (!found && hi > 0) {
-            u64 lo = 0;                                  // first index in [lo, hi] whose key is not less than target
-            while (lo < hi) {
-                const u64 span = hi - lo;
-                const u64 p = span > 32 ? lo + (span / 33) * (lane + 1) : lo + lane;   // 32 probes, increasing with the lane
-                bool ge = true;
-                if (p < hi) { load_key<W>(a.keys, p, probe); ge = !key_lt<W>(probe, target); }
-                const u32 gem = __ballot_sync(0xffffffffu, ge);    // monotone: 0..0 1..1
-                const u32 f = gem ? (u32)__ffs(gem) - 1u : 32u;    // first probe inside the run (or none)
-                const u64 pf = __shfl_sync(0xffffffffu, p, (int)(f < 32u ? f : 31u));
-                const u64 pb = __shfl_sync(0xffffffffu, p, (int)(f ? f - 1u : 0u));
-                if (f < 32u && pf < hi) hi = pf;
-                if (f > 0u) lo = (pb < hi ? pb : hi - 1) + 1;      // the probe before the first hit is outside the run
+            for (int r = 0; r < 4 && !found && hi > 0; ++r) {
+                const bool inb = hi > (u64)lane;
+                if (inb) load_key<W>(a.keys, hi - 1 - lane, probe);
+                const u32 eqm = __ballot_sync(0xffffffffu, inb && !key_ne<W>(probe, target));
+                const u32 lead = (eqm == 0xffffffffu) ? 32u : (u32)__ffs(~eqm) - 1u;   // equal records right below hi
+                hi -= lead;
+                found = lead < 32u;
             }
-            hi = lo;
+            if (!found && hi > 0) {
+                u64 lo = 0;                                  // first index in [lo, hi] whose key is not less than target
+                while (lo < hi) {
+                    const u64 span = hi - lo;
+                    const u64 p = span > 32 ? lo + (span / 33) * (lane + 1) : lo + lane;   // 32 probes, increasing with the lane
+                    bool ge = true;
+                    if (p < hi) { load_key<W>(a.keys, p, probe); ge = !key_lt<W>(probe, target); }
+                    const u32 gem = __ballot_sync(0xffffffffu, ge);    // monotone: 0..0 1..1
+                    const u32 f = gem ? (u32)__ffs(gem) - 1u : 32u;    // first probe inside the run (or none)
+                    const u64 pf = __shfl_sync(0xffffffffu, p, (int)(f < 32u ? f : 31u));
+                    const u64 pb = __shfl_sync(0xffffffffu, p, (int)(f ? f - 1u : 0u));
+                    if (f < 32u && pf < hi) hi = pf;
+                    if (f > 0u) lo = (pb < hi ? pb : hi - 1) + 1;      // the probe before the first hit is outside the run
+                }
+                hi = lo;
+            }
+            carry = (u32)(hi - c0);                          // modulo 2^32 when the run began before the chunk
         }
-        wstart = (u32)(hi - tile_base);                  // modulo 2^32 when the run began before the tile
-    }
-    u32 prev = excl_max ? excl_max : wstart;
 
-    // ---- run lengths, solid flags, statistics --------------------------------------------------------------------
-    u32 solid = 0, n_solid = 0;
-    u32 len[IPT];
-    u32 sum_mult = 0;   // solid runs ending in one warp are disjoint intervals of one range: their lengths add up to < 2^32
-    u64 csum = 0;
+        // ---- rounds --------------------------------------------------------------------------------------------
+        u64 out_pos = 0;
+        if constexpr (WRITE) {   // solid edges of earlier ranges + of earlier blocks + of the lower warps of this block
+            out_pos = st->out_cursor[a.range_parity] + a.tile_sums[blockIdx.x];
+            const u32 *ws = reinterpret_cast<const u32 *>(a.tile_sums + gridDim.x) + (u64)blockIdx.x * kCountWarps;
+            for (u32 w = 0; w < warp; ++w) out_pos += ws[w];
+        }
+        // one round: FULL = every record of the round and its successor exist (no index checks)
+        auto round = [&](auto full_tag, u32 r, const u64 (&k)[W], const u64 (&k_next_round)[W]) {
+            constexpr bool FULL = decltype(full_tag)::value;
+            const u32 i = r * 32u + lane;
+            u64 kn[W];                                              // the record after mine: lane l+1, or lane 0 of the next round
 #pragma unroll
-    for (int j = 0; j < IPT; ++j) {
-        len[j] = 0;
-        if ((tails >> j) & 1u) {
-            const u32 e = li0 + j + 1;
-            len[j] = e - prev;
-            prev = e;
-            if (len[j] >= a.d) { solid |= 1u << j; ++n_solid; sum_mult += len[j]; }
-            if (!WRITE && a.want_csum) csum += (u64)len[j] * mix_key<W>(key[j]);
+            for (int q = 0; q < W; ++q) kn[q] = __shfl_sync(0xffffffffu, lane == 0 ? k_next_round[q] : k[q], (int)((lane + 1u) & 31u));
+            bool tail = key_ne<W>(k, kn);
+            if constexpr (!FULL) tail = i < rem && ((i + 1u == rem && !has_succ) || tail);
+            const u32 T = __ballot_sync(0xffffffffu, tail);
+            const u32 below = T & lt;
+            const u32 start = below ? r * 32u + (32u - (u32)__clz(below)) : carry;   // place after the previous tail
+            const u32 len = i + 1u - start;
+            const bool solid = tail && len >= a.d;
+            const u32 S = __ballot_sync(0xffffffffu, solid);
+            if (T) carry = r * 32u + (32u - (u32)__clz(T));
+            if constexpr (!WRITE) {
+                n_tails += (u32)__popc(T);
+                n_solid += (u32)__popc(S);
+                if (solid) sum_mult += len;
+                if (a.want_csum && tail) csum += (u64)len * mix_key<W>(k);
+            } else {
+                if (solid) {
+                    const u64 pos = out_pos + (u32)__popc(S & lt);
+                    if (pos < a.out_cap) {
+#pragma unroll
+                        for (int q = 0; q < W; ++q) a.out_keys[pos * W + q] = k[q];
+                        a.out_mult[pos] = len;   // < 2^32 by the range bound: the saturation of A9 cannot be reached
+                    }
+                }
+                out_pos += (u32)__popc(S);
+            }
+        };
+        if (rem == kCountChunk && c0 + kCountChunk + 32u <= a.n) {
+            // full chunk with at least 32 records behind it: plain loads, G rounds in flight
+#pragma unroll 1
+            for (u32 r0 = 0; r0 < kCountChunk / 32u; r0 += G) {
+#pragma unroll
+                for (int g = 1; g <= G; ++g) load_key<W>(kp, (r0 + g) * 32u + lane, key[g]);
+#pragma unroll
+                for (int g = 0; g < G; ++g) round(std::true_type{}, r0 + g, key[g], key[g + 1]);
+#pragma unroll
+                for (int q = 0; q < W; ++q) key[0][q] = key[G][q];
+            }
+        } else {
+            const u32 nrounds = (rem + 31u) / 32u;
+#pragma unroll 1
+            for (u32 r = 0; r < nrounds; ++r) {
+                load_round(r + 1, key[1]);
+                round(std::false_type{}, r, key[0], key[1]);
+#pragma unroll
+                for (int q = 0; q < W; ++q) key[0][q] = key[1][q];
+            }
         }
     }
-    const u32 incl = warp_incl_scan_add(n_solid);
-    if (lane == 31) s_wsolid[warp] = incl;
     if constexpr (!WRITE) {
-        const u32 nt = __reduce_add_sync(0xffffffffu, (u32)__popc(tails));
+        // per-warp and per-block numbers of solid edges; statistics: block reduction, one atomic per block and
+        // counter, spread over 32 slots
+        __shared__ u32 s_solid[kCountWarps];
         sum_mult = __reduce_add_sync(0xffffffffu, sum_mult);
         if (a.want_csum) csum = warp_reduce_add64(csum);
-        if (lane == 0) { s_red[0][warp] = nt; s_red[1][warp] = sum_mult; s_red[2][warp] = csum; }
-    }
-    __syncthreads();
-    if constexpr (!WRITE) {
-        if (tid == 0) {
-            u32 tile_solid = 0;
-#pragma unroll
-            for (int w = 0; w < WARPS; ++w) tile_solid += s_wsolid[w];
-            a.tile_sums[tile] = tile_solid;
-        } else if (warp == 1 && lane < 3) {   // statistics: one atomic per block and counter, spread over 32 slots
+        if (lane == 0) {
+            s_red[0][warp] = n_tails; s_red[1][warp] = sum_mult; s_red[2][warp] = csum; s_solid[warp] = n_solid;
+            reinterpret_cast<u32 *>(a.tile_sums + gridDim.x)[chunk] = n_solid;
+        }
+        __syncthreads();
+        if (tid < 3) {
             u64 v = 0;
 #pragma unroll
-            for (int w = 0; w < WARPS; ++w) v += s_red[lane][w];
-            if (v) atomicAdd(&a.stat_slots[(tile & (kStatSlots - 1)) * kStatSlotWords + lane], v);
-        }
-    } else {
-        u32 woff = 0;
+            for (int w = 0; w < kCountWarps; ++w) v += s_red[tid][w];
+            if (v) atomicAdd(&a.stat_slots[(blockIdx.x & (kStatSlots - 1)) * kStatSlotWords + tid], v);
+        } else if (tid == 32) {
+            u64 v = 0;
 #pragma unroll
-        for (int w = 0; w < WARPS; ++w) woff += (w < (int)warp) ? s_wsolid[w] : 0u;
-        // solid edges appended by earlier ranges + solid edges of the tiles before this one + rank in the tile
-        u64 pos = st->out_cursor[a.range_parity] + a.tile_sums[tile] + woff + incl - n_solid;
-#pragma unroll
-        for (int j = 0; j < IPT; ++j) {
-            if ((solid >> j) & 1u) {
-                if (pos < a.out_cap) {
-#pragma unroll
-                    for (int q = 0; q < W; ++q) a.out_keys[pos * W + q] = key[j][q];
-                    a.out_mult[pos] = len[j];   // < 2^32 by the range bound: the saturation of A9 cannot be reached
-                }
-                ++pos;
-            }
+            for (int w = 0; w < kCountWarps; ++w) v += s_solid[w];
+            a.tile_sums[blockIdx.x] = v;
         }
     }
 }
 
-// tile_sums -> exclusive prefix, in place; total added to the output cursor of the next range. One block (the array
-// has one word per 16 KiB of records), 16 words per thread and round.
+// tile_sums (one word per block of the sweeps = 64 KiB of records) -> exclusive prefix, in place; total added to the
+// output cursor of the next range. One block, 4 words per thread and round.
 __global__ void __launch_bounds__(1024) scan_tiles_kernel(u64 *tile_sums, u32 ntiles, DevState *st, int range_parity) {
-    constexpr u32 PER = 16, ROUND = 1024 * PER;
+    constexpr u32 PER = 4, ROUND = 1024 * PER;   // 32 contiguous bytes per thread: whole sectors
     __shared__ u64 s_w[32];
     __shared__ u64 s_carry;
     const u32 tid = threadIdx.x, lane = tid & 31u, warp = tid >> 5;
@@ -315,21 +321,17 @@ __global__ void __launch_bounds__(1024) scan_tiles_kernel(u64 *tile_sums, u32 nt
     if (tid == 0) st->out_cursor[range_parity ^ 1] = st->out_cursor[range_parity] + s_carry;
 }
 
-template <int W> static constexpr u64 count_tile() { return (u64)CountCfg<W>::THREADS * CountCfg<W>::IPT; }
-
-u64 count_tile_records(u32 W) {
-    switch (W) { case 1: return count_tile<1>(); case 2: return count_tile<2>(); case 3: return count_tile<3>(); case 4: return count_tile<4>(); }
-    return 0;
-}
+u64 count_tile_records(u32) { return kCountChunk; }
 
 template <int W>
 static int launch_count_w(const CountArgs &a, DevState *st, cudaStream_t s) {
-    const u64 tiles = (a.n + count_tile<W>() - 1) / count_tile<W>();
-    if (tiles == 0) return 0;
-    if (tiles > 0x7fffffffull) return (int)cudaErrorInvalidValue;
-    count_tiles_kernel<W, false><<<(unsigned)tiles, CountCfg<W>::THREADS, 0, s>>>(a, st);
-    scan_tiles_kernel<<<1, 1024, 0, s>>>(a.tile_sums, (u32)tiles, st, a.range_parity);
-    count_tiles_kernel<W, true><<<(unsigned)tiles, CountCfg<W>::THREADS, 0, s>>>(a, st);
+    const u64 chunks = (a.n + kCountChunk - 1) / kCountChunk;
+    if (chunks == 0) return 0;
+    const u64 blocks = (chunks + kCountWarps - 1) / kCountWarps;
+    if (blocks > 0x7fffffffull) return (int)cudaErrorInvalidValue;
+    count_chunks_kernel<W, false><<<(unsigned)blocks, kCountWarps * 32, 0, s>>>(a, st);
+    scan_tiles_kernel<<<1, 1024, 0, s>>>(a.tile_sums, (u32)blocks, st, a.range_parity);
+    count_chunks_kernel<W, true><<<(unsigned)blocks, kCountWarps * 32, 0, s>>>(a, st);
     return (int)cudaGetLastError();
 }
 

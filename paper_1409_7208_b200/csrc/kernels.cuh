@@ -74,7 +74,8 @@ void launch_key_hist(const u64 *keys, u64 n, u32 W, const PassTable &pt, u64 *di
 struct CountArgs {
     const u64 *keys; u64 n; u32 W, d;
     u64 *out_keys; u32 *out_mult; u64 out_cap;
-    u64 *tile_sums;          // u64[tiles] scratch: solid edges per tile, then their exclusive prefix
+    u64 *tile_sums;          // scratch of 8 bytes per count_tile_records() records: u64 per block of the sweeps (solid
+                             // edges, then their exclusive prefix), behind them u32 per warp chunk
     u64 *stat_slots;         // u64[kStatSlots][kStatSlotWords], accumulated
     int want_csum;
     int range_parity;        // reads st->out_cursor[parity], writes st->out_cursor[parity^1]
