@@ -38,8 +38,8 @@ namespace sdbg {
 template <int W, bool HAS_VAL> struct RadixCfg;
 // THREADS x KPT records per tile; keys are staged in shared memory (TILE * 8W bytes).
 #ifndef SDBG_R1_THREADS
-#define SDBG_R1_THREADS 512
-#define SDBG_R1_KPT 16
+#define SDBG_R1_THREADS 384   // 384 x 21 = 8,064 keys per tile, 2 CTAs per SM, up to 80 registers (measured best)
+#define SDBG_R1_KPT 21
 #define SDBG_R1_MINB 2
 #endif
 template <> struct RadixCfg<1, false> { static constexpr int THREADS = SDBG_R1_THREADS, KPT = SDBG_R1_KPT, MINB = SDBG_R1_MINB; };
