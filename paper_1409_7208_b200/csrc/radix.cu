@@ -45,7 +45,12 @@ template <int W, bool HAS_VAL> struct RadixCfg;
 template <> struct RadixCfg<1, false> { static constexpr int THREADS = SDBG_R1_THREADS, KPT = SDBG_R1_KPT, MINB = SDBG_R1_MINB; };
 template <> struct RadixCfg<2, false> { static constexpr int THREADS = 512, KPT = 8,  MINB = 2; };
 template <> struct RadixCfg<3, false> { static constexpr int THREADS = 512, KPT = 5,  MINB = 2; };
-template <> struct RadixCfg<4, false> { static constexpr int THREADS = 512, KPT = 4,  MINB = 2; };
+#ifndef SDBG_R4_THREADS
+#define SDBG_R4_THREADS 256   // 256 x 8 four-word keys = 64 KiB per tile (measured best on config 4)
+#define SDBG_R4_KPT 8
+#define SDBG_R4_MINB 2
+#endif
+template <> struct RadixCfg<4, false> { static constexpr int THREADS = SDBG_R4_THREADS, KPT = SDBG_R4_KPT, MINB = SDBG_R4_MINB; };
 template <> struct RadixCfg<1, true>  { static constexpr int THREADS = 512, KPT = 10, MINB = 2; };
 template <> struct RadixCfg<2, true>  { static constexpr int THREADS = 512, KPT = 6,  MINB = 2; };
 template <> struct RadixCfg<3, true>  { static constexpr int THREADS = 512, KPT = 4,  MINB = 2; };
