@@ -139,7 +139,7 @@ __device__ __forceinline__ void shfl_key(u64 (&dst)[W], const u64 (&src)[W], int
     for (int q = 0; q < W; ++q) dst[q] = __shfl_sync(0xffffffffu, src[q], src_lane);
 }
 
-template <int W, bool WRITE>
+template <int W, bool WRITE, bool CSUM>
 __global__ void __launch_bounds__(kCountWarps * 32, W == 1 ? 6 : W == 2 ? 4 : 2) count_chunks_kernel(CountArgs a, DevState *st) {
     constexpr int G = kCountGroup;
     __shared__ u64 s_red[3][kCountWarps];
@@ -228,7 +228,7 @@ __global__ void __launch_bounds__(kCountWarps * 32, W == 1 ? 6 : W == 2 ? 4 : 2)
                 n_tails += (u32)__popc(T);
                 n_solid += (u32)__popc(S);
                 if (solid) sum_mult += len;
-                if (a.want_csum && tail) csum += (u64)len * mix_key<W>(k);
+                if constexpr (CSUM) { if (tail) csum += (u64)len * mix_key<W>(k); }
             } else {
                 if (solid) {
                     const u64 pos = out_pos + (u32)__popc(S & lt);
@@ -268,7 +268,7 @@ __global__ void __launch_bounds__(kCountWarps * 32, W == 1 ? 6 : W == 2 ? 4 : 2)
         // counter, spread over 32 slots
         __shared__ u32 s_solid[kCountWarps];
         sum_mult = __reduce_add_sync(0xffffffffu, sum_mult);
-        if (a.want_csum) csum = warp_reduce_add64(csum);
+        if constexpr (CSUM) csum = warp_reduce_add64(csum);
         if (lane == 0) {
             s_red[0][warp] = n_tails; s_red[1][warp] = sum_mult; s_red[2][warp] = csum; s_solid[warp] = n_solid;
             reinterpret_cast<u32 *>(a.tile_sums + gridDim.x)[chunk] = n_solid;
@@ -329,9 +329,10 @@ static int launch_count_w(const CountArgs &a, DevState *st, cudaStream_t s) {
     if (chunks == 0) return 0;
     const u64 blocks = (chunks + kCountWarps - 1) / kCountWarps;
     if (blocks > 0x7fffffffull) return (int)cudaErrorInvalidValue;
-    count_chunks_kernel<W, false><<<(unsigned)blocks, kCountWarps * 32, 0, s>>>(a, st);
+    if (a.want_csum) count_chunks_kernel<W, false, true><<<(unsigned)blocks, kCountWarps * 32, 0, s>>>(a, st);
+    else             count_chunks_kernel<W, false, false><<<(unsigned)blocks, kCountWarps * 32, 0, s>>>(a, st);
     scan_tiles_kernel<<<1, 1024, 0, s>>>(a.tile_sums, (u32)blocks, st, a.range_parity);
-    count_chunks_kernel<W, true><<<(unsigned)blocks, kCountWarps * 32, 0, s>>>(a, st);
+    count_chunks_kernel<W, true, false><<<(unsigned)blocks, kCountWarps * 32, 0, s>>>(a, st);
     return (int)cudaGetLastError();
 }
 
