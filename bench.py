@@ -124,6 +124,26 @@ def cpu_baseline(w, n_reads):
             "sample": f"first {n_reads} reads of {w.name} ({n_rec} records), {dt:.1f} s, single thread"}
 
 
+def rank_seed(base_seed: int, rank: int) -> int:
+    """Replicas only: every rank sorts its own read set."""
+    return base_seed + 1000003 * rank
+
+
+def max_over_ranks(values, device="cpu"):
+    """Element-wise MAX of a list of floats over all ranks of the default process group (identity without one)."""
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor(list(values), dtype=torch.float64, device=device)
+    if dist.is_available() and dist.is_initialized() and dist.get_world_size() > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return [float(x) for x in t]
+
+
+def whole_job_value(records_per_rank: int, world: int, steps: int, ms_max: float) -> float:
+    """Records all ranks processed / the slowest rank's time (weak scaling: per-rank work is fixed)."""
+    return world * records_per_rank * steps / (ms_max * 1e-3)
+
+
 def run_gpu(args, w):
     import torch
     import torch.distributed as dist
@@ -139,7 +159,7 @@ def run_gpu(args, w):
 
     # ---- inputs resident in HBM: every rank an independent replica (own seed) ------------------------------
     from dataclasses import replace
-    wl = replace(w, seed=w.seed + 1000003 * rank) if rank else w
+    wl = replace(w, seed=rank_seed(w.seed, rank)) if rank else w
     gen = ReadGenerator(wl)
     bases_d, offs_d = gen.device()
     torch.cuda.synchronize()
@@ -213,10 +233,7 @@ def run_gpu(args, w):
     h2d = n_bases + 8 * (n_reads + 1)
     d2h = S * (1 + 4 + K) + 8 * ((S + 63) // 64)
 
-    t = torch.tensor([ms_total, ms_e2e], dtype=torch.float64, device="cuda")
-    if world > 1:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    ms_total, ms_e2e = float(t[0]), float(t[1])
+    ms_total, ms_e2e = max_over_ranks([ms_total, ms_e2e], device="cuda")
     if rank != 0:
         if world > 1:
             dist.destroy_process_group()
@@ -228,7 +245,7 @@ def run_gpu(args, w):
     algo_bytes = 2 * N * K                       # one pass reads and writes every key once
     achieved = algo_bytes / (radix_ms * 1e-3) / 1e9 if radix_ms > 0 else 0.0
     line = {
-        "metric": METRIC, "value": world * N * args.steps / (ms_total * 1e-3), "unit": UNIT, "n_gpus": world,
+        "metric": METRIC, "value": whole_job_value(N, world, args.steps, ms_total), "unit": UNIT, "n_gpus": world,
         "steps": args.steps, "warmup": max(args.warmup, 3), "ms_per_step": ms_total / args.steps,
         "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "u64", "data": "synthetic",
         "config": {"workload": wl.name, "k": wl.k, "d": wl.d, "reads": n_reads, "read_len": wl.read_len, "bases": n_bases,
@@ -236,7 +253,7 @@ def run_gpu(args, w):
                    "l2": "inputs larger than L2 (keys %.2f GB, reads %.0f MB ASCII)" % (N * K / 1e9, n_bases / 1e6)},
         "read_bases_per_s": world * n_bases * args.steps / (ms_total * 1e-3),
         "clocks": clocks,
-        "e2e": {"value": world * N * args.steps / (ms_e2e * 1e-3), "unit": UNIT, "h2d_bytes_per_step": h2d,
+        "e2e": {"value": whole_job_value(N, world, args.steps, ms_e2e), "unit": UNIT, "h2d_bytes_per_step": h2d,
                 "d2h_bytes_per_step": d2h, "ms_per_step": ms_e2e / args.steps},
         "gpu_launches": int(tim.total_launches),
         "roofline": {"kernel": "onesweep_kernel (one LSD radix pass)", "bound": "hbm", "achieved": achieved, "peak": peak,
