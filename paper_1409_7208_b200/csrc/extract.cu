@@ -73,6 +73,15 @@ struct KeyMaker {
         rot(Y, fwd);
         rot(win, rc);
     }
+    // l=8 partitions (top 16 key bits) of both keys of window i = 16 HALF + ii, for k >= 8: symbols 1..8 of the
+    // reversed-stream window (forward key) and of the complemented forward window (rc-strand key); two funnel shifts
+    template <int HALF>
+    __device__ __forceinline__ void buckets_h(u32 ii, u32 &bf, u32 &br) const {
+        const u32 wh = __funnelshift_l(w32(B, HALF + 1), w32(B, HALF), 2 * ii);
+        const u32 yh = __funnelshift_l(w32(R, 2 - HALF), w32(R, 1 - HALF), 30 - 2 * ii);
+        bf = (yh >> 14) & 0xffffu;
+        br = (~wh >> 14) & 0xffffu;
+    }
     // 32-bit word m of a stream of u64 words, most significant first
     static __device__ __forceinline__ u32 w32(const u64 (&S)[W + 1], int m) { return (m & 1) ? (u32)S[m >> 1] : (u32)(S[m >> 1] >> 32); }
     __device__ __forceinline__ void keys(u32 i, u64 (&fwd)[W], u64 (&rc)[W]) const {
@@ -133,7 +142,26 @@ __global__ void __launch_bounds__(256) extract_kernel(ExtractArgs a, DevState *s
         km.load(a.words, g < ngroups ? g : 0, a.k);
 
         u32 vf = valid, vr = valid;   // per-strand keep masks
-        if (FILTER) {
+        if (FILTER && a.k >= 8) {
+            // which keys fall into the range of partitions: only the top 16 bits of each key are needed
+            const u32 lo = a.bucket_lo, span = a.bucket_hi - a.bucket_lo;
+            u32 mf = 0, mr = 0;
+#pragma unroll 4
+            for (u32 ii = 0; ii < 16; ++ii) {
+                u32 bf, br;
+                km.template buckets_h<0>(ii, bf, br);
+                mf |= (u32)(bf - lo < span) << ii;
+                mr |= (u32)(br - lo < span) << ii;
+            }
+#pragma unroll 4
+            for (u32 ii = 0; ii < 16; ++ii) {
+                u32 bf, br;
+                km.template buckets_h<1>(ii, bf, br);
+                mf |= (u32)(bf - lo < span) << (16 + ii);
+                mr |= (u32)(br - lo < span) << (16 + ii);
+            }
+            vf = mf & valid; vr = mr & valid;
+        } else if (FILTER) {
             vf = 0; vr = 0;
             for (u32 i = 0; i < 32; ++i) {
                 if (!((valid >> i) & 1)) continue;
@@ -153,56 +181,85 @@ __global__ void __launch_bounds__(256) extract_kernel(ExtractArgs a, DevState *s
             base = __shfl_sync(0xffffffffu, base, 0);
             if (base + total > a.out_cap) continue;   // cannot happen when the caller sized out_cap from the histogram
         }
-        const u32 any_mask = __reduce_or_sync(0xffffffffu, valid);
-        auto emit_window = [&](u32 i, const u64 (&f)[W], const u64 (&r)[W]) {
-            const bool kf = (vf >> i) & 1, kr = (vr >> i) & 1;
-            if (a.keys_out) {
-                const u32 mf = __ballot_sync(0xffffffffu, kf), mr = __ballot_sync(0xffffffffu, kr);
-                if (kf) store_key<W>(a.keys_out, base + __popc(mf & lt), f);
-                base += __popc(mf);
-                if (kr) store_key<W>(a.keys_out, base + __popc(mr & lt), r);
-                base += __popc(mr);
-            }
-            if (do_hist) {
-                // every pass is one whole byte of a key word (api.cu make_passes): byte b of word q is pass
-                // (b - b0) for the last word and (8 - b0) + 8 (W-2-q) + b for the others, b0 = first significant byte
-                auto add_key = [&](const u64 (&key)[W]) {
+        // digit histograms of one key: every pass is one whole byte of a key word (api.cu make_passes): byte b of word
+        // q is pass (b - b0) for the last word and (8 - b0) + 8 (W-2-q) + b for the others, b0 = first significant byte
+        auto add_digits = [&](const u64 (&key)[W]) {
 #pragma unroll
-                    for (int q = W - 1; q >= 0; --q) {
-                        u32 *hq = (q == W - 1) ? h_last : h_last + ((8 - b0) + 8 * (W - 2 - q) + b0) * kRadix;
-                        const u32 lo = (u32)key[q], hi = (u32)(key[q] >> 32);
+            for (int q = W - 1; q >= 0; --q) {
+                u32 *hq = (q == W - 1) ? h_last : h_last + ((8 - b0) + 8 * (W - 2 - q) + b0) * kRadix;
+                const u32 lo = (u32)key[q], hi = (u32)(key[q] >> 32);
 #pragma unroll
-                        for (int b = 0; b < 8; ++b) {
-                            if (q == W - 1 && b < (int)b0) continue;     // padding bytes of the last word: no pass
-                            atomicAdd(&hq[b * kRadix + __byte_perm(b < 4 ? lo : hi, 0u, 0x4440u | (b & 3))], 1u);
-                        }
-                    }
-                };
-                if (kf) add_key(f);
-                if (kr) add_key(r);
-            }
-            if (a.bucket_hist && ((valid >> i) & 1)) {
-                atomicAdd(&a.bucket_hist[f[0] >> 48], 1ull);
-                atomicAdd(&a.bucket_hist[r[0] >> 48], 1ull);
-            }
-            if (a.want_csum) {
-                if (kf) csum += mix_key<W>(f);
-                if (kr) csum += mix_key<W>(r);
+                for (int b = 0; b < 8; ++b) {
+                    if (q == W - 1 && b < (int)b0) continue;     // padding bytes of the last word: no pass
+                    atomicAdd(&hq[b * kRadix + __byte_perm(b < 4 ? lo : hi, 0u, 0x4440u | (b & 3))], 1u);
+                }
             }
         };
+        // one key per lane (or none): coalesced store at the warp's running position, digit histograms, checksum
+        auto emit_key = [&](bool keep, const u64 (&key)[W]) {
+            if (a.keys_out) {
+                const u32 m = __ballot_sync(0xffffffffu, keep);
+                if (keep) store_key<W>(a.keys_out, base + __popc(m & lt), key);
+                base += __popc(m);
+            }
+            if (keep) {
+                if (do_hist) add_digits(key);
+                if (a.want_csum) csum += mix_key<W>(key);
+            }
+        };
+        if (FILTER && a.k >= 8) {
+            // block-wise pass: a lane keeps only a few of its 64 keys, so it walks over the set bits of its keep masks
+            // (its own window index per step) instead of over all 32 windows
+            u32 rem_f = vf, rem_r = vr;
+            while (__any_sync(0xffffffffu, (rem_f | rem_r) != 0)) {
+                const bool hf = rem_f != 0, hr = rem_r != 0;
+                const u32 i_f = hf ? (u32)__ffs(rem_f) - 1u : 0u, i_r = hr ? (u32)__ffs(rem_r) - 1u : 0u;
+                rem_f &= rem_f - 1u;
+                rem_r &= rem_r - 1u;
+                u64 f[W], r[W], unused[W];
+                km.keys(i_f, f, unused);
+                km.keys(i_r, unused, r);
+                emit_key(hf, f);
+                emit_key(hr, r);
+            }
+        } else {
+            const u32 any_mask = __reduce_or_sync(0xffffffffu, valid);
+            auto emit_window = [&](u32 i, const u64 (&f)[W], const u64 (&r)[W]) {
+                const bool kf = (vf >> i) & 1, kr = (vr >> i) & 1;
+                if (a.keys_out) {
+                    const u32 mf = __ballot_sync(0xffffffffu, kf), mr = __ballot_sync(0xffffffffu, kr);
+                    if (kf) store_key<W>(a.keys_out, base + __popc(mf & lt), f);
+                    base += __popc(mf);
+                    if (kr) store_key<W>(a.keys_out, base + __popc(mr & lt), r);
+                    base += __popc(mr);
+                }
+                if (do_hist) {
+                    if (kf) add_digits(f);
+                    if (kr) add_digits(r);
+                }
+                if (a.want_csum) {
+                    if (kf) csum += mix_key<W>(f);
+                    if (kr) csum += mix_key<W>(r);
+                }
+                if (a.bucket_hist && ((valid >> i) & 1)) {
+                    atomicAdd(&a.bucket_hist[f[0] >> 48], 1ull);
+                    atomicAdd(&a.bucket_hist[r[0] >> 48], 1ull);
+                }
+            };
 #pragma unroll 1
-        for (u32 ii = 0; ii < 16; ++ii) {
-            if (!((any_mask >> ii) & 1)) continue;     // warp-uniform
-            u64 f[W], r[W];
-            km.template keys_h<0>(ii, f, r);
-            emit_window(ii, f, r);
-        }
+            for (u32 ii = 0; ii < 16; ++ii) {
+                if (!((any_mask >> ii) & 1)) continue;     // warp-uniform
+                u64 f[W], r[W];
+                km.template keys_h<0>(ii, f, r);
+                emit_window(ii, f, r);
+            }
 #pragma unroll 1
-        for (u32 ii = 0; ii < 16; ++ii) {
-            if (!((any_mask >> (16 + ii)) & 1)) continue;
-            u64 f[W], r[W];
-            km.template keys_h<1>(ii, f, r);
-            emit_window(16 + ii, f, r);
+            for (u32 ii = 0; ii < 16; ++ii) {
+                if (!((any_mask >> (16 + ii)) & 1)) continue;
+                u64 f[W], r[W];
+                km.template keys_h<1>(ii, f, r);
+                emit_window(16 + ii, f, r);
+            }
         }
     }
     if (a.want_csum) {
