@@ -14,7 +14,6 @@
 // HBM traffic per pass: read n*K + write n*K bytes (K = 8w) — the algorithmic 2nK of DESIGN.md "Byte model" — plus
 // 2 KiB of look-back state per tile.
 #include "kernels.cuh"
-#include <cstdio>
 
 namespace sdbg {
 
@@ -350,19 +349,13 @@ onesweep_kernel(RadixArgs a) {
         bin_start = s_bstart[wbin];
         lb_excl = 0;
         lb_done = true;
-#ifndef SDBG_EXP_LBSKIP
         if (t != 0) {
             lb_done = false;
             lb_t = t - 1;
             lb_pend = ld_relaxed(lb + (u64)lb_t * kRadix);
         }
-#endif
     };
 
-#ifdef SDBG_EXP_TRACE
-    long long tr_block = 0, tr_start = clock64();
-    u32 tr_polls = 0, tr_depth = 0, tr_pre = 0, tr_tiles = 0;
-#endif
     // ---- prologue: first tile up to the point where its (warp, digit) positions are known ---------------------------
     if (tid == 0) s_tick[0] = atomicAdd(a.ticket, 1u);
     zero_rows();
@@ -388,11 +381,6 @@ onesweep_kernel(RadixArgs a) {
             const u32 d = digit8_again<W, HI>(key[j], word, psel);
             const int method = rank_method(j);                        // constant after unrolling
             u32 m;
-#ifdef SDBG_EXP_NORANK
-            m = 1u << lane;
-            if (true) {
-            } else
-#endif
             if (method == kMethodA) {
                 atomicOr(&wm[d], 1u << lane);
                 __syncwarp();
@@ -447,9 +435,6 @@ onesweep_kernel(RadixArgs a) {
 #pragma unroll
             for (int q = 0; q < W; ++q) kk[q] = s_keys[q * TILE + p];
             const u32 d = digit8<W, HI>(kk, word, psel);
-#ifdef SDBG_EXP_NOSTORE
-            if (kk[0] == 0x123456789abcdefull)
-#endif
             store_rec<W>(reinterpret_cast<u64 *>(s_binaddr[d] + (u64)p * (8u * W)), kk);
             if constexpr (HAS_VAL) *reinterpret_cast<u32 *>(s_valaddr[d] + (u64)p * 4u) = s_vals[p];
         };
@@ -460,11 +445,6 @@ onesweep_kernel(RadixArgs a) {
 #pragma unroll 1
             for (u32 p = tid; p < cur_cnt; p += THREADS) write_place(p);
         }
-#ifdef SDBG_EXP_TRACE
-        if (next >= ntiles && tid == 0 && a.epoch == 4 && blockIdx.x % 29 == 0)
-            printf("TRACE cta %u tiles %u total_cyc %lld blocked_cyc %lld blocking_polls/tile %.2f depth_before_block %.2f final_depth %.2f\n", blockIdx.x, tr_tiles,
-                   clock64() - tr_start, tr_block, (double)tr_polls / tr_tiles, (double)tr_pre / tr_tiles, (double)tr_depth / tr_tiles);
-#endif
         if (next >= ntiles) break;
         tile = next;
         __syncthreads();   // s_keys is rewritten by the rank steps that follow
