@@ -10,75 +10,6 @@
 
 namespace sdbg {
 
-// Decoupled look-back over per-tile status words, exclusive SUM over tiles [0, tile); called by all 32 lanes of ONE warp.
-// Word of tile u: [63:62] status, [61:40] span s, [39:0] value v.
-//   LOCAL : v = aggregate of tiles (u-s, u]   (s = 1 when first published: the tile's own aggregate)
-//   GLOBAL: v = aggregate of tiles [0, u]
-// A round reads the 32 words below the current position at once and walks through them, jumping over the span each
-// word covers; after every round the tile RE-PUBLISHES its own word with the span covered so far, so that later tiles
-// jump over it in one step (pointer doubling). Without the spans a round advances at most 32 tiles per L2 round trip,
-// which caps the whole kernel at 32 tiles per round-trip time however many tiles are in flight.
-constexpr u64 kLbVal = (1ull << 40) - 1;
-constexpr u32 kLbSpanMask = (1u << 22) - 1u;
-template <bool IS_MAX>
-__device__ __forceinline__ u64 tile_lookback(u64 *state, u32 tile, u64 aggregate) {
-    static_assert(!IS_MAX, "sum only");
-    const u32 lane = lane_id();
-    if (tile == 0) {
-        if (lane == 0) st_relaxed(state, (kStGlobal << 62) | aggregate);
-        return 0;
-    }
-    if (lane == 0) st_relaxed(state + tile, (kStLocal << 62) | (1ull << 40) | aggregate);
-    u64 excl = 0;
-    long long t = (long long)tile - 1;
-    while (true) {
-        const long long idx = t - (long long)lane;
-        u64 v = kStGlobal << 62;   // virtual tiles before the first: inclusive identity
-        if (idx >= 0) v = ld_relaxed(state + idx);
-        u32 k = 0;
-        bool done = false;
-        while (k < 32u) {
-            const u64 e = __shfl_sync(0xffffffffu, v, (int)k);
-            const u32 status = (u32)(e >> 62);
-            if (status == (u32)kStInvalid) break;           // not published yet: read again from here
-            excl += e & kLbVal;
-            if (status == (u32)kStGlobal) { done = true; break; }
-            k += (u32)(e >> 40) & kLbSpanMask;
-        }
-        if (done) break;
-        t -= (long long)k;
-        if (k && lane == 0) st_relaxed(state + tile, (kStLocal << 62) | ((u64)(tile - 1 - t) + 1ull) << 40 | (excl + aggregate));
-    }
-    if (lane == 0) st_relaxed(state + tile, (kStGlobal << 62) | (excl + aggregate));
-    return excl;
-}
-
-// Block-wide exclusive scan of one u32 per thread (add or max; identity 0). All threads must call it.
-template <int THREADS, bool IS_MAX>
-__device__ __forceinline__ u32 block_excl_scan(u32 v, u32 *s_warp /*[THREADS/32]*/, u32 &total) {
-    const u32 lane = lane_id(), warp = threadIdx.x >> 5;
-    u32 incl = v;
-#pragma unroll
-    for (int o = 1; o < 32; o <<= 1) {
-        const u32 t = __shfl_up_sync(0xffffffffu, incl, o);
-        if (lane >= (u32)o) incl = IS_MAX ? max(incl, t) : incl + t;
-    }
-    u32 excl = __shfl_up_sync(0xffffffffu, incl, 1);
-    if (lane == 0) excl = 0;
-    __syncthreads();   // protect s_warp reuse
-    if (lane == 31) s_warp[warp] = incl;
-    __syncthreads();
-    u32 off = 0, tot = 0;
-#pragma unroll
-    for (int w = 0; w < THREADS / 32; ++w) {
-        const u32 t = s_warp[w];
-        if (w < (int)warp) off = IS_MAX ? max(off, t) : off + t;
-        tot = IS_MAX ? max(tot, t) : tot + t;
-    }
-    total = tot;
-    return IS_MAX ? max(off, excl) : off + excl;
-}
-
 template <int W>
 __device__ __forceinline__ void load_key(const u64 *__restrict__ keys, u64 idx, u64 (&k)[W]) {
     const u64 *src = keys + idx * W;
@@ -318,7 +249,10 @@ __global__ void __launch_bounds__(1024) scan_tiles_kernel(u64 *tile_sums, u32 nt
         if (tid == 1023) s_carry = run;
         __syncthreads();
     }
-    if (tid == 0) st->out_cursor[range_parity ^ 1] = st->out_cursor[range_parity] + s_carry;
+    if (tid == 0) {
+        if (range_parity < 0) st->merge_heads = s_carry;   // sdbg_build's merge: number of distinct keys
+        else st->out_cursor[range_parity ^ 1] = st->out_cursor[range_parity] + s_carry;
+    }
 }
 
 u64 count_tile_records(u32) { return kCountChunk; }
@@ -347,45 +281,99 @@ int launch_count_filter(const CountArgs &a, DevState *st, cudaStream_t s) {
 }
 
 // ---- sdbg_build unsorted path: merge equal adjacent keys, summing mult ------------------------------------------------
-// Pass 1: head flags -> distinct index of every record (inclusive sum-scan, look-back across tiles); heads write their
-// key, every record adds its mult into acc[distinct index]. Pass 2: saturate acc into out_mult.
-constexpr int kMergeThreads = 256;
-
-template <int W>
-__global__ void __launch_bounds__(kMergeThreads) merge_kernel(MergeArgs a, DevState *st) {
-    __shared__ u32 s_tile;
-    __shared__ u32 s_warp[kMergeThreads / 32];
-    __shared__ u64 s_bcast;
+// Same shape as the count sweeps: one warp per 1,024-record chunk, rounds of 32 records.
+//   sweep 1 (WRITE = false): heads (records that differ from their predecessor) per chunk and per block
+//   scan                   : block sums -> exclusive prefix; total -> st->merge_heads
+//   sweep 2 (WRITE = true) : distinct index of a record = heads before it (inclusive) - 1; heads write their key; the
+//                            multiplicities of a run are added up inside the round by a segmented scan over the lanes,
+//                            and the last lane of a segment writes its sum into acc[distinct index]: with a plain store
+//                            when the whole run lies inside the round, with an atomic add when the run crosses a round.
+//   finish                 : acc (u64, zeroed before) saturates into out_mult (u32, reading A9).
+template <int W, bool WRITE>
+__global__ void __launch_bounds__(kCountWarps * 32) merge_chunks_kernel(MergeArgs a, DevState *st) {
+    __shared__ u32 s_heads[kCountWarps];
     const u32 tid = threadIdx.x, lane = tid & 31u, warp = tid >> 5;
-    if (tid == 0) s_tile = atomicAdd(a.ticket, 1u);
-    __syncthreads();
-    const u32 tile = s_tile;
-    const u32 ntiles = (u32)((a.n + kMergeThreads - 1) / kMergeThreads);
-    const u64 idx = (u64)tile * kMergeThreads + tid;
-    u64 key[W], prevk[W];
-    bool head = false;
-    if (idx < a.n) {
-        load_key<W>(a.keys, idx, key);
-        if (idx == 0) head = true;
-        else { load_key<W>(a.keys, idx - 1, prevk); head = key_ne<W>(key, prevk); }
-    }
-    u32 tile_heads;
-    const u32 excl = block_excl_scan<kMergeThreads, false>(head ? 1u : 0u, s_warp, tile_heads);
-    if (warp == 0) {
-        const u64 p = tile_lookback<false>(a.lookback, tile, (u64)tile_heads);
-        if (lane == 0) {
-            s_bcast = p;
-            if (tile == ntiles - 1) st->merge_heads = p + tile_heads;
+    const u32 le = lanemask_lt() | (1u << lane);
+    const u64 chunk = (u64)blockIdx.x * kCountWarps + warp;
+    const u64 c0 = chunk * kCountChunk;
+    u32 n_heads = 0;
+    u64 *block_sums = a.sums;
+    u32 *chunk_sums = reinterpret_cast<u32 *>(a.sums + gridDim.x);
+    if (c0 < a.n) {
+        const u32 rem = (a.n - c0 < (u64)kCountChunk) ? (u32)(a.n - c0) : kCountChunk;
+        u64 base = 0;                                        // heads before this chunk
+        if constexpr (WRITE) {
+            base = block_sums[blockIdx.x];
+            for (u32 w = 0; w < warp; ++w) base += chunk_sums[(u64)blockIdx.x * kCountWarps + w];
         }
-    }
-    __syncthreads();
-    if (idx < a.n) {
-        const u64 di = s_bcast + excl + (head ? 1u : 0u) - 1u;   // distinct index of this record
-        if (head) {
+        u64 carry_key[W];                                    // the record before the round's first one (lane 0 uses it)
+        const bool first_chunk = c0 == 0;
+        if (!first_chunk) load_key<W>(a.keys, c0 - 1, carry_key);
+        else {
 #pragma unroll
-            for (int q = 0; q < W; ++q) a.out_keys[di * W + q] = key[q];
+            for (int q = 0; q < W; ++q) carry_key[q] = 0;
         }
-        atomicAdd(&a.acc[di], (u64)a.mult[idx]);
+        const u32 nrounds = (rem + 31u) / 32u;
+#pragma unroll 1
+        for (u32 r = 0; r < nrounds; ++r) {
+            const u32 i = r * 32u + lane;
+            const bool valid = i < rem;
+            u64 k[W], kp[W];
+            if (valid) load_key<W>(a.keys, c0 + i, k);
+            else {
+#pragma unroll
+                for (int q = 0; q < W; ++q) k[q] = 0;
+            }
+#pragma unroll
+            for (int q = 0; q < W; ++q) {
+                const u64 up = __shfl_up_sync(0xffffffffu, k[q], 1);
+                kp[q] = lane == 0 ? carry_key[q] : up;
+            }
+            const bool head = valid && ((first_chunk && i == 0) || key_ne<W>(k, kp));
+            const u32 H = __ballot_sync(0xffffffffu, head);
+            if constexpr (!WRITE) {
+                n_heads += (u32)__popc(H);
+            } else {
+                const u32 V = __ballot_sync(0xffffffffu, valid);
+                const u64 di = base + n_heads + (u32)__popc(H & le) - 1u;   // n_heads: heads of the earlier rounds
+                if (head) {
+#pragma unroll
+                    for (int q = 0; q < W; ++q) a.out_keys[di * W + q] = k[q];
+                }
+                // inclusive sum of mult over the lanes of my segment (segments begin at heads and at lane 0)
+                u64 s = valid ? (u64)a.mult[c0 + i] : 0ull;
+#pragma unroll
+                for (int o = 1; o < 32; o <<= 1) {
+                    const u64 t = __shfl_up_sync(0xffffffffu, s, o);
+                    const u32 between = le & ~(le >> o);                  // lanes (lane-o, lane]
+                    if (lane >= (u32)o && (H & between) == 0) s += t;     // no head in between: same segment
+                }
+                // last lane of a segment: the next lane is a head, or there is no next valid lane in the round
+                const bool seg_last = valid && (lane == 31u || ((H >> (lane + 1u)) & 1u) || !((V >> (lane + 1u)) & 1u));
+                if (seg_last) {
+                    const bool whole = (H & le) != 0 && lane != 31u && ((H >> (lane + 1u)) & 1u);   // began and ended inside the round
+                    if (whole) a.acc[di] = s;
+                    else atomicAdd(&a.acc[di], s);
+                }
+                n_heads += (u32)__popc(H);
+            }
+            const u32 last = 31u;                            // the round's last record (only read by a following round: full)
+#pragma unroll
+            for (int q = 0; q < W; ++q) carry_key[q] = __shfl_sync(0xffffffffu, k[q], (int)last);
+        }
+    }
+    if constexpr (!WRITE) {
+        if (lane == 0) {
+            s_heads[warp] = n_heads;
+            chunk_sums[chunk] = n_heads;
+        }
+        __syncthreads();
+        if (tid == 0) {
+            u64 v = 0;
+#pragma unroll
+            for (int w = 0; w < kCountWarps; ++w) v += s_heads[w];
+            block_sums[blockIdx.x] = v;
+        }
     }
 }
 
@@ -395,16 +383,23 @@ __global__ void __launch_bounds__(256) merge_finish_kernel(const u64 *acc, u32 *
         out_mult[i] = acc[i] > 0xffffffffull ? 0xffffffffu : (u32)acc[i];
 }
 
-u64 merge_tile_records() { return kMergeThreads; }
+u64 merge_tile_records() { return kCountChunk; }
+
+template <int W>
+static void launch_merge_w(const MergeArgs &a, DevState *st, cudaStream_t s) {
+    const u64 chunks = (a.n + kCountChunk - 1) / kCountChunk, blocks = (chunks + kCountWarps - 1) / kCountWarps;
+    merge_chunks_kernel<W, false><<<(unsigned)blocks, kCountWarps * 32, 0, s>>>(a, st);
+    scan_tiles_kernel<<<1, 1024, 0, s>>>(a.sums, (u32)blocks, st, -1);
+    merge_chunks_kernel<W, true><<<(unsigned)blocks, kCountWarps * 32, 0, s>>>(a, st);
+}
 
 void launch_merge(const MergeArgs &a, DevState *st, cudaStream_t s) {
     if (a.n == 0) return;
-    const u64 tiles = (a.n + kMergeThreads - 1) / kMergeThreads;
     switch (a.W) {
-        case 1: merge_kernel<1><<<(unsigned)tiles, kMergeThreads, 0, s>>>(a, st); break;
-        case 2: merge_kernel<2><<<(unsigned)tiles, kMergeThreads, 0, s>>>(a, st); break;
-        case 3: merge_kernel<3><<<(unsigned)tiles, kMergeThreads, 0, s>>>(a, st); break;
-        case 4: merge_kernel<4><<<(unsigned)tiles, kMergeThreads, 0, s>>>(a, st); break;
+        case 1: launch_merge_w<1>(a, st, s); break;
+        case 2: launch_merge_w<2>(a, st, s); break;
+        case 3: launch_merge_w<3>(a, st, s); break;
+        case 4: launch_merge_w<4>(a, st, s); break;
     }
     u64 blocks = (a.n + 255) / 256;
     if (blocks > (u64)kNumSMs * 8) blocks = (u64)kNumSMs * 8;

@@ -93,7 +93,7 @@ void launch_emit(const EmitArgs &a, cudaStream_t s);
 struct MergeArgs {
     const u64 *keys; const u32 *mult; u64 n; u32 W;
     u64 *out_keys; u32 *out_mult;        // capacity n
-    u64 *lookback; u32 *ticket;          // u64[tiles], zeroed
+    u64 *sums;                           // scratch of 8 bytes per merge_tile_records() records (block and chunk sums)
     u64 *acc;                            // u64[n] scratch accumulators, zeroed
 };
 u64 merge_tile_records();

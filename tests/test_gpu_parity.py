@@ -180,3 +180,40 @@ def test_build_unsorted_equals_count(k):
     assert np.array_equal(ed.keys_np(), orc.distinct_keys)
     assert np.array_equal(ed.mult_np(), orc.distinct_cnt)
     assert np.array_equal(g.W_np(), orc.Wbyte) and np.array_equal(g.last_bits_np(), orc.last_bits)
+
+
+@pytest.mark.parametrize("k", [21, 99])
+def test_build_unsorted_many_chunks_and_long_runs(k):
+    """sdbg_build on unsorted input whose runs of equal keys cross rounds (32), chunks (1,024) and blocks (8,192):
+    raw records of a synthetic workload (every distinct key repeated by its count) plus one key repeated 20,000
+    times with large multiplicities (saturating sum, reading A9)."""
+    import torch
+    import paper_1409_7208_b200 as sd
+    from workloads import ReadGenerator, get_config
+    cfg = get_config(1, scale=0.05) if k < 99 else get_config(2, scale=0.001)
+    bases, offs = ReadGenerator(cfg).host()
+    orc = run_oracle((bases, offs), k, 1)
+    w = orc.w
+    keys = np.repeat(orc.distinct_keys, orc.distinct_cnt.astype(np.int64), axis=0)
+    mult = np.ones(len(keys), dtype=np.uint32)
+    big = orc.distinct_keys[len(orc.distinct_keys) // 2]
+    keys = np.concatenate([keys, np.repeat(big[None, :], 20000, axis=0)])
+    mult = np.concatenate([mult, np.full(20000, 300000, dtype=np.uint32)])          # 20,000 x 300,000 > 2^32
+    perm = np.random.default_rng(7 + k).permutation(len(keys))
+    keys, mult = np.ascontiguousarray(keys[perm]), np.ascontiguousarray(mult[perm])
+    n = len(keys)
+    ctx = sd.Context(sd.sdbg_min_workspace() + 64 * n * w)
+    ed = sd.Edges(n, k)
+    ed.keys[: n * w] = torch.from_numpy(keys.reshape(-1).view(np.int64)).cuda()
+    ed.mult[:n] = torch.from_numpy(mult.view(np.int32)).cuda()
+    ed.c.n = n
+    g = sd.Graph(n)
+    sd.sdbg_build(ctx, ed, 0, g)
+    torch.cuda.synchronize()
+    want = orc.distinct_cnt.astype(np.uint64)
+    want[len(orc.distinct_keys) // 2] += np.uint64(20000) * np.uint64(300000)
+    want = np.minimum(want, np.uint64(2 ** 32 - 1)).astype(np.uint32)
+    assert ed.n == orc.n_distinct == g.n
+    assert np.array_equal(ed.keys_np(), orc.distinct_keys)
+    assert np.array_equal(ed.mult_np(), want) and np.array_equal(g.mult_np(), want)
+    assert np.array_equal(g.W_np(), orc.Wbyte) and np.array_equal(g.last_bits_np(), orc.last_bits)
