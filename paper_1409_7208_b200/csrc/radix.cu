@@ -25,7 +25,7 @@ namespace sdbg {
 // The kernel is bound by instruction issue and shared-memory wavefronts at the same time,
 // so the steps are split between B and A to load both pipes equally.
 #ifndef SDBG_LB_EVERY
-#define SDBG_LB_EVERY 2      // rank steps between two look-back polls (power of two)
+#define SDBG_LB_EVERY 4      // rank steps between two look-back polls (power of two)
 #endif
 #ifndef SDBG_PERSISTENT
 #define SDBG_PERSISTENT 1    // 1: persistent CTAs holding the ticket of their next tile; 0: one tile per CTA
