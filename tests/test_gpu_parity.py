@@ -217,3 +217,72 @@ def test_build_unsorted_many_chunks_and_long_runs(k):
     assert np.array_equal(ed.keys_np(), orc.distinct_keys)
     assert np.array_equal(ed.mult_np(), want) and np.array_equal(g.mult_np(), want)
     assert np.array_equal(g.W_np(), orc.Wbyte) and np.array_equal(g.last_bits_np(), orc.last_bits)
+
+
+def test_degenerate_long_runs_poly_A():
+    """Thousands of identical reads of one letter: every record of a strand is the same key, so one run spans every
+    chunk and block of the count sweeps (32-ary run-start search), every radix tile holds one digit value per pass,
+    and the multiplicity is the whole record count. Mixed with ordinary reads so that other keys surround the runs."""
+    from workloads import ReadGenerator, get_config
+    k = 31
+    bases, offs = ReadGenerator(get_config(1, scale=0.02)).host()
+    extra = ["A" * 150] * 2500 + ["T" * 150] * 500 + ["ACGT" * 40] * 300
+    eb, eo = to_arrays(extra)
+    bases2 = np.concatenate([bases, eb])
+    offs2 = np.concatenate([offs, eo[1:] + offs[-1]])
+    orc = run_oracle((bases2, offs2), k, 2)
+    assert int(orc.mult.max()) >= 3000 * (150 - k)          # poly-A forward + poly-T reverse strand
+    import paper_1409_7208_b200 as sd
+    assert_matches_oracle(run_gpu((bases2, offs2), k, 2), orc)
+    # block-wise: the poly-A partition alone holds 357,000 records; a workspace for 400,000 forces several ranges
+    res = run_gpu((bases2, offs2), k, 2, workspace_bytes=sd.sdbg_workspace_for_records(400000, k))
+    assert res.stats.n_ranges >= 3
+    assert_matches_oracle(res, orc)
+    # and a workspace smaller than that partition is refused (reading A12)
+    with pytest.raises(sd.SdbgError) as ei:
+        run_gpu((bases2, offs2), k, 2, workspace_bytes=sd.sdbg_min_workspace())
+    assert ei.value.name == "SDBG_E_WORKSPACE" and "largest l=8 partition" in str(ei.value)
+
+
+def test_P9_reverse_complement_closure_of_the_gpu_output():
+    """Pin P9 on the CUDA path alone (no oracle involved): the solid set is closed under reverse complement and
+    cnt(e) = cnt(rc(e)); the rc of a key is recomputed here from the key's symbols."""
+    from workloads import ReadGenerator, get_config
+    for k in (21, 31, 40):
+        bases, offs = ReadGenerator(get_config(1, scale=0.05)).host()
+        res = run_gpu((bases, offs), k, 2)
+        w = res.W_words
+        vals = [int.from_bytes(b"".join(int(x).to_bytes(8, "big") for x in row), "big") for row in res.keys]
+        pad = 64 * w - 2 * (k + 1)
+        table = {}
+        for v, m in zip(vals, res.mult):
+            sym = [((v >> pad) >> (2 * (k - t))) & 3 for t in range(k + 1)]      # key symbols (e[k-1],...,e[0],e[k])
+            e = sym[:k][::-1] + [sym[k]]                                         # edge e[0..k]
+            table[tuple(e)] = int(m)
+        for e, m in table.items():
+            r = tuple(3 - x for x in reversed(e))
+            assert table.get(r) == m, (k, e)
+
+
+def test_k_schedule_on_one_resident_read_set():
+    """The multi-k loop of the paper (options --k-min 27 --k-max 87 --k-step 10 at PAPER.md:82) as far as
+    this path goes: reads are packed once and stay in HBM, sdbg_count_edges + sdbg_build run per k."""
+    import torch
+    import paper_1409_7208_b200 as sd
+    from workloads import ReadGenerator, get_config
+    cfg = get_config(2, scale=0.002)
+    bases, offs = ReadGenerator(cfg).host()
+    ctx = sd.Context(sd.sdbg_full_workspace(cfg.n_bases, 99))
+    rd = sd.Reads(cfg.n_bases)
+    sd.sdbg_pack_reads(ctx, torch.from_numpy(bases).cuda(), torch.from_numpy(offs.view(np.int64)).cuda(), cfg.n_reads, rd)
+    for k in (27, 37, 47, 57, 67, 77, 87, 99):
+        orc = run_oracle((bases, offs), k, 2)
+        ed = sd.Edges(max(orc.n_solid, 1), k)
+        st = sd.Stats(want_checksums=True)
+        sd.sdbg_count_edges(ctx, rd, cfg.n_reads, k, 2, ed, st)
+        g = sd.Graph(max(ed.n, 1))
+        sd.sdbg_build(ctx, ed, sd.SDBG_SORTED, g)
+        torch.cuda.synchronize()
+        assert ed.n == orc.n_solid and st.n_distinct == orc.n_distinct and st.csum_raw == st.csum_distinct
+        assert np.array_equal(ed.keys_np(), orc.keys) and np.array_equal(ed.mult_np(), orc.mult)
+        assert np.array_equal(g.W_np(), orc.Wbyte) and np.array_equal(g.last_bits_np(), orc.last_bits)
