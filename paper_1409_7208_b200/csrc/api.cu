@@ -109,11 +109,12 @@ u64 range_need(u64 n, u32 W) {
     const u64 rt = radix_tile_records(W, false), ct = count_tile_records(W);
     return 2 * align_up(n * K) + align_up(((n + rt - 1) / rt + 1) * kRadix * 8) + align_up(((n + ct - 1) / ct + 1) * 8);
 }
-// largest n with range_need(n) <= avail; one sort range holds fewer than 2^32 records (the look-back words of the
-// radix passes carry 32-bit counts), larger inputs are split into block-wise ranges like any input that does not fit
-constexpr u64 kMaxRangeRecords = 0xffffffffull;
+// largest n with range_need(n) <= avail; one sort range is also capped by the layout of the radix passes' look-back
+// words (radix_max_records: 2^34-1 records or 2^22 tiles); larger inputs are split into block-wise ranges like any
+// input that does not fit
+constexpr u64 kMaxRangeRecords = 0xffffffffull;   // sdbg_build's sort with payloads
 u64 range_capacity(u64 avail, u32 W) {
-    u64 lo = 0, hi = std::min<u64>(avail / (16ull * W) + 1, kMaxRangeRecords);
+    u64 lo = 0, hi = std::min<u64>(avail / (16ull * W) + 1, radix_max_records(W, false));
     while (lo < hi) {
         u64 mid = lo + (hi - lo + 1) / 2;
         if (range_need(mid, W) <= avail) lo = mid; else hi = mid - 1;

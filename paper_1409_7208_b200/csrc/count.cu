@@ -58,7 +58,7 @@ __device__ __forceinline__ bool key_lt(const u64 (&a)[W], const u64 (&b)[W]) {  
 // (one ballot, one find-leading-one) or the warp-uniform carry from the rounds before. For the run that is open at
 // the chunk's first record the start is found by looking at the records right before it, 32 at a time, and, past
 // 128 of them, by a 32-ary search for the first record equal to it (the records are sorted). So no state about runs
-// travels between warps. Indices are chunk-relative u32 (modulo 2^32: a sort range holds fewer than 2^32 records, so
+// travels between warps. Indices are chunk-relative u32 (modulo 2^32: if the range holds fewer than 2^32 records,
 // run lengths come out right even when a run began long before the chunk).
 constexpr u32 kCountChunk = 1024;        // records per warp
 constexpr int kCountWarps = 8;           // warps per block
@@ -70,15 +70,19 @@ __device__ __forceinline__ void shfl_key(u64 (&dst)[W], const u64 (&src)[W], int
     for (int q = 0; q < W; ++q) dst[q] = __shfl_sync(0xffffffffu, src[q], src_lane);
 }
 
-template <int W, bool WRITE, bool CSUM>
+// WIDE: the range holds 2^32 records or more, so a run may be that long: run starts and lengths are 64-bit and the
+// multiplicity saturates at 2^32-1 (reading A9); otherwise 32-bit modular arithmetic is exact.
+template <int W, bool WRITE, bool CSUM, bool WIDE>
 __global__ void __launch_bounds__(kCountWarps * 32, W == 1 ? 6 : W == 2 ? 4 : 2) count_chunks_kernel(CountArgs a, DevState *st) {
+    using len_t = std::conditional_t<WIDE, u64, u32>;
     constexpr int G = kCountGroup;
     __shared__ u64 s_red[3][kCountWarps];
     const u32 tid = threadIdx.x, lane = tid & 31u, warp = tid >> 5;
     const u32 lt = lanemask_lt();
     const u64 chunk = (u64)blockIdx.x * kCountWarps + warp;
     const u64 c0 = chunk * kCountChunk;                     // global index of the chunk's first record
-    u32 n_tails = 0, n_solid = 0, sum_mult = 0;             // lengths of the runs ending in one chunk add up to < 2^32
+    u32 n_tails = 0, n_solid = 0;
+    len_t sum_mult = 0;                                     // !WIDE: lengths of the runs ending in one chunk add up to < 2^32
     u64 csum = 0;
     if (c0 < a.n) {
         const u32 rem = (a.n - c0 < (u64)kCountChunk) ? (u32)(a.n - c0) : kCountChunk;   // records of this chunk
@@ -96,7 +100,7 @@ __global__ void __launch_bounds__(kCountWarps * 32, W == 1 ? 6 : W == 2 ? 4 : 2)
         load_round(0, key[0]);
 
         // ---- start of the run that is open at the chunk's first record ----------------------------------------
-        u32 carry;                                           // chunk-relative start of the run in progress
+        len_t carry;                                         // chunk-relative start of the run in progress (modular)
         {
             u64 target[W], probe[W];
             shfl_key<W>(target, key[0], 0);
@@ -129,7 +133,7 @@ __global__ void __launch_bounds__(kCountWarps * 32, W == 1 ? 6 : W == 2 ? 4 : 2)
                 }
                 hi = lo;
             }
-            carry = (u32)(hi - c0);                          // modulo 2^32 when the run began before the chunk
+            carry = (len_t)(hi - c0);                        // modular when the run began before the chunk
         }
 
         // ---- rounds --------------------------------------------------------------------------------------------
@@ -150,11 +154,11 @@ __global__ void __launch_bounds__(kCountWarps * 32, W == 1 ? 6 : W == 2 ? 4 : 2)
             if constexpr (!FULL) tail = i < rem && ((i + 1u == rem && !has_succ) || tail);
             const u32 T = __ballot_sync(0xffffffffu, tail);
             const u32 below = T & lt;
-            const u32 start = below ? r * 32u + (32u - (u32)__clz(below)) : carry;   // place after the previous tail
-            const u32 len = i + 1u - start;
-            const bool solid = tail && len >= a.d;
+            const len_t start = below ? (len_t)(r * 32u + (32u - (u32)__clz(below))) : carry;   // place after the previous tail
+            const len_t len = (len_t)(i + 1u) - start;
+            const bool solid = tail && len >= (len_t)a.d;
             const u32 S = __ballot_sync(0xffffffffu, solid);
-            if (T) carry = r * 32u + (32u - (u32)__clz(T));
+            if (T) carry = (len_t)(r * 32u + (32u - (u32)__clz(T)));
             if constexpr (!WRITE) {
                 n_tails += (u32)__popc(T);
                 n_solid += (u32)__popc(S);
@@ -166,7 +170,7 @@ __global__ void __launch_bounds__(kCountWarps * 32, W == 1 ? 6 : W == 2 ? 4 : 2)
                     if (pos < a.out_cap) {
 #pragma unroll
                         for (int q = 0; q < W; ++q) a.out_keys[pos * W + q] = k[q];
-                        a.out_mult[pos] = len;   // < 2^32 by the range bound: the saturation of A9 cannot be reached
+                        a.out_mult[pos] = (WIDE && len > (len_t)0xffffffffu) ? 0xffffffffu : (u32)len;   // A9
                     }
                 }
                 out_pos += (u32)__popc(S);
@@ -198,7 +202,8 @@ __global__ void __launch_bounds__(kCountWarps * 32, W == 1 ? 6 : W == 2 ? 4 : 2)
         // per-warp and per-block numbers of solid edges; statistics: block reduction, one atomic per block and
         // counter, spread over 32 slots
         __shared__ u32 s_solid[kCountWarps];
-        sum_mult = __reduce_add_sync(0xffffffffu, sum_mult);
+        if constexpr (WIDE) sum_mult = (len_t)warp_reduce_add64((u64)sum_mult);
+        else sum_mult = (len_t)__reduce_add_sync(0xffffffffu, (u32)sum_mult);
         if constexpr (CSUM) csum = warp_reduce_add64(csum);
         if (lane == 0) {
             s_red[0][warp] = n_tails; s_red[1][warp] = sum_mult; s_red[2][warp] = csum; s_solid[warp] = n_solid;
@@ -263,10 +268,18 @@ static int launch_count_w(const CountArgs &a, DevState *st, cudaStream_t s) {
     if (chunks == 0) return 0;
     const u64 blocks = (chunks + kCountWarps - 1) / kCountWarps;
     if (blocks > 0x7fffffffull) return (int)cudaErrorInvalidValue;
-    if (a.want_csum) count_chunks_kernel<W, false, true><<<(unsigned)blocks, kCountWarps * 32, 0, s>>>(a, st);
-    else             count_chunks_kernel<W, false, false><<<(unsigned)blocks, kCountWarps * 32, 0, s>>>(a, st);
+    const bool wide = a.n > 0xffffffffull;
+    const unsigned g = (unsigned)blocks, t = kCountWarps * 32;
+    if (wide) {
+        if (a.want_csum) count_chunks_kernel<W, false, true, true><<<g, t, 0, s>>>(a, st);
+        else             count_chunks_kernel<W, false, false, true><<<g, t, 0, s>>>(a, st);
+    } else {
+        if (a.want_csum) count_chunks_kernel<W, false, true, false><<<g, t, 0, s>>>(a, st);
+        else             count_chunks_kernel<W, false, false, false><<<g, t, 0, s>>>(a, st);
+    }
     scan_tiles_kernel<<<1, 1024, 0, s>>>(a.tile_sums, (u32)blocks, st, a.range_parity);
-    count_chunks_kernel<W, true, false><<<(unsigned)blocks, kCountWarps * 32, 0, s>>>(a, st);
+    if (wide) count_chunks_kernel<W, true, false, true><<<g, t, 0, s>>>(a, st);
+    else      count_chunks_kernel<W, true, false, false><<<g, t, 0, s>>>(a, st);
     return (int)cudaGetLastError();
 }
 

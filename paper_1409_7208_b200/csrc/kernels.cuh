@@ -65,6 +65,7 @@ struct RadixArgs {
     PassDesc pass; u32 epoch;
 };
 u64 radix_tile_records(u32 W, bool has_vals);
+u64 radix_max_records(u32 W, bool has_vals);   // cap of one sort range (look-back word layout)
 int launch_radix_pass(const RadixArgs &a, cudaStream_t s);
 int radix_setup();   // sets max dynamic shared memory attributes; once per process
 

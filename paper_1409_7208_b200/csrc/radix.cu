@@ -146,21 +146,37 @@ __device__ __forceinline__ void store_rec(u64 *__restrict__ o, const u64 (&k)[W]
 // span it covers, RE-PUBLISHES its own entry with the span it has covered so far (so later tiles jump over it in
 // one step: pointer doubling, the walk is logarithmic in the distance to the nearest GLOBAL entry instead of
 // linear), and requests the next entry. On reaching a GLOBAL entry it publishes its inclusive prefix.
-// One sort range holds fewer than 2^32 records (api.cu range_capacity), so counts fit 32 bits.
+// Two layouts of the word: ranges of fewer than 2^32 records (every benchmarked single-range config) keep 32-bit counts
+// and 32-bit arithmetic in the walker; larger ranges (block-wise passes over a big workspace) use 34-bit counts.
+template <bool WIDE> struct LbFmt;
+template <> struct LbFmt<false> {   // [63:62] status [61:54] epoch [53:32] span [31:0] count
+    using cnt_t = u32;
+    static constexpr int kEpochBits = 8, kTagShift = 54, kSpanShift = 32;
+    static constexpr u64 kCntMask = 0xffffffffull;
+};
+template <> struct LbFmt<true> {    // [63:62] status [61:56] epoch [55:34] span [33:0] count
+    using cnt_t = u64;
+    static constexpr int kEpochBits = 6, kTagShift = 56, kSpanShift = 34;
+    static constexpr u64 kCntMask = (1ull << 34) - 1ull;
+};
 constexpr u32 kSpanMask = (1u << 22) - 1u;
-__device__ __forceinline__ void lookback_poll(u64 *lb, u32 tile, u32 &t, u64 &pend, u32 &excl, bool &done, u32 real_cnt,
-                                              u32 tagL, u32 tagG) {
+constexpr u64 kMaxTilesPerRange = 1ull << 22, kMaxRecordsWide = (1ull << 34) - 1ull;
+
+template <bool WIDE>
+__device__ __forceinline__ void lookback_poll(u64 *lb, u32 tile, u32 &t, u64 &pend, typename LbFmt<WIDE>::cnt_t &excl, bool &done,
+                                              u32 real_cnt, u32 tagL, u32 tagG) {
+    using F = LbFmt<WIDE>;
     if (done) return;
-    const u32 tag = (u32)(pend >> 54);
+    const u32 tag = (u32)(pend >> F::kTagShift);
     if (tag == tagL || tag == tagG) {
-        excl += (u32)pend;
+        excl += (typename F::cnt_t)(pend & F::kCntMask);
         if (tag == tagG) {
             done = true;
-            st_relaxed(lb + (u64)tile * kRadix, ((u64)tagG << 54) | (u64)(excl + real_cnt));
+            st_relaxed(lb + (u64)tile * kRadix, ((u64)tagG << F::kTagShift) | (u64)(excl + real_cnt));
             return;
         }
-        t -= (u32)(pend >> 32) & kSpanMask;   // tile 0 always publishes GLOBAL, so t never passes it
-        st_relaxed(lb + (u64)tile * kRadix, ((u64)tagL << 54) | ((u64)(tile - t) << 32) | (u64)(excl + real_cnt));
+        t -= (u32)(pend >> F::kSpanShift) & kSpanMask;   // tile 0 always publishes GLOBAL, so t never passes it
+        st_relaxed(lb + (u64)tile * kRadix, ((u64)tagL << F::kTagShift) | ((u64)(tile - t) << F::kSpanShift) | (u64)(excl + real_cnt));
     }
     pend = ld_relaxed(lb + (u64)t * kRadix);
 }
@@ -242,10 +258,11 @@ __device__ __forceinline__ void prefetch_l2_bulk(const void *p, u32 bytes) {
 //   5 write-out: place p of the tile goes to bin_address[digit] + p, coalesced per digit run.
 // Forward progress: a CTA's current tile is always older than the ticket it holds in reserve, so the oldest
 // unfinished tile is always being worked on by a resident CTA.
-template <int W, bool HAS_VAL, bool HI>
+template <int W, bool HAS_VAL, bool HI, bool WIDE>
 __global__ void __launch_bounds__(RadixCfg<W, HAS_VAL>::THREADS, RadixCfg<W, HAS_VAL>::MINB)
 onesweep_kernel(RadixArgs a) {
     using L = RadixSmem<W, HAS_VAL>;
+    using F = LbFmt<WIDE>;
     constexpr int THREADS = L::THREADS, KPT = L::KPT, WARPS = L::WARPS, TILE = L::TILE;
     constexpr bool USE_A = L::USE_A;
     static_assert(THREADS >= kRadix, "one thread per bin");
@@ -269,7 +286,7 @@ onesweep_kernel(RadixArgs a) {
     const u32 wbase = warp * 32u * KPT + lane;
     u32 *wp = s_pos + warp * kRadix;
     u32 *wm = s_mask + warp * kRadix;
-    const u32 tagL = ((u32)kStLocal << 8) | a.epoch, tagG = ((u32)kStGlobal << 8) | a.epoch;
+    const u32 tagL = ((u32)kStLocal << F::kEpochBits) | a.epoch, tagG = ((u32)kStGlobal << F::kEpochBits) | a.epoch;
     // two roles of one thread per bin: the first 256 threads scan the histograms, the LAST 256 run the look-back,
     // so that the two chains of dependent shared / L2 round trips proceed side by side
     const bool scanner = tid < kRadix, walker = tid >= THREADS - kRadix;
@@ -316,7 +333,7 @@ onesweep_kernel(RadixArgs a) {
         for (int v = 0; v < WARPS; ++v) my_cnt += s_pos[v * kRadix + tid];
         u32 rc = my_cnt;                                                  // my_cnt includes the pads (bin 255)
         if (tid == kRadix - 1) rc -= (u32)TILE - tcnt;
-        st_relaxed(a.lookback + tid + (u64)t * kRadix, ((u64)(t == 0 ? tagG : tagL) << 54) | (t == 0 ? 0ull : 1ull << 32) | rc);
+        st_relaxed(a.lookback + tid + (u64)t * kRadix, ((u64)(t == 0 ? tagG : tagL) << F::kTagShift) | (t == 0 ? 0ull : 1ull << F::kSpanShift) | rc);
         s_real[tid] = rc;
         incl = warp_incl_scan_add(my_cnt);
         if (lane == 31) s_wtot[warp] = incl;
@@ -342,7 +359,8 @@ onesweep_kernel(RadixArgs a) {
     // tile and, in the shadow of the next tile's count and scan, until the write-out needs it. lb_t = predecessor
     // tile being examined; lb_pend = its entry as last read.
     u64 lb_pend = 0;
-    u32 lb_excl = 0, lb_t = 0, real_cnt = 0, bin_start = 0;
+    typename F::cnt_t lb_excl = 0;
+    u32 lb_t = 0, real_cnt = 0, bin_start = 0;
     bool lb_done = true;
     auto lookback_begin = [&](u32 t) {   // after the barrier that follows scan_warps of tile t
         real_cnt = s_real[wbin];
@@ -402,7 +420,7 @@ onesweep_kernel(RadixArgs a) {
             if constexpr (HAS_VAL) s_vals[pos] = val[j];
             __syncwarp();
             if ((j & (SDBG_LB_EVERY - 1)) == SDBG_LB_EVERY - 1 && walker)
-                lookback_poll(lb, tile, lb_t, lb_pend, lb_excl, lb_done, real_cnt, tagL, tagG);
+                lookback_poll<WIDE>(lb, tile, lb_t, lb_pend, lb_excl, lb_done, real_cnt, tagL, tagG);
         }
         zero_rows();   // own rows only; their last readers were the scan threads, two barriers ago
 
@@ -416,12 +434,12 @@ onesweep_kernel(RadixArgs a) {
         }
         __syncthreads();
         if (scanner && next < ntiles) scan_bins(next, cnt);
-        if (walker) lookback_poll(lb, tile, lb_t, lb_pend, lb_excl, lb_done, real_cnt, tagL, tagG);
+        if (walker) lookback_poll<WIDE>(lb, tile, lb_t, lb_pend, lb_excl, lb_done, real_cnt, tagL, tagG);
         __syncthreads();
         if (scanner && next < ntiles) scan_warps();
         if (walker) {
             // ---- 4: the look-back result is needed now -------------------------------------------------------------
-            while (!lb_done) lookback_poll(lb, tile, lb_t, lb_pend, lb_excl, lb_done, real_cnt, tagL, tagG);
+            while (!lb_done) lookback_poll<WIDE>(lb, tile, lb_t, lb_pend, lb_excl, lb_done, real_cnt, tagL, tagG);
             const u64 first = a.bin_base[wbin] + lb_excl - bin_start;   // output index of tile place 0 if it were in this bin
             s_binaddr[wbin] = reinterpret_cast<u64>(a.keys_out) + first * (8ull * W);
             if constexpr (HAS_VAL) s_valaddr[wbin] = reinterpret_cast<u64>(a.vals_out) + first * 4ull;
@@ -454,9 +472,13 @@ onesweep_kernel(RadixArgs a) {
 template <int W, bool HAS_VAL>
 static int setup_one() {
     const int bytes = (int)RadixSmem<W, HAS_VAL>::kBytes;
-    int e = (int)cudaFuncSetAttribute(onesweep_kernel<W, HAS_VAL, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
+    int e = (int)cudaFuncSetAttribute(onesweep_kernel<W, HAS_VAL, false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
     if (e) return e;
-    return (int)cudaFuncSetAttribute(onesweep_kernel<W, HAS_VAL, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
+    e = (int)cudaFuncSetAttribute(onesweep_kernel<W, HAS_VAL, true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
+    if (e || HAS_VAL) return e;   // ranges of 2^32 records and more exist only in sdbg_count_edges (keys without payload)
+    e = (int)cudaFuncSetAttribute(onesweep_kernel<W, false, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
+    if (e) return e;
+    return (int)cudaFuncSetAttribute(onesweep_kernel<W, false, true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
 }
 
 int radix_setup() {
@@ -475,6 +497,13 @@ int radix_setup() {
 template <int W, bool HAS_VAL>
 static constexpr u64 tile_of() { return (u64)RadixCfg<W, HAS_VAL>::THREADS * RadixCfg<W, HAS_VAL>::KPT; }
 
+// most records one sort may hold: 22-bit spans (tiles) and 34-bit counts in the look-back words; payloads: 32-bit counts
+u64 radix_max_records(u32 W, bool v) {
+    const u64 by_tiles = kMaxTilesPerRange * radix_tile_records(W, v);
+    const u64 by_count = v ? 0xffffffffull : kMaxRecordsWide;
+    return by_tiles < by_count ? by_tiles : by_count;
+}
+
 u64 radix_tile_records(u32 W, bool v) {
     switch (W) {
         case 1: return v ? tile_of<1, true>() : tile_of<1, false>();
@@ -489,14 +518,24 @@ template <int W, bool HAS_VAL>
 static int launch_one(const RadixArgs &a, cudaStream_t s) {
     const u64 tiles = (a.n + tile_of<W, HAS_VAL>() - 1) / tile_of<W, HAS_VAL>();
     if (tiles == 0) return 0;
-    if (tiles > 0x7fffffffull) return (int)cudaErrorInvalidValue;
+    if (tiles > kMaxTilesPerRange || a.n > kMaxRecordsWide) return (int)cudaErrorInvalidValue;   // look-back word layout
+    const bool wide = a.n > 0xffffffffull;
+    if (wide && HAS_VAL) return (int)cudaErrorInvalidValue;
     if (a.pass.bits != kRadixBits || (a.pass.shift & 7u)) return (int)cudaErrorInvalidValue;   // byte-aligned digits only
     // persistent CTAs: every SM filled to the occupancy the kernel was built for
     const u64 resident = SDBG_PERSISTENT ? (u64)kNumSMs * RadixCfg<W, HAS_VAL>::MINB : tiles;
     const unsigned g = (unsigned)(tiles < resident ? tiles : resident), t = RadixCfg<W, HAS_VAL>::THREADS;
     const size_t sm = RadixSmem<W, HAS_VAL>::kBytes;
-    if (a.pass.shift >= 32) onesweep_kernel<W, HAS_VAL, true><<<g, t, sm, s>>>(a);
-    else                    onesweep_kernel<W, HAS_VAL, false><<<g, t, sm, s>>>(a);
+    const bool hi = a.pass.shift >= 32;
+    if constexpr (!HAS_VAL) {
+        if (wide) {
+            if (hi) onesweep_kernel<W, false, true, true><<<g, t, sm, s>>>(a);
+            else    onesweep_kernel<W, false, false, true><<<g, t, sm, s>>>(a);
+            return (int)cudaGetLastError();
+        }
+    }
+    if (hi) onesweep_kernel<W, HAS_VAL, true, false><<<g, t, sm, s>>>(a);
+    else    onesweep_kernel<W, HAS_VAL, false, false><<<g, t, sm, s>>>(a);
     return (int)cudaGetLastError();
 }
 
