@@ -242,7 +242,9 @@ def run_gpu(args, w):
     peak, peak_src = _peaks()
     radix_launches = tim.launches["radix"]
     radix_ms = tim.ms["radix"] / max(radix_launches, 1)
-    algo_bytes = 2 * N * K                       # one pass reads and writes every key once
+    # algorithmic bytes of one pass as the library accounts them: one-word keys are read and
+    # written once (2 N K); multi-word keys travel as (key word, u32 index) pairs (2 N 12)
+    algo_bytes = tim.bytes["radix"] // max(radix_launches, 1)
     achieved = algo_bytes / (radix_ms * 1e-3) / 1e9 if radix_ms > 0 else 0.0
     line = {
         "metric": METRIC, "value": whole_job_value(N, world, args.steps, ms_total), "unit": UNIT, "n_gpus": world,

@@ -104,17 +104,20 @@ bool is_device_ptr(const void *p) {
 }
 
 // bytes of dynamic workspace a sort+count of n records needs (keys only)
+// records per look-back row of the sorter that handles W-word keys: the keys themselves (W = 1) or (word, index) pairs
+u64 sort_tile_records(u32 W) { return W == 1 ? radix_tile_records(1, false) : radix_tile_records(1, true); }
 u64 range_need(u64 n, u32 W) {
     const u64 K = 8ull * W;
-    const u64 rt = radix_tile_records(W, false), ct = count_tile_records(W);
-    return 2 * align_up(n * K) + align_up(((n + rt - 1) / rt + 1) * kRadix * 8) + align_up(((n + ct - 1) / ct + 1) * 8);
+    const u64 rt = sort_tile_records(W), ct = count_tile_records(W);
+    const u64 pairs = W == 1 ? 0 : 2 * align_up(n * 8) + 2 * align_up(n * 4);   // (word, index) ping-pong buffers
+    return 2 * align_up(n * K) + pairs + align_up(((n + rt - 1) / rt + 1) * kRadix * 8) + align_up(((n + ct - 1) / ct + 1) * 8);
 }
 // largest n with range_need(n) <= avail; one sort range is also capped by the layout of the radix passes' look-back
 // words (radix_max_records: 2^34-1 records or 2^22 tiles); larger inputs are split into block-wise ranges like any
 // input that does not fit
 constexpr u64 kMaxRangeRecords = 0xffffffffull;   // sdbg_build's sort with payloads
 u64 range_capacity(u64 avail, u32 W) {
-    u64 lo = 0, hi = std::min<u64>(avail / (16ull * W) + 1, radix_max_records(W, false));
+    u64 lo = 0, hi = std::min<u64>(avail / (16ull * W) + 1, W == 1 ? radix_max_records(1, false) : radix_max_records(1, true));
     while (lo < hi) {
         u64 mid = lo + (hi - lo + 1) / 2;
         if (range_need(mid, W) <= avail) lo = mid; else hi = mid - 1;

@@ -67,6 +67,9 @@ struct RadixArgs {
 u64 radix_tile_records(u32 W, bool has_vals);
 u64 radix_max_records(u32 W, bool has_vals);   // cap of one sort range (look-back word layout)
 int launch_radix_pass(const RadixArgs &a, cudaStream_t s);
+// multi-word keys (radix.cu "word-wise LSD with an index payload")
+void launch_gather_word(const u64 *recs, u32 W, u32 q, const u32 *idx_in, u64 *word_out, u32 *idx_out, u64 n, cudaStream_t s);
+void launch_gather_recs(const u64 *recs, u32 W, const u32 *idx, u64 *out, u64 n, cudaStream_t s);
 int radix_setup();   // sets max dynamic shared memory attributes; once per process
 
 // keys-only digit histograms over an existing key array (sdbg_build unsorted path)

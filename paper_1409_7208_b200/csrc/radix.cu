@@ -550,6 +550,45 @@ int launch_radix_pass(const RadixArgs &a, cudaStream_t s) {
     return (int)cudaErrorInvalidValue;
 }
 
+// ---- multi-word keys: word-wise LSD with an index payload -------------------------------------------------------------
+// Keys of W > 1 words are not moved through the passes themselves: the sorter moves (one key word, u32 record index)
+// pairs with the one-word kernel, least significant word first, and fetches the word of the next level through the
+// index; one last gather puts the whole records in order. Per record a pass then moves 2 x 12 bytes instead of
+// 2 x 8W, at the price of W + 1 gathers (32-byte sectors). Stable passes make this the same LSD sort.
+__global__ void __launch_bounds__(256) gather_word_kernel(const u64 *__restrict__ recs, u32 W, u32 q, const u32 *__restrict__ idx_in,
+                                                          u64 *__restrict__ word_out, u32 *__restrict__ idx_out, u64 n) {
+    for (u64 j = (u64)blockIdx.x * blockDim.x + threadIdx.x; j < n; j += (u64)gridDim.x * blockDim.x) {
+        const u64 i = idx_in ? (u64)idx_in[j] : j;
+        word_out[j] = __ldg(recs + i * W + q);
+        if (idx_out) idx_out[j] = (u32)i;     // first level: identity
+    }
+}
+template <int W>
+__global__ void __launch_bounds__(256) gather_recs_kernel(const u64 *__restrict__ recs, const u32 *__restrict__ idx, u64 *__restrict__ out, u64 n) {
+    for (u64 j = (u64)blockIdx.x * blockDim.x + threadIdx.x; j < n; j += (u64)gridDim.x * blockDim.x) {
+        u64 k[W];
+        load_rec<W>(recs + (u64)idx[j] * W, k);
+        store_rec<W>(out + j * W, k);
+    }
+}
+static unsigned gather_blocks(u64 n) {
+    u64 b = (n + 255) / 256;
+    const u64 cap = (u64)kNumSMs * 16;
+    return (unsigned)(b < cap ? b : cap);
+}
+void launch_gather_word(const u64 *recs, u32 W, u32 q, const u32 *idx_in, u64 *word_out, u32 *idx_out, u64 n, cudaStream_t s) {
+    if (n) gather_word_kernel<<<gather_blocks(n), 256, 0, s>>>(recs, W, q, idx_in, word_out, idx_out, n);
+}
+void launch_gather_recs(const u64 *recs, u32 W, const u32 *idx, u64 *out, u64 n, cudaStream_t s) {
+    if (!n) return;
+    switch (W) {
+        case 2: gather_recs_kernel<2><<<gather_blocks(n), 256, 0, s>>>(recs, idx, out, n); break;
+        case 3: gather_recs_kernel<3><<<gather_blocks(n), 256, 0, s>>>(recs, idx, out, n); break;
+        case 4: gather_recs_kernel<4><<<gather_blocks(n), 256, 0, s>>>(recs, idx, out, n); break;
+        default: gather_recs_kernel<1><<<gather_blocks(n), 256, 0, s>>>(recs, idx, out, n); break;
+    }
+}
+
 // ---- histogram helpers ------------------------------------------------------------------------------------------
 
 // in-place exclusive scan of each pass's 256 u64 bins; one block per pass
