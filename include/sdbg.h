@@ -57,7 +57,10 @@ typedef struct sdbg_ctx sdbg_ctx;
 
 /* Binds a device, a CUDA stream (cudaStream_t passed as void*, NULL = legacy default stream) and a caller-owned
  * device workspace. The workspace plays the role of MEGAHIT's "-m" memory budget: the sorter
- * sizes its block-wise passes to it. workspace must be 256-byte aligned. */
+ * sizes its block-wise passes to it. workspace must be 256-byte aligned.
+ * Test hook: with SDBG_FORCE_WIDE=1 in the environment when the context is created, one-word-key ranges of any size
+ * take the code path of ranges of 2^32 records and more (wide look-back words in the radix passes, 64-bit run lengths
+ * in the count sweeps), which otherwise only very large block-wise runs reach. Results are identical. */
 int sdbg_ctx_create(sdbg_ctx **ctx, int device, void *cuda_stream, void *workspace, uint64_t workspace_bytes);
 void sdbg_ctx_destroy(sdbg_ctx *ctx);
 const char *sdbg_strerror(int status);           /* static string */

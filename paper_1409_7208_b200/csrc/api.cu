@@ -6,6 +6,7 @@
 
 #include <algorithm>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <string>
 #include <vector>
@@ -39,6 +40,7 @@ struct sdbg_ctx {
     u64 ws_bytes = 0;
     std::string err;
     bool timing = false;
+    bool force_wide = false;   // SDBG_FORCE_WIDE=1 in the environment at sdbg_ctx_create: see include/sdbg.h
     std::vector<EventPair> pending;
     std::vector<cudaEvent_t> free_events;
     sdbg_timing acc{};
@@ -158,6 +160,8 @@ int sdbg_ctx_create(sdbg_ctx **out, int device, void *cuda_stream, void *workspa
     c->stream = (cudaStream_t)cuda_stream;
     c->ws = (char *)workspace;
     c->ws_bytes = workspace_bytes;
+    const char *fw = getenv("SDBG_FORCE_WIDE");
+    c->force_wide = fw && fw[0] == '1';
     *out = c;
     return SDBG_OK;
 }

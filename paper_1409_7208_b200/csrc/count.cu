@@ -268,7 +268,7 @@ static int launch_count_w(const CountArgs &a, DevState *st, cudaStream_t s) {
     if (chunks == 0) return 0;
     const u64 blocks = (chunks + kCountWarps - 1) / kCountWarps;
     if (blocks > 0x7fffffffull) return (int)cudaErrorInvalidValue;
-    const bool wide = a.n > 0xffffffffull;
+    const bool wide = a.n > 0xffffffffull || a.force_wide;
     const unsigned g = (unsigned)blocks, t = kCountWarps * 32;
     if (wide) {
         if (a.want_csum) count_chunks_kernel<W, false, true, true><<<g, t, 0, s>>>(a, st);

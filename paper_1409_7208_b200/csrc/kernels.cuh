@@ -63,6 +63,7 @@ struct RadixArgs {
     u64 *lookback;                       // u64[tiles*256], zeroed once per sort; epoch-tagged per pass
     u32 *ticket;                         // zeroed
     PassDesc pass; u32 epoch;
+    bool force_wide;                     // use the layout for ranges of 2^32 records and more whatever n is (tests)
 };
 u64 radix_tile_records(u32 W, bool has_vals);
 u64 radix_max_records(u32 W, bool has_vals);   // cap of one sort range (look-back word layout)
@@ -82,6 +83,7 @@ struct CountArgs {
                              // edges, then their exclusive prefix), behind them u32 per warp chunk
     u64 *stat_slots;         // u64[kStatSlots][kStatSlotWords], accumulated
     int want_csum;
+    bool force_wide;         // 64-bit run lengths whatever n is (tests)
     int range_parity;        // reads st->out_cursor[parity], writes st->out_cursor[parity^1]
 };
 u64 count_tile_records(u32 W);

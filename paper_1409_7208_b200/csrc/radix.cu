@@ -519,7 +519,7 @@ static int launch_one(const RadixArgs &a, cudaStream_t s) {
     const u64 tiles = (a.n + tile_of<W, HAS_VAL>() - 1) / tile_of<W, HAS_VAL>();
     if (tiles == 0) return 0;
     if (tiles > kMaxTilesPerRange || a.n > kMaxRecordsWide) return (int)cudaErrorInvalidValue;   // look-back word layout
-    const bool wide = a.n > 0xffffffffull;
+    const bool wide = a.n > 0xffffffffull || (a.force_wide && !HAS_VAL);
     if (wide && HAS_VAL) return (int)cudaErrorInvalidValue;
     if (a.pass.bits != kRadixBits || (a.pass.shift & 7u)) return (int)cudaErrorInvalidValue;   // byte-aligned digits only
     // persistent CTAs: every SM filled to the occupancy the kernel was built for

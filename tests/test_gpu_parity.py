@@ -286,3 +286,16 @@ def test_k_schedule_on_one_resident_read_set():
         assert ed.n == orc.n_solid and st.n_distinct == orc.n_distinct and st.csum_raw == st.csum_distinct
         assert np.array_equal(ed.keys_np(), orc.keys) and np.array_equal(ed.mult_np(), orc.mult)
         assert np.array_equal(g.W_np(), orc.Wbyte) and np.array_equal(g.last_bits_np(), orc.last_bits)
+
+
+def test_wide_range_code_path_at_small_size(monkeypatch):
+    """Ranges of 2^32 records and more use other kernels (wide look-back words, 64-bit run lengths); SDBG_FORCE_WIDE=1
+    sends small inputs down that path (include/sdbg.h), so that it is covered here and not only by config 5."""
+    from workloads import ReadGenerator, get_config
+    monkeypatch.setenv("SDBG_FORCE_WIDE", "1")
+    import paper_1409_7208_b200 as sd
+    for k, scale in ((21, 0.3), (31, 0.1)):
+        bases, offs = ReadGenerator(get_config(1, scale=scale)).host()
+        orc = run_oracle((bases, offs), k, 2)
+        assert_matches_oracle(run_gpu((bases, offs), k, 2), orc)
+        assert_matches_oracle(run_gpu((bases, offs), k, 2, workspace_bytes=sd.sdbg_min_workspace()), orc)
