@@ -236,3 +236,93 @@ void orc_encode_graph(const orc *o, uint8_t *Wbyte, uint64_t *last_bits) {
         if (o->last[i]) last_bits[i / 64] |= 1ull << (i % 64);
     }
 }
+
+/* ---- the lossless extras of PAPER.md:31 (readings A18-A20 in DESIGN.md) -------------------------
+ * "a bit-vector of length m to mark the validity of each edge ... and an auxiliary vector of 2kt bits (where k is the
+ * k-mer size and t is the number of zero-indegree vertices) to store the sequence of zero-indegree vertices to ensure
+ * the graph being lossless"; outgoing `$` edges as in Bowe et al..
+ *   nodes: src(e) = e[0..k), tgt(e) = e[1..k] over the solid edges S.
+ *   Z_out = tgt(S) \ src(S): nodes without an outgoing edge; each gets the dummy edge (v, '$').
+ *   Z_in  = src(S) \ tgt(S): nodes without an incoming edge; their k-mers, in colex order of the node, are the
+ *           auxiliary vector (t = |Z_in|); no incoming dummy edges are made (the vector stands in for them).
+ *   F = S + dummies, sorted by (colex of the node, outgoing symbol) with '$' < A < C < G < T.
+ *   Over F, by the rules of step 5 applied literally: W (0 for '$'), last, minus ('$' edges never carry it), mult
+ *   (0 for dummies); validity = all ones. */
+typedef struct orc_full {
+    uint64_t m, t, n_zero_out;
+    char *F;            /* m edges, k+1 chars, '$' as the outgoing symbol of a dummy */
+    uint8_t *W, *last;  /* W: 0 for '$', else 1 + code, + 4 with the minus flag */
+    uint32_t *mult;
+    char *aux;          /* t nodes, k chars each, sequence order v[0..k) */
+} orc_full;
+
+static uint32_t g_kcmp;   /* length for cmp_kmers (qsort has no context argument in C11) */
+static int cmp_kmers(const void *pa, const void *pb) {   /* colex: last character first */
+    const char *a = (const char *)pa, *b = (const char *)pb;
+    for (uint32_t t = g_kcmp; t-- > 0;) if (a[t] != b[t]) return a[t] < b[t] ? -1 : 1;
+    return 0;
+}
+static uint64_t uniq_kmers(char *a, uint64_t n, uint32_t k) {
+    uint64_t m = 0;
+    for (uint64_t i = 0; i < n; ++i) if (i == 0 || memcmp(a + i * k, a + (m - 1) * k, k) != 0) { memmove(a + m * k, a + i * k, k); ++m; }
+    return m;
+}
+static int sym_rank(char c) { return c == '$' ? 0 : c == 'A' ? 1 : c == 'C' ? 2 : c == 'G' ? 3 : 4; }
+
+orc_full *orc_full_graph(const orc *o) {
+    const uint32_t k = o->k, R = k + 1;
+    const uint64_t ns = o->n_solid;
+    orc_full *f = (orc_full *)calloc(1, sizeof(orc_full));
+    char *src = (char *)malloc(ns * k + 1), *tgt = (char *)malloc(ns * k + 1);
+    if (!f || !src || !tgt) return NULL;
+    for (uint64_t i = 0; i < ns; ++i) { memcpy(src + i * k, o->S + i * R, k); memcpy(tgt + i * k, o->S + i * R + 1, k); }
+    g_kcmp = k;
+    qsort(src, ns, k, cmp_kmers); qsort(tgt, ns, k, cmp_kmers);
+    const uint64_t nsrc = uniq_kmers(src, ns, k), ntgt = uniq_kmers(tgt, ns, k);
+    /* set differences of two colex-sorted lists */
+    char *zout = (char *)malloc(ntgt * k + 1), *zin = (char *)malloc(nsrc * k + 1);
+    uint64_t nzo = 0, nzi = 0, a = 0, b = 0;
+    while (a < nsrc || b < ntgt) {
+        int c = a == nsrc ? 1 : b == ntgt ? -1 : cmp_kmers(src + a * k, tgt + b * k);
+        if (c < 0) { memcpy(zin + nzi++ * k, src + a++ * k, k); }
+        else if (c > 0) { memcpy(zout + nzo++ * k, tgt + b++ * k, k); }
+        else { ++a; ++b; }
+    }
+    f->t = nzi; f->n_zero_out = nzo; f->aux = zin; f->m = ns + nzo;
+    /* F: merge S (sorted by node, then symbol) with the dummies (sorted by node) */
+    f->F = (char *)malloc(f->m * R + 1); f->mult = (uint32_t *)malloc(f->m * 4 + 4);
+    f->W = (uint8_t *)malloc(f->m + 1); f->last = (uint8_t *)malloc(f->m + 1);
+    uint64_t i = 0, j = 0, p = 0;
+    while (i < ns || j < nzo) {
+        int take_dummy;
+        if (i == ns) take_dummy = 1;
+        else if (j == nzo) take_dummy = 0;
+        else { int c = cmp_kmers(zout + j * k, o->S + i * R); take_dummy = c <= 0; }   /* equal node: '$' first */
+        if (take_dummy) { memcpy(f->F + p * R, zout + j * k, k); f->F[p * R + k] = '$'; f->mult[p] = 0; ++j; }
+        else { memcpy(f->F + p * R, o->S + i * R, R); f->mult[p] = o->mult[i]; ++i; }
+        ++p;
+    }
+    for (uint64_t q = 0; q < f->m; ++q) {   /* step 5 on F, literally */
+        const char *e = f->F + q * R;
+        f->last[q] = (q == f->m - 1) || memcmp(f->F + (q + 1) * R, e, k) != 0;
+        uint8_t minus = 0;
+        if (e[k] != '$')
+            for (uint64_t r = q; r-- > 0;) {
+                const char *g = f->F + r * R;
+                if (memcmp(g + 1, e + 1, k - 1) != 0) break;
+                if (g[k] == e[k]) { minus = 1; break; }
+            }
+        f->W[q] = (uint8_t)(e[k] == '$' ? 0 : sym_rank(e[k]) + (minus ? 4 : 0));
+    }
+    free(src); free(tgt); free(zout);
+    return f;
+}
+void orc_full_free(orc_full *f) { if (f) { free(f->F); free(f->W); free(f->last); free(f->mult); free(f->aux); free(f); } }
+uint64_t orc_full_m(const orc_full *f) { return f->m; }
+uint64_t orc_full_t(const orc_full *f) { return f->t; }
+uint64_t orc_full_n_zero_out(const orc_full *f) { return f->n_zero_out; }
+const char *orc_full_edges(const orc_full *f) { return f->F; }
+const uint8_t *orc_full_W(const orc_full *f) { return f->W; }
+const uint8_t *orc_full_last(const orc_full *f) { return f->last; }
+const uint32_t *orc_full_mult(const orc_full *f) { return f->mult; }
+const char *orc_full_aux(const orc_full *f) { return f->aux; }

@@ -38,6 +38,12 @@ def _load():
             getattr(L, "orc_" + f).argtypes = [vp]; getattr(L, "orc_" + f).restype = vp
         L.orc_encode_keys.argtypes = [vp, vp, u64, vp]; L.orc_encode_keys.restype = None
         L.orc_encode_graph.argtypes = [vp, vp, vp]; L.orc_encode_graph.restype = None
+        L.orc_full_graph.argtypes = [vp]; L.orc_full_graph.restype = vp
+        L.orc_full_free.argtypes = [vp]; L.orc_full_free.restype = None
+        for f in ("m", "t", "n_zero_out"):
+            getattr(L, "orc_full_" + f).argtypes = [vp]; getattr(L, "orc_full_" + f).restype = u64
+        for f in ("edges", "W", "last", "mult", "aux"):
+            getattr(L, "orc_full_" + f).argtypes = [vp]; getattr(L, "orc_full_" + f).restype = vp
         _lib = L
     return _lib
 
@@ -142,6 +148,39 @@ class Oracle:
             mult=_copy(L.orc_mult(h), ns, np.uint32), W=_copy(L.orc_W(h), ns, np.uint8),
             last=_copy(L.orc_last(h), ns, np.uint8), minus=_copy(L.orc_minus(h), ns, np.uint8),
             keys=keys.reshape(-1, w), distinct_keys=dkeys.reshape(-1, w), Wbyte=Wb, last_bits=lb)
+
+    def full_graph(self) -> dict:
+        """The lossless extras of PAPER.md:31 over the solid edges (call after finish): see sdbg_oracle.c.
+        Returns m, t, n_zero_out, edges (m, k+1) letters with '$', W bytes, last 0/1, mult, aux (t, k) letters, and the
+        encodings compared with the CUDA library: last_bits (LSB first), valid_bits (all ones), aux_bits (2 bits per
+        base A0 C1 G2 T3, node i at stream bits [2k i, 2k (i+1)), stream bit 0 = most significant bit of word 0)."""
+        L = _load()
+        f = L.orc_full_graph(self._h)
+        if not f:
+            raise MemoryError("oracle: full graph")
+        try:
+            k, m, t = self.k, L.orc_full_m(f), L.orc_full_t(f)
+            out = dict(m=m, t=t, n_zero_out=L.orc_full_n_zero_out(f),
+                       edges=_copy(L.orc_full_edges(f), m * (k + 1), np.uint8).reshape(-1, k + 1),
+                       W=_copy(L.orc_full_W(f), m, np.uint8), last=_copy(L.orc_full_last(f), m, np.uint8),
+                       mult=_copy(L.orc_full_mult(f), m, np.uint32), aux=_copy(L.orc_full_aux(f), t * k, np.uint8).reshape(-1, k))
+        finally:
+            L.orc_full_free(f)
+        lb = np.zeros((m + 63) // 64, dtype=np.uint64)
+        vb = np.zeros((m + 63) // 64, dtype=np.uint64)
+        for i in range(m):       # plain loops: this is the definition of the packing
+            if out["last"][i]:
+                lb[i // 64] |= np.uint64(1) << np.uint64(i % 64)
+            vb[i // 64] |= np.uint64(1) << np.uint64(i % 64)
+        code = {65: 0, 67: 1, 71: 2, 84: 3}
+        ab = np.zeros((2 * k * t + 63) // 64, dtype=np.uint64)
+        pos = 0
+        for row in out["aux"]:
+            for ch in row:
+                ab[pos // 64] |= np.uint64(code[int(ch)]) << np.uint64(62 - pos % 64)
+                pos += 2
+        out.update(last_bits=lb, valid_bits=vb, aux_bits=ab)
+        return out
 
     def close(self):
         if self._h:

@@ -96,3 +96,22 @@ def key_mix_np(keys):
             z = (z ^ (z >> np.uint64(27))) * np.uint64(_M2)
             h = z ^ (z >> np.uint64(31))
     return h
+
+
+def brute_force_full(reads, k, d):
+    """The lossless extras of PAPER.md:31 (readings A18-A20) from brute_force(): sets and sorted() only."""
+    b = brute_force(reads, k, d)
+    S = b["solid"]
+    src, tgt = {e[:k] for e in S}, {e[1:] for e in S}
+    order = {"$": 0, "A": 1, "C": 2, "G": 3, "T": 4}
+    zout = sorted(tgt - src, key=lambda v: v[::-1])
+    zin = sorted(src - tgt, key=lambda v: v[::-1])
+    F = sorted(S + [v + "$" for v in zout], key=lambda e: (e[:k][::-1], order[e[k]]))
+    mult = dict(zip(S, b["mult"]))
+    W, last, M = [], [], []
+    for i, e in enumerate(F):
+        last.append(1 if (i == len(F) - 1 or F[i + 1][:k] != e[:k]) else 0)
+        minus = e[k] != "$" and any(F[j][1:k] == e[1:k] and F[j][k] == e[k] for j in range(i))
+        W.append(0 if e[k] == "$" else order[e[k]] + (4 if minus else 0))
+        M.append(mult.get(e, 0))
+    return dict(F=F, W=W, last=last, mult=M, aux=zin, zout=zout)

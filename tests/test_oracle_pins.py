@@ -242,3 +242,75 @@ def test_several_partitions_and_split_scans_match_the_full_run():
     res = parent.finish()
     assert res.solid_strings() == multi.solid_strings() and np.array_equal(res.mult, multi.mult)
     assert np.array_equal(res.keys, multi.keys) and np.array_equal(res.last_bits, multi.last_bits)
+
+
+# ---- the lossless extras of PAPER.md:31 (Oracle.full_graph; readings A18-A20) -----------------------------------------------
+
+def _full(reads, k, d):
+    from oracle import Oracle
+    from oracle.sdbg_oracle import reads_to_arrays
+    o = Oracle(k, d)
+    o.add_reads(*reads_to_arrays(list(reads)))
+    res = o.finish()
+    f = o.full_graph()
+    o.close()
+    return res, f
+
+
+def test_full_graph_closed_form_of_a_simple_path():
+    """One read without repeated k-mers, given twice (d=2): the graph is two disjoint paths (the read and its reverse
+    complement), so exactly their last k-mers lack an outgoing edge and their first k-mers an incoming one."""
+    from tests.helpers import rc
+    r, k = "ACGGATTCAGCA", 4
+    res, f = _full([r, r], k, 2)
+    assert res.n_solid == 2 * (len(r) - k) and f["t"] == 2 and f["n_zero_out"] == 2 and f["m"] == res.n_solid + 2
+    aux = sorted(bytes(a).decode() for a in f["aux"])
+    assert aux == sorted([r[:k], rc(r)[:k]])
+    dummies = sorted(bytes(e[:k]).decode() for e in f["edges"] if e[k] == ord("$"))
+    assert dummies == sorted([r[-k:], rc(r)[-k:]])
+    for e, w, l, m in zip(f["edges"], f["W"], f["last"], f["mult"]):
+        if e[k] == ord("$"):
+            assert w == 0 and l == 1 and m == 0
+        else:
+            assert m == 2 and 1 <= w <= 8
+    # aux packing: 2k bits per node, first base in the most significant bits
+    first = bytes(f["aux"][0]).decode()
+    v = 0
+    for c in first:
+        v = (v << 2) | "ACGT".index(c)
+    assert int(f["aux_bits"][0]) >> (64 - 2 * k) == v
+
+
+def test_full_graph_of_the_complete_de_bruijn_graph_has_no_dummies():
+    from tests.helpers import de_bruijn
+    for k in (2, 3):
+        res, f = _full([de_bruijn("ACGT", k + 1)], k, 2)
+        assert f["t"] == 0 and f["n_zero_out"] == 0 and f["m"] == res.n_solid == 4 ** (k + 1)
+        assert np.array_equal(f["W"], res.Wbyte) and np.array_equal(f["last"], res.last) and np.array_equal(f["mult"], res.mult)
+
+
+@pytest.mark.parametrize("k", [2, 3, 5, 8, 11])
+def test_full_graph_bruteforce_and_strand_symmetry(k):
+    """Independent brute force (sets, sorted()) and the invariant that follows from taking both strands: the reverse
+    complement of a node without outgoing edge is a node without incoming edge, so t = number of '$' edges."""
+    import random
+    from tests.helpers import brute_force_full, rc
+    rng = random.Random(77 + k)
+    for trial in range(6):
+        src = ["".join(rng.choice("ACGT") for _ in range(rng.randint(k + 1, k + 40))) for _ in range(3)]
+        reads = []
+        for _ in range(25):
+            s = rng.choice(src)
+            a = rng.randint(0, len(s)); b = rng.randint(a, len(s))
+            reads.append(s[a:b] if rng.random() < 0.6 else rc(s[a:b]))
+        for d in (1, 2):
+            res, f = _full(reads, k, d)
+            bf = brute_force_full(reads, k, d)
+            assert [bytes(e).decode() for e in f["edges"]] == bf["F"]
+            assert list(f["W"]) == bf["W"] and list(f["last"]) == bf["last"] and list(f["mult"]) == bf["mult"]
+            assert [bytes(a).decode() for a in f["aux"]] == bf["aux"]
+            assert f["t"] == f["n_zero_out"] == len(bf["zout"])
+            assert sorted(rc(v) for v in bf["zout"]) == sorted(bf["aux"])
+            # the dummies change no flag of a real edge
+            real = [i for i, e in enumerate(f["edges"]) if e[k] != ord("$")]
+            assert np.array_equal(f["W"][real], res.Wbyte) and np.array_equal(f["last"][real], res.last)
