@@ -172,6 +172,36 @@ typedef struct {
  * synchronises. Errors: SDBG_E_CAPACITY (out->n = needed), SDBG_E_WORKSPACE, SDBG_E_INVAL. */
 int sdbg_build(sdbg_ctx *ctx, sdbg_edges *edges, uint32_t flags, sdbg_graph *out);
 
+/* ---- lossless extras of the SdBG ------------------------------------------ */
+
+typedef struct {
+    uint8_t *W;            /* m bytes: 0 = '$' (dummy outgoing edge), 1..4 = A,C,G,T, +4 with the minus flag */
+    uint64_t *last_bits;   /* ceil(cap/64) u64, LSB first, tail bits zero */
+    uint64_t *valid_bits;  /* ceil(cap/64) u64: the validity bit-vector of PAPER.md:31, all ones for the m edges */
+    uint32_t *mult;        /* m multiplicities, 0 for '$' edges */
+    uint64_t *aux_bits;    /* the "auxiliary vector of 2kt bits": ceil(2*k*aux_cap/64) u64 */
+    uint64_t cap;          /* capacity in edges of W / last_bits / valid_bits / mult */
+    uint64_t aux_cap;      /* capacity in nodes of aux_bits */
+    uint64_t m;            /* out: edges = solid edges + '$' edges */
+    uint64_t t;            /* out: zero-indegree nodes */
+    uint64_t n_zero_out;   /* out: '$' edges = nodes without outgoing edge */
+} sdbg_full_graph;
+
+/* "Our implementation has added a bit-vector of length m to mark the validity of each edge ... and an auxiliary vector
+ * of 2kt bits (where k is the k-mer size and t is the number of zero-indegree vertices) to store the sequence of
+ * zero-indegree vertices to ensure the graph being lossless". Readings A18-A20 of DESIGN.md:
+ *   - nodes: src(e) = e[0..k), tgt(e) = e[1..k] over the given edges;
+ *   - every node of tgt \ src (no outgoing edge) gets the dummy edge (node, '$') as in Bowe et al.;
+ *   - the nodes of src \ tgt (no incoming edge), in colex order, are the auxiliary vector: node i occupies stream
+ *     bits [2k i, 2k (i+1)), bases in sequence order v[0..k) at 2 bits each, stream bit 0 = most significant bit of
+ *     aux_bits[0]; no incoming dummy edges are made;
+ *   - the arrays list solid and '$' edges together, sorted by (colex of the node, outgoing symbol), '$' < A;
+ *     W / last / minus by the rules of sdbg_build ('$' edges: W = 0, last = 1, mult = 0); valid_bits = m ones.
+ * `edges` must be sorted and distinct (the output of sdbg_count_edges), 2 <= k <= 127, fewer than 2^32 edges.
+ * Synchronises the stream. Errors: SDBG_E_CAPACITY (out->m / out->t hold the needed values), SDBG_E_WORKSPACE
+ * (needs about 40 + 16 w bytes of workspace per edge), SDBG_E_UNSUPPORTED, SDBG_E_INVAL. */
+int sdbg_build_full(sdbg_ctx *ctx, const sdbg_edges *edges, sdbg_full_graph *out);
+
 /* ---- measurement hooks ---------------------------------------------------------------------------------- */
 
 enum { SDBG_T_PACK = 0, SDBG_T_EXTRACT = 1, SDBG_T_RADIX = 2, SDBG_T_COUNT = 3, SDBG_T_EMIT = 4, SDBG_T_OTHER = 5, SDBG_T_NUM = 6 };

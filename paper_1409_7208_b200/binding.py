@@ -50,6 +50,12 @@ class _Graph(C.Structure):
     _fields_ = [("W", C.c_void_p), ("last_bits", C.c_void_p), ("mult", C.c_void_p), ("cap", C.c_uint64), ("n", C.c_uint64)]
 
 
+class _FullGraph(C.Structure):
+    _fields_ = [("W", C.c_void_p), ("last_bits", C.c_void_p), ("valid_bits", C.c_void_p), ("mult", C.c_void_p),
+                ("aux_bits", C.c_void_p), ("cap", C.c_uint64), ("aux_cap", C.c_uint64), ("m", C.c_uint64),
+                ("t", C.c_uint64), ("n_zero_out", C.c_uint64)]
+
+
 class _Timing(C.Structure):
     _fields_ = [("ms", C.c_double * 6), ("launches", C.c_uint64 * 6), ("bytes", C.c_uint64 * 6)]
 
@@ -81,6 +87,7 @@ def lib():
         L.sdbg_count_edges.restype = i32
         L.sdbg_plan_ranges.argtypes = [vp, u64, vp, u64]; L.sdbg_plan_ranges.restype = C.c_int64
         L.sdbg_build.argtypes = [vp, C.POINTER(_Edges), u32, C.POINTER(_Graph)]; L.sdbg_build.restype = i32
+        L.sdbg_build_full.argtypes = [vp, C.POINTER(_Edges), C.POINTER(_FullGraph)]; L.sdbg_build_full.restype = i32
         L.sdbg_ctx_set_timing.argtypes = [vp, i32]; L.sdbg_ctx_set_timing.restype = i32
         L.sdbg_ctx_get_timing.argtypes = [vp, C.POINTER(_Timing)]; L.sdbg_ctx_get_timing.restype = i32
         _lib = L
@@ -233,6 +240,41 @@ class Graph:
         return self.mult[: self.n].cpu().numpy().view(np.uint32)
 
 
+class FullGraph:
+    """Device buffers of sdbg_full_graph: cap edges, aux_cap zero-indegree nodes of k bases."""
+
+    def __init__(self, cap: int, aux_cap: int, k: int, device=None):
+        torch = _torch()
+        dev = device or "cuda"
+        self.k = k
+        self.W = torch.empty(max(cap, 1), dtype=torch.uint8, device=dev)
+        self.last_bits = torch.empty((max(cap, 1) + 63) // 64, dtype=torch.int64, device=dev)
+        self.valid_bits = torch.empty((max(cap, 1) + 63) // 64, dtype=torch.int64, device=dev)
+        self.mult = torch.empty(max(cap, 1), dtype=torch.int32, device=dev)
+        self.aux_bits = torch.empty((2 * k * max(aux_cap, 1) + 63) // 64, dtype=torch.int64, device=dev)
+        self.c = _FullGraph(self.W.data_ptr(), self.last_bits.data_ptr(), self.valid_bits.data_ptr(), self.mult.data_ptr(),
+                            self.aux_bits.data_ptr(), cap, aux_cap, 0, 0, 0)
+
+    m = property(lambda self: self.c.m)
+    t = property(lambda self: self.c.t)
+    n_zero_out = property(lambda self: self.c.n_zero_out)
+
+    def W_np(self):
+        return self.W[: self.m].cpu().numpy()
+
+    def mult_np(self):
+        return self.mult[: self.m].cpu().numpy().view(np.uint32)
+
+    def last_bits_np(self):
+        return self.last_bits[: (self.m + 63) // 64].cpu().numpy().view(np.uint64)
+
+    def valid_bits_np(self):
+        return self.valid_bits[: (self.m + 63) // 64].cpu().numpy().view(np.uint64)
+
+    def aux_bits_np(self):
+        return self.aux_bits[: (2 * self.k * self.t + 63) // 64].cpu().numpy().view(np.uint64)
+
+
 class Stats:
     def __init__(self, want_checksums: bool = False, want_bucket_hist: bool = False):
         self.c = _Stats()
@@ -265,6 +307,11 @@ def sdbg_count_edges(ctx: Context, reads: Reads, n: int, k: int, d: int, out: Ed
     rc = lib().sdbg_count_edges(ctx._h, C.byref(reads.c), n, k, d, C.byref(out.c), C.byref(stats.c) if stats else None)
     ctx.check(rc)
     return out.c.n
+
+
+def sdbg_build_full(ctx: Context, edges: Edges, out: FullGraph) -> int:
+    ctx.check(lib().sdbg_build_full(ctx._h, C.byref(edges.c), C.byref(out.c)))
+    return out.c.m
 
 
 def sdbg_build(ctx: Context, edges: Edges, flags: int, out: Graph) -> int:

@@ -95,6 +95,22 @@ struct EmitArgs {
 };
 void launch_emit(const EmitArgs &a, cudaStream_t s);
 
+// lossless extras (dummies.cu): `$` edges, zero-indegree vector, validity bits
+struct FullArgs {
+    const u64 *keys; const u32 *mult_in; u64 n; u32 k;     // sorted solid edges
+    const uint8_t *W_real; const u32 *last_real32;         // their emitted arrays
+    const u64 *tk;                                         // sorted target node keys (WT words each)
+    const u32 *zout_idx; u64 n_zero_out;                   // indices into tk of the nodes without outgoing edge
+    const u32 *zin_idx; u64 t;                             // indices of edges whose node has no incoming edge
+    uint8_t *out_W; u32 *out_last32; u64 *out_valid; u32 *out_mult; u64 *aux_bits;
+};
+int launch_target_keys(const u64 *keys, u64 n, u32 k, u32 W, u32 WT, u64 *out, cudaStream_t s);
+int launch_zero_flags(const u64 *keys, u64 n, u32 k, u32 W, u32 WT, const u64 *tk_sorted, const u32 *last_real32,
+                      uint8_t *flag_out, uint8_t *flag_in, cudaStream_t s);
+u64 flag_scratch_bytes(u64 n);
+void launch_compact_flags(const uint8_t *flag, u64 n, u64 *scratch, u32 *out_idx, u64 *total_out, cudaStream_t s);
+int launch_full_assemble(const FullArgs &a, u32 W, u32 WT, cudaStream_t s);
+
 // sdbg_build unsorted path: merge equal adjacent keys of a sorted (key, mult) list, summing mult (saturating).
 struct MergeArgs {
     const u64 *keys; const u32 *mult; u64 n; u32 W;
