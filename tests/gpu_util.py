@@ -219,6 +219,40 @@ def check_global_invariants(res, w):
     return n_nodes
 
 
+def check_full_graph(res, w, n_nodes):
+    """sdbg_build_full at full size: properties that tie its arrays to those of sdbg_build (checked bit for bit against
+    the oracle in tests/test_gpu_full_graph.py at sizes the oracle can hold): the real edges are an order-preserving
+    subsequence with unchanged W / last / mult, every '$' edge is the only edge of its node, validity bits are m ones,
+    and, both strands being present, the nodes without outgoing edge mirror the nodes without incoming edge."""
+    import torch
+    ed, g, S = res.edges, res.graph, res.n
+    ws = 64 * S * ed.w + (1 << 28)
+    ctx = sd.Context(ws)
+    probe = sd.FullGraph(0, 0, w.k)
+    try:
+        sd.sdbg_build_full(ctx, ed, probe)
+    except sd.SdbgError as e:
+        assert e.name == "SDBG_E_CAPACITY", e
+    fg = sd.FullGraph(probe.m, probe.t, w.k)
+    sd.sdbg_build_full(ctx, ed, fg)
+    m, t, nzo = fg.m, fg.t, fg.n_zero_out
+    assert m == S + nzo and t == nzo
+    Wf = fg.W[:m]
+    real = Wf != 0
+    assert int(real.sum()) == S
+    assert torch.equal(Wf[real], g.W[:S]) and torch.equal(fg.mult[:m][real], g.mult[:S])
+    assert int(fg.mult[:m][~real].abs().sum()) == 0
+    bits = ((fg.last_bits[:(m + 63) // 64].unsqueeze(1) >> torch.arange(64, device="cuda")) & 1).reshape(-1)[:m].bool()
+    gbits = ((g.last_bits[:(S + 63) // 64].unsqueeze(1) >> torch.arange(64, device="cuda")) & 1).reshape(-1)[:S].bool()
+    assert torch.equal(bits[real], gbits) and bool(bits[~real].all())
+    assert int(bits.sum()) == n_nodes + nzo
+    vb = fg.valid_bits[:(m + 63) // 64]
+    ones = ((vb.unsqueeze(1) >> torch.arange(64, device="cuda")) & 1).reshape(-1)
+    assert int(ones[:m].sum()) == m and int(ones[m:].sum()) == 0
+    ctx.close(); ctx.workspace = None
+    return m, t
+
+
 def compare_partitions(res, w, orc, buckets):
     """Bit-exact comparison of the GPU output slices of the given l=8 partitions with the oracle's result for them."""
     import torch

@@ -10,7 +10,8 @@ import time
 import numpy as np
 import pytest
 
-from tests.gpu_util import (check_global_invariants, compare_partitions, oracle_partitions, run_gpu_workload)
+from tests.gpu_util import (check_full_graph, check_global_invariants, compare_partitions, oracle_partitions,
+                            run_gpu_workload)
 
 pytestmark = pytest.mark.gpu
 LARGE = {int(x) for x in os.environ.get("SDBG_LARGE", "").replace(",", " ").split()}
@@ -26,7 +27,7 @@ def _pick_buckets(hist, seed, n=16):
     return sorted(picks)
 
 
-def _run_config(cfg, workspace_bytes=None, min_ranges=1, n_buckets=16):
+def _run_config(cfg, workspace_bytes=None, min_ranges=1, n_buckets=16, full_graph=True):
     from workloads import get_config
     w = get_config(cfg)
     t0 = time.time()
@@ -38,6 +39,9 @@ def _run_config(cfg, workspace_bytes=None, min_ranges=1, n_buckets=16):
     res.ctx.close(); res.ctx.workspace = None; res.reads = None      # the checks below need the HBM
     torch.cuda.empty_cache()
     n_nodes = check_global_invariants(res, w)
+    tf0 = time.time()
+    m_full, t_full = check_full_graph(res, w, n_nodes) if full_graph else (0, 0)
+    tf1 = time.time()
     hist = st.bucket_hist.cpu().numpy()
     assert int(hist.sum()) == w.n_raw_edges
     buckets = _pick_buckets(hist, w.seed, n_buckets)
@@ -49,7 +53,8 @@ def _run_config(cfg, workspace_bytes=None, min_ranges=1, n_buckets=16):
     n_cmp = compare_partitions(res, w, orc, buckets)
     print(f"\n[{w.name}] N={st.n_raw} distinct={st.n_distinct} solid={res.n} nodes={n_nodes} ranges={st.n_ranges} "
           f"max_range={st.max_range_records} | gpu path {t1 - t0:.1f}s invariants {t2 - t1:.1f}s "
-          f"oracle({len(buckets)} partitions, {orc.n_raw} records, {n_cmp} solid edges compared bit-exact) {t3 - t2:.1f}s")
+          f"oracle({len(buckets)} partitions, {orc.n_raw} records, {n_cmp} solid edges compared bit-exact) {t3 - t2:.1f}s"
+          f" | full graph m={m_full} t={t_full} ({tf1 - tf0:.1f}s)")
 
 
 def test_config2_full_size_sampled_partitions():
@@ -67,4 +72,4 @@ def test_config4_full_size_sampled_partitions():
 @pytest.mark.skipif(5 not in LARGE, reason="set SDBG_LARGE=5 (2 minutes of 16 host cores, 20 GB of host RAM, ~170 GB of HBM)")
 def test_config5_full_size_blockwise():
     # 20 Gbp of reads stay packed in HBM; the 31.6 G records go through block-wise ranges of l=8 partitions
-    _run_config(5, workspace_bytes=100 * 2 ** 30, min_ranges=4, n_buckets=8)
+    _run_config(5, workspace_bytes=100 * 2 ** 30, min_ranges=4, n_buckets=8, full_graph=False)   # HBM is full already
