@@ -326,3 +326,95 @@ const uint8_t *orc_full_W(const orc_full *f) { return f->W; }
 const uint8_t *orc_full_last(const orc_full *f) { return f->last; }
 const uint32_t *orc_full_mult(const orc_full *f) { return f->mult; }
 const char *orc_full_aux(const orc_full *f) { return f->aux; }
+
+/* ---- mercy-kmers (readings A21-A23 in DESIGN.md) ---------------------------------
+ * "Given two solid (k+1)-mers x and y from the same read, where x has no outdegree and y has no indegree. If all
+ * (k+1)-mers between x and y in that read are not solid, they will be added to the de Bruijn graph as mercy-kmers."
+ *   For every read (as given), windows w_i = r[i..i+k]; w_i is solid iff it is one of the solid edges S.
+ *   For every maximal run w_a..w_b of non-solid windows that has a solid window on both sides (x = w_{a-1},
+ *   y = w_{b+1}): if tgt(x) = x[1..k] has no outgoing solid edge and src(y) = y[0..k) has no incoming solid edge, every
+ *   w_i of the run and its reverse complement are recorded once (both strands, as in step 1).
+ * Output: the recorded (k+1)-mers in the order they were met (a multiset; the caller sorts / merges them). */
+static int64_t find_edge(const orc *o, const char *e) {   /* index of e among the solid edges, or -1 (binary search, step-2 order) */
+    uint64_t lo = 0, hi = o->n_solid;
+    const uint32_t R = o->k + 1;
+    while (lo < hi) {
+        uint64_t mid = lo + (hi - lo) / 2;
+        int c = cmp_edges(o->S + mid * R, e, (void *)&o->k);
+        if (c == 0) return (int64_t)mid;
+        if (c < 0) lo = mid + 1; else hi = mid;
+    }
+    return -1;
+}
+static int kmer_in(const char *list, uint64_t n, uint32_t k, const char *v) {   /* colex-sorted list of k-mers */
+    uint64_t lo = 0, hi = n;
+    g_kcmp = k;
+    while (lo < hi) {
+        uint64_t mid = lo + (hi - lo) / 2;
+        int c = cmp_kmers(list + mid * k, v);
+        if (c == 0) return 1;
+        if (c < 0) lo = mid + 1; else hi = mid;
+    }
+    return 0;
+}
+
+typedef struct orc_mercy { uint64_t n, cap; char *E; } orc_mercy;
+
+static int mercy_push(orc_mercy *m, const char *e, uint32_t R) {
+    if (m->n == m->cap) {
+        uint64_t nc = m->cap ? m->cap * 2 : 256;
+        char *p = (char *)realloc(m->E, nc * R);
+        if (!p) return ORC_E_NOMEM;
+        m->E = p; m->cap = nc;
+    }
+    memcpy(m->E + m->n * R, e, R);
+    m->n++;
+    return ORC_OK;
+}
+
+/* reads as in orc_add_reads; call after orc_finish. Returns NULL on error. */
+orc_mercy *orc_mercy_scan(const orc *o, const char *bases, const uint64_t *offsets, uint64_t n) {
+    const uint32_t k = o->k, R = k + 1;
+    orc_full *f = orc_full_graph(o);
+    orc_mercy *m = (orc_mercy *)calloc(1, sizeof(orc_mercy));
+    if (!f || !m) return NULL;
+    /* nodes without outgoing edge: the nodes of the '$' edges of F, in colex order */
+    char *zout = (char *)malloc(f->n_zero_out * k + 1);
+    uint64_t nzo = 0;
+    for (uint64_t q = 0; q < f->m; ++q) if (f->F[q * R + k] == '$') memcpy(zout + nzo++ * k, f->F + q * R, k);
+    char *rd = NULL, *rc = (char *)malloc(R);
+    uint8_t *sol = NULL;
+    uint64_t cap = 0;
+    int st = ORC_OK;
+    for (uint64_t r = 0; r < n && st == ORC_OK; ++r) {
+        const uint64_t L = offsets[r + 1] - offsets[r];
+        if (L < R) continue;
+        if (L > cap) { free(rd); free(sol); rd = (char *)malloc(L); sol = (uint8_t *)malloc(L); cap = L; }
+        for (uint64_t j = 0; j < L; ++j) { char c = bases[offsets[r] + j]; rd[j] = (c >= 'a' && c <= 'z') ? (char)(c - 'a' + 'A') : c; }
+        const uint64_t nw = L - k;
+        for (uint64_t i = 0; i < nw; ++i) sol[i] = find_edge(o, rd + i) >= 0;
+        for (uint64_t a = 1; a + 1 < nw && st == ORC_OK;) {
+            if (sol[a] || !sol[a - 1]) { ++a; continue; }
+            uint64_t b = a;                                   /* run of non-solid windows a..b, x = w_{a-1} */
+            while (b + 1 < nw && !sol[b + 1]) ++b;
+            if (b + 1 < nw) {                                 /* y = w_{b+1} is solid */
+                const char *x = rd + a - 1, *y = rd + b + 1;
+                if (kmer_in(zout, nzo, k, x + 1) && kmer_in(f->aux, f->t, k, y)) {
+                    for (uint64_t i = a; i <= b && st == ORC_OK; ++i) {
+                        for (uint32_t t = 0; t <= k; ++t) rc[t] = comp(rd[i + k - t]);
+                        st = mercy_push(m, rd + i, R);
+                        if (st == ORC_OK) st = mercy_push(m, rc, R);
+                    }
+                }
+            }
+            a = b + 1;
+        }
+    }
+    free(rd); free(sol); free(rc); free(zout);
+    orc_full_free(f);
+    if (st != ORC_OK) { free(m->E); free(m); return NULL; }
+    return m;
+}
+uint64_t orc_mercy_n(const orc_mercy *m) { return m->n; }
+const char *orc_mercy_edges(const orc_mercy *m) { return m->E; }
+void orc_mercy_free(orc_mercy *m) { if (m) { free(m->E); free(m); } }

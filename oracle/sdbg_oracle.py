@@ -44,6 +44,10 @@ def _load():
             getattr(L, "orc_full_" + f).argtypes = [vp]; getattr(L, "orc_full_" + f).restype = u64
         for f in ("edges", "W", "last", "mult", "aux"):
             getattr(L, "orc_full_" + f).argtypes = [vp]; getattr(L, "orc_full_" + f).restype = vp
+        L.orc_mercy_scan.argtypes = [vp, vp, vp, u64]; L.orc_mercy_scan.restype = vp
+        L.orc_mercy_n.argtypes = [vp]; L.orc_mercy_n.restype = u64
+        L.orc_mercy_edges.argtypes = [vp]; L.orc_mercy_edges.restype = vp
+        L.orc_mercy_free.argtypes = [vp]; L.orc_mercy_free.restype = None
         _lib = L
     return _lib
 
@@ -181,6 +185,26 @@ class Oracle:
                 pos += 2
         out.update(last_bits=lb, valid_bits=vb, aux_bits=ab)
         return out
+
+    def mercy(self, bases, offsets):
+        """Mercy-kmers of PAPER.md:35 (call after finish, with the reads again): dict with `edges` (n, k+1) letters in
+        the order met (a multiset holding both strands) and `keys` (n, w) their step-6 keys."""
+        L = _load()
+        b = np.frombuffer(bases, dtype=np.uint8) if isinstance(bases, (bytes, bytearray)) else np.ascontiguousarray(bases, dtype=np.uint8)
+        o = np.ascontiguousarray(offsets, dtype=np.uint64)
+        m = L.orc_mercy_scan(self._h, b.ctypes.data if b.size else None, o.ctypes.data, len(o) - 1)
+        if not m:
+            raise MemoryError("oracle: mercy scan")
+        try:
+            n, k = L.orc_mercy_n(m), self.k
+            w = (2 * (k + 1) + 63) // 64
+            edges = _copy(L.orc_mercy_edges(m), n * (k + 1), np.uint8).reshape(-1, k + 1)
+            keys = np.zeros(n * w, dtype=np.uint64)
+            if n:
+                L.orc_encode_keys(self._h, edges.ctypes.data, n, keys.ctypes.data)
+        finally:
+            L.orc_mercy_free(m)
+        return dict(edges=edges, keys=keys.reshape(-1, w))
 
     def close(self):
         if self._h:

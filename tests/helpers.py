@@ -115,3 +115,28 @@ def brute_force_full(reads, k, d):
         W.append(0 if e[k] == "$" else order[e[k]] + (4 if minus else 0))
         M.append(mult.get(e, 0))
     return dict(F=F, W=W, last=last, mult=M, aux=zin, zout=zout)
+
+
+def brute_force_mercy(reads, k, d):
+    """Mercy-kmers of PAPER.md:35 (readings A21-A23) from brute_force(): sets and plain loops."""
+    b = brute_force(reads, k, d)
+    S = set(b["solid"])
+    src, tgt = {e[:k] for e in S}, {e[1:] for e in S}
+    no_out, no_in = tgt - src, src - tgt
+    out = []
+    for r in reads:
+        r = r.upper()
+        w = [r[i:i + k + 1] for i in range(len(r) - k)]
+        i = 0
+        while i < len(w):
+            if w[i] in S:
+                i += 1
+                continue
+            j = i
+            while j + 1 < len(w) and w[j + 1] not in S:
+                j += 1
+            if i >= 1 and j + 1 < len(w) and w[i - 1][1:] in no_out and w[j + 1][:k] in no_in:
+                for e in w[i:j + 1]:
+                    out += [e, rc(e)]
+            i = j + 1
+    return out

@@ -314,3 +314,57 @@ def test_full_graph_bruteforce_and_strand_symmetry(k):
             # the dummies change no flag of a real edge
             real = [i for i, e in enumerate(f["edges"]) if e[k] != ord("$")]
             assert np.array_equal(f["W"][real], res.Wbyte) and np.array_equal(f["last"][real], res.last)
+
+
+# ---- mercy-kmers of PAPER.md:35 (Oracle.mercy; readings A21-A23) --------------------------------------------------------
+
+def _mercy(reads, k, d):
+    from oracle import Oracle
+    from oracle.sdbg_oracle import reads_to_arrays
+    b, o = reads_to_arrays(list(reads))
+    orc = Oracle(k, d)
+    orc.add_reads(b, o)
+    orc.finish()
+    m = orc.mercy(b, o)
+    orc.close()
+    return sorted(bytes(e).decode() for e in m["edges"])
+
+
+def test_mercy_closed_form_of_a_bridged_gap():
+    """Two segments of a random sequence at coverage 3 and ONE read bridging the gap between them: the windows of the
+    bridge that lie in the gap are not solid, their neighbours are the open ends of the two segments, so exactly these
+    windows (and their reverse complements) are mercy-kmers. A second copy of the bridge makes them solid: no mercy."""
+    import random
+    from tests.helpers import rc
+    rng = random.Random(3)
+    g = "".join(rng.choice("ACGT") for _ in range(120))
+    k = 11
+    seg = [g[0:50]] * 3 + [g[70:120]] * 3
+    got = _mercy(seg + [g[30:90]], k, 2)
+    gap = [g[i:i + k + 1] for i in range(39, 70)]          # windows 39..69: not inside either segment
+    assert got == sorted(gap + [rc(e) for e in gap])
+    assert _mercy(seg + [g[30:90]] * 2, k, 2) == []        # solid now
+    assert _mercy(seg + [g[30:75]], k, 2) == []            # the run of non-solid windows reaches the read end: no y
+    # x must have no outgoing edge: a branch at the end of the first segment (another continuation, solid) forbids it
+    branch = g[30:50] + "".join(rng.choice("ACGT") for _ in range(20))
+    assert _mercy(seg + [branch] * 2 + [g[30:90]], k, 2) == []
+
+
+@pytest.mark.parametrize("k", [3, 5, 8, 11])
+def test_mercy_bruteforce_and_strand_symmetry(k):
+    import random
+    from tests.helpers import brute_force_mercy, rc
+    rng = random.Random(500 + k)
+    hits = 0
+    for trial in range(8):
+        src = ["".join(rng.choice("ACGT") for _ in range(rng.randint(3 * k, 3 * k + 60))) for _ in range(3)]
+        reads = []
+        for _ in range(30):
+            s = rng.choice(src)
+            a = rng.randint(0, len(s)); b = rng.randint(a, len(s))
+            reads.append(s[a:b] if rng.random() < 0.6 else rc(s[a:b]))
+        got = _mercy(reads, k, 2)
+        assert got == sorted(brute_force_mercy(reads, k, 2))
+        assert got == _mercy([rc(r) for r in reads], k, 2)       # the same multiset from the other strand of every read
+        hits += len(got)
+    assert hits > 0 or k < 8        # tiny k: nearly every window is solid, gaps are rare
