@@ -202,6 +202,18 @@ typedef struct {
  * (needs about 40 + 16 w bytes of workspace per edge), SDBG_E_UNSUPPORTED, SDBG_E_INVAL. */
 int sdbg_build_full(sdbg_ctx *ctx, const sdbg_edges *edges, sdbg_full_graph *out);
 
+/* Mercy-kmers (§2 ¶3; readings A21-A23 of DESIGN.md): "Given two solid (k+1)-mers x
+ * and y from the same read, where x has no outdegree and y has no indegree. If all (k+1)-mers between x and y in that
+ * read are not solid, they will be added to the de Bruijn graph as mercy-kmers." For every read (as packed), every
+ * maximal run of non-solid windows with a solid window x right before it and a solid window y right behind it: if
+ * tgt(x) has no outgoing solid edge and src(y) has no incoming solid edge, every window of the run and its reverse
+ * complement are appended to `out` (keys, mult = 1; unsorted, with repeats: out->n records). `solid` is the output of
+ * sdbg_count_edges over the same reads (sorted, distinct; 2 <= k <= 127; fewer than 2^32 edges). To build the graph
+ * with them, put solid and mercy records into one sdbg_edges and call sdbg_build without SDBG_SORTED (equal keys are
+ * merged, mult summed). Synchronises. Errors: SDBG_E_CAPACITY (out->n = needed count), SDBG_E_WORKSPACE,
+ * SDBG_E_UNSUPPORTED, SDBG_E_INVAL. */
+int sdbg_mercy_edges(sdbg_ctx *ctx, const sdbg_reads *reads, const sdbg_edges *solid, sdbg_edges *out);
+
 /* ---- measurement hooks ---------------------------------------------------------------------------------- */
 
 enum { SDBG_T_PACK = 0, SDBG_T_EXTRACT = 1, SDBG_T_RADIX = 2, SDBG_T_COUNT = 3, SDBG_T_EMIT = 4, SDBG_T_OTHER = 5, SDBG_T_NUM = 6 };

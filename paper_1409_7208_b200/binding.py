@@ -88,6 +88,7 @@ def lib():
         L.sdbg_plan_ranges.argtypes = [vp, u64, vp, u64]; L.sdbg_plan_ranges.restype = C.c_int64
         L.sdbg_build.argtypes = [vp, C.POINTER(_Edges), u32, C.POINTER(_Graph)]; L.sdbg_build.restype = i32
         L.sdbg_build_full.argtypes = [vp, C.POINTER(_Edges), C.POINTER(_FullGraph)]; L.sdbg_build_full.restype = i32
+        L.sdbg_mercy_edges.argtypes = [vp, C.POINTER(_Reads), C.POINTER(_Edges), C.POINTER(_Edges)]; L.sdbg_mercy_edges.restype = i32
         L.sdbg_ctx_set_timing.argtypes = [vp, i32]; L.sdbg_ctx_set_timing.restype = i32
         L.sdbg_ctx_get_timing.argtypes = [vp, C.POINTER(_Timing)]; L.sdbg_ctx_get_timing.restype = i32
         _lib = L
@@ -306,6 +307,11 @@ def sdbg_pack_reads(ctx: Context, bases, offsets, n: int, out: Reads) -> None:
 def sdbg_count_edges(ctx: Context, reads: Reads, n: int, k: int, d: int, out: Edges, stats: Stats | None = None) -> int:
     rc = lib().sdbg_count_edges(ctx._h, C.byref(reads.c), n, k, d, C.byref(out.c), C.byref(stats.c) if stats else None)
     ctx.check(rc)
+    return out.c.n
+
+
+def sdbg_mercy_edges(ctx: Context, reads: Reads, solid: Edges, out: Edges) -> int:
+    ctx.check(lib().sdbg_mercy_edges(ctx._h, C.byref(reads.c), C.byref(solid.c), C.byref(out.c)))
     return out.c.n
 
 
