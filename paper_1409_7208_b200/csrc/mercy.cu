@@ -54,9 +54,32 @@ __device__ void window_keys(const u64 *__restrict__ words, u64 slot, u32 k, u64 
     }
 }
 
+// Index over the sorted solid edges by the top kMercyIndexBits key bits: index[p] = first edge whose prefix is >= p
+// (index[2^bits] = n), so that a look-up searches one slice only (a few hundred edges instead of all of them).
+template <int W>
+__global__ void __launch_bounds__(256) prefix_index_kernel(const u64 *__restrict__ keys, u64 n, u64 *__restrict__ index) {
+    constexpr u32 sh = 64 - kMercyIndexBits;
+    for (u64 i = (u64)blockIdx.x * blockDim.x + threadIdx.x; i <= n; i += (u64)gridDim.x * blockDim.x) {
+        const u64 cur = i < n ? keys[i * W] >> sh : (1ull << kMercyIndexBits);   // sentinel: one past the last prefix
+        const u64 prev = i ? (keys[(i - 1) * W] >> sh) + 1 : 0;                   // prefixes (prev-1, cur] begin at edge i
+        for (u64 p = prev; p <= cur; ++p) index[p] = i;
+    }
+}
+void launch_prefix_index(const u64 *keys, u64 n, u32 W, u64 *index, cudaStream_t s) {
+    u64 blocks = (n + 256) / 256;
+    if (blocks > (u64)kNumSMs * 16) blocks = (u64)kNumSMs * 16;
+    switch (W) {
+        case 1: prefix_index_kernel<1><<<(unsigned)blocks, 256, 0, s>>>(keys, n, index); break;
+        case 2: prefix_index_kernel<2><<<(unsigned)blocks, 256, 0, s>>>(keys, n, index); break;
+        case 3: prefix_index_kernel<3><<<(unsigned)blocks, 256, 0, s>>>(keys, n, index); break;
+        default: prefix_index_kernel<4><<<(unsigned)blocks, 256, 0, s>>>(keys, n, index); break;
+    }
+}
+
 template <int W>
 __device__ __forceinline__ bool is_solid(const MercyArgs &a, const u64 (&key)[W]) {
-    u64 lo = 0, hi = a.n;
+    const u64 pfx = key[0] >> (64 - kMercyIndexBits);
+    u64 lo = __ldg(a.index + pfx), hi = __ldg(a.index + pfx + 1);
     while (lo < hi) {
         const u64 mid = lo + ((hi - lo) >> 1);
         u64 e[W];
