@@ -253,6 +253,31 @@ def check_full_graph(res, w, n_nodes):
     return m, t
 
 
+def check_mercy(res, w, reads):
+    """sdbg_mercy_edges at full size (bit-exact against the oracle in tests/test_gpu_mercy.py at oracle sizes):
+    records come as (window, reverse complement) pairs, and no mercy record is a solid edge."""
+    import torch
+    ed, S = res.edges, res.n
+    ctx = sd.Context(64 * S * ed.w + (1 << 28))
+    probe = sd.Edges(0, w.k)
+    try:
+        sd.sdbg_mercy_edges(ctx, reads, ed, probe)
+    except sd.SdbgError as e:
+        assert e.name == "SDBG_E_CAPACITY", e
+    M = probe.n
+    me = sd.Edges(M, w.k)
+    sd.sdbg_mercy_edges(ctx, reads, ed, me)
+    assert me.n == M and M % 2 == 0
+    if M:
+        assert int(me.mult[:M].min()) == 1 and int(me.mult[:M].max()) == 1
+        if ed.w == 1:
+            sk = _u64_sorted_view(ed.keys[:S]); mk = _u64_sorted_view(me.keys[:M])
+            pos = torch.searchsorted(sk, mk).clamp(max=S - 1)
+            assert int((sk[pos] == mk).sum()) == 0, "a mercy record is a solid edge"
+    ctx.close(); ctx.workspace = None
+    return M
+
+
 def compare_partitions(res, w, orc, buckets):
     """Bit-exact comparison of the GPU output slices of the given l=8 partitions with the oracle's result for them."""
     import torch

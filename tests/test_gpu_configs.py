@@ -10,7 +10,7 @@ import time
 import numpy as np
 import pytest
 
-from tests.gpu_util import (check_full_graph, check_global_invariants, compare_partitions, oracle_partitions,
+from tests.gpu_util import (check_full_graph, check_global_invariants, check_mercy, compare_partitions, oracle_partitions,
                             run_gpu_workload)
 
 pytestmark = pytest.mark.gpu
@@ -36,7 +36,10 @@ def _run_config(cfg, workspace_bytes=None, min_ranges=1, n_buckets=16, full_grap
     st = res.stats
     assert st.n_ranges >= min_ranges, st.n_ranges
     import torch
-    res.ctx.close(); res.ctx.workspace = None; res.reads = None      # the checks below need the HBM
+    res.ctx.close(); res.ctx.workspace = None                        # the checks below need the HBM
+    torch.cuda.empty_cache()
+    n_mercy = check_mercy(res, w, res.reads) if full_graph else 0
+    res.reads = None
     torch.cuda.empty_cache()
     n_nodes = check_global_invariants(res, w)
     tf0 = time.time()
@@ -54,7 +57,7 @@ def _run_config(cfg, workspace_bytes=None, min_ranges=1, n_buckets=16, full_grap
     print(f"\n[{w.name}] N={st.n_raw} distinct={st.n_distinct} solid={res.n} nodes={n_nodes} ranges={st.n_ranges} "
           f"max_range={st.max_range_records} | gpu path {t1 - t0:.1f}s invariants {t2 - t1:.1f}s "
           f"oracle({len(buckets)} partitions, {orc.n_raw} records, {n_cmp} solid edges compared bit-exact) {t3 - t2:.1f}s"
-          f" | full graph m={m_full} t={t_full} ({tf1 - tf0:.1f}s)")
+          f" | full graph m={m_full} t={t_full} ({tf1 - tf0:.1f}s) | mercy records {n_mercy}")
 
 
 def test_config2_full_size_sampled_partitions():
