@@ -271,6 +271,58 @@ def run_gpu(args, w):
         dist.destroy_process_group()
 
 
+def run_next_rows(args, w):
+    """`--next`: the two widened rows (DESIGN.md §0 f-1, f-2) on the same workload, timed by CUDA events around the
+    C-ABI calls: sdbg_build_full and sdbg_mercy_edges over the solid edges of one sdbg_count_edges run. Not part of
+    the step that `value` measures."""
+    import torch
+    import paper_1409_7208_b200 as sd
+    from workloads import ReadGenerator
+    torch.cuda.set_device(0)
+    bases_d, offs_d = ReadGenerator(w).device()
+    N = w.n_raw_edges
+    ctx = sd.Context(sd.sdbg_workspace_for_records(N, w.k))
+    reads = sd.Reads(w.n_bases)
+    sd.sdbg_pack_reads(ctx, bases_d, offs_d, w.n_reads, reads)
+    edges = sd.Edges(N // w.d, w.k)
+    sd.sdbg_count_edges(ctx, reads, w.n_reads, w.k, w.d, edges, None)
+    S = edges.n
+
+    def sized(call, make):
+        probe = make(0)
+        try:
+            call(probe)
+        except sd.SdbgError as e:
+            if e.name != "SDBG_E_CAPACITY":
+                raise
+        return probe
+
+    pf = sized(lambda g: sd.sdbg_build_full(ctx, edges, g), lambda c: sd.FullGraph(c, c, w.k))
+    fg = sd.FullGraph(pf.m, pf.t, w.k)
+    pm = sized(lambda e: sd.sdbg_mercy_edges(ctx, reads, edges, e), lambda c: sd.Edges(c, w.k))
+    me = sd.Edges(pm.n, w.k)
+
+    def timed(fn):
+        for _ in range(2):
+            fn()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        torch.cuda.synchronize()
+        e0.record()
+        for _ in range(args.steps):
+            fn()
+        e1.record()
+        torch.cuda.synchronize()
+        return e0.elapsed_time(e1) / args.steps
+
+    ms_full = timed(lambda: sd.sdbg_build_full(ctx, edges, fg))
+    ms_mercy = timed(lambda: sd.sdbg_mercy_edges(ctx, reads, edges, me))
+    print(json.dumps({"impl": "next_rows", "config": {"workload": w.name, "k": w.k, "d": w.d, "solid_edges": int(S)},
+                      "sdbg_build_full": {"ms": ms_full, "m": int(fg.m), "t": int(fg.t), "dollar_edges": int(fg.n_zero_out),
+                                          "solid_edges_per_s": S / (ms_full * 1e-3)},
+                      "sdbg_mercy_edges": {"ms": ms_mercy, "mercy_records": int(me.n),
+                                           "read_bases_per_s": w.n_bases / (ms_mercy * 1e-3)}}), flush=True)
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -281,9 +333,14 @@ def main():
     ap.add_argument("--ref-reads", type=int, default=40000, help="reads in the oracle's bounded sample")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true", help="development runs: skip the host-buffer end-to-end leg")
+    ap.add_argument("--next", action="store_true", help="time the widened rows (sdbg_build_full, sdbg_mercy_edges) instead")
     args = ap.parse_args()
     from workloads import get_config
     w = get_config(args.config)
+    if args.next:
+        if int(os.environ.get("RANK", "0")) == 0:
+            run_next_rows(args, w)
+        return
     if args.impl == "reference":
         if int(os.environ.get("RANK", "0")) == 0:
             run_reference(args, w)
