@@ -54,41 +54,47 @@ __device__ void window_keys(const u64 *__restrict__ words, u64 slot, u32 k, u64 
     }
 }
 
-// Index over the sorted solid edges by the top kMercyIndexBits key bits: index[p] = first edge whose prefix is >= p
-// (index[2^bits] = n), so that a look-up searches one slice only (a few hundred edges instead of all of them).
+// Hash table over the solid edges (open addressing, linear probing, load <= 1/2): slot = edge index + 1, 0 = empty.
+// A look-up costs one or two dependent random reads instead of the ~30 of a binary search over the whole list.
 template <int W>
-__global__ void __launch_bounds__(256) prefix_index_kernel(const u64 *__restrict__ keys, u64 n, u64 *__restrict__ index) {
-    constexpr u32 sh = 64 - kMercyIndexBits;
-    for (u64 i = (u64)blockIdx.x * blockDim.x + threadIdx.x; i <= n; i += (u64)gridDim.x * blockDim.x) {
-        const u64 cur = i < n ? keys[i * W] >> sh : (1ull << kMercyIndexBits);   // sentinel: one past the last prefix
-        const u64 prev = i ? (keys[(i - 1) * W] >> sh) + 1 : 0;                   // prefixes (prev-1, cur] begin at edge i
-        for (u64 p = prev; p <= cur; ++p) index[p] = i;
+__device__ __forceinline__ u64 hash_key(const u64 (&key)[W]) {
+    u64 h = 0;
+#pragma unroll
+    for (int q = 0; q < W; ++q) h = mix64(h ^ key[q]);
+    return h;
+}
+template <int W>
+__global__ void __launch_bounds__(256) hash_build_kernel(const u64 *__restrict__ keys, u64 n, u32 *__restrict__ table, u64 mask) {
+    for (u64 i = (u64)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (u64)gridDim.x * blockDim.x) {
+        u64 key[W];
+        ldk<W>(keys, i, key);
+        u64 h = hash_key<W>(key) & mask;
+        while (atomicCAS(&table[h], 0u, (u32)i + 1u) != 0u) h = (h + 1) & mask;
     }
 }
-void launch_prefix_index(const u64 *keys, u64 n, u32 W, u64 *index, cudaStream_t s) {
-    u64 blocks = (n + 256) / 256;
+void launch_hash_build(const u64 *keys, u64 n, u32 W, u32 *table, u64 slots, cudaStream_t s) {
+    u64 blocks = (n + 255) / 256;
     if (blocks > (u64)kNumSMs * 16) blocks = (u64)kNumSMs * 16;
+    if (blocks == 0) return;
     switch (W) {
-        case 1: prefix_index_kernel<1><<<(unsigned)blocks, 256, 0, s>>>(keys, n, index); break;
-        case 2: prefix_index_kernel<2><<<(unsigned)blocks, 256, 0, s>>>(keys, n, index); break;
-        case 3: prefix_index_kernel<3><<<(unsigned)blocks, 256, 0, s>>>(keys, n, index); break;
-        default: prefix_index_kernel<4><<<(unsigned)blocks, 256, 0, s>>>(keys, n, index); break;
+        case 1: hash_build_kernel<1><<<(unsigned)blocks, 256, 0, s>>>(keys, n, table, slots - 1); break;
+        case 2: hash_build_kernel<2><<<(unsigned)blocks, 256, 0, s>>>(keys, n, table, slots - 1); break;
+        case 3: hash_build_kernel<3><<<(unsigned)blocks, 256, 0, s>>>(keys, n, table, slots - 1); break;
+        default: hash_build_kernel<4><<<(unsigned)blocks, 256, 0, s>>>(keys, n, table, slots - 1); break;
     }
 }
 
 template <int W>
 __device__ __forceinline__ bool is_solid(const MercyArgs &a, const u64 (&key)[W]) {
-    const u64 pfx = key[0] >> (64 - kMercyIndexBits);
-    u64 lo = __ldg(a.index + pfx), hi = __ldg(a.index + pfx + 1);
-    while (lo < hi) {
-        const u64 mid = lo + ((hi - lo) >> 1);
+    u64 h = hash_key<W>(key) & a.table_mask;
+    while (true) {
+        const u32 v = __ldg(a.table + h);
+        if (v == 0u) return false;
         u64 e[W];
-        ldk<W>(a.keys, mid, e);
-        const int c = cmpk<W>(e, key);
-        if (c == 0) return true;
-        if (c < 0) lo = mid + 1; else hi = mid;
+        ldk<W>(a.keys, (u64)v - 1u, e);
+        if (cmpk<W>(e, key) == 0) return true;
+        h = (h + 1) & a.table_mask;
     }
-    return false;
 }
 
 // node (top 2k bits of `key`, W words) among the nodes without outgoing edge (tk rows listed by zout_idx, WT words)
