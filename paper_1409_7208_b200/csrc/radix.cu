@@ -50,7 +50,12 @@ template <> struct RadixCfg<3, false> { static constexpr int THREADS = 512, KPT 
 #define SDBG_R4_MINB 2
 #endif
 template <> struct RadixCfg<4, false> { static constexpr int THREADS = SDBG_R4_THREADS, KPT = SDBG_R4_KPT, MINB = SDBG_R4_MINB; };
-template <> struct RadixCfg<1, true>  { static constexpr int THREADS = 512, KPT = 10, MINB = 2; };
+#ifndef SDBG_R1V_THREADS
+#define SDBG_R1V_THREADS 384   // (key word, u32 payload): 384 x 14 (measured best on the pair passes of config 4)
+#define SDBG_R1V_KPT 14
+#define SDBG_R1V_MINB 2
+#endif
+template <> struct RadixCfg<1, true>  { static constexpr int THREADS = SDBG_R1V_THREADS, KPT = SDBG_R1V_KPT, MINB = SDBG_R1V_MINB; };
 template <> struct RadixCfg<2, true>  { static constexpr int THREADS = 512, KPT = 6,  MINB = 2; };
 template <> struct RadixCfg<3, true>  { static constexpr int THREADS = 512, KPT = 4,  MINB = 2; };
 template <> struct RadixCfg<4, true>  { static constexpr int THREADS = 512, KPT = 3,  MINB = 2; };
