@@ -140,3 +140,60 @@ def brute_force_mercy(reads, k, d):
                     out += [e, rc(e)]
             i = j + 1
     return out
+
+
+def brute_force_navigation(F, aux, k):
+    """forward / backward / zin / F-array of the full edge list F (strings, '$' for dummies) by loops over strings
+    (readings A24-A26): nothing but comparisons of node strings."""
+    m = len(F)
+    zin = [1 if (F[i][:k] in set(aux) and (i == m - 1 or F[i + 1][:k] != F[i][:k])) else 0 for i in range(m)]
+    Farr = [min([i for i in range(m) if F[i][k - 1] >= c], default=m) for c in "ACGT"] + [m]
+    fwd, bwd = [], []
+    for i in range(m):
+        if F[i][k] == "$":
+            fwd.append(-1)
+        else:
+            fwd.append(max(j for j in range(m) if F[j][:k] == F[i][1:]))
+        inc = [j for j in range(m) if F[j][k] != "$" and F[j][1:] == F[i][:k]]
+        bwd.append(min(inc) if inc else -1)
+    return dict(zin=zin, F=Farr, forward=fwd, backward=bwd)
+
+
+def boss_navigation(W, last, zin, Farr):
+    """The same two maps from the succinct arrays alone, by the rank/select formulas of Bowe et al.
+    adapted to the graph without incoming dummy edges (reading A26), with counting loops for rank and select:
+      H[i] = last[i] and not zin[i]                 (last edge of a node that has an incoming edge)
+      B_c[i] = (W[i] == c, minus flag clear)
+      forward(i)  = select_H(rank_H(F[c]) + rank_{B_c}(i + 1)),   c = base of W[i]
+      backward(j) = select_{B_c}(rank_H(p + 1) - rank_H(F[c])),   p = last edge of the node of j, c = its class in F."""
+    m = len(W)
+    H = [1 if (last[i] and not zin[i]) else 0 for i in range(m)]
+
+    def rank(bits, x):
+        return sum(bits[:x])
+
+    def select(bits, r):
+        seen = 0
+        for i, b in enumerate(bits):
+            seen += b
+            if b and seen == r:
+                return i
+        raise AssertionError("select out of range")
+
+    B = [[1 if W[i] == c + 1 else 0 for i in range(m)] for c in range(4)]
+    fwd, bwd = [], []
+    for i in range(m):
+        if W[i] == 0:
+            fwd.append(-1)
+        else:
+            c = (W[i] - 1) & 3
+            fwd.append(select(H, rank(H, Farr[c]) + rank(B[c], i + 1)))
+        p = i
+        while not last[p]:
+            p += 1
+        if not H[p]:
+            bwd.append(-1)
+        else:
+            c = max(c for c in range(4) if Farr[c] <= p)
+            bwd.append(select(B[c], rank(H, p + 1) - rank(H, Farr[c])))
+    return dict(forward=fwd, backward=bwd)

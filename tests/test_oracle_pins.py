@@ -368,3 +368,89 @@ def test_mercy_bruteforce_and_strand_symmetry(k):
         assert got == _mercy([rc(r) for r in reads], k, 2)       # the same multiset from the other strand of every read
         hits += len(got)
     assert hits > 0 or k < 8        # tiny k: nearly every window is solid, gaps are rare
+
+
+# ---- traversal (oracle/sdbg_traverse.py; readings A24-A26) ------------------------------------------
+
+def _nav(reads, k, d):
+    from oracle.sdbg_traverse import navigation
+    res, f = _full(reads, k, d)
+    return res, f, navigation(f, k)
+
+
+def _random_reads(rng, k, n_src=3, n_reads=25):
+    from tests.helpers import rc
+    src = ["".join(rng.choice("ACGT") for _ in range(rng.randint(k + 1, k + 40))) for _ in range(n_src)]
+    reads = []
+    for _ in range(n_reads):
+        s = rng.choice(src)
+        a = rng.randint(0, len(s)); b = rng.randint(a, len(s))
+        reads.append(s[a:b] if rng.random() < 0.6 else rc(s[a:b]))
+    return reads
+
+
+@pytest.mark.parametrize("k", [2, 3, 5, 8, 11])
+def test_traversal_bruteforce_and_succinct_formulas(k):
+    """Two independent routes to the same maps: loops over node strings, and the rank/select formulas of Bowe et al.
+    evaluated on W / last / zin / F alone with counting loops. A wrong F boundary, a minus edge counted in a rank, a
+    zero-indegree node not skipped, or first/last edge mixed up fails one of them."""
+    import random
+    from tests.helpers import brute_force_navigation, boss_navigation
+    rng = random.Random(1409 + k)
+    seen_zin = seen_minus = 0
+    for trial in range(5):
+        reads = _random_reads(rng, k)
+        for d in (1, 2):
+            res, f, nav = _nav(reads, k, d)
+            F = [bytes(e).decode() for e in f["edges"]]
+            aux = [bytes(a).decode() for a in f["aux"]]
+            bf = brute_force_navigation(F, aux, k)
+            assert list(nav["zin"]) == bf["zin"] and list(nav["F"]) == bf["F"]
+            assert list(nav["forward"]) == bf["forward"] and list(nav["backward"]) == bf["backward"]
+            boss = boss_navigation([int(x) for x in f["W"]], [int(x) for x in f["last"]], bf["zin"], bf["F"])
+            assert boss["forward"] == bf["forward"] and boss["backward"] == bf["backward"]
+            assert int(nav["zin"].sum()) == f["t"]
+            seen_zin += f["t"]; seen_minus += int((f["W"] > 4).sum())
+    assert seen_zin > 0 and (seen_minus > 0 or k >= 8)   # minus edges need converging branches: rare in tiny graphs at large k
+
+
+def test_traversal_spells_a_read():
+    """Closed form: with d = 1 every window of a read is an edge, so starting at the node of its first k-mer and taking,
+    at every step, the edge labelled with the next base, forward() must visit the nodes read[j .. j+k) in order, and
+    backward() of each of them must name an edge that enters it."""
+    import random
+    rng = random.Random(5)
+    k = 7
+    read = "".join(rng.choice("ACGT") for _ in range(60))
+    res, f, nav = _nav([read, "".join(rng.choice("ACGT") for _ in range(40))], k, 1)
+    E = [bytes(e).decode() for e in f["edges"]]
+    first = {}
+    for i, e in enumerate(E):
+        first.setdefault(e[:k], i)
+    pos = first[read[:k]]
+    for j in range(len(read) - k):
+        assert E[pos][:k] == read[j:j + k]
+        i = pos
+        while E[i][:k] == read[j:j + k] and E[i][k] != read[j + k]:
+            i += 1
+        assert E[i] == read[j:j + k + 1]
+        nxt = int(nav["forward"][i])
+        assert E[nxt][:k] == read[j + 1:j + k + 1] and f["last"][nxt] == 1
+        b = int(nav["backward"][nxt])
+        assert b >= 0 and E[b][1:] == read[j + 1:j + k + 1]
+        pos = first[read[j + 1:j + k + 1]]
+
+
+def test_traversal_on_the_complete_de_bruijn_graph():
+    """Complete graph on 4^k nodes: no dummies, every node is entered by four edges; forward is onto the last edges,
+    each hit exactly four times, and backward(forward(i)) is the non-minus representative of edge i's target."""
+    from tests.helpers import de_bruijn
+    k = 3
+    res, f, nav = _nav([de_bruijn("ACGT", k + 1)], k, 2)
+    m = f["m"]
+    assert m == 4 ** (k + 1) and nav["F"] == [0, m // 4, m // 2, 3 * m // 4, m] and nav["zin"].sum() == 0
+    hits = np.bincount(nav["forward"], minlength=m)
+    assert np.array_equal(hits, 4 * f["last"].astype(np.int64))
+    rep = nav["backward"][nav["forward"]]
+    E = f["edges"]
+    assert np.all(f["W"][rep] <= 4) and np.all(E[rep][:, 1:] == E[:, 1:]) and np.all(rep <= np.arange(m))
