@@ -185,6 +185,10 @@ typedef struct {
     uint64_t m;            /* out: edges = solid edges + '$' edges */
     uint64_t t;            /* out: zero-indegree nodes */
     uint64_t n_zero_out;   /* out: '$' edges = nodes without outgoing edge */
+    uint64_t *zin_bits;    /* ceil(cap/64) u64, LSB first, tail bits zero: bit i = edge i is the last edge of a node without
+                              incoming edge, so that entry j of aux_bits is the node of the j-th set bit (reading A24) */
+    uint64_t F[5];         /* out (host): F[c] = index of the first edge whose node ends with a base >= c (A=0 .. T=3),
+                              F[4] = m: the F array of Bowe et al. in edge positions (reading A25) */
 } sdbg_full_graph;
 
 /* "Our implementation has added a bit-vector of length m to mark the validity of each edge ... and an auxiliary vector
@@ -196,7 +200,8 @@ typedef struct {
  *     bits [2k i, 2k (i+1)), bases in sequence order v[0..k) at 2 bits each, stream bit 0 = most significant bit of
  *     aux_bits[0]; no incoming dummy edges are made;
  *   - the arrays list solid and '$' edges together, sorted by (colex of the node, outgoing symbol), '$' < A;
- *     W / last / minus by the rules of sdbg_build ('$' edges: W = 0, last = 1, mult = 0); valid_bits = m ones.
+ *     W / last / minus by the rules of sdbg_build ('$' edges: W = 0, last = 1, mult = 0); valid_bits = m ones;
+ *   - zin_bits and F tie the auxiliary vector and the node classes to edge positions (A24, A25; used by sdbg_index_build).
  * `edges` must be sorted and distinct (the output of sdbg_count_edges), 2 <= k <= 127, fewer than 2^32 edges.
  * Synchronises the stream. Errors: SDBG_E_CAPACITY (out->m / out->t hold the needed values), SDBG_E_WORKSPACE
  * (needs about 40 + 16 w bytes of workspace per edge), SDBG_E_UNSUPPORTED, SDBG_E_INVAL. */
@@ -213,6 +218,41 @@ int sdbg_build_full(sdbg_ctx *ctx, const sdbg_edges *edges, sdbg_full_graph *out
  * merged, mult summed). Synchronises. Errors: SDBG_E_CAPACITY (out->n = needed count), SDBG_E_WORKSPACE,
  * SDBG_E_UNSUPPORTED, SDBG_E_INVAL. */
 int sdbg_mercy_edges(sdbg_ctx *ctx, const sdbg_reads *reads, const sdbg_edges *solid, sdbg_edges *out);
+
+/* ---- traversal: rank/select over the arrays of the full graph ------------------------- */
+
+/* "A succinct de Bruijn graph (SdBG) encodes a graph with m edges in O(m) bits, and supports O(1) time traversal from a
+ * vertex to its neighbors" (Bowe et al.). Readings A24-A26 of DESIGN.md. The index holds
+ * five bit-vectors over the m edges,
+ *     B_c[i] = (W[i] is base c, minus flag clear), c = A,C,G,T;     H[i] = last[i] and not zin[i],
+ * each as 64-byte cells {u64 ones before the cell, 448 bits}, so that a rank is one aligned 64-byte read, plus, per
+ * vector, the cell of every 512-th one for select. It borrows g->W and g->last_bits (they must outlive the index).
+ *     forward(i)  = -1 if W[i] == 0 ('$'), else the index of the last edge of the node e_i[1..k]
+ *                 = select_H(rank_H(F[c]) + rank_{B_c}(i + 1)),              c = base of W[i]
+ *     backward(j) = the smallest index of an edge that enters the node of edge j, -1 if the node has no incoming edge
+ *                 = select_{B_c}(rank_H(p + 1) - rank_H(F[c])),   p = last edge of j's node, c = its class in F
+ * The validity bits are not consulted. */
+typedef struct {
+    uint64_t *cells;        /* device, caller-owned: sdbg_index_bytes(cap) bytes, 64-byte aligned */
+    uint64_t bytes;         /* size of that block */
+    uint64_t m;             /* out: edges indexed */
+    uint64_t n_cells;       /* out: m / 448 + 1 */
+    uint64_t F[5];          /* out: copy of g->F */
+    uint64_t HF[5];         /* out: rank_H(F[c]) */
+    uint64_t ones[5];       /* out: set bits of B_A, B_C, B_G, B_T, H */
+    const uint8_t *W;       /* out: g->W (borrowed) */
+    const uint64_t *last_bits; /* out: g->last_bits (borrowed) */
+} sdbg_index;
+
+/* Bytes of `cells` for a graph of up to m edges. Host-only. */
+uint64_t sdbg_index_bytes(uint64_t m);
+/* Builds the index of g (the output of sdbg_build_full, zin_bits included) on the ctx stream; synchronises.
+ * Errors: SDBG_E_CAPACITY (ix->bytes too small), SDBG_E_INVAL (null arrays, no zin_bits), SDBG_E_UNSUPPORTED (m >= 2^32). */
+int sdbg_index_build(sdbg_ctx *ctx, const sdbg_full_graph *g, sdbg_index *ix);
+/* out[q] = forward(edge_idx[q]) / backward(edge_idx[q]) for n queries; edge_idx and out are DEVICE arrays; an index
+ * >= m yields -2. Launches on the ctx stream and does not synchronise. */
+int sdbg_forward(sdbg_ctx *ctx, const sdbg_index *ix, const uint64_t *edge_idx, uint64_t n, int64_t *out);
+int sdbg_backward(sdbg_ctx *ctx, const sdbg_index *ix, const uint64_t *edge_idx, uint64_t n, int64_t *out);
 
 /* ---- measurement hooks ---------------------------------------------------------------------------------- */
 

@@ -53,7 +53,13 @@ class _Graph(C.Structure):
 class _FullGraph(C.Structure):
     _fields_ = [("W", C.c_void_p), ("last_bits", C.c_void_p), ("valid_bits", C.c_void_p), ("mult", C.c_void_p),
                 ("aux_bits", C.c_void_p), ("cap", C.c_uint64), ("aux_cap", C.c_uint64), ("m", C.c_uint64),
-                ("t", C.c_uint64), ("n_zero_out", C.c_uint64)]
+                ("t", C.c_uint64), ("n_zero_out", C.c_uint64), ("zin_bits", C.c_void_p), ("F", C.c_uint64 * 5)]
+
+
+class _Index(C.Structure):
+    _fields_ = [("cells", C.c_void_p), ("bytes", C.c_uint64), ("m", C.c_uint64), ("n_cells", C.c_uint64),
+                ("F", C.c_uint64 * 5), ("HF", C.c_uint64 * 5), ("ones", C.c_uint64 * 5), ("W", C.c_void_p),
+                ("last_bits", C.c_void_p)]
 
 
 class _Timing(C.Structure):
@@ -89,6 +95,10 @@ def lib():
         L.sdbg_build.argtypes = [vp, C.POINTER(_Edges), u32, C.POINTER(_Graph)]; L.sdbg_build.restype = i32
         L.sdbg_build_full.argtypes = [vp, C.POINTER(_Edges), C.POINTER(_FullGraph)]; L.sdbg_build_full.restype = i32
         L.sdbg_mercy_edges.argtypes = [vp, C.POINTER(_Reads), C.POINTER(_Edges), C.POINTER(_Edges)]; L.sdbg_mercy_edges.restype = i32
+        L.sdbg_index_bytes.argtypes = [u64]; L.sdbg_index_bytes.restype = u64
+        L.sdbg_index_build.argtypes = [vp, C.POINTER(_FullGraph), C.POINTER(_Index)]; L.sdbg_index_build.restype = i32
+        L.sdbg_forward.argtypes = [vp, C.POINTER(_Index), vp, u64, vp]; L.sdbg_forward.restype = i32
+        L.sdbg_backward.argtypes = [vp, C.POINTER(_Index), vp, u64, vp]; L.sdbg_backward.restype = i32
         L.sdbg_ctx_set_timing.argtypes = [vp, i32]; L.sdbg_ctx_set_timing.restype = i32
         L.sdbg_ctx_get_timing.argtypes = [vp, C.POINTER(_Timing)]; L.sdbg_ctx_get_timing.restype = i32
         _lib = L
@@ -253,8 +263,9 @@ class FullGraph:
         self.valid_bits = torch.empty((max(cap, 1) + 63) // 64, dtype=torch.int64, device=dev)
         self.mult = torch.empty(max(cap, 1), dtype=torch.int32, device=dev)
         self.aux_bits = torch.empty((2 * k * max(aux_cap, 1) + 63) // 64, dtype=torch.int64, device=dev)
+        self.zin_bits = torch.empty((max(cap, 1) + 63) // 64, dtype=torch.int64, device=dev)
         self.c = _FullGraph(self.W.data_ptr(), self.last_bits.data_ptr(), self.valid_bits.data_ptr(), self.mult.data_ptr(),
-                            self.aux_bits.data_ptr(), cap, aux_cap, 0, 0, 0)
+                            self.aux_bits.data_ptr(), cap, aux_cap, 0, 0, 0, self.zin_bits.data_ptr())
 
     m = property(lambda self: self.c.m)
     t = property(lambda self: self.c.t)
@@ -274,6 +285,26 @@ class FullGraph:
 
     def aux_bits_np(self):
         return self.aux_bits[: (2 * self.k * self.t + 63) // 64].cpu().numpy().view(np.uint64)
+
+    def zin_bits_np(self):
+        return self.zin_bits[: (self.m + 63) // 64].cpu().numpy().view(np.uint64)
+
+    F = property(lambda self: [int(x) for x in self.c.F])
+
+
+class Index:
+    """Device block of sdbg_index for a graph of up to cap edges (rank/select cells; borrows the graph's W and last_bits)."""
+
+    def __init__(self, cap: int, device=None):
+        torch = _torch()
+        nbytes = lib().sdbg_index_bytes(cap)
+        self.cells = torch.empty((nbytes + 7) // 8, dtype=torch.int64, device=device or "cuda")
+        self.c = _Index(self.cells.data_ptr(), nbytes)
+        self.graph = None
+
+    m = property(lambda self: self.c.m)
+    ones = property(lambda self: [int(x) for x in self.c.ones])
+    HF = property(lambda self: [int(x) for x in self.c.HF])
 
 
 class Stats:
@@ -318,6 +349,24 @@ def sdbg_mercy_edges(ctx: Context, reads: Reads, solid: Edges, out: Edges) -> in
 def sdbg_build_full(ctx: Context, edges: Edges, out: FullGraph) -> int:
     ctx.check(lib().sdbg_build_full(ctx._h, C.byref(edges.c), C.byref(out.c)))
     return out.c.m
+
+
+def sdbg_index_bytes(m: int) -> int:
+    return lib().sdbg_index_bytes(m)
+
+
+def sdbg_index_build(ctx: Context, graph: FullGraph, out: Index) -> None:
+    ctx.check(lib().sdbg_index_build(ctx._h, C.byref(graph.c), C.byref(out.c)))
+    out.graph = graph                                    # the index borrows W and last_bits
+
+
+def sdbg_forward(ctx: Context, index: Index, edge_idx, n: int, out) -> None:
+    """edge_idx: n uint64/int64 on the device; out: n int64 on the device. Does not synchronise."""
+    ctx.check(lib().sdbg_forward(ctx._h, C.byref(index.c), _ptr(edge_idx), n, _ptr(out)))
+
+
+def sdbg_backward(ctx: Context, index: Index, edge_idx, n: int, out) -> None:
+    ctx.check(lib().sdbg_backward(ctx._h, C.byref(index.c), _ptr(edge_idx), n, _ptr(out)))
 
 
 def sdbg_build(ctx: Context, edges: Edges, flags: int, out: Graph) -> int:

@@ -237,3 +237,4 @@ int64_t sdbg_plan_ranges(const uint64_t *hist, uint64_t capacity, uint64_t *rang
 #include "api_count.inc"
 #include "api_build.inc"
 #include "api_full.inc"
+#include "api_index.inc"

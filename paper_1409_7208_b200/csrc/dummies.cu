@@ -208,7 +208,26 @@ __global__ void __launch_bounds__(256) merge_real_kernel(FullArgs a) {
         a.out_W[pos] = a.W_real[i];
         a.out_mult[pos] = a.mult_in[i];
         if ((a.last_real32[i >> 5] >> (i & 31)) & 1u) atomicOr(&a.out_last32[pos >> 5], 1u << (pos & 31));
+        if (a.out_zin32 && a.flag_in[i]) atomicOr(&a.out_zin32[pos >> 5], 1u << (pos & 31));
     }
+}
+
+// F[c] = first edge of the merged list whose node ends with a base >= c (A25): the node's last base is the first key
+// symbol, so it is a lower bound over the solid edges plus one over the `$` nodes. One thread per c.
+template <int W, int WT>
+__global__ void edge_F_kernel(FullArgs a) {
+    const u64 c = threadIdx.x;
+    u64 lo = 0, hi = a.n;
+    while (lo < hi) {
+        const u64 mid = lo + ((hi - lo) >> 1);
+        if ((a.keys[mid * W] >> 62) < c) lo = mid + 1; else hi = mid;
+    }
+    u64 lo2 = 0, hi2 = a.n_zero_out;
+    while (lo2 < hi2) {
+        const u64 mid = lo2 + ((hi2 - lo2) >> 1);
+        if ((a.tk[(u64)a.zout_idx[mid] * WT] >> 62) < c) lo2 = mid + 1; else hi2 = mid;
+    }
+    a.F_dev[c] = lo + lo2;
 }
 
 template <int W, int WT>
@@ -291,7 +310,8 @@ int launch_full_assemble(const FullArgs &a, u32 W_, u32 WT_, cudaStream_t s) {
     if (a.n == 0) return (int)cudaGetLastError();
     SDBG_DISPATCH_WWT(W_, WT_, (merge_real_kernel<W, WT><<<grid_for(a.n), 256, 0, s>>>(a),
                                 merge_dummy_kernel<W, WT><<<grid_for(a.n_zero_out), 256, 0, s>>>(a),
-                                aux_pack_kernel<W><<<grid_for(a.t), 256, 0, s>>>(a)));
+                                aux_pack_kernel<W><<<grid_for(a.t), 256, 0, s>>>(a),
+                                edge_F_kernel<W, WT><<<1, 4, 0, s>>>(a)));
     return (int)cudaGetLastError();
 }
 

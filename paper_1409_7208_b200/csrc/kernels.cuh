@@ -103,6 +103,8 @@ struct FullArgs {
     const u32 *zout_idx; u64 n_zero_out;                   // indices into tk of the nodes without outgoing edge
     const u32 *zin_idx; u64 t;                             // indices of edges whose node has no incoming edge
     uint8_t *out_W; u32 *out_last32; u64 *out_valid; u32 *out_mult; u64 *aux_bits;
+    const uint8_t *flag_in; u32 *out_zin32;                // per solid edge: last edge of a zero-indegree node -> zin bits (A24)
+    u64 *F_dev;                                            // u64[4] device scratch: F[0..3] of reading A25
 };
 int launch_target_keys(const u64 *keys, u64 n, u32 k, u32 W, u32 WT, u64 *out, cudaStream_t s);
 int launch_zero_flags(const u64 *keys, u64 n, u32 k, u32 W, u32 WT, const u64 *tk_sorted, const u32 *last_real32,
@@ -110,6 +112,19 @@ int launch_zero_flags(const u64 *keys, u64 n, u32 k, u32 W, u32 WT, const u64 *t
 u64 flag_scratch_bytes(u64 n);
 void launch_compact_flags(const uint8_t *flag, u64 n, u64 *scratch, u32 *out_idx, u64 *total_out, cudaStream_t s);
 int launch_full_assemble(const FullArgs &a, u32 W, u32 WT, cudaStream_t s);
+
+// traversal (rank.cu): rank/select cells over B_A, B_C, B_G, B_T, H and the forward / backward maps
+struct IndexView {
+    const u64 *cells; u64 n_cells, m;                      // vector v at cells + v * n_cells * 8 words
+    u32 *samples[5]; u64 n_samples[5];                     // cell of every 512-th one; (ones + 511) / 512 entries
+    u64 F[5], HF[5];                                       // F array (A25) and rank_H(F[c])
+    const uint8_t *W; const u64 *last_bits;                // borrowed from the graph
+};
+u64 index_cells(u64 m);
+u64 index_samples_cap(u64 m);
+void launch_index_build(const uint8_t *W, const u64 *last_bits, const u64 *zin_bits, const IndexView &ix, u64 *scalars /* u64[16] */, cudaStream_t s);
+void launch_forward(const IndexView &ix, const u64 *q, u64 n, long long *out, cudaStream_t s);
+void launch_backward(const IndexView &ix, const u64 *q, u64 n, long long *out, cudaStream_t s);
 
 // mercy-kmers (mercy.cu)
 struct MercyArgs {

@@ -1,0 +1,222 @@
+// rank.cu — rank/select over the arrays of the full graph and the two traversal maps built on them ("supports
+// O(1) time traversal from a vertex to its neighbors"; Bowe et al.; readings A24-A26).
+//
+// Five bit-vectors over the m edges: B_c = (W is base c, minus flag clear) for c = A,C,G,T, and H = last & ~zin. Each is
+// stored as 64-byte cells {u64 ones before the cell, 7 x 64 bits}: cell j covers edges [448 j, 448 j + 448), which are
+// words 7j .. 7j+6 of a plain bit-vector, so a rank is ONE aligned 64-byte read (two sectors of one line) and a
+// popcount of at most seven words. Select keeps, per vector, the cell of every 512-th one (a cell holds at most 448
+// ones, so at most one sample falls into a cell), binary-searches the count words of the few cells between two samples
+// and finishes inside the cell. A traversal query is a chain of three or four dependent random reads: the kernels are
+// latency/sector bound, one thread per query, nothing staged.
+#include "kernels.cuh"
+
+namespace sdbg {
+
+constexpr u32 kCellBits = 448, kCellWords = 8, kSelStep = 512;
+
+__device__ __forceinline__ const u64 *cell_ptr(const IndexView &ix, int v, u64 cell) {
+    return ix.cells + ((u64)v * ix.n_cells + cell) * kCellWords;
+}
+
+// ones of vector v at positions < x (x <= m)
+__device__ __forceinline__ u64 rank_v(const IndexView &ix, int v, u64 x) {
+    const u64 cell = x / kCellBits;
+    const u32 off = (u32)(x - cell * kCellBits);
+    const ulonglong2 *c2 = reinterpret_cast<const ulonglong2 *>(cell_ptr(ix, v, cell));
+    const ulonglong2 a = c2[0], b = c2[1], c = c2[2], d = c2[3];
+    const u64 w[7] = {a.y, b.x, b.y, c.x, c.y, d.x, d.y};
+    u64 r = a.x;
+#pragma unroll
+    for (u32 q = 0; q < 7; ++q) {
+        const int bits = (int)off - (int)(64 * q);
+        if (bits >= 64) r += __popcll(w[q]);
+        else if (bits > 0) r += __popcll(w[q] & (~0ull >> (64 - bits)));
+    }
+    return r;
+}
+
+// position of the r-th set bit of x (1 <= r <= popc(x)), LSB = position 0
+__device__ __forceinline__ u32 select_in_word(u64 x, u32 r) {
+    u32 pos = 0;
+#pragma unroll
+    for (u32 width = 32; width >= 1; width >>= 1) {
+        const u32 c = __popcll(x & ((1ull << width) - 1ull));
+        if (r > c) { r -= c; x >>= width; pos += width; }
+    }
+    return pos;
+}
+
+// position of the r-th one of vector v (1 <= r <= ones[v])
+__device__ __forceinline__ u64 select_v(const IndexView &ix, int v, u64 r) {
+    const u64 j = (r - 1) / kSelStep;
+    u64 lo = ix.samples[v][j];
+    u64 hi = (j + 1 < ix.n_samples[v]) ? ix.samples[v][j + 1] : ix.n_cells - 1;
+    while (lo < hi) {                                    // last cell whose count word is below r
+        const u64 mid = lo + ((hi - lo + 1) >> 1);
+        if (cell_ptr(ix, v, mid)[0] < r) lo = mid; else hi = mid - 1;
+    }
+    const ulonglong2 *c2 = reinterpret_cast<const ulonglong2 *>(cell_ptr(ix, v, lo));
+    const ulonglong2 a = c2[0], b = c2[1], c = c2[2], d = c2[3];
+    const u64 w[7] = {a.y, b.x, b.y, c.x, c.y, d.x, d.y};
+    u32 rem = (u32)(r - a.x);
+    u32 q = 0;
+    u64 word = w[0];
+#pragma unroll
+    for (u32 t = 0; t < 6; ++t) {
+        const u32 pc = __popcll(w[t]);
+        if (q == t && rem > pc) { rem -= pc; q = t + 1; word = w[t + 1]; }
+    }
+    return lo * kCellBits + 64ull * q + select_in_word(word, rem);
+}
+
+// ---- build ---------------------------------------------------------------------------------------------------------------
+// One thread per cell: 448 W bytes, seven words of last and zin -> seven words of each of the five vectors and their
+// popcounts (into word 0; scanned next).
+__global__ void __launch_bounds__(256) index_fill_kernel(const uint8_t *__restrict__ W, const u64 *__restrict__ last_bits,
+                                                         const u64 *__restrict__ zin_bits, u64 m, u64 n_cells, u64 *__restrict__ cells) {
+    const u64 n_words = (m + 63) / 64;
+    for (u64 cell = (u64)blockIdx.x * blockDim.x + threadIdx.x; cell < n_cells; cell += (u64)gridDim.x * blockDim.x) {
+        u64 cnt[5] = {0, 0, 0, 0, 0};
+        for (u32 q = 0; q < 7; ++q) {
+            const u64 wi = cell * 7 + q, e0 = wi * 64;
+            u64 bits[5] = {0, 0, 0, 0, 0};
+            if (e0 < m) {
+                const u32 lim = (u32)(m - e0 < 64 ? m - e0 : 64);
+                if (lim == 64) {
+                    const u64 *w8 = reinterpret_cast<const u64 *>(W + e0);   // e0 is a multiple of 64
+#pragma unroll
+                    for (u32 g = 0; g < 8; ++g) {
+                        const u64 x = w8[g];
+#pragma unroll
+                        for (u32 b = 0; b < 8; ++b) {
+                            const u32 lab = (u32)(x >> (8 * b)) & 0xffu;
+                            if (lab >= 1 && lab <= 4) bits[lab - 1] |= 1ull << (8 * g + b);
+                        }
+                    }
+                } else {
+                    for (u32 b = 0; b < lim; ++b) {
+                        const u32 lab = W[e0 + b];
+                        if (lab >= 1 && lab <= 4) bits[lab - 1] |= 1ull << b;
+                    }
+                }
+                if (wi < n_words) bits[4] = last_bits[wi] & ~zin_bits[wi];
+            }
+#pragma unroll
+            for (int v = 0; v < 5; ++v) {
+                cells[((u64)v * n_cells + cell) * kCellWords + 1 + q] = bits[v];
+                cnt[v] += __popcll(bits[v]);
+            }
+        }
+#pragma unroll
+        for (int v = 0; v < 5; ++v) cells[((u64)v * n_cells + cell) * kCellWords] = cnt[v];
+    }
+}
+
+// block v: exclusive scan of word 0 over the cells of vector v; totals[v] = ones of the vector
+__global__ void __launch_bounds__(1024) index_scan_kernel(u64 *cells, u64 n_cells, u64 *totals) {
+    __shared__ u64 s_w[32];
+    __shared__ u64 s_carry;
+    const u32 tid = threadIdx.x, lane = tid & 31u, warp = tid >> 5;
+    u64 *base = cells + (u64)blockIdx.x * n_cells * kCellWords;
+    if (tid == 0) s_carry = 0;
+    __syncthreads();
+    for (u64 b0 = 0; b0 < n_cells; b0 += 1024) {
+        const u64 i = b0 + tid;
+        const u64 v = i < n_cells ? base[i * kCellWords] : 0ull;
+        u64 incl = v;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            const u64 x = __shfl_up_sync(0xffffffffu, incl, o);
+            if (lane >= (u32)o) incl += x;
+        }
+        if (lane == 31) s_w[warp] = incl;
+        __syncthreads();
+        u64 off = s_carry;
+        for (u32 w = 0; w < warp; ++w) off += s_w[w];
+        if (i < n_cells) base[i * kCellWords] = off + incl - v;
+        __syncthreads();
+        if (tid == 1023) s_carry = off + incl;
+        __syncthreads();
+    }
+    if (tid == 0) totals[blockIdx.x] = s_carry;
+}
+
+// samples[v][j] = cell of the (512 j + 1)-th one of vector v
+__global__ void __launch_bounds__(256) index_samples_kernel(IndexView ix, const u64 *__restrict__ totals) {
+    const int v = blockIdx.y;
+    const u64 total = totals[v];
+    for (u64 cell = (u64)blockIdx.x * blockDim.x + threadIdx.x; cell < ix.n_cells; cell += (u64)gridDim.x * blockDim.x) {
+        const u64 before = cell_ptr(ix, v, cell)[0];
+        const u64 after = cell + 1 < ix.n_cells ? cell_ptr(ix, v, cell + 1)[0] : total;
+        const u64 j = (before + kSelStep - 1) / kSelStep;        // smallest j with 512 j + 1 > before
+        if (j * kSelStep + 1 <= after && after > before) ix.samples[v][j] = (u32)cell;
+    }
+}
+
+// consts[c] = rank_H(F[c]) for c = 0..4
+__global__ void index_consts_kernel(IndexView ix, u64 *consts) {
+    const u32 c = threadIdx.x;
+    if (c < 5) consts[c] = rank_v(ix, 4, ix.F[c]);
+}
+
+// ---- queries ---------------------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) forward_kernel(IndexView ix, const u64 *__restrict__ q, u64 n, long long *__restrict__ out) {
+    for (u64 t = (u64)blockIdx.x * blockDim.x + threadIdx.x; t < n; t += (u64)gridDim.x * blockDim.x) {
+        const u64 i = q[t];
+        long long r = -2;
+        if (i < ix.m) {
+            const u32 lab = ix.W[i];
+            r = -1;
+            if (lab) {
+                const u32 c = (lab - 1u) & 3u;
+                r = (long long)select_v(ix, 4, ix.HF[c] + rank_v(ix, (int)c, i + 1));
+            }
+        }
+        out[t] = r;
+    }
+}
+
+__global__ void __launch_bounds__(256) backward_kernel(IndexView ix, const u64 *__restrict__ q, u64 n, long long *__restrict__ out) {
+    for (u64 t = (u64)blockIdx.x * blockDim.x + threadIdx.x; t < n; t += (u64)gridDim.x * blockDim.x) {
+        const u64 j = q[t];
+        long long r = -2;
+        if (j < ix.m) {
+            u64 p = j;                                   // last edge of the node: at most four edges further on
+            u64 word = ix.last_bits[p >> 6] >> (p & 63);
+            if (word == 0) { p = (p | 63) + 1; word = ix.last_bits[p >> 6]; }
+            p += __ffsll((long long)word) - 1;
+            const u32 c = (p >= ix.F[1]) + (p >= ix.F[2]) + (p >= ix.F[3]);
+            const u64 upto = rank_v(ix, 4, p + 1);
+            const u64 before = rank_v(ix, 4, p);
+            r = -1;
+            if (upto != before) r = (long long)select_v(ix, (int)c, upto - ix.HF[c]);   // H[p] set: the node has an incoming edge
+        }
+        out[t] = r;
+    }
+}
+
+static unsigned grid_q(u64 n) {
+    u64 b = (n + 255) / 256;
+    if (b == 0) b = 1;
+    const u64 cap = (u64)kNumSMs * 32;
+    return (unsigned)(b < cap ? b : cap);
+}
+
+u64 index_cells(u64 m) { return m / kCellBits + 1; }
+u64 index_samples_cap(u64 m) { return m / kSelStep + 2; }
+
+void launch_index_build(const uint8_t *W, const u64 *last_bits, const u64 *zin_bits, const IndexView &ix, u64 *totals, cudaStream_t s) {
+    index_fill_kernel<<<grid_q(ix.n_cells), 256, 0, s>>>(W, last_bits, zin_bits, ix.m, ix.n_cells, const_cast<u64 *>(ix.cells));
+    index_scan_kernel<<<5, 1024, 0, s>>>(const_cast<u64 *>(ix.cells), ix.n_cells, totals);
+    index_samples_kernel<<<dim3(grid_q(ix.n_cells), 5), 256, 0, s>>>(ix, totals);
+    index_consts_kernel<<<1, 32, 0, s>>>(ix, totals + 8);
+}
+
+void launch_forward(const IndexView &ix, const u64 *q, u64 n, long long *out, cudaStream_t s) {
+    if (n) forward_kernel<<<grid_q(n), 256, 0, s>>>(ix, q, n, out);
+}
+void launch_backward(const IndexView &ix, const u64 *q, u64 n, long long *out, cudaStream_t s) {
+    if (n) backward_kernel<<<grid_q(n), 256, 0, s>>>(ix, q, n, out);
+}
+
+}  // namespace sdbg

@@ -249,8 +249,80 @@ def check_full_graph(res, w, n_nodes):
     vb = fg.valid_bits[:(m + 63) // 64]
     ones = ((vb.unsqueeze(1) >> torch.arange(64, device="cuda")) & 1).reshape(-1)
     assert int(ones[:m].sum()) == m and int(ones[m:].sum()) == 0
+    check_traversal(ctx, fg, ed, w, bits, real)
     ctx.close(); ctx.workspace = None
     return m, t
+
+
+def check_traversal(ctx, fg, ed, w, last, real, n_sample=1 << 22):
+    """sdbg_forward / sdbg_backward at full size (checked edge by edge against the oracle in tests/test_gpu_traverse.py
+    at sizes the oracle can hold): properties that pin the two maps without an oracle. For sampled edges q: forward(q)
+    is -1 exactly for '$' edges, else the last edge of a node that has an incoming edge; the first edge entering that
+    node carries the same base without the minus flag, does not come after q and has the same forward image; for
+    one-word keys the node of forward(q) IS e_q[1..k] (compared on the keys); backward is -1 exactly on the nodes of
+    the auxiliary vector, and forward(backward(p)) = p for the last edge p of every other sampled node."""
+    import torch
+    m, k = fg.m, w.k
+    ix = sd.Index(m)
+    sd.sdbg_index_build(ctx, fg, ix)
+    W = fg.W[:m]
+    zin = ((fg.zin_bits[:(m + 63) // 64].unsqueeze(1) >> torch.arange(64, device="cuda")) & 1).reshape(-1)[:m].bool()
+    assert int(zin.sum()) == fg.t and bool((last | ~zin).all())
+    F = fg.F
+    assert F[0] == 0 and F[4] == m and all(F[c] <= F[c + 1] for c in range(4))
+    assert ix.ones[4] == int(last.sum()) - fg.t
+    for c in range(4):
+        assert ix.ones[c] == int((W == c + 1).sum())
+    # BOSS counting property per class: has-incoming nodes ending with c == edges labelled c without the minus flag
+    H = last & ~zin
+    for c in range(4):
+        assert int(H[F[c]:F[c + 1]].sum()) == ix.ones[c], c
+    g = torch.Generator(device="cuda"); g.manual_seed(w.seed)
+    q = torch.randint(0, m, (min(n_sample, 4 * m),), device="cuda", generator=g)
+    f = torch.empty_like(q); b = torch.empty_like(q); f2 = torch.empty_like(q)
+    sd.sdbg_forward(ctx, ix, q, q.numel(), f)
+    torch.cuda.synchronize()
+    isreal = real[q]
+    assert bool((f[~isreal] == -1).all()) and bool((f[isreal] >= 0).all())
+    qr, fr = q[isreal], f[isreal].contiguous()
+    assert bool(H[fr].all())
+    br = torch.empty_like(fr)
+    sd.sdbg_backward(ctx, ix, fr, fr.numel(), br)
+    torch.cuda.synchronize()
+    assert bool((br >= 0).all()) and bool((br <= qr).all())
+    assert bool((W[br] == ((W[qr] - 1) & 3) + 1).all())
+    f2 = torch.empty_like(br)
+    sd.sdbg_forward(ctx, ix, br, br.numel(), f2)
+    torch.cuda.synchronize()
+    assert torch.equal(f2, fr)
+    if ed.w == 1:                                        # the node of forward(q) is e_q[1..k], on the keys themselves
+        rank_real = torch.cumsum(real, 0) - 1
+        keys = ed.keys[:ed.n]
+        pad = 64 - 2 * (k + 1)
+        mask2k = (1 << (2 * k)) - 1
+        kq = keys[rank_real[qr]]
+        node_q = (kq >> (64 - 2 * k)) & mask2k
+        tgt = (((kq >> pad) & 3) << (2 * (k - 1))) | (node_q >> 2)
+        to_real = real[fr]
+        kf = keys[rank_real[fr[to_real]]]
+        assert torch.equal((kf >> (64 - 2 * k)) & mask2k, tgt[to_real])
+        # a '$' image: the node has no real edge, so its predecessor and successor nodes in the list differ from tgt
+        del rank_real
+    # backward on the nodes of the auxiliary vector and on sampled other nodes
+    zpos = torch.nonzero(zin).reshape(-1)[:n_sample].contiguous()
+    if zpos.numel():
+        bz = torch.empty_like(zpos)
+        sd.sdbg_backward(ctx, ix, zpos, zpos.numel(), bz)
+        torch.cuda.synchronize()
+        assert bool((bz == -1).all())
+    hp = q[H[q]].contiguous()
+    bh = torch.empty_like(hp); fh = torch.empty_like(hp)
+    sd.sdbg_backward(ctx, ix, hp, hp.numel(), bh)
+    torch.cuda.synchronize()
+    assert bool((bh >= 0).all())
+    sd.sdbg_forward(ctx, ix, bh, bh.numel(), fh)
+    torch.cuda.synchronize()
+    assert torch.equal(fh, hp)
 
 
 def check_mercy(res, w, reads):
