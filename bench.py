@@ -272,8 +272,9 @@ def run_gpu(args, w):
 
 
 def run_next_rows(args, w):
-    """`--next`: the two widened rows (DESIGN.md §0 f-1, f-2) on the same workload, timed by CUDA events around the
-    C-ABI calls: sdbg_build_full and sdbg_mercy_edges over the solid edges of one sdbg_count_edges run. Not part of
+    """`--next`: the widened rows (DESIGN.md §0 f-1, f-2, f-3) on the same workload, timed by CUDA events around the
+    C-ABI calls: sdbg_build_full, sdbg_mercy_edges, sdbg_index_build and the two
+    traversal maps over the solid edges of one sdbg_count_edges run. Not part of
     the step that `value` measures."""
     import torch
     import paper_1409_7208_b200 as sd
@@ -316,7 +317,20 @@ def run_next_rows(args, w):
 
     ms_full = timed(lambda: sd.sdbg_build_full(ctx, edges, fg))
     ms_mercy = timed(lambda: sd.sdbg_mercy_edges(ctx, reads, edges, me))
+    # traversal (f-3): index build, then 2^24 random forward / backward queries (indices and answers resident in HBM)
+    ix = sd.Index(fg.m)
+    ms_index = timed(lambda: sd.sdbg_index_build(ctx, fg, ix))
+    nq = 1 << 24
+    gen = torch.Generator(device="cuda"); gen.manual_seed(w.seed)
+    q = torch.randint(0, max(int(fg.m), 1), (nq,), device="cuda", generator=gen)
+    ans = torch.empty(nq, dtype=torch.int64, device="cuda")
+    ms_fwd = timed(lambda: sd.sdbg_forward(ctx, ix, q, nq, ans))
+    ms_bwd = timed(lambda: sd.sdbg_backward(ctx, ix, q, nq, ans))
+    trav = {"index_build_ms": ms_index, "index_bytes": int(sd.sdbg_index_bytes(fg.m)), "queries": nq,
+            "forward_ms": ms_fwd, "forward_queries_per_s": nq / (ms_fwd * 1e-3),
+            "backward_ms": ms_bwd, "backward_queries_per_s": nq / (ms_bwd * 1e-3)}
     print(json.dumps({"impl": "next_rows", "config": {"workload": w.name, "k": w.k, "d": w.d, "solid_edges": int(S)},
+                      "traversal": trav,
                       "sdbg_build_full": {"ms": ms_full, "m": int(fg.m), "t": int(fg.t), "dollar_edges": int(fg.n_zero_out),
                                           "solid_edges_per_s": S / (ms_full * 1e-3)},
                       "sdbg_mercy_edges": {"ms": ms_mercy, "mercy_records": int(me.n),

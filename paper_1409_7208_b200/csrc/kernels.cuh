@@ -122,7 +122,8 @@ struct IndexView {
 };
 u64 index_cells(u64 m);
 u64 index_samples_cap(u64 m);
-void launch_index_build(const uint8_t *W, const u64 *last_bits, const u64 *zin_bits, const IndexView &ix, u64 *scalars /* u64[16] */, cudaStream_t s);
+u64 index_scratch_words(u64 m);
+void launch_index_build(const uint8_t *W, const u64 *last_bits, const u64 *zin_bits, const IndexView &ix, u64 *scratch /* u64[index_scratch_words(m)] */, cudaStream_t s);
 void launch_forward(const IndexView &ix, const u64 *q, u64 n, long long *out, cudaStream_t s);
 void launch_backward(const IndexView &ix, const u64 *q, u64 n, long long *out, cudaStream_t s);
 

@@ -70,59 +70,82 @@ __device__ __forceinline__ u64 select_v(const IndexView &ix, int v, u64 r) {
 }
 
 // ---- build ---------------------------------------------------------------------------------------------------------------
-// One thread per cell: 448 W bytes, seven words of last and zin -> seven words of each of the five vectors and their
-// popcounts (into word 0; scanned next).
-__global__ void __launch_bounds__(256) index_fill_kernel(const uint8_t *__restrict__ W, const u64 *__restrict__ last_bits,
-                                                         const u64 *__restrict__ zin_bits, u64 m, u64 n_cells, u64 *__restrict__ cells) {
+// 64 cells per block. Fill: one thread per 64-edge word (a warp reads 2 KiB of W in a row), seven words make a cell, so
+// the 448 threads of a block fill exactly 64 cells; popcounts meet in shared memory, word 0 of a cell gets its count and
+// the block its five sums. Then a one-block scan of the block sums, and a finish kernel that scans the 64 counts of a
+// block in place and lets every cell that holds a (512 j + 1)-th one write its select sample.
+constexpr u32 kIndexBlock = 64, kFillThreads = 7 * kIndexBlock;
+
+__global__ void __launch_bounds__(kFillThreads) index_fill_kernel(const uint8_t *__restrict__ W, const u64 *__restrict__ last_bits,
+                                                                  const u64 *__restrict__ zin_bits, u64 m, u64 n_cells, u64 *__restrict__ cells,
+                                                                  u64 *__restrict__ block_sums /* [5][gridDim.x] */) {
+    __shared__ uint8_t s_pc[5][kFillThreads];
+    __shared__ u32 s_sum[5][kIndexBlock / 32];
     const u64 n_words = (m + 63) / 64;
-    for (u64 cell = (u64)blockIdx.x * blockDim.x + threadIdx.x; cell < n_cells; cell += (u64)gridDim.x * blockDim.x) {
-        u64 cnt[5] = {0, 0, 0, 0, 0};
-        for (u32 q = 0; q < 7; ++q) {
-            const u64 wi = cell * 7 + q, e0 = wi * 64;
-            u64 bits[5] = {0, 0, 0, 0, 0};
-            if (e0 < m) {
-                const u32 lim = (u32)(m - e0 < 64 ? m - e0 : 64);
-                if (lim == 64) {
-                    const u64 *w8 = reinterpret_cast<const u64 *>(W + e0);   // e0 is a multiple of 64
+    const u32 tid = threadIdx.x;
+    const u64 wi = (u64)blockIdx.x * kFillThreads + tid, e0 = wi * 64;
+    const u64 cell = (u64)blockIdx.x * kIndexBlock + tid / 7;
+    u64 bits[5] = {0, 0, 0, 0, 0};
+    if (e0 < m) {
+        const u32 lim = (u32)(m - e0 < 64 ? m - e0 : 64);
+        if (lim == 64) {
+            const u64 *w8 = reinterpret_cast<const u64 *>(W + e0);           // e0 is a multiple of 64
 #pragma unroll
-                    for (u32 g = 0; g < 8; ++g) {
-                        const u64 x = w8[g];
+            for (u32 g = 0; g < 8; ++g) {
+                const u64 x = w8[g];
 #pragma unroll
-                        for (u32 b = 0; b < 8; ++b) {
-                            const u32 lab = (u32)(x >> (8 * b)) & 0xffu;
-                            if (lab >= 1 && lab <= 4) bits[lab - 1] |= 1ull << (8 * g + b);
-                        }
-                    }
-                } else {
-                    for (u32 b = 0; b < lim; ++b) {
-                        const u32 lab = W[e0 + b];
-                        if (lab >= 1 && lab <= 4) bits[lab - 1] |= 1ull << b;
-                    }
+                for (u32 b = 0; b < 8; ++b) {
+                    const u32 lab = (u32)(x >> (8 * b)) & 0xffu;
+#pragma unroll
+                    for (u32 c = 0; c < 4; ++c) bits[c] |= (u64)(lab == c + 1) << (8 * g + b);   // no dynamic index: registers
                 }
-                if (wi < n_words) bits[4] = last_bits[wi] & ~zin_bits[wi];
             }
+        } else {
+            for (u32 b = 0; b < lim; ++b) {
+                const u32 lab = W[e0 + b];
 #pragma unroll
-            for (int v = 0; v < 5; ++v) {
-                cells[((u64)v * n_cells + cell) * kCellWords + 1 + q] = bits[v];
-                cnt[v] += __popcll(bits[v]);
+                for (u32 c = 0; c < 4; ++c) bits[c] |= (u64)(lab == c + 1) << b;
             }
         }
+        if (wi < n_words) bits[4] = last_bits[wi] & ~zin_bits[wi];
+    }
 #pragma unroll
-        for (int v = 0; v < 5; ++v) cells[((u64)v * n_cells + cell) * kCellWords] = cnt[v];
+    for (int v = 0; v < 5; ++v) {
+        if (cell < n_cells) cells[((u64)v * n_cells + cell) * kCellWords + 1 + tid % 7] = bits[v];
+        s_pc[v][tid] = (uint8_t)__popcll(bits[v]);
+    }
+    __syncthreads();
+    if (tid < 5 * kIndexBlock) {                         // five groups of 64 threads: the counts of the 64 cells of vector v
+        const u32 v = tid / kIndexBlock, lc = tid % kIndexBlock;
+        u32 cnt = 0;
+#pragma unroll
+        for (u32 q = 0; q < 7; ++q) cnt += s_pc[v][7 * lc + q];
+        const u64 c = (u64)blockIdx.x * kIndexBlock + lc;
+        if (c < n_cells) cells[((u64)v * n_cells + c) * kCellWords] = cnt;
+        u32 x = cnt;
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) x += __shfl_xor_sync(0xffffffffu, x, o);
+        if ((tid & 31u) == 0) s_sum[v][(tid % kIndexBlock) >> 5] = x;
+    }
+    __syncthreads();
+    if (tid < 5) {
+        u64 t = 0;
+        for (u32 w = 0; w < kIndexBlock / 32; ++w) t += s_sum[tid][w];
+        block_sums[(u64)tid * gridDim.x + blockIdx.x] = t;
     }
 }
 
-// block v: exclusive scan of word 0 over the cells of vector v; totals[v] = ones of the vector
-__global__ void __launch_bounds__(1024) index_scan_kernel(u64 *cells, u64 n_cells, u64 *totals) {
+// block v: exclusive scan of the block sums of vector v; totals[v] = ones of the vector
+__global__ void __launch_bounds__(1024) index_scan_kernel(u64 *block_sums, u32 nblocks, u64 *totals) {
     __shared__ u64 s_w[32];
     __shared__ u64 s_carry;
     const u32 tid = threadIdx.x, lane = tid & 31u, warp = tid >> 5;
-    u64 *base = cells + (u64)blockIdx.x * n_cells * kCellWords;
+    u64 *base = block_sums + (u64)blockIdx.x * nblocks;
     if (tid == 0) s_carry = 0;
     __syncthreads();
-    for (u64 b0 = 0; b0 < n_cells; b0 += 1024) {
-        const u64 i = b0 + tid;
-        const u64 v = i < n_cells ? base[i * kCellWords] : 0ull;
+    for (u32 b0 = 0; b0 < nblocks; b0 += 1024) {
+        const u32 i = b0 + tid;
+        const u64 v = i < nblocks ? base[i] : 0ull;
         u64 incl = v;
 #pragma unroll
         for (int o = 1; o < 32; o <<= 1) {
@@ -133,7 +156,7 @@ __global__ void __launch_bounds__(1024) index_scan_kernel(u64 *cells, u64 n_cell
         __syncthreads();
         u64 off = s_carry;
         for (u32 w = 0; w < warp; ++w) off += s_w[w];
-        if (i < n_cells) base[i * kCellWords] = off + incl - v;
+        if (i < nblocks) base[i] = off + incl - v;
         __syncthreads();
         if (tid == 1023) s_carry = off + incl;
         __syncthreads();
@@ -141,15 +164,28 @@ __global__ void __launch_bounds__(1024) index_scan_kernel(u64 *cells, u64 n_cell
     if (tid == 0) totals[blockIdx.x] = s_carry;
 }
 
-// samples[v][j] = cell of the (512 j + 1)-th one of vector v
-__global__ void __launch_bounds__(256) index_samples_kernel(IndexView ix, const u64 *__restrict__ totals) {
-    const int v = blockIdx.y;
-    const u64 total = totals[v];
-    for (u64 cell = (u64)blockIdx.x * blockDim.x + threadIdx.x; cell < ix.n_cells; cell += (u64)gridDim.x * blockDim.x) {
-        const u64 before = cell_ptr(ix, v, cell)[0];
-        const u64 after = cell + 1 < ix.n_cells ? cell_ptr(ix, v, cell + 1)[0] : total;
+// word 0 of every cell: count -> ones before the cell; samples[v][j] = cell of the (512 j + 1)-th one of vector v
+__global__ void __launch_bounds__(kIndexBlock) index_finish_kernel(IndexView ix, const u64 *__restrict__ block_sums) {
+    __shared__ u32 s_w[5][kIndexBlock / 32];
+    const u32 lane = threadIdx.x & 31u, warp = threadIdx.x >> 5;
+    const u64 cell = (u64)blockIdx.x * kIndexBlock + threadIdx.x;
+    u64 *cells = const_cast<u64 *>(ix.cells);
+    u32 cnt[5], incl[5];
+#pragma unroll
+    for (int v = 0; v < 5; ++v) {
+        cnt[v] = cell < ix.n_cells ? (u32)cells[((u64)v * ix.n_cells + cell) * kCellWords] : 0u;
+        incl[v] = warp_incl_scan_add(cnt[v]);
+        if (lane == 31) s_w[v][warp] = incl[v];
+    }
+    __syncthreads();
+    if (cell >= ix.n_cells) return;
+#pragma unroll
+    for (int v = 0; v < 5; ++v) {
+        u64 before = block_sums[(u64)v * gridDim.x + blockIdx.x] + incl[v] - cnt[v];
+        for (u32 w = 0; w < warp; ++w) before += s_w[v][w];
+        cells[((u64)v * ix.n_cells + cell) * kCellWords] = before;
         const u64 j = (before + kSelStep - 1) / kSelStep;        // smallest j with 512 j + 1 > before
-        if (j * kSelStep + 1 <= after && after > before) ix.samples[v][j] = (u32)cell;
+        if (cnt[v] && j * kSelStep + 1 <= before + cnt[v]) ix.samples[v][j] = (u32)cell;
     }
 }
 
@@ -205,11 +241,16 @@ static unsigned grid_q(u64 n) {
 u64 index_cells(u64 m) { return m / kCellBits + 1; }
 u64 index_samples_cap(u64 m) { return m / kSelStep + 2; }
 
-void launch_index_build(const uint8_t *W, const u64 *last_bits, const u64 *zin_bits, const IndexView &ix, u64 *totals, cudaStream_t s) {
-    index_fill_kernel<<<grid_q(ix.n_cells), 256, 0, s>>>(W, last_bits, zin_bits, ix.m, ix.n_cells, const_cast<u64 *>(ix.cells));
-    index_scan_kernel<<<5, 1024, 0, s>>>(const_cast<u64 *>(ix.cells), ix.n_cells, totals);
-    index_samples_kernel<<<dim3(grid_q(ix.n_cells), 5), 256, 0, s>>>(ix, totals);
-    index_consts_kernel<<<1, 32, 0, s>>>(ix, totals + 8);
+u64 index_scratch_words(u64 m) { return 5 * ((index_cells(m) + kIndexBlock - 1) / kIndexBlock) + 16; }
+
+// scratch: u64[index_scratch_words(m)]: 16 scalars (ones of the five vectors at [0..4], rank_H(F[c]) at [8..12]), block sums
+void launch_index_build(const uint8_t *W, const u64 *last_bits, const u64 *zin_bits, const IndexView &ix, u64 *scratch, cudaStream_t s) {
+    const u32 nblocks = (u32)((ix.n_cells + kIndexBlock - 1) / kIndexBlock);
+    u64 *block_sums = scratch + 16;
+    index_fill_kernel<<<nblocks, kFillThreads, 0, s>>>(W, last_bits, zin_bits, ix.m, ix.n_cells, const_cast<u64 *>(ix.cells), block_sums);
+    index_scan_kernel<<<5, 1024, 0, s>>>(block_sums, nblocks, scratch);
+    index_finish_kernel<<<nblocks, kIndexBlock, 0, s>>>(ix, block_sums);
+    index_consts_kernel<<<1, 32, 0, s>>>(ix, scratch + 8);
 }
 
 void launch_forward(const IndexView &ix, const u64 *q, u64 n, long long *out, cudaStream_t s) {
