@@ -9,7 +9,7 @@
 //   Z_out = tgt(S) \ src(S)  (binary search of every distinct target in the edge list)   -> one `$` edge per node
 //   Z_in  = src(S) \ tgt(S)  (binary search of every node of the edge list in the targets) -> auxiliary vector
 // and the final arrays are the emitted arrays of S with the `$` edges merged in by node order (a `$` edge changes no
-// flag of a real edge: it has a node of its own and no outgoing base).
+// flag of a real edge: it has a node of its own and no outgoing base), written one output position per thread.
 #include "kernels.cuh"
 
 namespace sdbg {
@@ -52,10 +52,26 @@ __global__ void __launch_bounds__(256) target_keys_kernel(const u64 *__restrict_
     }
 }
 
+// Prefix index over a sorted key list (records of `stride` words): idx[b] = first record whose top pb bits are >= b, for
+// b = 0 .. 2^pb (idx[2^pb] = n). The searches below start inside one bucket (a few hundred records for 2^20 buckets)
+// instead of the whole list: ~9 steps over neighbouring lines instead of ~28 over gigabytes.
+__global__ void __launch_bounds__(256) prefix_index_kernel(const u64 *__restrict__ a, u64 n, u32 stride, u32 pb, u32 *__restrict__ idx) {
+    const u64 b = (u64)blockIdx.x * blockDim.x + threadIdx.x;
+    if (b > (1ull << pb)) return;
+    u64 lo = 0, hi = n;
+    if (b == (1ull << pb)) lo = n;
+    else
+        while (lo < hi) {
+            const u64 mid = lo + ((hi - lo) >> 1);
+            if ((a[mid * stride] >> (64 - pb)) < b) lo = mid + 1; else hi = mid;
+        }
+    idx[b] = (u32)lo;
+}
+
 // flag_out[j] = tk[j] is the first of its value and no edge has it as its node; tk sorted
 template <int W, int WT>
 __global__ void __launch_bounds__(256) flag_zero_out_kernel(const u64 *__restrict__ tk, u64 n, const u64 *__restrict__ keys, u32 k,
-                                                            uint8_t *__restrict__ flag) {
+                                                            const u32 *__restrict__ idx_edges, u32 pb, uint8_t *__restrict__ flag) {
     for (u64 j = (u64)blockIdx.x * blockDim.x + threadIdx.x; j < n; j += (u64)gridDim.x * blockDim.x) {
         u64 v[WT];
         ld_rec<WT>(tk, j, v);
@@ -68,14 +84,16 @@ __global__ void __launch_bounds__(256) flag_zero_out_kernel(const u64 *__restric
         }
         bool is_src = false;
         if (head) {
-            u64 lo = 0, hi = n;                          // first edge whose node is not less than v
+            const u64 b = v[0] >> (64 - pb);
+            u64 lo = idx_edges[b], hi = idx_edges[b + 1];  // first edge whose node is not less than v: inside v's bucket
+            const u64 end = hi;
             while (lo < hi) {
                 const u64 mid = lo + ((hi - lo) >> 1);
                 u64 e[W];
                 ld_rec<W>(keys, mid, e);
                 if (node_cmp<W, WT>(e, v, k) < 0) lo = mid + 1; else hi = mid;
             }
-            if (lo < n) {
+            if (lo < end) {
                 u64 e[W];
                 ld_rec<W>(keys, lo, e);
                 is_src = node_cmp<W, WT>(e, v, k) == 0;
@@ -88,13 +106,16 @@ __global__ void __launch_bounds__(256) flag_zero_out_kernel(const u64 *__restric
 // flag_in[i] = edge i is the last edge of its node and no target equals that node
 template <int W, int WT>
 __global__ void __launch_bounds__(256) flag_zero_in_kernel(const u64 *__restrict__ keys, u64 n, const u32 *__restrict__ last_bits32,
-                                                           const u64 *__restrict__ tk, u32 k, uint8_t *__restrict__ flag) {
+                                                           const u64 *__restrict__ tk, u32 k, const u32 *__restrict__ idx_tk, u32 pb,
+                                                           uint8_t *__restrict__ flag) {
     for (u64 i = (u64)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (u64)gridDim.x * blockDim.x) {
         bool z = false;
         if ((last_bits32[i >> 5] >> (i & 31)) & 1u) {
             u64 e[W];
             ld_rec<W>(keys, i, e);
-            u64 lo = 0, hi = n;                          // first target that is not less than the node
+            const u64 b = e[0] >> (64 - pb);             // pb <= 2k: only node bits
+            u64 lo = idx_tk[b], hi = idx_tk[b + 1];      // first target that is not less than the node: inside its bucket
+            const u64 end = hi;
             while (lo < hi) {
                 const u64 mid = lo + ((hi - lo) >> 1);
                 u64 v[WT];
@@ -102,7 +123,7 @@ __global__ void __launch_bounds__(256) flag_zero_in_kernel(const u64 *__restrict
                 if (node_cmp<W, WT>(e, v, k) > 0) lo = mid + 1; else hi = mid;
             }
             z = true;
-            if (lo < n) {
+            if (lo < end) {
                 u64 v[WT];
                 ld_rec<WT>(tk, lo, v);
                 z = node_cmp<W, WT>(e, v, k) != 0;
@@ -192,23 +213,70 @@ void launch_compact_flags(const uint8_t *flag, u64 n, u64 *scratch, u32 *out_idx
 namespace sdbg {
 
 // ---- final arrays: the emitted arrays of the real edges with the `$` edges merged in by node order ------------------------
+// A `$` edge j goes behind the real edges whose node is less than its own (never equal: it has no real edge) and behind
+// the j dummies before it: dpos[j] = j + lower bound of its node in the edge list, strictly increasing, t entries of
+// 4 bytes (L2-resident).
 template <int W, int WT>
-__global__ void __launch_bounds__(256) merge_real_kernel(FullArgs a) {
-    for (u64 i = (u64)blockIdx.x * blockDim.x + threadIdx.x; i < a.n; i += (u64)gridDim.x * blockDim.x) {
-        u64 e[W];
-        ld_rec<W>(a.keys, i, e);
-        u64 lo = 0, hi = a.n_zero_out;                   // `$` edges whose node is less than mine come before me
+__global__ void __launch_bounds__(256) dummy_pos_kernel(FullArgs a) {
+    for (u64 j = (u64)blockIdx.x * blockDim.x + threadIdx.x; j < a.n_zero_out; j += (u64)gridDim.x * blockDim.x) {
+        u64 v[WT];
+        ld_rec<WT>(a.tk, a.zout_idx[j], v);
+        u64 lo = 0, hi = a.n;
         while (lo < hi) {
             const u64 mid = lo + ((hi - lo) >> 1);
-            u64 v[WT];
-            ld_rec<WT>(a.tk, a.zout_idx[mid], v);
-            if (node_cmp<W, WT>(e, v, a.k) > 0) lo = mid + 1; else hi = mid;
+            u64 e[W];
+            ld_rec<W>(a.keys, mid, e);
+            if (node_cmp<W, WT>(e, v, a.k) < 0) lo = mid + 1; else hi = mid;
         }
-        const u64 pos = i + lo;
-        a.out_W[pos] = a.W_real[i];
-        a.out_mult[pos] = a.mult_in[i];
-        if ((a.last_real32[i >> 5] >> (i & 31)) & 1u) atomicOr(&a.out_last32[pos >> 5], 1u << (pos & 31));
-        if (a.out_zin32 && a.flag_in[i]) atomicOr(&a.out_zin32[pos >> 5], 1u << (pos & 31));
+        a.dpos[j] = (u32)(j + lo);
+    }
+}
+
+// One thread per OUTPUT position p, one warp per chunk of 1,024 consecutive positions: a warp-uniform lower bound over
+// dpos at the start of the chunk, then the chunk is walked in windows of 32 positions; the (at most 32) dummies inside a
+// window come as one coalesced load and a bit mask, which tells every lane whether it is a `$` edge and which real
+// edge it holds otherwise, and advances the bound. The last and zin words are assembled by ballots, 32 positions per
+// store: no atomic and no memset (every word up to ceil(m/64) u64 words is written, tail bits zero).
+constexpr u32 kAsmChunk = 1024;
+
+__global__ void __launch_bounds__(256) assemble_kernel(FullArgs a) {
+    const u64 m = a.n + a.n_zero_out, padded = (m + 63) / 64 * 64;
+    const u32 lane = threadIdx.x & 31u;
+    const u64 n_chunks = (padded + kAsmChunk - 1) / kAsmChunk;
+    for (u64 chunk = (u64)blockIdx.x * 8 + (threadIdx.x >> 5); chunk < n_chunks; chunk += (u64)gridDim.x * 8) {
+        const u64 c0 = chunk * kAsmChunk;
+        u64 lo0 = 0, hi = a.n_zero_out;
+        while (lo0 < hi) {
+            const u64 mid = lo0 + ((hi - lo0) >> 1);
+            if (a.dpos[mid] < c0) lo0 = mid + 1; else hi = mid;
+        }
+        for (u64 p0 = c0; p0 < c0 + kAsmChunk && p0 < padded; p0 += 32) {
+            const u64 p = p0 + lane, jd = lo0 + lane;
+            const u64 d = jd < a.n_zero_out ? a.dpos[jd] : ~0ull;
+            const u32 dmask = __reduce_or_sync(0xffffffffu, d - p0 < 32 ? 1u << (u32)(d - p0) : 0u);
+            bool last = false, zin = false;
+            if (p < m) {
+                const bool dummy = (dmask >> lane) & 1u;
+                const u64 i = p - (lo0 + __popc(dmask & lanemask_lt()));
+                uint8_t w = 0;
+                u32 mult = 0;
+                last = true;                             // a `$` edge is the only edge of its node
+                if (!dummy) {
+                    w = a.W_real[i];
+                    mult = a.mult_in[i];
+                    last = (a.last_real32[i >> 5] >> (i & 31)) & 1u;
+                    zin = a.flag_in[i] != 0;
+                }
+                a.out_W[p] = w;
+                a.out_mult[p] = mult;
+            }
+            const u32 lw = __ballot_sync(0xffffffffu, last), zw = __ballot_sync(0xffffffffu, zin);
+            if (lane == 0) {
+                a.out_last32[p0 >> 5] = lw;
+                if (a.out_zin32) a.out_zin32[p0 >> 5] = zw;
+            }
+            lo0 += __popc(dmask);
+        }
     }
 }
 
@@ -228,25 +296,6 @@ __global__ void edge_F_kernel(FullArgs a) {
         if ((a.tk[(u64)a.zout_idx[mid] * WT] >> 62) < c) lo2 = mid + 1; else hi2 = mid;
     }
     a.F_dev[c] = lo + lo2;
-}
-
-template <int W, int WT>
-__global__ void __launch_bounds__(256) merge_dummy_kernel(FullArgs a) {
-    for (u64 j = (u64)blockIdx.x * blockDim.x + threadIdx.x; j < a.n_zero_out; j += (u64)gridDim.x * blockDim.x) {
-        u64 v[WT];
-        ld_rec<WT>(a.tk, a.zout_idx[j], v);
-        u64 lo = 0, hi = a.n;                            // real edges whose node is less than mine come before me
-        while (lo < hi) {
-            const u64 mid = lo + ((hi - lo) >> 1);
-            u64 e[W];
-            ld_rec<W>(a.keys, mid, e);
-            if (node_cmp<W, WT>(e, v, a.k) < 0) lo = mid + 1; else hi = mid;
-        }
-        const u64 pos = j + lo;
-        a.out_W[pos] = 0;                                // '$'
-        a.out_mult[pos] = 0;
-        atomicOr(&a.out_last32[pos >> 5], 1u << (pos & 31));   // the only edge of its node
-    }
 }
 
 // auxiliary vector: node i = src of edge zin_idx[i], bases in sequence order v[0..k), 2 bits each, node i at stream
@@ -297,19 +346,27 @@ int launch_target_keys(const u64 *keys, u64 n, u32 k, u32 W_, u32 WT_, u64 *out,
     return (int)cudaGetLastError();
 }
 
+u32 zero_flags_prefix_bits(u32 k) { return 2 * k < 20 ? 2 * k : 20; }
+u64 zero_flags_index_bytes(u32 k) { return 2 * ((((1ull << zero_flags_prefix_bits(k)) + 1) * 4 + 255) / 256 * 256); }
+
 int launch_zero_flags(const u64 *keys, u64 n, u32 k, u32 W_, u32 WT_, const u64 *tk_sorted, const u32 *last_real32,
-                      uint8_t *flag_out, uint8_t *flag_in, cudaStream_t s) {
+                      u32 *prefix_index, uint8_t *flag_out, uint8_t *flag_in, cudaStream_t s) {
     if (n == 0) return 0;
-    SDBG_DISPATCH_WWT(W_, WT_, (flag_zero_out_kernel<W, WT><<<grid_for(n), 256, 0, s>>>(tk_sorted, n, keys, k, flag_out),
-                                flag_zero_in_kernel<W, WT><<<grid_for(n), 256, 0, s>>>(keys, n, last_real32, tk_sorted, k, flag_in)));
+    const u32 pb = zero_flags_prefix_bits(k);
+    const u64 entries = (1ull << pb) + 1;
+    u32 *idx_edges = prefix_index, *idx_tk = prefix_index + zero_flags_index_bytes(k) / 8;
+    prefix_index_kernel<<<(unsigned)((entries + 255) / 256), 256, 0, s>>>(keys, n, W_, pb, idx_edges);
+    prefix_index_kernel<<<(unsigned)((entries + 255) / 256), 256, 0, s>>>(tk_sorted, n, WT_, pb, idx_tk);
+    SDBG_DISPATCH_WWT(W_, WT_, (flag_zero_out_kernel<W, WT><<<grid_for(n), 256, 0, s>>>(tk_sorted, n, keys, k, idx_edges, pb, flag_out),
+                                flag_zero_in_kernel<W, WT><<<grid_for(n), 256, 0, s>>>(keys, n, last_real32, tk_sorted, k, idx_tk, pb, flag_in)));
     return (int)cudaGetLastError();
 }
 
 int launch_full_assemble(const FullArgs &a, u32 W_, u32 WT_, cudaStream_t s) {
     valid_fill_kernel<<<grid_for((a.n + a.n_zero_out + 63) / 64), 256, 0, s>>>(a.out_valid, a.n + a.n_zero_out);
     if (a.n == 0) return (int)cudaGetLastError();
-    SDBG_DISPATCH_WWT(W_, WT_, (merge_real_kernel<W, WT><<<grid_for(a.n), 256, 0, s>>>(a),
-                                merge_dummy_kernel<W, WT><<<grid_for(a.n_zero_out), 256, 0, s>>>(a),
+    SDBG_DISPATCH_WWT(W_, WT_, (dummy_pos_kernel<W, WT><<<grid_for(a.n_zero_out), 256, 0, s>>>(a),
+                                assemble_kernel<<<grid_for((a.n + a.n_zero_out + 63) / 4), 256, 0, s>>>(a),
                                 aux_pack_kernel<W><<<grid_for(a.t), 256, 0, s>>>(a),
                                 edge_F_kernel<W, WT><<<1, 4, 0, s>>>(a)));
     return (int)cudaGetLastError();

@@ -105,10 +105,12 @@ struct FullArgs {
     uint8_t *out_W; u32 *out_last32; u64 *out_valid; u32 *out_mult; u64 *aux_bits;
     const uint8_t *flag_in; u32 *out_zin32;                // per solid edge: last edge of a zero-indegree node -> zin bits (A24)
     u64 *F_dev;                                            // u64[4] device scratch: F[0..3] of reading A25
+    u32 *dpos;                                             // u32[n_zero_out] scratch: output position of each `$` edge
 };
 int launch_target_keys(const u64 *keys, u64 n, u32 k, u32 W, u32 WT, u64 *out, cudaStream_t s);
+u64 zero_flags_index_bytes(u32 k);   // scratch of the two prefix indices (edges, targets)
 int launch_zero_flags(const u64 *keys, u64 n, u32 k, u32 W, u32 WT, const u64 *tk_sorted, const u32 *last_real32,
-                      uint8_t *flag_out, uint8_t *flag_in, cudaStream_t s);
+                      u32 *prefix_index, uint8_t *flag_out, uint8_t *flag_in, cudaStream_t s);
 u64 flag_scratch_bytes(u64 n);
 void launch_compact_flags(const uint8_t *flag, u64 n, u64 *scratch, u32 *out_idx, u64 *total_out, cudaStream_t s);
 int launch_full_assemble(const FullArgs &a, u32 W, u32 WT, cudaStream_t s);
