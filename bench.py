@@ -204,32 +204,91 @@ def run_gpu(args, w):
     ctx.set_timing(False)
 
     # ---- end to end: HOST pinned buffers in, SdBG arrays out, copies inside the timed region ---------------------
-    bases_h = torch.empty(n_bases, dtype=torch.uint8, pin_memory=True)
-    offs_h = torch.empty(n_reads + 1, dtype=torch.int64, pin_memory=True)
-    bases_h.copy_(bases_d); offs_h.copy_(offs_d)
-    out_W = torch.empty(S, dtype=torch.uint8, pin_memory=True)
-    out_last = torch.empty((S + 63) // 64, dtype=torch.int64, pin_memory=True)
-    out_mult = torch.empty(S, dtype=torch.int32, pin_memory=True)
-    out_keys = torch.empty(S * wl.words_per_key, dtype=torch.int64, pin_memory=True)
-
-    def e2e_step():
-        s = step(bases_h, offs_h)
-        out_W.copy_(graph.W[:s], non_blocking=True)
-        out_last.copy_(graph.last_bits[:(s + 63) // 64], non_blocking=True)
-        out_mult.copy_(graph.mult[:s], non_blocking=True)
-        out_keys.copy_(edges.keys[:s * wl.words_per_key], non_blocking=True)
-
-    ms_e2e = float("nan")
+    # Every step copies its reads from pinned host memory, runs the whole path and copies the SdBG arrays back; the
+    # step is over when its results are on the host. `--e2e-pipelines P` (default 2) runs P such step loops at once,
+    # each with its own context, stream, workspace and output buffers, fed by one host thread each, so that the copies
+    # of one step overlap the kernels of another (PCIe is full duplex and idle while a step sorts).
+    ms_e2e, e2e_steps, n_pipes = float("nan"), 0, 0
     if not args.no_e2e:
-        e2e_step()
+        ws_bytes = sd.sdbg_workspace_for_records(N, wl.k)
+        ctx.close(); ctx.workspace = None
+        del reads, edges, graph
+        torch.cuda.empty_cache()
+        bases_h = torch.empty(n_bases, dtype=torch.uint8, pin_memory=True)
+        offs_h = torch.empty(n_reads + 1, dtype=torch.int64, pin_memory=True)
+        bases_h.copy_(bases_d); offs_h.copy_(offs_d)
+        del bases_d, offs_d
+        torch.cuda.empty_cache()
+        free_b = torch.cuda.mem_get_info()[0]
+        per_pipe = ws_bytes + n_bases // 2 + S * (K + 4 + 5 + 1) + (64 << 20)
+        n_pipes = max(1, min(args.e2e_pipelines, int(free_b * 0.9 // per_pipe)))
+
+        class Pipe:
+            pass
+
+        pipes = []
+        for _ in range(n_pipes):
+            pp = Pipe()
+            pp.stream = torch.cuda.Stream()
+            with torch.cuda.stream(pp.stream):
+                pp.ctx = sd.Context(ws_bytes)
+                pp.reads = sd.Reads(n_bases)
+                pp.edges = sd.Edges(S + 1024, wl.k)
+                pp.graph = sd.Graph(S + 1024)
+            pp.out_W = torch.empty(S, dtype=torch.uint8, pin_memory=True)
+            pp.out_last = torch.empty((S + 63) // 64, dtype=torch.int64, pin_memory=True)
+            pp.out_mult = torch.empty(S, dtype=torch.int32, pin_memory=True)
+            pp.out_keys = torch.empty(S * wl.words_per_key, dtype=torch.int64, pin_memory=True)
+            pp.done = torch.cuda.Event()
+            pipes.append(pp)
+
+        # one loop at a time in each phase: identical loops started together would otherwise stay in lockstep and share
+        # the link and the SMs phase by phase; with the locks one loop sorts while another copies
+        lock_in, lock_gpu, lock_out = threading.Lock(), threading.Lock(), threading.Lock()
+
+        def e2e_loop(pp, n_steps, start_event):
+            torch.cuda.set_device(local)
+            with torch.cuda.stream(pp.stream):
+                if start_event is not None:
+                    pp.stream.wait_event(start_event)
+                for _ in range(n_steps):
+                    pp.reads.c.n_reads = pp.reads.c.n_bases = pp.reads.c.n_slots = 0
+                    with lock_in:                        # host -> device copy of the reads (+ the pack kernel)
+                        sd.sdbg_pack_reads(pp.ctx, bases_h, offs_h, n_reads, pp.reads)
+                    with lock_gpu:                       # extract, sort, count, emit
+                        sd.sdbg_count_edges(pp.ctx, pp.reads, n_reads, wl.k, wl.d, pp.edges, None)
+                        sd.sdbg_build(pp.ctx, pp.edges, sd.SDBG_SORTED, pp.graph)
+                        pp.stream.synchronize()
+                    s_ = pp.edges.n
+                    with lock_out:                       # device -> host copy of the SdBG arrays
+                        pp.out_W.copy_(pp.graph.W[:s_], non_blocking=True)
+                        pp.out_last.copy_(pp.graph.last_bits[:(s_ + 63) // 64], non_blocking=True)
+                        pp.out_mult.copy_(pp.graph.mult[:s_], non_blocking=True)
+                        pp.out_keys.copy_(pp.edges.keys[:s_ * wl.words_per_key], non_blocking=True)
+                        pp.stream.synchronize()          # the step's results are on the host
+                pp.done.record(pp.stream)
+
+        def run_all(n_steps, start_event):
+            ths = [threading.Thread(target=e2e_loop, args=(pp, n_steps, start_event)) for pp in pipes]
+            for t in ths:
+                t.start()
+            for t in ths:
+                t.join()
+
+        run_all(1, None)                                 # warm-up: one step per pipeline
+        per = (args.steps + n_pipes - 1) // n_pipes
+        e2e_steps = per * n_pipes
         e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         barrier()
         e0.record()
-        for _ in range(args.steps):
-            e2e_step()
+        run_all(per, e0)
+        for pp in pipes:
+            torch.cuda.current_stream().wait_event(pp.done)
         e1.record()
         barrier()
-        ms_e2e = e0.elapsed_time(e1)
+        ms_e2e = e0.elapsed_time(e1) * args.steps / e2e_steps     # scaled to args.steps steps, as the other timings
+        for pp in pipes:
+            assert pp.edges.n == S
     h2d = n_bases + 8 * (n_reads + 1)
     d2h = S * (1 + 4 + K) + 8 * ((S + 63) // 64)
 
@@ -256,7 +315,8 @@ def run_gpu(args, w):
         "read_bases_per_s": world * n_bases * args.steps / (ms_total * 1e-3),
         "clocks": clocks,
         "e2e": {"value": whole_job_value(N, world, args.steps, ms_e2e), "unit": UNIT, "h2d_bytes_per_step": h2d,
-                "d2h_bytes_per_step": d2h, "ms_per_step": ms_e2e / args.steps},
+                "d2h_bytes_per_step": d2h, "ms_per_step": ms_e2e / args.steps, "pipelines": n_pipes,
+                "steps_timed": e2e_steps},
         "gpu_launches": int(tim.total_launches),
         "roofline": {"kernel": "onesweep_kernel (one LSD radix pass)", "bound": "hbm", "achieved": achieved, "peak": peak,
                      "unit": "GB/s", "frac": achieved / peak, "traffic": _traffic(wl.name), "peak_source": peak_src,
@@ -347,6 +407,7 @@ def main():
     ap.add_argument("--ref-reads", type=int, default=40000, help="reads in the oracle's bounded sample")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true", help="development runs: skip the host-buffer end-to-end leg")
+    ap.add_argument("--e2e-pipelines", type=int, default=2, help="concurrent host-to-host step loops of the end-to-end leg")
     ap.add_argument("--next", action="store_true", help="time the widened rows (sdbg_build_full, sdbg_mercy_edges) instead")
     args = ap.parse_args()
     from workloads import get_config
