@@ -133,12 +133,12 @@ void launch_backward(const IndexView &ix, const u64 *q, u64 n, long long *out, c
 struct MercyArgs {
     const u64 *words, *ends; u64 n_slots;                  // packed reads
     const u64 *keys; u64 n; u32 k;                         // sorted solid edges
-    const u32 *table; u64 table_mask;                      // hash table over the solid edges: edge index + 1, 0 = empty
+    const void *table; u64 table_mask;                     // hash table over the solid edges: 16-byte slots {first key word, edge index + 1 (0 = empty)}
     const u64 *tk; const u32 *zout_idx; u64 n_zero_out;    // nodes without outgoing edge (rows of tk)
     const u32 *zin_idx; u64 t;                             // nodes without incoming edge (edges whose node it is)
     u64 *out_keys; u32 *out_mult; u64 out_cap;             // appended at st->extract_cursor
 };
-void launch_hash_build(const u64 *keys, u64 n, u32 W, u32 *table, u64 slots /* power of two >= 2n */, cudaStream_t s);
+void launch_hash_build(const u64 *keys, u64 n, u32 W, void *table /* 16 bytes per slot, zeroed */, u64 slots /* power of two >= 2n */, cudaStream_t s);
 int launch_mercy(const MercyArgs &a, u32 W, u32 WT, DevState *st, cudaStream_t s);
 
 // sdbg_build unsorted path: merge equal adjacent keys of a sorted (key, mult) list, summing mult (saturating).

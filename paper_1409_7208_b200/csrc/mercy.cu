@@ -54,8 +54,11 @@ __device__ void window_keys(const u64 *__restrict__ words, u64 slot, u32 k, u64 
     }
 }
 
-// Hash table over the solid edges (open addressing, linear probing, load <= 1/2): slot = edge index + 1, 0 = empty.
-// A look-up costs one or two dependent random reads instead of the ~30 of a binary search over the whole list.
+// Hash table over the solid edges (open addressing, linear probing, load <= 1/2). A slot is 16 bytes: the first key word
+// and edge index + 1 (0 = empty), so a look-up of a one-word key is ONE random 16-byte read (the key is compared in the
+// slot itself); longer keys compare their first word there and the remaining words through the index only when it
+// matches. The build claims a slot with a CAS on the index field and then stores the key word: nothing reads the table
+// before the build kernel has ended, and the edges are distinct, so no key is compared while building.
 template <int W>
 __device__ __forceinline__ u64 hash_key(const u64 (&key)[W]) {
     u64 h = 0;
@@ -64,35 +67,42 @@ __device__ __forceinline__ u64 hash_key(const u64 (&key)[W]) {
     return h;
 }
 template <int W>
-__global__ void __launch_bounds__(256) hash_build_kernel(const u64 *__restrict__ keys, u64 n, u32 *__restrict__ table, u64 mask) {
+__global__ void __launch_bounds__(256) hash_build_kernel(const u64 *__restrict__ keys, u64 n, ulonglong2 *__restrict__ table, u64 mask) {
     for (u64 i = (u64)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (u64)gridDim.x * blockDim.x) {
         u64 key[W];
         ldk<W>(keys, i, key);
         u64 h = hash_key<W>(key) & mask;
-        while (atomicCAS(&table[h], 0u, (u32)i + 1u) != 0u) h = (h + 1) & mask;
+        while (atomicCAS(reinterpret_cast<u32 *>(&table[h].y), 0u, (u32)i + 1u) != 0u) h = (h + 1) & mask;
+        table[h].x = key[0];
     }
 }
-void launch_hash_build(const u64 *keys, u64 n, u32 W, u32 *table, u64 slots, cudaStream_t s) {
+void launch_hash_build(const u64 *keys, u64 n, u32 W, void *table, u64 slots, cudaStream_t s) {
     u64 blocks = (n + 255) / 256;
     if (blocks > (u64)kNumSMs * 16) blocks = (u64)kNumSMs * 16;
     if (blocks == 0) return;
+    ulonglong2 *t = reinterpret_cast<ulonglong2 *>(table);
     switch (W) {
-        case 1: hash_build_kernel<1><<<(unsigned)blocks, 256, 0, s>>>(keys, n, table, slots - 1); break;
-        case 2: hash_build_kernel<2><<<(unsigned)blocks, 256, 0, s>>>(keys, n, table, slots - 1); break;
-        case 3: hash_build_kernel<3><<<(unsigned)blocks, 256, 0, s>>>(keys, n, table, slots - 1); break;
-        default: hash_build_kernel<4><<<(unsigned)blocks, 256, 0, s>>>(keys, n, table, slots - 1); break;
+        case 1: hash_build_kernel<1><<<(unsigned)blocks, 256, 0, s>>>(keys, n, t, slots - 1); break;
+        case 2: hash_build_kernel<2><<<(unsigned)blocks, 256, 0, s>>>(keys, n, t, slots - 1); break;
+        case 3: hash_build_kernel<3><<<(unsigned)blocks, 256, 0, s>>>(keys, n, t, slots - 1); break;
+        default: hash_build_kernel<4><<<(unsigned)blocks, 256, 0, s>>>(keys, n, t, slots - 1); break;
     }
 }
 
 template <int W>
 __device__ __forceinline__ bool is_solid(const MercyArgs &a, const u64 (&key)[W]) {
+    const ulonglong2 *table = reinterpret_cast<const ulonglong2 *>(a.table);
     u64 h = hash_key<W>(key) & a.table_mask;
     while (true) {
-        const u32 v = __ldg(a.table + h);
-        if (v == 0u) return false;
-        u64 e[W];
-        ldk<W>(a.keys, (u64)v - 1u, e);
-        if (cmpk<W>(e, key) == 0) return true;
+        const ulonglong2 v = __ldg(table + h);
+        const u32 idx1 = (u32)v.y;
+        if (idx1 == 0u) return false;
+        if (v.x == key[0]) {
+            bool same = true;
+#pragma unroll
+            for (int q = 1; q < W; ++q) same = same && __ldg(a.keys + ((u64)idx1 - 1u) * W + q) == key[q];
+            if (same) return true;
+        }
         h = (h + 1) & a.table_mask;
     }
 }
@@ -185,9 +195,23 @@ __global__ void __launch_bounds__(128) mercy_kernel(MercyArgs a, DevState *st) {
                             const u64 cnt = 2 * (i - (u64)run_start);
                             const u64 base = atomicAdd(&st->extract_cursor, cnt);
                             if (base + cnt <= a.out_cap) {
+                                u64 f[W], r[W];
+                                window_keys<W>(a.words, first + (u64)run_start, k, f, r);
                                 for (u64 j = (u64)run_start; j < i; ++j) {
-                                    u64 f[W], r[W];
-                                    window_keys<W>(a.words, first + j, k, f, r);
+                                    if (j > (u64)run_start) {    // both keys roll on by the base that enters the window
+                                        const u64 nb = base_at(a.words, first + j + k);
+                                        const u64 f_last = (f[W - 1] >> pad) & 3ull, r_first = r[0] >> 62;
+#pragma unroll
+                                        for (int q = W - 1; q >= 0; --q) f[q] = (f[q] >> 2) | (q ? f[q - 1] << 62 : 0ull);
+                                        f[0] |= f_last << 62;
+                                        mask_top<W>(f, 2 * k);
+                                        set_sym<W>(f, k, nb);
+#pragma unroll
+                                        for (int q = 0; q < W; ++q) r[q] = (r[q] << 2) | (q + 1 < W ? r[q + 1] >> 62 : 0ull);
+                                        mask_top<W>(r, 2 * (k - 1));
+                                        set_sym<W>(r, k - 1, 3ull - nb);
+                                        set_sym<W>(r, k, r_first);
+                                    }
                                     const u64 o = base + 2 * (j - (u64)run_start);
 #pragma unroll
                                     for (int q = 0; q < W; ++q) { a.out_keys[o * W + q] = f[q]; a.out_keys[(o + 1) * W + q] = r[q]; }
