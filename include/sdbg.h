@@ -215,7 +215,8 @@ int sdbg_build_full(sdbg_ctx *ctx, const sdbg_edges *edges, sdbg_full_graph *out
  * complement are appended to `out` (keys, mult = 1; unsorted, with repeats: out->n records). `solid` is the output of
  * sdbg_count_edges over the same reads (sorted, distinct; 2 <= k <= 127; fewer than 2^32 edges). To build the graph
  * with them, put solid and mercy records into one sdbg_edges and call sdbg_build without SDBG_SORTED (equal keys are
- * merged, mult summed). Synchronises. Errors: SDBG_E_CAPACITY (out->n = needed count), SDBG_E_WORKSPACE,
+ * merged, mult summed). Workspace: about 40 + 16 w bytes per solid edge for the zero-degree lists plus a hash table of
+ * 16-byte slots, 2 to 4 per solid edge. Synchronises. Errors: SDBG_E_CAPACITY (out->n = needed count), SDBG_E_WORKSPACE,
  * SDBG_E_UNSUPPORTED, SDBG_E_INVAL. */
 int sdbg_mercy_edges(sdbg_ctx *ctx, const sdbg_reads *reads, const sdbg_edges *solid, sdbg_edges *out);
 

@@ -330,7 +330,7 @@ def check_mercy(res, w, reads):
     records come as (window, reverse complement) pairs, and no mercy record is a solid edge."""
     import torch
     ed, S = res.edges, res.n
-    ctx = sd.Context(64 * S * ed.w + (1 << 28))
+    ctx = sd.Context((112 + 16 * ed.w) * S + (1 << 28))   # zero-degree scratch + 16-byte hash slots, at most 4 per edge
     probe = sd.Edges(0, w.k)
     try:
         sd.sdbg_mercy_edges(ctx, reads, ed, probe)
