@@ -148,6 +148,30 @@ int sdbg_count_edges(sdbg_ctx *ctx, const sdbg_reads *reads, uint64_t n, uint32_
  * max_ranges is too small. */
 int64_t sdbg_plan_ranges(const uint64_t *hist, uint64_t capacity, uint64_t *ranges, uint64_t max_ranges);
 
+/* ---- sharding by ranges of l=8 partitions ------------------------------------------ */
+
+/* "we adopt a block-wise strategy that partitions the k-mers according to their length-l prefix (l=8 in our
+ * implementation). The k-mers in consecutive partitions ... are sorted together". The same partitions
+ * shard the path across GPUs: every GPU holds the packed reads (replicated: one broadcast) and counts only the edges
+ * of a contiguous range of partitions; the outputs of the ranges, concatenated in range order, are the output of
+ * sdbg_count_edges, and for k >= 9 no `last` / minus dependency crosses a partition, so the arrays of sdbg_build over
+ * each range concatenate too. No collective on the data path (an all-gather of the per-range counts gives offsets).
+ *
+ * sdbg_count_edges_range: sdbg_count_edges restricted to partitions [bucket_lo, bucket_hi) (partition = top 16 bits
+ * of the key). stats->n_raw counts the raw records of the range only; checksums cover the range; stats->bucket_hist,
+ * if asked for, is still the histogram of all partitions. Same errors as sdbg_count_edges, plus SDBG_E_INVAL for a
+ * bad range. */
+int sdbg_count_edges_range(sdbg_ctx *ctx, const sdbg_reads *reads, uint64_t n, uint32_t k, uint32_t d,
+                           uint32_t bucket_lo, uint32_t bucket_hi, sdbg_edges *out, sdbg_stats *stats /* nullable */);
+/* hist: DEVICE u64[65536] = raw records per l=8 partition of the packed reads at this k (one pass of the extractor
+ * without output). Launches on the ctx stream and does not synchronise. */
+int sdbg_bucket_hist(sdbg_ctx *ctx, const sdbg_reads *reads, uint32_t k, uint64_t *hist);
+/* Host logic: n_shards contiguous ranges of partitions balanced by records. hist: HOST u64[65536]; bounds: HOST
+ * u32[n_shards + 1], bounds[0] = 0, bounds[n_shards] = 65536, shard i = [bounds[i], bounds[i+1]); shard i starts at the
+ * first partition before which at least i/n_shards of the records lie (a shard may be empty). Deterministic: every
+ * rank computes the same plan from the same histogram. */
+int sdbg_plan_shards(const uint64_t *hist, uint32_t n_shards, uint32_t *bounds);
+
 /* ---- a5: SdBG arrays ------------------------------------------------------------------------------------ */
 
 #define SDBG_SORTED 1u   /* edges->keys are strictly increasing (the output of sdbg_count_edges) */

@@ -91,6 +91,10 @@ def lib():
         L.sdbg_workspace_for_records.argtypes = [u64, u32]; L.sdbg_workspace_for_records.restype = u64
         L.sdbg_count_edges.argtypes = [vp, C.POINTER(_Reads), u64, u32, u32, C.POINTER(_Edges), C.POINTER(_Stats)]
         L.sdbg_count_edges.restype = i32
+        L.sdbg_count_edges_range.argtypes = [vp, C.POINTER(_Reads), u64, u32, u32, u32, u32, C.POINTER(_Edges), C.POINTER(_Stats)]
+        L.sdbg_count_edges_range.restype = i32
+        L.sdbg_bucket_hist.argtypes = [vp, C.POINTER(_Reads), u32, vp]; L.sdbg_bucket_hist.restype = i32
+        L.sdbg_plan_shards.argtypes = [vp, u32, vp]; L.sdbg_plan_shards.restype = i32
         L.sdbg_plan_ranges.argtypes = [vp, u64, vp, u64]; L.sdbg_plan_ranges.restype = C.c_int64
         L.sdbg_build.argtypes = [vp, C.POINTER(_Edges), u32, C.POINTER(_Graph)]; L.sdbg_build.restype = i32
         L.sdbg_build_full.argtypes = [vp, C.POINTER(_Edges), C.POINTER(_FullGraph)]; L.sdbg_build_full.restype = i32
@@ -339,6 +343,30 @@ def sdbg_count_edges(ctx: Context, reads: Reads, n: int, k: int, d: int, out: Ed
     rc = lib().sdbg_count_edges(ctx._h, C.byref(reads.c), n, k, d, C.byref(out.c), C.byref(stats.c) if stats else None)
     ctx.check(rc)
     return out.c.n
+
+
+def sdbg_count_edges_range(ctx: Context, reads: Reads, n: int, k: int, d: int, bucket_lo: int, bucket_hi: int, out: Edges,
+                           stats: Stats | None = None) -> int:
+    rc = lib().sdbg_count_edges_range(ctx._h, C.byref(reads.c), n, k, d, bucket_lo, bucket_hi, C.byref(out.c),
+                                      C.byref(stats.c) if stats else None)
+    ctx.check(rc)
+    return out.c.n
+
+
+def sdbg_bucket_hist(ctx: Context, reads: Reads, k: int, hist) -> None:
+    """hist: 65,536 int64/uint64 on the device. Does not synchronise."""
+    ctx.check(lib().sdbg_bucket_hist(ctx._h, C.byref(reads.c), k, _ptr(hist)))
+
+
+def sdbg_plan_shards(hist: np.ndarray, n_shards: int) -> np.ndarray:
+    """hist: 65,536 uint64 on the host -> n_shards + 1 partition bounds (uint32)."""
+    h = np.ascontiguousarray(hist, dtype=np.uint64)
+    assert h.size == SDBG_NUM_BUCKETS
+    bounds = np.zeros(n_shards + 1, dtype=np.uint32)
+    rc = lib().sdbg_plan_shards(h.ctypes.data, n_shards, bounds.ctypes.data)
+    if rc != 0:
+        raise SdbgError(rc, sdbg_strerror(rc))
+    return bounds
 
 
 def sdbg_mercy_edges(ctx: Context, reads: Reads, solid: Edges, out: Edges) -> int:
