@@ -159,7 +159,7 @@ def run_gpu(args, w):
 
     # ---- inputs resident in HBM: every rank an independent replica (own seed) ------------------------------
     from dataclasses import replace
-    wl = replace(w, seed=rank_seed(w.seed, rank)) if rank else w
+    wl = replace(w, seed=rank_seed(w.seed, rank)) if (rank and not args.shard) else w   # --shard: the same reads on every rank
     gen = ReadGenerator(wl)
     bases_d, offs_d = gen.device()
     torch.cuda.synchronize()
@@ -175,6 +175,12 @@ def run_gpu(args, w):
     def step(src_b, src_o):
         reads.c.n_reads = reads.c.n_bases = reads.c.n_slots = 0
         sd.sdbg_pack_reads(ctx, src_b, src_o, n_reads, reads)
+        if args.shard:     # replicated reads, each rank counts its range of l=8 partitions
+            from paper_1409_7208_b200.shard import count_edges_sharded, gather_counts
+            n_local, _ = count_edges_sharded(ctx, reads, n_reads, wl.k, wl.d, edges, rank, world)
+            sd.sdbg_build(ctx, edges, sd.SDBG_SORTED, graph)
+            gather_counts(n_local, device="cuda")        # offsets of the concatenation: the only exchange
+            return edges.n
         sd.sdbg_count_edges(ctx, reads, n_reads, wl.k, wl.d, edges, None)
         sd.sdbg_build(ctx, edges, sd.SDBG_SORTED, graph)
         return edges.n
@@ -209,7 +215,7 @@ def run_gpu(args, w):
     # each with its own context, stream, workspace and output buffers, fed by one host thread each, so that the copies
     # of one step overlap the kernels of another (PCIe is full duplex and idle while a step sorts).
     ms_e2e, e2e_steps, n_pipes = float("nan"), 0, 0
-    if not args.no_e2e:
+    if not args.no_e2e and not args.shard:
         ws_bytes = sd.sdbg_workspace_for_records(N, wl.k)
         ctx.close(); ctx.workspace = None
         del reads, edges, graph
@@ -306,13 +312,13 @@ def run_gpu(args, w):
     algo_bytes = tim.bytes["radix"] // max(radix_launches, 1)
     achieved = algo_bytes / (radix_ms * 1e-3) / 1e9 if radix_ms > 0 else 0.0
     line = {
-        "metric": METRIC, "value": whole_job_value(N, world, args.steps, ms_total), "unit": UNIT, "n_gpus": world,
+        "metric": METRIC, "value": whole_job_value(N, 1 if args.shard else world, args.steps, ms_total), "unit": UNIT, "n_gpus": world,
         "steps": args.steps, "warmup": max(args.warmup, 3), "ms_per_step": ms_total / args.steps,
-        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "u64", "data": "synthetic",
+        "higher_is_better": True, "scaling": "strong" if args.shard else "weak", "vs_baseline": None, "dtype": "u64", "data": "synthetic",
         "config": {"workload": wl.name, "k": wl.k, "d": wl.d, "reads": n_reads, "read_len": wl.read_len, "bases": n_bases,
-                   "raw_edges": N, "solid_edges": int(S), "key_bytes": K, "parallelism": "replicas only" if world > 1 else "1 gpu",
+                   "raw_edges": N, "solid_edges": int(S), "key_bytes": K, "parallelism": ("sharded by ranges of l=8 partitions, reads replicated" if args.shard else "replicas only" if world > 1 else "1 gpu"),
                    "l2": "inputs larger than L2 (keys %.2f GB, reads %.0f MB ASCII)" % (N * K / 1e9, n_bases / 1e6)},
-        "read_bases_per_s": world * n_bases * args.steps / (ms_total * 1e-3),
+        "read_bases_per_s": (1 if args.shard else world) * n_bases * args.steps / (ms_total * 1e-3),
         "clocks": clocks,
         "e2e": {"value": whole_job_value(N, world, args.steps, ms_e2e), "unit": UNIT, "h2d_bytes_per_step": h2d,
                 "d2h_bytes_per_step": d2h, "ms_per_step": ms_e2e / args.steps, "pipelines": n_pipes,
@@ -408,6 +414,8 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true", help="development runs: skip the host-buffer end-to-end leg")
     ap.add_argument("--e2e-pipelines", type=int, default=2, help="concurrent host-to-host step loops of the end-to-end leg")
+    ap.add_argument("--shard", action="store_true", help="strong scaling: every rank holds the same reads and counts its own range "
+                    "of l=8 partitions (SURVEY.md §8(e)); default is independent replicas")
     ap.add_argument("--next", action="store_true", help="time the widened rows (sdbg_build_full, sdbg_mercy_edges) instead")
     args = ap.parse_args()
     from workloads import get_config
