@@ -110,3 +110,38 @@ def test_config1_at_full_size_every_edge():
     bases, offs = ReadGenerator(cfg).host()
     fg, want, nav, ix, _ = _check((bases, offs), cfg.k, 1)
     assert want["m"] > 448 * 1000
+
+
+def test_edge_count_a_multiple_of_the_cell_size():
+    """m = 448 j exactly: rank at position m reads the extra (empty) cell behind the last full one."""
+    from oracle import Oracle
+    from oracle.sdbg_oracle import reads_to_arrays
+    k, found = 5, None
+    for seed in range(4000):
+        rng = random.Random(seed)
+        n_src = rng.randint(1, 3)
+        src = ["".join(rng.choice("ACGT") for _ in range(rng.randint(150, 400))) for _ in range(n_src)]
+        o = Oracle(k, 1)
+        o.add_reads(*reads_to_arrays(src))
+        res = o.finish(want_distinct=False)
+        # m = solid edges + nodes without outgoing edge; computed here from the strings, cheaply
+        S = res.solid_strings()
+        src_nodes = {e[:k] for e in S}
+        m = len(S) + len({e[1:] for e in S} - src_nodes)
+        o.close()
+        if m >= 448 and m % 448 == 0:
+            found = src
+            break
+    assert found is not None, "no seed gave m = 448 j"
+    fg, want, nav, ix, _ = _check(found, k, 1)
+    assert want["m"] % 448 == 0
+
+
+def test_two_letter_reads_leave_two_classes_empty():
+    """Reads over {A, T} only (closed under reverse complement): no node ends with C or G, so F[1] = F[2] = F[3] and the
+    vectors B_C, B_G have no one at all."""
+    rng = random.Random(11)
+    reads = ["".join(rng.choice("AT") for _ in range(rng.randint(20, 90))) for _ in range(40)]
+    for k in (3, 7, 12):
+        fg, want, nav, ix, _ = _check(reads, k, 1)
+        assert fg.F[1] == fg.F[2] == fg.F[3] and ix.ones[1] == 0 and ix.ones[2] == 0 and ix.ones[0] > 0 and ix.ones[3] > 0
