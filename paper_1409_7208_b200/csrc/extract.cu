@@ -114,13 +114,25 @@ __device__ __forceinline__ void store_key(u64 *__restrict__ out, u64 pos, const 
     }
 }
 
-template <int W, bool FILTER>
+template <int W, bool FILTER, int T4>
 __global__ void __launch_bounds__(256) extract_kernel(ExtractArgs a, DevState *st) {
     extern __shared__ u32 s_hist[];   // [n_passes][256] when digit_hist != nullptr
     const int np = a.passes.n;
     const bool do_hist = a.digit_hist != nullptr;
+    // T4 >= 2 (one-word keys, dense pass, digit histograms wanted, T4 = floor(k/4)): the T4 top key bytes hold node symbols
+    // only, and byte t of the forward key of the window at slot p is the reversed 4-mer at x = p + k-4-4t, byte t of the
+    // rc-strand key the complemented 4-mer at x = p + 4t + 1. So a read position x contributes the SAME byte value to
+    // the histograms of a contiguous range of t (all T4 of them in the interior of a read, fewer near its ends: the
+    // window starts that exist are an interval). Positions are therefore counted as differences over t — +1 in row
+    // t_lo, -1 in row t_hi + 1 — in two position tables indexed by the plain 4-mer f4 (forward strand: its symbol
+    // reversal is the digit; rc strand: its complement), prefix-summed over t and folded into the pass rows when the
+    // block flushes. For k >= 8 exactly one key byte is left (byte 7 - T4 from the LSB, the one with e[k]): it is the
+    // only per-key atomic. Shared-memory atomics, the bottleneck of this kernel, drop from 8 per key to about 2.4.
+    constexpr bool shared4 = T4 >= 2;
+    constexpr u32 T = T4;
+    u32 *s_posf = s_hist + np * kRadix, *s_posr = s_posf + T * kRadix;   // [T][256] each (shared4 only)
     if (do_hist) {
-        for (int i = threadIdx.x; i < np * kRadix; i += blockDim.x) s_hist[i] = 0;
+        for (int i = threadIdx.x; i < (np + 2 * (int)T) * kRadix; i += blockDim.x) s_hist[i] = 0;
         __syncthreads();
     }
     // s_hist row of byte 0 of the last key word if it were a pass (rows of the padding bytes are never touched)
@@ -137,10 +149,41 @@ __global__ void __launch_bounds__(256) extract_kernel(ExtractArgs a, DevState *s
     for (u64 wg = (u64)blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5); wg < nwarp_groups; wg += warps_total) {
         const u64 g = wg * 32 + lane;
         u32 valid = (g < ngroups) ? valid_mask32(a.ends, g, a.k) : 0u;
-        if (__ballot_sync(0xffffffffu, valid != 0) == 0) continue;
+        u32 vprev = 0;                                   // valid window starts of the 32 slots before mine
+        if constexpr (shared4) {
+            vprev = __shfl_up_sync(0xffffffffu, valid, 1);
+            if (lane == 0) vprev = (g >= 1 && g - 1 < ngroups) ? valid_mask32(a.ends, g - 1, a.k) : 0u;
+        }
+        if (__ballot_sync(0xffffffffu, (valid | vprev) != 0) == 0) continue;
         KeyMaker<W> km;
         km.load(a.words, g < ngroups ? g : 0, a.k);
-
+        if constexpr (shared4) {
+            if (valid | vprev) {
+                // window starts [32g-32, 32g+32) as one mask: bit 32+j = start at my slot j
+                const u64 V = ((u64)valid << 32) | vprev;
+                constexpr u32 pat = 0x11111111u >> (4 * (8 - T));       // bits 0, 4, ..., 4(T-1)
+                const u32 off_f = 32 - (a.k - 4), off_r = 32 - 1 - 4 * (T - 1);
+                auto count_pos = [&](u32 j, u32 f4) {   // f4 = (r[x], r[x+1], r[x+2], r[x+3]) at my slot j
+                    const u32 mf = (u32)(V >> (off_f + j)) & pat;       // bit 4t: the window whose forward byte t I am
+                    const u32 mr = (u32)(V >> (off_r + j)) & pat;       // bit 4(T-1-t): the window whose rc byte t I am
+                    if (mf) {
+                        const u32 t_lo = ((u32)__ffs(mf) - 1u) >> 2, t_end = ((31u - (u32)__clz(mf)) >> 2) + 1u;
+                        atomicAdd(&s_posf[t_lo * kRadix + f4], 1u);
+                        if (t_end < T) atomicAdd(&s_posf[t_end * kRadix + f4], 0xffffffffu);
+                    }
+                    if (mr) {
+                        const u32 t_lo = T - 1u - ((31u - (u32)__clz(mr)) >> 2), t_end = T - (((u32)__ffs(mr) - 1u) >> 2);
+                        atomicAdd(&s_posr[t_lo * kRadix + f4], 1u);
+                        if (t_end < T) atomicAdd(&s_posr[t_end * kRadix + f4], 0xffffffffu);
+                    }
+                };
+                const u32 b0w = KeyMaker<W>::w32(km.B, 0), b1w = KeyMaker<W>::w32(km.B, 1), b2w = KeyMaker<W>::w32(km.B, 2);
+#pragma unroll 4
+                for (u32 jj = 0; jj < 16; ++jj) count_pos(jj, __funnelshift_l(b1w, b0w, 2 * jj) >> 24);
+#pragma unroll 4
+                for (u32 jj = 0; jj < 16; ++jj) count_pos(16 + jj, __funnelshift_l(b2w, b1w, 2 * jj) >> 24);
+            }
+        }
         u32 vf = valid, vr = valid;   // per-strand keep masks
         if (FILTER && a.k >= 8) {
             // which keys fall into the range of partitions: only the top 16 bits of each key are needed
@@ -184,14 +227,19 @@ __global__ void __launch_bounds__(256) extract_kernel(ExtractArgs a, DevState *s
         // digit histograms of one key: every pass is one whole byte of a key word (api.cu make_passes): byte b of word
         // q is pass (b - b0) for the last word and (8 - b0) + 8 (W-2-q) + b for the others, b0 = first significant byte
         auto add_digits = [&](const u64 (&key)[W]) {
+            if constexpr (shared4) {   // the one byte that is not counted by position: byte 7 - T from the LSB = pass 0
+                constexpr u32 b = 7 - T;
+                atomicAdd(&s_hist[__byte_perm(b < 4 ? (u32)key[0] : (u32)(key[0] >> 32), 0u, 0x4440u | (b & 3))], 1u);
+            } else {
 #pragma unroll
-            for (int q = W - 1; q >= 0; --q) {
-                u32 *hq = (q == W - 1) ? h_last : h_last + ((8 - b0) + 8 * (W - 2 - q) + b0) * kRadix;
-                const u32 lo = (u32)key[q], hi = (u32)(key[q] >> 32);
+                for (int q = W - 1; q >= 0; --q) {
+                    u32 *hq = (q == W - 1) ? h_last : h_last + ((8 - b0) + 8 * (W - 2 - q) + b0) * kRadix;
+                    const u32 lo = (u32)key[q], hi = (u32)(key[q] >> 32);
 #pragma unroll
-                for (int b = 0; b < 8; ++b) {
-                    if (q == W - 1 && b < (int)b0) continue;     // padding bytes of the last word: no pass
-                    atomicAdd(&hq[b * kRadix + __byte_perm(b < 4 ? lo : hi, 0u, 0x4440u | (b & 3))], 1u);
+                    for (int b = 0; b < 8; ++b) {
+                        if (q == W - 1 && b < (int)b0) continue;     // padding bytes of the last word: no pass
+                        atomicAdd(&hq[b * kRadix + __byte_perm(b < 4 ? lo : hi, 0u, 0x4440u | (b & 3))], 1u);
+                    }
                 }
             }
         };
@@ -246,19 +294,51 @@ __global__ void __launch_bounds__(256) extract_kernel(ExtractArgs a, DevState *s
                     atomicAdd(&a.bucket_hist[r[0] >> 48], 1ull);
                 }
             };
+            // the plain case of the hot path (one-word keys, keys and digit histograms wanted, no checksum, no partition
+            // histogram): both keys of a window leave as ONE 16-byte store under one predicate (the warp's running
+            // position stays even: every lane adds two keys per window)
+            bool fast = false;
+            if constexpr (W == 1) fast = a.keys_out && do_hist && !a.want_csum && !a.bucket_hist;
+            auto emit_fast = [&](u32 i, const u64 (&f)[W], const u64 (&r)[W]) {
+                const bool v = (valid >> i) & 1;
+                const u32 m = __ballot_sync(0xffffffffu, v);
+                if (v) {
+                    *reinterpret_cast<ulonglong2 *>(a.keys_out + base + 2 * __popc(m & lt)) = make_ulonglong2(f[0], r[0]);
+                    add_digits(f);
+                    add_digits(r);
+                }
+                base += 2 * __popc(m);
+            };
+            if (fast) {
 #pragma unroll 1
-            for (u32 ii = 0; ii < 16; ++ii) {
-                if (!((any_mask >> ii) & 1)) continue;     // warp-uniform
-                u64 f[W], r[W];
-                km.template keys_h<0>(ii, f, r);
-                emit_window(ii, f, r);
-            }
+                for (u32 ii = 0; ii < 16; ++ii) {
+                    if (!((any_mask >> ii) & 1)) continue;     // warp-uniform
+                    u64 f[W], r[W];
+                    km.template keys_h<0>(ii, f, r);
+                    emit_fast(ii, f, r);
+                }
 #pragma unroll 1
-            for (u32 ii = 0; ii < 16; ++ii) {
-                if (!((any_mask >> (16 + ii)) & 1)) continue;
-                u64 f[W], r[W];
-                km.template keys_h<1>(ii, f, r);
-                emit_window(16 + ii, f, r);
+                for (u32 ii = 0; ii < 16; ++ii) {
+                    if (!((any_mask >> (16 + ii)) & 1)) continue;
+                    u64 f[W], r[W];
+                    km.template keys_h<1>(ii, f, r);
+                    emit_fast(16 + ii, f, r);
+                }
+            } else {
+#pragma unroll 1
+                for (u32 ii = 0; ii < 16; ++ii) {
+                    if (!((any_mask >> ii) & 1)) continue;     // warp-uniform
+                    u64 f[W], r[W];
+                    km.template keys_h<0>(ii, f, r);
+                    emit_window(ii, f, r);
+                }
+#pragma unroll 1
+                for (u32 ii = 0; ii < 16; ++ii) {
+                    if (!((any_mask >> (16 + ii)) & 1)) continue;
+                    u64 f[W], r[W];
+                    km.template keys_h<1>(ii, f, r);
+                    emit_window(16 + ii, f, r);
+                }
             }
         }
     }
@@ -268,6 +348,25 @@ __global__ void __launch_bounds__(256) extract_kernel(ExtractArgs a, DevState *s
     }
     if (do_hist) {
         __syncthreads();
+        if constexpr (shared4) {
+            // position tables: differences over t -> counts (prefix sums, top byte first) ...
+            for (u32 dgt = threadIdx.x; dgt < (u32)kRadix; dgt += blockDim.x) {
+                u32 rf = 0, rr = 0;
+                for (u32 t = 0; t < T; ++t) {
+                    rf += s_posf[t * kRadix + dgt]; s_posf[t * kRadix + dgt] = rf;
+                    rr += s_posr[t * kRadix + dgt]; s_posr[t * kRadix + dgt] = rr;
+                }
+            }
+            __syncthreads();
+            // ... folded into the pass rows: byte t is pass T - t; digit d of the forward strand is the symbol reversal of
+            // f4, of the rc strand its complement
+            for (u32 i = threadIdx.x; i < T * (u32)kRadix; i += blockDim.x) {
+                const u32 t = i >> kRadixBits, dgt = i & (kRadix - 1);
+                const u32 rev = ((dgt & 0x03u) << 6) | ((dgt & 0x0cu) << 2) | ((dgt & 0x30u) >> 2) | ((dgt & 0xc0u) >> 6);
+                s_hist[(T - t) * kRadix + dgt] = s_posf[t * kRadix + rev] + s_posr[t * kRadix + (~dgt & 0xffu)];
+            }
+            __syncthreads();
+        }
         for (int i = threadIdx.x; i < np * kRadix; i += blockDim.x) {
             u32 v = s_hist[i];
             if (v) atomicAdd(&a.digit_hist[i], (u64)v);
@@ -283,9 +382,21 @@ static int launch_extract_w(const ExtractArgs &a, DevState *st, cudaStream_t s) 
     u64 blocks = (ngroups + 255) / 256;
     const u64 maxb = (u64)kNumSMs * 8;
     if (blocks > maxb) blocks = maxb;
-    size_t smem = a.digit_hist ? (size_t)a.passes.n * kRadix * sizeof(u32) : 0;
-    if (filter) extract_kernel<W, true><<<(unsigned)blocks, 256, smem, s>>>(a, st);
-    else        extract_kernel<W, false><<<(unsigned)blocks, 256, smem, s>>>(a, st);
+    const u32 T = (W == 1 && !filter && a.digit_hist && a.k >= 8) ? a.k / 4 : 0;   // 2..7: shared position tables
+    size_t smem = a.digit_hist ? (size_t)(a.passes.n + 2 * T) * kRadix * sizeof(u32) : 0;
+    if (filter) { extract_kernel<W, true, 0><<<(unsigned)blocks, 256, smem, s>>>(a, st); return (int)cudaGetLastError(); }
+    if constexpr (W == 1) {
+        switch (T) {
+            case 2: extract_kernel<1, false, 2><<<(unsigned)blocks, 256, smem, s>>>(a, st); return (int)cudaGetLastError();
+            case 3: extract_kernel<1, false, 3><<<(unsigned)blocks, 256, smem, s>>>(a, st); return (int)cudaGetLastError();
+            case 4: extract_kernel<1, false, 4><<<(unsigned)blocks, 256, smem, s>>>(a, st); return (int)cudaGetLastError();
+            case 5: extract_kernel<1, false, 5><<<(unsigned)blocks, 256, smem, s>>>(a, st); return (int)cudaGetLastError();
+            case 6: extract_kernel<1, false, 6><<<(unsigned)blocks, 256, smem, s>>>(a, st); return (int)cudaGetLastError();
+            case 7: extract_kernel<1, false, 7><<<(unsigned)blocks, 256, smem, s>>>(a, st); return (int)cudaGetLastError();
+            default: break;
+        }
+    }
+    extract_kernel<W, false, 0><<<(unsigned)blocks, 256, smem, s>>>(a, st);
     return (int)cudaGetLastError();
 }
 

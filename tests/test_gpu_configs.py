@@ -36,6 +36,14 @@ def _run_config(cfg, workspace_bytes=None, min_ranges=1, n_buckets=16, full_grap
     st = res.stats
     assert st.n_ranges >= min_ranges, st.n_ranges
     import torch
+    if min_ranges == 1:
+        # the launch configuration bench.py times: no statistics asked for (the extractor's plain path, paired 16-byte
+        # stores and position-counted digit histograms) must give the same edges as the run with checksums above
+        import paper_1409_7208_b200 as sd
+        ed2 = sd.Edges(res.n, w.k)
+        assert sd.sdbg_count_edges(res.ctx, res.reads, w.n_reads, w.k, w.d, ed2, None) == res.n
+        assert torch.equal(ed2.keys[:res.n * ed2.w], res.edges.keys[:res.n * ed2.w]) and torch.equal(ed2.mult[:res.n], res.edges.mult[:res.n])
+        del ed2
     res.ctx.close(); res.ctx.workspace = None                        # the checks below need the HBM
     torch.cuda.empty_cache()
     n_mercy = check_mercy(res, w, res.reads) if full_graph else 0

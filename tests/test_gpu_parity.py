@@ -299,3 +299,25 @@ def test_wide_range_code_path_at_small_size(monkeypatch):
         orc = run_oracle((bases, offs), k, 2)
         assert_matches_oracle(run_gpu((bases, offs), k, 2), orc)
         assert_matches_oracle(run_gpu((bases, offs), k, 2, workspace_bytes=sd.sdbg_min_workspace()), orc)
+
+
+@pytest.mark.parametrize("k", [1, 3, 7, 8, 9, 11, 12, 15, 16, 19, 20, 21, 23, 24, 27, 28, 30, 31, 32, 47, 64, 99])
+def test_plain_path_without_statistics(k):
+    """No checksums, no partition histogram: the extractor's plain path (both keys of a window in one 16-byte store;
+    for one-word keys and k >= 8 the digit histograms of the node bytes counted per read position as differences over
+    the key bytes). Every boundary of floor(k/4) and of the padding bytes is here; reads of ragged lengths, some
+    shorter than a window, put many positions next to a read end."""
+    import random
+    from oracle import run_oracle
+    from tests.gpu_util import run_gpu, assert_matches_oracle
+    from tests.helpers import rc
+    rng = random.Random(500 + k)
+    src = ["".join(rng.choice("ACGT") for _ in range(rng.randint(k + 1, k + 300))) for _ in range(5)]
+    reads = []
+    for _ in range(300):
+        s_ = rng.choice(src)
+        a = rng.randint(0, len(s_)); b = min(len(s_), a + rng.randint(0, k + 80))
+        reads.append(s_[a:b] if rng.random() < 0.5 else rc(s_[a:b]))
+    for d in (1, 2):
+        res = run_gpu(reads, k, d, checksums=False)
+        assert_matches_oracle(res, run_oracle(reads, k, d), check_stats=False)
