@@ -130,9 +130,9 @@ __global__ void __launch_bounds__(256) extract_kernel(ExtractArgs a, DevState *s
     // only per-key atomic. Shared-memory atomics, the bottleneck of this kernel, drop from 8 per key to about 2.4.
     constexpr bool shared4 = T4 >= 2;
     constexpr u32 T = T4;
-    u32 *s_posf = s_hist + np * kRadix, *s_posr = s_posf + T * kRadix;   // [T][256] each (shared4 only)
+    u32 *s_posf = s_hist + np * kRadix, *s_posr = s_posf + (T + 1) * kRadix;   // [T + 1][256] each (shared4 only); row T is a spare
     if (do_hist) {
-        for (int i = threadIdx.x; i < (np + 2 * (int)T) * kRadix; i += blockDim.x) s_hist[i] = 0;
+        for (int i = threadIdx.x; i < (np + (shared4 ? 2 * (int)T + 2 : 0)) * kRadix; i += blockDim.x) s_hist[i] = 0;
         __syncthreads();
     }
     // s_hist row of byte 0 of the last key word if it were a pass (rows of the padding bytes are never touched)
@@ -166,16 +166,13 @@ __global__ void __launch_bounds__(256) extract_kernel(ExtractArgs a, DevState *s
                 auto count_pos = [&](u32 j, u32 f4) {   // f4 = (r[x], r[x+1], r[x+2], r[x+3]) at my slot j
                     const u32 mf = (u32)(V >> (off_f + j)) & pat;       // bit 4t: the window whose forward byte t I am
                     const u32 mr = (u32)(V >> (off_r + j)) & pat;       // bit 4(T-1-t): the window whose rc byte t I am
-                    if (mf) {
-                        const u32 t_lo = ((u32)__ffs(mf) - 1u) >> 2, t_end = ((31u - (u32)__clz(mf)) >> 2) + 1u;
-                        atomicAdd(&s_posf[t_lo * kRadix + f4], 1u);
-                        if (t_end < T) atomicAdd(&s_posf[t_end * kRadix + f4], 0xffffffffu);
-                    }
-                    if (mr) {
-                        const u32 t_lo = T - 1u - ((31u - (u32)__clz(mr)) >> 2), t_end = T - (((u32)__ffs(mr) - 1u) >> 2);
-                        atomicAdd(&s_posr[t_lo * kRadix + f4], 1u);
-                        if (t_end < T) atomicAdd(&s_posr[t_end * kRadix + f4], 0xffffffffu);
-                    }
+                    // branch-free: a position without window (mask 0) and a range that ends at T go to the spare row T
+                    const u32 f_lo = ((u32)__ffs(mf) - 1u) >> 2, f_end = ((31u - (u32)__clz(mf)) >> 2) + 1u;
+                    atomicAdd(&s_posf[(mf ? f_lo : T) * kRadix + f4], 1u);
+                    atomicAdd(&s_posf[(mf ? f_end : T) * kRadix + f4], 0xffffffffu);
+                    const u32 r_lo = T - 1u - ((31u - (u32)__clz(mr)) >> 2), r_end = T - (((u32)__ffs(mr) - 1u) >> 2);
+                    atomicAdd(&s_posr[(mr ? r_lo : T) * kRadix + f4], 1u);
+                    atomicAdd(&s_posr[(mr ? r_end : T) * kRadix + f4], 0xffffffffu);
                 };
                 const u32 b0w = KeyMaker<W>::w32(km.B, 0), b1w = KeyMaker<W>::w32(km.B, 1), b2w = KeyMaker<W>::w32(km.B, 2);
 #pragma unroll 4
@@ -383,7 +380,7 @@ static int launch_extract_w(const ExtractArgs &a, DevState *st, cudaStream_t s) 
     const u64 maxb = (u64)kNumSMs * 8;
     if (blocks > maxb) blocks = maxb;
     const u32 T = (W == 1 && !filter && a.digit_hist && a.k >= 8) ? a.k / 4 : 0;   // 2..7: shared position tables
-    size_t smem = a.digit_hist ? (size_t)(a.passes.n + 2 * T) * kRadix * sizeof(u32) : 0;
+    size_t smem = a.digit_hist ? (size_t)(a.passes.n + (T ? 2 * T + 2 : 0)) * kRadix * sizeof(u32) : 0;
     if (filter) { extract_kernel<W, true, 0><<<(unsigned)blocks, 256, smem, s>>>(a, st); return (int)cudaGetLastError(); }
     if constexpr (W == 1) {
         switch (T) {
