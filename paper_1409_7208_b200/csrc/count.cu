@@ -2,7 +2,8 @@
 // "all (k+1)-mers from the input reads are sorted and counted, and only (k+1)-mers that appear at least d (2 by
 // default) times are kept" (§2 ¶3; cnt >= d, reading A8; counts saturate at 2^32-1, A9).
 //
-// Two streaming sweeps and a scan between them; see count_chunks_kernel.
+// One streaming sweep over the sorted records, a scan, and a short second kernel that copies the solid edges out from
+// what the sweep has noted about them; see count_chunks_kernel and count_write_kernel.
 //
 // Also here: the merge kernels of sdbg_build's unsorted path (equal keys merged by summing mult).
 #include "kernels.cuh"
@@ -43,13 +44,17 @@ __device__ __forceinline__ bool key_lt(const u64 (&a)[W], const u64 (&b)[W]) {  
     return lt;
 }
 
-// Two sweeps over the sorted records with one small scan between them, instead of one sweep whose tiles are chained by
-// a decoupled look-back: a tile lives a few microseconds, and a chain that costs several L2 round trips per tile
-// (measured: ~5 us of a ~9 us tile life) caps the single-sweep kernel far below the cost of simply
-// reading the records twice.
-//   sweep 1 (WRITE = false): solid edges of every chunk -> chunk_sums[chunk]; statistics
+// One sweep over the sorted records, a small scan, and a kernel that copies the solid edges out, instead of one sweep
+// whose tiles are chained by a decoupled look-back: a tile lives a few microseconds, and a chain that costs several
+// L2 round trips per tile (measured: ~5 us of a ~9 us tile life) caps such a kernel far below the
+// cost of the sweep itself.
+//   sweep (this kernel)    : solid edges of every chunk -> chunk_sums[chunk]; statistics; into the stash (the sorter's
+//                            spare buffer, 8 bytes per record at most) the place in the chunk and the multiplicity of
+//                            every solid edge, in order
 //   scan                   : chunk_sums -> exclusive prefix, total -> output cursor
-//   sweep 2 (WRITE = true) : the same arithmetic again, solid edges written at out_base + prefix[chunk] + rank in chunk
+//   count_write_kernel     : the solid edges copied out at out_base + prefix[chunk] + rank in chunk; only their keys
+//                            are fetched again (1.34 -> 1.05 ms on config 2, where 3.6 % of the records end a solid
+//                            run, against a second sweep that redid the arithmetic over all records)
 //
 // A chunk is kCountChunk consecutive records and belongs to ONE WARP, which walks it in rounds of 32 records, lane l
 // holding record 32 r + l (coalesced loads, several rounds in flight). A record i is a run TAIL iff i == n-1 or
@@ -72,7 +77,7 @@ __device__ __forceinline__ void shfl_key(u64 (&dst)[W], const u64 (&src)[W], int
 
 // WIDE: the range holds 2^32 records or more, so a run may be that long: run starts and lengths are 64-bit and the
 // multiplicity saturates at 2^32-1 (reading A9); otherwise 32-bit modular arithmetic is exact.
-template <int W, bool WRITE, bool CSUM, bool WIDE>
+template <int W, bool CSUM, bool WIDE>
 __global__ void __launch_bounds__(kCountWarps * 32, W == 1 ? 6 : W == 2 ? 4 : 2) count_chunks_kernel(CountArgs a, DevState *st) {
     using len_t = std::conditional_t<WIDE, u64, u32>;
     constexpr int G = kCountGroup;
@@ -137,12 +142,6 @@ __global__ void __launch_bounds__(kCountWarps * 32, W == 1 ? 6 : W == 2 ? 4 : 2)
         }
 
         // ---- rounds --------------------------------------------------------------------------------------------
-        u64 out_pos = 0;
-        if constexpr (WRITE) {   // solid edges of earlier ranges + of earlier blocks + of the lower warps of this block
-            out_pos = st->out_cursor[a.range_parity] + a.tile_sums[blockIdx.x];
-            const u32 *ws = reinterpret_cast<const u32 *>(a.tile_sums + gridDim.x) + (u64)blockIdx.x * kCountWarps;
-            for (u32 w = 0; w < warp; ++w) out_pos += ws[w];
-        }
         // one round: FULL = every record of the round and its successor exist (no index checks)
         auto round = [&](auto full_tag, u32 r, const u64 (&k)[W], const u64 (&k_next_round)[W]) {
             constexpr bool FULL = decltype(full_tag)::value;
@@ -159,22 +158,12 @@ __global__ void __launch_bounds__(kCountWarps * 32, W == 1 ? 6 : W == 2 ? 4 : 2)
             const bool solid = tail && len >= (len_t)a.d;
             const u32 S = __ballot_sync(0xffffffffu, solid);
             if (T) carry = (len_t)(r * 32u + (32u - (u32)__clz(T)));
-            if constexpr (!WRITE) {
-                n_tails += (u32)__popc(T);
-                n_solid += (u32)__popc(S);
-                if (solid) sum_mult += len;
-                if constexpr (CSUM) { if (tail) csum += (u64)len * mix_key<W>(k); }
-            } else {
-                if (solid) {
-                    const u64 pos = out_pos + (u32)__popc(S & lt);
-                    if (pos < a.out_cap) {
-#pragma unroll
-                        for (int q = 0; q < W; ++q) a.out_keys[pos * W + q] = k[q];
-                        a.out_mult[pos] = (WIDE && len > (len_t)0xffffffffu) ? 0xffffffffu : (u32)len;   // A9
-                    }
-                }
-                out_pos += (u32)__popc(S);
-            }
+            n_tails += (u32)__popc(T);
+            if (solid)    // where the solid edge sits in its chunk and its multiplicity (A9: saturated), in chunk order
+                a.stash[c0 + n_solid + (u32)__popc(S & lt)] = ((u64)i << 32) | (u64)((WIDE && len > (len_t)0xffffffffu) ? 0xffffffffu : (u32)len);
+            n_solid += (u32)__popc(S);
+            if (solid) sum_mult += len;
+            if constexpr (CSUM) { if (tail) csum += (u64)len * mix_key<W>(k); }
         };
         if (rem == kCountChunk && c0 + kCountChunk + 32u <= a.n) {
             // full chunk with at least 32 records behind it: plain loads, G rounds in flight
@@ -198,7 +187,7 @@ __global__ void __launch_bounds__(kCountWarps * 32, W == 1 ? 6 : W == 2 ? 4 : 2)
             }
         }
     }
-    if constexpr (!WRITE) {
+    {
         // per-warp and per-block numbers of solid edges; statistics: block reduction, one atomic per block and
         // counter, spread over 32 slots
         __shared__ u32 s_solid[kCountWarps];
@@ -260,6 +249,33 @@ __global__ void __launch_bounds__(1024) scan_tiles_kernel(u64 *tile_sums, u32 nt
     }
 }
 
+// Sweep 2 when sweep 1 has left a stash (the spare buffer of the sorter: one 8-byte entry per record at most, chunk by
+// chunk): the solid edges of a chunk are copied out from their (place in chunk, multiplicity) entries — the sorted
+// records are not read a second time, only the keys of the solid edges are fetched (they are a few per cent of the
+// records and their lines were read microseconds ago).
+template <int W>
+__global__ void __launch_bounds__(kCountWarps * 32) count_write_kernel(CountArgs a, const DevState *st) {
+    const u32 lane = threadIdx.x & 31u, warp = threadIdx.x >> 5;
+    const u64 chunk = (u64)blockIdx.x * kCountWarps + warp;
+    const u64 c0 = chunk * kCountChunk;
+    if (c0 >= a.n) return;
+    const u32 *ws = reinterpret_cast<const u32 *>(a.tile_sums + gridDim.x) + (u64)blockIdx.x * kCountWarps;
+    u64 out_pos = st->out_cursor[a.range_parity] + a.tile_sums[blockIdx.x];
+    for (u32 w = 0; w < warp; ++w) out_pos += ws[w];
+    const u32 cnt = ws[warp];
+    for (u32 e = lane; e < cnt; e += 32u) {
+        const u64 ent = a.stash[c0 + e];
+        const u64 pos = out_pos + e;
+        if (pos < a.out_cap) {
+            u64 k[W];
+            load_key<W>(a.keys, c0 + (ent >> 32), k);
+#pragma unroll
+            for (int q = 0; q < W; ++q) a.out_keys[pos * W + q] = k[q];
+            a.out_mult[pos] = (u32)ent;
+        }
+    }
+}
+
 u64 count_tile_records(u32) { return kCountChunk; }
 
 template <int W>
@@ -271,15 +287,14 @@ static int launch_count_w(const CountArgs &a, DevState *st, cudaStream_t s) {
     const bool wide = a.n > 0xffffffffull || a.force_wide;
     const unsigned g = (unsigned)blocks, t = kCountWarps * 32;
     if (wide) {
-        if (a.want_csum) count_chunks_kernel<W, false, true, true><<<g, t, 0, s>>>(a, st);
-        else             count_chunks_kernel<W, false, false, true><<<g, t, 0, s>>>(a, st);
+        if (a.want_csum) count_chunks_kernel<W, true, true><<<g, t, 0, s>>>(a, st);
+        else             count_chunks_kernel<W, false, true><<<g, t, 0, s>>>(a, st);
     } else {
-        if (a.want_csum) count_chunks_kernel<W, false, true, false><<<g, t, 0, s>>>(a, st);
-        else             count_chunks_kernel<W, false, false, false><<<g, t, 0, s>>>(a, st);
+        if (a.want_csum) count_chunks_kernel<W, true, false><<<g, t, 0, s>>>(a, st);
+        else             count_chunks_kernel<W, false, false><<<g, t, 0, s>>>(a, st);
     }
     scan_tiles_kernel<<<1, 1024, 0, s>>>(a.tile_sums, (u32)blocks, st, a.range_parity);
-    if (wide) count_chunks_kernel<W, true, false, true><<<g, t, 0, s>>>(a, st);
-    else      count_chunks_kernel<W, true, false, false><<<g, t, 0, s>>>(a, st);
+    count_write_kernel<W><<<g, t, 0, s>>>(a, st);
     return (int)cudaGetLastError();
 }
 

@@ -81,6 +81,8 @@ struct CountArgs {
     u64 *out_keys; u32 *out_mult; u64 out_cap;
     u64 *tile_sums;          // scratch of 8 bytes per count_tile_records() records: u64 per block of the sweeps (solid
                              // edges, then their exclusive prefix), behind them u32 per warp chunk
+    u64 *stash;              // scratch of 8 bytes per record (the sorter's spare buffer): the sweep leaves (place in chunk,
+                             // multiplicity) of every solid edge there, chunk by chunk
     u64 *stat_slots;         // u64[kStatSlots][kStatSlotWords], accumulated
     int want_csum;
     bool force_wide;         // 64-bit run lengths whatever n is (tests)
