@@ -41,6 +41,7 @@ struct sdbg_ctx {
     std::string err;
     bool timing = false;
     bool force_wide = false;   // SDBG_FORCE_WIDE=1 in the environment at sdbg_ctx_create: see include/sdbg.h
+    bool no_partial = false;   // SDBG_NO_PARTIAL=1 in the environment at sdbg_ctx_create: always sort all records through all passes
     std::vector<EventPair> pending;
     std::vector<cudaEvent_t> free_events;
     sdbg_timing acc{};
@@ -162,6 +163,8 @@ int sdbg_ctx_create(sdbg_ctx **out, int device, void *cuda_stream, void *workspa
     c->ws_bytes = workspace_bytes;
     const char *fw = getenv("SDBG_FORCE_WIDE");
     c->force_wide = fw && fw[0] == '1';
+    const char *np_ = getenv("SDBG_NO_PARTIAL");
+    c->no_partial = np_ && np_[0] == '1';
     *out = c;
     return SDBG_OK;
 }
@@ -200,17 +203,20 @@ uint64_t sdbg_read_slots(uint64_t n_bases, uint64_t n_calls) {
     return (n_bases + 64 * std::max<u64>(n_calls, 1) + 63) / 64 * 64 + SDBG_READ_GUARD_SLOTS;
 }
 
+// room for the (key, count) entries of the partial-sort path (api_count.inc): 12 bytes for up to a sixth of the records
+static u64 partial_slack(u64 n, u32 W) { return W == 1 ? align_up(n * 2) + kStatBytes + 8192 : 0; }
+
 uint64_t sdbg_min_workspace(void) { return kFixedBytes + range_need(1ull << 16, 4); }
 
 uint64_t sdbg_full_workspace(uint64_t n_bases, uint32_t k) {
     if (k < 1 || k > SDBG_MAX_K) return 0;
-    const u64 need = kFixedBytes + range_need(2 * n_bases, sdbg_key_words(k)) + 4096;
+    const u64 need = kFixedBytes + range_need(2 * n_bases, sdbg_key_words(k)) + partial_slack(2 * n_bases, sdbg_key_words(k)) + 4096;
     return std::max<u64>(need, sdbg_min_workspace());
 }
 
 uint64_t sdbg_workspace_for_records(uint64_t n_records, uint32_t k) {
     if (k < 1 || k > SDBG_MAX_K) return 0;
-    const u64 need = kFixedBytes + range_need(n_records, sdbg_key_words(k)) + 4096;
+    const u64 need = kFixedBytes + range_need(n_records, sdbg_key_words(k)) + partial_slack(n_records, sdbg_key_words(k)) + 4096;
     return std::max<u64>(need, sdbg_min_workspace());
 }
 

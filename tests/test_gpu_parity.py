@@ -234,9 +234,9 @@ def test_degenerate_long_runs_poly_A():
     assert int(orc.mult.max()) >= 3000 * (150 - k)          # poly-A forward + poly-T reverse strand
     import paper_1409_7208_b200 as sd
     assert_matches_oracle(run_gpu((bases2, offs2), k, 2), orc)
-    # block-wise: the poly-A partition alone holds 357,000 records; a workspace for 400,000 forces several ranges
+    # block-wise: the poly-A partition alone holds 357,000 records; a workspace for 400,000 forces more than one range
     res = run_gpu((bases2, offs2), k, 2, workspace_bytes=sd.sdbg_workspace_for_records(400000, k))
-    assert res.stats.n_ranges >= 3
+    assert res.stats.n_ranges >= 2
     assert_matches_oracle(res, orc)
     # and a workspace smaller than that partition is refused (reading A12)
     with pytest.raises(sd.SdbgError) as ei:
@@ -321,3 +321,37 @@ def test_plain_path_without_statistics(k):
     for d in (1, 2):
         res = run_gpu(reads, k, d, checksums=False)
         assert_matches_oracle(res, run_oracle(reads, k, d), check_stats=False)
+
+
+@pytest.mark.parametrize("k", [15, 21, 31])
+def test_partial_sort_path_and_its_way_back(k):
+    """The partial-sort path (sort by the first passes on mixed keys, count inside the buckets, sort only the kept
+    entries): (1) high coverage, d = 2: few entries, the path completes; (2) reads without repeats, d = 1: every record
+    is an entry, more than a quarter of the records, so the range is extracted again and sorted the plain way; (3)
+    the same inputs with the path switched off (SDBG_NO_PARTIAL=1 at context creation) give the same edges."""
+    import os
+    import random
+    from oracle import run_oracle
+    from tests.gpu_util import run_gpu, assert_matches_oracle
+    from tests.helpers import rc
+    rng = random.Random(900 + k)
+    genome = "".join(rng.choice("ACGT") for _ in range(3000))
+    covered = []
+    for _ in range(1500):
+        a = rng.randint(0, len(genome) - 100)
+        x = list(genome[a:a + 100])
+        if rng.random() < 0.3:
+            x[rng.randrange(100)] = rng.choice("ACGT")          # one-mismatch copies: the case the key mixing is for
+        x = "".join(x)
+        covered.append(x if rng.random() < 0.5 else rc(x))
+    unique = ["".join(rng.choice("ACGT") for _ in range(120)) for _ in range(400)]
+    for reads, d in ((covered, 2), (unique, 1), (covered + unique, 1)):
+        orc = run_oracle(reads, k, d)
+        res = run_gpu(reads, k, d, checksums=False)
+        assert_matches_oracle(res, orc, check_stats=True)
+        os.environ["SDBG_NO_PARTIAL"] = "1"
+        try:
+            res2 = run_gpu(reads, k, d, checksums=False)
+        finally:
+            del os.environ["SDBG_NO_PARTIAL"]
+        assert_matches_oracle(res2, orc, check_stats=True)
