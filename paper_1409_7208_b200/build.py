@@ -7,7 +7,7 @@ import subprocess
 _DIR = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(_DIR, "csrc")
 LIB = os.path.join(CSRC, "libsdbg.so")
-SOURCES = ["pack.cu", "extract.cu", "radix.cu", "count.cu", "emit.cu", "dummies.cu", "mercy.cu", "rank.cu", "api.cu"]
+SOURCES = ["pack.cu", "extract.cu", "radix.cu", "count.cu", "hashcount.cu", "emit.cu", "dummies.cu", "mercy.cu", "rank.cu", "api.cu"]
 NVCC_FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
               "-Xcompiler", "-fPIC", "-shared"]
 

@@ -41,6 +41,7 @@ struct sdbg_ctx {
     std::string err;
     bool timing = false;
     bool force_wide = false;   // SDBG_FORCE_WIDE=1 in the environment at sdbg_ctx_create: see include/sdbg.h
+    bool no_hash = false;      // SDBG_NO_HASH=1: never count top-sorted records in shared-memory tables (api_count.inc count_range_hash)
     bool no_partial = false;   // SDBG_NO_PARTIAL=1 in the environment at sdbg_ctx_create: always sort all records through all passes
     std::vector<EventPair> pending;
     std::vector<cudaEvent_t> free_events;
@@ -156,6 +157,7 @@ int sdbg_ctx_create(sdbg_ctx **out, int device, void *cuda_stream, void *workspa
     if (cudaGetDeviceCount(&ndev) != cudaSuccess || device < 0 || device >= ndev) { cudaGetLastError(); return SDBG_E_CUDA; }
     if (cudaSetDevice(device) != cudaSuccess) return SDBG_E_CUDA;
     if (radix_setup() != 0) { cudaGetLastError(); return SDBG_E_CUDA; }
+    if (hash_setup() != 0) { cudaGetLastError(); return SDBG_E_CUDA; }
     sdbg_ctx *c = new sdbg_ctx();
     c->device = device;
     c->stream = (cudaStream_t)cuda_stream;
@@ -165,6 +167,8 @@ int sdbg_ctx_create(sdbg_ctx **out, int device, void *cuda_stream, void *workspa
     c->force_wide = fw && fw[0] == '1';
     const char *np_ = getenv("SDBG_NO_PARTIAL");
     c->no_partial = np_ && np_[0] == '1';
+    const char *nh_ = getenv("SDBG_NO_HASH");
+    c->no_hash = c->no_partial || (nh_ && nh_[0] == '1');
     *out = c;
     return SDBG_OK;
 }

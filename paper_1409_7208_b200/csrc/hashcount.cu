@@ -1,0 +1,232 @@
+// hashcount.cu — step a4 for records that are sorted by their TOP key bytes only: "all (k+1)-mers
+// from the input reads are sorted and counted ... only (k+1)-mers that appear at least d (2 by default) times are
+// kept" (§2 ¶4). This is the paper's own partition idea (the k-mers are partitioned by a
+// length-l prefix and consecutive partitions are handled together) carried one level down: after P_hi radix passes over
+// the most significant key bytes all copies of an edge lie inside one run of equal top bytes (a bucket), and a segment
+// of consecutive whole buckets is small enough to be counted in SHARED memory. One CTA per segment:
+//   1 every record of the segment is inserted into an open-addressing table of (key, count) slots in shared memory;
+//   2 the slots with count >= d are sorted by key inside shared memory (bitonic network) — buckets are consecutive in
+//     key order and segments too, so the sorted solid edges of a segment are a contiguous piece of the final output;
+//   3 they are written, with their counts, to the place of the segment in a staging buffer, and the number of them to
+//     seg_count[segment]; a scan and a copy kernel (hash_scan_kernel, hash_copy_kernel) append them in order.
+// Nothing but the solid edges goes through any further pass. Segment borders are found by hash_bounds_kernel.
+// Whatever does not fit (a bucket longer than the search window, a full table, more solid edges than sort places)
+// raises *overflow; the caller then sorts the range the plain way (api_count.inc), so the result is the same.
+#include "kernels.cuh"
+
+namespace sdbg {
+
+constexpr u64 kEmpty = ~0ull;   // an all-ones key (edge T...T at k = 31) is counted beside the table
+
+// first index i in [lo, hi] with (keys[i] >> shift) != t, where the predicate is monotone on [lo, hi) and taken as
+// true at hi; one warp, 32-ary search (every lane returns the result)
+__device__ __forceinline__ u64 warp_first_other(const u64 *__restrict__ keys, u64 lo, u64 hi, u32 shift, u64 t) {
+    const u32 lane = lane_id();
+    while (hi - lo >= 32) {
+        const u64 stride = (hi - lo + 31) / 32;
+        u64 p = lo + (u64)(lane + 1) * stride - 1;      // probes lo+stride-1, lo+2*stride-1, ..., clamped to hi-1
+        if (p > hi - 1) p = hi - 1;
+        const u32 b = __ballot_sync(0xffffffffu, (keys[p] >> shift) != t);
+        if (b == 0) { lo = hi; break; }                  // no record of [lo, hi) differs
+        const u32 f = __ffs(b) - 1;                      // the answer lies behind probe f-1 and not behind probe f
+        hi = __shfl_sync(0xffffffffu, p, f);
+        lo = lo + (u64)f * stride;
+    }
+    const u64 p = lo + lane;
+    const u32 b = __ballot_sync(0xffffffffu, p < hi ? (keys[p] >> shift) != t : true);   // lane hi-lo <= 31 says true
+    return lo + (u64)(__ffs(b) - 1);
+}
+
+// seg_start[c], c in [0, nchunks]: the first bucket border at or after record c * chunk (n for c = nchunks). A bucket
+// that runs on for more than `window` records past the nominal place raises *overflow.
+__global__ void __launch_bounds__(256) hash_bounds_kernel(const u64 *__restrict__ keys, u64 n, u32 shift, u32 chunk, u32 window,
+                                                          u64 nchunks, u64 *__restrict__ seg_start, u32 *overflow) {
+    const u64 c = (u64)blockIdx.x * 8 + (threadIdx.x >> 5);
+    if (c > nchunks) return;
+    u64 res;
+    const u64 x = c * chunk;
+    if (c == 0) res = 0;
+    else if (x >= n) res = n;
+    else {
+        const u64 t = keys[x - 1] >> shift;
+        if ((keys[x] >> shift) != t) res = x;
+        else {
+            const u64 lim = x + window < n ? x + window : n;
+            res = warp_first_other(keys, x, lim, shift, t);
+            if (res == lim && lim < n && lane_id() == 0) atomicOr(overflow, 1u);   // not a border (or unknown): give up
+        }
+    }
+    if (lane_id() == 0) seg_start[c] = res;
+}
+
+template <int THREADS>
+__global__ void __launch_bounds__(THREADS, 2)
+hash_count_kernel(HashCountArgs a) {
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    const u32 TS = a.table_slots, mask = TS - 1u, hshift = 32u - (u32)__ffs(TS) + 1u;
+    u64 *t_key = reinterpret_cast<u64 *>(smem_raw);                  // u64[TS]
+    u32 *t_cnt = reinterpret_cast<u32 *>(smem_raw + (size_t)TS * 8); // u32[TS]
+    __shared__ u32 s_ones, s_full, s_nsolid, s_distinct;
+    __shared__ u64 s_sum;
+    const u32 tid = threadIdx.x;
+    const u64 seg = blockIdx.x;
+    const u64 s = a.seg_start[seg], e = a.seg_start[seg + 1];
+    if (e <= s) { if (tid == 0) a.seg_count[seg] = 0; return; }
+
+    for (u32 i = tid; i < TS; i += THREADS) { t_key[i] = kEmpty; t_cnt[i] = 0; }
+    if (tid == 0) { s_ones = 0; s_full = 0; s_nsolid = 0; s_distinct = 0; s_sum = 0; }
+    __syncthreads();
+
+    // ---- 1: insert ---------------------------------------------------------------------------------------------------
+    u32 created = 0;
+    for (u64 i = s + tid; i < e; i += THREADS) {
+        const u64 key = ld_stream(a.keys + i);
+        if (key == kEmpty) { atomicAdd(&s_ones, 1u); continue; }
+        u32 h = ((u32)key ^ (u32)(key >> 32)) * 0x9E3779B1u;
+        h ^= (u32)(key >> 20);
+        u32 slot = (h * 0x85EBCA6Bu) >> hshift;
+        for (u32 probes = 0;; ++probes) {
+            u64 cur = t_key[slot];
+            if (cur == kEmpty) {
+                cur = atomicCAS(&t_key[slot], kEmpty, key);
+                if (cur == kEmpty) { ++created; cur = key; }
+            }
+            if (cur == key) { atomicAdd(&t_cnt[slot], 1u); break; }
+            slot = (slot + 1u) & mask;
+            if (probes >= TS) { s_full = 1; break; }
+        }
+    }
+    if (created) atomicAdd(&s_distinct, created);
+    __syncthreads();
+    if (s_full) { if (tid == 0) { atomicOr(a.overflow, 2u); a.seg_count[seg] = 0; } return; }
+
+    // ---- 2: the solid slots, compacted to the front of a list in shared memory (reusing the table in place is not
+    //         possible while it is read, so the list lives behind it) ------------------------------------------------------
+    u64 *l_key = reinterpret_cast<u64 *>(smem_raw + (size_t)TS * 12);               // u64[kMaxSolid]
+    u32 *l_cnt = reinterpret_cast<u32 *>(smem_raw + (size_t)TS * 12 + (size_t)a.max_solid * 8);
+    u64 sum = 0;
+    for (u32 i = tid; i < TS; i += THREADS) {
+        const u32 c = t_cnt[i];
+        if (c >= a.d) {
+            const u32 p = atomicAdd(&s_nsolid, 1u);
+            if (p < a.max_solid) { l_key[p] = t_key[i]; l_cnt[p] = c; }
+            sum += c;
+        }
+    }
+    if (tid == 0 && s_ones) {
+        ++s_distinct;                                    // nobody else touches it between the barriers
+        if (s_ones >= a.d) {
+            const u32 p = atomicAdd(&s_nsolid, 1u);
+            if (p < a.max_solid) { l_key[p] = kEmpty; l_cnt[p] = s_ones; }
+            sum += s_ones;
+        }
+    }
+    sum = warp_reduce_add64(sum);
+    if ((tid & 31u) == 0 && sum) atomicAdd(&s_sum, sum);
+    __syncthreads();
+    const u32 ns = s_nsolid;
+    if (ns > a.max_solid) { if (tid == 0) { atomicOr(a.overflow, 4u); a.seg_count[seg] = 0; } return; }
+    if (tid == 0) {
+        a.seg_count[seg] = ns;
+        u64 *slot = a.stat_slots + (size_t)(blockIdx.x & (kStatSlots - 1)) * kStatSlotWords;
+        atomicAdd(&slot[0], (u64)s_distinct);
+        if (s_sum) atomicAdd(&slot[1], s_sum);
+    }
+    if (ns == 0) return;
+
+    // ---- 3: bitonic sort of the list by key (padded with all-ones keys behind place ns; a real all-ones key is the
+    //         largest key anyway and comes with a count > 0, pads have count 0 and are never written) -------------------
+    u32 np = 1; while (np < ns) np <<= 1;
+    for (u32 i = ns + tid; i < np; i += THREADS) { l_key[i] = kEmpty; l_cnt[i] = 0; }
+    __syncthreads();
+    for (u32 k2 = 2; k2 <= np; k2 <<= 1) {
+        for (u32 j = k2 >> 1; j > 0; j >>= 1) {
+            for (u32 i = tid; i < (np >> 1); i += THREADS) {
+                const u32 lo = ((i & ~(j - 1u)) << 1) | (i & (j - 1u)), hi = lo | j;   // the pair (lo, lo + j)
+                const bool up = (lo & k2) == 0;
+                const u64 ka = l_key[lo], kb = l_key[hi];
+                const u32 ca = l_cnt[lo], cb = l_cnt[hi];
+                // order by (key, count > 0 first): a real all-ones key stays in front of the pads
+                const bool gt = ka > kb || (ka == kb && ca < cb);
+                if (gt == up) { l_key[lo] = kb; l_key[hi] = ka; l_cnt[lo] = cb; l_cnt[hi] = ca; }
+            }
+            __syncthreads();
+        }
+    }
+    // ---- write the sorted solid edges of the segment to its place in the staging buffer ---------------------------------
+    // staging (8 bytes per record, the sorter's spare buffer): the segment owns places [s, e); its ns <= (e - s) / d solid
+    // keys (d >= 2) fill the first half at most, their u32 counts start at the middle place
+    u32 *stage_cnt = reinterpret_cast<u32 *>(a.stage_keys + s + ((e - s + 1) >> 1));
+    for (u32 i = tid; i < ns; i += THREADS) { a.stage_keys[s + i] = l_key[i]; stage_cnt[i] = l_cnt[i]; }
+}
+
+// seg_count -> exclusive prefix in place (u64), total to *total; one block, sequential over tiles of 1024 (the array has
+// n / chunk entries: 97 k on config 2, 775 k on config 3)
+__global__ void __launch_bounds__(1024) hash_scan_kernel(u64 *__restrict__ seg_count, u64 nseg, u64 *total) {
+    __shared__ u64 s_w[32];
+    __shared__ u64 s_carry;
+    const u32 tid = threadIdx.x, lane = tid & 31u, warp = tid >> 5;
+    if (tid == 0) s_carry = 0;
+    __syncthreads();
+    for (u64 base = 0; base < nseg; base += 1024) {
+        const u64 i = base + tid;
+        const u64 v = i < nseg ? seg_count[i] : 0;
+        u64 incl = v;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            u64 t = __shfl_up_sync(0xffffffffu, incl, o);
+            if (lane >= (u32)o) incl += t;
+        }
+        if (lane == 31) s_w[warp] = incl;
+        __syncthreads();
+        u64 off = s_carry;
+        for (u32 w = 0; w < warp; ++w) off += s_w[w];
+        if (i < nseg) seg_count[i] = off + incl - v;
+        __syncthreads();
+        if (tid == 1023) s_carry = off + incl;
+        __syncthreads();
+    }
+    if (tid == 0) *total = s_carry;
+}
+
+// the staged solid edges of every segment appended to the output, in segment (= key) order; one warp per segment
+__global__ void __launch_bounds__(256) hash_copy_kernel(HashCountArgs a, const u64 *__restrict__ total, DevState *st, int range_parity) {
+    const u64 base = st->out_cursor[range_parity];
+    const u32 lane = lane_id();
+    for (u64 seg = (u64)blockIdx.x * 8 + (threadIdx.x >> 5); seg < a.nseg; seg += (u64)gridDim.x * 8) {
+        const u64 off = a.seg_count[seg];
+        const u64 cnt = (seg + 1 < a.nseg ? a.seg_count[seg + 1] : *total) - off;
+        const u64 s = a.seg_start[seg], e = a.seg_start[seg + 1];
+        const u32 *stage_cnt = reinterpret_cast<const u32 *>(a.stage_keys + s + ((e - s + 1) >> 1));
+        for (u64 i = lane; i < cnt; i += 32) {
+            const u64 pos = base + off + i;
+            if (pos < a.out_cap) { a.out_keys[pos] = a.stage_keys[s + i]; a.out_mult[pos] = stage_cnt[i]; }
+        }
+    }
+    if (blockIdx.x == 0 && threadIdx.x == 0) st->out_cursor[range_parity ^ 1] = base + *total;
+}
+
+constexpr int kHashThreads = 512;
+u64 hash_smem_bytes(u32 table_slots, u32 max_solid) { return (u64)table_slots * 12 + (u64)max_solid * 12; }
+
+int hash_setup() {
+    return (int)cudaFuncSetAttribute(hash_count_kernel<kHashThreads>, cudaFuncAttributeMaxDynamicSharedMemorySize, 110 * 1024);
+}
+
+void launch_hash_bounds(const HashCountArgs &a, cudaStream_t s) {
+    const u64 warps = a.nseg + 1, blocks = (warps + 7) / 8;
+    hash_bounds_kernel<<<(unsigned)blocks, 256, 0, s>>>(a.keys, a.n, a.top_shift, a.chunk, a.window, a.nseg, a.seg_start, a.overflow);
+}
+int launch_hash_count(const HashCountArgs &a, cudaStream_t s) {
+    if (a.nseg == 0 || a.nseg > 0x7fffffffull) return (int)cudaErrorInvalidValue;
+    hash_count_kernel<kHashThreads><<<(unsigned)a.nseg, kHashThreads, hash_smem_bytes(a.table_slots, a.max_solid), s>>>(a);
+    return (int)cudaGetLastError();
+}
+void launch_hash_append(const HashCountArgs &a, u64 *total, DevState *st, int range_parity, cudaStream_t s) {
+    hash_scan_kernel<<<1, 1024, 0, s>>>(a.seg_count, a.nseg, total);
+    u64 blocks = (a.nseg + 7) / 8;
+    if (blocks > (u64)kNumSMs * 16) blocks = (u64)kNumSMs * 16;
+    hash_copy_kernel<<<(unsigned)blocks, 256, 0, s>>>(a, total, st, range_parity);
+}
+
+}  // namespace sdbg

@@ -102,6 +102,25 @@ void launch_solid_flags(const u32 *mult, u64 n, u32 d, uint8_t *flags, u64 *stat
 void launch_append_solid(const u64 *keys, const u32 *mult, const u32 *idx, const u64 *n_idx, u64 n_max, u64 *out_keys, u32 *out_mult,
                          u64 out_cap, DevState *st, int range_parity, cudaStream_t s);
 
+// records sorted by their top key bytes only: count in shared-memory tables, segment by segment (hashcount.cu)
+struct HashCountArgs {
+    const u64 *keys; u64 n;              // one-word keys sorted by key >> top_shift
+    u32 top_shift, chunk, window;        // nominal records per segment; how far a bucket may run past a nominal border
+    u32 table_slots, max_solid, d;       // table slots (power of two) and sort places of a CTA; d >= 2
+    u64 nseg;                            // ceil(n / chunk)
+    u64 *seg_start;                      // u64[nseg + 1] scratch
+    u64 *seg_count;                      // u64[nseg + 1] scratch: solid edges per segment, then their exclusive prefix
+    u32 *overflow;                       // zeroed; nonzero afterwards: something did not fit, nothing may be used
+    u64 *stage_keys;                     // u64[n] scratch (the sorter's spare buffer)
+    u64 *stat_slots;
+    u64 *out_keys; u32 *out_mult; u64 out_cap;
+};
+int hash_setup();
+u64 hash_smem_bytes(u32 table_slots, u32 max_solid);
+void launch_hash_bounds(const HashCountArgs &a, cudaStream_t s);
+int launch_hash_count(const HashCountArgs &a, cudaStream_t s);
+void launch_hash_append(const HashCountArgs &a, u64 *total, DevState *st, int range_parity, cudaStream_t s);
+
 struct EmitArgs {
     const u64 *keys; const u32 *mult_in; u64 n; u32 k, W;
     uint8_t *Wout; u32 *last_bits32; u32 *mult_out;
