@@ -5,8 +5,9 @@
 // the most significant key bytes all copies of an edge lie inside one run of equal top bytes (a bucket), and a segment
 // of consecutive whole buckets is small enough to be counted in SHARED memory. One CTA per segment:
 //   1 every record of the segment is inserted into an open-addressing table of (key, count) slots in shared memory;
-//   2 the slots with count >= d are sorted by key inside shared memory (bitonic network) — buckets are consecutive in
-//     key order and segments too, so the sorted solid edges of a segment are a contiguous piece of the final output;
+//   2 the slots with count >= d are put in key order inside shared memory (one pass of order-preserving binning, then
+//     insertion inside the tiny bins) — buckets are consecutive in key order and segments too, so the ordered solid edges
+//     of a segment are a contiguous piece of the final output;
 //   3 they are written, with their counts, to the place of the segment in a staging buffer, and the number of them to
 //     seg_count[segment]; a scan and a copy kernel (hash_scan_kernel, hash_copy_kernel) append them in order.
 // Nothing but the solid edges goes through any further pass. Segment borders are found by hash_bounds_kernel.
@@ -63,25 +64,37 @@ template <int THREADS>
 __global__ void __launch_bounds__(THREADS, 2)
 hash_count_kernel(HashCountArgs a) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    const u32 TS = a.table_slots, mask = TS - 1u, hshift = 32u - (u32)__ffs(TS) + 1u;
-    u64 *t_key = reinterpret_cast<u64 *>(smem_raw);                  // u64[TS]
-    u32 *t_cnt = reinterpret_cast<u32 *>(smem_raw + (size_t)TS * 8); // u32[TS]
+    constexpr int U = 8;                                              // loads in flight per thread
+    u64 *t_key = reinterpret_cast<u64 *>(smem_raw);                  // u64[table_slots]
+    u32 *t_cnt = reinterpret_cast<u32 *>(smem_raw + (size_t)a.table_slots * 8); // u32[table_slots]
     __shared__ u32 s_ones, s_full, s_nsolid, s_distinct;
     __shared__ u64 s_sum;
     const u32 tid = threadIdx.x;
     const u64 seg = blockIdx.x;
     const u64 s = a.seg_start[seg], e = a.seg_start[seg + 1];
     if (e <= s) { if (tid == 0) a.seg_count[seg] = 0; return; }
-
-    for (u32 i = tid; i < TS; i += THREADS) { t_key[i] = kEmpty; t_cnt[i] = 0; }
+    const u64 kfirst = a.keys[s] >> a.top_shift, klast = a.keys[e - 1] >> a.top_shift;   // first and last bucket of the segment
+    // the first U records of every thread are on their way while the table is cleared
+    u64 kq[U];
+#pragma unroll
+    for (int u = 0; u < U; ++u) { const u64 i = s + (u64)u * THREADS + tid; kq[u] = i < e ? ld_stream(a.keys + i) : 0ull; }
+    // table size: the power of two from 1.5 x the records of the segment on (all of them might be distinct)
+    u32 TS = 1024;
+    while (TS < a.table_slots && (u64)TS * 2 < (e - s) * 3) TS <<= 1;
+    const u32 mask = TS - 1u, hshift = 32u - (u32)__ffs(TS) + 1u;
+    {
+        uint4 *k4 = reinterpret_cast<uint4 *>(t_key), *c4 = reinterpret_cast<uint4 *>(t_cnt);
+        const uint4 ones = make_uint4(~0u, ~0u, ~0u, ~0u), zero = make_uint4(0u, 0u, 0u, 0u);
+        for (u32 i = tid; i < TS / 2; i += THREADS) k4[i] = ones;
+        for (u32 i = tid; i < TS / 4; i += THREADS) c4[i] = zero;
+    }
     if (tid == 0) { s_ones = 0; s_full = 0; s_nsolid = 0; s_distinct = 0; s_sum = 0; }
     __syncthreads();
 
     // ---- 1: insert ---------------------------------------------------------------------------------------------------
     u32 created = 0;
-    for (u64 i = s + tid; i < e; i += THREADS) {
-        const u64 key = ld_stream(a.keys + i);
-        if (key == kEmpty) { atomicAdd(&s_ones, 1u); continue; }
+    auto insert = [&](u64 key) {
+        if (key == kEmpty) { atomicAdd(&s_ones, 1u); return; }
         u32 h = ((u32)key ^ (u32)(key >> 32)) * 0x9E3779B1u;
         h ^= (u32)(key >> 20);
         u32 slot = (h * 0x85EBCA6Bu) >> hshift;
@@ -95,6 +108,14 @@ hash_count_kernel(HashCountArgs a) {
             slot = (slot + 1u) & mask;
             if (probes >= TS) { s_full = 1; break; }
         }
+    };
+    for (u64 base = s;;) {
+#pragma unroll
+        for (int u = 0; u < U; ++u) if (base + (u64)u * THREADS + tid < e) insert(kq[u]);
+        base += (u64)U * THREADS;
+        if (base >= e) break;
+#pragma unroll
+        for (int u = 0; u < U; ++u) { const u64 i = base + (u64)u * THREADS + tid; kq[u] = i < e ? ld_stream(a.keys + i) : 0ull; }
     }
     if (created) atomicAdd(&s_distinct, created);
     __syncthreads();
@@ -102,10 +123,10 @@ hash_count_kernel(HashCountArgs a) {
 
     // ---- 2: the solid slots, compacted to the front of a list in shared memory (reusing the table in place is not
     //         possible while it is read, so the list lives behind it) ------------------------------------------------------
-    u64 *l_key = reinterpret_cast<u64 *>(smem_raw + (size_t)TS * 12);               // u64[kMaxSolid]
-    u32 *l_cnt = reinterpret_cast<u32 *>(smem_raw + (size_t)TS * 12 + (size_t)a.max_solid * 8);
+    u64 *l_key = reinterpret_cast<u64 *>(smem_raw + (size_t)a.table_slots * 12);    // u64[max_solid]
+    u32 *l_cnt = reinterpret_cast<u32 *>(smem_raw + (size_t)a.table_slots * 12 + (size_t)a.max_solid * 8);
     u64 sum = 0;
-    for (u32 i = tid; i < TS; i += THREADS) {
+    for (u32 i = tid; i < TS; i += THREADS) {                    // the live part of the table
         const u32 c = t_cnt[i];
         if (c >= a.d) {
             const u32 p = atomicAdd(&s_nsolid, 1u);
@@ -134,30 +155,57 @@ hash_count_kernel(HashCountArgs a) {
     }
     if (ns == 0) return;
 
-    // ---- 3: bitonic sort of the list by key (padded with all-ones keys behind place ns; a real all-ones key is the
-    //         largest key anyway and comes with a count > 0, pads have count 0 and are never written) -------------------
-    u32 np = 1; while (np < ns) np <<= 1;
-    for (u32 i = ns + tid; i < np; i += THREADS) { l_key[i] = kEmpty; l_cnt[i] = 0; }
+    // ---- 3: order the list by key. The solid edges of a segment are spread evenly over its key range, so one pass of
+    //         order-preserving binning (1,024 bins over the range of the segment's buckets) leaves bins of one or two
+    //         entries, which the owner of the bin puts in order by insertion. The table is dead: bins and the ordered
+    //         list live in its place. -----------------------------------------------------------------------------------
+    constexpr int NB = 2 * THREADS;                                   // bins; also the most entries a segment may have
+    u32 *bins = t_cnt;
+    u64 *o_key = t_key;
+    u32 *o_cnt = reinterpret_cast<u32 *>(t_key + NB);
+    const u64 k0 = kfirst << a.top_shift;
+    const u64 rm1 = ((klast - kfirst + 1ull) << a.top_shift) - 1ull;  // largest offset inside the segment's buckets
+    const int sh0 = 54 - __clzll((long long)rm1), sh = sh0 > 0 ? sh0 : 0;   // (rm1 >> sh) < 1024
+    bins[tid] = 0; bins[tid + THREADS] = 0;
     __syncthreads();
-    for (u32 k2 = 2; k2 <= np; k2 <<= 1) {
-        for (u32 j = k2 >> 1; j > 0; j >>= 1) {
-            for (u32 i = tid; i < (np >> 1); i += THREADS) {
-                const u32 lo = ((i & ~(j - 1u)) << 1) | (i & (j - 1u)), hi = lo | j;   // the pair (lo, lo + j)
-                const bool up = (lo & k2) == 0;
-                const u64 ka = l_key[lo], kb = l_key[hi];
-                const u32 ca = l_cnt[lo], cb = l_cnt[hi];
-                // order by (key, count > 0 first): a real all-ones key stays in front of the pads
-                const bool gt = ka > kb || (ka == kb && ca < cb);
-                if (gt == up) { l_key[lo] = kb; l_key[hi] = ka; l_cnt[lo] = cb; l_cnt[hi] = ca; }
-            }
-            __syncthreads();
+    u32 myb[2] = {0, 0}, myr[2] = {0, 0};
+#pragma unroll
+    for (int q = 0; q < 2; ++q) {
+        const u32 i = tid + q * THREADS;
+        if (i < ns) { myb[q] = (u32)((l_key[i] - k0) >> sh); myr[q] = atomicAdd(&bins[myb[q]], 1u); }
+    }
+    __syncthreads();
+    __shared__ u32 s_w[THREADS / 32];
+    const u32 c0 = bins[2 * tid], c1 = bins[2 * tid + 1];
+    const u32 incl = warp_incl_scan_add(c0 + c1);
+    if ((tid & 31u) == 31u) s_w[tid >> 5] = incl;
+    __syncthreads();
+    u32 base0 = incl - (c0 + c1);
+    for (u32 w = 0; w < (tid >> 5); ++w) base0 += s_w[w];
+    bins[2 * tid] = base0; bins[2 * tid + 1] = base0 + c0;
+    __syncthreads();
+#pragma unroll
+    for (int q = 0; q < 2; ++q) {
+        const u32 i = tid + q * THREADS;
+        if (i < ns) { const u32 p = bins[myb[q]] + myr[q]; o_key[p] = l_key[i]; o_cnt[p] = l_cnt[i]; }
+    }
+    __syncthreads();
+#pragma unroll
+    for (int q = 0; q < 2; ++q) {
+        const u32 c = q ? c1 : c0, b0 = q ? base0 + c0 : base0;
+        for (u32 x = 1; x < c; ++x) {                                  // insertion sort of places [b0, b0 + c)
+            const u64 kx = o_key[b0 + x]; const u32 cx = o_cnt[b0 + x];
+            u32 y = x;
+            while (y > 0 && o_key[b0 + y - 1] > kx) { o_key[b0 + y] = o_key[b0 + y - 1]; o_cnt[b0 + y] = o_cnt[b0 + y - 1]; --y; }
+            o_key[b0 + y] = kx; o_cnt[b0 + y] = cx;
         }
     }
+    __syncthreads();
     // ---- write the sorted solid edges of the segment to its place in the staging buffer ---------------------------------
     // staging (8 bytes per record, the sorter's spare buffer): the segment owns places [s, e); its ns <= (e - s) / d solid
     // keys (d >= 2) fill the first half at most, their u32 counts start at the middle place
     u32 *stage_cnt = reinterpret_cast<u32 *>(a.stage_keys + s + ((e - s + 1) >> 1));
-    for (u32 i = tid; i < ns; i += THREADS) { a.stage_keys[s + i] = l_key[i]; stage_cnt[i] = l_cnt[i]; }
+    for (u32 i = tid; i < ns; i += THREADS) { a.stage_keys[s + i] = o_key[i]; stage_cnt[i] = o_cnt[i]; }
 }
 
 // seg_count -> exclusive prefix in place (u64), total to *total; one block, sequential over tiles of 1024 (the array has
