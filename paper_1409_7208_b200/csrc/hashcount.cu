@@ -60,11 +60,10 @@ __global__ void __launch_bounds__(256) hash_bounds_kernel(const u64 *__restrict_
     if (lane_id() == 0) seg_start[c] = res;
 }
 
-template <int THREADS>
-__global__ void __launch_bounds__(THREADS, 2)
+template <int THREADS, int MINB, int U>   // U = loads in flight per thread
+__global__ void __launch_bounds__(THREADS, MINB)
 hash_count_kernel(HashCountArgs a) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    constexpr int U = 8;                                              // loads in flight per thread
     u64 *t_key = reinterpret_cast<u64 *>(smem_raw);                  // u64[table_slots]
     u32 *t_cnt = reinterpret_cast<u32 *>(smem_raw + (size_t)a.table_slots * 8); // u32[table_slots]
     __shared__ u32 s_ones, s_full, s_nsolid, s_distinct;
@@ -159,45 +158,56 @@ hash_count_kernel(HashCountArgs a) {
     //         order-preserving binning (1,024 bins over the range of the segment's buckets) leaves bins of one or two
     //         entries, which the owner of the bin puts in order by insertion. The table is dead: bins and the ordered
     //         list live in its place. -----------------------------------------------------------------------------------
-    constexpr int NB = 2 * THREADS;                                   // bins; also the most entries a segment may have
+    constexpr int NB = 1024, Q = NB / THREADS;                        // bins (also the most entries of a segment); per thread
     u32 *bins = t_cnt;
     u64 *o_key = t_key;
     u32 *o_cnt = reinterpret_cast<u32 *>(t_key + NB);
     const u64 k0 = kfirst << a.top_shift;
     const u64 rm1 = ((klast - kfirst + 1ull) << a.top_shift) - 1ull;  // largest offset inside the segment's buckets
     const int sh0 = 54 - __clzll((long long)rm1), sh = sh0 > 0 ? sh0 : 0;   // (rm1 >> sh) < 1024
-    bins[tid] = 0; bins[tid + THREADS] = 0;
-    __syncthreads();
-    u32 myb[2] = {0, 0}, myr[2] = {0, 0};
 #pragma unroll
-    for (int q = 0; q < 2; ++q) {
+    for (int q = 0; q < Q; ++q) bins[tid + q * THREADS] = 0;
+    __syncthreads();
+    u32 myb[Q], myr[Q];
+#pragma unroll
+    for (int q = 0; q < Q; ++q) {
         const u32 i = tid + q * THREADS;
+        myb[q] = 0; myr[q] = 0;
         if (i < ns) { myb[q] = (u32)((l_key[i] - k0) >> sh); myr[q] = atomicAdd(&bins[myb[q]], 1u); }
     }
     __syncthreads();
     __shared__ u32 s_w[THREADS / 32];
-    const u32 c0 = bins[2 * tid], c1 = bins[2 * tid + 1];
-    const u32 incl = warp_incl_scan_add(c0 + c1);
+    u32 c[Q], csum = 0;
+#pragma unroll
+    for (int q = 0; q < Q; ++q) { c[q] = bins[Q * tid + q]; csum += c[q]; }
+    const u32 incl = warp_incl_scan_add(csum);
     if ((tid & 31u) == 31u) s_w[tid >> 5] = incl;
     __syncthreads();
-    u32 base0 = incl - (c0 + c1);
+    u32 base0 = incl - csum;
     for (u32 w = 0; w < (tid >> 5); ++w) base0 += s_w[w];
-    bins[2 * tid] = base0; bins[2 * tid + 1] = base0 + c0;
+    {
+        u32 run = base0;
+#pragma unroll
+        for (int q = 0; q < Q; ++q) { bins[Q * tid + q] = run; run += c[q]; }
+    }
     __syncthreads();
 #pragma unroll
-    for (int q = 0; q < 2; ++q) {
+    for (int q = 0; q < Q; ++q) {
         const u32 i = tid + q * THREADS;
         if (i < ns) { const u32 p = bins[myb[q]] + myr[q]; o_key[p] = l_key[i]; o_cnt[p] = l_cnt[i]; }
     }
     __syncthreads();
+    {
+        u32 b0 = base0;
 #pragma unroll
-    for (int q = 0; q < 2; ++q) {
-        const u32 c = q ? c1 : c0, b0 = q ? base0 + c0 : base0;
-        for (u32 x = 1; x < c; ++x) {                                  // insertion sort of places [b0, b0 + c)
-            const u64 kx = o_key[b0 + x]; const u32 cx = o_cnt[b0 + x];
-            u32 y = x;
-            while (y > 0 && o_key[b0 + y - 1] > kx) { o_key[b0 + y] = o_key[b0 + y - 1]; o_cnt[b0 + y] = o_cnt[b0 + y - 1]; --y; }
-            o_key[b0 + y] = kx; o_cnt[b0 + y] = cx;
+        for (int q = 0; q < Q; ++q) {
+            for (u32 x = 1; x < c[q]; ++x) {                           // insertion sort of places [b0, b0 + c)
+                const u64 kx = o_key[b0 + x]; const u32 cx = o_cnt[b0 + x];
+                u32 y = x;
+                while (y > 0 && o_key[b0 + y - 1] > kx) { o_key[b0 + y] = o_key[b0 + y - 1]; o_cnt[b0 + y] = o_cnt[b0 + y - 1]; --y; }
+                o_key[b0 + y] = kx; o_cnt[b0 + y] = cx;
+            }
+            b0 += c[q];
         }
     }
     __syncthreads();
@@ -208,18 +218,21 @@ hash_count_kernel(HashCountArgs a) {
     for (u32 i = tid; i < ns; i += THREADS) { a.stage_keys[s + i] = o_key[i]; stage_cnt[i] = o_cnt[i]; }
 }
 
-// seg_count -> exclusive prefix in place (u64), total to *total; one block, sequential over tiles of 1024 (the array has
-// n / chunk entries: 97 k on config 2, 775 k on config 3)
+// seg_count -> exclusive prefix in place (u64), total to *total; one block, tiles of 4,096 (the array has n / chunk
+// entries: 97 k on config 2, 1.5 M on config 3)
 __global__ void __launch_bounds__(1024) hash_scan_kernel(u64 *__restrict__ seg_count, u64 nseg, u64 *total) {
     __shared__ u64 s_w[32];
     __shared__ u64 s_carry;
     const u32 tid = threadIdx.x, lane = tid & 31u, warp = tid >> 5;
     if (tid == 0) s_carry = 0;
     __syncthreads();
-    for (u64 base = 0; base < nseg; base += 1024) {
-        const u64 i = base + tid;
-        const u64 v = i < nseg ? seg_count[i] : 0;
-        u64 incl = v;
+    for (u64 base = 0; base < nseg; base += 4096) {
+        const u64 i = base + 4ull * tid;
+        u64 v[4];
+#pragma unroll
+        for (int q = 0; q < 4; ++q) v[q] = i + q < nseg ? seg_count[i + q] : 0;
+        const u64 sum = v[0] + v[1] + v[2] + v[3];
+        u64 incl = sum;
 #pragma unroll
         for (int o = 1; o < 32; o <<= 1) {
             u64 t = __shfl_up_sync(0xffffffffu, incl, o);
@@ -229,7 +242,9 @@ __global__ void __launch_bounds__(1024) hash_scan_kernel(u64 *__restrict__ seg_c
         __syncthreads();
         u64 off = s_carry;
         for (u32 w = 0; w < warp; ++w) off += s_w[w];
-        if (i < nseg) seg_count[i] = off + incl - v;
+        u64 run = off + incl - sum;
+#pragma unroll
+        for (int q = 0; q < 4; ++q) { if (i + q < nseg) seg_count[i + q] = run; run += v[q]; }
         __syncthreads();
         if (tid == 1023) s_carry = off + incl;
         __syncthreads();
@@ -254,11 +269,14 @@ __global__ void __launch_bounds__(256) hash_copy_kernel(HashCountArgs a, const u
     if (blockIdx.x == 0 && threadIdx.x == 0) st->out_cursor[range_parity ^ 1] = base + *total;
 }
 
-constexpr int kHashThreads = 512;
+// two shapes: big segments (chunk 4,096: one or two long buckets) 512 threads x 2 CTAs per SM with 8,192 slots; small
+// segments (chunk 2,048: many short buckets) 256 threads x 3 CTAs per SM with 4,096 slots
 u64 hash_smem_bytes(u32 table_slots, u32 max_solid) { return (u64)table_slots * 12 + (u64)max_solid * 12; }
 
 int hash_setup() {
-    return (int)cudaFuncSetAttribute(hash_count_kernel<kHashThreads>, cudaFuncAttributeMaxDynamicSharedMemorySize, 110 * 1024);
+    int e = (int)cudaFuncSetAttribute(hash_count_kernel<512, 2, 8>, cudaFuncAttributeMaxDynamicSharedMemorySize, 110 * 1024);
+    if (e) return e;
+    return (int)cudaFuncSetAttribute(hash_count_kernel<256, 3, 9>, cudaFuncAttributeMaxDynamicSharedMemorySize, 62 * 1024);
 }
 
 void launch_hash_bounds(const HashCountArgs &a, cudaStream_t s) {
@@ -266,14 +284,15 @@ void launch_hash_bounds(const HashCountArgs &a, cudaStream_t s) {
     hash_bounds_kernel<<<(unsigned)blocks, 256, 0, s>>>(a.keys, a.n, a.top_shift, a.chunk, a.window, a.nseg, a.seg_start, a.overflow);
 }
 int launch_hash_count(const HashCountArgs &a, cudaStream_t s) {
-    if (a.nseg == 0 || a.nseg > 0x7fffffffull) return (int)cudaErrorInvalidValue;
-    hash_count_kernel<kHashThreads><<<(unsigned)a.nseg, kHashThreads, hash_smem_bytes(a.table_slots, a.max_solid), s>>>(a);
+    if (a.nseg == 0 || a.nseg > 0x7fffffffull || a.max_solid != 1024) return (int)cudaErrorInvalidValue;
+    const size_t smem = hash_smem_bytes(a.table_slots, a.max_solid);
+    if (a.table_slots > 4096) hash_count_kernel<512, 2, 8><<<(unsigned)a.nseg, 512, smem, s>>>(a);
+    else hash_count_kernel<256, 3, 9><<<(unsigned)a.nseg, 256, smem, s>>>(a);
     return (int)cudaGetLastError();
 }
 void launch_hash_append(const HashCountArgs &a, u64 *total, DevState *st, int range_parity, cudaStream_t s) {
     hash_scan_kernel<<<1, 1024, 0, s>>>(a.seg_count, a.nseg, total);
-    u64 blocks = (a.nseg + 7) / 8;
-    if (blocks > (u64)kNumSMs * 16) blocks = (u64)kNumSMs * 16;
+    const u64 blocks = (a.nseg + 7) / 8;
     hash_copy_kernel<<<(unsigned)blocks, 256, 0, s>>>(a, total, st, range_parity);
 }
 
