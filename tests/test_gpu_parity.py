@@ -355,3 +355,62 @@ def test_partial_sort_path_and_its_way_back(k):
         finally:
             del os.environ["SDBG_NO_PARTIAL"]
         assert_matches_oracle(res2, orc, check_stats=True)
+
+
+def _radix_launches(res):
+    """Radix passes over all records since the context was created (launch accounting of sdbg_ctx_get_timing)."""
+    return res.ctx.get_timing().launches["radix"]
+
+
+@pytest.mark.parametrize("k", [15, 21, 31])
+def test_table_count_path_and_its_way_back(k):
+    """The top-sort + table-count path (api_count.inc count_range_hash, hashcount.cu): records sorted by the most
+    significant passes only, segments of whole buckets counted in shared-memory tables. Checked against the oracle and
+    against the two other paths (SDBG_NO_HASH=1: partial-sort path; SDBG_NO_PARTIAL=1: every pass over every record),
+    statistics included; the number of radix launches says which path ran. Cases: (1) covered reads with one-mismatch
+    copies, d = 2 and 3: the path completes with fewer passes than the key has bytes; (2) the all-ones key (T...T at
+    k = 31 fills the word) and its all-zero twin; (3) a bucket longer than the search window (poly-A): overflow, the
+    records are sorted the plain way from where the top passes left them; (4) reads over two letters only: far more
+    distinct keys per bucket than a table holds: overflow; (5) every read twice at d = 2: half of the records of a
+    segment are solid edges, more than its 1,024 sort places: overflow."""
+    import os
+    import random
+    from oracle import run_oracle
+    from tests.gpu_util import run_gpu, assert_matches_oracle
+    from tests.helpers import rc
+    rng = random.Random(1700 + k)
+    P = (2 * (k + 1) + 7) // 8
+    genome = "".join(rng.choice("ACGT") for _ in range(3000))
+    covered = []
+    for _ in range(1500):
+        a = rng.randint(0, len(genome) - 100)
+        x = list(genome[a:a + 100])
+        if rng.random() < 0.3:
+            x[rng.randrange(100)] = rng.choice("ACGT")
+        x = "".join(x)
+        covered.append(x if rng.random() < 0.5 else rc(x))
+    poly_t = covered + ["T" * 70] * 5 + ["GATTACA" + "T" * 50] * 3
+    poly_a = covered + ["A" * 150] * 400
+    two_letters = ["".join(rng.choice("AC") for _ in range(120)) for _ in range(1200)]
+    twice = ["".join(rng.choice("ACGT") for _ in range(130)) for _ in range(600)] * 2
+    cases = [("covered", covered, 2, True), ("covered", covered, 3, True), ("poly_t", poly_t, 2, True),
+             ("poly_a", poly_a, 2, False), ("two_letters", two_letters, 2, False), ("twice", twice, 2, False)]
+    for name, reads, d, completes in cases:
+        orc = run_oracle(reads, k, d)
+        res = run_gpu(reads, k, d, checksums=False)
+        assert_matches_oracle(res, orc, check_stats=True)
+        n_hash = _radix_launches(res)
+        if completes:
+            assert 1 <= n_hash < P, (name, k, d, n_hash)              # top passes only
+        else:
+            assert P < n_hash < 2 * P, (name, k, d, n_hash)            # top passes, then all passes (the way back)
+        for var in ("SDBG_NO_HASH", "SDBG_NO_PARTIAL"):
+            os.environ[var] = "1"
+            try:
+                res2 = run_gpu(reads, k, d, checksums=False)
+            finally:
+                del os.environ[var]
+            assert_matches_oracle(res2, orc, check_stats=True)
+            if var == "SDBG_NO_PARTIAL":
+                assert _radix_launches(res2) == P, (name, k, d)
+            assert res2.edges.n == res.edges.n
