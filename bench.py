@@ -327,6 +327,14 @@ def run_gpu(args, w):
         "roofline": {"kernel": "onesweep_kernel (one LSD radix pass)", "bound": "hbm", "achieved": achieved, "peak": peak,
                      "unit": "GB/s", "frac": achieved / peak, "traffic": _traffic(wl.name), "peak_source": peak_src,
                      "launches": int(radix_launches), "avg_launch_ms": radix_ms, "algorithmic_bytes_per_launch": algo_bytes},
+        # the count step beside it (hashcount.cu on the default path): its algorithmic bytes are one read of the records
+        # plus the solid edges staged and copied; it is bound by instruction issue, not by HBM (DESIGN.md section 6 a4')
+        "roofline_count": {"kernel": "count step (hash_count_kernel and helpers, or the sweeps of count.cu)", "bound": "hbm",
+                           "achieved": (tim.bytes["count"] / (tim.ms["count"] * 1e-3) / 1e9) if tim.ms["count"] > 0 else 0.0,
+                           "peak": peak, "unit": "GB/s",
+                           "frac": (tim.bytes["count"] / (tim.ms["count"] * 1e-3) / 1e9 / peak) if tim.ms["count"] > 0 else 0.0,
+                           "ms_per_step": tim.ms["count"] / args.steps, "algorithmic_bytes_per_step": tim.bytes["count"] // max(args.steps, 1),
+                           "note": "instruction-issue bound (profiles/r01_hash_count_full.md)"},
         "kernel_ms_per_step": {c: tim.ms[c] / args.steps for c in tim.ms},
         "kernel_launches_per_step": {c: tim.launches[c] / args.steps for c in tim.launches},
     }

@@ -60,7 +60,13 @@ typedef struct sdbg_ctx sdbg_ctx;
  * sizes its block-wise passes to it. workspace must be 256-byte aligned.
  * Test hook: with SDBG_FORCE_WIDE=1 in the environment when the context is created, one-word-key ranges of any size
  * take the code path of ranges of 2^32 records and more (wide look-back words in the radix passes, 64-bit run lengths
- * in the count sweeps), which otherwise only very large block-wise runs reach. Results are identical. */
+ * in the count sweeps), which otherwise only very large block-wise runs reach. Results are identical.
+ * Path switches, read at the same moment, results identical as well: sdbg_count_edges has three ways through the sort and
+ * count of one-word keys (PAPER.md:33-35 fix the result, not the way): by default the records are sorted by their most
+ * significant key bytes only and counted bucket by bucket in shared-memory tables (d >= 2); SDBG_NO_HASH=1 takes the
+ * partial-sort path instead (sort by the low bytes of mixed keys, count inside the buckets, sort only the kept
+ * entries); SDBG_NO_PARTIAL=1 sorts every record through every pass and counts by one sweep. Whatever does not fit the
+ * default path (an over-long bucket, a full table) is redone the plain way inside the same call. */
 int sdbg_ctx_create(sdbg_ctx **ctx, int device, void *cuda_stream, void *workspace, uint64_t workspace_bytes);
 void sdbg_ctx_destroy(sdbg_ctx *ctx);
 const char *sdbg_strerror(int status);           /* static string */
