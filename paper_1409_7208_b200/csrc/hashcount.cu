@@ -60,12 +60,15 @@ __global__ void __launch_bounds__(256) hash_bounds_kernel(const u64 *__restrict_
     if (lane_id() == 0) seg_start[c] = res;
 }
 
-template <int THREADS, int MINB, int U>   // U = loads in flight per thread
+// U = loads in flight per thread; PACK16: counts are 16-bit halves of u32 words (a segment has at most window + chunk
+// < 65,536 records), which brings the short-bucket shape to 52 KiB and four CTAs per SM
+template <int THREADS, int MINB, int U, bool PACK16>
 __global__ void __launch_bounds__(THREADS, MINB)
 hash_count_kernel(HashCountArgs a) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     u64 *t_key = reinterpret_cast<u64 *>(smem_raw);                  // u64[table_slots]
-    u32 *t_cnt = reinterpret_cast<u32 *>(smem_raw + (size_t)a.table_slots * 8); // u32[table_slots]
+    u32 *t_cnt = reinterpret_cast<u32 *>(smem_raw + (size_t)a.table_slots * 8); // u32[table_slots] (PACK16: u16 pairs)
+    constexpr u32 CB = PACK16 ? 2u : 4u;                              // bytes of a count
     __shared__ u32 s_ones, s_full, s_nsolid, s_distinct;
     __shared__ u64 s_sum;
     const u32 tid = threadIdx.x;
@@ -85,7 +88,7 @@ hash_count_kernel(HashCountArgs a) {
         uint4 *k4 = reinterpret_cast<uint4 *>(t_key), *c4 = reinterpret_cast<uint4 *>(t_cnt);
         const uint4 ones = make_uint4(~0u, ~0u, ~0u, ~0u), zero = make_uint4(0u, 0u, 0u, 0u);
         for (u32 i = tid; i < TS / 2; i += THREADS) k4[i] = ones;
-        for (u32 i = tid; i < TS / 4; i += THREADS) c4[i] = zero;
+        for (u32 i = tid; i < TS * CB / 16; i += THREADS) c4[i] = zero;
     }
     if (tid == 0) { s_ones = 0; s_full = 0; s_nsolid = 0; s_distinct = 0; s_sum = 0; }
     __syncthreads();
@@ -103,7 +106,11 @@ hash_count_kernel(HashCountArgs a) {
                 cur = atomicCAS(&t_key[slot], kEmpty, key);
                 if (cur == kEmpty) { ++created; cur = key; }
             }
-            if (cur == key) { atomicAdd(&t_cnt[slot], 1u); break; }
+            if (cur == key) {
+                if constexpr (PACK16) atomicAdd(&t_cnt[slot >> 1], 1u << ((slot & 1u) * 16u));
+                else atomicAdd(&t_cnt[slot], 1u);
+                break;
+            }
             slot = (slot + 1u) & mask;
             if (probes >= TS) { s_full = 1; break; }
         }
@@ -122,11 +129,11 @@ hash_count_kernel(HashCountArgs a) {
 
     // ---- 2: the solid slots, compacted to the front of a list in shared memory (reusing the table in place is not
     //         possible while it is read, so the list lives behind it) ------------------------------------------------------
-    u64 *l_key = reinterpret_cast<u64 *>(smem_raw + (size_t)a.table_slots * 12);    // u64[max_solid]
-    u32 *l_cnt = reinterpret_cast<u32 *>(smem_raw + (size_t)a.table_slots * 12 + (size_t)a.max_solid * 8);
+    u64 *l_key = reinterpret_cast<u64 *>(smem_raw + (size_t)a.table_slots * (8 + CB));    // u64[max_solid]
+    u32 *l_cnt = reinterpret_cast<u32 *>(smem_raw + (size_t)a.table_slots * (8 + CB) + (size_t)a.max_solid * 8);
     u64 sum = 0;
     for (u32 i = tid; i < TS; i += THREADS) {                    // the live part of the table
-        const u32 c = t_cnt[i];
+        const u32 c = PACK16 ? (t_cnt[i >> 1] >> ((i & 1u) * 16u)) & 0xffffu : t_cnt[i];
         if (c >= a.d) {
             const u32 p = atomicAdd(&s_nsolid, 1u);
             if (p < a.max_solid) { l_key[p] = t_key[i]; l_cnt[p] = c; }
@@ -270,13 +277,13 @@ __global__ void __launch_bounds__(256) hash_copy_kernel(HashCountArgs a, const u
 }
 
 // two shapes: big segments (chunk 4,096: one or two long buckets) 512 threads x 2 CTAs per SM with 8,192 slots; small
-// segments (chunk 2,048: many short buckets) 256 threads x 3 CTAs per SM with 4,096 slots
-u64 hash_smem_bytes(u32 table_slots, u32 max_solid) { return (u64)table_slots * 12 + (u64)max_solid * 12; }
+// segments (chunk 2,048: many short buckets) 256 threads x 4 CTAs per SM with 4,096 slots and 16-bit counts
+u64 hash_smem_bytes(u32 table_slots, u32 max_solid) { return (u64)table_slots * (table_slots > 4096 ? 12 : 10) + (u64)max_solid * 12; }
 
 int hash_setup() {
-    int e = (int)cudaFuncSetAttribute(hash_count_kernel<512, 2, 8>, cudaFuncAttributeMaxDynamicSharedMemorySize, 110 * 1024);
+    int e = (int)cudaFuncSetAttribute(hash_count_kernel<512, 2, 8, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, 110 * 1024);
     if (e) return e;
-    return (int)cudaFuncSetAttribute(hash_count_kernel<256, 3, 9>, cudaFuncAttributeMaxDynamicSharedMemorySize, 62 * 1024);
+    return (int)cudaFuncSetAttribute(hash_count_kernel<256, 4, 9, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 54 * 1024);
 }
 
 void launch_hash_bounds(const HashCountArgs &a, cudaStream_t s) {
@@ -284,10 +291,10 @@ void launch_hash_bounds(const HashCountArgs &a, cudaStream_t s) {
     hash_bounds_kernel<<<(unsigned)blocks, 256, 0, s>>>(a.keys, a.n, a.top_shift, a.chunk, a.window, a.nseg, a.seg_start, a.overflow);
 }
 int launch_hash_count(const HashCountArgs &a, cudaStream_t s) {
-    if (a.nseg == 0 || a.nseg > 0x7fffffffull || a.max_solid != 1024) return (int)cudaErrorInvalidValue;
+    if (a.nseg == 0 || a.nseg > 0x7fffffffull || a.max_solid != 1024 || (u64)a.window + a.chunk >= 65536) return (int)cudaErrorInvalidValue;
     const size_t smem = hash_smem_bytes(a.table_slots, a.max_solid);
-    if (a.table_slots > 4096) hash_count_kernel<512, 2, 8><<<(unsigned)a.nseg, 512, smem, s>>>(a);
-    else hash_count_kernel<256, 3, 9><<<(unsigned)a.nseg, 256, smem, s>>>(a);
+    if (a.table_slots > 4096) hash_count_kernel<512, 2, 8, false><<<(unsigned)a.nseg, 512, smem, s>>>(a);
+    else hash_count_kernel<256, 4, 9, true><<<(unsigned)a.nseg, 256, smem, s>>>(a);
     return (int)cudaGetLastError();
 }
 void launch_hash_append(const HashCountArgs &a, u64 *total, DevState *st, int range_parity, cudaStream_t s) {

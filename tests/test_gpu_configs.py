@@ -41,7 +41,12 @@ def _run_config(cfg, workspace_bytes=None, min_ranges=1, n_buckets=16, full_grap
         # stores and position-counted digit histograms) must give the same edges as the run with checksums above
         import paper_1409_7208_b200 as sd
         ed2 = sd.Edges(res.n, w.k)
+        res.ctx.get_timing()                                         # resets the launch accounting
         assert sd.sdbg_count_edges(res.ctx, res.reads, w.n_reads, w.k, w.d, ed2, None) == res.n
+        if ed2.w == 1 and w.d >= 2:
+            # one-word keys: the top-sort + table-count path (DESIGN.md section 6 a4') ran to its end, i.e. the records
+            # went through the most significant passes only and nothing overflowed
+            assert 1 <= res.ctx.get_timing().launches["radix"] <= 3, "table-count path fell back at full size"
         assert torch.equal(ed2.keys[:res.n * ed2.w], res.edges.keys[:res.n * ed2.w]) and torch.equal(ed2.mult[:res.n], res.edges.mult[:res.n])
         del ed2
     res.ctx.close(); res.ctx.workspace = None                        # the checks below need the HBM
