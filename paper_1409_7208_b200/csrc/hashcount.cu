@@ -95,8 +95,9 @@ hash_count_kernel(HashCountArgs a) {
 
     // ---- 1: insert ---------------------------------------------------------------------------------------------------
     u32 created = 0;
+    const bool may_ones = klast == (~0ull >> a.top_shift);            // only the last bucket of all can hold the all-ones key
     auto insert = [&](u64 key) {
-        if (key == kEmpty) { atomicAdd(&s_ones, 1u); return; }
+        if (may_ones && key == kEmpty) { atomicAdd(&s_ones, 1u); return; }
         u32 h = ((u32)key ^ (u32)(key >> 32)) * 0x9E3779B1u;
         h ^= (u32)(key >> 20);
         u32 slot = (h * 0x85EBCA6Bu) >> hshift;
@@ -115,13 +116,18 @@ hash_count_kernel(HashCountArgs a) {
             if (probes >= TS) { s_full = 1; break; }
         }
     };
-    for (u64 base = s;;) {
+    // a segment has fewer than 2^16 records: 32-bit positions relative to its start
+    const u32 m = (u32)(e - s);
+    for (u32 base = 0;;) {
+        const u32 rem = m - base > tid ? m - base - tid : 0u;          // my records of this round: u * THREADS < rem
 #pragma unroll
-        for (int u = 0; u < U; ++u) if (base + (u64)u * THREADS + tid < e) insert(kq[u]);
-        base += (u64)U * THREADS;
-        if (base >= e) break;
+        for (int u = 0; u < U; ++u) if ((u32)u * THREADS < rem) insert(kq[u]);
+        base += (u32)U * THREADS;
+        if (base >= m) break;
+        const u64 *src = a.keys + s + base + tid;
+        const u32 rem2 = m - base > tid ? m - base - tid : 0u;
 #pragma unroll
-        for (int u = 0; u < U; ++u) { const u64 i = base + (u64)u * THREADS + tid; kq[u] = i < e ? ld_stream(a.keys + i) : 0ull; }
+        for (int u = 0; u < U; ++u) kq[u] = (u32)u * THREADS < rem2 ? ld_stream(src + u * THREADS) : 0ull;
     }
     if (created) atomicAdd(&s_distinct, created);
     __syncthreads();
