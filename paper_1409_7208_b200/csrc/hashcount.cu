@@ -138,12 +138,31 @@ hash_count_kernel(HashCountArgs a) {
     u64 *l_key = reinterpret_cast<u64 *>(smem_raw + (size_t)a.table_slots * (8 + CB));    // u64[max_solid]
     u32 *l_cnt = reinterpret_cast<u32 *>(smem_raw + (size_t)a.table_slots * (8 + CB) + (size_t)a.max_solid * 8);
     u64 sum = 0;
-    for (u32 i = tid; i < TS; i += THREADS) {                    // the live part of the table
-        const u32 c = PACK16 ? (t_cnt[i >> 1] >> ((i & 1u) * 16u)) & 0xffffu : t_cnt[i];
-        if (c >= a.d) {
-            const u32 p = atomicAdd(&s_nsolid, 1u);
-            if (p < a.max_solid) { l_key[p] = t_key[i]; l_cnt[p] = c; }
-            sum += c;
+    {   // the live part of the table, 16 bytes of counts (4 or 8 slots) per load; most vectors hold no solid edge
+        constexpr u32 SPV = PACK16 ? 8u : 4u;
+        const uint4 *c4 = reinterpret_cast<const uint4 *>(t_cnt);
+        const u32 d = a.d;
+        for (u32 v = tid; v < TS / SPV; v += THREADS) {
+            const uint4 w = c4[v];
+            u32 cs[SPV];
+            if constexpr (PACK16) {
+                cs[0] = w.x & 0xffffu; cs[1] = w.x >> 16; cs[2] = w.y & 0xffffu; cs[3] = w.y >> 16;
+                cs[4] = w.z & 0xffffu; cs[5] = w.z >> 16; cs[6] = w.w & 0xffffu; cs[7] = w.w >> 16;
+            } else {
+                cs[0] = w.x; cs[1] = w.y; cs[2] = w.z; cs[3] = w.w;
+            }
+            u32 mx = 0;
+#pragma unroll
+            for (u32 q = 0; q < SPV; ++q) mx = cs[q] > mx ? cs[q] : mx;
+            if (mx < d) continue;
+#pragma unroll
+            for (u32 q = 0; q < SPV; ++q) {
+                if (cs[q] >= d) {
+                    const u32 p = atomicAdd(&s_nsolid, 1u);
+                    if (p < a.max_solid) { l_key[p] = t_key[v * SPV + q]; l_cnt[p] = cs[q]; }
+                    sum += cs[q];
+                }
+            }
         }
     }
     if (tid == 0 && s_ones) {
