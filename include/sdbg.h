@@ -66,7 +66,8 @@ typedef struct sdbg_ctx sdbg_ctx;
  * significant key bytes only and counted bucket by bucket in shared-memory tables (d >= 2); SDBG_NO_HASH=1 takes the
  * partial-sort path instead (sort by the low bytes of mixed keys, count inside the buckets, sort only the kept
  * entries); SDBG_NO_PARTIAL=1 sorts every record through every pass and counts by one sweep. Whatever does not fit the
- * default path (an over-long bucket, a full table) is redone the plain way inside the same call. */
+ * default path (an over-long bucket, a full table) is redone the plain way inside the same call.
+ * SDBG_NO_UNSTABLE=1: the first radix pass of a sort (whose input order is arbitrary) uses the stable kernel too. */
 int sdbg_ctx_create(sdbg_ctx **ctx, int device, void *cuda_stream, void *workspace, uint64_t workspace_bytes);
 void sdbg_ctx_destroy(sdbg_ctx *ctx);
 const char *sdbg_strerror(int status);           /* static string */

@@ -41,6 +41,7 @@ struct sdbg_ctx {
     std::string err;
     bool timing = false;
     bool force_wide = false;   // SDBG_FORCE_WIDE=1 in the environment at sdbg_ctx_create: see include/sdbg.h
+    bool no_unstable = false;  // SDBG_NO_UNSTABLE=1: the first radix pass uses the stable kernel like the others
     bool no_hash = false;      // SDBG_NO_HASH=1: never count top-sorted records in shared-memory tables (api_count.inc count_range_hash)
     bool no_partial = false;   // SDBG_NO_PARTIAL=1 in the environment at sdbg_ctx_create: always sort all records through all passes
     std::vector<EventPair> pending;
@@ -167,6 +168,8 @@ int sdbg_ctx_create(sdbg_ctx **out, int device, void *cuda_stream, void *workspa
     c->force_wide = fw && fw[0] == '1';
     const char *np_ = getenv("SDBG_NO_PARTIAL");
     c->no_partial = np_ && np_[0] == '1';
+    const char *nu_ = getenv("SDBG_NO_UNSTABLE");
+    c->no_unstable = nu_ && nu_[0] == '1';
     const char *nh_ = getenv("SDBG_NO_HASH");
     c->no_hash = c->no_partial || (nh_ && nh_[0] == '1');
     *out = c;

@@ -66,6 +66,7 @@ struct RadixArgs {
     u32 *ticket;                         // zeroed
     PassDesc pass; u32 epoch;
     bool force_wide;                     // use the layout for ranges of 2^32 records and more whatever n is (tests)
+    bool unstable;                       // the pass need not keep the order of equal digits (first pass of a sort; one-word keys without payload)
 };
 u64 radix_tile_records(u32 W, bool has_vals);
 u64 radix_max_records(u32 W, bool has_vals);   // cap of one sort range (look-back word layout)

@@ -263,7 +263,10 @@ __device__ __forceinline__ void prefetch_l2_bulk(const void *p, u32 bytes) {
 //   5 write-out: place p of the tile goes to bin_address[digit] + p, coalesced per digit run.
 // Forward progress: a CTA's current tile is always older than the ticket it holds in reserve, so the oldest
 // unfinished tile is always being worked on by a resident CTA.
-template <int W, bool HAS_VAL, bool HI, bool WIDE>
+// FIRST: the first pass of a sort. Its input order is arbitrary, so the pass need not be stable: the rank of a key
+// inside (warp, digit) is what the count atomic returned, and the match step of phase 3 is not needed (full tiles
+// only: the pads of the last tile rely on the stable order).
+template <int W, bool HAS_VAL, bool HI, bool WIDE, bool FIRST = false>
 __global__ void __launch_bounds__(RadixCfg<W, HAS_VAL>::THREADS, RadixCfg<W, HAS_VAL>::MINB)
 onesweep_kernel(RadixArgs a) {
     using L = RadixSmem<W, HAS_VAL>;
@@ -326,9 +329,17 @@ onesweep_kernel(RadixArgs a) {
     };
     auto tile_count = [&](u32 t) { return (a.n - (u64)t * TILE < (u64)TILE) ? (u32)(a.n - (u64)t * TILE) : (u32)TILE; };
     // phase 1: digits of the keys in registers -> warp-private histogram
+    u32 rkp[FIRST ? (KPT + 1) / 2 : 1];   // FIRST: arrival rank inside (warp, digit), 16 bits each
     auto count_keys = [&]() {
 #pragma unroll
-        for (int j = 0; j < KPT; ++j) atomicAdd(&wp[digit8<W, HI>(key[j], word, psel)], 1u);
+        for (int j = 0; j < KPT; ++j) {
+            if constexpr (FIRST) {
+                const u32 r = atomicAdd(&wp[digit8<W, HI>(key[j], word, psel)], 1u);
+                if (j & 1) rkp[j / 2] |= r << 16; else rkp[j / 2] = r;
+            } else {
+                atomicAdd(&wp[digit8<W, HI>(key[j], word, psel)], 1u);
+            }
+        }
     };
     // phase 2a (one thread per bin, after a block barrier): tile count, published LOCAL at once; scan over the bins
     u32 my_cnt = 0, incl = 0;
@@ -399,6 +410,24 @@ onesweep_kernel(RadixArgs a) {
     for (;; ++it) {
         const u32 next = SDBG_PERSISTENT ? s_tick[(it + 1) & 1] : ntiles;
         // ---- 3: rank within the warp (stable in tile order), scatter to shared memory in bin-sorted order ------
+        bool ranked = false;
+        if constexpr (FIRST) {
+            if (cnt == (u32)TILE) {
+                ranked = true;
+#pragma unroll
+                for (int j = 0; j < KPT; ++j) {
+                    const u32 d = digit8_again<W, HI>(key[j], word, psel);
+                    const u32 pos = wp[d] + ((rkp[j / 2] >> (16 * (j & 1))) & 0xffffu);
+#pragma unroll
+                    for (int q = 0; q < W; ++q) s_keys[q * TILE + pos] = key[j][q];
+                    if constexpr (HAS_VAL) s_vals[pos] = val[j];
+                    if ((j & (SDBG_LB_EVERY - 1)) == SDBG_LB_EVERY - 1 && walker)
+                        lookback_poll<WIDE>(lb, tile, lb_t, lb_pend, lb_excl, lb_done, real_cnt, tagL, tagG);
+                }
+                __syncwarp();
+            }
+        }
+        if (!ranked) {
 #pragma unroll
         for (int j = 0; j < KPT; ++j) {
             const u32 d = digit8_again<W, HI>(key[j], word, psel);
@@ -426,6 +455,7 @@ onesweep_kernel(RadixArgs a) {
             __syncwarp();
             if ((j & (SDBG_LB_EVERY - 1)) == SDBG_LB_EVERY - 1 && walker)
                 lookback_poll<WIDE>(lb, tile, lb_t, lb_pend, lb_excl, lb_done, real_cnt, tagL, tagG);
+        }
         }
         zero_rows();   // own rows only; their last readers were the scan threads, two barriers ago
 
@@ -481,6 +511,12 @@ static int setup_one() {
     if (e) return e;
     e = (int)cudaFuncSetAttribute(onesweep_kernel<W, HAS_VAL, true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
     if (e || HAS_VAL) return e;   // ranges of 2^32 records and more exist only in sdbg_count_edges (keys without payload)
+    if constexpr (W == 1) {
+        e = (int)cudaFuncSetAttribute(onesweep_kernel<1, false, false, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
+        if (e) return e;
+        e = (int)cudaFuncSetAttribute(onesweep_kernel<1, false, true, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
+        if (e) return e;
+    }
     e = (int)cudaFuncSetAttribute(onesweep_kernel<W, false, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
     if (e) return e;
     return (int)cudaFuncSetAttribute(onesweep_kernel<W, false, true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
@@ -536,6 +572,13 @@ static int launch_one(const RadixArgs &a, cudaStream_t s) {
         if (wide) {
             if (hi) onesweep_kernel<W, false, true, true><<<g, t, sm, s>>>(a);
             else    onesweep_kernel<W, false, false, true><<<g, t, sm, s>>>(a);
+            return (int)cudaGetLastError();
+        }
+    }
+    if constexpr (W == 1 && !HAS_VAL) {
+        if (a.unstable) {
+            if (hi) onesweep_kernel<1, false, true, false, true><<<g, t, sm, s>>>(a);
+            else    onesweep_kernel<1, false, false, false, true><<<g, t, sm, s>>>(a);
             return (int)cudaGetLastError();
         }
     }

@@ -404,7 +404,7 @@ def test_table_count_path_and_its_way_back(k):
             assert 1 <= n_hash < P, (name, k, d, n_hash)              # top passes only
         else:
             assert P < n_hash < 2 * P, (name, k, d, n_hash)            # top passes, then all passes (the way back)
-        for var in ("SDBG_NO_HASH", "SDBG_NO_PARTIAL"):
+        for var in ("SDBG_NO_HASH", "SDBG_NO_PARTIAL", "SDBG_NO_UNSTABLE"):   # the last: stable kernel for the first pass too
             os.environ[var] = "1"
             try:
                 res2 = run_gpu(reads, k, d, checksums=False)
