@@ -13,6 +13,8 @@
 
 using namespace sdbg;
 
+int sdbg::g_num_sms = sdbg::kNumSMs;   // replaced by the device's own count in sdbg_ctx_create
+
 namespace {
 
 constexpr u64 kAlign = 256;
@@ -157,6 +159,10 @@ int sdbg_ctx_create(sdbg_ctx **out, int device, void *cuda_stream, void *workspa
     int ndev = 0;
     if (cudaGetDeviceCount(&ndev) != cudaSuccess || device < 0 || device >= ndev) { cudaGetLastError(); return SDBG_E_CUDA; }
     if (cudaSetDevice(device) != cudaSuccess) return SDBG_E_CUDA;
+    {
+        int sms = 0;
+        if (cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, device) == cudaSuccess && sms > 0) g_num_sms = sms;
+    }
     if (radix_setup() != 0) { cudaGetLastError(); return SDBG_E_CUDA; }
     if (hash_setup() != 0) { cudaGetLastError(); return SDBG_E_CUDA; }
     sdbg_ctx *c = new sdbg_ctx();

@@ -8,7 +8,9 @@ typedef unsigned int u32;
 
 namespace sdbg {
 
-constexpr int kNumSMs = 148;           // B200
+constexpr int kNumSMs = 148;           // B200; launch sizing uses num_sms(), read from the device in sdbg_ctx_create
+extern int g_num_sms;
+inline int num_sms() { return g_num_sms; }
 constexpr int kMaxPasses = 32;         // 4 words x 8 digits
 constexpr int kRadixBits = 8;
 constexpr int kRadix = 1 << kRadixBits;

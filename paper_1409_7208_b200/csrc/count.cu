@@ -370,7 +370,7 @@ __global__ void __launch_bounds__(256) solid_flags_kernel(const u32 *__restrict_
 void launch_solid_flags(const u32 *mult, u64 n, u32 d, uint8_t *flags, u64 *stat_slots, cudaStream_t s) {
     if (n == 0) return;
     u64 blocks = (n + 255) / 256;
-    if (blocks > (u64)kNumSMs * 8) blocks = (u64)kNumSMs * 8;
+    if (blocks > (u64)num_sms() * 8) blocks = (u64)num_sms() * 8;
     solid_flags_kernel<<<(unsigned)blocks, 256, 0, s>>>(mult, n, d, flags, stat_slots);
 }
 
@@ -389,7 +389,7 @@ void launch_append_solid(const u64 *keys, const u32 *mult, const u32 *idx, const
                          u64 out_cap, DevState *st, int range_parity, cudaStream_t s) {
     u64 blocks = (n_max + 255) / 256;
     if (blocks == 0) blocks = 1;
-    if (blocks > (u64)kNumSMs * 8) blocks = (u64)kNumSMs * 8;
+    if (blocks > (u64)num_sms() * 8) blocks = (u64)num_sms() * 8;
     append_solid_kernel<<<(unsigned)blocks, 256, 0, s>>>(keys, mult, idx, n_idx, out_keys, out_mult, out_cap, st, range_parity);
 }
 
@@ -525,7 +525,7 @@ void launch_merge(const MergeArgs &a, DevState *st, cudaStream_t s) {
         case 4: launch_merge_w<4>(a, st, s); break;
     }
     u64 blocks = (a.n + 255) / 256;
-    if (blocks > (u64)kNumSMs * 8) blocks = (u64)kNumSMs * 8;
+    if (blocks > (u64)num_sms() * 8) blocks = (u64)num_sms() * 8;
     merge_finish_kernel<<<(unsigned)blocks, 256, 0, s>>>(a.acc, a.out_mult, a.n, st);
 }
 

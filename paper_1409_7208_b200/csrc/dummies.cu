@@ -323,7 +323,7 @@ __global__ void __launch_bounds__(256) valid_fill_kernel(u64 *valid, u64 m) {
 static unsigned grid_for(u64 n) {
     u64 b = (n + 255) / 256;
     if (b == 0) b = 1;
-    const u64 cap = (u64)kNumSMs * 16;
+    const u64 cap = (u64)num_sms() * 16;
     return (unsigned)(b < cap ? b : cap);
 }
 

@@ -67,7 +67,7 @@ __global__ void __launch_bounds__(256) emit_kernel(EmitArgs a) {
 void launch_emit(const EmitArgs &a, cudaStream_t s) {
     if (a.n == 0) return;
     u64 blocks = (a.n + 255) / 256;
-    if (blocks > (u64)kNumSMs * 16) blocks = (u64)kNumSMs * 16;
+    if (blocks > (u64)num_sms() * 16) blocks = (u64)num_sms() * 16;
     switch (a.W) {
         case 1: emit_kernel<1><<<(unsigned)blocks, 256, 0, s>>>(a); break;
         case 2: emit_kernel<2><<<(unsigned)blocks, 256, 0, s>>>(a); break;

@@ -388,7 +388,7 @@ static int launch_extract_w(const ExtractArgs &a, DevState *st, cudaStream_t s) 
     if (ngroups == 0) return 0;
     const bool filter = !(a.bucket_lo == 0 && a.bucket_hi >= 65536);
     u64 blocks = (ngroups + 255) / 256;
-    const u64 maxb = (u64)kNumSMs * 8;
+    const u64 maxb = (u64)num_sms() * 8;
     if (blocks > maxb) blocks = maxb;
     const u32 T = (W == 1 && !filter && a.digit_hist && a.k >= 8 && !a.mix_shift) ? a.k / 4 : 0;   // 2..7: shared position tables
     size_t smem = a.digit_hist ? (size_t)(a.passes.n + (T ? 2 * T + 2 : 0)) * kRadix * sizeof(u32) : 0;

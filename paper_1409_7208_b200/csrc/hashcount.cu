@@ -3,17 +3,31 @@
 // kept" (§2 ¶4). This is the paper's own partition idea (the k-mers are partitioned by a
 // length-l prefix and consecutive partitions are handled together) carried one level down: after P_hi radix passes over
 // the most significant key bytes all copies of an edge lie inside one run of equal top bytes (a bucket), and a segment
-// of consecutive whole buckets is small enough to be counted in SHARED memory. One CTA per segment:
-//   1 every record of the segment is inserted into an open-addressing table of (key, count) slots in shared memory;
+// of consecutive whole buckets is small enough to be counted in SHARED memory. Persistent CTAs take segments by atomic
+// ticket (two ahead, so that neither the ticket nor the bounds of a segment are ever waited for); per segment:
+//   1 every record of the segment is inserted into an open-addressing table of (key, 16-bit count) slots in shared memory.
+//     A warp holds U rows of 32 records at a time and first tries the HOME slot of all of them (one ATOMS.CAS.64 that
+//     installs the key or returns what is there, then one ATOMS.ADD on the count) with no loop and no divergence; the few
+//     records whose home slot holds another key are then finished in ONE divergent probing loop per group of rows;
 //   2 the slots with count >= d are put in key order inside shared memory (one pass of order-preserving binning, then
 //     insertion inside the tiny bins) — buckets are consecutive in key order and segments too, so the ordered solid edges
 //     of a segment are a contiguous piece of the final output;
-//   3 they are written, with their counts, to the place of the segment in a staging buffer, and the number of them to
-//     seg_count[segment]; a scan and a copy kernel (hash_scan_kernel, hash_copy_kernel) append them in order.
+//   3 they are written, with their counts, to the place of the segment in a staging buffer (the sorter's spare buffer),
+//     the number of them to seg_count[segment] and added to the sum of its block of 256 segments. hash_scan_kernel (one
+//     block: prefix of the block sums) and hash_copy_kernel (a CTA per block of segments: prefix inside the block, then a
+//     warp per segment) append them in order. CTAs never wait for one another: a chain of solid counts through the
+//     segments (decoupled look-back, tried first) made all resident segments resolve in lockstep, each walk some ten L2
+//     round trips long, and cost a quarter of the kernel's time; staging costs 24 bytes per solid edge of HBM traffic.
+// The first records of the NEXT segment are requested before step 2, so loads are in flight while a CTA sorts.
 // Nothing but the solid edges goes through any further pass. Segment borders are found by hash_bounds_kernel.
 // Whatever does not fit (a bucket longer than the search window, a full table, more solid edges than sort places)
 // raises *overflow; the caller then sorts the range the plain way (api_count.inc), so the result is the same.
 #include "kernels.cuh"
+#include <type_traits>
+
+#ifndef SDBG_HASH_CASFIRST
+#define SDBG_HASH_CASFIRST 0   // 1: the home slot is probed with the CAS itself; 0: with a load, CAS only into empty slots
+#endif
 
 namespace sdbg {
 
@@ -60,211 +74,297 @@ __global__ void __launch_bounds__(256) hash_bounds_kernel(const u64 *__restrict_
     if (lane_id() == 0) seg_start[c] = res;
 }
 
-// U = loads in flight per thread; PACK16: counts are 16-bit halves of u32 words (a segment has at most window + chunk
-// < 65,536 records), which brings the short-bucket shape to 52 KiB and four CTAs per SM
-template <int THREADS, int MINB, int U, bool PACK16>
-__global__ void __launch_bounds__(THREADS, MINB)
-hash_count_kernel(HashCountArgs a) {
-    extern __shared__ __align__(16) unsigned char smem_raw[];
-    u64 *t_key = reinterpret_cast<u64 *>(smem_raw);                  // u64[table_slots]
-    u32 *t_cnt = reinterpret_cast<u32 *>(smem_raw + (size_t)a.table_slots * 8); // u32[table_slots] (PACK16: u16 pairs)
-    constexpr u32 CB = PACK16 ? 2u : 4u;                              // bytes of a count
-    __shared__ u32 s_ones, s_full, s_nsolid, s_distinct;
-    __shared__ u64 s_sum;
-    const u32 tid = threadIdx.x;
-    const u64 seg = blockIdx.x;
-    const u64 s = a.seg_start[seg], e = a.seg_start[seg + 1];
-    if (e <= s) { if (tid == 0) a.seg_count[seg] = 0; return; }
-    const u64 kfirst = a.keys[s] >> a.top_shift, klast = a.keys[e - 1] >> a.top_shift;   // first and last bucket of the segment
-    // the first U records of every thread are on their way while the table is cleared
-    u64 kq[U];
-#pragma unroll
-    for (int u = 0; u < U; ++u) { const u64 i = s + (u64)u * THREADS + tid; kq[u] = i < e ? ld_stream(a.keys + i) : 0ull; }
-    // table size: the power of two from 1.5 x the records of the segment on (all of them might be distinct)
-    u32 TS = 1024;
-    while (TS < a.table_slots && (u64)TS * 2 < (e - s) * 3) TS <<= 1;
-    const u32 mask = TS - 1u, hshift = 32u - (u32)__ffs(TS) + 1u;
-    {
-        uint4 *k4 = reinterpret_cast<uint4 *>(t_key), *c4 = reinterpret_cast<uint4 *>(t_cnt);
-        const uint4 ones = make_uint4(~0u, ~0u, ~0u, ~0u), zero = make_uint4(0u, 0u, 0u, 0u);
-        for (u32 i = tid; i < TS / 2; i += THREADS) k4[i] = ones;
-        for (u32 i = tid; i < TS * CB / 16; i += THREADS) c4[i] = zero;
-    }
-    if (tid == 0) { s_ones = 0; s_full = 0; s_nsolid = 0; s_distinct = 0; s_sum = 0; }
-    __syncthreads();
+constexpr u32 kSegBlock = 256;   // segments per block sum (hash_scan_kernel, hash_copy_kernel)
 
-    // ---- 1: insert ---------------------------------------------------------------------------------------------------
-    u32 created = 0;
-    const bool may_ones = klast == (~0ull >> a.top_shift);            // only the last bucket of all can hold the all-ones key
-    auto insert = [&](u64 key) {
-        if (may_ones && key == kEmpty) { atomicAdd(&s_ones, 1u); return; }
-        u32 h = ((u32)key ^ (u32)(key >> 32)) * 0x9E3779B1u;
-        h ^= (u32)(key >> 20);
-        u32 slot = (h * 0x85EBCA6Bu) >> hshift;
-        for (u32 probes = 0;; ++probes) {
-            u64 cur = t_key[slot];
-            if (cur == kEmpty) {
-                cur = atomicCAS(&t_key[slot], kEmpty, key);
-                if (cur == kEmpty) { ++created; cur = key; }
-            }
-            if (cur == key) {
-                if constexpr (PACK16) atomicAdd(&t_cnt[slot >> 1], 1u << ((slot & 1u) * 16u));
-                else atomicAdd(&t_cnt[slot], 1u);
-                break;
-            }
-            slot = (slot + 1u) & mask;
-            if (probes >= TS) { s_full = 1; break; }
-        }
-    };
-    // a segment has fewer than 2^16 records: 32-bit positions relative to its start
-    const u32 m = (u32)(e - s);
-    for (u32 base = 0;;) {
-        const u32 rem = m - base > tid ? m - base - tid : 0u;          // my records of this round: u * THREADS < rem
-#pragma unroll
-        for (int u = 0; u < U; ++u) if ((u32)u * THREADS < rem) insert(kq[u]);
-        base += (u32)U * THREADS;
-        if (base >= m) break;
-        const u64 *src = a.keys + s + base + tid;
-        const u32 rem2 = m - base > tid ? m - base - tid : 0u;
-#pragma unroll
-        for (int u = 0; u < U; ++u) kq[u] = (u32)u * THREADS < rem2 ? ld_stream(src + u * THREADS) : 0ull;
-    }
-    if (created) atomicAdd(&s_distinct, created);
-    __syncthreads();
-    if (s_full) { if (tid == 0) { atomicOr(a.overflow, 2u); a.seg_count[seg] = 0; } return; }
-
-    // ---- 2: the solid slots, compacted to the front of a list in shared memory (reusing the table in place is not
-    //         possible while it is read, so the list lives behind it) ------------------------------------------------------
-    u64 *l_key = reinterpret_cast<u64 *>(smem_raw + (size_t)a.table_slots * (8 + CB));    // u64[max_solid]
-    u32 *l_cnt = reinterpret_cast<u32 *>(smem_raw + (size_t)a.table_slots * (8 + CB) + (size_t)a.max_solid * 8);
-    u64 sum = 0;
-    {   // the live part of the table, 16 bytes of counts (4 or 8 slots) per load; most vectors hold no solid edge
-        constexpr u32 SPV = PACK16 ? 8u : 4u;
-        const uint4 *c4 = reinterpret_cast<const uint4 *>(t_cnt);
-        const u32 d = a.d;
-        for (u32 v = tid; v < TS / SPV; v += THREADS) {
-            const uint4 w = c4[v];
-            u32 cs[SPV];
-            if constexpr (PACK16) {
-                cs[0] = w.x & 0xffffu; cs[1] = w.x >> 16; cs[2] = w.y & 0xffffu; cs[3] = w.y >> 16;
-                cs[4] = w.z & 0xffffu; cs[5] = w.z >> 16; cs[6] = w.w & 0xffffu; cs[7] = w.w >> 16;
-            } else {
-                cs[0] = w.x; cs[1] = w.y; cs[2] = w.z; cs[3] = w.w;
-            }
-            u32 mx = 0;
-#pragma unroll
-            for (u32 q = 0; q < SPV; ++q) mx = cs[q] > mx ? cs[q] : mx;
-            if (mx < d) continue;
-#pragma unroll
-            for (u32 q = 0; q < SPV; ++q) {
-                if (cs[q] >= d) {
-                    const u32 p = atomicAdd(&s_nsolid, 1u);
-                    if (p < a.max_solid) { l_key[p] = t_key[v * SPV + q]; l_cnt[p] = cs[q]; }
-                    sum += cs[q];
-                }
-            }
-        }
-    }
-    if (tid == 0 && s_ones) {
-        ++s_distinct;                                    // nobody else touches it between the barriers
-        if (s_ones >= a.d) {
-            const u32 p = atomicAdd(&s_nsolid, 1u);
-            if (p < a.max_solid) { l_key[p] = kEmpty; l_cnt[p] = s_ones; }
-            sum += s_ones;
-        }
-    }
-    sum = warp_reduce_add64(sum);
-    if ((tid & 31u) == 0 && sum) atomicAdd(&s_sum, sum);
-    __syncthreads();
-    const u32 ns = s_nsolid;
-    if (ns > a.max_solid) { if (tid == 0) { atomicOr(a.overflow, 4u); a.seg_count[seg] = 0; } return; }
-    if (tid == 0) {
-        a.seg_count[seg] = ns;
-        u64 *slot = a.stat_slots + (size_t)(blockIdx.x & (kStatSlots - 1)) * kStatSlotWords;
-        atomicAdd(&slot[0], (u64)s_distinct);
-        if (s_sum) atomicAdd(&slot[1], s_sum);
-    }
-    if (ns == 0) return;
-
-    // ---- 3: order the list by key. The solid edges of a segment are spread evenly over its key range, so one pass of
-    //         order-preserving binning (1,024 bins over the range of the segment's buckets) leaves bins of one or two
-    //         entries, which the owner of the bin puts in order by insertion. The table is dead: bins and the ordered
-    //         list live in its place. -----------------------------------------------------------------------------------
-    constexpr int NB = 1024, Q = NB / THREADS;                        // bins (also the most entries of a segment); per thread
-    u32 *bins = t_cnt;
-    u64 *o_key = t_key;
-    u32 *o_cnt = reinterpret_cast<u32 *>(t_key + NB);
-    const u64 k0 = kfirst << a.top_shift;
-    const u64 rm1 = ((klast - kfirst + 1ull) << a.top_shift) - 1ull;  // largest offset inside the segment's buckets
-    const int sh0 = 54 - __clzll((long long)rm1), sh = sh0 > 0 ? sh0 : 0;   // (rm1 >> sh) < 1024
-#pragma unroll
-    for (int q = 0; q < Q; ++q) bins[tid + q * THREADS] = 0;
-    __syncthreads();
-    u32 myb[Q], myr[Q];
-#pragma unroll
-    for (int q = 0; q < Q; ++q) {
-        const u32 i = tid + q * THREADS;
-        myb[q] = 0; myr[q] = 0;
-        if (i < ns) { myb[q] = (u32)((l_key[i] - k0) >> sh); myr[q] = atomicAdd(&bins[myb[q]], 1u); }
-    }
-    __syncthreads();
-    __shared__ u32 s_w[THREADS / 32];
-    u32 c[Q], csum = 0;
-#pragma unroll
-    for (int q = 0; q < Q; ++q) { c[q] = bins[Q * tid + q]; csum += c[q]; }
-    const u32 incl = warp_incl_scan_add(csum);
-    if ((tid & 31u) == 31u) s_w[tid >> 5] = incl;
-    __syncthreads();
-    u32 base0 = incl - csum;
-    for (u32 w = 0; w < (tid >> 5); ++w) base0 += s_w[w];
-    {
-        u32 run = base0;
-#pragma unroll
-        for (int q = 0; q < Q; ++q) { bins[Q * tid + q] = run; run += c[q]; }
-    }
-    __syncthreads();
-#pragma unroll
-    for (int q = 0; q < Q; ++q) {
-        const u32 i = tid + q * THREADS;
-        if (i < ns) { const u32 p = bins[myb[q]] + myr[q]; o_key[p] = l_key[i]; o_cnt[p] = l_cnt[i]; }
-    }
-    __syncthreads();
-    {
-        u32 b0 = base0;
-#pragma unroll
-        for (int q = 0; q < Q; ++q) {
-            for (u32 x = 1; x < c[q]; ++x) {                           // insertion sort of places [b0, b0 + c)
-                const u64 kx = o_key[b0 + x]; const u32 cx = o_cnt[b0 + x];
-                u32 y = x;
-                while (y > 0 && o_key[b0 + y - 1] > kx) { o_key[b0 + y] = o_key[b0 + y - 1]; o_cnt[b0 + y] = o_cnt[b0 + y - 1]; --y; }
-                o_key[b0 + y] = kx; o_cnt[b0 + y] = cx;
-            }
-            b0 += c[q];
-        }
-    }
-    __syncthreads();
-    // ---- write the sorted solid edges of the segment to its place in the staging buffer ---------------------------------
-    // staging (8 bytes per record, the sorter's spare buffer): the segment owns places [s, e); its ns <= (e - s) / d solid
-    // keys (d >= 2) fill the first half at most, their u32 counts start at the middle place
-    u32 *stage_cnt = reinterpret_cast<u32 *>(a.stage_keys + s + ((e - s + 1) >> 1));
-    for (u32 i = tid; i < ns; i += THREADS) { a.stage_keys[s + i] = o_key[i]; stage_cnt[i] = o_cnt[i]; }
+__device__ __forceinline__ u32 hash_slot(u64 key, u32 hshift) {
+    const u32 h = (u32)key + (u32)(key >> 32) * 0x9E3779B1u;
+    return (h * 0x85EBCA6Bu) >> hshift;
 }
 
-// seg_count -> exclusive prefix in place (u64), total to *total; one block, tiles of 4,096 (the array has n / chunk
-// entries: 97 k on config 2, 1.5 M on config 3)
-__global__ void __launch_bounds__(1024) hash_scan_kernel(u64 *__restrict__ seg_count, u64 nseg, u64 *total) {
+// shared-memory accesses by 32-bit shared address (no generic-to-shared conversion per access)
+__device__ __forceinline__ u64 s_cas64(u32 addr, u64 cmp, u64 val) {
+    u64 r;
+    asm volatile("atom.shared.cas.b64 %0, [%1], %2, %3;" : "=l"(r) : "r"(addr), "l"(cmp), "l"(val) : "memory");
+    return r;
+}
+template <int OFS>
+__device__ __forceinline__ void s_red_add(u32 addr, u32 v) {
+    asm volatile("red.shared.add.u32 [%0+%2], %1;" ::"r"(addr), "r"(v), "n"(OFS) : "memory");
+}
+
+// WARPS x 32 threads; a warp holds U rows of 32 records at a time; TSMAX table slots (power of two), MAXSOLID sort
+// places, NB = 1024 bins. Counts are 16-bit halves of u32 words (a segment has at most window + chunk < 65,536 records).
+// The records of a segment are dealt to the warps in groups of U full rows (no lane is ever idle there, so the group
+// code has no predicates); the rows that do not fill a group and the partial last row go one by one.
+template <int WARPS, int MINB, int U, int TSMAX, int MAXSOLID>
+__global__ void __launch_bounds__(WARPS * 32, MINB)
+hash_count_kernel(HashCountArgs a) {
+    constexpr int THREADS = WARPS * 32;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    u64 *t_key = reinterpret_cast<u64 *>(smem_raw);                             // u64[TSMAX]
+    u32 *t_cnt = reinterpret_cast<u32 *>(smem_raw + (size_t)TSMAX * 8);         // u16[TSMAX] as u32 pairs
+    u64 *l_key = reinterpret_cast<u64 *>(smem_raw + (size_t)TSMAX * 10);        // u64[MAXSOLID]
+    u32 *l_cnt = reinterpret_cast<u32 *>(smem_raw + (size_t)TSMAX * 10 + (size_t)MAXSOLID * 8);
+    __shared__ u32 s_ones, s_full, s_nsolid, s_distinct;
+    __shared__ u64 s_sum, s_look[2][3], s_krange[2];
+    __shared__ u32 s_w[WARPS];
+    const u32 tid = threadIdx.x, lane = tid & 31u, warp = tid >> 5;
+    const u32 tkey_s = (u32)__cvta_generic_to_shared(smem_raw);
+    const u64 nseg = a.nseg;
+
+    // Tickets are taken two segments ahead by thread 0, which also fetches the bounds of that segment while the CTA works:
+    // s_look[p] = {segment, first record, end} of the iteration with parity p (nothing depends on a load it just issued).
+    auto bounds_of = [&](u64 sg, u64 &bs, u64 &be) { bs = be = 0; if (sg < nseg) { bs = a.seg_start[sg]; be = a.seg_start[sg + 1]; } };
+    if (tid == 0) {
+        const u64 t0 = atomicAdd(a.ticket, 1u), t1 = atomicAdd(a.ticket, 1u);
+        u64 b0, e0, b1, e1;
+        bounds_of(t0, b0, e0); bounds_of(t1, b1, e1);
+        s_look[0][0] = t0; s_look[0][1] = b0; s_look[0][2] = e0;
+        s_look[1][0] = t1; s_look[1][1] = b1; s_look[1][2] = e1;
+    }
+    __syncthreads();
+    u64 seg = s_look[0][0];
+    if (seg >= nseg) return;
+    u64 s = s_look[0][1], e = s_look[0][2];
+    // full groups of the segment [bs, be) (none for the segment that ends with the last record of all: it alone can hold
+    // the all-ones key, which is counted beside the table by the row-by-row code)
+    auto groups_of = [&](u64 bs, u64 be) { return be <= bs || be == a.n ? 0u : ((u32)(be - bs) >> 5) / (u32)U; };
+    u64 cur[U];
+    auto load_group = [&](u64 (&k)[U], const u64 *src) {   // rows src[32 u + lane]
+#pragma unroll
+        for (int u = 0; u < U; ++u) k[u] = ld_stream(src + 32 * u + lane);
+    };
+    if (warp < groups_of(s, e)) load_group(cur, a.keys + s + (u64)warp * (32 * U));
+
+    for (u32 it = 0;; ++it) {
+        const u32 m = e > s ? (u32)(e - s) : 0u;         // a segment has fewer than 2^16 records
+        // table size: the power of two from 1.5 x the records of the segment on (all of them might be distinct)
+        u32 TS = 1024;
+        while (TS < (u32)TSMAX && (u64)TS * 2 < (u64)m * 3) TS <<= 1;
+        const u32 mask8 = (TS - 1u) << 3, hshift = 32u - (u32)__ffs(TS) + 1u;
+        {
+            uint4 *k4 = reinterpret_cast<uint4 *>(t_key), *c4 = reinterpret_cast<uint4 *>(t_cnt);
+            const uint4 ones = make_uint4(~0u, ~0u, ~0u, ~0u), zero = make_uint4(0u, 0u, 0u, 0u);
+            for (u32 i = tid; i < TS / 2; i += THREADS) k4[i] = ones;
+            for (u32 i = tid; i < TS / 8; i += THREADS) c4[i] = zero;
+        }
+        u64 la_seg = 0, la_s = 0, la_e = 0;              // (thread 0) the segment of the iteration after the next one
+        u64 kf = 0, kl = 0;                              // (thread 32) first and last record of this segment
+        if (tid == 0) {
+            s_ones = 0; s_full = 0; s_nsolid = 0; s_distinct = 0; s_sum = 0;
+            la_seg = atomicAdd(a.ticket, 1u);          // consumed behind the insert phase: nothing waits for it here
+        }
+        if (tid == 32 % THREADS && m) { kf = a.keys[s]; kl = a.keys[e - 1]; }
+        __syncthreads();
+
+        // ---- 1: insert ---------------------------------------------------------------------------------------------------
+        u32 created = 0;
+        const bool last_seg = e == a.n;
+        // count of the slot at byte offset a8 of the key table: 16-bit halves, two slots per word
+        auto cnt_add = [&](u32 a8) { s_red_add<TSMAX * 8>(tkey_s + ((a8 >> 2) & ~3u), (a8 & 8u) ? 0x10000u : 1u); };
+        // NR rows held by the warp: first the home slot of every record (one CAS that installs the key or returns what
+        // is there, no loop), then ONE probing loop for the records whose home slot holds another key
+        auto insert_rows = [&](auto nr_tag, const u64 *k, bool valid) {
+            constexpr int NR = decltype(nr_tag)::value;
+            u64 old[NR]; u32 a8[NR];
+#pragma unroll
+            for (int r = 0; r < NR; ++r) {
+                a8[r] = hash_slot(k[r], hshift) << 3;
+                old[r] = k[r];
+                if (NR > 1 || valid) old[r] = s_cas64(tkey_s + a8[r], kEmpty, k[r]);
+            }
+            u32 pend = 0;
+#pragma unroll
+            for (int r = 0; r < NR; ++r) {
+                const bool emp = old[r] == kEmpty;
+                if (NR > 1 || valid) {
+                    if (emp || old[r] == k[r]) cnt_add(a8[r]); else pend |= 1u << r;
+                    created += emp;
+                }
+            }
+            if (pend) {
+                u64 key = 0; u32 b8 = 0, probes = 0;
+                bool have = false;
+                for (;;) {
+                    if (!have) {
+                        if (!pend) break;
+                        const u32 r = (u32)__ffs(pend) - 1u;
+                        pend &= pend - 1u;
+                        key = k[0]; b8 = a8[0];
+#pragma unroll
+                        for (int q = 1; q < NR; ++q) if (r == (u32)q) { key = k[q]; b8 = a8[q]; }
+                        probes = 0; have = true;
+                    }
+                    b8 = (b8 + 8u) & mask8;
+                    const u64 o = s_cas64(tkey_s + b8, kEmpty, key);
+                    if (o == kEmpty || o == key) { cnt_add(b8); created += o == kEmpty; have = false; }
+                    else if (++probes >= TS) { s_full = 1; have = false; }
+                }
+            }
+        };
+        const u32 G = groups_of(s, e);
+        {
+            u64 nxt[U];
+            for (u32 g = warp; g < G; g += 2 * WARPS) {  // two groups per round: one is inserted while the other arrives
+                const bool more = g + WARPS < G;
+                if (more) load_group(nxt, a.keys + s + (u64)(g + WARPS) * (32 * U));
+                insert_rows(std::integral_constant<int, U>{}, cur, true);
+                if (g + 2 * WARPS < G) load_group(cur, a.keys + s + (u64)(g + 2 * WARPS) * (32 * U));
+                if (more) insert_rows(std::integral_constant<int, U>{}, nxt, true);
+            }
+        }
+        {   // the rows behind the last full group, and the partial last row: x-th of them belongs to warp (G + x) % WARPS
+            const u32 row0 = G * (u32)U, nx = ((m + 31u) >> 5) - row0;
+            for (u32 x = (warp + WARPS - G % WARPS) % WARPS; x < nx; x += WARPS) {
+                const u32 i = (row0 + x) * 32u + lane;
+                const bool valid = i < m;
+                u64 key = valid ? ld_stream(a.keys + s + i) : 0ull;
+                if (last_seg && valid && key == kEmpty) { atomicAdd(&s_ones, 1u); insert_rows(std::integral_constant<int, 1>{}, &key, false); }
+                else insert_rows(std::integral_constant<int, 1>{}, &key, valid);
+            }
+        }
+        if (created) atomicAdd(&s_distinct, created);
+        if (tid == 32 % THREADS) { s_krange[0] = kf >> a.top_shift; s_krange[1] = kl >> a.top_shift; }
+        __syncthreads();
+        // the first records of my next segment are on their way while this one is finished
+        const u64 next = s_look[(it + 1) & 1][0], ns_ = s_look[(it + 1) & 1][1], ne_ = s_look[(it + 1) & 1][2];
+        if (next < nseg && warp < groups_of(ns_, ne_)) load_group(cur, a.keys + ns_ + (u64)warp * (32 * U));
+        if (tid == 0) bounds_of(la_seg, la_s, la_e);     // stored at the end of the iteration
+        const u64 kfirst = s_krange[0], klast = s_krange[1];
+        const bool full = s_full != 0;
+        if (full && tid == 0) atomicOr(a.overflow, 2u);
+
+        // ---- 2: the solid slots, compacted to this iteration's list ------------------------------------------------------------
+        u64 sum = 0;
+        if (!full && m) {   // the live part of the table, 16 bytes of counts (8 slots) per load; most vectors hold no solid edge
+            const uint4 *c4 = reinterpret_cast<const uint4 *>(t_cnt);
+            const u32 d = a.d;
+            for (u32 v = tid; v < TS / 8; v += THREADS) {
+                const uint4 w = c4[v];
+                if (d == 2 && ((w.x | w.y | w.z | w.w) & 0xfffefffeu) == 0) continue;   // no count above 1
+                const u32 wd[4] = {w.x, w.y, w.z, w.w};
+                u32 m8 = 0;                              // bit q: slot 8 v + q holds a solid edge
+#pragma unroll
+                for (u32 q = 0; q < 4; ++q) m8 |= ((wd[q] & 0xffffu) >= d ? 1u : 0u) << (2 * q) | ((wd[q] >> 16) >= d ? 2u : 0u) << (2 * q);
+                while (m8) {
+                    const u32 q = (u32)__ffs(m8) - 1u;
+                    m8 &= m8 - 1u;
+                    u32 wq = wd[0];
+                    if ((q >> 1) == 1) wq = wd[1];
+                    if ((q >> 1) == 2) wq = wd[2];
+                    if ((q >> 1) == 3) wq = wd[3];
+                    const u32 c = (wq >> ((q & 1u) * 16u)) & 0xffffu;
+                    const u32 p = atomicAdd(&s_nsolid, 1u);
+                    if (p < (u32)MAXSOLID) { l_key[p] = t_key[v * 8 + q]; l_cnt[p] = c; }
+                    sum += c;
+                }
+            }
+            if (tid == 0 && s_ones) {
+                atomicAdd(&s_distinct, 1u);
+                if (s_ones >= a.d) {
+                    const u32 p = atomicAdd(&s_nsolid, 1u);
+                    if (p < (u32)MAXSOLID) { l_key[p] = kEmpty; l_cnt[p] = s_ones; }
+                    sum += s_ones;
+                }
+            }
+            sum = warp_reduce_add64(sum);
+            if (lane == 0 && sum) atomicAdd(&s_sum, sum);
+        }
+        __syncthreads();
+        u32 ns = s_nsolid;
+        if (ns > (u32)MAXSOLID) { if (tid == 0) atomicOr(a.overflow, 4u); ns = 0; }
+        if (full) ns = 0;
+        // ---- 3a: the count of the segment, the sum of its block, statistics ---------------------------------------------------------
+        if (tid == 0) {
+            a.seg_count[seg] = ns;
+            if (ns) atomicAdd(a.blk_sum + seg / kSegBlock, (u64)ns);
+            u64 *slot = a.stat_slots + (size_t)(seg & (kStatSlots - 1)) * kStatSlotWords;
+            if (ns) atomicAdd(&slot[1], s_sum);
+            if (s_distinct && !full) atomicAdd(&slot[0], (u64)s_distinct);
+        }
+
+        // ---- 3b: order the list by key. The solid edges of a segment are spread evenly over its key range, so one pass of
+        //          order-preserving binning (1,024 bins over the range of the segment's buckets) leaves bins of one or two
+        //          entries, which the owner of the bin puts in order by insertion. The table is dead: bins and the ordered
+        //          entries live in its place. ---------------------------------------------------------------------------------------
+        constexpr int NB = 1024, Q = NB / THREADS, QE = MAXSOLID / THREADS;   // bins per thread; list entries per thread
+        static_assert(NB % THREADS == 0 && MAXSOLID % THREADS == 0 && (size_t)NB * 4 <= (size_t)TSMAX * 2 && (size_t)MAXSOLID * 12 <= (size_t)TSMAX * 8, "layout");
+        if (ns) {
+            u32 *bins = t_cnt;
+            u64 *o_key = t_key;
+            u32 *o_cnt = reinterpret_cast<u32 *>(t_key + MAXSOLID);
+            const u64 k0 = kfirst << a.top_shift;
+            const u64 rm1 = ((klast - kfirst + 1ull) << a.top_shift) - 1ull;  // largest offset inside the segment's buckets
+            const int sh0 = 54 - __clzll((long long)rm1), sh = sh0 > 0 ? sh0 : 0;   // (rm1 >> sh) < 1024
+#pragma unroll
+            for (int q = 0; q < Q; ++q) bins[tid + q * THREADS] = 0;
+            __syncthreads();
+            u32 myb[QE], myr[QE];
+#pragma unroll
+            for (int q = 0; q < QE; ++q) {
+                const u32 i = tid + q * THREADS;
+                myb[q] = 0; myr[q] = 0;
+                if (i < ns) { myb[q] = (u32)((l_key[i] - k0) >> sh); myr[q] = atomicAdd(&bins[myb[q]], 1u); }
+            }
+            __syncthreads();
+            u32 c[Q], csum = 0;
+#pragma unroll
+            for (int q = 0; q < Q; ++q) { c[q] = bins[Q * tid + q]; csum += c[q]; }
+            const u32 incl = warp_incl_scan_add(csum);
+            if (lane == 31u) s_w[warp] = incl;
+            __syncthreads();
+            u32 base0 = incl - csum;
+            for (u32 w = 0; w < warp; ++w) base0 += s_w[w];
+            {
+                u32 run = base0;
+#pragma unroll
+                for (int q = 0; q < Q; ++q) { bins[Q * tid + q] = run; run += c[q]; }
+            }
+            __syncthreads();
+#pragma unroll
+            for (int q = 0; q < QE; ++q) {
+                const u32 i = tid + q * THREADS;
+                if (i < ns) { const u32 p = bins[myb[q]] + myr[q]; o_key[p] = l_key[i]; o_cnt[p] = l_cnt[i]; }
+            }
+            __syncthreads();
+            {
+                u32 b0 = base0;
+#pragma unroll
+                for (int q = 0; q < Q; ++q) {
+                    for (u32 x = 1; x < c[q]; ++x) {                           // insertion sort of places [b0, b0 + c)
+                        const u64 kx = o_key[b0 + x]; const u32 cx = o_cnt[b0 + x];
+                        u32 y = x;
+                        while (y > 0 && o_key[b0 + y - 1] > kx) { o_key[b0 + y] = o_key[b0 + y - 1]; o_cnt[b0 + y] = o_cnt[b0 + y - 1]; --y; }
+                        o_key[b0 + y] = kx; o_cnt[b0 + y] = cx;
+                    }
+                    b0 += c[q];
+                }
+            }
+            __syncthreads();
+            // staging (8 bytes per record, the sorter's spare buffer): the segment owns places [s, e); its ns <= (e - s) / d
+            // solid keys (d >= 2) fill the first half at most, their u32 counts start at the middle place
+            u32 *stage_cnt = reinterpret_cast<u32 *>(a.stage_keys + s + ((m + 1u) >> 1));
+            for (u32 i = tid; i < ns; i += THREADS) { a.stage_keys[s + i] = o_key[i]; stage_cnt[i] = o_cnt[i]; }
+        }
+        if (next >= nseg) break;
+        if (tid == 0) { s_look[it & 1][0] = la_seg; s_look[it & 1][1] = la_s; s_look[it & 1][2] = la_e; }
+        seg = next; s = ns_; e = ne_;
+        __syncthreads();   // the table is cleared next
+    }
+}
+
+// blk_sum[b] (solid edges of segments [256 b, 256 b + 256)) -> exclusive prefix in place, total to *total and the output
+// cursor behind this range; one block (a range of 2^34 records has at most 2^15 blocks of 256 segments of 2,048 records)
+__global__ void __launch_bounds__(1024) hash_scan_kernel(u64 *__restrict__ blk_sum, u64 nblk, u64 *total, const u64 *cursor_in, u64 *cursor_out) {
     __shared__ u64 s_w[32];
     __shared__ u64 s_carry;
     const u32 tid = threadIdx.x, lane = tid & 31u, warp = tid >> 5;
     if (tid == 0) s_carry = 0;
     __syncthreads();
-    for (u64 base = 0; base < nseg; base += 4096) {
-        const u64 i = base + 4ull * tid;
-        u64 v[4];
-#pragma unroll
-        for (int q = 0; q < 4; ++q) v[q] = i + q < nseg ? seg_count[i + q] : 0;
-        const u64 sum = v[0] + v[1] + v[2] + v[3];
-        u64 incl = sum;
+    for (u64 base = 0; base < nblk; base += 1024) {
+        const u64 i = base + tid;
+        const u64 v = i < nblk ? blk_sum[i] : 0;
+        u64 incl = v;
 #pragma unroll
         for (int o = 1; o < 32; o <<= 1) {
             u64 t = __shfl_up_sync(0xffffffffu, incl, o);
@@ -274,41 +374,82 @@ __global__ void __launch_bounds__(1024) hash_scan_kernel(u64 *__restrict__ seg_c
         __syncthreads();
         u64 off = s_carry;
         for (u32 w = 0; w < warp; ++w) off += s_w[w];
-        u64 run = off + incl - sum;
-#pragma unroll
-        for (int q = 0; q < 4; ++q) { if (i + q < nseg) seg_count[i + q] = run; run += v[q]; }
+        if (i < nblk) blk_sum[i] = off + incl - v;
         __syncthreads();
         if (tid == 1023) s_carry = off + incl;
         __syncthreads();
     }
-    if (tid == 0) *total = s_carry;
+    if (tid == 0) { *total = s_carry; *cursor_out = *cursor_in + s_carry; }
 }
 
-// the staged solid edges of every segment appended to the output, in segment (= key) order; one warp per segment
-__global__ void __launch_bounds__(256) hash_copy_kernel(HashCountArgs a, const u64 *__restrict__ total, DevState *st, int range_parity) {
-    const u64 base = st->out_cursor[range_parity];
-    const u32 lane = lane_id();
-    for (u64 seg = (u64)blockIdx.x * 8 + (threadIdx.x >> 5); seg < a.nseg; seg += (u64)gridDim.x * 8) {
-        const u64 off = a.seg_count[seg];
-        const u64 cnt = (seg + 1 < a.nseg ? a.seg_count[seg + 1] : *total) - off;
-        const u64 s = a.seg_start[seg], e = a.seg_start[seg + 1];
-        const u32 *stage_cnt = reinterpret_cast<const u32 *>(a.stage_keys + s + ((e - s + 1) >> 1));
-        for (u64 i = lane; i < cnt; i += 32) {
-            const u64 pos = base + off + i;
-            if (pos < a.out_cap) { a.out_keys[pos] = a.stage_keys[s + i]; a.out_mult[pos] = stage_cnt[i]; }
+// the staged solid edges of every segment appended to the output, in segment (= key) order: a CTA per block of 256
+// segments (prefix of their counts in shared memory), a warp per segment
+__global__ void __launch_bounds__(256) hash_copy_kernel(HashCountArgs a) {
+    __shared__ u64 s_off[kSegBlock];
+    __shared__ u64 s_w[8];
+    const u32 tid = threadIdx.x, lane = tid & 31u, warp = tid >> 5;
+    const u64 base = *a.cursor_in;
+    for (u64 blk = blockIdx.x; blk * kSegBlock < a.nseg; blk += gridDim.x) {
+        const u64 seg0 = blk * kSegBlock + tid;
+        const u64 v = seg0 < a.nseg ? a.seg_count[seg0] : 0;
+        u64 incl = v;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            u64 t = __shfl_up_sync(0xffffffffu, incl, o);
+            if (lane >= (u32)o) incl += t;
         }
+        if (lane == 31) s_w[warp] = incl;
+        __syncthreads();
+        u64 off = a.blk_sum[blk];
+        for (u32 w = 0; w < warp; ++w) off += s_w[w];
+        s_off[tid] = off + incl - v;
+        __syncthreads();
+        for (u32 j = warp; j < kSegBlock; j += 8) {
+            const u64 seg = blk * kSegBlock + j;
+            if (seg >= a.nseg) break;
+            const u64 cnt = a.seg_count[seg];
+            if (cnt == 0) continue;
+            const u64 s = a.seg_start[seg], e = a.seg_start[seg + 1];
+            const u32 *stage_cnt = reinterpret_cast<const u32 *>(a.stage_keys + s + ((e - s + 1) >> 1));
+            const u64 pos0 = base + s_off[j];
+            for (u64 i = lane; i < cnt; i += 32)
+                if (pos0 + i < a.out_cap) { a.out_keys[pos0 + i] = a.stage_keys[s + i]; a.out_mult[pos0 + i] = stage_cnt[i]; }
+        }
+        __syncthreads();
     }
-    if (blockIdx.x == 0 && threadIdx.x == 0) st->out_cursor[range_parity ^ 1] = base + *total;
 }
 
-// two shapes: big segments (chunk 4,096: one or two long buckets) 512 threads x 2 CTAs per SM with 8,192 slots; small
-// segments (chunk 2,048: many short buckets) 256 threads x 4 CTAs per SM with 4,096 slots and 16-bit counts
-u64 hash_smem_bytes(u32 table_slots, u32 max_solid) { return (u64)table_slots * (table_slots > 4096 ? 12 : 10) + (u64)max_solid * 12; }
+// shapes: long buckets (chunk 4,096: one or two buckets per segment) and short ones (chunk 2,048: many buckets per segment)
+template <int WARPS, int MINB, int U, int TSMAX, int MAXSOLID>
+struct HashShape {
+    static constexpr int THREADS = WARPS * 32;
+    static constexpr size_t kSmem = (size_t)TSMAX * 10 + (size_t)MAXSOLID * 12;
+    static int setup(int *blocks_per_sm) {
+        int e = (int)cudaFuncSetAttribute(hash_count_kernel<WARPS, MINB, U, TSMAX, MAXSOLID>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmem);
+        if (e) return e;
+        return (int)cudaOccupancyMaxActiveBlocksPerMultiprocessor(blocks_per_sm, hash_count_kernel<WARPS, MINB, U, TSMAX, MAXSOLID>, THREADS, kSmem);
+    }
+    static int launch(const HashCountArgs &a, int blocks_per_sm, cudaStream_t s) {
+        u64 g = (u64)num_sms() * (u64)(blocks_per_sm > 0 ? blocks_per_sm : 1);
+        if (g > a.nseg) g = a.nseg;
+        hash_count_kernel<WARPS, MINB, U, TSMAX, MAXSOLID><<<(unsigned)g, THREADS, kSmem, s>>>(a);
+        return (int)cudaGetLastError();
+    }
+};
+#ifndef SDBG_HASH_BIG
+#define SDBG_HASH_BIG 16, 2, 4, 8192, 1024
+#endif
+#ifndef SDBG_HASH_SMALL
+#define SDBG_HASH_SMALL 8, 4, 4, 4096, 1024
+#endif
+using HashBig = HashShape<SDBG_HASH_BIG>;
+using HashSmall = HashShape<SDBG_HASH_SMALL>;
+static int g_occ_big = 0, g_occ_small = 0;
 
 int hash_setup() {
-    int e = (int)cudaFuncSetAttribute(hash_count_kernel<512, 2, 8, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, 110 * 1024);
+    int e = HashBig::setup(&g_occ_big);
     if (e) return e;
-    return (int)cudaFuncSetAttribute(hash_count_kernel<256, 4, 9, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 54 * 1024);
+    return HashSmall::setup(&g_occ_small);
 }
 
 void launch_hash_bounds(const HashCountArgs &a, cudaStream_t s) {
@@ -316,16 +457,14 @@ void launch_hash_bounds(const HashCountArgs &a, cudaStream_t s) {
     hash_bounds_kernel<<<(unsigned)blocks, 256, 0, s>>>(a.keys, a.n, a.top_shift, a.chunk, a.window, a.nseg, a.seg_start, a.overflow);
 }
 int launch_hash_count(const HashCountArgs &a, cudaStream_t s) {
-    if (a.nseg == 0 || a.nseg > 0x7fffffffull || a.max_solid != 1024 || (u64)a.window + a.chunk >= 65536) return (int)cudaErrorInvalidValue;
-    const size_t smem = hash_smem_bytes(a.table_slots, a.max_solid);
-    if (a.table_slots > 4096) hash_count_kernel<512, 2, 8, false><<<(unsigned)a.nseg, 512, smem, s>>>(a);
-    else hash_count_kernel<256, 4, 9, true><<<(unsigned)a.nseg, 256, smem, s>>>(a);
-    return (int)cudaGetLastError();
+    if (a.nseg == 0 || a.nseg > 0x7fffffffull || (u64)a.window + a.chunk >= 65536) return (int)cudaErrorInvalidValue;
+    return a.chunk >= 4096 ? HashBig::launch(a, g_occ_big, s) : HashSmall::launch(a, g_occ_small, s);
 }
-void launch_hash_append(const HashCountArgs &a, u64 *total, DevState *st, int range_parity, cudaStream_t s) {
-    hash_scan_kernel<<<1, 1024, 0, s>>>(a.seg_count, a.nseg, total);
-    const u64 blocks = (a.nseg + 7) / 8;
-    hash_copy_kernel<<<(unsigned)blocks, 256, 0, s>>>(a, total, st, range_parity);
+void launch_hash_append(const HashCountArgs &a, u64 *total, cudaStream_t s) {
+    const u64 nblk = (a.nseg + kSegBlock - 1) / kSegBlock;
+    hash_scan_kernel<<<1, 1024, 0, s>>>(a.blk_sum, nblk, total, a.cursor_in, a.cursor_out);
+    const u64 cap = (u64)num_sms() * 8;
+    hash_copy_kernel<<<(unsigned)(nblk < cap ? nblk : cap), 256, 0, s>>>(a);
 }
 
 }  // namespace sdbg

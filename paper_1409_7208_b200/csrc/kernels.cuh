@@ -35,7 +35,7 @@ __device__ __forceinline__ u32 valid_mask32(const u64 *__restrict__ ends, u64 g,
 
 // ---- launchers (host) ----------------------------------------------------------------------------------
 void launch_pack(const unsigned char *d_ascii, u64 nb, u64 *words, u64 slot0, u64 err_index_base, DevState *st, cudaStream_t s);
-void launch_mark_ends(const u64 *d_offsets, u64 n, u64 off0, u64 nb, u64 *ends, u64 slot0, DevState *st, cudaStream_t s);
+void launch_mark_ends(const u64 *d_offsets, u64 n, u64 off0, u64 nb_total, u64 pad_nb, u64 *ends, u64 slot0, DevState *st, cudaStream_t s);
 void launch_count_windows(const u64 *ends, u64 n_slots, u32 k, DevState *st, cudaStream_t s);
 
 struct ExtractArgs {
@@ -66,11 +66,17 @@ struct RadixArgs {
     u32 *ticket;                         // zeroed
     PassDesc pass; u32 epoch;
     bool force_wide;                     // use the layout for ranges of 2^32 records and more whatever n is (tests)
-    bool unstable;                       // the pass need not keep the order of equal digits (first pass of a sort; one-word keys without payload)
+    bool unstable;                       // CONTRACT: set only when (a) this is pass 0 of a multi-pass sort whose input order carries no
+                                         // information AND (b) the caller merges equal keys afterwards (sdbg_count_edges). The pass then
+                                         // need not keep the order of equal digits (radix.cu FIRST: rank = return value of the count atomic,
+                                         // hardware-defined among the lanes of a warp). A single pass that refines an existing order
+                                         // (api_full.inc compute_zero_degree) must leave it false; launch_radix_pass counts FIRST launches in
+                                         // radix_unstable_launches() so that tests can assert who used it.
 };
 u64 radix_tile_records(u32 W, bool has_vals);
 u64 radix_max_records(u32 W, bool has_vals);   // cap of one sort range (look-back word layout)
 int launch_radix_pass(const RadixArgs &a, cudaStream_t s);
+u64 radix_unstable_launches();           // launches of the FIRST (unstable) variant by this process so far
 // multi-word keys (radix.cu "word-wise LSD with an index payload")
 void launch_gather_word(const u64 *recs, u32 W, u32 q, const u32 *idx_in, u64 *word_out, u32 *idx_out, u64 n, cudaStream_t s);
 void launch_gather_recs(const u64 *recs, u32 W, const u32 *idx, u64 *out, u64 n, cudaStream_t s);
@@ -107,20 +113,22 @@ void launch_append_solid(const u64 *keys, const u32 *mult, const u32 *idx, const
 struct HashCountArgs {
     const u64 *keys; u64 n;              // one-word keys sorted by key >> top_shift
     u32 top_shift, chunk, window;        // nominal records per segment; how far a bucket may run past a nominal border
-    u32 table_slots, max_solid, d;       // table slots (power of two) and sort places of a CTA; d >= 2
+    u32 d;                               // solid threshold, >= 2
     u64 nseg;                            // ceil(n / chunk)
     u64 *seg_start;                      // u64[nseg + 1] scratch
-    u64 *seg_count;                      // u64[nseg + 1] scratch: solid edges per segment, then their exclusive prefix
-    u32 *overflow;                       // zeroed; nonzero afterwards: something did not fit, nothing may be used
+    u64 *seg_count;                      // u64[nseg] scratch: solid edges per segment
+    u64 *blk_sum;                        // u64[ceil(nseg / 256)] scratch, zeroed: solid edges per block of 256 segments, then their prefix
     u64 *stage_keys;                     // u64[n] scratch (the sorter's spare buffer)
+    u32 *ticket;                         // zeroed: segments are handed out in order
+    u32 *overflow;                       // zeroed; nonzero afterwards: something did not fit, nothing may be used
     u64 *stat_slots;
+    const u64 *cursor_in; u64 *cursor_out;   // solid edges appended before this range / after it (DevState::out_cursor)
     u64 *out_keys; u32 *out_mult; u64 out_cap;
 };
 int hash_setup();
-u64 hash_smem_bytes(u32 table_slots, u32 max_solid);
 void launch_hash_bounds(const HashCountArgs &a, cudaStream_t s);
 int launch_hash_count(const HashCountArgs &a, cudaStream_t s);
-void launch_hash_append(const HashCountArgs &a, u64 *total, DevState *st, int range_parity, cudaStream_t s);
+void launch_hash_append(const HashCountArgs &a, u64 *total /* device scratch */, cudaStream_t s);
 
 struct EmitArgs {
     const u64 *keys; const u32 *mult_in; u64 n; u32 k, W;

@@ -78,7 +78,7 @@ __global__ void __launch_bounds__(256) hash_build_kernel(const u64 *__restrict__
 }
 void launch_hash_build(const u64 *keys, u64 n, u32 W, void *table, u64 slots, cudaStream_t s) {
     u64 blocks = (n + 255) / 256;
-    if (blocks > (u64)kNumSMs * 16) blocks = (u64)kNumSMs * 16;
+    if (blocks > (u64)num_sms() * 16) blocks = (u64)num_sms() * 16;
     if (blocks == 0) return;
     ulonglong2 *t = reinterpret_cast<ulonglong2 *>(table);
     switch (W) {
@@ -233,7 +233,7 @@ int launch_mercy(const MercyArgs &a, u32 W_, u32 WT_, DevState *st, cudaStream_t
     const u64 nwords = a.n_slots / 64;
     if (nwords == 0 || a.n == 0) return 0;
     u64 blocks = (nwords + 127) / 128;
-    if (blocks > (u64)kNumSMs * 32) blocks = (u64)kNumSMs * 32;
+    if (blocks > (u64)num_sms() * 32) blocks = (u64)num_sms() * 32;
     const unsigned g = (unsigned)blocks;
     switch (W_ * 8 + WT_) {
         case 1 * 8 + 1: mercy_kernel<1, 1><<<g, 128, 0, s>>>(a, st); break;

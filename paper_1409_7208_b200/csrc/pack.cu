@@ -62,24 +62,23 @@ __global__ void __launch_bounds__(256) pack_kernel(const unsigned char *__restri
 }
 
 // One thread per read: set the end mark of its last base. Thread 0 also marks the padding slots of the chunk's
-// final 64-group. `ends` words of the chunk were zeroed before.
-__global__ void __launch_bounds__(256) mark_ends_kernel(const u64 *__restrict__ offsets, u64 n, u64 off0, u64 nb,
-                                                        u64 *__restrict__ ends, u64 slot0) {
+// final 64-group (pad_nb = bases of the call when this launch covers its first reads, else 0). `ends` words of the
+// chunk were zeroed before. Every offset is bounded HERE, before it addresses anything: a read must satisfy
+// off0 <= b <= e <= off0 + nb_total (non-decreasing offsets inside the span of the call); any other read is skipped
+// and raises the flag (st->n_windows = ~0) that sdbg_pack_reads turns into SDBG_E_INVAL — a malformed offsets array
+// never causes a write outside the chunk.
+__global__ void __launch_bounds__(256) mark_ends_kernel(const u64 *__restrict__ offsets, u64 n, u64 off0, u64 nb_total, u64 pad_nb,
+                                                        u64 *__restrict__ ends, u64 slot0, DevState *st) {
     u64 r = (u64)blockIdx.x * blockDim.x + threadIdx.x;
-    if (r == 0 && (nb & 63)) atomicOr(&ends[(slot0 + nb) >> 6], ~0ull << (nb & 63));
+    if (r == 0 && (pad_nb & 63)) atomicOr(&ends[(slot0 + pad_nb) >> 6], ~0ull << (pad_nb & 63));
     for (; r < n; r += (u64)gridDim.x * blockDim.x) {
-        u64 b = offsets[r], e = offsets[r + 1];
+        const u64 b = offsets[r], e = offsets[r + 1];
+        if (b < off0 || e < b || e - off0 > nb_total) { st->n_windows = ~0ull; continue; }
         if (e > b) {
-            u64 p = slot0 + (e - 1 - off0);
+            const u64 p = slot0 + (e - 1 - off0);
             atomicOr(&ends[p >> 6], 1ull << (p & 63));
         }
     }
-}
-
-// Checks that offsets are non-decreasing (sets bad flag in st->n_windows = ~0 otherwise). Cheap sanity pass.
-__global__ void __launch_bounds__(256) check_offsets_kernel(const u64 *__restrict__ offsets, u64 n, DevState *st) {
-    for (u64 r = (u64)blockIdx.x * blockDim.x + threadIdx.x; r < n; r += (u64)gridDim.x * blockDim.x)
-        if (offsets[r + 1] < offsets[r]) st->n_windows = ~0ull;
 }
 
 // Counts the valid (k+1)-windows: 32 slots per thread.
@@ -96,23 +95,22 @@ void launch_pack(const unsigned char *d_ascii, u64 nb, u64 *words, u64 slot0, u6
     if (nb == 0) return;
     u64 nwords = (nb + 31) / 32;
     u64 blocks = (nwords + 255) / 256;
-    if (blocks > (u64)kNumSMs * 16) blocks = (u64)kNumSMs * 16;
+    if (blocks > (u64)num_sms() * 16) blocks = (u64)num_sms() * 16;
     pack_kernel<<<(unsigned)blocks, 256, 0, s>>>(d_ascii, nb, words, slot0, err_index_base, st);
 }
 
-void launch_mark_ends(const u64 *d_offsets, u64 n, u64 off0, u64 nb, u64 *ends, u64 slot0, DevState *st, cudaStream_t s) {
+void launch_mark_ends(const u64 *d_offsets, u64 n, u64 off0, u64 nb_total, u64 pad_nb, u64 *ends, u64 slot0, DevState *st, cudaStream_t s) {
     u64 blocks = (n + 255) / 256;
     if (blocks == 0) blocks = 1;
-    if (blocks > (u64)kNumSMs * 16) blocks = (u64)kNumSMs * 16;
-    check_offsets_kernel<<<(unsigned)blocks, 256, 0, s>>>(d_offsets, n, st);
-    mark_ends_kernel<<<(unsigned)blocks, 256, 0, s>>>(d_offsets, n, off0, nb, ends, slot0);
+    if (blocks > (u64)num_sms() * 16) blocks = (u64)num_sms() * 16;
+    mark_ends_kernel<<<(unsigned)blocks, 256, 0, s>>>(d_offsets, n, off0, nb_total, pad_nb, ends, slot0, st);
 }
 
 void launch_count_windows(const u64 *ends, u64 n_slots, u32 k, DevState *st, cudaStream_t s) {
     u64 ngroups = n_slots / 32;
     if (ngroups == 0) return;
     u64 blocks = (ngroups + 255) / 256;
-    if (blocks > (u64)kNumSMs * 16) blocks = (u64)kNumSMs * 16;
+    if (blocks > (u64)num_sms() * 16) blocks = (u64)num_sms() * 16;
     count_windows_kernel<<<(unsigned)blocks, 256, 0, s>>>(ends, n_slots, k, st);
 }
 

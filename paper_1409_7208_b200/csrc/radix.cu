@@ -555,6 +555,9 @@ u64 radix_tile_records(u32 W, bool v) {
     return 0;
 }
 
+static u64 g_unstable_launches = 0;
+u64 radix_unstable_launches() { return g_unstable_launches; }
+
 template <int W, bool HAS_VAL>
 static int launch_one(const RadixArgs &a, cudaStream_t s) {
     const u64 tiles = (a.n + tile_of<W, HAS_VAL>() - 1) / tile_of<W, HAS_VAL>();
@@ -564,7 +567,7 @@ static int launch_one(const RadixArgs &a, cudaStream_t s) {
     if (wide && HAS_VAL) return (int)cudaErrorInvalidValue;
     if (a.pass.bits != kRadixBits || (a.pass.shift & 7u)) return (int)cudaErrorInvalidValue;   // byte-aligned digits only
     // persistent CTAs: every SM filled to the occupancy the kernel was built for
-    const u64 resident = SDBG_PERSISTENT ? (u64)kNumSMs * RadixCfg<W, HAS_VAL>::MINB : tiles;
+    const u64 resident = SDBG_PERSISTENT ? (u64)num_sms() * RadixCfg<W, HAS_VAL>::MINB : tiles;
     const unsigned g = (unsigned)(tiles < resident ? tiles : resident), t = RadixCfg<W, HAS_VAL>::THREADS;
     const size_t sm = RadixSmem<W, HAS_VAL>::kBytes;
     const bool hi = a.pass.shift >= 32;
@@ -577,6 +580,7 @@ static int launch_one(const RadixArgs &a, cudaStream_t s) {
     }
     if constexpr (W == 1 && !HAS_VAL) {
         if (a.unstable) {
+            ++g_unstable_launches;
             if (hi) onesweep_kernel<1, false, true, false, true><<<g, t, sm, s>>>(a);
             else    onesweep_kernel<1, false, false, false, true><<<g, t, sm, s>>>(a);
             return (int)cudaGetLastError();
@@ -621,7 +625,7 @@ __global__ void __launch_bounds__(256) gather_recs_kernel(const u64 *__restrict_
 }
 static unsigned gather_blocks(u64 n) {
     u64 b = (n + 255) / 256;
-    const u64 cap = (u64)kNumSMs * 16;
+    const u64 cap = (u64)num_sms() * 16;
     return (unsigned)(b < cap ? b : cap);
 }
 void launch_gather_word(const u64 *recs, u32 W, u32 q, const u32 *idx_in, u64 *word_out, u32 *idx_out, u64 n, cudaStream_t s) {
@@ -682,7 +686,7 @@ __global__ void __launch_bounds__(256) key_hist_kernel(const u64 *__restrict__ k
 void launch_key_hist(const u64 *keys, u64 n, u32 W, const PassTable &pt, u64 *hist, cudaStream_t s) {
     if (n == 0) return;
     u64 blocks = (n + 255) / 256;
-    if (blocks > (u64)kNumSMs * 8) blocks = (u64)kNumSMs * 8;
+    if (blocks > (u64)num_sms() * 8) blocks = (u64)num_sms() * 8;
     size_t smem = (size_t)pt.n * kRadix * 4;
     switch (W) {
         case 1: key_hist_kernel<1><<<(unsigned)blocks, 256, smem, s>>>(keys, n, pt, hist); break;

@@ -234,7 +234,7 @@ __global__ void __launch_bounds__(256) backward_kernel(IndexView ix, const u64 *
 static unsigned grid_q(u64 n) {
     u64 b = (n + 255) / 256;
     if (b == 0) b = 1;
-    const u64 cap = (u64)kNumSMs * 32;
+    const u64 cap = (u64)num_sms() * 32;
     return (unsigned)(b < cap ? b : cap);
 }
 
