@@ -96,15 +96,16 @@ __device__ __forceinline__ void s_red_add(u32 addr, u32 v) {
 // places, NB = 1024 bins. Counts are 16-bit halves of u32 words (a segment has at most window + chunk < 65,536 records).
 // The records of a segment are dealt to the warps in groups of U full rows (no lane is ever idle there, so the group
 // code has no predicates); the rows that do not fill a group and the partial last row go one by one.
-template <int WARPS, int MINB, int U, int TSMAX, int MAXSOLID>
+template <int WARPS, int MINB, int U, int TSMAX, int MAXSOLID, int CB>
 __global__ void __launch_bounds__(WARPS * 32, MINB)
 hash_count_kernel(HashCountArgs a) {
+    static_assert(CB == 2 || CB == 4, "counts are 16-bit halves of u32 words or u32 words");
     constexpr int THREADS = WARPS * 32;
     extern __shared__ __align__(16) unsigned char smem_raw[];
     u64 *t_key = reinterpret_cast<u64 *>(smem_raw);                             // u64[TSMAX]
-    u32 *t_cnt = reinterpret_cast<u32 *>(smem_raw + (size_t)TSMAX * 8);         // u16[TSMAX] as u32 pairs
-    u64 *l_key = reinterpret_cast<u64 *>(smem_raw + (size_t)TSMAX * 10);        // u64[MAXSOLID]
-    u32 *l_cnt = reinterpret_cast<u32 *>(smem_raw + (size_t)TSMAX * 10 + (size_t)MAXSOLID * 8);
+    u32 *t_cnt = reinterpret_cast<u32 *>(smem_raw + (size_t)TSMAX * 8);         // CB = 2: u16[TSMAX] as u32 pairs; CB = 4: u32[TSMAX]
+    u64 *l_key = reinterpret_cast<u64 *>(smem_raw + (size_t)TSMAX * (8 + CB));  // u64[MAXSOLID]
+    u32 *l_cnt = reinterpret_cast<u32 *>(smem_raw + (size_t)TSMAX * (8 + CB) + (size_t)MAXSOLID * 8);
     __shared__ u32 s_ones, s_full, s_nsolid, s_distinct;
     __shared__ u64 s_sum, s_look[2][3], s_krange[2];
     __shared__ u32 s_w[WARPS];
@@ -146,7 +147,7 @@ hash_count_kernel(HashCountArgs a) {
             uint4 *k4 = reinterpret_cast<uint4 *>(t_key), *c4 = reinterpret_cast<uint4 *>(t_cnt);
             const uint4 ones = make_uint4(~0u, ~0u, ~0u, ~0u), zero = make_uint4(0u, 0u, 0u, 0u);
             for (u32 i = tid; i < TS / 2; i += THREADS) k4[i] = ones;
-            for (u32 i = tid; i < TS / 8; i += THREADS) c4[i] = zero;
+            for (u32 i = tid; i < TS * CB / 16; i += THREADS) c4[i] = zero;
         }
         u64 la_seg = 0, la_s = 0, la_e = 0;              // (thread 0) the segment of the iteration after the next one
         u64 kf = 0, kl = 0;                              // (thread 32) first and last record of this segment
@@ -160,8 +161,11 @@ hash_count_kernel(HashCountArgs a) {
         // ---- 1: insert ---------------------------------------------------------------------------------------------------
         u32 created = 0;
         const bool last_seg = e == a.n;
-        // count of the slot at byte offset a8 of the key table: 16-bit halves, two slots per word
-        auto cnt_add = [&](u32 a8) { s_red_add<TSMAX * 8>(tkey_s + ((a8 >> 2) & ~3u), (a8 & 8u) ? 0x10000u : 1u); };
+        // count of the slot at byte offset a8 of the key table (CB = 2: 16-bit halves, two slots per word)
+        auto cnt_add = [&](u32 a8) {
+            if constexpr (CB == 2) s_red_add<TSMAX * 8>(tkey_s + ((a8 >> 2) & ~3u), (a8 & 8u) ? 0x10000u : 1u);
+            else s_red_add<TSMAX * 8>(tkey_s + (a8 >> 1), 1u);
+        };
         // NR rows held by the warp: first the home slot of every record (one CAS that installs the key or returns what
         // is there, no loop), then ONE probing loop for the records whose home slot holds another key
         auto insert_rows = [&](auto nr_tag, const u64 *k, bool valid) {
@@ -223,12 +227,12 @@ hash_count_kernel(HashCountArgs a) {
                 else insert_rows(std::integral_constant<int, 1>{}, &key, valid);
             }
         }
+        // the first records of my next segment are on their way while this one is finished (its bounds came an iteration ago)
+        const u64 next = s_look[(it + 1) & 1][0], ns_ = s_look[(it + 1) & 1][1], ne_ = s_look[(it + 1) & 1][2];
+        if (next < nseg && warp < groups_of(ns_, ne_)) load_group(cur, a.keys + ns_ + (u64)warp * (32 * U));
         if (created) atomicAdd(&s_distinct, created);
         if (tid == 32 % THREADS) { s_krange[0] = kf >> a.top_shift; s_krange[1] = kl >> a.top_shift; }
         __syncthreads();
-        // the first records of my next segment are on their way while this one is finished
-        const u64 next = s_look[(it + 1) & 1][0], ns_ = s_look[(it + 1) & 1][1], ne_ = s_look[(it + 1) & 1][2];
-        if (next < nseg && warp < groups_of(ns_, ne_)) load_group(cur, a.keys + ns_ + (u64)warp * (32 * U));
         if (tid == 0) bounds_of(la_seg, la_s, la_e);     // stored at the end of the iteration
         const u64 kfirst = s_krange[0], klast = s_krange[1];
         const bool full = s_full != 0;
@@ -236,26 +240,31 @@ hash_count_kernel(HashCountArgs a) {
 
         // ---- 2: the solid slots, compacted to this iteration's list ------------------------------------------------------------
         u64 sum = 0;
-        if (!full && m) {   // the live part of the table, 16 bytes of counts (8 slots) per load; most vectors hold no solid edge
+        if (!full && m) {   // the live part of the table, 16 bytes of counts (8 or 4 slots) per load; most vectors hold no solid edge
             const uint4 *c4 = reinterpret_cast<const uint4 *>(t_cnt);
             const u32 d = a.d;
-            for (u32 v = tid; v < TS / 8; v += THREADS) {
+            constexpr u32 SPV = 16 / CB;                 // slots per vector
+            for (u32 v = tid; v < TS / SPV; v += THREADS) {
                 const uint4 w = c4[v];
-                if (d == 2 && ((w.x | w.y | w.z | w.w) & 0xfffefffeu) == 0) continue;   // no count above 1
+                if (d == 2 && ((w.x | w.y | w.z | w.w) & (CB == 2 ? 0xfffefffeu : 0xfffffffeu)) == 0) continue;   // no count above 1
                 const u32 wd[4] = {w.x, w.y, w.z, w.w};
-                u32 m8 = 0;                              // bit q: slot 8 v + q holds a solid edge
+                u32 mq = 0;                              // bit q: slot SPV v + q holds a solid edge
 #pragma unroll
-                for (u32 q = 0; q < 4; ++q) m8 |= ((wd[q] & 0xffffu) >= d ? 1u : 0u) << (2 * q) | ((wd[q] >> 16) >= d ? 2u : 0u) << (2 * q);
-                while (m8) {
-                    const u32 q = (u32)__ffs(m8) - 1u;
-                    m8 &= m8 - 1u;
+                for (u32 q = 0; q < 4; ++q) {
+                    if constexpr (CB == 2) mq |= ((wd[q] & 0xffffu) >= d ? 1u : 0u) << (2 * q) | ((wd[q] >> 16) >= d ? 2u : 0u) << (2 * q);
+                    else mq |= (wd[q] >= d ? 1u : 0u) << q;
+                }
+                while (mq) {
+                    const u32 q = (u32)__ffs(mq) - 1u;
+                    mq &= mq - 1u;
+                    const u32 wi = CB == 2 ? q >> 1 : q;
                     u32 wq = wd[0];
-                    if ((q >> 1) == 1) wq = wd[1];
-                    if ((q >> 1) == 2) wq = wd[2];
-                    if ((q >> 1) == 3) wq = wd[3];
-                    const u32 c = (wq >> ((q & 1u) * 16u)) & 0xffffu;
+                    if (wi == 1) wq = wd[1];
+                    if (wi == 2) wq = wd[2];
+                    if (wi == 3) wq = wd[3];
+                    const u32 c = CB == 2 ? (wq >> ((q & 1u) * 16u)) & 0xffffu : wq;
                     const u32 p = atomicAdd(&s_nsolid, 1u);
-                    if (p < (u32)MAXSOLID) { l_key[p] = t_key[v * 8 + q]; l_cnt[p] = c; }
+                    if (p < (u32)MAXSOLID) { l_key[p] = t_key[v * SPV + q]; l_cnt[p] = c; }
                     sum += c;
                 }
             }
@@ -288,7 +297,7 @@ hash_count_kernel(HashCountArgs a) {
         //          entries, which the owner of the bin puts in order by insertion. The table is dead: bins and the ordered
         //          entries live in its place. ---------------------------------------------------------------------------------------
         constexpr int NB = 1024, Q = NB / THREADS, QE = MAXSOLID / THREADS;   // bins per thread; list entries per thread
-        static_assert(NB % THREADS == 0 && MAXSOLID % THREADS == 0 && (size_t)NB * 4 <= (size_t)TSMAX * 2 && (size_t)MAXSOLID * 12 <= (size_t)TSMAX * 8, "layout");
+        static_assert(NB % THREADS == 0 && MAXSOLID % THREADS == 0 && (size_t)NB * 4 <= (size_t)TSMAX * CB && (size_t)MAXSOLID * 12 <= (size_t)TSMAX * 8, "layout");
         if (ns) {
             u32 *bins = t_cnt;
             u64 *o_key = t_key;
@@ -420,27 +429,33 @@ __global__ void __launch_bounds__(256) hash_copy_kernel(HashCountArgs a) {
 }
 
 // shapes: long buckets (chunk 4,096: one or two buckets per segment) and short ones (chunk 2,048: many buckets per segment)
-template <int WARPS, int MINB, int U, int TSMAX, int MAXSOLID>
+template <int WARPS, int MINB, int U, int TSMAX, int MAXSOLID, int CB>
 struct HashShape {
     static constexpr int THREADS = WARPS * 32;
-    static constexpr size_t kSmem = (size_t)TSMAX * 10 + (size_t)MAXSOLID * 12;
+    static constexpr size_t kSmem = (size_t)TSMAX * (8 + CB) + (size_t)MAXSOLID * 12;
     static int setup(int *blocks_per_sm) {
-        int e = (int)cudaFuncSetAttribute(hash_count_kernel<WARPS, MINB, U, TSMAX, MAXSOLID>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmem);
+        int e = (int)cudaFuncSetAttribute(hash_count_kernel<WARPS, MINB, U, TSMAX, MAXSOLID, CB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmem);
         if (e) return e;
-        return (int)cudaOccupancyMaxActiveBlocksPerMultiprocessor(blocks_per_sm, hash_count_kernel<WARPS, MINB, U, TSMAX, MAXSOLID>, THREADS, kSmem);
+        return (int)cudaOccupancyMaxActiveBlocksPerMultiprocessor(blocks_per_sm, hash_count_kernel<WARPS, MINB, U, TSMAX, MAXSOLID, CB>, THREADS, kSmem);
     }
     static int launch(const HashCountArgs &a, int blocks_per_sm, cudaStream_t s) {
         u64 g = (u64)num_sms() * (u64)(blocks_per_sm > 0 ? blocks_per_sm : 1);
         if (g > a.nseg) g = a.nseg;
-        hash_count_kernel<WARPS, MINB, U, TSMAX, MAXSOLID><<<(unsigned)g, THREADS, kSmem, s>>>(a);
+        hash_count_kernel<WARPS, MINB, U, TSMAX, MAXSOLID, CB><<<(unsigned)g, THREADS, kSmem, s>>>(a);
         return (int)cudaGetLastError();
     }
 };
+#ifndef SDBG_HASH_BIG_TS
+#define SDBG_HASH_BIG_TS 8192
+#endif
+#ifndef SDBG_HASH_BIG_CB
+#define SDBG_HASH_BIG_CB 4
+#endif
 #ifndef SDBG_HASH_BIG
-#define SDBG_HASH_BIG 16, 2, 4, 8192, 1024
+#define SDBG_HASH_BIG 16, 2, 4, SDBG_HASH_BIG_TS, 1024, SDBG_HASH_BIG_CB
 #endif
 #ifndef SDBG_HASH_SMALL
-#define SDBG_HASH_SMALL 8, 4, 4, 4096, 1024
+#define SDBG_HASH_SMALL 8, 4, 4, 4096, 1024, 2
 #endif
 using HashBig = HashShape<SDBG_HASH_BIG>;
 using HashSmall = HashShape<SDBG_HASH_SMALL>;
