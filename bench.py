@@ -39,16 +39,16 @@ def _peaks():
     return 6650.0, "fallback (B200_PROFILING.md)"
 
 
-def _traffic(workload_name):
-    """DRAM bytes (read + write) per launch of the dominant kernel, from the committed ncu --set full capture of this
-    workload (profiles/*_traffic.csv, newest round last), or None."""
+def _traffic(workload_name, kernel_class):
+    """DRAM bytes (read + write) per launch of a kernel class, from the committed ncu --set full capture of this
+    workload (profiles/*_traffic.csv, newest round last; columns workload, kernel_class, dram_bytes_per_launch), or None."""
     import csv
     import glob
     val = None
     for p in sorted(glob.glob(os.path.join(ROOT, "profiles", "*_traffic.csv"))):
         try:
             for row in csv.DictReader(open(p)):
-                if row.get("workload") == workload_name:
+                if row.get("workload") == workload_name and row.get("kernel_class", "radix") == kernel_class:
                     val = int(row["dram_bytes_per_launch"])
         except Exception:
             pass
@@ -56,15 +56,45 @@ def _traffic(workload_name):
 
 
 class ClockSampler(threading.Thread):
-    """Samples nvidia-smi clocks / throttle reasons while the timed region runs."""
+    """Samples SM clocks / throttle reasons while the timed region runs: NVML every 5 ms when the module is there,
+    otherwise nvidia-smi (one process per sample, ~10 per second)."""
     Q = ("clocks.sm,clocks.max.sm,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
          "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+    NAMES = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
 
     def __init__(self, gpu_index):
         super().__init__(daemon=True)
-        self.gpu, self.stop_flag, self.rows = gpu_index, threading.Event(), []
+        self.gpu, self.stop_flag, self.rows, self.source = gpu_index, threading.Event(), [], "nvidia-smi"
+        self.mark0 = self.mark1 = None                   # sample counts at the start / end of the timed region
+
+    def _nvml_loop(self):
+        import pynvml as nv
+        nv.nvmlInit()
+        vis = os.environ.get("CUDA_VISIBLE_DEVICES", "")
+        idx = self.gpu
+        if vis and all(x.strip().isdigit() for x in vis.split(",")):
+            idx = int(vis.split(",")[self.gpu])
+        h = nv.nvmlDeviceGetHandleByIndex(idx)
+        mx = float(nv.nvmlDeviceGetMaxClockInfo(h, nv.NVML_CLOCK_SM))
+        bits = [getattr(nv, n) for n in ("nvmlClocksEventReasonHwSlowdown", "nvmlClocksEventReasonHwThermalSlowdown",
+                                         "nvmlClocksEventReasonSwThermalSlowdown", "nvmlClocksEventReasonSwPowerCap")] \
+            if hasattr(nv, "nvmlClocksEventReasonHwSlowdown") else \
+            [nv.nvmlClocksThrottleReasonHwSlowdown, nv.nvmlClocksThrottleReasonHwThermalSlowdown,
+             nv.nvmlClocksThrottleReasonSwThermalSlowdown, nv.nvmlClocksThrottleReasonSwPowerCap]
+        get_reasons = getattr(nv, "nvmlDeviceGetCurrentClocksEventReasons", None) or nv.nvmlDeviceGetCurrentClocksThrottleReasons
+        self.source = "nvml"
+        while not self.stop_flag.is_set():
+            r = get_reasons(h)
+            self.rows.append([str(float(nv.nvmlDeviceGetClockInfo(h, nv.NVML_CLOCK_SM))), str(mx)] +
+                             ["Active" if r & b else "Not Active" for b in bits])
+            self.stop_flag.wait(0.005)
 
     def run(self):
+        try:
+            self._nvml_loop()
+            return
+        except Exception:
+            self.source = "nvidia-smi"
         while not self.stop_flag.is_set():
             try:
                 out = subprocess.run(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits", "-i", str(self.gpu)],
@@ -75,15 +105,23 @@ class ClockSampler(threading.Thread):
                 pass
             self.stop_flag.wait(0.1)
 
+    def mark(self, which):
+        if which == 0:
+            self.mark0 = len(self.rows)
+        else:
+            self.mark1 = len(self.rows)
+
     def summary(self):
         self.stop_flag.set()
         self.join(timeout=6)
-        sm = sorted(float(r[0]) for r in self.rows if r and r[0].replace(".", "").isdigit())
-        mx = [float(r[1]) for r in self.rows if len(r) > 1 and r[1].replace(".", "").isdigit()]
-        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
-        reasons = sorted({n for r in self.rows if len(r) >= 6 for n, v in zip(names, r[2:6]) if v.lower().startswith("active")})
+        rows = self.rows
+        if self.mark0 is not None and self.mark1 is not None and self.mark1 - self.mark0 >= 3:
+            rows = rows[self.mark0:self.mark1]           # the timed region only (else everything seen, warm-up included)
+        sm = sorted(float(r[0]) for r in rows if r and r[0].replace(".", "").isdigit())
+        mx = [float(r[1]) for r in rows if len(r) > 1 and r[1].replace(".", "").isdigit()]
+        reasons = sorted({n for r in rows if len(r) >= 6 for n, v in zip(self.NAMES, r[2:6]) if v.lower().startswith("active")})
         return {"sm_mhz": sm[len(sm) // 2] if sm else None, "sm_max_mhz": max(mx) if mx else None,
-                "reasons": reasons, "samples": len(self.rows)}
+                "reasons": reasons, "samples": len(rows), "source": self.source}
 
 
 def run_reference(args, w):
@@ -144,11 +182,133 @@ def whole_job_value(records_per_rank: int, world: int, steps: int, ms_max: float
     return world * records_per_rank * steps / (ms_max * 1e-3)
 
 
+NOMINAL_HBM_GBS = 8000.0    # the denominator BASELINE.json:north_star names ("~8 TB/s HBM3e peak")
+
+KERNEL_OF_CLASS = {
+    "pack": "pack_kernel + mark_ends_kernel",
+    "extract": "extract_kernel",
+    "radix": "onesweep_kernel (one LSD radix pass over all records)",
+    "table": "hash_count_kernel (table count of the top-sorted records)",
+    "count": "count step helpers (hash_bounds/scan/copy kernels, or the sweeps of count.cu)",
+    "emit": "emit_kernel",
+    "other": "memsets, histogram scan, gathers",
+}
+
+
+def full_lsd_model_bytes_per_record(k: int) -> int:
+    """K (2P + 2) bytes per raw record for a full LSD sort with 8-bit digits (144 at k = 31)."""
+    bits = 2 * (k + 1)
+    K = 8 * ((bits + 63) // 64)
+    P = sum(-(-min(64, bits - 64 * q) // 8) for q in range((bits + 63) // 64))
+    return K * (2 * P + 2)
+
+
+def roofline_blocks(tim, steps, ms_per_step, peak, peak_src, wl_name, k, value):
+    """`roofline` for the kernel class with the largest share of the step, the same figures for the other classes, the
+    whole step on the bytes the library accounted, and records/s against the full-LSD byte model."""
+    per = {}
+    for c in tim.ms:
+        n, ms, by = tim.launches[c], tim.ms[c], tim.bytes[c]
+        if n == 0 or ms <= 0:
+            continue
+        ach = by / (ms * 1e-3) / 1e9
+        per[c] = {"kernel": KERNEL_OF_CLASS.get(c, c), "bound": "hbm", "achieved": ach, "peak": peak, "unit": "GB/s",
+                  "frac": ach / peak, "frac_of_measured": ach / peak, "frac_of_nominal_8TBps": ach / NOMINAL_HBM_GBS,
+                  "traffic": _traffic(wl_name, c), "peak_source": peak_src, "launches": int(n),
+                  "avg_launch_ms": ms / n, "algorithmic_bytes_per_launch": by // n,
+                  "ms_per_step": ms / steps, "share_of_step": ms / steps / ms_per_step}
+    top = max(per, key=lambda c: per[c]["ms_per_step"])
+    step_bytes = sum(tim.bytes.values()) / steps
+    step_ach = step_bytes / (ms_per_step * 1e-3) / 1e9
+    model = full_lsd_model_bytes_per_record(k)
+    out = {
+        "roofline": dict(per[top], kernel_class=top),
+        "roofline_other_kernels": {c: v for c, v in per.items() if c != top},
+        "roofline_step": {"bound": "hbm", "achieved": step_ach, "peak": peak, "unit": "GB/s", "frac": step_ach / peak,
+                          "frac_of_nominal_8TBps": step_ach / NOMINAL_HBM_GBS,
+                          "algorithmic_bytes_per_step": int(step_bytes), "bytes_per_record": None,
+                          "note": "bytes the library accounted for every kernel of the step / device time of the step"},
+        "records_per_s_vs_full_lsd_model": {
+            "model_bytes_per_record": model, "model_records_per_s_at_measured_peak": peak * 1e9 / model,
+            "ratio": value / (peak * 1e9 / model),
+            "note": "SURVEY.md 8(d): a full LSD sort moves K(2P+2) bytes per record; this path moves fewer (top passes + table count)"},
+    }
+    return out
+
+
+def device_steps(sd, torch, wl, args, steps, warmup, rank, world, local, barrier, sampler=None):
+    """`steps` timed steps of the whole hot path with the ASCII reads resident in HBM. Returns (ms_total, timing, S,
+    device tensors for the end-to-end leg)."""
+    from workloads import ReadGenerator
+    gen = ReadGenerator(wl)
+    bases_d, offs_d = gen.device()
+    torch.cuda.synchronize()
+    n_reads, N = wl.n_reads, wl.n_raw_edges
+    ctx = sd.Context(sd.sdbg_workspace_for_records(N, wl.k))
+    reads = sd.Reads(wl.n_bases)
+    edges = sd.Edges(N // wl.d, wl.k)
+    graph = sd.Graph(N // wl.d)
+
+    def step():
+        reads.c.n_reads = reads.c.n_bases = reads.c.n_slots = 0
+        sd.sdbg_pack_reads(ctx, bases_d, offs_d, n_reads, reads)
+        if args.shard:     # SURVEY.md 8(e)(i): replicated reads, each rank counts its range of l=8 partitions
+            from paper_1409_7208_b200.shard import count_edges_sharded, gather_counts
+            n_local, _ = count_edges_sharded(ctx, reads, n_reads, wl.k, wl.d, edges, rank, world)
+            sd.sdbg_build(ctx, edges, sd.SDBG_SORTED, graph)
+            gather_counts(n_local, device="cuda")        # offsets of the concatenation: the only exchange
+            return edges.n
+        sd.sdbg_count_edges(ctx, reads, n_reads, wl.k, wl.d, edges, None)
+        sd.sdbg_build(ctx, edges, sd.SDBG_SORTED, graph)
+        return edges.n
+
+    S = 0
+    for _ in range(max(warmup, 3)):
+        S = step()
+    ctx.get_timing()
+    ctx.set_timing(True)
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    if sampler is not None:
+        sampler.mark(0)
+    ev0.record()
+    for _ in range(steps):
+        step()
+    ev1.record()
+    barrier()
+    if sampler is not None:
+        sampler.mark(1)
+    ms_total = ev0.elapsed_time(ev1)
+    tim = ctx.get_timing()
+    ctx.set_timing(False)
+    ctx.close(); ctx.workspace = None
+    del reads, edges, graph
+    torch.cuda.empty_cache()
+    return ms_total, tim, S, bases_d, offs_d
+
+
+def pcie_rates(torch, nbytes=256 << 20):
+    """Measured host<->device copy rates of this box (pinned memory, one direction at a time), GB/s."""
+    h = torch.empty(nbytes, dtype=torch.uint8, pin_memory=True)
+    d = torch.empty(nbytes, dtype=torch.uint8, device="cuda")
+    out = []
+    for src, dst in ((h, d), (d, h)):
+        dst.copy_(src, non_blocking=True)
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        for _ in range(3):
+            dst.copy_(src, non_blocking=True)
+        e1.record()
+        torch.cuda.synchronize()
+        out.append(3 * nbytes / (e0.elapsed_time(e1) * 1e-3) / 1e9)
+    return out
+
+
 def run_gpu(args, w):
     import torch
     import torch.distributed as dist
     import paper_1409_7208_b200 as sd
-    from workloads import ReadGenerator
 
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
@@ -160,30 +320,9 @@ def run_gpu(args, w):
     # ---- inputs resident in HBM: every rank an independent replica (own seed) ------------------------------
     from dataclasses import replace
     wl = replace(w, seed=rank_seed(w.seed, rank)) if (rank and not args.shard) else w   # --shard: the same reads on every rank
-    gen = ReadGenerator(wl)
-    bases_d, offs_d = gen.device()
-    torch.cuda.synchronize()
     n_bases, n_reads = wl.n_bases, wl.n_reads
     N = wl.n_raw_edges
     K = 8 * wl.words_per_key
-
-    ctx = sd.Context(sd.sdbg_workspace_for_records(N, wl.k))
-    reads = sd.Reads(n_bases)
-    edges = sd.Edges(N // wl.d, wl.k)
-    graph = sd.Graph(N // wl.d)
-
-    def step(src_b, src_o):
-        reads.c.n_reads = reads.c.n_bases = reads.c.n_slots = 0
-        sd.sdbg_pack_reads(ctx, src_b, src_o, n_reads, reads)
-        if args.shard:     # replicated reads, each rank counts its range of l=8 partitions
-            from paper_1409_7208_b200.shard import count_edges_sharded, gather_counts
-            n_local, _ = count_edges_sharded(ctx, reads, n_reads, wl.k, wl.d, edges, rank, world)
-            sd.sdbg_build(ctx, edges, sd.SDBG_SORTED, graph)
-            gather_counts(n_local, device="cuda")        # offsets of the concatenation: the only exchange
-            return edges.n
-        sd.sdbg_count_edges(ctx, reads, n_reads, wl.k, wl.d, edges, None)
-        sd.sdbg_build(ctx, edges, sd.SDBG_SORTED, graph)
-        return edges.n
 
     def barrier():
         torch.cuda.synchronize()
@@ -191,40 +330,26 @@ def run_gpu(args, w):
             dist.barrier()
         torch.cuda.synchronize()
 
-    for _ in range(max(args.warmup, 3)):
-        S = step(bases_d, offs_d)
-    ctx.get_timing()
-    ctx.set_timing(True)
     sampler = ClockSampler(local)
     sampler.start()
-    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    barrier()
-    ev0.record()
-    for _ in range(args.steps):
-        step(bases_d, offs_d)
-    ev1.record()
-    barrier()
-    ms_total = ev0.elapsed_time(ev1)
-    tim = ctx.get_timing()
+    ms_total, tim, S, bases_d, offs_d = device_steps(sd, torch, wl, args, args.steps, args.warmup, rank, world, local, barrier, sampler)
     clocks = sampler.summary()
-    ctx.set_timing(False)
 
     # ---- end to end: HOST pinned buffers in, SdBG arrays out, copies inside the timed region ---------------------
     # Every step copies its reads from pinned host memory, runs the whole path and copies the SdBG arrays back; the
-    # step is over when its results are on the host. `--e2e-pipelines P` (default 2) runs P such step loops at once,
+    # step is over when its results are on the host. `--e2e-pipelines P` (default 3) runs P such step loops at once,
     # each with its own context, stream, workspace and output buffers, fed by one host thread each, so that the copies
     # of one step overlap the kernels of another (PCIe is full duplex and idle while a step sorts).
     ms_e2e, e2e_steps, n_pipes = float("nan"), 0, 0
+    h2d_gbs = d2h_gbs = None
     if not args.no_e2e and not args.shard:
         ws_bytes = sd.sdbg_workspace_for_records(N, wl.k)
-        ctx.close(); ctx.workspace = None
-        del reads, edges, graph
-        torch.cuda.empty_cache()
         bases_h = torch.empty(n_bases, dtype=torch.uint8, pin_memory=True)
         offs_h = torch.empty(n_reads + 1, dtype=torch.int64, pin_memory=True)
         bases_h.copy_(bases_d); offs_h.copy_(offs_d)
         del bases_d, offs_d
         torch.cuda.empty_cache()
+        h2d_gbs, d2h_gbs = pcie_rates(torch)
         free_b = torch.cuda.mem_get_info()[0]
         per_pipe = ws_bytes + n_bases // 2 + S * (K + 4 + 5 + 1) + (64 << 20)
         n_pipes = max(1, min(args.e2e_pipelines, int(free_b * 0.9 // per_pipe)))
@@ -236,6 +361,7 @@ def run_gpu(args, w):
         for _ in range(n_pipes):
             pp = Pipe()
             pp.stream = torch.cuda.Stream()
+            pp.copy_stream = torch.cuda.Stream()
             with torch.cuda.stream(pp.stream):
                 pp.ctx = sd.Context(ws_bytes)
                 pp.reads = sd.Reads(n_bases)
@@ -245,11 +371,14 @@ def run_gpu(args, w):
             pp.out_last = torch.empty((S + 63) // 64, dtype=torch.int64, pin_memory=True)
             pp.out_mult = torch.empty(S, dtype=torch.int32, pin_memory=True)
             pp.out_keys = torch.empty(S * wl.words_per_key, dtype=torch.int64, pin_memory=True)
+            pp.gpu_done = torch.cuda.Event()
             pp.done = torch.cuda.Event()
             pipes.append(pp)
 
         # one loop at a time in each phase: identical loops started together would otherwise stay in lockstep and share
-        # the link and the SMs phase by phase; with the locks one loop sorts while another copies
+        # the link and the SMs phase by phase; with the locks one loop sorts while another copies. The device-to-host
+        # copy of a step runs on the pipe's copy stream behind an event, so the host thread never waits for the kernels
+        # of its own step before it queues the copy, and the GPU lock is free as soon as the last kernel is queued.
         lock_in, lock_gpu, lock_out = threading.Lock(), threading.Lock(), threading.Lock()
 
         def e2e_loop(pp, n_steps, start_event):
@@ -261,17 +390,20 @@ def run_gpu(args, w):
                     pp.reads.c.n_reads = pp.reads.c.n_bases = pp.reads.c.n_slots = 0
                     with lock_in:                        # host -> device copy of the reads (+ the pack kernel)
                         sd.sdbg_pack_reads(pp.ctx, bases_h, offs_h, n_reads, pp.reads)
-                    with lock_gpu:                       # extract, sort, count, emit
+                    with lock_gpu:                       # extract, sort, count (returns with the count), emit
                         sd.sdbg_count_edges(pp.ctx, pp.reads, n_reads, wl.k, wl.d, pp.edges, None)
                         sd.sdbg_build(pp.ctx, pp.edges, sd.SDBG_SORTED, pp.graph)
-                        pp.stream.synchronize()
+                        pp.gpu_done.record(pp.stream)
                     s_ = pp.edges.n
                     with lock_out:                       # device -> host copy of the SdBG arrays
-                        pp.out_W.copy_(pp.graph.W[:s_], non_blocking=True)
-                        pp.out_last.copy_(pp.graph.last_bits[:(s_ + 63) // 64], non_blocking=True)
-                        pp.out_mult.copy_(pp.graph.mult[:s_], non_blocking=True)
-                        pp.out_keys.copy_(pp.edges.keys[:s_ * wl.words_per_key], non_blocking=True)
-                        pp.stream.synchronize()          # the step's results are on the host
+                        pp.copy_stream.wait_event(pp.gpu_done)
+                        with torch.cuda.stream(pp.copy_stream):
+                            pp.out_W.copy_(pp.graph.W[:s_], non_blocking=True)
+                            pp.out_last.copy_(pp.graph.last_bits[:(s_ + 63) // 64], non_blocking=True)
+                            pp.out_mult.copy_(pp.graph.mult[:s_], non_blocking=True)
+                            pp.out_keys.copy_(pp.edges.keys[:s_ * wl.words_per_key], non_blocking=True)
+                        pp.copy_stream.synchronize()     # the step's results are on the host
+                    pp.stream.wait_stream(pp.copy_stream)
                 pp.done.record(pp.stream)
 
         def run_all(n_steps, start_event):
@@ -295,8 +427,31 @@ def run_gpu(args, w):
         ms_e2e = e0.elapsed_time(e1) * args.steps / e2e_steps     # scaled to args.steps steps, as the other timings
         for pp in pipes:
             assert pp.edges.n == S
+            pp.ctx.close(); pp.ctx.workspace = None
+        del pipes, bases_h, offs_h
+        torch.cuda.empty_cache()
+    else:
+        del bases_d, offs_d
+        torch.cuda.empty_cache()
     h2d = n_bases + 8 * (n_reads + 1)
     d2h = S * (1 + 4 + K) + 8 * ((S + 63) // 64)
+
+    # ---- the second headline config of SURVEY.md 8(d) (config 3: mock metagenome, k = 31) in the same process ------------
+    also = {}
+    if world == 1 and not args.shard and not args.no_also and args.config == 2:
+        from workloads import get_config
+        w3 = get_config(3)
+        ms3, tim3, S3, b3, o3 = device_steps(sd, torch, w3, args, args.also_steps, 3, 0, 1, local, barrier, None)
+        del b3, o3
+        torch.cuda.empty_cache()
+        peak3, src3 = _peaks()
+        v3 = w3.n_raw_edges * args.also_steps / (ms3 * 1e-3)
+        blk = {"ms_per_step": ms3 / args.also_steps, "value": v3, "unit": UNIT, "steps": args.also_steps, "warmup": 3,
+               "raw_edges": w3.n_raw_edges, "solid_edges": int(S3), "k": w3.k, "d": w3.d,
+               "kernel_ms_per_step": {c: tim3.ms[c] / args.also_steps for c in tim3.ms},
+               "kernel_launches_per_step": {c: tim3.launches[c] / args.also_steps for c in tim3.launches}}
+        blk.update(roofline_blocks(tim3, args.also_steps, ms3 / args.also_steps, peak3, src3, w3.name, w3.k, v3))
+        also[w3.name] = blk
 
     ms_total, ms_e2e = max_over_ranks([ms_total, ms_e2e], device="cuda")
     if rank != 0:
@@ -305,14 +460,9 @@ def run_gpu(args, w):
         return
 
     peak, peak_src = _peaks()
-    radix_launches = tim.launches["radix"]
-    radix_ms = tim.ms["radix"] / max(radix_launches, 1)
-    # algorithmic bytes of one pass as the library accounts them: one-word keys are read and
-    # written once (2 N K); multi-word keys travel as (key word, u32 index) pairs (2 N 12)
-    algo_bytes = tim.bytes["radix"] // max(radix_launches, 1)
-    achieved = algo_bytes / (radix_ms * 1e-3) / 1e9 if radix_ms > 0 else 0.0
+    value = whole_job_value(N, 1 if args.shard else world, args.steps, ms_total)
     line = {
-        "metric": METRIC, "value": whole_job_value(N, 1 if args.shard else world, args.steps, ms_total), "unit": UNIT, "n_gpus": world,
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world,
         "steps": args.steps, "warmup": max(args.warmup, 3), "ms_per_step": ms_total / args.steps,
         "higher_is_better": True, "scaling": "strong" if args.shard else "weak", "vs_baseline": None, "dtype": "u64", "data": "synthetic",
         "config": {"workload": wl.name, "k": wl.k, "d": wl.d, "reads": n_reads, "read_len": wl.read_len, "bases": n_bases,
@@ -322,22 +472,15 @@ def run_gpu(args, w):
         "clocks": clocks,
         "e2e": {"value": whole_job_value(N, world, args.steps, ms_e2e), "unit": UNIT, "h2d_bytes_per_step": h2d,
                 "d2h_bytes_per_step": d2h, "ms_per_step": ms_e2e / args.steps, "pipelines": n_pipes,
-                "steps_timed": e2e_steps},
+                "steps_timed": e2e_steps, "h2d_gbs_measured": h2d_gbs, "d2h_gbs_measured": d2h_gbs,
+                "pcie_lower_bound_ms": (max(h2d / (h2d_gbs * 1e9), d2h / (d2h_gbs * 1e9)) * 1e3) if h2d_gbs and d2h_gbs else None},
         "gpu_launches": int(tim.total_launches),
-        "roofline": {"kernel": "onesweep_kernel (one LSD radix pass)", "bound": "hbm", "achieved": achieved, "peak": peak,
-                     "unit": "GB/s", "frac": achieved / peak, "traffic": _traffic(wl.name), "peak_source": peak_src,
-                     "launches": int(radix_launches), "avg_launch_ms": radix_ms, "algorithmic_bytes_per_launch": algo_bytes},
-        # the count step beside it (hashcount.cu on the default path): its algorithmic bytes are one read of the records
-        # plus the solid edges staged and copied; it is bound by instruction issue, not by HBM (DESIGN.md section 6 a4')
-        "roofline_count": {"kernel": "count step (hash_count_kernel and helpers, or the sweeps of count.cu)", "bound": "hbm",
-                           "achieved": (tim.bytes["count"] / (tim.ms["count"] * 1e-3) / 1e9) if tim.ms["count"] > 0 else 0.0,
-                           "peak": peak, "unit": "GB/s",
-                           "frac": (tim.bytes["count"] / (tim.ms["count"] * 1e-3) / 1e9 / peak) if tim.ms["count"] > 0 else 0.0,
-                           "ms_per_step": tim.ms["count"] / args.steps, "algorithmic_bytes_per_step": tim.bytes["count"] // max(args.steps, 1),
-                           "note": "instruction-issue bound (profiles/r01_hash_count_full.md)"},
         "kernel_ms_per_step": {c: tim.ms[c] / args.steps for c in tim.ms},
         "kernel_launches_per_step": {c: tim.launches[c] / args.steps for c in tim.launches},
     }
+    line.update(roofline_blocks(tim, args.steps, ms_total / args.steps, peak, peak_src, wl.name, wl.k, value / (1 if args.shard else world)))
+    if also:
+        line["also"] = also
     if world == 1 and not args.no_cpu_baseline:
         line["cpu_baseline"] = cpu_baseline(wl, args.ref_reads)
     print(json.dumps(line), flush=True)
@@ -421,7 +564,9 @@ def main():
     ap.add_argument("--ref-reads", type=int, default=40000, help="reads in the oracle's bounded sample")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true", help="development runs: skip the host-buffer end-to-end leg")
-    ap.add_argument("--e2e-pipelines", type=int, default=2, help="concurrent host-to-host step loops of the end-to-end leg")
+    ap.add_argument("--e2e-pipelines", type=int, default=3, help="concurrent host-to-host step loops of the end-to-end leg")
+    ap.add_argument("--no-also", action="store_true", help="skip the config-3 sub-record of the default run")
+    ap.add_argument("--also-steps", type=int, default=3, help="timed steps of the config-3 sub-record")
     ap.add_argument("--shard", action="store_true", help="strong scaling: every rank holds the same reads and counts its own range "
                     "of l=8 partitions (SURVEY.md §8(e)); default is independent replicas")
     ap.add_argument("--next", action="store_true", help="time the widened rows (sdbg_build_full, sdbg_mercy_edges) instead")

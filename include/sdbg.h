@@ -288,7 +288,10 @@ int sdbg_backward(sdbg_ctx *ctx, const sdbg_index *ix, const uint64_t *edge_idx,
 
 /* ---- measurement hooks ---------------------------------------------------------------------------------- */
 
-enum { SDBG_T_PACK = 0, SDBG_T_EXTRACT = 1, SDBG_T_RADIX = 2, SDBG_T_COUNT = 3, SDBG_T_EMIT = 4, SDBG_T_OTHER = 5, SDBG_T_NUM = 6 };
+/* kernel classes: RADIX = onesweep_kernel launches over all records of a range; TABLE = hash_count_kernel (the table
+ * count of the default path, one launch per range); COUNT = everything else of step a4 (segment bounds, block-sum scan and
+ * copy of the staged edges on the default path; the sweeps of count.cu otherwise) */
+enum { SDBG_T_PACK = 0, SDBG_T_EXTRACT = 1, SDBG_T_RADIX = 2, SDBG_T_COUNT = 3, SDBG_T_EMIT = 4, SDBG_T_OTHER = 5, SDBG_T_TABLE = 6, SDBG_T_NUM = 7 };
 
 typedef struct {
     double ms[SDBG_T_NUM];          /* device time per kernel class, CUDA events on the ctx stream */

@@ -19,7 +19,7 @@ SDBG_SORTED = 1
 SDBG_NUM_BUCKETS = 65536
 STATUS = {0: "SDBG_OK", -1: "SDBG_E_INVAL", -2: "SDBG_E_BADBASE", -3: "SDBG_E_CAPACITY", -4: "SDBG_E_WORKSPACE",
           -5: "SDBG_E_CUDA", -6: "SDBG_E_UNSUPPORTED"}
-T_CLASSES = ("pack", "extract", "radix", "count", "emit", "other")
+T_CLASSES = ("pack", "extract", "radix", "count", "emit", "other", "table")
 
 
 class SdbgError(RuntimeError):
@@ -63,7 +63,7 @@ class _Index(C.Structure):
 
 
 class _Timing(C.Structure):
-    _fields_ = [("ms", C.c_double * 6), ("launches", C.c_uint64 * 6), ("bytes", C.c_uint64 * 6)]
+    _fields_ = [("ms", C.c_double * 7), ("launches", C.c_uint64 * 7), ("bytes", C.c_uint64 * 7)]
 
 
 def lib_path() -> str:
