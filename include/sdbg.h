@@ -58,18 +58,25 @@ typedef struct sdbg_ctx sdbg_ctx;
 /* Binds a device, a CUDA stream (cudaStream_t passed as void*, NULL = legacy default stream) and a caller-owned
  * device workspace. The workspace plays the role of MEGAHIT's "-m" memory budget: the sorter
  * sizes its block-wise passes to it. workspace must be 256-byte aligned.
- * Test hook: with SDBG_FORCE_WIDE=1 in the environment when the context is created, one-word-key ranges of any size
- * take the code path of ranges of 2^32 records and more (wide look-back words in the radix passes, 64-bit run lengths
- * in the count sweeps), which otherwise only very large block-wise runs reach. Results are identical.
- * Path switches, read at the same moment, results identical as well: sdbg_count_edges has three ways through the sort and
- * count of one-word keys (PAPER.md:33-35 fix the result, not the way): by default the records are sorted by their most
- * significant key bytes only and counted bucket by bucket in shared-memory tables (d >= 2); SDBG_NO_HASH=1 takes the
- * partial-sort path instead (sort by the low bytes of mixed keys, count inside the buckets, sort only the kept
- * entries); SDBG_NO_PARTIAL=1 sorts every record through every pass and counts by one sweep. Whatever does not fit the
- * default path (an over-long bucket, a full table) is redone the plain way inside the same call.
- * SDBG_NO_UNSTABLE=1: the first radix pass of a sort (whose input order is arbitrary) uses the stable kernel too. */
+ * Errors: SDBG_E_INVAL (null or misaligned workspace), SDBG_E_WORKSPACE (below sdbg_min_workspace()), SDBG_E_CUDA (no such
+ * device, or the kernels could not be set up: the library has no CPU fallback). */
 int sdbg_ctx_create(sdbg_ctx **ctx, int device, void *cuda_stream, void *workspace, uint64_t workspace_bytes);
 void sdbg_ctx_destroy(sdbg_ctx *ctx);
+/* Options of a context (all off after sdbg_ctx_create). They choose among ways through the sort and count that give the
+ * SAME result bit for bit (PAPER.md:33-35 fix the result, not the way); the tests use them to reach every way at sizes
+ * the oracle can check, and to compare the ways with one another.
+ *   SDBG_OPT_FORCE_WIDE        one-word-key ranges of any size take the code path of ranges of 2^32 records and more (wide
+ *                              look-back words in the radix passes, 64-bit run lengths in the count sweeps)
+ *   SDBG_OPT_NO_TABLE_COUNT    sdbg_count_edges sorts every record through every radix pass and counts by one sweep
+ *                              (count.cu). Default for one-word keys and d >= 2: the records go through the most
+ *                              significant passes only and are counted bucket by bucket in shared-memory tables
+ *                              (hashcount.cu); whatever does not fit there (an over-long bucket, a full table) is redone
+ *                              the plain way inside the same call
+ *   SDBG_OPT_STABLE_FIRST_PASS the first radix pass of sdbg_count_edges' sorts uses the stable kernel like the others
+ *                              (default: unstable, equal keys are merged afterwards)
+ * Errors: SDBG_E_INVAL (null ctx, unknown option). */
+enum { SDBG_OPT_FORCE_WIDE = 1, SDBG_OPT_NO_TABLE_COUNT = 2, SDBG_OPT_STABLE_FIRST_PASS = 3 };
+int sdbg_ctx_set_option(sdbg_ctx *ctx, int option, int value);
 const char *sdbg_strerror(int status);           /* static string */
 const char *sdbg_last_error(const sdbg_ctx *ctx); /* detail of the last failure on this ctx ("" if none) */
 
@@ -298,6 +305,11 @@ typedef struct {
     uint64_t launches[SDBG_T_NUM];  /* kernel launches per class */
     uint64_t bytes[SDBG_T_NUM];     /* algorithmic bytes per class */
 } sdbg_timing;
+
+/* Launches, by this process so far, of the UNSTABLE variant of the radix pass (radix.cu FIRST: the order of equal digits is
+ * hardware-defined). Only the sorts of sdbg_count_edges may use it (they merge equal keys afterwards); sdbg_build,
+ * sdbg_build_full and sdbg_mercy_edges depend on stable passes, and the tests assert that they leave this counter alone. */
+uint64_t sdbg_unstable_radix_launches(void);
 
 /* on != 0: bracket every kernel class with CUDA events (a few microseconds each). Launch counters always run. */
 int sdbg_ctx_set_timing(sdbg_ctx *ctx, int on);

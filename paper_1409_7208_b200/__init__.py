@@ -7,5 +7,6 @@ from .binding import (  # noqa: F401
     sdbg_index_bytes, sdbg_index_build, sdbg_forward, sdbg_backward,
     sdbg_count_edges_range, sdbg_bucket_hist, sdbg_plan_shards,
     sdbg_key_words, sdbg_read_slots, sdbg_full_workspace, sdbg_workspace_for_records, sdbg_min_workspace, sdbg_strerror,
-    SDBG_SORTED, STATUS,
+    sdbg_unstable_radix_launches,
+    SDBG_SORTED, STATUS, SDBG_OPT_FORCE_WIDE, SDBG_OPT_NO_TABLE_COUNT, SDBG_OPT_STABLE_FIRST_PASS,
 )

@@ -19,6 +19,7 @@ SDBG_SORTED = 1
 SDBG_NUM_BUCKETS = 65536
 STATUS = {0: "SDBG_OK", -1: "SDBG_E_INVAL", -2: "SDBG_E_BADBASE", -3: "SDBG_E_CAPACITY", -4: "SDBG_E_WORKSPACE",
           -5: "SDBG_E_CUDA", -6: "SDBG_E_UNSUPPORTED"}
+SDBG_OPT_FORCE_WIDE, SDBG_OPT_NO_TABLE_COUNT, SDBG_OPT_STABLE_FIRST_PASS = 1, 2, 3
 T_CLASSES = ("pack", "extract", "radix", "count", "emit", "other", "table")
 
 
@@ -81,6 +82,8 @@ def lib():
         vp, u64, u32, i32 = C.c_void_p, C.c_uint64, C.c_uint32, C.c_int
         L.sdbg_ctx_create.argtypes = [C.POINTER(vp), i32, vp, vp, u64]; L.sdbg_ctx_create.restype = i32
         L.sdbg_ctx_destroy.argtypes = [vp]; L.sdbg_ctx_destroy.restype = None
+        L.sdbg_ctx_set_option.argtypes = [vp, i32, i32]; L.sdbg_ctx_set_option.restype = i32
+        L.sdbg_unstable_radix_launches.argtypes = []; L.sdbg_unstable_radix_launches.restype = u64
         L.sdbg_strerror.argtypes = [i32]; L.sdbg_strerror.restype = C.c_char_p
         L.sdbg_last_error.argtypes = [vp]; L.sdbg_last_error.restype = C.c_char_p
         L.sdbg_read_slots.argtypes = [u64, u64]; L.sdbg_read_slots.restype = u64
@@ -110,6 +113,10 @@ def lib():
 
 
 # ---- host-only helpers (no GPU needed) -----------------------------------------------------------------------------
+
+def sdbg_unstable_radix_launches() -> int:
+    return int(lib().sdbg_unstable_radix_launches())
+
 
 def sdbg_strerror(status: int) -> str:
     return lib().sdbg_strerror(status).decode()
@@ -173,6 +180,9 @@ class Context:
     def check(self, rc: int):
         if rc != 0:
             raise SdbgError(rc, lib().sdbg_last_error(self._h).decode() or sdbg_strerror(rc))
+
+    def set_option(self, option: int, value: int = 1):
+        self.check(lib().sdbg_ctx_set_option(self._h, int(option), int(value)))
 
     def set_timing(self, on: bool):
         self.check(lib().sdbg_ctx_set_timing(self._h, 1 if on else 0))

@@ -52,10 +52,9 @@ struct sdbg_ctx {
     u64 ws_bytes = 0;
     std::string err;
     bool timing = false;
-    bool force_wide = false;   // SDBG_FORCE_WIDE=1 in the environment at sdbg_ctx_create: see include/sdbg.h
-    bool no_unstable = false;  // SDBG_NO_UNSTABLE=1: the first radix pass uses the stable kernel like the others
-    bool no_hash = false;      // SDBG_NO_HASH=1: never count top-sorted records in shared-memory tables (api_count.inc count_range_hash)
-    bool no_partial = false;   // SDBG_NO_PARTIAL=1 in the environment at sdbg_ctx_create: always sort all records through all passes
+    bool force_wide = false;   // SDBG_OPT_FORCE_WIDE (sdbg_ctx_set_option, include/sdbg.h)
+    bool no_unstable = false;  // SDBG_OPT_STABLE_FIRST_PASS: the first radix pass uses the stable kernel like the others
+    bool no_hash = false;      // SDBG_OPT_NO_TABLE_COUNT: every record through every radix pass, then the sweeps of count.cu
     std::vector<EventPair> pending;
     std::vector<cudaEvent_t> free_events;
     char *fetch_buf = nullptr;   // kFetchBytes of mapped pinned host memory
@@ -209,14 +208,6 @@ int sdbg_ctx_create(sdbg_ctx **out, int device, void *cuda_stream, void *workspa
     c->stream = (cudaStream_t)cuda_stream;
     c->ws = (char *)workspace;
     c->ws_bytes = workspace_bytes;
-    const char *fw = getenv("SDBG_FORCE_WIDE");
-    c->force_wide = fw && fw[0] == '1';
-    const char *np_ = getenv("SDBG_NO_PARTIAL");
-    c->no_partial = np_ && np_[0] == '1';
-    const char *nu_ = getenv("SDBG_NO_UNSTABLE");
-    c->no_unstable = nu_ && nu_[0] == '1';
-    const char *nh_ = getenv("SDBG_NO_HASH");
-    c->no_hash = c->no_partial || (nh_ && nh_[0] == '1');
     *out = c;
     return SDBG_OK;
 }
@@ -227,6 +218,16 @@ void sdbg_ctx_destroy(sdbg_ctx *ctx) {
     for (auto e : ctx->free_events) cudaEventDestroy(e);
     if (ctx->fetch_buf) cudaFreeHost(ctx->fetch_buf);
     delete ctx;
+}
+
+int sdbg_ctx_set_option(sdbg_ctx *ctx, int option, int value) {
+    if (!ctx) return SDBG_E_INVAL;
+    switch (option) {
+        case SDBG_OPT_FORCE_WIDE: ctx->force_wide = value != 0; return SDBG_OK;
+        case SDBG_OPT_STABLE_FIRST_PASS: ctx->no_unstable = value != 0; return SDBG_OK;
+        case SDBG_OPT_NO_TABLE_COUNT: ctx->no_hash = value != 0; return SDBG_OK;
+    }
+    return ctx->fail(SDBG_E_INVAL, "unknown option");
 }
 
 int sdbg_ctx_set_timing(sdbg_ctx *ctx, int on) {
@@ -250,26 +251,29 @@ int sdbg_ctx_get_timing(sdbg_ctx *ctx, sdbg_timing *out) {
     return SDBG_OK;
 }
 
+uint64_t sdbg_unstable_radix_launches(void) { return radix_unstable_launches(); }
+
 uint32_t sdbg_key_words(uint32_t k) { return (2 * (k + 1) + 63) / 64; }
 
 uint64_t sdbg_read_slots(uint64_t n_bases, uint64_t n_calls) {
     return (n_bases + 64 * std::max<u64>(n_calls, 1) + 63) / 64 * 64 + SDBG_READ_GUARD_SLOTS;
 }
 
-// room for the (key, count) entries of the partial-sort path (api_count.inc): 12 bytes for up to a sixth of the records
-static u64 partial_slack(u64 n, u32 W) { return W == 1 ? align_up(n * 2) + kStatBytes + 8192 : 0; }
+// room behind the buffers of a one-word range for the scratch of the table-count path (api_count.inc): segment borders
+// and counts (16 bytes per 2,048 records), block sums, a copy of the statistics
+static u64 table_slack(u64 n, u32 W) { return W == 1 ? align_up(n / 64) + kStatBytes + 16384 : 0; }
 
 uint64_t sdbg_min_workspace(void) { return kFixedBytes + range_need(1ull << 16, 4); }
 
 uint64_t sdbg_full_workspace(uint64_t n_bases, uint32_t k) {
     if (k < 1 || k > SDBG_MAX_K) return 0;
-    const u64 need = kFixedBytes + range_need(2 * n_bases, sdbg_key_words(k)) + partial_slack(2 * n_bases, sdbg_key_words(k)) + 4096;
+    const u64 need = kFixedBytes + range_need(2 * n_bases, sdbg_key_words(k)) + table_slack(2 * n_bases, sdbg_key_words(k)) + 4096;
     return std::max<u64>(need, sdbg_min_workspace());
 }
 
 uint64_t sdbg_workspace_for_records(uint64_t n_records, uint32_t k) {
     if (k < 1 || k > SDBG_MAX_K) return 0;
-    const u64 need = kFixedBytes + range_need(n_records, sdbg_key_words(k)) + partial_slack(n_records, sdbg_key_words(k)) + 4096;
+    const u64 need = kFixedBytes + range_need(n_records, sdbg_key_words(k)) + table_slack(n_records, sdbg_key_words(k)) + 4096;
     return std::max<u64>(need, sdbg_min_workspace());
 }
 

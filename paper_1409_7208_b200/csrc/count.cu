@@ -77,14 +77,7 @@ __device__ __forceinline__ void shfl_key(u64 (&dst)[W], const u64 (&src)[W], int
 
 // WIDE: the range holds 2^32 records or more, so a run may be that long: run starts and lengths are 64-bit and the
 // multiplicity saturates at 2^32-1 (reading A9); otherwise 32-bit modular arithmetic is exact.
-// PARTIAL (one-word keys): the records are sorted by the key bits of a.low_mask only (the first passes of the LSD sort),
-// so all copies of a key lie inside one run of equal masked bits ("bucket"), in arbitrary order among the other keys of
-// that bucket. Runs of equal FULL keys ("fragments") are cut at chunk borders (no look behind the chunk). A fragment
-// that is a whole bucket (the record before it and the record after it have other masked bits) holds every copy of its
-// key: it is kept iff its length is >= d (and counted as a distinct edge here if dropped). Every other fragment (its
-// bucket holds more keys, or it is cut by a chunk border) is kept whatever its length: the caller sorts the kept entries
-// and adds up the entries of equal keys. Nothing else about the kernel changes.
-template <int W, bool CSUM, bool WIDE, bool PARTIAL = false>
+template <int W, bool CSUM, bool WIDE>
 __global__ void __launch_bounds__(kCountWarps * 32, W == 1 ? 6 : W == 2 ? 4 : 2) count_chunks_kernel(CountArgs a, DevState *st) {
     using len_t = std::conditional_t<WIDE, u64, u32>;
     constexpr int G = kCountGroup;
@@ -113,13 +106,7 @@ __global__ void __launch_bounds__(kCountWarps * 32, W == 1 ? 6 : W == 2 ? 4 : 2)
 
         // ---- start of the run that is open at the chunk's first record ----------------------------------------
         len_t carry = 0;                                     // chunk-relative start of the run in progress (modular)
-        bool carry_head = false;                             // PARTIAL: the run in progress begins a bucket
-        u64 prev_key = 0;                                    // PARTIAL: the record before the round's first one
-        if constexpr (PARTIAL) {
-            if (c0 > 0) prev_key = a.keys[c0 - 1];
-            const u64 first = __shfl_sync(0xffffffffu, key[0][0], 0);
-            carry_head = c0 == 0 || ((prev_key ^ first) & a.low_mask) != 0;
-        } else {
+        {
             u64 target[W], probe[W];
             shfl_key<W>(target, key[0], 0);
             // hi = lowest index known to belong to the run. Up to 4 rounds over the 32 records right below hi (these
@@ -164,37 +151,18 @@ __global__ void __launch_bounds__(kCountWarps * 32, W == 1 ? 6 : W == 2 ? 4 : 2)
             for (int q = 0; q < W; ++q) kn[q] = __shfl_sync(0xffffffffu, lane == 0 ? k_next_round[q] : k[q], (int)((lane + 1u) & 31u));
             bool tail = key_ne<W>(k, kn);
             if constexpr (!FULL) tail = i < rem && ((i + 1u == rem && !has_succ) || tail);
-            if constexpr (PARTIAL) tail = tail || (i + 1u == rem);           // fragments end at the chunk border
             const u32 T = __ballot_sync(0xffffffffu, tail);
             const u32 below = T & lt;
             const len_t start = below ? (len_t)(r * 32u + (32u - (u32)__clz(below))) : carry;   // place after the previous tail
             const len_t len = (len_t)(i + 1u) - start;
             bool solid = tail && len >= (len_t)a.d;
-            u32 n_whole = 0;
-            if constexpr (PARTIAL) {
-                // bucket borders: before me (HM) and after me (TM); the record after the data's last one counts as another bucket
-                const u64 up = __shfl_up_sync(0xffffffffu, k[0], 1);
-                const u64 kp = lane == 0 ? prev_key : up;
-                const bool bhead = (c0 + i == 0) || ((kp ^ k[0]) & a.low_mask) != 0;
-                const bool btail = (i < rem) && ((i + 1u == rem && !has_succ) || ((kn[0] ^ k[0]) & a.low_mask) != 0);
-                const u32 HM = __ballot_sync(0xffffffffu, bhead), TM = __ballot_sync(0xffffffffu, btail);
-                const bool frag_head = below ? ((HM >> (32u - (u32)__clz(below))) & 1u) != 0 : carry_head;
-                const bool whole = tail && frag_head && btail;                // the fragment is a whole bucket
-                solid = tail && (whole ? len >= (len_t)a.d : true);
-                n_whole = (u32)__popc(__ballot_sync(0xffffffffu, whole && !solid));   // distinct edges that end here (dropped)
-                if (T) {
-                    const u32 p = 32u - (u32)__clz(T);                        // place after the round's last tail
-                    carry_head = p < 32u ? ((HM >> p) & 1u) != 0 : ((TM >> 31) & 1u) != 0;
-                }
-                prev_key = __shfl_sync(0xffffffffu, k[0], 31);
-            }
             const u32 S = __ballot_sync(0xffffffffu, solid);
             if (T) carry = (len_t)(r * 32u + (32u - (u32)__clz(T)));
-            n_tails += PARTIAL ? n_whole : (u32)__popc(T);
+            n_tails += (u32)__popc(T);
             if (solid)    // where the solid edge sits in its chunk and its multiplicity (A9: saturated), in chunk order
                 a.stash[c0 + n_solid + (u32)__popc(S & lt)] = ((u64)i << 32) | (u64)((WIDE && len > (len_t)0xffffffffu) ? 0xffffffffu : (u32)len);
             n_solid += (u32)__popc(S);
-            if constexpr (!PARTIAL) { if (solid) sum_mult += len; }
+            if (solid) sum_mult += len;
             if constexpr (CSUM) { if (tail) csum += (u64)len * mix_key<W>(k); }
         };
         if (rem == kCountChunk && c0 + kCountChunk + 32u <= a.n) {
@@ -292,7 +260,7 @@ __global__ void __launch_bounds__(kCountWarps * 32) count_write_kernel(CountArgs
     const u64 c0 = chunk * kCountChunk;
     if (c0 >= a.n) return;
     const u32 *ws = reinterpret_cast<const u32 *>(a.tile_sums + gridDim.x) + (u64)blockIdx.x * kCountWarps;
-    u64 out_pos = (a.range_parity < 0 ? 0ull : st->out_cursor[a.range_parity]) + a.tile_sums[blockIdx.x];   // < 0: partial mode
+    u64 out_pos = st->out_cursor[a.range_parity] + a.tile_sums[blockIdx.x];
     for (u32 w = 0; w < warp; ++w) out_pos += ws[w];
     const u32 cnt = ws[warp];
     for (u32 e = lane; e < cnt; e += 32u) {
@@ -301,11 +269,6 @@ __global__ void __launch_bounds__(kCountWarps * 32) count_write_kernel(CountArgs
         if (pos < a.out_cap) {
             u64 k[W];
             load_key<W>(a.keys, c0 + (ent >> 32), k);
-            if (a.mix_shift) {   // partial mode: k' = k ^ ((k >> s) & M) back to k; every round fixes s more bits from the top (s >= 16)
-                const u64 kp = k[0];
-#pragma unroll
-                for (int it = 0; it < 4; ++it) k[0] = kp ^ ((k[0] >> a.mix_shift) & a.mix_mask);
-            }
 #pragma unroll
             for (int q = 0; q < W; ++q) a.out_keys[pos * W + q] = k[q];
             a.out_mult[pos] = (u32)ent;
@@ -333,64 +296,6 @@ static int launch_count_w(const CountArgs &a, DevState *st, cudaStream_t s) {
     scan_tiles_kernel<<<1, 1024, 0, s>>>(a.tile_sums, (u32)blocks, st, a.range_parity);
     count_write_kernel<W><<<g, t, 0, s>>>(a, st);
     return (int)cudaGetLastError();
-}
-
-int launch_count_partial_sweep(const CountArgs &a, DevState *st, cudaStream_t s) {
-    const u64 chunks = (a.n + kCountChunk - 1) / kCountChunk, blocks = (chunks + kCountWarps - 1) / kCountWarps;
-    if (blocks == 0 || blocks > 0x7fffffffull || a.W != 1) return (int)cudaErrorInvalidValue;
-    count_chunks_kernel<1, false, false, true><<<(unsigned)blocks, kCountWarps * 32, 0, s>>>(a, st);
-    scan_tiles_kernel<<<1, 1024, 0, s>>>(a.tile_sums, (u32)blocks, st, -1);      // entries -> st->merge_heads
-    return (int)cudaGetLastError();
-}
-void launch_count_partial_write(const CountArgs &a, DevState *st, cudaStream_t s) {
-    const u64 chunks = (a.n + kCountChunk - 1) / kCountChunk, blocks = (chunks + kCountWarps - 1) / kCountWarps;
-    count_write_kernel<1><<<(unsigned)blocks, kCountWarps * 32, 0, s>>>(a, st);   // a.range_parity < 0: entries from position 0
-}
-
-// Entries with final multiplicities (distinct keys): flag mult >= d; statistics (every entry is a distinct edge).
-__global__ void __launch_bounds__(256) solid_flags_kernel(const u32 *__restrict__ mult, u64 n, u32 d, uint8_t *__restrict__ flags, u64 *stat_slots) {
-    __shared__ u64 s_sum[8];
-    u64 sum = 0;
-    for (u64 i = (u64)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (u64)gridDim.x * blockDim.x) {
-        const u32 m = mult[i];
-        const bool solid = m >= d;
-        flags[i] = solid;
-        if (solid) sum += m;
-    }
-    sum = warp_reduce_add64(sum);
-    if ((threadIdx.x & 31u) == 0) s_sum[threadIdx.x >> 5] = sum;
-    __syncthreads();
-    if (threadIdx.x == 0) {
-        u64 v = 0;
-        for (int w = 0; w < 8; ++w) v += s_sum[w];
-        if (v) atomicAdd(&stat_slots[(blockIdx.x & (kStatSlots - 1)) * kStatSlotWords + 1], v);
-        if (blockIdx.x == 0) atomicAdd(&stat_slots[0], n);
-    }
-}
-void launch_solid_flags(const u32 *mult, u64 n, u32 d, uint8_t *flags, u64 *stat_slots, cudaStream_t s) {
-    if (n == 0) return;
-    u64 blocks = (n + 255) / 256;
-    if (blocks > (u64)num_sms() * 8) blocks = (u64)num_sms() * 8;
-    solid_flags_kernel<<<(unsigned)blocks, 256, 0, s>>>(mult, n, d, flags, stat_slots);
-}
-
-// The flagged entries (ascending index list) appended to the output at the cursor of this range; cursor of the next range set.
-__global__ void __launch_bounds__(256) append_solid_kernel(const u64 *__restrict__ keys, const u32 *__restrict__ mult, const u32 *__restrict__ idx,
-                                                           const u64 *__restrict__ n_idx, u64 *__restrict__ out_keys, u32 *__restrict__ out_mult,
-                                                           u64 out_cap, DevState *st, int range_parity) {
-    const u64 n = *n_idx, base = st->out_cursor[range_parity];
-    for (u64 i = (u64)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (u64)gridDim.x * blockDim.x) {
-        const u64 pos = base + i;
-        if (pos < out_cap) { out_keys[pos] = keys[idx[i]]; out_mult[pos] = mult[idx[i]]; }
-    }
-    if (blockIdx.x == 0 && threadIdx.x == 0) st->out_cursor[range_parity ^ 1] = base + n;
-}
-void launch_append_solid(const u64 *keys, const u32 *mult, const u32 *idx, const u64 *n_idx, u64 n_max, u64 *out_keys, u32 *out_mult,
-                         u64 out_cap, DevState *st, int range_parity, cudaStream_t s) {
-    u64 blocks = (n_max + 255) / 256;
-    if (blocks == 0) blocks = 1;
-    if (blocks > (u64)num_sms() * 8) blocks = (u64)num_sms() * 8;
-    append_solid_kernel<<<(unsigned)blocks, 256, 0, s>>>(keys, mult, idx, n_idx, out_keys, out_mult, out_cap, st, range_parity);
 }
 
 int launch_count_filter(const CountArgs &a, DevState *st, cudaStream_t s) {

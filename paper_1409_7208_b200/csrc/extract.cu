@@ -128,8 +128,7 @@ __global__ void __launch_bounds__(256) extract_kernel(ExtractArgs a, DevState *s
     // reversal is the digit; rc strand: its complement), prefix-summed over t and folded into the pass rows when the
     // block flushes. For k >= 8 exactly one key byte is left (byte 7 - T4 from the LSB, the one with e[k]): it is the
     // only per-key atomic. Shared-memory atomics, the bottleneck of this kernel, drop from 8 per key to about 2.4.
-    constexpr bool mixed = T4 == 8;                      // partial-sort path: mixed keys, digits of the first passes only
-    constexpr bool shared4 = T4 >= 2 && !mixed;
+    constexpr bool shared4 = T4 >= 2;
     constexpr u32 T = shared4 ? T4 : 0;
     u32 *s_posf = s_hist + np * kRadix, *s_posr = s_posf + (T + 1) * kRadix;   // [T + 1][256] each (shared4 only); row T is a spare
     if (do_hist) {
@@ -301,19 +300,9 @@ __global__ void __launch_bounds__(256) extract_kernel(ExtractArgs a, DevState *s
                 const bool v = (valid >> i) & 1;
                 const u32 m = __ballot_sync(0xffffffffu, v);
                 if (v) {
-                    if constexpr (mixed) {
-                        const u64 fm = f[0] ^ ((f[0] >> a.mix_shift) & a.mix_mask), rm = r[0] ^ ((r[0] >> a.mix_shift) & a.mix_mask);
-                        *reinterpret_cast<ulonglong2 *>(a.keys_out + base + 2 * __popc(m & lt)) = make_ulonglong2(fm, rm);
-                        for (u32 q = 0; q < a.mix_passes; ++q) {
-                            const u32 sh = 8u * (b0 + q);
-                            atomicAdd(&s_hist[q * kRadix + (u32)((fm >> sh) & 0xffull)], 1u);
-                            atomicAdd(&s_hist[q * kRadix + (u32)((rm >> sh) & 0xffull)], 1u);
-                        }
-                    } else {
-                        *reinterpret_cast<ulonglong2 *>(a.keys_out + base + 2 * __popc(m & lt)) = make_ulonglong2(f[0], r[0]);
-                        add_digits(f);
-                        add_digits(r);
-                    }
+                    *reinterpret_cast<ulonglong2 *>(a.keys_out + base + 2 * __popc(m & lt)) = make_ulonglong2(f[0], r[0]);
+                    add_digits(f);
+                    add_digits(r);
                 }
                 base += 2 * __popc(m);
             };
@@ -390,11 +379,10 @@ static int launch_extract_w(const ExtractArgs &a, DevState *st, cudaStream_t s) 
     u64 blocks = (ngroups + 255) / 256;
     const u64 maxb = (u64)num_sms() * 8;
     if (blocks > maxb) blocks = maxb;
-    const u32 T = (W == 1 && !filter && a.digit_hist && a.k >= 8 && !a.mix_shift) ? a.k / 4 : 0;   // 2..7: shared position tables
+    const u32 T = (W == 1 && !filter && a.digit_hist && a.k >= 8) ? a.k / 4 : 0;   // 2..7: shared position tables
     size_t smem = a.digit_hist ? (size_t)(a.passes.n + (T ? 2 * T + 2 : 0)) * kRadix * sizeof(u32) : 0;
     if (filter) { extract_kernel<W, true, 0><<<(unsigned)blocks, 256, smem, s>>>(a, st); return (int)cudaGetLastError(); }
     if constexpr (W == 1) {
-        if (a.mix_shift) { extract_kernel<1, false, 8><<<(unsigned)blocks, 256, smem, s>>>(a, st); return (int)cudaGetLastError(); }
         switch (T) {
             case 2: extract_kernel<1, false, 2><<<(unsigned)blocks, 256, smem, s>>>(a, st); return (int)cudaGetLastError();
             case 3: extract_kernel<1, false, 3><<<(unsigned)blocks, 256, smem, s>>>(a, st); return (int)cudaGetLastError();

@@ -46,8 +46,6 @@ struct ExtractArgs {
     u64 *keys_out;                // nullptr: histogram-only
     u64 out_cap;                  // records keys_out can hold
     u64 *digit_hist;              // nullptr or u64[n_passes][256], accumulated
-    u32 mix_shift, mix_passes;    // != 0 (one-word keys, plain dense pass only): emit k' = k ^ ((k >> mix_shift) & mix_mask) and
-    u64 mix_mask;                 // count the digits of k' for the first mix_passes passes only (partial-sort path, api_count.inc)
     u64 *bucket_hist;             // nullptr or u64[65536], accumulated (all buckets, ignores lo/hi)
     int want_csum;
     PassTable passes;
@@ -92,8 +90,6 @@ struct CountArgs {
                              // edges, then their exclusive prefix), behind them u32 per warp chunk
     u64 *stash;              // scratch of 8 bytes per record (the sorter's spare buffer): the sweep leaves (place in chunk,
                              // multiplicity) of every solid edge there, chunk by chunk
-    u64 low_mask;            // partial mode (see count.cu): the key bits the records are sorted by so far; 0 = normal mode
-    u32 mix_shift; u64 mix_mask;   // partial mode: the records are mixed keys k' = k ^ ((k >> mix_shift) & mix_mask); copied out un-mixed
     u64 *stat_slots;         // u64[kStatSlots][kStatSlotWords], accumulated
     int want_csum;
     bool force_wide;         // 64-bit run lengths whatever n is (tests)
@@ -101,14 +97,6 @@ struct CountArgs {
 };
 u64 count_tile_records(u32 W);
 int launch_count_filter(const CountArgs &a, DevState *st, cudaStream_t s);
-// partial mode, one-word keys: sweep + scan (entries -> st->merge_heads), then the copy of the entries
-int launch_count_partial_sweep(const CountArgs &a, DevState *st, cudaStream_t s);
-void launch_count_partial_write(const CountArgs &a, DevState *st, cudaStream_t s);
-// entries (distinct keys with final multiplicities): flag mult >= d, statistics; then append the flagged ones in order
-void launch_solid_flags(const u32 *mult, u64 n, u32 d, uint8_t *flags, u64 *stat_slots, cudaStream_t s);
-void launch_append_solid(const u64 *keys, const u32 *mult, const u32 *idx, const u64 *n_idx, u64 n_max, u64 *out_keys, u32 *out_mult,
-                         u64 out_cap, DevState *st, int range_parity, cudaStream_t s);
-
 // records sorted by their top key bytes only: count in shared-memory tables, segment by segment (hashcount.cu)
 struct HashCountArgs {
     const u64 *keys; u64 n;              // one-word keys sorted by key >> top_shift

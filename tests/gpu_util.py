@@ -19,8 +19,9 @@ class GpuResult:
 
 
 def run_gpu(reads, k, d, workspace_bytes=None, host_input=False, cap=None, checksums=True, bucket_hist=False,
-            n_calls=1, ctx=None):
-    """reads: list[str] or (bases uint8, offsets uint64) numpy pair or (torch cuda bases, torch cuda offsets)."""
+            n_calls=1, ctx=None, options=()):
+    """reads: list[str] or (bases uint8, offsets uint64) numpy pair or (torch cuda bases, torch cuda offsets).
+    options: SDBG_OPT_* switched on in the context made here (include/sdbg.h sdbg_ctx_set_option)."""
     import torch
     if isinstance(reads, list):
         bases, offs = to_arrays(reads)
@@ -43,6 +44,8 @@ def run_gpu(reads, k, d, workspace_bytes=None, host_input=False, cap=None, check
     if ctx is None:
         ws = workspace_bytes if workspace_bytes is not None else sd.sdbg_full_workspace(nb, k) + max(nb, 1 << 20)
         ctx = sd.Context(ws)
+        for opt in options:
+            ctx.set_option(opt, 1)
     rd = sd.Reads(nb, n_calls)
     if n_calls == 1:
         sd.sdbg_pack_reads(ctx, bases_t, offs_t, n, rd)
@@ -180,10 +183,108 @@ def _u64_sorted_view(t):
     return t ^ (-(2 ** 63))
 
 
+# ---- multi-word keys as lists of int64 tensors holding u64 bit patterns (word 0 most significant); any device ------------
+
+def _lsr(x, n):
+    """Logical shift right of u64 bit patterns held in int64."""
+    if n == 0:
+        return x
+    if n >= 64:
+        return x * 0
+    return (x >> n) & ((1 << (64 - n)) - 1)
+
+
+def _shl(x, n):
+    if n == 0:
+        return x
+    if n >= 64:
+        return x * 0
+    return x << n
+
+
+def _mw_shl(words, nbits):
+    """(w0:w1:...:w_{W-1}) << nbits, zeros shifted in."""
+    W = len(words)
+    q, r = divmod(nbits, 64)
+    out = []
+    for j in range(W):
+        hi = words[j + q] if j + q < W else None
+        lo = words[j + q + 1] if j + q + 1 < W else None
+        v = _shl(hi, r) if hi is not None else words[0] * 0
+        if r and lo is not None:
+            v = v | _lsr(lo, 64 - r)
+        out.append(v)
+    return out
+
+
+def _mw_shr(words, nbits):
+    W = len(words)
+    q, r = divmod(nbits, 64)
+    out = []
+    for j in range(W):
+        lo = words[j - q] if j - q >= 0 else None
+        hi = words[j - q - 1] if j - q - 1 >= 0 else None
+        v = _lsr(lo, r) if lo is not None else words[0] * 0
+        if r and hi is not None:
+            v = v | _shl(hi, 64 - r)
+        out.append(v)
+    return out
+
+
+def _s64(v):
+    """Python int in [0, 2^64) -> the int64 with the same bit pattern."""
+    v &= 2 ** 64 - 1
+    return v - 2 ** 64 if v >= 2 ** 63 else v
+
+
+def _rev2(x):
+    """Reverses the order of the 32 two-bit groups of every u64 pattern."""
+    for sh, m in ((2, 0x3333333333333333), (4, 0x0F0F0F0F0F0F0F0F), (8, 0x00FF00FF00FF00FF), (16, 0x0000FFFF0000FFFF)):
+        x = (_lsr(x, sh) & m) | ((x & m) << sh)
+    return _lsr(x, 32) | (x << 32)
+
+
+def rc_key_words(words, k):
+    """Key of rc(e) from the key of e, on the integer keys alone (tests/test_oracle_pins.py checks it against strings).
+    Key symbols of e: s = (e[k-1], ..., e[0], e[k]); of rc(e): (c(s[k-2]), ..., c(s[0]), c(s[k]), c(s[k-1])), c = 3 - x
+    ("useful identities")."""
+    W = len(words)
+    pad = 64 * W - 2 * (k + 1)
+    R = [_rev2(x) for x in reversed(words)]              # (pad zeros, s[k], s[k-1], ..., s[0])
+    X = _mw_shl(R, pad)                                  # (s[k], s[k-1], s[k-2], ..., s[0], zeros)
+    T = [X[0] & _s64(0xF << 60)] + [x * 0 for x in X[1:]]   # the two leading symbols alone
+    Y = _mw_shl(X, 4)                                    # (s[k-2], ..., s[0], 0, 0, zeros)
+    Tm = _mw_shr(T, 2 * (k - 1))                         # (zeros, s[k], s[k-1]) at symbol places k-1, k
+    out = []
+    for q in range(W):
+        nb = min(64, max(0, 2 * (k + 1) - 64 * q))       # significant bits of word q
+        sig = _s64(((1 << nb) - 1) << (64 - nb)) if nb else 0
+        out.append((Y[q] | Tm[q]) ^ sig)
+    return out
+
+
+_M1, _M2 = _s64(0xBF58476D1CE4E5B9), _s64(0x94D049BB133111EB)
+
+
+def _mix64_t(z):
+    z = (z ^ _lsr(z, 30)) * _M1
+    z = (z ^ _lsr(z, 27)) * _M2
+    return z ^ _lsr(z, 31)
+
+
+def key_mix_t(words):
+    """include/sdbg.h checksum of a key, on int64 tensors (wrapping arithmetic)."""
+    h = words[0] * 0
+    for x in words:
+        h = _mix64_t(h ^ x)
+    return h
+
+
 def check_global_invariants(res, w):
-    """Properties that hold at any size (SURVEY.md §8c P3-P6), evaluated on the device."""
+    """Properties that hold at any size (SURVEY.md §8c P3-P7, P9), evaluated on the device."""
     import torch
     st, ed, g, S, W = res.stats, res.edges, res.graph, res.n, res.edges.w
+    k = w.k
     assert st.n_raw == w.n_raw_edges                                   # P3: N = 2 sum max(0, L - k)
     assert st.csum_raw == st.csum_distinct                             # P4: the sort/count lost or duplicated nothing
     assert st.n_solid == S and S <= st.n_distinct <= st.n_raw
@@ -200,7 +301,7 @@ def check_global_invariants(res, w):
         a, b = col[:-1], col[1:]
         gt |= eq & (b > a)
         eq &= (b == a)
-        nb = min(64, max(0, 2 * w.k - 64 * q))                        # bits of this word that belong to the node
+        nb = min(64, max(0, 2 * k - 64 * q))                          # bits of this word that belong to the node
         if nb == 64:
             node_eq &= (b == a)
         elif nb > 0:
@@ -212,10 +313,50 @@ def check_global_invariants(res, w):
     bits = ((lb.unsqueeze(1) >> torch.arange(64, device="cuda")) & 1).reshape(-1)[:S]
     assert int(bits.sum()) == n_nodes                                  # P6: one `last` per distinct node
     assert torch.equal(bits[:-1].bool(), ~node_eq) and int(bits[-1]) == 1
+    del bits, gt, eq, node_eq
     Wb = g.W[:S]
     assert int(Wb.min()) >= 1 and int(Wb.max()) <= 8
-    sym = (keys[:, W - 1] >> (64 * W - 2 * (w.k + 1))) & 3            # outgoing base = last symbol of the key
+    sym = (keys[:, W - 1] >> (64 * W - 2 * (k + 1))) & 3              # outgoing base = last symbol of the key
     assert torch.equal(((Wb - 1) & 3).to(torch.int64), sym)
+    del sym
+    # P7 (north_star): the minus flag is set iff an earlier edge sharing the (k-1)-suffix of the node has
+    # the same outgoing base. Such edges share the top 2(k-1) key bits, so they are at most 15 places back (a group has
+    # at most 4 x 4 edges): c = (top 2(k-1) bits, outgoing base) equal to that of one of the 15 edges before.
+    pad = 64 * W - 2 * (k + 1)
+    cw = []
+    for q in range(W):
+        nb = min(64, max(0, 2 * (k - 1) - 64 * q))
+        m = ((1 << nb) - 1) << (64 - nb) if nb else 0
+        if q == W - 1:
+            m |= 3 << pad
+        cw.append(keys[:, q] & _s64(m))
+    want_minus = torch.zeros(S, dtype=torch.bool, device="cuda")
+    for dist in range(1, 16):
+        if dist >= S:
+            break
+        same = torch.ones(S - dist, dtype=torch.bool, device="cuda")
+        for q in range(W):
+            same &= cw[q][dist:] == cw[q][:-dist]
+        want_minus[dist:] |= same
+        del same
+    got_minus = Wb > 4
+    assert torch.equal(got_minus, want_minus), "minus flags differ from the rule"
+    n_targets = int((~want_minus).sum())                               # #(minus = 0) = distinct target k-mers
+    assert int((Wb <= 4).sum()) == n_targets
+    del cw, want_minus, got_minus
+    # P9 (reading A4): the solid set is closed under reverse complement with equal multiplicities. Checksums over
+    # (key, mult) and over (key of the reverse complement, mult) agree; for one-word keys the sorted reverse-complement
+    # keys ARE the key list and carry the same multiplicities.
+    kw = [keys[:, q].contiguous() for q in range(W)]
+    rw = rc_key_words(kw, k)
+    m64 = mult.to(torch.int64)
+    assert int((key_mix_t(kw) * m64).sum()) == int((key_mix_t(rw) * m64).sum()), "not closed under reverse complement"
+    if W == 1:
+        order = torch.argsort(_u64_sorted_view(rw[0]))
+        assert torch.equal(rw[0][order], kw[0]), "reverse complements of the solid edges are not the solid edges"
+        assert torch.equal(mult[order], mult), "an edge and its reverse complement differ in multiplicity"
+        del order
+    del kw, rw, m64
     return n_nodes
 
 

@@ -1,8 +1,10 @@
 """-m gpu: BASELINE.json configs at FULL size, in the launch configuration bench.py times (one range, through the C
 ABI), checked on oracle-verified sampled l=8 partitions plus the global invariants (north_star: "for configs too
-large for the oracle ..."). Configs 2, 3 and 4 run always (15 s each: the oracle's scan of the reads runs in forked
-processes); config 5 (20 Gbp of reads, block-wise) runs when SDBG_LARGE names it (SDBG_LARGE=5); its log is kept
-under profiles/.
+large for the oracle ..."). Configs 2, 3 and 4 run always (the oracle's scan of the reads runs in forked processes:
+256 sampled partitions on config 2, 64 on configs 3 and 4). Config 5 runs always at 0.45 of its size (9 Gbp of reads,
+14.2 G records) with a workspace for 4.4 G records: at least four block-wise ranges, one of them of 2^32 records or more,
+so the wide (64-bit count) layout of the sorter runs for real; the full 20 Gbp run (20 GB of host RAM for the oracle's
+copy of the reads, ~170 GB of HBM) runs when SDBG_LARGE names it (SDBG_LARGE=5); its log is kept under profiles/.
 """
 import os
 import time
@@ -27,14 +29,15 @@ def _pick_buckets(hist, seed, n=16):
     return sorted(picks)
 
 
-def _run_config(cfg, workspace_bytes=None, min_ranges=1, n_buckets=16, full_graph=True):
+def _run_config(cfg, workspace_bytes=None, min_ranges=1, n_buckets=16, full_graph=True, scale=1.0, min_max_range=0):
     from workloads import get_config
-    w = get_config(cfg)
+    w = get_config(cfg, scale)
     t0 = time.time()
     res = run_gpu_workload(w, workspace_bytes=workspace_bytes, keep_ascii=True)
     t1 = time.time()
     st = res.stats
     assert st.n_ranges >= min_ranges, st.n_ranges
+    assert st.max_range_records >= min_max_range, st.max_range_records
     import torch
     if min_ranges == 1:
         # the launch configuration bench.py times: no statistics asked for (the extractor's plain path, paired 16-byte
@@ -74,15 +77,24 @@ def _run_config(cfg, workspace_bytes=None, min_ranges=1, n_buckets=16, full_grap
 
 
 def test_config2_full_size_sampled_partitions():
-    _run_config(2)
+    _run_config(2, n_buckets=256)
 
 
 def test_config3_full_size_sampled_partitions():
-    _run_config(3)
+    _run_config(3, n_buckets=64)
 
 
 def test_config4_full_size_sampled_partitions():
-    _run_config(4)
+    _run_config(4, n_buckets=64)
+
+
+def test_config5_blockwise_ranges_with_a_wide_range():
+    """Config 5 at 0.45 of its size ("k-mers in consecutive partitions that fit within the GPU memory are
+    sorted together"): the workspace holds 4.4 G records, the 14.2 G records need four ranges, the first three of 2^32
+    records or more."""
+    import paper_1409_7208_b200 as sd
+    _run_config(5, workspace_bytes=sd.sdbg_workspace_for_records(4_400_000_000, 21), min_ranges=4, n_buckets=8,
+                full_graph=False, scale=0.45, min_max_range=2 ** 32)
 
 
 @pytest.mark.skipif(5 not in LARGE, reason="set SDBG_LARGE=5 (2 minutes of 16 host cores, 20 GB of host RAM, ~170 GB of HBM)")

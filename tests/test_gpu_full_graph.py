@@ -30,7 +30,10 @@ def _run(reads, k, d, workspace_extra=0):
     sd.sdbg_count_edges(ctx, rd, rd.n_reads, k, d, ed, None)
     assert ed.n == res.n_solid
     fg = sd.FullGraph(want["m"], want["t"], k)
+    unstable_before = sd.sdbg_unstable_radix_launches()
     sd.sdbg_build_full(ctx, ed, fg)
+    # its single radix pass refines an existing order: it must be the stable kernel (include/sdbg.h, kernels.cuh RadixArgs)
+    assert sd.sdbg_unstable_radix_launches() == unstable_before, "sdbg_build_full launched the unstable radix pass"
     assert (fg.m, fg.t, fg.n_zero_out) == (want["m"], want["t"], want["n_zero_out"])
     assert np.array_equal(fg.W_np(), want["W"]), "W differs"
     assert np.array_equal(fg.mult_np(), want["mult"]), "mult differs"

@@ -35,7 +35,9 @@ def _run(reads, k, d):
     sd.sdbg_count_edges(ctx, rd, rd.n_reads, k, d, ed, None)
     n_want = len(want["keys"])
     me = sd.Edges(max(n_want, 1), k)
+    unstable_before = sd.sdbg_unstable_radix_launches()
     n = sd.sdbg_mercy_edges(ctx, rd, ed, me)
+    assert sd.sdbg_unstable_radix_launches() == unstable_before, "sdbg_mercy_edges launched the unstable radix pass"
     assert n == n_want
     got = me.keys_np()
     assert np.array_equal(_sorted_rows(got), _sorted_rows(want["keys"])), "mercy records differ"

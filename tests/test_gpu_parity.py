@@ -288,16 +288,16 @@ def test_k_schedule_on_one_resident_read_set():
         assert np.array_equal(g.W_np(), orc.Wbyte) and np.array_equal(g.last_bits_np(), orc.last_bits)
 
 
-def test_wide_range_code_path_at_small_size(monkeypatch):
-    """Ranges of 2^32 records and more use other kernels (wide look-back words, 64-bit run lengths); SDBG_FORCE_WIDE=1
-    sends small inputs down that path (include/sdbg.h), so that it is covered here and not only by config 5."""
+def test_wide_range_code_path_at_small_size():
+    """Ranges of 2^32 records and more use other kernels (wide look-back words, 64-bit run lengths); the option
+    SDBG_OPT_FORCE_WIDE sends small inputs down that path (include/sdbg.h), so that it is covered here and not only by
+    config 5 (tests/test_gpu_configs.py runs a range of more than 2^32 records for real)."""
     from workloads import ReadGenerator, get_config
-    monkeypatch.setenv("SDBG_FORCE_WIDE", "1")
     import paper_1409_7208_b200 as sd
     for k, scale in ((21, 0.3), (31, 0.1)):
         bases, offs = ReadGenerator(get_config(1, scale=scale)).host()
         orc = run_oracle((bases, offs), k, 2)
-        assert_matches_oracle(run_gpu((bases, offs), k, 2), orc)
+        assert_matches_oracle(run_gpu((bases, offs), k, 2, options=[sd.SDBG_OPT_FORCE_WIDE]), orc)
         assert_matches_oracle(run_gpu((bases, offs), k, 2, workspace_bytes=sd.sdbg_min_workspace()), orc)
 
 
@@ -323,40 +323,6 @@ def test_plain_path_without_statistics(k):
         assert_matches_oracle(res, run_oracle(reads, k, d), check_stats=False)
 
 
-@pytest.mark.parametrize("k", [15, 21, 31])
-def test_partial_sort_path_and_its_way_back(k):
-    """The partial-sort path (sort by the first passes on mixed keys, count inside the buckets, sort only the kept
-    entries): (1) high coverage, d = 2: few entries, the path completes; (2) reads without repeats, d = 1: every record
-    is an entry, more than a quarter of the records, so the range is extracted again and sorted the plain way; (3)
-    the same inputs with the path switched off (SDBG_NO_PARTIAL=1 at context creation) give the same edges."""
-    import os
-    import random
-    from oracle import run_oracle
-    from tests.gpu_util import run_gpu, assert_matches_oracle
-    from tests.helpers import rc
-    rng = random.Random(900 + k)
-    genome = "".join(rng.choice("ACGT") for _ in range(3000))
-    covered = []
-    for _ in range(1500):
-        a = rng.randint(0, len(genome) - 100)
-        x = list(genome[a:a + 100])
-        if rng.random() < 0.3:
-            x[rng.randrange(100)] = rng.choice("ACGT")          # one-mismatch copies: the case the key mixing is for
-        x = "".join(x)
-        covered.append(x if rng.random() < 0.5 else rc(x))
-    unique = ["".join(rng.choice("ACGT") for _ in range(120)) for _ in range(400)]
-    for reads, d in ((covered, 2), (unique, 1), (covered + unique, 1)):
-        orc = run_oracle(reads, k, d)
-        res = run_gpu(reads, k, d, checksums=False)
-        assert_matches_oracle(res, orc, check_stats=True)
-        os.environ["SDBG_NO_PARTIAL"] = "1"
-        try:
-            res2 = run_gpu(reads, k, d, checksums=False)
-        finally:
-            del os.environ["SDBG_NO_PARTIAL"]
-        assert_matches_oracle(res2, orc, check_stats=True)
-
-
 def _radix_launches(res):
     """Radix passes over all records since the context was created (launch accounting of sdbg_ctx_get_timing)."""
     return res.ctx.get_timing().launches["radix"]
@@ -366,8 +332,8 @@ def _radix_launches(res):
 def test_table_count_path_and_its_way_back(k):
     """The top-sort + table-count path (api_count.inc count_range_hash, hashcount.cu): records sorted by the most
     significant passes only, segments of whole buckets counted in shared-memory tables. Checked against the oracle and
-    against the two other paths (SDBG_NO_HASH=1: partial-sort path; SDBG_NO_PARTIAL=1: every pass over every record),
-    statistics included; the number of radix launches says which path ran. Cases: (1) covered reads with one-mismatch
+    against the plain path (option SDBG_OPT_NO_TABLE_COUNT: every pass over every record) and the stable first pass
+    (SDBG_OPT_STABLE_FIRST_PASS), statistics included; the number of radix launches says which path ran. Cases: (1) covered reads with one-mismatch
     copies, d = 2 and 3: the path completes with fewer passes than the key has bytes; (2) the all-ones key (T...T at
     k = 31 fills the word) and its all-zero twin; (3) a bucket longer than the search window (poly-A): overflow, the
     records are sorted the plain way from where the top passes left them; (4) reads over two letters only: far more
@@ -404,13 +370,14 @@ def test_table_count_path_and_its_way_back(k):
             assert 1 <= n_hash < P, (name, k, d, n_hash)              # top passes only
         else:
             assert P < n_hash < 2 * P, (name, k, d, n_hash)            # top passes, then all passes (the way back)
-        for var in ("SDBG_NO_HASH", "SDBG_NO_PARTIAL", "SDBG_NO_UNSTABLE"):   # the last: stable kernel for the first pass too
-            os.environ[var] = "1"
-            try:
-                res2 = run_gpu(reads, k, d, checksums=False)
-            finally:
-                del os.environ[var]
+        import paper_1409_7208_b200 as sd
+        for opt in (sd.SDBG_OPT_NO_TABLE_COUNT, sd.SDBG_OPT_STABLE_FIRST_PASS):
+            res2 = run_gpu(reads, k, d, checksums=False, options=[opt])
             assert_matches_oracle(res2, orc, check_stats=True)
-            if var == "SDBG_NO_PARTIAL":
+            if opt == sd.SDBG_OPT_NO_TABLE_COUNT:
                 assert _radix_launches(res2) == P, (name, k, d)
             assert res2.edges.n == res.edges.n
+    # d = 1 keeps every distinct edge: the table count is not used, the records go through all passes exactly once
+    res1 = run_gpu(covered, k, 1, checksums=False)
+    assert_matches_oracle(res1, run_oracle(covered, k, 1), check_stats=True)
+    assert _radix_launches(res1) == P

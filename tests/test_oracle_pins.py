@@ -454,3 +454,85 @@ def test_traversal_on_the_complete_de_bruijn_graph():
     rep = nav["backward"][nav["forward"]]
     E = f["edges"]
     assert np.all(f["W"][rep] <= 4) and np.all(E[rep][:, 1:] == E[:, 1:]) and np.all(rep <= np.arange(m))
+
+
+# ---- packing pins beyond the first word (VERDICT r1 "parity unpinned": aux_bits, zin_bits, last_bits, valid_bits) -----------
+
+def _bigint_words(value, nbits_total):
+    """Big integer holding a bit stream whose bit 0 is the MOST significant bit of word 0 -> list of u64 words."""
+    nwords = (nbits_total + 63) // 64
+    value <<= 64 * nwords - nbits_total
+    return [(value >> (64 * (nwords - 1 - j))) & (2 ** 64 - 1) for j in range(nwords)]
+
+
+def test_aux_bits_packing_across_word_borders():
+    """k = 20: 40 bits per node, so node 1 straddles aux_bits[0] / aux_bits[1] and node 3 aux_bits[1] / aux_bits[2].
+    Two reads without repeated k-mers, each given twice (d = 2): four open paths, i.e. four zero-indegree nodes (the first
+    k-mers of the reads and of their reverse complements), in colex order of the node. The expected words are written
+    with shifts of the four 40-bit node values, not with the oracle's packing loop."""
+    from tests.helpers import rc
+    k = 20
+    r1 = "ACGGATTCAGCATTGACCGTAGGCTAAC"
+    r2 = "TTGCACGATCGGGATACCAGTGCATCAAGG"
+    res, f = _full([r1, r1, r2, r2], k, 2)
+    assert f["t"] == 4
+    want_nodes = sorted([r1[:k], rc(r1)[:k], r2[:k], rc(r2)[:k]], key=lambda s: s[::-1])
+    assert [bytes(a).decode() for a in f["aux"]] == want_nodes
+    v = []
+    for s in want_nodes:
+        x = 0
+        for c in s:
+            x = (x << 2) | "ACGT".index(c)
+        v.append(x)
+    w0 = ((v[0] << 24) | (v[1] >> 16)) & (2 ** 64 - 1)                 # node 0: bits 63..24; first 24 bits of node 1
+    w1 = (((v[1] & 0xFFFF) << 48) | (v[2] << 8) | (v[3] >> 32)) & (2 ** 64 - 1)   # last 16 of node 1, node 2, first 8 of node 3
+    w2 = ((v[3] & 0xFFFFFFFF) << 32) & (2 ** 64 - 1)                   # last 32 bits of node 3, zero padding
+    assert [int(x) for x in f["aux_bits"]] == [w0, w1, w2]
+    assert [int(x) for x in f["aux_bits"]] == _bigint_words((v[0] << 120) | (v[1] << 80) | (v[2] << 40) | v[3], 160)
+
+
+def test_last_valid_zin_bits_packing_beyond_64_edges():
+    """m > 128 edges: last_bits, valid_bits (Oracle.full_graph) and zin_bits (sdbg_traverse.navigation) against big
+    integers built from the per-edge 0/1 arrays and, for zin, from the node strings (bit i % 64 of word i / 64)."""
+    from oracle.sdbg_traverse import navigation
+    from tests.helpers import rc
+    import random
+    rng = random.Random(4242)
+    k = 5
+    reads = ["".join(rng.choice("ACGT") for _ in range(60)) for _ in range(3)]
+    res, f = _full(reads + reads, k, 2)
+    m = f["m"]
+    assert m > 128
+    def lsb_words(bits01):
+        v = 0
+        for i, b in enumerate(bits01):
+            v |= int(b) << i
+        return [(v >> (64 * j)) & (2 ** 64 - 1) for j in range((len(bits01) + 63) // 64)]
+    assert [int(x) for x in f["last_bits"]] == lsb_words(f["last"])
+    assert [int(x) for x in f["valid_bits"]] == lsb_words([1] * m)
+    nav = navigation(f, k)
+    aux = {bytes(a).decode() for a in f["aux"]}
+    nodes = [bytes(e[:k]).decode() for e in f["edges"]]
+    zin = [1 if (nodes[i] in aux and (i == m - 1 or nodes[i + 1] != nodes[i])) else 0 for i in range(m)]
+    assert sum(zin) == f["t"] and any(zin[64:])
+    assert [int(x) for x in nav["zin_bits"]] == lsb_words(zin)
+
+
+@pytest.mark.parametrize("k", [1, 2, 3, 8, 15, 21, 30, 31, 32, 33, 47, 62, 63, 64, 65, 95, 99, 126, 127])
+def test_integer_reverse_complement_of_keys_used_by_the_full_size_invariants(k):
+    """tests/gpu_util.py rc_key_words / key_mix_t (the P9 check at full size works on integer keys alone) against strings:
+    key(rc(e)) from helpers.key_words(rc(e)), the key checksum from helpers.key_mix."""
+    import random
+    import torch
+    from tests.gpu_util import rc_key_words, key_mix_t, _s64
+    from tests.helpers import key_words, rc, key_mix
+    rng = random.Random(900 + k)
+    es = ["".join(rng.choice("ACGT") for _ in range(k + 1)) for _ in range(64)] + ["A" * (k + 1), "T" * (k + 1)]
+    kw = [key_words(e, k) for e in es]
+    W = len(kw[0])
+    words = [torch.tensor([_s64(x[q]) for x in kw], dtype=torch.int64) for q in range(W)]
+    got = rc_key_words(words, k)
+    want = [key_words(rc(e), k) for e in es]
+    for q in range(W):
+        assert [int(v) & (2 ** 64 - 1) for v in got[q]] == [x[q] for x in want]
+    assert [int(v) & (2 ** 64 - 1) for v in key_mix_t(words)] == [key_mix(x) for x in kw]
