@@ -244,10 +244,21 @@ def device_steps(sd, torch, wl, args, steps, warmup, rank, world, local, barrier
     bases_d, offs_d = gen.device()
     torch.cuda.synchronize()
     n_reads, N = wl.n_reads, wl.n_raw_edges
-    ctx = sd.Context(sd.sdbg_workspace_for_records(N, wl.k))
+    ws_bytes = int(args.workspace_gb * 2 ** 30) if args.workspace_gb else sd.sdbg_workspace_for_records(N, wl.k)
+    ctx = sd.Context(ws_bytes)
     reads = sd.Reads(wl.n_bases)
-    edges = sd.Edges(N // wl.d, wl.k)
-    graph = sd.Graph(N // wl.d)
+    cap = N // wl.d
+    if cap * (8 * wl.words_per_key + 10) > 40 * 2 ** 30:      # the safe bound N / d would not fit: ask for the count first
+        sd.sdbg_pack_reads(ctx, bases_d, offs_d, n_reads, reads)
+        probe = sd.Edges(0, wl.k)
+        try:
+            sd.sdbg_count_edges(ctx, reads, n_reads, wl.k, wl.d, probe, None)
+        except sd.SdbgError as e:
+            if e.name != "SDBG_E_CAPACITY":
+                raise
+        cap = probe.n + 1024
+    edges = sd.Edges(cap, wl.k)
+    graph = sd.Graph(cap)
 
     def step():
         reads.c.n_reads = reads.c.n_bases = reads.c.n_slots = 0
@@ -467,7 +478,8 @@ def run_gpu(args, w):
         "higher_is_better": True, "scaling": "strong" if args.shard else "weak", "vs_baseline": None, "dtype": "u64", "data": "synthetic",
         "config": {"workload": wl.name, "k": wl.k, "d": wl.d, "reads": n_reads, "read_len": wl.read_len, "bases": n_bases,
                    "raw_edges": N, "solid_edges": int(S), "key_bytes": K, "parallelism": ("sharded by ranges of l=8 partitions, reads replicated" if args.shard else "replicas only" if world > 1 else "1 gpu"),
-                   "l2": "inputs larger than L2 (keys %.2f GB, reads %.0f MB ASCII)" % (N * K / 1e9, n_bases / 1e6)},
+                   "l2": "inputs larger than L2 (keys %.2f GB, reads %.0f MB ASCII)" % (N * K / 1e9, n_bases / 1e6),
+                   "workspace_gib": args.workspace_gb or None},
         "read_bases_per_s": (1 if args.shard else world) * n_bases * args.steps / (ms_total * 1e-3),
         "clocks": clocks,
         "e2e": {"value": whole_job_value(N, world, args.steps, ms_e2e), "unit": UNIT, "h2d_bytes_per_step": h2d,
@@ -559,7 +571,9 @@ def main():
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=10)
     ap.add_argument("--warmup", type=int, default=3)
-    ap.add_argument("--config", type=int, default=2, help="BASELINE.json config number (1-4); default 2 = configs[1]")
+    ap.add_argument("--config", type=int, default=2, help="BASELINE.json config number (1-5); default 2 = configs[1]; 5 (20 Gbp, "
+                    "block-wise) needs --workspace-gb (default 100) and skips the end-to-end leg")
+    ap.add_argument("--workspace-gb", type=float, default=0.0, help="workspace of the context in GiB (default: what holds all records in one range)")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--ref-reads", type=int, default=40000, help="reads in the oracle's bounded sample")
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -573,6 +587,9 @@ def main():
     args = ap.parse_args()
     from workloads import get_config
     w = get_config(args.config)
+    if args.config == 5:
+        args.no_e2e = True
+        args.workspace_gb = args.workspace_gb or 100.0
     if args.next:
         if int(os.environ.get("RANK", "0")) == 0:
             run_next_rows(args, w)

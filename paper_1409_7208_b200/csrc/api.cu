@@ -150,11 +150,14 @@ bool is_device_ptr(const void *p) {
 // bytes of dynamic workspace a sort+count of n records needs (keys only)
 // records per look-back row of the sorter that handles W-word keys: the keys themselves (W = 1) or (word, index) pairs
 u64 sort_tile_records(u32 W) { return W == 1 ? radix_tile_records(1, false) : radix_tile_records(1, true); }
+// room behind the buffers of a one-word range for the scratch of the table-count path (api_count.inc hash_scratch_bytes:
+// segment borders and counts, 16 bytes per 2,048 records, block sums, a copy of the statistics)
+u64 table_slack(u64 n, u32 W) { return W == 1 ? align_up(n / 64) + kStatBytes + 16384 : 0; }
 u64 range_need(u64 n, u32 W) {
     const u64 K = 8ull * W;
     const u64 rt = sort_tile_records(W), ct = count_tile_records(W);
     const u64 pairs = W == 1 ? 0 : 2 * align_up(n * 8) + 2 * align_up(n * 4);   // (word, index) ping-pong buffers
-    return 2 * align_up(n * K) + pairs + align_up(((n + rt - 1) / rt + 1) * kRadix * 8) + align_up(((n + ct - 1) / ct + 1) * 8);
+    return 2 * align_up(n * K) + pairs + align_up(((n + rt - 1) / rt + 1) * kRadix * 8) + align_up(((n + ct - 1) / ct + 1) * 8) + table_slack(n, W);
 }
 // largest n with range_need(n) <= avail; one sort range is also capped by the layout of the radix passes' look-back
 // words (radix_max_records: 2^34-1 records or 2^22 tiles); larger inputs are split into block-wise ranges like any
@@ -259,21 +262,17 @@ uint64_t sdbg_read_slots(uint64_t n_bases, uint64_t n_calls) {
     return (n_bases + 64 * std::max<u64>(n_calls, 1) + 63) / 64 * 64 + SDBG_READ_GUARD_SLOTS;
 }
 
-// room behind the buffers of a one-word range for the scratch of the table-count path (api_count.inc): segment borders
-// and counts (16 bytes per 2,048 records), block sums, a copy of the statistics
-static u64 table_slack(u64 n, u32 W) { return W == 1 ? align_up(n / 64) + kStatBytes + 16384 : 0; }
-
 uint64_t sdbg_min_workspace(void) { return kFixedBytes + range_need(1ull << 16, 4); }
 
 uint64_t sdbg_full_workspace(uint64_t n_bases, uint32_t k) {
     if (k < 1 || k > SDBG_MAX_K) return 0;
-    const u64 need = kFixedBytes + range_need(2 * n_bases, sdbg_key_words(k)) + table_slack(2 * n_bases, sdbg_key_words(k)) + 4096;
+    const u64 need = kFixedBytes + range_need(2 * n_bases, sdbg_key_words(k)) + 4096;
     return std::max<u64>(need, sdbg_min_workspace());
 }
 
 uint64_t sdbg_workspace_for_records(uint64_t n_records, uint32_t k) {
     if (k < 1 || k > SDBG_MAX_K) return 0;
-    const u64 need = kFixedBytes + range_need(n_records, sdbg_key_words(k)) + table_slack(n_records, sdbg_key_words(k)) + 4096;
+    const u64 need = kFixedBytes + range_need(n_records, sdbg_key_words(k)) + 4096;
     return std::max<u64>(need, sdbg_min_workspace());
 }
 

@@ -138,6 +138,8 @@ __global__ void __launch_bounds__(256) extract_kernel(ExtractArgs a, DevState *s
     // s_hist row of byte 0 of the last key word if it were a pass (rows of the padding bytes are never touched)
     const u32 b0 = a.passes.n ? (u32)a.passes.p[0].shift >> 3 : 0u;
     u32 *h_last = s_hist - b0 * kRadix;
+    // one-word keys, a.hist_top most significant passes wanted only: bytes below bmin of the key word are not counted
+    const u32 bmin = (W == 1 && a.hist_top && (int)a.hist_top < np) ? b0 + (u32)np - a.hist_top : b0;
     const u64 ngroups = a.n_slots / 32;
     const u32 lane = lane_id();
     const u32 lt = lanemask_lt();
@@ -226,7 +228,7 @@ __global__ void __launch_bounds__(256) extract_kernel(ExtractArgs a, DevState *s
         auto add_digits = [&](const u64 (&key)[W]) {
             if constexpr (shared4) {   // the one byte that is not counted by position: byte 7 - T from the LSB = pass 0
                 constexpr u32 b = 7 - T;
-                atomicAdd(&s_hist[__byte_perm(b < 4 ? (u32)key[0] : (u32)(key[0] >> 32), 0u, 0x4440u | (b & 3))], 1u);
+                if (bmin <= b) atomicAdd(&s_hist[__byte_perm(b < 4 ? (u32)key[0] : (u32)(key[0] >> 32), 0u, 0x4440u | (b & 3))], 1u);
             } else {
 #pragma unroll
                 for (int q = W - 1; q >= 0; --q) {
@@ -234,7 +236,7 @@ __global__ void __launch_bounds__(256) extract_kernel(ExtractArgs a, DevState *s
                     const u32 lo = (u32)key[q], hi = (u32)(key[q] >> 32);
 #pragma unroll
                     for (int b = 0; b < 8; ++b) {
-                        if (q == W - 1 && b < (int)b0) continue;     // padding bytes of the last word: no pass
+                        if (q == W - 1 && b < (int)bmin) continue;   // padding bytes of the last word (and passes not wanted): no row
                         atomicAdd(&hq[b * kRadix + __byte_perm(b < 4 ? lo : hi, 0u, 0x4440u | (b & 3))], 1u);
                     }
                 }

@@ -46,6 +46,7 @@ struct ExtractArgs {
     u64 *keys_out;                // nullptr: histogram-only
     u64 out_cap;                  // records keys_out can hold
     u64 *digit_hist;              // nullptr or u64[n_passes][256], accumulated
+    u32 hist_top;                 // != 0: only the rows of the hist_top most significant passes are needed (the others may stay short)
     u64 *bucket_hist;             // nullptr or u64[65536], accumulated (all buckets, ignores lo/hi)
     int want_csum;
     PassTable passes;

@@ -104,6 +104,17 @@ def test_P8_plan_independence_blockwise(k):
     res = run_gpu((bases, offs), k, 2, workspace_bytes=sd.sdbg_min_workspace())
     assert res.stats.n_ranges >= 3, res.stats.n_ranges
     assert_matches_oracle(res, orc)
+    # without checksums one-word keys take the default path INSIDE every block-wise range: the most significant passes
+    # for the record density of the range, then the table count (launch accounting: table launches, and fewer radix
+    # launches than ranges x passes; a last range of a few records alone may go the plain way)
+    res2 = run_gpu((bases, offs), k, 2, workspace_bytes=sd.sdbg_min_workspace(), checksums=False)
+    assert_matches_oracle(res2, orc)
+    tim = res2.ctx.get_timing()
+    P = (2 * (k + 1) + 7) // 8
+    if k <= 31:
+        assert tim.launches["table"] >= res2.stats.n_ranges - 1 and tim.launches["radix"] < res2.stats.n_ranges * P, tim.launches
+    else:
+        assert tim.launches["table"] == 0
 
 
 def test_edge_cases():

@@ -67,6 +67,15 @@ def _check(w, ctx, reads, n_shards, workspace_ctx=None, min_ranges=1):
             torch.cuda.synchronize()
             assert torch.equal(g.W[:n_r], g_full.W[off:off + n_r]), f"shard {r}: W differs"
             assert torch.equal(_bits(g.last_bits, n_r), _bits(g_full.last_bits, S)[off:off + n_r]), f"shard {r}: last differs"
+        if w.d >= 2 and full.w == 1 and w.k >= 15 and ps.n_raw >= 4096:
+            # the launch configuration of bench.py --shard: no checksums asked for, so the shard takes the default path
+            # (top passes for the record density of its range, then the table count) and must give the same edges
+            part2 = sd.Edges(S, w.k)
+            cctx.get_timing()
+            n2, _ = count_edges_sharded(cctx, reads, w.n_reads, w.k, w.d, part2, r, n_shards, None, bounds)
+            assert cctx.get_timing().launches["table"] >= 1, "the shard did not take the table-count path"
+            assert n2 == n_r and torch.equal(part2.keys[:n_r], part.keys[:n_r]) and torch.equal(part2.mult[:n_r], part.mult[:n_r])
+            del part2
         for f in ("n_raw", "n_distinct", "sum_solid_mult"):
             tot[f] += getattr(ps, f)
         for f in ("csum_raw", "csum_distinct"):
