@@ -72,10 +72,13 @@ void sdbg_ctx_destroy(sdbg_ctx *ctx);
  *                              significant passes only and are counted bucket by bucket in shared-memory tables
  *                              (hashcount.cu); whatever does not fit there (an over-long bucket, a full table) is redone
  *                              the plain way inside the same call
+ *   SDBG_OPT_NO_FUSED_EXTRACT  on the default path the extractor writes the keys in read order and the first top pass reads
+ *                              them back (default for one dense range of one-word keys, k >= 8: extraction is fused with
+ *                              that pass, the keys go from the key maker straight into its 256 bins)
  *   SDBG_OPT_STABLE_FIRST_PASS the first radix pass of sdbg_count_edges' sorts uses the stable kernel like the others
  *                              (default: unstable, equal keys are merged afterwards)
  * Errors: SDBG_E_INVAL (null ctx, unknown option). */
-enum { SDBG_OPT_FORCE_WIDE = 1, SDBG_OPT_NO_TABLE_COUNT = 2, SDBG_OPT_STABLE_FIRST_PASS = 3 };
+enum { SDBG_OPT_FORCE_WIDE = 1, SDBG_OPT_NO_TABLE_COUNT = 2, SDBG_OPT_STABLE_FIRST_PASS = 3, SDBG_OPT_NO_FUSED_EXTRACT = 4 };
 int sdbg_ctx_set_option(sdbg_ctx *ctx, int option, int value);
 const char *sdbg_strerror(int status);           /* static string */
 const char *sdbg_last_error(const sdbg_ctx *ctx); /* detail of the last failure on this ctx ("" if none) */

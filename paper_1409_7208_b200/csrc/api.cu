@@ -54,6 +54,7 @@ struct sdbg_ctx {
     bool timing = false;
     bool force_wide = false;   // SDBG_OPT_FORCE_WIDE (sdbg_ctx_set_option, include/sdbg.h)
     bool no_unstable = false;  // SDBG_OPT_STABLE_FIRST_PASS: the first radix pass uses the stable kernel like the others
+    bool no_fused = false;     // SDBG_OPT_NO_FUSED_EXTRACT: the keys are written in read order and the first top pass reads them back
     bool no_hash = false;      // SDBG_OPT_NO_TABLE_COUNT: every record through every radix pass, then the sweeps of count.cu
     std::vector<EventPair> pending;
     std::vector<cudaEvent_t> free_events;
@@ -205,6 +206,7 @@ int sdbg_ctx_create(sdbg_ctx **out, int device, void *cuda_stream, void *workspa
     }
     if (radix_setup() != 0) { cudaGetLastError(); return SDBG_E_CUDA; }
     if (hash_setup() != 0) { cudaGetLastError(); return SDBG_E_CUDA; }
+    if (extract_scatter_setup() != 0) { cudaGetLastError(); return SDBG_E_CUDA; }
     sdbg_ctx *c = new sdbg_ctx();
     if (cudaHostAlloc(reinterpret_cast<void **>(&c->fetch_buf), kFetchBytes, cudaHostAllocMapped) != cudaSuccess) { cudaGetLastError(); delete c; return SDBG_E_CUDA; }
     c->device = device;
@@ -229,6 +231,7 @@ int sdbg_ctx_set_option(sdbg_ctx *ctx, int option, int value) {
         case SDBG_OPT_FORCE_WIDE: ctx->force_wide = value != 0; return SDBG_OK;
         case SDBG_OPT_STABLE_FIRST_PASS: ctx->no_unstable = value != 0; return SDBG_OK;
         case SDBG_OPT_NO_TABLE_COUNT: ctx->no_hash = value != 0; return SDBG_OK;
+        case SDBG_OPT_NO_FUSED_EXTRACT: ctx->no_fused = value != 0; return SDBG_OK;
     }
     return ctx->fail(SDBG_E_INVAL, "unknown option");
 }

@@ -183,6 +183,11 @@ __global__ void __launch_bounds__(256) extract_kernel(ExtractArgs a, DevState *s
                 for (u32 jj = 0; jj < 16; ++jj) count_pos(16 + jj, __funnelshift_l(b2w, b1w, 2 * jj) >> 24);
             }
         }
+        if constexpr (shared4) {
+            // histogram-only call for the top passes (the pre-scan of the fused extract-and-scatter path): the position
+            // tables hold everything that is wanted, no key is made
+            if (!a.keys_out && !a.bucket_hist && !a.want_csum && bmin > 7u - T) continue;
+        }
         u32 vf = valid, vr = valid;   // per-strand keep masks
         if (FILTER && a.k >= 8) {
             // which keys fall into the range of partitions: only the top 16 bits of each key are needed
@@ -371,6 +376,140 @@ __global__ void __launch_bounds__(256) extract_kernel(ExtractArgs a, DevState *s
             if (v) atomicAdd(&a.digit_hist[i], (u64)v);
         }
     }
+}
+
+// ---- extraction fused with the first (unstable) radix pass --------------------------------------------------------------
+// One-word keys, dense range, default path (api_count.inc): the keys are not written in read order and re-read by the
+// first top pass; they go straight from the key maker into the 256 bins of that pass. The bin sizes come from a
+// histogram-only pre-scan of the packed reads (extract_kernel without output: position tables, 0.375 bytes per base).
+// The digit is key byte `t` from the top (t < floor(k / 4): a byte of node symbols only), so that for the window at slot p
+//   forward key: digit = symbol reversal of the 4-mer at slot p + k - 4 - 4t,   rc-strand key: complement of the 4-mer at
+//   slot p + 4t + 1  (the identity extract_kernel's position tables use).
+// Per tile of 4,096 slots (8 warps x 32 lanes x 16 slots; a lane owns half a group of 32 slots):
+//   A  digits of all valid windows counted by the plain 4-mer in two 256-entry tables (no key is made), folded into the
+//      tile's bin counts (reversal / complement of the index);
+//   B  one thread per bin: exclusive scan -> tile place of the bin; its run in the output is reserved with ONE atomicAdd
+//      on the bin's global cursor (the order of the records inside a bin is free: they are merged or sorted later);
+//   C  the keys are made, each takes the next place of its bin in shared memory (shared atomic), 
+//   D  and the tile leaves in bin order: place p goes to (reserved run of its bin) + (p - tile place of the bin), one
+//      coalesced run per bin.
+struct ScatterSmem {
+    static constexpr int THREADS = 256, TILE_GROUPS = 128, MAX_KEYS = TILE_GROUPS * 32 * 2;
+    static constexpr size_t kStage = 0;                                   // u64[MAX_KEYS]
+    static constexpr size_t kCntF = kStage + (size_t)MAX_KEYS * 8;        // u32[256] digits of forward keys by plain 4-mer
+    static constexpr size_t kCntR = kCntF + 1024;                         // u32[256] digits of rc-strand keys by plain 4-mer
+    static constexpr size_t kCur = kCntR + 1024;                          // u32[256] next free tile place of the bin
+    static constexpr size_t kOff = kCur + 1024;                           // u64[256] output index of tile place 0 if it were in this bin
+    static constexpr size_t kBytes = kOff + 2048;
+};
+
+template <int HALF>
+__device__ __forceinline__ void scatter_count_half(const KeyMaker<1> &km, u32 valid16, u64 S0f, u64 S1f, u64 S0r, u64 S1r,
+                                                   u32 *s_cntF, u32 *s_cntR) {
+#pragma unroll
+    for (u32 ii = 0; ii < 16; ++ii) {
+        constexpr u32 base = 16u * HALF;
+        const u32 j = base + ii;                          // window = slot j of the group; its 4-mers start at symbol j of S
+        const u32 f4 = j <= 28 ? (u32)(S0f >> (56 - 2 * j)) & 0xffu : (u32)(funnel(S0f, S1f, 2 * j) >> 56);
+        const u32 r4 = j <= 28 ? (u32)(S0r >> (56 - 2 * j)) & 0xffu : (u32)(funnel(S0r, S1r, 2 * j) >> 56);
+        if ((valid16 >> ii) & 1u) { atomicAdd(&s_cntF[f4], 1u); atomicAdd(&s_cntR[r4], 1u); }
+    }
+}
+
+template <int HALF>
+__device__ __forceinline__ void scatter_place_half(const KeyMaker<1> &km, u32 valid16, u32 dshift, u32 *s_cur, u64 *s_stage) {
+#pragma unroll
+    for (u32 ii = 0; ii < 16; ++ii) {
+        u64 f[1], r[1];
+        km.template keys_h<HALF>(ii, f, r);
+        if ((valid16 >> ii) & 1u) {
+            const u32 pf = atomicAdd(&s_cur[(u32)(f[0] >> dshift) & 0xffu], 1u);
+            s_stage[pf] = f[0];
+            const u32 pr = atomicAdd(&s_cur[(u32)(r[0] >> dshift) & 0xffu], 1u);
+            s_stage[pr] = r[0];
+        }
+    }
+}
+
+__global__ void __launch_bounds__(ScatterSmem::THREADS, 3) extract_scatter_kernel(ScatterArgs a) {
+    using L = ScatterSmem;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    u64 *s_stage = reinterpret_cast<u64 *>(smem_raw + L::kStage);
+    u32 *s_cntF = reinterpret_cast<u32 *>(smem_raw + L::kCntF), *s_cntR = reinterpret_cast<u32 *>(smem_raw + L::kCntR);
+    u32 *s_cur = reinterpret_cast<u32 *>(smem_raw + L::kCur);
+    u64 *s_off = reinterpret_cast<u64 *>(smem_raw + L::kOff);
+    __shared__ u32 s_wtot[8];
+    __shared__ u32 s_total;
+    const u32 tid = threadIdx.x, lane = tid & 31u, warp = tid >> 5;
+    const u32 half = warp >> 2;                          // warps 0-3: slots 0-15 of their groups, warps 4-7: slots 16-31
+    const u64 ngroups = a.n_slots / 32;
+    const u64 ntiles = (ngroups + L::TILE_GROUPS - 1) / L::TILE_GROUPS;
+    const u32 off_f = a.k - 4u - 4u * a.t, off_r = 4u * a.t + 1u, dshift = 56u - 8u * a.t;
+    s_cntF[tid] = 0; s_cntR[tid] = 0;
+    __syncthreads();
+    for (u64 tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
+        const u64 g = tile * L::TILE_GROUPS + 32u * (warp & 3u) + lane;
+        u32 valid16 = 0;
+        KeyMaker<1> km;
+        if (g < ngroups) valid16 = (valid_mask32(a.ends, g, a.k) >> (16u * half)) & 0xffffu;
+        const bool any = __any_sync(0xffffffffu, valid16 != 0);
+        if (any) km.load(a.words, g < ngroups ? g : 0, a.k);
+        // ---- A: digits by plain 4-mer
+        if (valid16) {
+            const u64 S0f = funnel(km.B[0], km.B[1], 2 * off_f), S1f = off_f ? km.B[1] << (2 * off_f) : km.B[1];
+            const u64 S0r = funnel(km.B[0], km.B[1], 2 * off_r), S1r = km.B[1] << (2 * off_r);
+            if (half) scatter_count_half<1>(km, valid16, S0f, S1f, S0r, S1r, s_cntF, s_cntR);
+            else scatter_count_half<0>(km, valid16, S0f, S1f, S0r, S1r, s_cntF, s_cntR);
+        }
+        __syncthreads();
+        // ---- B: bin tid: count (fold), exclusive scan over the bins, reservation of its run in the output
+        {
+            const u32 rev = ((tid & 0x03u) << 6) | ((tid & 0x0cu) << 2) | ((tid & 0x30u) >> 2) | ((tid & 0xc0u) >> 6);
+            const u32 c = s_cntF[rev] + s_cntR[~tid & 0xffu];
+            const u32 incl = warp_incl_scan_add(c);
+            if (lane == 31) s_wtot[warp] = incl;
+            __syncthreads();
+            u32 start = incl - c;
+            for (u32 w = 0; w < warp; ++w) start += s_wtot[w];
+            s_cur[tid] = start;
+            u64 gpos = 0;
+            if (c) gpos = atomicAdd(&a.bin_cursor[tid], (u64)c);
+            s_off[tid] = gpos - start;
+            if (tid == 255) s_total = start + c;
+            __syncthreads();
+            s_cntF[tid] = 0; s_cntR[tid] = 0;            // for the next tile (their readers are past the barrier above)
+        }
+        // ---- C: keys into their bins in shared memory
+        if (valid16) {
+            if (half) scatter_place_half<1>(km, valid16, dshift, s_cur, s_stage);
+            else scatter_place_half<0>(km, valid16, dshift, s_cur, s_stage);
+        }
+        __syncthreads();
+        // ---- D: the tile leaves in bin order
+        const u32 total = s_total;
+        for (u32 p = tid; p < total; p += L::THREADS) {
+            const u64 key = s_stage[p];
+            const u64 dst = s_off[(u32)(key >> dshift) & 0xffu] + p;
+            if (dst < a.out_cap) a.keys_out[dst] = key;
+        }
+        __syncthreads();
+    }
+}
+
+int extract_scatter_setup() {
+    return (int)cudaFuncSetAttribute(extract_scatter_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ScatterSmem::kBytes);
+}
+
+bool extract_scatter_supported(u32 k, u32 t) { return k >= 8 && k <= 31 && t < k / 4; }
+
+int launch_extract_scatter(const ScatterArgs &a, cudaStream_t s) {
+    const u64 ngroups = a.n_slots / 32;
+    if (ngroups == 0) return 0;
+    if (!extract_scatter_supported(a.k, a.t)) return (int)cudaErrorInvalidValue;
+    const u64 ntiles = (ngroups + ScatterSmem::TILE_GROUPS - 1) / ScatterSmem::TILE_GROUPS;
+    const u64 cap = (u64)num_sms() * 3;
+    extract_scatter_kernel<<<(unsigned)(ntiles < cap ? ntiles : cap), ScatterSmem::THREADS, ScatterSmem::kBytes, s>>>(a);
+    return (int)cudaGetLastError();
 }
 
 template <int W>

@@ -53,6 +53,19 @@ struct ExtractArgs {
 };
 int launch_extract(const ExtractArgs &a, DevState *st, cudaStream_t s);
 
+// extraction fused with the first radix pass (extract.cu): one-word keys of a dense range scattered into the 256 bins of
+// key byte t (0 = most significant); bin_cursor[b] = first output place of bin b, advanced by the kernel
+struct ScatterArgs {
+    const u64 *words, *ends;
+    u64 n_slots;
+    u32 k, t;
+    u64 *keys_out; u64 out_cap;
+    u64 *bin_cursor;              // u64[256], exclusive prefix of the bin sizes (from the histogram pre-scan)
+};
+int extract_scatter_setup();
+bool extract_scatter_supported(u32 k, u32 t);
+int launch_extract_scatter(const ScatterArgs &a, cudaStream_t s);
+
 // exclusive scan of each pass's 256-bin histogram, in place (u64)
 void launch_scan_hist(u64 *digit_hist, int n_passes, cudaStream_t s);
 

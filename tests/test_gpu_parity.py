@@ -378,11 +378,11 @@ def test_table_count_path_and_its_way_back(k):
         assert_matches_oracle(res, orc, check_stats=True)
         n_hash = _radix_launches(res)
         if completes:
-            assert 1 <= n_hash < P, (name, k, d, n_hash)              # top passes only
+            assert 0 <= n_hash < P - 1, (name, k, d, n_hash)           # top passes only, the first of them fused with extraction
         else:
-            assert P < n_hash < 2 * P, (name, k, d, n_hash)            # top passes, then all passes (the way back)
+            assert P <= n_hash < 2 * P, (name, k, d, n_hash)           # top passes, then all passes (the way back)
         import paper_1409_7208_b200 as sd
-        for opt in (sd.SDBG_OPT_NO_TABLE_COUNT, sd.SDBG_OPT_STABLE_FIRST_PASS):
+        for opt in (sd.SDBG_OPT_NO_TABLE_COUNT, sd.SDBG_OPT_STABLE_FIRST_PASS, sd.SDBG_OPT_NO_FUSED_EXTRACT):
             res2 = run_gpu(reads, k, d, checksums=False, options=[opt])
             assert_matches_oracle(res2, orc, check_stats=True)
             if opt == sd.SDBG_OPT_NO_TABLE_COUNT:
