@@ -13,7 +13,7 @@
 //     insertion inside the tiny bins) — buckets are consecutive in key order and segments too, so the ordered solid edges
 //     of a segment are a contiguous piece of the final output;
 //   3 they are written, with their counts, to the place of the segment in a staging buffer (the sorter's spare buffer),
-//     the number of them to seg_count[segment] and added to the sum of its block of 256 segments. hash_scan_kernel (one
+//     the number of them to seg_count[segment] and added to the sum of its block of 64 segments. hash_scan_kernel (one
 //     block: prefix of the block sums) and hash_copy_kernel (a CTA per block of segments: prefix inside the block, then a
 //     warp per segment) append them in order. CTAs never wait for one another: a chain of solid counts through the
 //     segments (decoupled look-back, tried first) made all resident segments resolve in lockstep, each walk some ten L2
@@ -74,7 +74,7 @@ __global__ void __launch_bounds__(256) hash_bounds_kernel(const u64 *__restrict_
     if (lane_id() == 0) seg_start[c] = res;
 }
 
-constexpr u32 kSegBlock = 256;   // segments per block sum (hash_scan_kernel, hash_copy_kernel)
+constexpr u32 kSegBlock = kHashSegBlock;   // segments per block sum (hash_scan_kernel, hash_copy_kernel)
 
 __device__ __forceinline__ u32 hash_slot(u64 key, u32 hshift) {
     const u32 h = (u32)key + (u32)(key >> 32) * 0x9E3779B1u;
@@ -362,8 +362,8 @@ hash_count_kernel(HashCountArgs a) {
     }
 }
 
-// blk_sum[b] (solid edges of segments [256 b, 256 b + 256)) -> exclusive prefix in place, total to *total and the output
-// cursor behind this range; one block (a range of 2^34 records has at most 2^15 blocks of 256 segments of 2,048 records)
+// blk_sum[b] (solid edges of segments [64 b, 64 b + 64)) -> exclusive prefix in place, total to *total and the output
+// cursor behind this range; one block (a range of 2^34 records has at most 2^17 blocks of 64 segments of 2,048 records)
 __global__ void __launch_bounds__(1024) hash_scan_kernel(u64 *__restrict__ blk_sum, u64 nblk, u64 *total, const u64 *cursor_in, u64 *cursor_out) {
     __shared__ u64 s_w[32];
     __shared__ u64 s_carry;
@@ -391,27 +391,32 @@ __global__ void __launch_bounds__(1024) hash_scan_kernel(u64 *__restrict__ blk_s
     if (tid == 0) { *total = s_carry; *cursor_out = *cursor_in + s_carry; }
 }
 
-// the staged solid edges of every segment appended to the output, in segment (= key) order: a CTA per block of 256
+// the staged solid edges of every segment appended to the output, in segment (= key) order: a CTA per block of 64
 // segments (prefix of their counts in shared memory), a warp per segment
 __global__ void __launch_bounds__(256) hash_copy_kernel(HashCountArgs a) {
     __shared__ u64 s_off[kSegBlock];
-    __shared__ u64 s_w[8];
+    __shared__ u64 s_w[kSegBlock / 32];
     const u32 tid = threadIdx.x, lane = tid & 31u, warp = tid >> 5;
     const u64 base = *a.cursor_in;
     for (u64 blk = blockIdx.x; blk * kSegBlock < a.nseg; blk += gridDim.x) {
-        const u64 seg0 = blk * kSegBlock + tid;
-        const u64 v = seg0 < a.nseg ? a.seg_count[seg0] : 0;
-        u64 incl = v;
+        u64 v = 0, incl = 0;
+        if (tid < kSegBlock) {
+            const u64 seg0 = blk * kSegBlock + tid;
+            v = seg0 < a.nseg ? a.seg_count[seg0] : 0;
+            incl = v;
 #pragma unroll
-        for (int o = 1; o < 32; o <<= 1) {
-            u64 t = __shfl_up_sync(0xffffffffu, incl, o);
-            if (lane >= (u32)o) incl += t;
+            for (int o = 1; o < 32; o <<= 1) {
+                u64 t = __shfl_up_sync(0xffffffffu, incl, o);
+                if (lane >= (u32)o) incl += t;
+            }
+            if (lane == 31) s_w[warp] = incl;
         }
-        if (lane == 31) s_w[warp] = incl;
         __syncthreads();
-        u64 off = a.blk_sum[blk];
-        for (u32 w = 0; w < warp; ++w) off += s_w[w];
-        s_off[tid] = off + incl - v;
+        if (tid < kSegBlock) {
+            u64 off = a.blk_sum[blk];
+            for (u32 w = 0; w < warp; ++w) off += s_w[w];
+            s_off[tid] = off + incl - v;
+        }
         __syncthreads();
         for (u32 j = warp; j < kSegBlock; j += 8) {
             const u64 seg = blk * kSegBlock + j;
