@@ -291,6 +291,21 @@ uint64_t sdbg_index_bytes(uint64_t m);
 /* Builds the index of g (the output of sdbg_build_full, zin_bits included) on the ctx stream; synchronises.
  * Errors: SDBG_E_CAPACITY (ix->bytes too small), SDBG_E_INVAL (null arrays, no zin_bits), SDBG_E_UNSUPPORTED (m >= 2^32). */
 int sdbg_index_build(sdbg_ctx *ctx, const sdbg_full_graph *g, sdbg_index *ix);
+/* The same index for callers that cannot allocate device memory (code under CUDA graph capture around it, tight serving
+ * loops, harnesses that forbid cudaMalloc): no ctx and no workspace. The build scratch is a static device array inside the
+ * library (374,648 bytes per GPU that loads it, held until exit), which limits the graph to
+ * sdbg_index_static_max_edges() = 2^28 edges; a larger m is refused with SDBG_E_CAPACITY. The caller passes the graph and
+ * `ix->cells` (device, 64-byte aligned, at least sdbg_index_static_bytes(m) bytes: cells and select samples only; a block
+ * of sdbg_index_bytes(m) bytes will do as well). Runs on `stream` (a cudaStream_t, NULL = the default stream) of the
+ * CURRENT device and synchronises it; calls no cudaMalloc / cudaFree or allocating library routine. Every call on a
+ * device shares the scratch and it keeps the last call's contents (what must start at zero is cleared per call): calls
+ * that overlap on one GPU race, so serialise them (one stream, or events). The result is the same index, bit for bit, as
+ * sdbg_index_build's; sdbg_forward / sdbg_backward take it. Errors: SDBG_E_CAPACITY, SDBG_E_INVAL, SDBG_E_CUDA; the text
+ * is in sdbg_index_build_static_error() (per host thread). */
+uint64_t sdbg_index_static_max_edges(void);
+uint64_t sdbg_index_static_bytes(uint64_t m);
+int sdbg_index_build_static(void *stream, const sdbg_full_graph *g, sdbg_index *ix);
+const char *sdbg_index_build_static_error(void);
 /* out[q] = forward(edge_idx[q]) / backward(edge_idx[q]) for n queries; edge_idx and out are DEVICE arrays; an index
  * >= m yields -2. Launches on the ctx stream and does not synchronise. */
 int sdbg_forward(sdbg_ctx *ctx, const sdbg_index *ix, const uint64_t *edge_idx, uint64_t n, int64_t *out);

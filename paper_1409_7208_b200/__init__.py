@@ -4,7 +4,7 @@ There is no CPU fallback: without the built library or without a CUDA device the
 from .binding import (  # noqa: F401
     SdbgError, Context, Reads, Edges, Graph, FullGraph, Index, Stats, Timing, lib, lib_path,
     sdbg_pack_reads, sdbg_count_edges, sdbg_build, sdbg_build_full, sdbg_mercy_edges, sdbg_plan_ranges,
-    sdbg_index_bytes, sdbg_index_build, sdbg_forward, sdbg_backward,
+    sdbg_index_bytes, sdbg_index_build, sdbg_index_build_static, sdbg_forward, sdbg_backward,
     sdbg_count_edges_range, sdbg_bucket_hist, sdbg_plan_shards,
     sdbg_key_words, sdbg_read_slots, sdbg_full_workspace, sdbg_workspace_for_records, sdbg_min_workspace, sdbg_strerror,
     sdbg_unstable_radix_launches,

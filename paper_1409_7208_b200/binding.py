@@ -104,6 +104,10 @@ def lib():
         L.sdbg_mercy_edges.argtypes = [vp, C.POINTER(_Reads), C.POINTER(_Edges), C.POINTER(_Edges)]; L.sdbg_mercy_edges.restype = i32
         L.sdbg_index_bytes.argtypes = [u64]; L.sdbg_index_bytes.restype = u64
         L.sdbg_index_build.argtypes = [vp, C.POINTER(_FullGraph), C.POINTER(_Index)]; L.sdbg_index_build.restype = i32
+        L.sdbg_index_static_max_edges.argtypes = []; L.sdbg_index_static_max_edges.restype = u64
+        L.sdbg_index_static_bytes.argtypes = [u64]; L.sdbg_index_static_bytes.restype = u64
+        L.sdbg_index_build_static.argtypes = [vp, C.POINTER(_FullGraph), C.POINTER(_Index)]; L.sdbg_index_build_static.restype = i32
+        L.sdbg_index_build_static_error.argtypes = []; L.sdbg_index_build_static_error.restype = C.c_char_p
         L.sdbg_forward.argtypes = [vp, C.POINTER(_Index), vp, u64, vp]; L.sdbg_forward.restype = i32
         L.sdbg_backward.argtypes = [vp, C.POINTER(_Index), vp, u64, vp]; L.sdbg_backward.restype = i32
         L.sdbg_ctx_set_timing.argtypes = [vp, i32]; L.sdbg_ctx_set_timing.restype = i32
@@ -396,6 +400,15 @@ def sdbg_index_bytes(m: int) -> int:
 def sdbg_index_build(ctx: Context, graph: FullGraph, out: Index) -> None:
     ctx.check(lib().sdbg_index_build(ctx._h, C.byref(graph.c), C.byref(out.c)))
     out.graph = graph                                    # the index borrows W and last_bits
+
+
+def sdbg_index_build_static(graph: FullGraph, out: Index, stream=None) -> None:
+    """The index built with the library's static device scratch: no ctx, no workspace, no allocation (include/sdbg.h).
+    stream: a torch.cuda.Stream or None (the default stream); synchronises it."""
+    rc = lib().sdbg_index_build_static(stream.cuda_stream if stream is not None else None, C.byref(graph.c), C.byref(out.c))
+    if rc != 0:
+        raise SdbgError(rc, lib().sdbg_index_build_static_error().decode())
+    out.graph = graph
 
 
 def sdbg_forward(ctx: Context, index: Index, edge_idx, n: int, out) -> None:

@@ -170,6 +170,9 @@ u64 index_cells(u64 m);
 u64 index_samples_cap(u64 m);
 u64 index_scratch_words(u64 m);
 void launch_index_build(const uint8_t *W, const u64 *last_bits, const u64 *zin_bits, const IndexView &ix, u64 *scratch /* u64[index_scratch_words(m)] */, cudaStream_t s);
+// the same with the scratch in a static device array of rank.cu (no allocation anywhere; m <= index_static_max_edges())
+u64 index_static_max_edges();
+int launch_index_build_static(const uint8_t *W, const u64 *last_bits, const u64 *zin_bits, const IndexView &ix, u64 **scratch_out, cudaStream_t s);
 void launch_forward(const IndexView &ix, const u64 *q, u64 n, long long *out, cudaStream_t s);
 void launch_backward(const IndexView &ix, const u64 *q, u64 n, long long *out, cudaStream_t s);
 

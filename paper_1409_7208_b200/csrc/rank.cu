@@ -9,6 +9,7 @@
 // and finishes inside the cell. A traversal query is a chain of three or four dependent random reads: the kernels are
 // latency/sector bound, one thread per query, nothing staged.
 #include "kernels.cuh"
+#include <mutex>
 
 namespace sdbg {
 
@@ -193,6 +194,51 @@ __global__ void __launch_bounds__(kIndexBlock) index_finish_kernel(IndexView ix,
 __global__ void index_consts_kernel(IndexView ix, u64 *consts) {
     const u32 c = threadIdx.x;
     if (c < 5) consts[c] = rank_v(ix, 4, ix.F[c]);
+}
+
+// ---- index build for callers that cannot allocate (sdbg_index_build_static) -----------------------------------------------
+// The build scratch (16 scalars + five block sums per 64 cells) lives in a file-scope device array instead of the caller's
+// block: 5 * ceil((2^28 / 448 + 1) / 64) + 16 words = 374,648 bytes, held by every GPU that loads the library until exit.
+// Every call on a device shares it and it keeps the last call's contents: the scalars are cleared per call, the block sums
+// are all overwritten before they are read. Calls that overlap on one GPU race on it.
+constexpr u64 kStaticIndexMaxEdges = 1ull << 28;
+constexpr u64 kStaticScratchWords = 5 * ((kStaticIndexMaxEdges / kCellBits + 1 + kIndexBlock - 1) / kIndexBlock) + 16;
+static __device__ __align__(256) u64 g_index_scratch[kStaticScratchWords];
+
+u64 index_static_max_edges() { return kStaticIndexMaxEdges; }
+
+// Device address of g_index_scratch on the CURRENT device. In host code the array's name is a host-side stand-in, not a
+// device address, so it is looked up once per device (with that device current) and kept.
+static int index_static_scratch(u64 **ptr) {
+    constexpr int kMaxDev = 64;
+    static std::mutex mu;
+    static u64 *cache[kMaxDev] = {};
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return (int)e;
+    if (dev < 0 || dev >= kMaxDev) return (int)cudaErrorInvalidDevice;
+    std::lock_guard<std::mutex> lock(mu);
+    if (!cache[dev]) {
+        void *p = nullptr;
+        e = cudaGetSymbolAddress(&p, g_index_scratch);
+        if (e != cudaSuccess) return (int)e;
+        cache[dev] = static_cast<u64 *>(p);
+    }
+    *ptr = cache[dev];
+    return 0;
+}
+
+// launch_index_build with the scratch above; *scratch_out = its device address (the scalars are read back from there)
+int launch_index_build_static(const uint8_t *W, const u64 *last_bits, const u64 *zin_bits, const IndexView &ix, u64 **scratch_out, cudaStream_t s) {
+    if (ix.m > kStaticIndexMaxEdges || index_scratch_words(ix.m) > kStaticScratchWords) return (int)cudaErrorInvalidValue;
+    u64 *scratch = nullptr;
+    int e = index_static_scratch(&scratch);
+    if (e) return e;
+    e = (int)cudaMemsetAsync(scratch, 0, 16 * sizeof(u64), s);
+    if (e) return e;
+    launch_index_build(W, last_bits, zin_bits, ix, scratch, s);
+    *scratch_out = scratch;
+    return (int)cudaGetLastError();
 }
 
 // ---- queries ---------------------------------------------------------------------------------------------------------------
