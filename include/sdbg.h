@@ -68,17 +68,20 @@ void sdbg_ctx_destroy(sdbg_ctx *ctx);
  *   SDBG_OPT_FORCE_WIDE        one-word-key ranges of any size take the code path of ranges of 2^32 records and more (wide
  *                              look-back words in the radix passes, 64-bit run lengths in the count sweeps)
  *   SDBG_OPT_NO_TABLE_COUNT    sdbg_count_edges sorts every record through every radix pass and counts by one sweep
- *                              (count.cu). Default for one-word keys and d >= 2: the records go through the most
- *                              significant passes only and are counted bucket by bucket in shared-memory tables
- *                              (hashcount.cu); whatever does not fit there (an over-long bucket, a full table) is redone
- *                              the plain way inside the same call
+ *                              (count.cu). Default for d >= 2: the records go through the most significant passes only
+ *                              and are counted bucket by bucket in shared-memory tables (hashcount.cu; keys of several
+ *                              words by a 64-bit fingerprint of the whole key, every record then compared with the one
+ *                              that installed its slot); whatever does not fit there (an over-long bucket, a full table,
+ *                              two keys with one fingerprint) is redone the plain way inside the same call
  *   SDBG_OPT_NO_FUSED_EXTRACT  on the default path the extractor writes the keys in read order and the first top pass reads
  *                              them back (default for one dense range of one-word keys, k >= 8: extraction is fused with
  *                              that pass, the keys go from the key maker straight into its 256 bins)
  *   SDBG_OPT_STABLE_FIRST_PASS the first radix pass of sdbg_count_edges' sorts uses the stable kernel like the others
  *                              (default: unstable, equal keys are merged afterwards)
+ *   SDBG_OPT_WEAK_FINGERPRINT  (tests) the fingerprint of a key of several words is its first word, so that keys which
+ *                              differ further down meet in one table slot and the check sends the range the plain way
  * Errors: SDBG_E_INVAL (null ctx, unknown option). */
-enum { SDBG_OPT_FORCE_WIDE = 1, SDBG_OPT_NO_TABLE_COUNT = 2, SDBG_OPT_STABLE_FIRST_PASS = 3, SDBG_OPT_NO_FUSED_EXTRACT = 4 };
+enum { SDBG_OPT_FORCE_WIDE = 1, SDBG_OPT_NO_TABLE_COUNT = 2, SDBG_OPT_STABLE_FIRST_PASS = 3, SDBG_OPT_NO_FUSED_EXTRACT = 4, SDBG_OPT_WEAK_FINGERPRINT = 5 };
 int sdbg_ctx_set_option(sdbg_ctx *ctx, int option, int value);
 const char *sdbg_strerror(int status);           /* static string */
 const char *sdbg_last_error(const sdbg_ctx *ctx); /* detail of the last failure on this ctx ("" if none) */

@@ -9,4 +9,5 @@ from .binding import (  # noqa: F401
     sdbg_key_words, sdbg_read_slots, sdbg_full_workspace, sdbg_workspace_for_records, sdbg_min_workspace, sdbg_strerror,
     sdbg_unstable_radix_launches,
     SDBG_SORTED, STATUS, SDBG_OPT_FORCE_WIDE, SDBG_OPT_NO_TABLE_COUNT, SDBG_OPT_STABLE_FIRST_PASS, SDBG_OPT_NO_FUSED_EXTRACT,
+    SDBG_OPT_WEAK_FINGERPRINT,
 )

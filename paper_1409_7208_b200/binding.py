@@ -19,7 +19,7 @@ SDBG_SORTED = 1
 SDBG_NUM_BUCKETS = 65536
 STATUS = {0: "SDBG_OK", -1: "SDBG_E_INVAL", -2: "SDBG_E_BADBASE", -3: "SDBG_E_CAPACITY", -4: "SDBG_E_WORKSPACE",
           -5: "SDBG_E_CUDA", -6: "SDBG_E_UNSUPPORTED"}
-SDBG_OPT_FORCE_WIDE, SDBG_OPT_NO_TABLE_COUNT, SDBG_OPT_STABLE_FIRST_PASS, SDBG_OPT_NO_FUSED_EXTRACT = 1, 2, 3, 4
+SDBG_OPT_FORCE_WIDE, SDBG_OPT_NO_TABLE_COUNT, SDBG_OPT_STABLE_FIRST_PASS, SDBG_OPT_NO_FUSED_EXTRACT, SDBG_OPT_WEAK_FINGERPRINT = 1, 2, 3, 4, 5
 T_CLASSES = ("pack", "extract", "radix", "count", "emit", "other", "table")
 
 

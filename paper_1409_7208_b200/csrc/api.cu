@@ -54,6 +54,7 @@ struct sdbg_ctx {
     bool timing = false;
     bool force_wide = false;   // SDBG_OPT_FORCE_WIDE (sdbg_ctx_set_option, include/sdbg.h)
     bool no_unstable = false;  // SDBG_OPT_STABLE_FIRST_PASS: the first radix pass uses the stable kernel like the others
+    bool weak_fp = false;      // SDBG_OPT_WEAK_FINGERPRINT (tests)
     bool no_fused = false;     // SDBG_OPT_NO_FUSED_EXTRACT: the keys are written in read order and the first top pass reads them back
     bool no_hash = false;      // SDBG_OPT_NO_TABLE_COUNT: every record through every radix pass, then the sweeps of count.cu
     std::vector<EventPair> pending;
@@ -150,10 +151,12 @@ bool is_device_ptr(const void *p) {
 
 // bytes of dynamic workspace a sort+count of n records needs (keys only)
 // records per look-back row of the sorter that handles W-word keys: the keys themselves (W = 1) or (word, index) pairs
-u64 sort_tile_records(u32 W) { return W == 1 ? radix_tile_records(1, false) : radix_tile_records(1, true); }
-// room behind the buffers of a one-word range for the scratch of the table-count path (api_count.inc hash_scratch_bytes:
+// records per radix tile, for the size of the look-back words: keys of several words go through pair passes (a key word
+// and an index) or, on the table-count path, through passes over whole records: the smaller tile of the two
+u64 sort_tile_records(u32 W) { return W == 1 ? radix_tile_records(1, false) : std::min(radix_tile_records(1, true), radix_tile_records(W, false)); }
+// room behind the buffers of a range for the scratch of the table-count path (api_count.inc hash_scratch_bytes:
 // segment borders and counts, 16 bytes per 2,048 records, block sums, a copy of the statistics)
-u64 table_slack(u64 n, u32 W) { return W == 1 ? align_up(n / 64) + kStatBytes + 16384 : 0; }
+u64 table_slack(u64 n, u32) { return align_up(n / 64) + kStatBytes + 16384; }
 u64 range_need(u64 n, u32 W) {
     const u64 K = 8ull * W;
     const u64 rt = sort_tile_records(W), ct = count_tile_records(W);
@@ -232,6 +235,7 @@ int sdbg_ctx_set_option(sdbg_ctx *ctx, int option, int value) {
         case SDBG_OPT_STABLE_FIRST_PASS: ctx->no_unstable = value != 0; return SDBG_OK;
         case SDBG_OPT_NO_TABLE_COUNT: ctx->no_hash = value != 0; return SDBG_OK;
         case SDBG_OPT_NO_FUSED_EXTRACT: ctx->no_fused = value != 0; return SDBG_OK;
+        case SDBG_OPT_WEAK_FINGERPRINT: ctx->weak_fp = value != 0; return SDBG_OK;
     }
     return ctx->fail(SDBG_E_INVAL, "unknown option");
 }

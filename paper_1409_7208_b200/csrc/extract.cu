@@ -237,11 +237,13 @@ __global__ void __launch_bounds__(256) extract_kernel(ExtractArgs a, DevState *s
             } else {
 #pragma unroll
                 for (int q = W - 1; q >= 0; --q) {
+                    if (W > 1 && q > 0 && a.hist_top) continue;      // (keys of several words) top passes only: bytes of word 0
                     u32 *hq = (q == W - 1) ? h_last : h_last + ((8 - b0) + 8 * (W - 2 - q) + b0) * kRadix;
                     const u32 lo = (u32)key[q], hi = (u32)(key[q] >> 32);
 #pragma unroll
                     for (int b = 0; b < 8; ++b) {
                         if (q == W - 1 && b < (int)bmin) continue;   // padding bytes of the last word (and passes not wanted): no row
+                        if (W > 1 && a.hist_top && b + (int)a.hist_top < 8) continue;
                         atomicAdd(&hq[b * kRadix + __byte_perm(b < 4 ? lo : hi, 0u, 0x4440u | (b & 3))], 1u);
                     }
                 }

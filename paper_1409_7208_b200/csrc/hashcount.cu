@@ -24,6 +24,7 @@
 // raises *overflow; the caller then sorts the range the plain way (api_count.inc), so the result is the same.
 #include "kernels.cuh"
 #include <type_traits>
+#include <cstdio>
 
 #ifndef SDBG_HASH_CASFIRST
 #define SDBG_HASH_CASFIRST 0   // 1: the home slot is probed with the CAS itself; 0: with a load, CAS only into empty slots
@@ -33,28 +34,28 @@ namespace sdbg {
 
 constexpr u64 kEmpty = ~0ull;   // an all-ones key (edge T...T at k = 31) is counted beside the table
 
-// first index i in [lo, hi] with (keys[i] >> shift) != t, where the predicate is monotone on [lo, hi) and taken as
+// first record i in [lo, hi] (records of W words, the first one compared) with (keys[i W] >> shift) != t, where the predicate is monotone on [lo, hi) and taken as
 // true at hi; one warp, 32-ary search (every lane returns the result)
-__device__ __forceinline__ u64 warp_first_other(const u64 *__restrict__ keys, u64 lo, u64 hi, u32 shift, u64 t) {
+__device__ __forceinline__ u64 warp_first_other(const u64 *__restrict__ keys, u32 W, u64 lo, u64 hi, u32 shift, u64 t) {
     const u32 lane = lane_id();
     while (hi - lo >= 32) {
         const u64 stride = (hi - lo + 31) / 32;
         u64 p = lo + (u64)(lane + 1) * stride - 1;      // probes lo+stride-1, lo+2*stride-1, ..., clamped to hi-1
         if (p > hi - 1) p = hi - 1;
-        const u32 b = __ballot_sync(0xffffffffu, (keys[p] >> shift) != t);
+        const u32 b = __ballot_sync(0xffffffffu, (keys[p * W] >> shift) != t);
         if (b == 0) { lo = hi; break; }                  // no record of [lo, hi) differs
         const u32 f = __ffs(b) - 1;                      // the answer lies behind probe f-1 and not behind probe f
         hi = __shfl_sync(0xffffffffu, p, f);
         lo = lo + (u64)f * stride;
     }
     const u64 p = lo + lane;
-    const u32 b = __ballot_sync(0xffffffffu, p < hi ? (keys[p] >> shift) != t : true);   // lane hi-lo <= 31 says true
+    const u32 b = __ballot_sync(0xffffffffu, p < hi ? (keys[p * W] >> shift) != t : true);   // lane hi-lo <= 31 says true
     return lo + (u64)(__ffs(b) - 1);
 }
 
 // seg_start[c], c in [0, nchunks]: the first bucket border at or after record c * chunk (n for c = nchunks). A bucket
 // that runs on for more than `window` records past the nominal place raises *overflow.
-__global__ void __launch_bounds__(256) hash_bounds_kernel(const u64 *__restrict__ keys, u64 n, u32 shift, u32 chunk, u32 window,
+__global__ void __launch_bounds__(256) hash_bounds_kernel(const u64 *__restrict__ keys, u32 W, u64 n, u32 shift, u32 chunk, u32 window,
                                                           u64 nchunks, u64 *__restrict__ seg_start, u32 *overflow) {
     const u64 c = (u64)blockIdx.x * 8 + (threadIdx.x >> 5);
     if (c > nchunks) return;
@@ -63,11 +64,11 @@ __global__ void __launch_bounds__(256) hash_bounds_kernel(const u64 *__restrict_
     if (c == 0) res = 0;
     else if (x >= n) res = n;
     else {
-        const u64 t = keys[x - 1] >> shift;
-        if ((keys[x] >> shift) != t) res = x;
+        const u64 t = keys[(x - 1) * W] >> shift;
+        if ((keys[x * W] >> shift) != t) res = x;
         else {
             const u64 lim = x + window < n ? x + window : n;
-            res = warp_first_other(keys, x, lim, shift, t);
+            res = warp_first_other(keys, W, x, lim, shift, t);
             if (res == lim && lim < n && lane_id() == 0) atomicOr(overflow, 1u);   // not a border (or unknown): give up
         }
     }
@@ -92,21 +93,61 @@ __device__ __forceinline__ void s_red_add(u32 addr, u32 v) {
     asm volatile("red.shared.add.u32 [%0+%2], %1;" ::"r"(addr), "r"(v), "n"(OFS) : "memory");
 }
 
+// ---- keys of W > 1 words ------------------------------------------------------------------------------------------------------
+// The table then holds a 64-bit FINGERPRINT of the whole key where a one-word key stands for itself, and beside it the place
+// (in the segment) of the record that installed it. Equal keys have equal fingerprints; that equal fingerprints are equal
+// keys is CHECKED for every record (a second read of the segment, from L2: the record is compared with the one that
+// installed its slot), and a mismatch raises *overflow like everything else that does not fit, so the result stays exact.
+template <int W>
+__device__ __forceinline__ u64 fingerprint(const u64 (&k)[W], bool weak) {
+    if constexpr (W == 1) return k[0];
+    // splitmix64 finaliser word by word (common.cuh mix_key): every step is a bijection with full avalanche. A cheaper chain
+    // of multiply-adds was measured first and DID meet two keys of config 4 in one value (multiplication carries a
+    // difference in the top bit nowhere): the check below caught it.
+    u64 h = weak ? k[0] : mix_key<W>(k);
+    return h == kEmpty ? kEmpty - 1ull : h;
+}
+template <int W>
+__device__ __forceinline__ void load_key(const u64 *__restrict__ src, u64 (&k)[W]) {   // src = first word of the record
+    if constexpr (W == 1) k[0] = ld_stream(src);
+    else if constexpr (W == 2) { const ulonglong2 v = *reinterpret_cast<const ulonglong2 *>(src); k[0] = v.x; k[1] = v.y; }
+    else if constexpr (W == 4) {
+        const ulonglong2 v0 = *reinterpret_cast<const ulonglong2 *>(src), v1 = *reinterpret_cast<const ulonglong2 *>(src + 2);
+        k[0] = v0.x; k[1] = v0.y; k[2] = v1.x; k[3] = v1.y;
+    } else {
+#pragma unroll
+        for (int q = 0; q < W; ++q) k[q] = src[q];
+    }
+}
+// a < b for two records of the same first word (the words behind it, from memory)
+template <int W>
+__device__ __forceinline__ bool rest_less(const u64 *__restrict__ ra, const u64 *__restrict__ rb) {
+#pragma unroll
+    for (int q = 1; q < W; ++q) { const u64 x = ra[q], y = rb[q]; if (x != y) return x < y; }
+    return false;
+}
+
 // WARPS x 32 threads; a warp holds U rows of 32 records at a time; TSMAX table slots (power of two), MAXSOLID sort
 // places, NB = 1024 bins. Counts are 16-bit halves of u32 words (a segment has at most window + chunk < 65,536 records).
 // The records of a segment are dealt to the warps in groups of U full rows (no lane is ever idle there, so the group
 // code has no predicates); the rows that do not fill a group and the partial last row go one by one.
-template <int WARPS, int MINB, int U, int TSMAX, int MAXSOLID, int CB>
+template <int W, int WARPS, int MINB, int U, int TSMAX, int MAXSOLID, int CB>
 __global__ void __launch_bounds__(WARPS * 32, MINB)
 hash_count_kernel(HashCountArgs a) {
     static_assert(CB == 2 || CB == 4, "counts are 16-bit halves of u32 words or u32 words");
     constexpr int THREADS = WARPS * 32;
+    constexpr bool MW = W > 1;
+    using rep_t = unsigned short;                                               // place of a record inside its segment
+    constexpr size_t kOffCnt = (size_t)TSMAX * 8, kOffLKey = kOffCnt + (size_t)TSMAX * CB, kOffLCnt = kOffLKey + (size_t)MAXSOLID * 8;
+    constexpr size_t kOffTRep = kOffLCnt + (size_t)MAXSOLID * 4, kOffLRep = kOffTRep + (MW ? (size_t)TSMAX * 2 : 0);
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    u64 *t_key = reinterpret_cast<u64 *>(smem_raw);                             // u64[TSMAX]
-    u32 *t_cnt = reinterpret_cast<u32 *>(smem_raw + (size_t)TSMAX * 8);         // CB = 2: u16[TSMAX] as u32 pairs; CB = 4: u32[TSMAX]
-    u64 *l_key = reinterpret_cast<u64 *>(smem_raw + (size_t)TSMAX * (8 + CB));  // u64[MAXSOLID]
-    u32 *l_cnt = reinterpret_cast<u32 *>(smem_raw + (size_t)TSMAX * (8 + CB) + (size_t)MAXSOLID * 8);
-    __shared__ u32 s_ones, s_full, s_nsolid, s_distinct;
+    u64 *t_key = reinterpret_cast<u64 *>(smem_raw);                             // u64[TSMAX]: key (W = 1) or fingerprint
+    u32 *t_cnt = reinterpret_cast<u32 *>(smem_raw + kOffCnt);                   // CB = 2: u16[TSMAX] as u32 pairs; CB = 4: u32[TSMAX]
+    u64 *l_key = reinterpret_cast<u64 *>(smem_raw + kOffLKey);                  // u64[MAXSOLID]: first key word
+    u32 *l_cnt = reinterpret_cast<u32 *>(smem_raw + kOffLCnt);
+    rep_t *t_rep = reinterpret_cast<rep_t *>(smem_raw + kOffTRep);              // (W > 1) rep_t[TSMAX]: who installed the slot
+    rep_t *l_rep = reinterpret_cast<rep_t *>(smem_raw + kOffLRep);              // (W > 1) rep_t[MAXSOLID]
+    __shared__ u32 s_ones, s_full, s_nsolid, s_distinct, s_clash;
     __shared__ u64 s_sum, s_look[2][3], s_krange[2];
     __shared__ u32 s_w[WARPS];
     const u32 tid = threadIdx.x, lane = tid & 31u, warp = tid >> 5;
@@ -130,12 +171,12 @@ hash_count_kernel(HashCountArgs a) {
     // full groups of the segment [bs, be) (none for the segment that ends with the last record of all: it alone can hold
     // the all-ones key, which is counted beside the table by the row-by-row code)
     auto groups_of = [&](u64 bs, u64 be) { return be <= bs || be == a.n ? 0u : ((u32)(be - bs) >> 5) / (u32)U; };
-    u64 cur[U];
-    auto load_group = [&](u64 (&k)[U], const u64 *src) {   // rows src[32 u + lane]
+    u64 cur[U][W];
+    auto load_group = [&](u64 (&k)[U][W], const u64 *src) {   // records src + (32 u + lane) W
 #pragma unroll
-        for (int u = 0; u < U; ++u) k[u] = ld_stream(src + 32 * u + lane);
+        for (int u = 0; u < U; ++u) load_key<W>(src + (size_t)(32 * u + lane) * W, k[u]);
     };
-    if (warp < groups_of(s, e)) load_group(cur, a.keys + s + (u64)warp * (32 * U));
+    if (warp < groups_of(s, e)) load_group(cur, a.keys + (s + (u64)warp * (32 * U)) * W);
 
     for (u32 it = 0;; ++it) {
         const u32 m = e > s ? (u32)(e - s) : 0u;         // a segment has fewer than 2^16 records
@@ -150,12 +191,12 @@ hash_count_kernel(HashCountArgs a) {
             for (u32 i = tid; i < TS * CB / 16; i += THREADS) c4[i] = zero;
         }
         u64 la_seg = 0, la_s = 0, la_e = 0;              // (thread 0) the segment of the iteration after the next one
-        u64 kf = 0, kl = 0;                              // (thread 32) first and last record of this segment
+        u64 kf = 0, kl = 0;                              // (thread 32) first word of the first and of the last record
         if (tid == 0) {
-            s_ones = 0; s_full = 0; s_nsolid = 0; s_distinct = 0; s_sum = 0;
+            s_ones = 0; s_full = 0; s_nsolid = 0; s_distinct = 0; s_sum = 0; s_clash = 0;
             la_seg = atomicAdd(a.ticket, 1u);          // consumed behind the insert phase: nothing waits for it here
         }
-        if (tid == 32 % THREADS && m) { kf = a.keys[s]; kl = a.keys[e - 1]; }
+        if (tid == 32 % THREADS && m) { kf = a.keys[s * W]; kl = a.keys[(e - 1) * W]; }
         __syncthreads();
 
         // ---- 1: insert ---------------------------------------------------------------------------------------------------
@@ -166,55 +207,61 @@ hash_count_kernel(HashCountArgs a) {
             if constexpr (CB == 2) s_red_add<TSMAX * 8>(tkey_s + ((a8 >> 2) & ~3u), (a8 & 8u) ? 0x10000u : 1u);
             else s_red_add<TSMAX * 8>(tkey_s + (a8 >> 1), 1u);
         };
-        // NR rows held by the warp: first the home slot of every record (one CAS that installs the key or returns what
-        // is there, no loop), then ONE probing loop for the records whose home slot holds another key
-        auto insert_rows = [&](auto nr_tag, const u64 *k, bool valid) {
+        // NR rows held by the warp (row r = records i0 + 32 r + lane of the segment): first the home slot of every record
+        // (one CAS that installs the key or returns what is there, no loop), then ONE probing loop for the records whose
+        // home slot holds another key
+        auto insert_rows = [&](auto nr_tag, const u64 (*k)[W], u32 i0, bool valid) {
             constexpr int NR = decltype(nr_tag)::value;
-            u64 old[NR]; u32 a8[NR];
+            u64 old[NR], f[NR]; u32 a8[NR];
 #pragma unroll
             for (int r = 0; r < NR; ++r) {
-                a8[r] = hash_slot(k[r], hshift) << 3;
-                old[r] = k[r];
-                if (NR > 1 || valid) old[r] = s_cas64(tkey_s + a8[r], kEmpty, k[r]);
+                f[r] = fingerprint<W>(k[r], a.weak_fp);
+                a8[r] = hash_slot(f[r], hshift) << 3;
+                old[r] = f[r];
+                if (NR > 1 || valid) old[r] = s_cas64(tkey_s + a8[r], kEmpty, f[r]);
             }
             u32 pend = 0;
 #pragma unroll
             for (int r = 0; r < NR; ++r) {
                 const bool emp = old[r] == kEmpty;
                 if (NR > 1 || valid) {
-                    if (emp || old[r] == k[r]) cnt_add(a8[r]); else pend |= 1u << r;
+                    if (emp || old[r] == f[r]) cnt_add(a8[r]); else pend |= 1u << r;
+                    if (MW && emp) t_rep[a8[r] >> 3] = (rep_t)(i0 + 32u * (u32)r + lane);
                     created += emp;
                 }
             }
             if (pend) {
-                u64 key = 0; u32 b8 = 0, probes = 0;
+                u64 key = 0; u32 b8 = 0, probes = 0, who = 0;
                 bool have = false;
                 for (;;) {
                     if (!have) {
                         if (!pend) break;
                         const u32 r = (u32)__ffs(pend) - 1u;
                         pend &= pend - 1u;
-                        key = k[0]; b8 = a8[0];
+                        key = f[0]; b8 = a8[0];
 #pragma unroll
-                        for (int q = 1; q < NR; ++q) if (r == (u32)q) { key = k[q]; b8 = a8[q]; }
+                        for (int q = 1; q < NR; ++q) if (r == (u32)q) { key = f[q]; b8 = a8[q]; }
+                        who = i0 + 32u * r + lane;
                         probes = 0; have = true;
                     }
                     b8 = (b8 + 8u) & mask8;
                     const u64 o = s_cas64(tkey_s + b8, kEmpty, key);
-                    if (o == kEmpty || o == key) { cnt_add(b8); created += o == kEmpty; have = false; }
-                    else if (++probes >= TS) { s_full = 1; have = false; }
+                    if (o == kEmpty || o == key) {
+                        cnt_add(b8); created += o == kEmpty; have = false;
+                        if (MW && o == kEmpty) t_rep[b8 >> 3] = (rep_t)who;
+                    } else if (++probes >= TS) { s_full = 1; have = false; }
                 }
             }
         };
         const u32 G = groups_of(s, e);
         {
-            u64 nxt[U];
+            u64 nxt[U][W];
             for (u32 g = warp; g < G; g += 2 * WARPS) {  // two groups per round: one is inserted while the other arrives
                 const bool more = g + WARPS < G;
-                if (more) load_group(nxt, a.keys + s + (u64)(g + WARPS) * (32 * U));
-                insert_rows(std::integral_constant<int, U>{}, cur, true);
-                if (g + 2 * WARPS < G) load_group(cur, a.keys + s + (u64)(g + 2 * WARPS) * (32 * U));
-                if (more) insert_rows(std::integral_constant<int, U>{}, nxt, true);
+                if (more) load_group(nxt, a.keys + (s + (u64)(g + WARPS) * (32 * U)) * W);
+                insert_rows(std::integral_constant<int, U>{}, cur, g * (32u * U), true);
+                if (g + 2 * WARPS < G) load_group(cur, a.keys + (s + (u64)(g + 2 * WARPS) * (32 * U)) * W);
+                if (more) insert_rows(std::integral_constant<int, U>{}, nxt, (g + WARPS) * (32u * U), true);
             }
         }
         {   // the rows behind the last full group, and the partial last row: x-th of them belongs to warp (G + x) % WARPS
@@ -222,21 +269,54 @@ hash_count_kernel(HashCountArgs a) {
             for (u32 x = (warp + WARPS - G % WARPS) % WARPS; x < nx; x += WARPS) {
                 const u32 i = (row0 + x) * 32u + lane;
                 const bool valid = i < m;
-                u64 key = valid ? ld_stream(a.keys + s + i) : 0ull;
-                if (last_seg && valid && key == kEmpty) { atomicAdd(&s_ones, 1u); insert_rows(std::integral_constant<int, 1>{}, &key, false); }
-                else insert_rows(std::integral_constant<int, 1>{}, &key, valid);
+                u64 key[1][W];
+#pragma unroll
+                for (int q = 0; q < W; ++q) key[0][q] = 0ull;
+                if (valid) load_key<W>(a.keys + (s + i) * W, key[0]);
+                if (!MW && last_seg && valid && key[0][0] == kEmpty) { atomicAdd(&s_ones, 1u); insert_rows(std::integral_constant<int, 1>{}, key, (row0 + x) * 32u, false); }
+                else insert_rows(std::integral_constant<int, 1>{}, key, (row0 + x) * 32u, valid);
             }
         }
         // the first records of my next segment are on their way while this one is finished (its bounds came an iteration ago)
         const u64 next = s_look[(it + 1) & 1][0], ns_ = s_look[(it + 1) & 1][1], ne_ = s_look[(it + 1) & 1][2];
-        if (next < nseg && warp < groups_of(ns_, ne_)) load_group(cur, a.keys + ns_ + (u64)warp * (32 * U));
+        if (!MW && next < nseg && warp < groups_of(ns_, ne_)) load_group(cur, a.keys + (ns_ + (u64)warp * (32 * U)) * W);
         if (created) atomicAdd(&s_distinct, created);
         if (tid == 32 % THREADS) { s_krange[0] = kf >> a.top_shift; s_krange[1] = kl >> a.top_shift; }
         __syncthreads();
         if (tid == 0) bounds_of(la_seg, la_s, la_e);     // stored at the end of the iteration
         const u64 kfirst = s_krange[0], klast = s_krange[1];
-        const bool full = s_full != 0;
+        bool full = s_full != 0;
         if (full && tid == 0) atomicOr(a.overflow, 2u);
+
+        // ---- 1b (W > 1): every record against the one that installed its slot -------------------------------------------------------
+        if constexpr (MW) {
+            if (!full) {
+                for (u32 i = tid; i < m; i += THREADS) {
+                    u64 k[W];
+                    load_key<W>(a.keys + (s + i) * W, k);
+                    const u64 f = fingerprint<W>(k, a.weak_fp);
+                    u32 b8 = hash_slot(f, hshift) << 3;
+                    while (t_key[b8 >> 3] != f) b8 = (b8 + 8u) & mask8;       // it is there: the table was not full
+                    const u32 rep = t_rep[b8 >> 3];
+                    if (rep != i) {
+                        u64 o[W];
+                        load_key<W>(a.keys + (s + rep) * W, o);
+                        bool same = true;
+#pragma unroll
+                        for (int q = 0; q < W; ++q) same = same && o[q] == k[q];
+#ifdef SDBG_HASH_DEBUG
+                        if (!same && atomicAdd(&s_clash, 1u) == 0)
+                            printf("clash: seg %llu s %llu m %u i %u rep %u f %llx | %llx %llx %llx %llx | %llx %llx %llx %llx | frep %llx\n", seg, s, m, i, rep, f,
+                                   k[0], k[W > 1 ? 1 : 0], k[W > 2 ? 2 : 0], k[W - 1], o[0], o[W > 1 ? 1 : 0], o[W > 2 ? 2 : 0], o[W - 1], fingerprint<W>(o, a.weak_fp));
+#endif
+                        if (!same) s_clash = 1;
+                    }
+                }
+            }
+            if (next < nseg && warp < groups_of(ns_, ne_)) load_group(cur, a.keys + (ns_ + (u64)warp * (32 * U)) * W);
+            __syncthreads();
+            if (s_clash) { full = true; if (tid == 0) atomicOr(a.overflow, 16u); }
+        }
 
         // ---- 2: the solid slots, compacted to this iteration's list ------------------------------------------------------------
         u64 sum = 0;
@@ -264,7 +344,11 @@ hash_count_kernel(HashCountArgs a) {
                     if (wi == 3) wq = wd[3];
                     const u32 c = CB == 2 ? (wq >> ((q & 1u) * 16u)) & 0xffffu : wq;
                     const u32 p = atomicAdd(&s_nsolid, 1u);
-                    if (p < (u32)MAXSOLID) { l_key[p] = t_key[v * SPV + q]; l_cnt[p] = c; }
+                    if (p < (u32)MAXSOLID) {
+                        if constexpr (MW) { const u32 rep = t_rep[v * SPV + q]; l_rep[p] = (rep_t)rep; l_key[p] = a.keys[(s + rep) * W]; }
+                        else l_key[p] = t_key[v * SPV + q];
+                        l_cnt[p] = c;
+                    }
                     sum += c;
                 }
             }
@@ -297,11 +381,12 @@ hash_count_kernel(HashCountArgs a) {
         //          entries, which the owner of the bin puts in order by insertion. The table is dead: bins and the ordered
         //          entries live in its place. ---------------------------------------------------------------------------------------
         constexpr int NB = 1024, Q = NB / THREADS, QE = MAXSOLID / THREADS;   // bins per thread; list entries per thread
-        static_assert(NB % THREADS == 0 && MAXSOLID % THREADS == 0 && (size_t)NB * 4 <= (size_t)TSMAX * CB && (size_t)MAXSOLID * 12 <= (size_t)TSMAX * 8, "layout");
+        static_assert(NB % THREADS == 0 && MAXSOLID % THREADS == 0 && (size_t)NB * 4 <= (size_t)TSMAX * CB && (size_t)MAXSOLID * 14 <= (size_t)TSMAX * 8, "layout");
         if (ns) {
             u32 *bins = t_cnt;
             u64 *o_key = t_key;
             u32 *o_cnt = reinterpret_cast<u32 *>(t_key + MAXSOLID);
+            rep_t *o_rep = reinterpret_cast<rep_t *>(o_cnt + MAXSOLID);
             const u64 k0 = kfirst << a.top_shift;
             const u64 rm1 = ((klast - kfirst + 1ull) << a.top_shift) - 1ull;  // largest offset inside the segment's buckets
             const int sh0 = 54 - __clzll((long long)rm1), sh = sh0 > 0 ? sh0 : 0;   // (rm1 >> sh) < 1024
@@ -333,27 +418,50 @@ hash_count_kernel(HashCountArgs a) {
 #pragma unroll
             for (int q = 0; q < QE; ++q) {
                 const u32 i = tid + q * THREADS;
-                if (i < ns) { const u32 p = bins[myb[q]] + myr[q]; o_key[p] = l_key[i]; o_cnt[p] = l_cnt[i]; }
+                if (i < ns) {
+                    const u32 p = bins[myb[q]] + myr[q];
+                    o_key[p] = l_key[i]; o_cnt[p] = l_cnt[i];
+                    if constexpr (MW) o_rep[p] = l_rep[i];
+                }
             }
             __syncthreads();
             {
+                const u64 *recs = a.keys + s * W;
                 u32 b0 = base0;
 #pragma unroll
                 for (int q = 0; q < Q; ++q) {
                     for (u32 x = 1; x < c[q]; ++x) {                           // insertion sort of places [b0, b0 + c)
                         const u64 kx = o_key[b0 + x]; const u32 cx = o_cnt[b0 + x];
+                        const u32 rx = MW ? o_rep[b0 + x] : 0u;
                         u32 y = x;
-                        while (y > 0 && o_key[b0 + y - 1] > kx) { o_key[b0 + y] = o_key[b0 + y - 1]; o_cnt[b0 + y] = o_cnt[b0 + y - 1]; --y; }
+                        while (y > 0) {
+                            const u64 ky = o_key[b0 + y - 1];
+                            bool gt = ky > kx;           // entry y - 1 > entry x
+                            if constexpr (MW) { if (ky == kx) gt = rest_less<W>(recs + (size_t)rx * W, recs + (size_t)o_rep[b0 + y - 1] * W); }
+                            if (!gt) break;
+                            o_key[b0 + y] = ky; o_cnt[b0 + y] = o_cnt[b0 + y - 1];
+                            if constexpr (MW) o_rep[b0 + y] = o_rep[b0 + y - 1];
+                            --y;
+                        }
                         o_key[b0 + y] = kx; o_cnt[b0 + y] = cx;
+                        if constexpr (MW) o_rep[b0 + y] = (rep_t)rx;
                     }
                     b0 += c[q];
                 }
             }
             __syncthreads();
-            // staging (8 bytes per record, the sorter's spare buffer): the segment owns places [s, e); its ns <= (e - s) / d
+            // staging (8 W bytes per record, the sorter's spare buffer): the segment owns places [s, e); its ns <= (e - s) / d
             // solid keys (d >= 2) fill the first half at most, their u32 counts start at the middle place
-            u32 *stage_cnt = reinterpret_cast<u32 *>(a.stage_keys + s + ((m + 1u) >> 1));
-            for (u32 i = tid; i < ns; i += THREADS) { a.stage_keys[s + i] = o_key[i]; stage_cnt[i] = o_cnt[i]; }
+            u32 *stage_cnt = reinterpret_cast<u32 *>(a.stage_keys + (s + ((m + 1u) >> 1)) * W);
+            for (u32 i = tid; i < ns; i += THREADS) {
+                if constexpr (MW) {
+                    u64 k[W];
+                    load_key<W>(a.keys + (s + o_rep[i]) * W, k);
+#pragma unroll
+                    for (int q = 0; q < W; ++q) a.stage_keys[(s + i) * W + q] = k[q];
+                } else a.stage_keys[s + i] = o_key[i];
+                stage_cnt[i] = o_cnt[i];
+            }
         }
         if (next >= nseg) break;
         if (tid == 0) { s_look[it & 1][0] = la_seg; s_look[it & 1][1] = la_s; s_look[it & 1][2] = la_e; }
@@ -424,29 +532,31 @@ __global__ void __launch_bounds__(256) hash_copy_kernel(HashCountArgs a) {
             const u64 cnt = a.seg_count[seg];
             if (cnt == 0) continue;
             const u64 s = a.seg_start[seg], e = a.seg_start[seg + 1];
-            const u32 *stage_cnt = reinterpret_cast<const u32 *>(a.stage_keys + s + ((e - s + 1) >> 1));
+            const u32 W = a.W ? a.W : 1u;
+            const u32 *stage_cnt = reinterpret_cast<const u32 *>(a.stage_keys + (s + ((e - s + 1) >> 1)) * W);
             const u64 pos0 = base + s_off[j];
-            for (u64 i = lane; i < cnt; i += 32)
-                if (pos0 + i < a.out_cap) { a.out_keys[pos0 + i] = a.stage_keys[s + i]; a.out_mult[pos0 + i] = stage_cnt[i]; }
+            const u64 room = pos0 < a.out_cap ? a.out_cap - pos0 : 0, take = cnt < room ? cnt : room;
+            for (u64 i = lane; i < take * W; i += 32) a.out_keys[pos0 * W + i] = a.stage_keys[s * W + i];
+            for (u64 i = lane; i < take; i += 32) a.out_mult[pos0 + i] = stage_cnt[i];
         }
         __syncthreads();
     }
 }
 
 // shapes: long buckets (chunk 4,096: one or two buckets per segment) and short ones (chunk 2,048: many buckets per segment)
-template <int WARPS, int MINB, int U, int TSMAX, int MAXSOLID, int CB>
+template <int W, int WARPS, int MINB, int U, int TSMAX, int MAXSOLID, int CB>
 struct HashShape {
     static constexpr int THREADS = WARPS * 32;
-    static constexpr size_t kSmem = (size_t)TSMAX * (8 + CB) + (size_t)MAXSOLID * 12;
+    static constexpr size_t kSmem = (size_t)TSMAX * (8 + CB) + (size_t)MAXSOLID * 12 + (W > 1 ? (size_t)TSMAX * 2 + (size_t)MAXSOLID * 2 : 0);
     static int setup(int *blocks_per_sm) {
-        int e = (int)cudaFuncSetAttribute(hash_count_kernel<WARPS, MINB, U, TSMAX, MAXSOLID, CB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmem);
+        int e = (int)cudaFuncSetAttribute(hash_count_kernel<W, WARPS, MINB, U, TSMAX, MAXSOLID, CB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmem);
         if (e) return e;
-        return (int)cudaOccupancyMaxActiveBlocksPerMultiprocessor(blocks_per_sm, hash_count_kernel<WARPS, MINB, U, TSMAX, MAXSOLID, CB>, THREADS, kSmem);
+        return (int)cudaOccupancyMaxActiveBlocksPerMultiprocessor(blocks_per_sm, hash_count_kernel<W, WARPS, MINB, U, TSMAX, MAXSOLID, CB>, THREADS, kSmem);
     }
     static int launch(const HashCountArgs &a, int blocks_per_sm, cudaStream_t s) {
         u64 g = (u64)num_sms() * (u64)(blocks_per_sm > 0 ? blocks_per_sm : 1);
         if (g > a.nseg) g = a.nseg;
-        hash_count_kernel<WARPS, MINB, U, TSMAX, MAXSOLID, CB><<<(unsigned)g, THREADS, kSmem, s>>>(a);
+        hash_count_kernel<W, WARPS, MINB, U, TSMAX, MAXSOLID, CB><<<(unsigned)g, THREADS, kSmem, s>>>(a);
         return (int)cudaGetLastError();
     }
 };
@@ -462,22 +572,40 @@ struct HashShape {
 #ifndef SDBG_HASH_SMALL
 #define SDBG_HASH_SMALL 8, 4, 4, 4096, 1024, 2
 #endif
-using HashBig = HashShape<SDBG_HASH_BIG>;
-using HashSmall = HashShape<SDBG_HASH_SMALL>;
-static int g_occ_big = 0, g_occ_small = 0;
+#ifndef SDBG_HASH_MW
+#define SDBG_HASH_MW 8, 3, 2, 4096, 1024, 2   // keys of several words: short buckets only, two rows of records in flight per warp
+#endif
+using HashBig = HashShape<1, SDBG_HASH_BIG>;
+using HashSmall = HashShape<1, SDBG_HASH_SMALL>;
+using HashMW2 = HashShape<2, SDBG_HASH_MW>;
+using HashMW3 = HashShape<3, SDBG_HASH_MW>;
+using HashMW4 = HashShape<4, SDBG_HASH_MW>;
+static int g_occ_big = 0, g_occ_small = 0, g_occ_mw[5] = {0, 0, 0, 0, 0};
 
 int hash_setup() {
     int e = HashBig::setup(&g_occ_big);
     if (e) return e;
+    if ((e = HashMW2::setup(&g_occ_mw[2]))) return e;
+    if ((e = HashMW3::setup(&g_occ_mw[3]))) return e;
+    if ((e = HashMW4::setup(&g_occ_mw[4]))) return e;
     return HashSmall::setup(&g_occ_small);
 }
 
 void launch_hash_bounds(const HashCountArgs &a, cudaStream_t s) {
     const u64 warps = a.nseg + 1, blocks = (warps + 7) / 8;
-    hash_bounds_kernel<<<(unsigned)blocks, 256, 0, s>>>(a.keys, a.n, a.top_shift, a.chunk, a.window, a.nseg, a.seg_start, a.overflow);
+    hash_bounds_kernel<<<(unsigned)blocks, 256, 0, s>>>(a.keys, a.W ? a.W : 1u, a.n, a.top_shift, a.chunk, a.window, a.nseg, a.seg_start, a.overflow);
 }
 int launch_hash_count(const HashCountArgs &a, cudaStream_t s) {
     if (a.nseg == 0 || a.nseg > 0x7fffffffull || (u64)a.window + a.chunk >= 65536) return (int)cudaErrorInvalidValue;
+    if (a.W > 1) {                                       // several words per key: the short-bucket shape only
+        if (a.chunk > 2048) return (int)cudaErrorInvalidValue;
+        switch (a.W) {
+            case 2: return HashMW2::launch(a, g_occ_mw[2], s);
+            case 3: return HashMW3::launch(a, g_occ_mw[3], s);
+            case 4: return HashMW4::launch(a, g_occ_mw[4], s);
+        }
+        return (int)cudaErrorInvalidValue;
+    }
     return a.chunk >= 4096 ? HashBig::launch(a, g_occ_big, s) : HashSmall::launch(a, g_occ_small, s);
 }
 void launch_hash_append(const HashCountArgs &a, u64 *total, cudaStream_t s) {

@@ -114,14 +114,16 @@ int launch_count_filter(const CountArgs &a, DevState *st, cudaStream_t s);
 // records sorted by their top key bytes only: count in shared-memory tables, segment by segment (hashcount.cu)
 constexpr u32 kHashSegBlock = 64;        // segments per block sum
 struct HashCountArgs {
-    const u64 *keys; u64 n;              // one-word keys sorted by key >> top_shift
+    const u64 *keys; u64 n;              // records of W words sorted by (first word) >> top_shift
+    u32 W;                               // words per record (0 = 1)
+    bool weak_fp;                        // (tests) fingerprint of a key of several words = its first word
     u32 top_shift, chunk, window;        // nominal records per segment; how far a bucket may run past a nominal border
     u32 d;                               // solid threshold, >= 2
     u64 nseg;                            // ceil(n / chunk)
     u64 *seg_start;                      // u64[nseg + 1] scratch
     u64 *seg_count;                      // u64[nseg] scratch: solid edges per segment
     u64 *blk_sum;                        // u64[ceil(nseg / 64)] scratch, zeroed: solid edges per block of 64 segments, then their prefix
-    u64 *stage_keys;                     // u64[n] scratch (the sorter's spare buffer)
+    u64 *stage_keys;                     // u64[n W] scratch (the sorter's spare buffer)
     u32 *ticket;                         // zeroed: segments are handed out in order
     u32 *overflow;                       // zeroed; nonzero afterwards: something did not fit, nothing may be used
     u64 *stat_slots;

@@ -113,8 +113,8 @@ def test_P8_plan_independence_blockwise(k):
     P = (2 * (k + 1) + 7) // 8
     if k <= 31:
         assert tim.launches["table"] >= res2.stats.n_ranges - 1 and tim.launches["radix"] < res2.stats.n_ranges * P, tim.launches
-    else:
-        assert tim.launches["table"] == 0
+    else:   # keys of several words take it too where a range holds enough records (short ranges go the plain way)
+        assert tim.launches["table"] <= res2.stats.n_ranges
 
 
 def test_edge_cases():
@@ -237,16 +237,16 @@ def test_degenerate_long_runs_poly_A():
     from workloads import ReadGenerator, get_config
     k = 31
     bases, offs = ReadGenerator(get_config(1, scale=0.02)).host()
-    extra = ["A" * 150] * 2500 + ["T" * 150] * 500 + ["ACGT" * 40] * 300
+    extra = ["A" * 150] * 3500 + ["T" * 150] * 500 + ["ACGT" * 40] * 300
     eb, eo = to_arrays(extra)
     bases2 = np.concatenate([bases, eb])
     offs2 = np.concatenate([offs, eo[1:] + offs[-1]])
     orc = run_oracle((bases2, offs2), k, 2)
-    assert int(orc.mult.max()) >= 3000 * (150 - k)          # poly-A forward + poly-T reverse strand
+    assert int(orc.mult.max()) >= 4000 * (150 - k)          # poly-A forward + poly-T reverse strand
     import paper_1409_7208_b200 as sd
     assert_matches_oracle(run_gpu((bases2, offs2), k, 2), orc)
-    # block-wise: the poly-A partition alone holds 357,000 records; a workspace for 400,000 forces more than one range
-    res = run_gpu((bases2, offs2), k, 2, workspace_bytes=sd.sdbg_workspace_for_records(400000, k))
+    # block-wise: the poly-A partition alone holds 476,000 records; a workspace for 520,000 forces more than one range
+    res = run_gpu((bases2, offs2), k, 2, workspace_bytes=sd.sdbg_workspace_for_records(520000, k))
     assert res.stats.n_ranges >= 2
     assert_matches_oracle(res, orc)
     # and a workspace smaller than that partition is refused (reading A12)
@@ -339,7 +339,7 @@ def _radix_launches(res):
     return res.ctx.get_timing().launches["radix"]
 
 
-@pytest.mark.parametrize("k", [15, 21, 31])
+@pytest.mark.parametrize("k", [15, 21, 31, 40, 70, 99])
 def test_table_count_path_and_its_way_back(k):
     """The top-sort + table-count path (api_count.inc count_range_hash, hashcount.cu): records sorted by the most
     significant passes only, segments of whole buckets counted in shared-memory tables. Checked against the oracle and
@@ -349,7 +349,10 @@ def test_table_count_path_and_its_way_back(k):
     k = 31 fills the word) and its all-zero twin; (3) a bucket longer than the search window (poly-A): overflow, the
     records are sorted the plain way from where the top passes left them; (4) reads over two letters only: far more
     distinct keys per bucket than a table holds: overflow; (5) every read twice at d = 2: half of the records of a
-    segment are solid edges, more than its 1,024 sort places: overflow."""
+    segment are solid edges, more than its 1,024 sort places: overflow. Keys of several words (k = 40, 70, 99: whole
+    records go through the top passes of the first key word, the tables hold fingerprints of whole keys and every record
+    is compared with the one that installed its slot) run the same cases with longer reads; where the outcome depends on
+    how the buckets fall, only the result is checked."""
     import os
     import random
     from oracle import run_oracle
@@ -359,27 +362,30 @@ def test_table_count_path_and_its_way_back(k):
     P = (2 * (k + 1) + 7) // 8
     genome = "".join(rng.choice("ACGT") for _ in range(3000))
     covered = []
+    L = 100 if k <= 31 else k + 60
     for _ in range(1500):
-        a = rng.randint(0, len(genome) - 100)
-        x = list(genome[a:a + 100])
+        a = rng.randint(0, len(genome) - L)
+        x = list(genome[a:a + L])
         if rng.random() < 0.3:
-            x[rng.randrange(100)] = rng.choice("ACGT")
+            x[rng.randrange(L)] = rng.choice("ACGT")
         x = "".join(x)
         covered.append(x if rng.random() < 0.5 else rc(x))
-    poly_t = covered + ["T" * 70] * 5 + ["GATTACA" + "T" * 50] * 3
-    poly_a = covered + ["A" * 150] * 400
-    two_letters = ["".join(rng.choice("AC") for _ in range(120)) for _ in range(1200)]
-    twice = ["".join(rng.choice("ACGT") for _ in range(130)) for _ in range(600)] * 2
+    poly_t = covered + ["T" * (L - 30)] * 5 + ["GATTACA" + "T" * (L - 50)] * 3
+    poly_a = covered + ["A" * (L + 50)] * 400
+    two_letters = ["".join(rng.choice("AC") for _ in range(L + 20)) for _ in range(1200)]
+    twice = ["".join(rng.choice("ACGT") for _ in range(L + 30)) for _ in range(600)] * 2
+    multi = k > 31                                        # None: only the result is checked
     cases = [("covered", covered, 2, True), ("covered", covered, 3, True), ("poly_t", poly_t, 2, True),
-             ("poly_a", poly_a, 2, False), ("two_letters", two_letters, 2, False), ("twice", twice, 2, False)]
+             ("poly_a", poly_a, 2, False), ("two_letters", two_letters, 2, None if multi else False),
+             ("twice", twice, 2, None if multi else False)]
     for name, reads, d, completes in cases:
         orc = run_oracle(reads, k, d)
         res = run_gpu(reads, k, d, checksums=False)
         assert_matches_oracle(res, orc, check_stats=True)
         n_hash = _radix_launches(res)
-        if completes:
+        if completes is True:
             assert 0 <= n_hash < P - 1, (name, k, d, n_hash)           # top passes only, the first of them fused with extraction
-        else:
+        elif completes is False:
             assert P <= n_hash < 2 * P, (name, k, d, n_hash)           # top passes, then all passes (the way back)
         import paper_1409_7208_b200 as sd
         for opt in (sd.SDBG_OPT_NO_TABLE_COUNT, sd.SDBG_OPT_STABLE_FIRST_PASS, sd.SDBG_OPT_NO_FUSED_EXTRACT):
@@ -388,6 +394,10 @@ def test_table_count_path_and_its_way_back(k):
             if opt == sd.SDBG_OPT_NO_TABLE_COUNT:
                 assert _radix_launches(res2) == P, (name, k, d)
             assert res2.edges.n == res.edges.n
+    if multi:   # keys that share their first word under the weak fingerprint: caught by the check, redone the plain way
+        resw = run_gpu(covered, k, 2, checksums=False, options=[sd.SDBG_OPT_WEAK_FINGERPRINT])
+        assert_matches_oracle(resw, run_oracle(covered, k, 2), check_stats=True)
+        assert P <= _radix_launches(resw) < 2 * P, (k, _radix_launches(resw))
     # d = 1 keeps every distinct edge: the table count is not used, the records go through all passes exactly once
     res1 = run_gpu(covered, k, 1, checksums=False)
     assert_matches_oracle(res1, run_oracle(covered, k, 1), check_stats=True)
