@@ -140,6 +140,7 @@ hash_count_kernel(HashCountArgs a) {
     using rep_t = unsigned short;                                               // place of a record inside its segment
     constexpr size_t kOffCnt = (size_t)TSMAX * 8, kOffLKey = kOffCnt + (size_t)TSMAX * CB, kOffLCnt = kOffLKey + (size_t)MAXSOLID * 8;
     constexpr size_t kOffTRep = kOffLCnt + (size_t)MAXSOLID * 4, kOffLRep = kOffTRep + (MW ? (size_t)TSMAX * 2 : 0);
+    constexpr size_t kOffSlot = kOffLRep + (MW ? (size_t)MAXSOLID * 2 : 0);     // (W > 1) rep_t[TSMAX]: the slot of each of the first TSMAX records
     extern __shared__ __align__(16) unsigned char smem_raw[];
     u64 *t_key = reinterpret_cast<u64 *>(smem_raw);                             // u64[TSMAX]: key (W = 1) or fingerprint
     u32 *t_cnt = reinterpret_cast<u32 *>(smem_raw + kOffCnt);                   // CB = 2: u16[TSMAX] as u32 pairs; CB = 4: u32[TSMAX]
@@ -147,6 +148,7 @@ hash_count_kernel(HashCountArgs a) {
     u32 *l_cnt = reinterpret_cast<u32 *>(smem_raw + kOffLCnt);
     rep_t *t_rep = reinterpret_cast<rep_t *>(smem_raw + kOffTRep);              // (W > 1) rep_t[TSMAX]: who installed the slot
     rep_t *l_rep = reinterpret_cast<rep_t *>(smem_raw + kOffLRep);              // (W > 1) rep_t[MAXSOLID]
+    rep_t *s_slot = reinterpret_cast<rep_t *>(smem_raw + kOffSlot);
     __shared__ u32 s_ones, s_full, s_nsolid, s_distinct, s_clash;
     __shared__ u64 s_sum, s_look[2][3], s_krange[2];
     __shared__ u32 s_w[WARPS];
@@ -226,7 +228,11 @@ hash_count_kernel(HashCountArgs a) {
                 const bool emp = old[r] == kEmpty;
                 if (NR > 1 || valid) {
                     if (emp || old[r] == f[r]) cnt_add(a8[r]); else pend |= 1u << r;
-                    if (MW && emp) t_rep[a8[r] >> 3] = (rep_t)(i0 + 32u * (u32)r + lane);
+                    if constexpr (MW) {
+                        const u32 idx = i0 + 32u * (u32)r + lane;
+                        if (emp) t_rep[a8[r] >> 3] = (rep_t)idx;
+                        if (idx < (u32)TSMAX && (emp || old[r] == f[r])) s_slot[idx] = (rep_t)(a8[r] >> 3);
+                    }
                     created += emp;
                 }
             }
@@ -248,7 +254,10 @@ hash_count_kernel(HashCountArgs a) {
                     const u64 o = s_cas64(tkey_s + b8, kEmpty, key);
                     if (o == kEmpty || o == key) {
                         cnt_add(b8); created += o == kEmpty; have = false;
-                        if (MW && o == kEmpty) t_rep[b8 >> 3] = (rep_t)who;
+                        if constexpr (MW) {
+                            if (o == kEmpty) t_rep[b8 >> 3] = (rep_t)who;
+                            if (who < (u32)TSMAX) s_slot[who] = (rep_t)(b8 >> 3);
+                        }
                     } else if (++probes >= TS) { s_full = 1; have = false; }
                 }
             }
@@ -293,22 +302,25 @@ hash_count_kernel(HashCountArgs a) {
             if (!full) {
                 for (u32 i = tid; i < m; i += THREADS) {
                     u64 k[W];
-                    load_key<W>(a.keys + (s + i) * W, k);
-                    const u64 f = fingerprint<W>(k, a.weak_fp);
-                    u32 b8 = hash_slot(f, hshift) << 3;
-                    while (t_key[b8 >> 3] != f) b8 = (b8 + 8u) & mask8;       // it is there: the table was not full
-                    const u32 rep = t_rep[b8 >> 3];
+                    u32 slot;
+                    bool loaded = false;
+                    if (i < (u32)TSMAX) slot = s_slot[i];       // noted when the record was inserted
+                    else {
+                        load_key<W>(a.keys + (s + i) * W, k);
+                        loaded = true;
+                        const u64 f = fingerprint<W>(k, a.weak_fp);
+                        u32 b8 = hash_slot(f, hshift) << 3;
+                        while (t_key[b8 >> 3] != f) b8 = (b8 + 8u) & mask8;   // it is there: the table was not full
+                        slot = b8 >> 3;
+                    }
+                    const u32 rep = t_rep[slot];
                     if (rep != i) {
                         u64 o[W];
+                        if (!loaded) load_key<W>(a.keys + (s + i) * W, k);
                         load_key<W>(a.keys + (s + rep) * W, o);
                         bool same = true;
 #pragma unroll
                         for (int q = 0; q < W; ++q) same = same && o[q] == k[q];
-#ifdef SDBG_HASH_DEBUG
-                        if (!same && atomicAdd(&s_clash, 1u) == 0)
-                            printf("clash: seg %llu s %llu m %u i %u rep %u f %llx | %llx %llx %llx %llx | %llx %llx %llx %llx | frep %llx\n", seg, s, m, i, rep, f,
-                                   k[0], k[W > 1 ? 1 : 0], k[W > 2 ? 2 : 0], k[W - 1], o[0], o[W > 1 ? 1 : 0], o[W > 2 ? 2 : 0], o[W - 1], fingerprint<W>(o, a.weak_fp));
-#endif
                         if (!same) s_clash = 1;
                     }
                 }
@@ -547,7 +559,7 @@ __global__ void __launch_bounds__(256) hash_copy_kernel(HashCountArgs a) {
 template <int W, int WARPS, int MINB, int U, int TSMAX, int MAXSOLID, int CB>
 struct HashShape {
     static constexpr int THREADS = WARPS * 32;
-    static constexpr size_t kSmem = (size_t)TSMAX * (8 + CB) + (size_t)MAXSOLID * 12 + (W > 1 ? (size_t)TSMAX * 2 + (size_t)MAXSOLID * 2 : 0);
+    static constexpr size_t kSmem = (size_t)TSMAX * (8 + CB) + (size_t)MAXSOLID * 12 + (W > 1 ? (size_t)TSMAX * 4 + (size_t)MAXSOLID * 2 : 0);
     static int setup(int *blocks_per_sm) {
         int e = (int)cudaFuncSetAttribute(hash_count_kernel<W, WARPS, MINB, U, TSMAX, MAXSOLID, CB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmem);
         if (e) return e;
