@@ -114,6 +114,8 @@ __device__ __forceinline__ void store_key(u64 *__restrict__ out, u64 pos, const 
     }
 }
 
+constexpr int kCoarseBins = 4096;   // groups of 16 consecutive l=8 partitions (ExtractArgs::coarse_hist)
+
 template <int W, bool FILTER, int T4>
 __global__ void __launch_bounds__(256) extract_kernel(ExtractArgs a, DevState *st) {
     extern __shared__ u32 s_hist[];   // [n_passes][256] when digit_hist != nullptr
@@ -133,6 +135,9 @@ __global__ void __launch_bounds__(256) extract_kernel(ExtractArgs a, DevState *s
     u32 *s_posf = s_hist + np * kRadix, *s_posr = s_posf + (T + 1) * kRadix;   // [T + 1][256] each (shared4 only); row T is a spare
     if (do_hist) {
         for (int i = threadIdx.x; i < (np + (shared4 ? 2 * (int)T + 2 : 0)) * kRadix; i += blockDim.x) s_hist[i] = 0;
+        __syncthreads();
+    } else if (a.coarse_hist) {
+        for (int i = threadIdx.x; i < kCoarseBins; i += blockDim.x) s_hist[i] = 0;
         __syncthreads();
     }
     // s_hist row of byte 0 of the last key word if it were a pass (rows of the padding bytes are never touched)
@@ -159,6 +164,23 @@ __global__ void __launch_bounds__(256) extract_kernel(ExtractArgs a, DevState *s
         if (__ballot_sync(0xffffffffu, (valid | vprev) != 0) == 0) continue;
         KeyMaker<W> km;
         km.load(a.words, g < ngroups ? g : 0, a.k);
+        if constexpr (!FILTER && !shared4) {
+            if (a.coarse_hist) {   // planner's histogram: top 12 key bits of both keys of every window, shared-memory counters
+#pragma unroll 4
+                for (u32 ii = 0; ii < 16; ++ii) {
+                    u32 bf, br;
+                    km.template buckets_h<0>(ii, bf, br);
+                    if ((valid >> ii) & 1u) { atomicAdd(&s_hist[bf >> 4], 1u); atomicAdd(&s_hist[br >> 4], 1u); }
+                }
+#pragma unroll 4
+                for (u32 ii = 0; ii < 16; ++ii) {
+                    u32 bf, br;
+                    km.template buckets_h<1>(ii, bf, br);
+                    if ((valid >> (16 + ii)) & 1u) { atomicAdd(&s_hist[bf >> 4], 1u); atomicAdd(&s_hist[br >> 4], 1u); }
+                }
+                continue;
+            }
+        }
         if constexpr (shared4) {
             if (valid | vprev) {
                 // window starts [32g-32, 32g+32) as one mask: bit 32+j = start at my slot j
@@ -352,6 +374,13 @@ __global__ void __launch_bounds__(256) extract_kernel(ExtractArgs a, DevState *s
         csum = warp_reduce_add64(csum);
         if (lane == 0 && csum) atomicAdd(&st->csum_raw, csum);
     }
+    if (!do_hist && a.coarse_hist) {
+        __syncthreads();
+        for (int i = threadIdx.x; i < kCoarseBins; i += blockDim.x) {
+            const u32 v = s_hist[i];
+            if (v) atomicAdd(&a.coarse_hist[i], (u64)v);
+        }
+    }
     if (do_hist) {
         __syncthreads();
         if constexpr (shared4) {
@@ -524,6 +553,10 @@ static int launch_extract_w(const ExtractArgs &a, DevState *st, cudaStream_t s) 
     if (blocks > maxb) blocks = maxb;
     const u32 T = (W == 1 && !filter && a.digit_hist && a.k >= 8) ? a.k / 4 : 0;   // 2..7: shared position tables
     size_t smem = a.digit_hist ? (size_t)(a.passes.n + (T ? 2 * T + 2 : 0)) * kRadix * sizeof(u32) : 0;
+    if (a.coarse_hist) {   // histogram-only call of the planner
+        if (a.digit_hist || a.bucket_hist || a.keys_out || a.want_csum || filter || a.k < 8) return (int)cudaErrorInvalidValue;
+        smem = (size_t)kCoarseBins * sizeof(u32);
+    }
     if (filter) { extract_kernel<W, true, 0><<<(unsigned)blocks, 256, smem, s>>>(a, st); return (int)cudaGetLastError(); }
     if constexpr (W == 1) {
         switch (T) {

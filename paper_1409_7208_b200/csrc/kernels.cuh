@@ -48,6 +48,8 @@ struct ExtractArgs {
     u64 *digit_hist;              // nullptr or u64[n_passes][256], accumulated
     u32 hist_top;                 // != 0: only the rows of the hist_top most significant passes are needed (the others may stay short)
     u64 *bucket_hist;             // nullptr or u64[65536], accumulated (all buckets, ignores lo/hi)
+    u64 *coarse_hist;             // nullptr or u64[4096], accumulated: records per group of 16 consecutive l=8 partitions (top 12 key
+                                  // bits). Histogram-only call (nothing else set), k >= 8: counted in shared memory, no key is made
     int want_csum;
     PassTable passes;
 };
