@@ -7,7 +7,10 @@ from a vertex to its neighbors" (readin
 
 Input: the dict of Oracle.full_graph() — the m edges as letters ((k+1) bytes each, '$' as the outgoing symbol of a
 dummy edge), sorted by (colex of the node, outgoing symbol), and the auxiliary vector of the t zero-indegree nodes.
-Everything here compares node strings; nothing uses W, last or a rank/select formula.
+Everything here compares node strings; nothing uses W, last or a rank/select formula. The searches below are numpy
+library steps (searchsorted over reversed byte strings, one stable argsort); the definition to check by eye, in plain
+loops over the same strings, is tests/helpers.py (brute_force_navigation, and boss_navigation for the formulas), and pin P13 holds this
+module to it.
 
   node(i)      = edges[i][0..k)
   zin[i]       = 1 iff edge i is the last edge of its node and that node is one of the auxiliary vector (A24)
