@@ -584,8 +584,13 @@ struct HashShape {
 #ifndef SDBG_HASH_SMALL
 #define SDBG_HASH_SMALL 8, 4, 4, 4096, 1024, 2
 #endif
-#ifndef SDBG_HASH_MW
-#define SDBG_HASH_MW 8, 3, 2, 4096, 1024, 2   // keys of several words: short buckets only, two rows of records in flight per warp
+#ifndef SDBG_MW_WARPS
+#define SDBG_MW_WARPS 8
+#define SDBG_MW_MINB 3
+#define SDBG_MW_U 2
+#endif
+#ifndef SDBG_HASH_MW   // keys of several words: short buckets only, two rows of records in flight per warp
+#define SDBG_HASH_MW SDBG_MW_WARPS, SDBG_MW_MINB, SDBG_MW_U, 4096, 1024, 2
 #endif
 using HashBig = HashShape<1, SDBG_HASH_BIG>;
 using HashSmall = HashShape<1, SDBG_HASH_SMALL>;
