@@ -145,6 +145,11 @@ __global__ void __launch_bounds__(256) extract_kernel(ExtractArgs a, DevState *s
     u32 *h_last = s_hist - b0 * kRadix;
     // one-word keys, a.hist_top most significant passes wanted only: bytes below bmin of the key word are not counted
     const u32 bmin = (W == 1 && a.hist_top && (int)a.hist_top < np) ? b0 + (u32)np - a.hist_top : b0;
+    // the same for any key width, without position tables: rows of word 0 start at h_word0 (indexed by the byte of the word),
+    // its bytes top_lo .. 7 are wanted
+    const bool top_only = !shared4 && a.hist_top != 0 && a.hist_top <= 4u && (W > 1 || (int)a.hist_top < np);
+    u32 *h_word0 = W == 1 ? h_last : s_hist + ((8 - b0) + 8 * (W - 2)) * kRadix;
+    const u32 top_lo = W == 1 ? bmin : 8u - a.hist_top;
     const u64 ngroups = a.n_slots / 32;
     const u32 lane = lane_id();
     const u32 lt = lanemask_lt();
@@ -256,6 +261,12 @@ __global__ void __launch_bounds__(256) extract_kernel(ExtractArgs a, DevState *s
             if constexpr (shared4) {   // the one byte that is not counted by position: byte 7 - T from the LSB = pass 0
                 constexpr u32 b = 7 - T;
                 if (bmin <= b) atomicAdd(&s_hist[__byte_perm(b < 4 ? (u32)key[0] : (u32)(key[0] >> 32), 0u, 0x4440u | (b & 3))], 1u);
+            } else if (top_only) {
+                // rows of the hist_top most significant passes only: the top bytes of word 0, a short loop without predicates
+                const u32 hi = (u32)(key[0] >> 32);                  // at most four top passes (api_count.inc plan_hash)
+#pragma unroll
+                for (u32 b = 7; b >= 4; --b)
+                    if (b >= top_lo) atomicAdd(&h_word0[b * kRadix + __byte_perm(hi, 0u, 0x4440u | (b & 3u))], 1u);
             } else {
 #pragma unroll
                 for (int q = W - 1; q >= 0; --q) {
