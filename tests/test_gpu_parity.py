@@ -76,6 +76,24 @@ def test_synthetic_medium(k, d):
     assert res.stats.csum_raw == res.stats.csum_distinct == want
 
 
+@pytest.mark.parametrize("k", [8, 12, 16, 27, 32, 33, 47, 48, 63, 64, 65, 80, 95, 96, 97, 127])
+@pytest.mark.parametrize("d", [2, 3])
+def test_default_path_every_key_shape(k, d):
+    """The default path (no checksums: top passes + table count) at a few hundred thousand records for the key shapes
+    where something changes: the last word just begun (k = 32, 64, 96), just filled (31 is covered elsewhere; 63, 95, 127),
+    one past (33, 65, 97), keys whose top passes are all there is of a word (k = 8: 18 bits), and both d. The number of
+    table launches says that the path ran; the result and the statistics are the oracle's."""
+    from workloads import ReadGenerator, get_config
+    cfg = get_config(1, scale=0.1) if k < 80 else get_config(2, scale=0.003)      # 150 bp reads for the long keys
+    bases, offs = ReadGenerator(cfg).host()
+    orc = run_oracle((bases, offs), k, d)
+    res = run_gpu((bases, offs), k, d, checksums=False)
+    assert_matches_oracle(res, orc, check_stats=True)
+    tim = res.ctx.get_timing()
+    P = (2 * (k + 1) + 7) // 8
+    assert tim.launches["table"] == 1 and tim.launches["radix"] < P, (k, d, tim.launches)
+
+
 def test_config1_full_and_host_input():
     from workloads import ReadGenerator, get_config
     w = get_config(1)
