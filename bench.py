@@ -494,7 +494,7 @@ def run_gpu(args, w):
     if also:
         line["also"] = also
     if world == 1 and not args.no_cpu_baseline:
-        line["cpu_baseline"] = cpu_baseline(wl, args.ref_reads)
+        line["cpu_baseline"] = cpu_baseline(wl, 2 * args.ref_reads)   # ~11 s of one host core (the reference arm: half of it per step)
     print(json.dumps(line), flush=True)
     if world > 1:
         dist.destroy_process_group()
