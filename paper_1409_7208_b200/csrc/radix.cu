@@ -248,6 +248,32 @@ __device__ __forceinline__ void prefetch_l2_bulk(const void *p, u32 bytes) {
     if (bytes) asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(p), "r"(bytes) : "memory");
 }
 
+// Staging of a record in shared memory at tile place pos: one-word keys as u64[TILE]; keys of an even number of words as
+// 16-byte halves, half h at ((ulonglong2 *)base)[h * TILE + pos] (one 128-bit access per two words: half the shared-memory
+// wavefronts of word-wise accesses at random places); three words word by word.
+template <int W, int TILE>
+__device__ __forceinline__ void stage_put(u64 *base, u32 pos, const u64 (&k)[W]) {
+    if constexpr (W == 2 || W == 4) {
+        ulonglong2 *b2 = reinterpret_cast<ulonglong2 *>(base);
+#pragma unroll
+        for (int h = 0; h < W / 2; ++h) b2[h * TILE + pos] = make_ulonglong2(k[2 * h], k[2 * h + 1]);
+    } else {
+#pragma unroll
+        for (int q = 0; q < W; ++q) base[q * TILE + pos] = k[q];
+    }
+}
+template <int W, int TILE>
+__device__ __forceinline__ void stage_get(const u64 *base, u32 pos, u64 (&k)[W]) {
+    if constexpr (W == 2 || W == 4) {
+        const ulonglong2 *b2 = reinterpret_cast<const ulonglong2 *>(base);
+#pragma unroll
+        for (int h = 0; h < W / 2; ++h) { const ulonglong2 v = b2[h * TILE + pos]; k[2 * h] = v.x; k[2 * h + 1] = v.y; }
+    } else {
+#pragma unroll
+        for (int q = 0; q < W; ++q) k[q] = base[q * TILE + pos];
+    }
+}
+
 // One LSD pass over an 8-bit, byte-aligned digit. Persistent CTAs; tiles are handed out by an atomic ticket, one
 // tile AHEAD: while a CTA works on a tile it already holds the ticket of its next one, has asked the TMA unit to
 // prefetch that tile into L2, and loads it into the (then free) key registers before the write-out of the current
@@ -418,8 +444,7 @@ onesweep_kernel(RadixArgs a) {
                 for (int j = 0; j < KPT; ++j) {
                     const u32 d = digit8_again<W, HI>(key[j], word, psel);
                     const u32 pos = wp[d] + ((rkp[j / 2] >> (16 * (j & 1))) & 0xffffu);
-#pragma unroll
-                    for (int q = 0; q < W; ++q) s_keys[q * TILE + pos] = key[j][q];
+                    stage_put<W, TILE>(s_keys, pos, key[j]);
                     if constexpr (HAS_VAL) s_vals[pos] = val[j];
                     if ((j & (SDBG_LB_EVERY - 1)) == SDBG_LB_EVERY - 1 && walker)
                         lookback_poll<WIDE>(lb, tile, lb_t, lb_pend, lb_excl, lb_done, real_cnt, tagL, tagG);
@@ -449,8 +474,7 @@ onesweep_kernel(RadixArgs a) {
                 if (method == kMethodA) wm[d] = 0;
             }
             const u32 pos = prev + __popc(m & lt);
-#pragma unroll
-            for (int q = 0; q < W; ++q) s_keys[q * TILE + pos] = key[j][q];
+            stage_put<W, TILE>(s_keys, pos, key[j]);
             if constexpr (HAS_VAL) s_vals[pos] = val[j];
             __syncwarp();
             if ((j & (SDBG_LB_EVERY - 1)) == SDBG_LB_EVERY - 1 && walker)
@@ -485,8 +509,7 @@ onesweep_kernel(RadixArgs a) {
         // ---- 5: coalesced write-out: place p of the tile goes to bin address[digit] + p ----------------------------
         auto write_place = [&](u32 p) {
             u64 kk[W];
-#pragma unroll
-            for (int q = 0; q < W; ++q) kk[q] = s_keys[q * TILE + p];
+            stage_get<W, TILE>(s_keys, p, kk);
             const u32 d = digit8<W, HI>(kk, word, psel);
             store_rec<W>(reinterpret_cast<u64 *>(s_binaddr[d] + (u64)p * (8u * W)), kk);
             if constexpr (HAS_VAL) *reinterpret_cast<u32 *>(s_valaddr[d] + (u64)p * 4u) = s_vals[p];
