@@ -65,6 +65,37 @@ __device__ __forceinline__ u64 mix_key(const u64 (&k)[W]) {
     return h;
 }
 
+// one-word stand-in of a key of W > 1 words (kernels.cuh ExtractArgs::pair_keys): the top `top_bits` bits (8 .. 32) of the
+// first word, so that stand-ins sort like keys as far as the top radix passes look, and below them a fingerprint of the
+// whole key: the HIGH bits of the form  sum over the 32-bit halves w_i of  w_i * c_i + brev(w_i) * d_i  (mod 2^64).
+// A product carries a bit of its factor upwards only, so w_i * c_i alone hardly sees the top bits of w_i; the bit-reversed
+// copy sees exactly those. The extractor makes two fingerprints per window, so they must be cheap (one multiply-add per
+// term), and the keys it meets are full of near-twins — every two copies of an edge with sequencing errors differ in a
+// few symbols, and at 10^9 records every pattern of two or three changed symbols occurs — so no such pattern may cancel.
+// Measured on config 4 (1.36 G records): a splitmix64 finaliser per word never met two keys but doubled the time of the
+// extractor; sum(w_i * c_i) alone met thousands (2 c_1 - 12 c_4 happened to lie below 2^24); sum((w ^ (w >> 32)) * C_w)
+// met the keys that differ in bits 62 and 30 of a word (the fold cancels them). For the form and the constants below all
+// patterns of one, two and three changed symbols were enumerated (it is linear over Z / 2^64, so a pattern has ONE
+// difference whatever the keys are): none comes closer than 2^30 (tests/test_fingerprint.py redoes it). Never all ones
+// (the empty mark of the tables). Equal keys give equal stand-ins; the converse is CHECKED by the table count
+// (hashcount.cu), which sends the range the plain way when two keys meet.
+template <int W>
+__device__ __forceinline__ u64 pair_key(const u64 (&k)[W], u32 top_bits, bool weak) {
+    constexpr u32 c[8] = {0xbc91727fu, 0xc1835ef9u, 0xe0a95433u, 0xf9a8cb5du, 0x84760c67u, 0x9273d27bu, 0xe95637e9u, 0xf96d5857u};
+    constexpr u32 d[8] = {0x9fe6b955u, 0xa7ea17d1u, 0xef3c3825u, 0xb62f8fa3u, 0xa2f73693u, 0xe9f22899u, 0xa0e51d65u, 0xb460a327u};
+    static_assert(W <= 4, "eight pairs of constants");
+    u64 h = 0;
+#pragma unroll
+    for (int q = 0; q < W; ++q) {
+        const u32 lo = (u32)k[q], hi = (u32)(k[q] >> 32);
+        h += (u64)lo * c[2 * q] + (u64)hi * c[2 * q + 1] + (u64)__brev(lo) * d[2 * q] + (u64)__brev(hi) * d[2 * q + 1];
+    }
+    const u64 low = ~0ull >> top_bits;
+    const u64 fp = weak ? k[0] & low : h >> top_bits;
+    const u64 p = (k[0] & ~low) | fp;
+    return p == ~0ull ? p - 1ull : p;
+}
+
 __device__ __forceinline__ u32 warp_incl_scan_add(u32 v) {
 #pragma unroll
     for (int o = 1; o < 32; o <<= 1) {

@@ -282,11 +282,19 @@ __global__ void __launch_bounds__(256) extract_kernel(ExtractArgs a, DevState *s
                 }
             }
         };
+        // (keys of several words, table-count path) the one-word stand-in of the record at output place pos, and its index
+        auto put_pair = [&](u64 pos, const u64 (&key)[W]) {
+            a.pair_keys[pos] = pair_key<W>(key, a.pair_top_bits & 0xffu, (a.pair_top_bits >> 8) != 0);
+            a.pair_idx[pos] = (u32)pos;
+        };
         // one key per lane (or none): coalesced store at the warp's running position, digit histograms, checksum
         auto emit_key = [&](bool keep, const u64 (&key)[W]) {
             if (a.keys_out) {
                 const u32 m = __ballot_sync(0xffffffffu, keep);
-                if (keep) store_key<W>(a.keys_out, base + __popc(m & lt), key);
+                if (keep) {
+                    store_key<W>(a.keys_out, base + __popc(m & lt), key);
+                    if constexpr (W > 1) if (a.pair_keys) put_pair(base + __popc(m & lt), key);
+                }
                 base += __popc(m);
             }
             if (keep) {
@@ -315,9 +323,15 @@ __global__ void __launch_bounds__(256) extract_kernel(ExtractArgs a, DevState *s
                 const bool kf = (vf >> i) & 1, kr = (vr >> i) & 1;
                 if (a.keys_out) {
                     const u32 mf = __ballot_sync(0xffffffffu, kf), mr = __ballot_sync(0xffffffffu, kr);
-                    if (kf) store_key<W>(a.keys_out, base + __popc(mf & lt), f);
+                    if (kf) {
+                        store_key<W>(a.keys_out, base + __popc(mf & lt), f);
+                        if constexpr (W > 1) if (a.pair_keys) put_pair(base + __popc(mf & lt), f);
+                    }
                     base += __popc(mf);
-                    if (kr) store_key<W>(a.keys_out, base + __popc(mr & lt), r);
+                    if (kr) {
+                        store_key<W>(a.keys_out, base + __popc(mr & lt), r);
+                        if constexpr (W > 1) if (a.pair_keys) put_pair(base + __popc(mr & lt), r);
+                    }
                     base += __popc(mr);
                 }
                 if (do_hist) {

@@ -94,19 +94,14 @@ __device__ __forceinline__ void s_red_add(u32 addr, u32 v) {
 }
 
 // ---- keys of W > 1 words ------------------------------------------------------------------------------------------------------
-// The table then holds a 64-bit FINGERPRINT of the whole key where a one-word key stands for itself, and beside it the place
-// (in the segment) of the record that installed it. Equal keys have equal fingerprints; that equal fingerprints are equal
-// keys is CHECKED for every record (a second read of the segment, from L2: the record is compared with the one that
-// installed its slot), and a mismatch raises *overflow like everything else that does not fit, so the result stays exact.
-template <int W>
-__device__ __forceinline__ u64 fingerprint(const u64 (&k)[W], bool weak) {
-    if constexpr (W == 1) return k[0];
-    // splitmix64 finaliser word by word (common.cuh mix_key): every step is a bijection with full avalanche. A cheaper chain
-    // of multiply-adds was measured first and DID meet two keys of config 4 in one value (multiplication carries a
-    // difference in the top bit nowhere): the check below caught it.
-    u64 h = weak ? k[0] : mix_key<W>(k);
-    return h == kEmpty ? kEmpty - 1ull : h;
-}
+// The records stay where the extractor wrote them (a.recs, any order). What is sorted by the top passes and counted here
+// is a one-word STAND-IN of every record (a.keys: the top bits of its first word, which the passes look at, and below
+// them a fingerprint of the whole key; common.cuh pair_key) with the index of the record as payload (a.vals): 12 bytes
+// move per record and pass instead of 8 W. The table holds stand-ins, and beside each the place (in the segment) of the
+// record that installed it. Equal keys have equal stand-ins; that equal stand-ins are equal keys is CHECKED for every
+// record that did not install its slot (word by word against the record that did: two reads through the indices), and a
+// mismatch raises *overflow like everything else that does not fit, so the result stays exact. Records that are alone in
+// their slot (most of them at large k) are never read here at all.
 template <int W>
 __device__ __forceinline__ void load_key(const u64 *__restrict__ src, u64 (&k)[W]) {   // src = first word of the record
     if constexpr (W == 1) k[0] = ld_stream(src);
@@ -173,12 +168,14 @@ hash_count_kernel(HashCountArgs a) {
     // full groups of the segment [bs, be) (none for the segment that ends with the last record of all: it alone can hold
     // the all-ones key, which is counted beside the table by the row-by-row code)
     auto groups_of = [&](u64 bs, u64 be) { return be <= bs || be == a.n ? 0u : ((u32)(be - bs) >> 5) / (u32)U; };
-    u64 cur[U][W];
-    auto load_group = [&](u64 (&k)[U][W], const u64 *src) {   // records src + (32 u + lane) W
+    u64 cur[U][1];
+    auto load_group = [&](u64 (&k)[U][1], const u64 *src) {   // rows src[32 u + lane]
 #pragma unroll
-        for (int u = 0; u < U; ++u) load_key<W>(src + (size_t)(32 * u + lane) * W, k[u]);
+        for (int u = 0; u < U; ++u) k[u][0] = ld_stream(src + 32 * u + lane);
     };
-    if (warp < groups_of(s, e)) load_group(cur, a.keys + (s + (u64)warp * (32 * U)) * W);
+    // (W > 1) the record of the i-th key of the segment that starts at s0
+    auto rec_of = [&](u64 s0, u32 i) { return a.recs + (size_t)a.vals[s0 + i] * W; };
+    if (warp < groups_of(s, e)) load_group(cur, a.keys + s + (u64)warp * (32 * U));
 
     for (u32 it = 0;; ++it) {
         const u32 m = e > s ? (u32)(e - s) : 0u;         // a segment has fewer than 2^16 records
@@ -198,7 +195,7 @@ hash_count_kernel(HashCountArgs a) {
             s_ones = 0; s_full = 0; s_nsolid = 0; s_distinct = 0; s_sum = 0; s_clash = 0;
             la_seg = atomicAdd(a.ticket, 1u);          // consumed behind the insert phase: nothing waits for it here
         }
-        if (tid == 32 % THREADS && m) { kf = a.keys[s * W]; kl = a.keys[(e - 1) * W]; }
+        if (tid == 32 % THREADS && m) { kf = a.keys[s]; kl = a.keys[e - 1]; }
         __syncthreads();
 
         // ---- 1: insert ---------------------------------------------------------------------------------------------------
@@ -212,12 +209,12 @@ hash_count_kernel(HashCountArgs a) {
         // NR rows held by the warp (row r = records i0 + 32 r + lane of the segment): first the home slot of every record
         // (one CAS that installs the key or returns what is there, no loop), then ONE probing loop for the records whose
         // home slot holds another key
-        auto insert_rows = [&](auto nr_tag, const u64 (*k)[W], u32 i0, bool valid) {
+        auto insert_rows = [&](auto nr_tag, const u64 (*k)[1], u32 i0, bool valid) {
             constexpr int NR = decltype(nr_tag)::value;
             u64 old[NR], f[NR]; u32 a8[NR];
 #pragma unroll
             for (int r = 0; r < NR; ++r) {
-                f[r] = fingerprint<W>(k[r], a.weak_fp);
+                f[r] = k[r][0];
                 a8[r] = hash_slot(f[r], hshift) << 3;
                 old[r] = f[r];
                 if (NR > 1 || valid) old[r] = s_cas64(tkey_s + a8[r], kEmpty, f[r]);
@@ -264,12 +261,12 @@ hash_count_kernel(HashCountArgs a) {
         };
         const u32 G = groups_of(s, e);
         {
-            u64 nxt[U][W];
+            u64 nxt[U][1];
             for (u32 g = warp; g < G; g += 2 * WARPS) {  // two groups per round: one is inserted while the other arrives
                 const bool more = g + WARPS < G;
-                if (more) load_group(nxt, a.keys + (s + (u64)(g + WARPS) * (32 * U)) * W);
+                if (more) load_group(nxt, a.keys + s + (u64)(g + WARPS) * (32 * U));
                 insert_rows(std::integral_constant<int, U>{}, cur, g * (32u * U), true);
-                if (g + 2 * WARPS < G) load_group(cur, a.keys + (s + (u64)(g + 2 * WARPS) * (32 * U)) * W);
+                if (g + 2 * WARPS < G) load_group(cur, a.keys + s + (u64)(g + 2 * WARPS) * (32 * U));
                 if (more) insert_rows(std::integral_constant<int, U>{}, nxt, (g + WARPS) * (32u * U), true);
             }
         }
@@ -278,17 +275,15 @@ hash_count_kernel(HashCountArgs a) {
             for (u32 x = (warp + WARPS - G % WARPS) % WARPS; x < nx; x += WARPS) {
                 const u32 i = (row0 + x) * 32u + lane;
                 const bool valid = i < m;
-                u64 key[1][W];
-#pragma unroll
-                for (int q = 0; q < W; ++q) key[0][q] = 0ull;
-                if (valid) load_key<W>(a.keys + (s + i) * W, key[0]);
+                u64 key[1][1];
+                key[0][0] = valid ? ld_stream(a.keys + s + i) : 0ull;
                 if (!MW && last_seg && valid && key[0][0] == kEmpty) { atomicAdd(&s_ones, 1u); insert_rows(std::integral_constant<int, 1>{}, key, (row0 + x) * 32u, false); }
                 else insert_rows(std::integral_constant<int, 1>{}, key, (row0 + x) * 32u, valid);
             }
         }
         // the first records of my next segment are on their way while this one is finished (its bounds came an iteration ago)
         const u64 next = s_look[(it + 1) & 1][0], ns_ = s_look[(it + 1) & 1][1], ne_ = s_look[(it + 1) & 1][2];
-        if (!MW && next < nseg && warp < groups_of(ns_, ne_)) load_group(cur, a.keys + (ns_ + (u64)warp * (32 * U)) * W);
+        if (!MW && next < nseg && warp < groups_of(ns_, ne_)) load_group(cur, a.keys + ns_ + (u64)warp * (32 * U));
         if (created) atomicAdd(&s_distinct, created);
         if (tid == 32 % THREADS) { s_krange[0] = kf >> a.top_shift; s_krange[1] = kl >> a.top_shift; }
         __syncthreads();
@@ -300,32 +295,50 @@ hash_count_kernel(HashCountArgs a) {
         // ---- 1b (W > 1): every record against the one that installed its slot -------------------------------------------------------
         if constexpr (MW) {
             if (!full) {
-                for (u32 i = tid; i < m; i += THREADS) {
-                    u64 k[W];
-                    u32 slot;
-                    bool loaded = false;
-                    if (i < (u32)TSMAX) slot = s_slot[i];       // noted when the record was inserted
-                    else {
-                        load_key<W>(a.keys + (s + i) * W, k);
-                        loaded = true;
-                        const u64 f = fingerprint<W>(k, a.weak_fp);
-                        u32 b8 = hash_slot(f, hshift) << 3;
-                        while (t_key[b8 >> 3] != f) b8 = (b8 + 8u) & mask8;   // it is there: the table was not full
-                        slot = b8 >> 3;
-                    }
-                    const u32 rep = t_rep[slot];
-                    if (rep != i) {
-                        u64 o[W];
-                        if (!loaded) load_key<W>(a.keys + (s + i) * W, k);
-                        load_key<W>(a.keys + (s + rep) * W, o);
-                        bool same = true;
+                // four keys per thread and round, so that the reads through the indices (two dependent loads per record,
+                // two records per check) of a round are in flight together
+                constexpr int VB = 4;
+                for (u32 i0 = tid; i0 < m; i0 += VB * THREADS) {
+                    u32 rep[VB], need = 0;
 #pragma unroll
-                        for (int q = 0; q < W; ++q) same = same && o[q] == k[q];
-                        if (!same) s_clash = 1;
+                    for (int u = 0; u < VB; ++u) {
+                        const u32 i = i0 + (u32)u * THREADS;
+                        rep[u] = i;
+                        if (i < m) {
+                            u32 slot;
+                            if (i < (u32)TSMAX) slot = s_slot[i];   // noted when the key was inserted
+                            else {
+                                const u64 f = a.keys[s + i];
+                                u32 b8 = hash_slot(f, hshift) << 3;
+                                while (t_key[b8 >> 3] != f) b8 = (b8 + 8u) & mask8;   // it is there: the table was not full
+                                slot = b8 >> 3;
+                            }
+                            rep[u] = t_rep[slot];
+                            need |= (rep[u] != i ? 1u : 0u) << u;
+                        }
                     }
+                    if (need == 0) continue;
+                    u32 vi[VB], vr[VB];
+#pragma unroll
+                    for (int u = 0; u < VB; ++u) {
+                        vi[u] = 0; vr[u] = 0;
+                        if ((need >> u) & 1u) { vi[u] = a.vals[s + i0 + (u32)u * THREADS]; vr[u] = a.vals[s + rep[u]]; }
+                    }
+                    bool same = true;
+#pragma unroll
+                    for (int u = 0; u < VB; ++u) {
+                        if ((need >> u) & 1u) {
+                            u64 k[W], o[W];
+                            load_key<W>(a.recs + (size_t)vi[u] * W, k);
+                            load_key<W>(a.recs + (size_t)vr[u] * W, o);
+#pragma unroll
+                            for (int q = 0; q < W; ++q) same = same && o[q] == k[q];
+                        }
+                    }
+                    if (!same) s_clash = 1;
                 }
             }
-            if (next < nseg && warp < groups_of(ns_, ne_)) load_group(cur, a.keys + (ns_ + (u64)warp * (32 * U)) * W);
+            if (next < nseg && warp < groups_of(ns_, ne_)) load_group(cur, a.keys + ns_ + (u64)warp * (32 * U));
             __syncthreads();
             if (s_clash) { full = true; if (tid == 0) atomicOr(a.overflow, 16u); }
         }
@@ -357,7 +370,7 @@ hash_count_kernel(HashCountArgs a) {
                     const u32 c = CB == 2 ? (wq >> ((q & 1u) * 16u)) & 0xffffu : wq;
                     const u32 p = atomicAdd(&s_nsolid, 1u);
                     if (p < (u32)MAXSOLID) {
-                        if constexpr (MW) { const u32 rep = t_rep[v * SPV + q]; l_rep[p] = (rep_t)rep; l_key[p] = a.keys[(s + rep) * W]; }
+                        if constexpr (MW) { const u32 rep = t_rep[v * SPV + q]; l_rep[p] = (rep_t)rep; l_key[p] = rec_of(s, rep)[0]; }
                         else l_key[p] = t_key[v * SPV + q];
                         l_cnt[p] = c;
                     }
@@ -438,7 +451,6 @@ hash_count_kernel(HashCountArgs a) {
             }
             __syncthreads();
             {
-                const u64 *recs = a.keys + s * W;
                 u32 b0 = base0;
 #pragma unroll
                 for (int q = 0; q < Q; ++q) {
@@ -449,7 +461,7 @@ hash_count_kernel(HashCountArgs a) {
                         while (y > 0) {
                             const u64 ky = o_key[b0 + y - 1];
                             bool gt = ky > kx;           // entry y - 1 > entry x
-                            if constexpr (MW) { if (ky == kx) gt = rest_less<W>(recs + (size_t)rx * W, recs + (size_t)o_rep[b0 + y - 1] * W); }
+                            if constexpr (MW) { if (ky == kx) gt = rest_less<W>(rec_of(s, rx), rec_of(s, o_rep[b0 + y - 1])); }
                             if (!gt) break;
                             o_key[b0 + y] = ky; o_cnt[b0 + y] = o_cnt[b0 + y - 1];
                             if constexpr (MW) o_rep[b0 + y] = o_rep[b0 + y - 1];
@@ -468,7 +480,7 @@ hash_count_kernel(HashCountArgs a) {
             for (u32 i = tid; i < ns; i += THREADS) {
                 if constexpr (MW) {
                     u64 k[W];
-                    load_key<W>(a.keys + (s + o_rep[i]) * W, k);
+                    load_key<W>(rec_of(s, o_rep[i]), k);
 #pragma unroll
                     for (int q = 0; q < W; ++q) a.stage_keys[(s + i) * W + q] = k[q];
                 } else a.stage_keys[s + i] = o_key[i];
@@ -587,9 +599,9 @@ struct HashShape {
 #ifndef SDBG_MW_WARPS
 #define SDBG_MW_WARPS 8
 #define SDBG_MW_MINB 3
-#define SDBG_MW_U 2
+#define SDBG_MW_U 4
 #endif
-#ifndef SDBG_HASH_MW   // keys of several words: short buckets only, two rows of records in flight per warp
+#ifndef SDBG_HASH_MW   // keys of several words (one-word stand-ins with an index payload): short buckets only
 #define SDBG_HASH_MW SDBG_MW_WARPS, SDBG_MW_MINB, SDBG_MW_U, 4096, 1024, 2
 #endif
 using HashBig = HashShape<1, SDBG_HASH_BIG>;
@@ -610,7 +622,7 @@ int hash_setup() {
 
 void launch_hash_bounds(const HashCountArgs &a, cudaStream_t s) {
     const u64 warps = a.nseg + 1, blocks = (warps + 7) / 8;
-    hash_bounds_kernel<<<(unsigned)blocks, 256, 0, s>>>(a.keys, a.W ? a.W : 1u, a.n, a.top_shift, a.chunk, a.window, a.nseg, a.seg_start, a.overflow);
+    hash_bounds_kernel<<<(unsigned)blocks, 256, 0, s>>>(a.keys, 1u, a.n, a.top_shift, a.chunk, a.window, a.nseg, a.seg_start, a.overflow);
 }
 int launch_hash_count(const HashCountArgs &a, cudaStream_t s) {
     if (a.nseg == 0 || a.nseg > 0x7fffffffull || (u64)a.window + a.chunk >= 65536) return (int)cudaErrorInvalidValue;

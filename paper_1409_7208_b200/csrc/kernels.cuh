@@ -52,6 +52,10 @@ struct ExtractArgs {
                                   // bits). Histogram-only call (nothing else set), k >= 8: counted in shared memory, no key is made
     int want_csum;
     PassTable passes;
+    // keys of several words on the table-count path: beside every record (same index) a sortable stand-in of one word,
+    // pair_keys[i] = top pair_top_bits bits of the first key word | fingerprint of the whole key below them (pair_key() in
+    // common.cuh), and pair_idx[i] = i. The top passes then move 12 bytes per record instead of 8 W.
+    u64 *pair_keys; u32 *pair_idx; u32 pair_top_bits;
 };
 int launch_extract(const ExtractArgs &a, DevState *st, cudaStream_t s);
 
@@ -116,16 +120,17 @@ int launch_count_filter(const CountArgs &a, DevState *st, cudaStream_t s);
 // records sorted by their top key bytes only: count in shared-memory tables, segment by segment (hashcount.cu)
 constexpr u32 kHashSegBlock = 64;        // segments per block sum
 struct HashCountArgs {
-    const u64 *keys; u64 n;              // records of W words sorted by (first word) >> top_shift
+    const u64 *keys; u64 n;              // one word per record, sorted by key >> top_shift: the key itself (W = 1) or its
+                                         // stand-in (ExtractArgs::pair_keys)
     u32 W;                               // words per record (0 = 1)
-    bool weak_fp;                        // (tests) fingerprint of a key of several words = its first word
+    const u32 *vals; const u64 *recs;    // (W > 1) vals[i] = index of the record of keys[i] in recs (W words each, any order)
     u32 top_shift, chunk, window;        // nominal records per segment; how far a bucket may run past a nominal border
     u32 d;                               // solid threshold, >= 2
     u64 nseg;                            // ceil(n / chunk)
     u64 *seg_start;                      // u64[nseg + 1] scratch
     u64 *seg_count;                      // u64[nseg] scratch: solid edges per segment
     u64 *blk_sum;                        // u64[ceil(nseg / 64)] scratch, zeroed: solid edges per block of 64 segments, then their prefix
-    u64 *stage_keys;                     // u64[n W] scratch (the sorter's spare buffer)
+    u64 *stage_keys;                     // u64[n W] scratch (the sorter's spare buffer, or the second record buffer)
     u32 *ticket;                         // zeroed: segments are handed out in order
     u32 *overflow;                       // zeroed; nonzero afterwards: something did not fit, nothing may be used
     u64 *stat_slots;
