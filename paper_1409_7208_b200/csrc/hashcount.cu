@@ -169,12 +169,20 @@ hash_count_kernel(HashCountArgs a) {
     // the all-ones key, which is counted beside the table by the row-by-row code)
     auto groups_of = [&](u64 bs, u64 be) { return be <= bs || be == a.n ? 0u : ((u32)(be - bs) >> 5) / (u32)U; };
     u64 cur[U][1];
-    auto load_group = [&](u64 (&k)[U][1], const u64 *src) {   // rows src[32 u + lane]
+    u32 cur_v[U];                                        // (W > 1) the record indices of the rows in cur
+    auto load_group_v = [&](u64 (&k)[U][1], u32 (&v)[U], u64 first) {   // rows first + 32 u + lane of keys (and vals)
 #pragma unroll
-        for (int u = 0; u < U; ++u) k[u][0] = ld_stream(src + 32 * u + lane);
+        for (int u = 0; u < U; ++u) {
+            k[u][0] = ld_stream(a.keys + first + 32 * u + lane);
+            if constexpr (MW) v[u] = a.vals[first + 32 * u + lane]; else v[u] = 0;
+        }
     };
+    auto load_group = [&](u64 (&k)[U][1], const u64 *src) { load_group_v(k, cur_v, (u64)(src - a.keys)); };
     // (W > 1) the record of the i-th key of the segment that starts at s0
     auto rec_of = [&](u64 s0, u32 i) { return a.recs + (size_t)a.vals[s0 + i] * W; };
+    // (W > 1) a key that met its slot taken will be compared with the record that installed it: its own record is asked
+    // for now (into L2), while the rest of the segment is inserted
+    auto want_rec = [&](u32 v) { asm volatile("prefetch.global.L2 [%0];" ::"l"(a.recs + (size_t)v * W)); };
     if (warp < groups_of(s, e)) load_group(cur, a.keys + s + (u64)warp * (32 * U));
 
     for (u32 it = 0;; ++it) {
@@ -209,7 +217,7 @@ hash_count_kernel(HashCountArgs a) {
         // NR rows held by the warp (row r = records i0 + 32 r + lane of the segment): first the home slot of every record
         // (one CAS that installs the key or returns what is there, no loop), then ONE probing loop for the records whose
         // home slot holds another key
-        auto insert_rows = [&](auto nr_tag, const u64 (*k)[1], u32 i0, bool valid) {
+        auto insert_rows = [&](auto nr_tag, const u64 (*k)[1], const u32 *kv, u32 i0, bool valid) {
             constexpr int NR = decltype(nr_tag)::value;
             u64 old[NR], f[NR]; u32 a8[NR];
 #pragma unroll
@@ -229,6 +237,7 @@ hash_count_kernel(HashCountArgs a) {
                         const u32 idx = i0 + 32u * (u32)r + lane;
                         if (emp) t_rep[a8[r] >> 3] = (rep_t)idx;
                         if (idx < (u32)TSMAX && (emp || old[r] == f[r])) s_slot[idx] = (rep_t)(a8[r] >> 3);
+                        if (!emp) want_rec(kv[r]);     // a copy, or a key that goes on probing (most of those end as copies)
                     }
                     created += emp;
                 }
@@ -262,12 +271,13 @@ hash_count_kernel(HashCountArgs a) {
         const u32 G = groups_of(s, e);
         {
             u64 nxt[U][1];
+            u32 nxt_v[U];
             for (u32 g = warp; g < G; g += 2 * WARPS) {  // two groups per round: one is inserted while the other arrives
                 const bool more = g + WARPS < G;
-                if (more) load_group(nxt, a.keys + s + (u64)(g + WARPS) * (32 * U));
-                insert_rows(std::integral_constant<int, U>{}, cur, g * (32u * U), true);
+                if (more) load_group_v(nxt, nxt_v, s + (u64)(g + WARPS) * (32 * U));
+                insert_rows(std::integral_constant<int, U>{}, cur, cur_v, g * (32u * U), true);
                 if (g + 2 * WARPS < G) load_group(cur, a.keys + s + (u64)(g + 2 * WARPS) * (32 * U));
-                if (more) insert_rows(std::integral_constant<int, U>{}, nxt, (g + WARPS) * (32u * U), true);
+                if (more) insert_rows(std::integral_constant<int, U>{}, nxt, nxt_v, (g + WARPS) * (32u * U), true);
             }
         }
         {   // the rows behind the last full group, and the partial last row: x-th of them belongs to warp (G + x) % WARPS
@@ -276,9 +286,11 @@ hash_count_kernel(HashCountArgs a) {
                 const u32 i = (row0 + x) * 32u + lane;
                 const bool valid = i < m;
                 u64 key[1][1];
+                u32 kv[1];
                 key[0][0] = valid ? ld_stream(a.keys + s + i) : 0ull;
-                if (!MW && last_seg && valid && key[0][0] == kEmpty) { atomicAdd(&s_ones, 1u); insert_rows(std::integral_constant<int, 1>{}, key, (row0 + x) * 32u, false); }
-                else insert_rows(std::integral_constant<int, 1>{}, key, (row0 + x) * 32u, valid);
+                kv[0] = (MW && valid) ? a.vals[s + i] : 0u;
+                if (!MW && last_seg && valid && key[0][0] == kEmpty) { atomicAdd(&s_ones, 1u); insert_rows(std::integral_constant<int, 1>{}, key, kv, (row0 + x) * 32u, false); }
+                else insert_rows(std::integral_constant<int, 1>{}, key, kv, (row0 + x) * 32u, valid);
             }
         }
         // the first records of my next segment are on their way while this one is finished (its bounds came an iteration ago)
