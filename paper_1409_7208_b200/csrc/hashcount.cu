@@ -202,6 +202,13 @@ hash_count_kernel(HashCountArgs a) {
         if (tid == 0) {
             s_ones = 0; s_full = 0; s_nsolid = 0; s_distinct = 0; s_sum = 0; s_clash = 0;
             la_seg = atomicAdd(a.ticket, 1u);          // consumed behind the insert phase: nothing waits for it here
+            // the keys of my NEXT segment (its bounds came an iteration ago) are asked for now, into L2, by the TMA unit: the
+            // loads of its insert phase, half of which are issued just before they are needed, then come from there
+            const u64 pn_s = s_look[(it + 1) & 1][1], pn_e = s_look[(it + 1) & 1][2];
+            if (pn_e > pn_s) {
+                const u64 p0 = (u64)(a.keys + pn_s) & ~15ull, p1 = ((u64)(a.keys + pn_e) + 15ull) & ~15ull;
+                asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(p0), "r"((u32)(p1 - p0)) : "memory");
+            }
         }
         if (tid == 32 % THREADS && m) { kf = a.keys[s]; kl = a.keys[e - 1]; }
         __syncthreads();
