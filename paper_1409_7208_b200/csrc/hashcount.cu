@@ -102,12 +102,18 @@ __device__ __forceinline__ void s_red_add(u32 addr, u32 v) {
 // record that did not install its slot (word by word against the record that did: two reads through the indices), and a
 // mismatch raises *overflow like everything else that does not fit, so the result stays exact. Records that are alone in
 // their slot (most of them at large k) are never read here at all.
+// 16 bytes of a record read at a random place: the L2 is told to fetch 64 bytes around it, not the 128 of its default
+__device__ __forceinline__ ulonglong2 ld_rec16(const u64 *p) {
+    ulonglong2 v;
+    asm volatile("ld.global.L2::64B.v2.u64 {%0,%1}, [%2];" : "=l"(v.x), "=l"(v.y) : "l"(p));
+    return v;
+}
 template <int W>
 __device__ __forceinline__ void load_key(const u64 *__restrict__ src, u64 (&k)[W]) {   // src = first word of the record
     if constexpr (W == 1) k[0] = ld_stream(src);
-    else if constexpr (W == 2) { const ulonglong2 v = *reinterpret_cast<const ulonglong2 *>(src); k[0] = v.x; k[1] = v.y; }
+    else if constexpr (W == 2) { const ulonglong2 v = ld_rec16(src); k[0] = v.x; k[1] = v.y; }
     else if constexpr (W == 4) {
-        const ulonglong2 v0 = *reinterpret_cast<const ulonglong2 *>(src), v1 = *reinterpret_cast<const ulonglong2 *>(src + 2);
+        const ulonglong2 v0 = ld_rec16(src), v1 = ld_rec16(src + 2);
         k[0] = v0.x; k[1] = v0.y; k[2] = v1.x; k[3] = v1.y;
     } else {
 #pragma unroll
