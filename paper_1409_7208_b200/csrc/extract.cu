@@ -13,6 +13,18 @@
 
 namespace sdbg {
 
+// shared-memory atomics by 32-bit shared address (one LEA in front of the ATOMS / RED instead of the address arithmetic
+// of a generic pointer); the hot loops below issue two to four of them per window
+__device__ __forceinline__ u32 smem_addr(const void *p) { return (u32)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void s_inc(u32 addr) { asm volatile("red.shared.add.u32 [%0], 1;" ::"r"(addr) : "memory"); }
+__device__ __forceinline__ void s_add(u32 addr, u32 v) { asm volatile("red.shared.add.u32 [%0], %1;" ::"r"(addr), "r"(v) : "memory"); }
+__device__ __forceinline__ u32 s_fetch_inc(u32 addr) {
+    u32 r;
+    asm volatile("atom.shared.add.u32 %0, [%1], 1;" : "=r"(r) : "r"(addr) : "memory");
+    return r;
+}
+__device__ __forceinline__ void s_st64(u32 addr, u64 v) { asm volatile("st.shared.u64 [%0], %1;" ::"r"(addr), "l"(v) : "memory"); }
+
 __device__ __forceinline__ u64 rev2(u64 x) {   // reverse the order of the 32 2-bit groups
     u32 lo = (u32)x, hi = (u32)(x >> 32);
     u64 y = ((u64)__brev(lo) << 32) | (u64)__brev(hi);
@@ -142,14 +154,15 @@ __global__ void __launch_bounds__(256) extract_kernel(ExtractArgs a, DevState *s
     }
     // s_hist row of byte 0 of the last key word if it were a pass (rows of the padding bytes are never touched)
     const u32 b0 = a.passes.n ? (u32)a.passes.p[0].shift >> 3 : 0u;
-    u32 *h_last = s_hist - b0 * kRadix;
     // one-word keys, a.hist_top most significant passes wanted only: bytes below bmin of the key word are not counted
     const u32 bmin = (W == 1 && a.hist_top && (int)a.hist_top < np) ? b0 + (u32)np - a.hist_top : b0;
     // the same for any key width, without position tables: rows of word 0 start at h_word0 (indexed by the byte of the word),
     // its bytes top_lo .. 7 are wanted
     const bool top_only = !shared4 && a.hist_top != 0 && a.hist_top <= 4u && (W > 1 || (int)a.hist_top < np);
-    u32 *h_word0 = W == 1 ? h_last : s_hist + ((8 - b0) + 8 * (W - 2)) * kRadix;
     const u32 top_lo = W == 1 ? bmin : 8u - a.hist_top;
+    const u32 hist_s = smem_addr(s_hist);
+    const u32 h_word0_s = hist_s + 4u * (u32)(W == 1 ? 0 : ((8 - b0) + 8 * (W - 2)) * kRadix) - (W == 1 ? 4u * b0 * kRadix : 0u);
+    const u32 posf_s = hist_s + 4u * (u32)(np * kRadix), posr_s = posf_s + 4u * (T + 1) * kRadix;
     const u64 ngroups = a.n_slots / 32;
     const u32 lane = lane_id();
     const u32 lt = lanemask_lt();
@@ -175,13 +188,13 @@ __global__ void __launch_bounds__(256) extract_kernel(ExtractArgs a, DevState *s
                 for (u32 ii = 0; ii < 16; ++ii) {
                     u32 bf, br;
                     km.template buckets_h<0>(ii, bf, br);
-                    if ((valid >> ii) & 1u) { atomicAdd(&s_hist[bf >> 4], 1u); atomicAdd(&s_hist[br >> 4], 1u); }
+                    if ((valid >> ii) & 1u) { s_inc(hist_s + 4u * (bf >> 4)); s_inc(hist_s + 4u * (br >> 4)); }
                 }
 #pragma unroll 4
                 for (u32 ii = 0; ii < 16; ++ii) {
                     u32 bf, br;
                     km.template buckets_h<1>(ii, bf, br);
-                    if ((valid >> (16 + ii)) & 1u) { atomicAdd(&s_hist[bf >> 4], 1u); atomicAdd(&s_hist[br >> 4], 1u); }
+                    if ((valid >> (16 + ii)) & 1u) { s_inc(hist_s + 4u * (bf >> 4)); s_inc(hist_s + 4u * (br >> 4)); }
                 }
                 continue;
             }
@@ -197,11 +210,11 @@ __global__ void __launch_bounds__(256) extract_kernel(ExtractArgs a, DevState *s
                     const u32 mr = (u32)(V >> (off_r + j)) & pat;       // bit 4(T-1-t): the window whose rc byte t I am
                     // branch-free: a position without window (mask 0) and a range that ends at T go to the spare row T
                     const u32 f_lo = ((u32)__ffs(mf) - 1u) >> 2, f_end = ((31u - (u32)__clz(mf)) >> 2) + 1u;
-                    atomicAdd(&s_posf[(mf ? f_lo : T) * kRadix + f4], 1u);
-                    atomicAdd(&s_posf[(mf ? f_end : T) * kRadix + f4], 0xffffffffu);
+                    s_inc(posf_s + 4u * ((mf ? f_lo : T) * kRadix + f4));
+                    s_add(posf_s + 4u * ((mf ? f_end : T) * kRadix + f4), 0xffffffffu);
                     const u32 r_lo = T - 1u - ((31u - (u32)__clz(mr)) >> 2), r_end = T - (((u32)__ffs(mr) - 1u) >> 2);
-                    atomicAdd(&s_posr[(mr ? r_lo : T) * kRadix + f4], 1u);
-                    atomicAdd(&s_posr[(mr ? r_end : T) * kRadix + f4], 0xffffffffu);
+                    s_inc(posr_s + 4u * ((mr ? r_lo : T) * kRadix + f4));
+                    s_add(posr_s + 4u * ((mr ? r_end : T) * kRadix + f4), 0xffffffffu);
                 };
                 const u32 b0w = KeyMaker<W>::w32(km.B, 0), b1w = KeyMaker<W>::w32(km.B, 1), b2w = KeyMaker<W>::w32(km.B, 2);
 #pragma unroll 4
@@ -260,24 +273,24 @@ __global__ void __launch_bounds__(256) extract_kernel(ExtractArgs a, DevState *s
         auto add_digits = [&](const u64 (&key)[W]) {
             if constexpr (shared4) {   // the one byte that is not counted by position: byte 7 - T from the LSB = pass 0
                 constexpr u32 b = 7 - T;
-                if (bmin <= b) atomicAdd(&s_hist[__byte_perm(b < 4 ? (u32)key[0] : (u32)(key[0] >> 32), 0u, 0x4440u | (b & 3))], 1u);
+                if (bmin <= b) s_inc(hist_s + 4u * __byte_perm(b < 4 ? (u32)key[0] : (u32)(key[0] >> 32), 0u, 0x4440u | (b & 3)));
             } else if (top_only) {
                 // rows of the hist_top most significant passes only: the top bytes of word 0, a short loop without predicates
                 const u32 hi = (u32)(key[0] >> 32);                  // at most four top passes (api_count.inc plan_hash)
 #pragma unroll
                 for (u32 b = 7; b >= 4; --b)
-                    if (b >= top_lo) atomicAdd(&h_word0[b * kRadix + __byte_perm(hi, 0u, 0x4440u | (b & 3u))], 1u);
+                    if (b >= top_lo) s_inc(h_word0_s + 4u * (b * kRadix + __byte_perm(hi, 0u, 0x4440u | (b & 3u))));
             } else {
 #pragma unroll
                 for (int q = W - 1; q >= 0; --q) {
                     if (W > 1 && q > 0 && a.hist_top) continue;      // (keys of several words) top passes only: bytes of word 0
-                    u32 *hq = (q == W - 1) ? h_last : h_last + ((8 - b0) + 8 * (W - 2 - q) + b0) * kRadix;
+                    const u32 hq_s = (q == W - 1) ? hist_s - 4u * b0 * kRadix : hist_s + 4u * (u32)(((8 - b0) + 8 * (W - 2 - q)) * kRadix);
                     const u32 lo = (u32)key[q], hi = (u32)(key[q] >> 32);
 #pragma unroll
                     for (int b = 0; b < 8; ++b) {
                         if (q == W - 1 && b < (int)bmin) continue;   // padding bytes of the last word (and passes not wanted): no row
                         if (W > 1 && a.hist_top && b + (int)a.hist_top < 8) continue;
-                        atomicAdd(&hq[b * kRadix + __byte_perm(b < 4 ? lo : hi, 0u, 0x4440u | (b & 3))], 1u);
+                        s_inc(hq_s + 4u * (b * kRadix + __byte_perm(b < 4 ? lo : hi, 0u, 0x4440u | (b & 3))));
                     }
                 }
             }
@@ -461,28 +474,28 @@ struct ScatterSmem {
 
 template <int HALF>
 __device__ __forceinline__ void scatter_count_half(const KeyMaker<1> &km, u32 valid16, u64 S0f, u64 S1f, u64 S0r, u64 S1r,
-                                                   u32 *s_cntF, u32 *s_cntR) {
+                                                   u32 cntF_s, u32 cntR_s) {   // 32-bit shared addresses of the two tables
 #pragma unroll
     for (u32 ii = 0; ii < 16; ++ii) {
         constexpr u32 base = 16u * HALF;
         const u32 j = base + ii;                          // window = slot j of the group; its 4-mers start at symbol j of S
         const u32 f4 = j <= 28 ? (u32)(S0f >> (56 - 2 * j)) & 0xffu : (u32)(funnel(S0f, S1f, 2 * j) >> 56);
         const u32 r4 = j <= 28 ? (u32)(S0r >> (56 - 2 * j)) & 0xffu : (u32)(funnel(S0r, S1r, 2 * j) >> 56);
-        if ((valid16 >> ii) & 1u) { atomicAdd(&s_cntF[f4], 1u); atomicAdd(&s_cntR[r4], 1u); }
+        if ((valid16 >> ii) & 1u) { s_inc(cntF_s + 4u * f4); s_inc(cntR_s + 4u * r4); }
     }
 }
 
 template <int HALF>
-__device__ __forceinline__ void scatter_place_half(const KeyMaker<1> &km, u32 valid16, u32 dshift, u32 *s_cur, u64 *s_stage) {
+__device__ __forceinline__ void scatter_place_half(const KeyMaker<1> &km, u32 valid16, u32 dshift, u32 cur_s, u32 stage_s) {
 #pragma unroll
     for (u32 ii = 0; ii < 16; ++ii) {
         u64 f[1], r[1];
         km.template keys_h<HALF>(ii, f, r);
         if ((valid16 >> ii) & 1u) {
-            const u32 pf = atomicAdd(&s_cur[(u32)(f[0] >> dshift) & 0xffu], 1u);
-            s_stage[pf] = f[0];
-            const u32 pr = atomicAdd(&s_cur[(u32)(r[0] >> dshift) & 0xffu], 1u);
-            s_stage[pr] = r[0];
+            const u32 pf = s_fetch_inc(cur_s + 4u * ((u32)(f[0] >> dshift) & 0xffu));
+            const u32 pr = s_fetch_inc(cur_s + 4u * ((u32)(r[0] >> dshift) & 0xffu));
+            s_st64(stage_s + 8u * pf, f[0]);
+            s_st64(stage_s + 8u * pr, r[0]);
         }
     }
 }
@@ -494,6 +507,8 @@ __global__ void __launch_bounds__(ScatterSmem::THREADS, 3) extract_scatter_kerne
     u32 *s_cntF = reinterpret_cast<u32 *>(smem_raw + L::kCntF), *s_cntR = reinterpret_cast<u32 *>(smem_raw + L::kCntR);
     u32 *s_cur = reinterpret_cast<u32 *>(smem_raw + L::kCur);
     u64 *s_off = reinterpret_cast<u64 *>(smem_raw + L::kOff);
+    const u32 smem_s = smem_addr(smem_raw);
+    const u32 stage_s = smem_s + (u32)L::kStage, cntF_s = smem_s + (u32)L::kCntF, cntR_s = smem_s + (u32)L::kCntR, cur_s = smem_s + (u32)L::kCur;
     __shared__ u32 s_wtot[8];
     __shared__ u32 s_total;
     const u32 tid = threadIdx.x, lane = tid & 31u, warp = tid >> 5;
@@ -514,8 +529,8 @@ __global__ void __launch_bounds__(ScatterSmem::THREADS, 3) extract_scatter_kerne
         if (valid16) {
             const u64 S0f = funnel(km.B[0], km.B[1], 2 * off_f), S1f = off_f ? km.B[1] << (2 * off_f) : km.B[1];
             const u64 S0r = funnel(km.B[0], km.B[1], 2 * off_r), S1r = km.B[1] << (2 * off_r);
-            if (half) scatter_count_half<1>(km, valid16, S0f, S1f, S0r, S1r, s_cntF, s_cntR);
-            else scatter_count_half<0>(km, valid16, S0f, S1f, S0r, S1r, s_cntF, s_cntR);
+            if (half) scatter_count_half<1>(km, valid16, S0f, S1f, S0r, S1r, cntF_s, cntR_s);
+            else scatter_count_half<0>(km, valid16, S0f, S1f, S0r, S1r, cntF_s, cntR_s);
         }
         __syncthreads();
         // ---- B: bin tid: count (fold), exclusive scan over the bins, reservation of its run in the output
@@ -537,8 +552,8 @@ __global__ void __launch_bounds__(ScatterSmem::THREADS, 3) extract_scatter_kerne
         }
         // ---- C: keys into their bins in shared memory
         if (valid16) {
-            if (half) scatter_place_half<1>(km, valid16, dshift, s_cur, s_stage);
-            else scatter_place_half<0>(km, valid16, dshift, s_cur, s_stage);
+            if (half) scatter_place_half<1>(km, valid16, dshift, cur_s, stage_s);
+            else scatter_place_half<0>(km, valid16, dshift, cur_s, stage_s);
         }
         __syncthreads();
         // ---- D: the tile leaves in bin order
