@@ -447,6 +447,71 @@ __global__ void __launch_bounds__(256) extract_kernel(ExtractArgs a, DevState *s
     }
 }
 
+// ---- keys of several words, table-count path, few valid windows per slot (ExtractArgs::by_rows) --------------------------------
+// A warp takes one group of 32 base slots per step, lane = slot. The valid-window mask of the group is the same for all
+// lanes, so a group without a window costs one mask; in a group with windows every lane that has one makes both keys (the
+// KeyMaker of the group, window = lane), and the records, their one-word stand-ins and indices leave the warp together.
+// Digit rows of the hist_top top passes only (the caller's table-count path), no filter, no checksum.
+template <int W>
+__global__ void __launch_bounds__(256) extract_rows_kernel(ExtractArgs a, DevState *st) {
+    extern __shared__ u32 s_hist[];   // [n_passes][256]; only the rows of the top passes of word 0 are touched
+    const int np = a.passes.n;
+    for (int i = threadIdx.x; i < np * kRadix; i += blockDim.x) s_hist[i] = 0;
+    __syncthreads();
+    const u32 b0 = a.passes.n ? (u32)a.passes.p[0].shift >> 3 : 0u;
+    const u32 top_lo = 8u - a.hist_top;
+    const u32 h_word0_s = smem_addr(s_hist) + 4u * (u32)(((8 - b0) + 8 * (W - 2)) * kRadix);
+    const u64 ngroups = a.n_slots / 32;
+    const u32 lane = lane_id(), lt = lanemask_lt();
+    const u32 top_bits = a.pair_top_bits & 0xffu;
+    const bool weak = (a.pair_top_bits >> 8) != 0;
+    const u64 warps_total = (u64)gridDim.x * (blockDim.x >> 5);
+    const u64 nspans = (ngroups + 31) / 32;              // a warp takes 32 consecutive groups at a time: one reservation of output
+    for (u64 sp = (u64)blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5); sp < nspans; sp += warps_total) {
+        const u64 g0 = sp * 32;
+        const u32 my_valid = g0 + lane < ngroups ? valid_mask32(a.ends, g0 + lane, a.k) : 0u;   // lane j: the mask of group g0 + j
+        const u32 total = 2u * (u32)__reduce_add_sync(0xffffffffu, (u32)__popc(my_valid));
+        if (total == 0) continue;
+        u64 base = 0;
+        if (lane == 0) base = atomicAdd(&st->extract_cursor, (u64)total);
+        base = __shfl_sync(0xffffffffu, base, 0);
+        if (base + total > a.out_cap) continue;          // cannot happen when the caller sized out_cap from the window count
+        u32 groups = __ballot_sync(0xffffffffu, my_valid != 0);
+        while (groups) {
+            const u32 j = (u32)__ffs(groups) - 1u;
+            groups &= groups - 1u;
+            const u32 valid = __shfl_sync(0xffffffffu, my_valid, j);
+            KeyMaker<W> km;
+            km.load(a.words, g0 + j, a.k);
+            u64 f[W], r[W];
+            km.keys(lane, f, r);
+            const bool v = (valid >> lane) & 1u;
+            if (v) {
+                const u64 pos = base + 2 * __popc(valid & lt);
+                store_key<W>(a.keys_out, pos, f);
+                store_key<W>(a.keys_out, pos + 1, r);
+                a.pair_keys[pos] = pair_key<W>(f, top_bits, weak);
+                a.pair_keys[pos + 1] = pair_key<W>(r, top_bits, weak);
+                *reinterpret_cast<uint2 *>(a.pair_idx + pos) = make_uint2((u32)pos, (u32)pos + 1u);   // pos is even
+                const u32 fh = (u32)(f[0] >> 32), rh = (u32)(r[0] >> 32);
+#pragma unroll
+                for (u32 b = 7; b >= 4; --b) {
+                    if (b >= top_lo) {
+                        s_inc(h_word0_s + 4u * (b * kRadix + __byte_perm(fh, 0u, 0x4440u | (b & 3u))));
+                        s_inc(h_word0_s + 4u * (b * kRadix + __byte_perm(rh, 0u, 0x4440u | (b & 3u))));
+                    }
+                }
+            }
+            base += 2 * __popc(valid);
+        }
+    }
+    __syncthreads();
+    for (int i = threadIdx.x; i < np * kRadix; i += blockDim.x) {
+        const u32 c = s_hist[i];
+        if (c) atomicAdd(&a.digit_hist[i], (u64)c);
+    }
+}
+
 // ---- extraction fused with the first (unstable) radix pass --------------------------------------------------------------
 // One-word keys, dense range, default path (api_count.inc): the keys are not written in read order and re-read by the
 // first top pass; they go straight from the key maker into the 256 bins of that pass. The bin sizes come from a
@@ -598,6 +663,14 @@ static int launch_extract_w(const ExtractArgs &a, DevState *st, cudaStream_t s) 
         smem = (size_t)kCoarseBins * sizeof(u32);
     }
     if (filter) { extract_kernel<W, true, 0><<<(unsigned)blocks, 256, smem, s>>>(a, st); return (int)cudaGetLastError(); }
+    if constexpr (W > 1) {
+        if (a.by_rows) {
+            if (!a.pair_keys || !a.keys_out || !a.digit_hist || !a.hist_top || a.hist_top > 4 || a.want_csum || a.bucket_hist || a.coarse_hist)
+                return (int)cudaErrorInvalidValue;
+            extract_rows_kernel<W><<<(unsigned)maxb, 256, smem, s>>>(a, st);
+            return (int)cudaGetLastError();
+        }
+    }
     if constexpr (W == 1) {
         switch (T) {
             case 2: extract_kernel<1, false, 2><<<(unsigned)blocks, 256, smem, s>>>(a, st); return (int)cudaGetLastError();
