@@ -314,7 +314,7 @@ hash_count_kernel(HashCountArgs a) {
         __syncthreads();
         if (tid == 0) bounds_of(la_seg, la_s, la_e);     // stored at the end of the iteration
         const u64 kfirst = s_krange[0], klast = s_krange[1];
-        bool full = s_full != 0;
+        const bool full = s_full != 0;
         if (full && tid == 0) atomicOr(a.overflow, 2u);
 
         // ---- 1b (W > 1): every record against the one that installed its slot -------------------------------------------------------
@@ -364,8 +364,9 @@ hash_count_kernel(HashCountArgs a) {
                 }
             }
             if (next < nseg && warp < groups_of(ns_, ne_)) load_group(cur, a.keys + ns_ + (u64)warp * (32 * U));
-            __syncthreads();
-            if (s_clash) { full = true; if (tid == 0) atomicOr(a.overflow, 16u); }
+            // no barrier here: the check only reads the table, and so does the scan that follows; a warp that had little to
+            // check goes on. A mismatch is reported behind the next barrier; until then the segment is handled as usual
+            // (its sizes are sound, its content is discarded with everything else when the flag is set)
         }
 
         // ---- 2: the solid slots, compacted to this iteration's list ------------------------------------------------------------
@@ -414,6 +415,7 @@ hash_count_kernel(HashCountArgs a) {
             if (lane == 0 && sum) atomicAdd(&s_sum, sum);
         }
         __syncthreads();
+        if constexpr (MW) { if (tid == 0 && s_clash) atomicOr(a.overflow, 16u); }
         u32 ns = s_nsolid;
         if (ns > (u32)MAXSOLID) { if (tid == 0) atomicOr(a.overflow, 4u); ns = 0; }
         if (full) ns = 0;
