@@ -56,9 +56,9 @@ struct ExtractArgs {
     // pair_keys[i] = top pair_top_bits bits of the first key word | fingerprint of the whole key below them (pair_key() in
     // common.cuh), and pair_idx[i] = i. The top passes then move 12 bytes per record instead of 8 W.
     u64 *pair_keys; u32 *pair_idx; u32 pair_top_bits;
-    // with pair_keys: a warp takes the 32 slots of ONE group per step (lane = slot) instead of a lane taking 32 consecutive
-    // slots, so that groups without a valid window are skipped warp-wide: for long keys on short reads (k = 99 on 150
-    // bases: a third of the slots start a window) the lanes of the other mapping idle two steps out of three
+    // with pair_keys, dense range: a warp takes the 32 slots of ONE group per step (lane = slot) instead of a lane taking 32
+    // consecutive slots: groups without a valid window are skipped warp-wide (at k = 99 on 150 bases a third of the slots
+    // start a window, and the lanes of the other mapping idle two steps out of three)
     bool by_rows;
 };
 int launch_extract(const ExtractArgs &a, DevState *st, cudaStream_t s);
