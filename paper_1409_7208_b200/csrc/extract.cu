@@ -490,9 +490,11 @@ __global__ void __launch_bounds__(256) extract_rows_kernel(ExtractArgs a, DevSta
                 const u64 pos = base + 2 * __popc(valid & lt);
                 store_key<W>(a.keys_out, pos, f);
                 store_key<W>(a.keys_out, pos + 1, r);
-                a.pair_keys[pos] = pair_key<W>(f, top_bits, weak);
-                a.pair_keys[pos + 1] = pair_key<W>(r, top_bits, weak);
-                *reinterpret_cast<uint2 *>(a.pair_idx + pos) = make_uint2((u32)pos, (u32)pos + 1u);   // pos is even
+                if (a.pair_keys) {
+                    a.pair_keys[pos] = pair_key<W>(f, top_bits, weak);
+                    a.pair_keys[pos + 1] = pair_key<W>(r, top_bits, weak);
+                    *reinterpret_cast<uint2 *>(a.pair_idx + pos) = make_uint2((u32)pos, (u32)pos + 1u);   // pos is even
+                }
                 const u32 fh = (u32)(f[0] >> 32), rh = (u32)(r[0] >> 32);
 #pragma unroll
                 for (u32 b = 7; b >= 4; --b) {
@@ -665,7 +667,7 @@ static int launch_extract_w(const ExtractArgs &a, DevState *st, cudaStream_t s) 
     if (filter) { extract_kernel<W, true, 0><<<(unsigned)blocks, 256, smem, s>>>(a, st); return (int)cudaGetLastError(); }
     if constexpr (W > 1) {
         if (a.by_rows) {
-            if (!a.pair_keys || !a.keys_out || !a.digit_hist || !a.hist_top || a.hist_top > 4 || a.want_csum || a.bucket_hist || a.coarse_hist)
+            if (!a.keys_out || !a.digit_hist || !a.hist_top || a.hist_top > 4 || a.want_csum || a.bucket_hist || a.coarse_hist)
                 return (int)cudaErrorInvalidValue;
             extract_rows_kernel<W><<<(unsigned)maxb, 256, smem, s>>>(a, st);
             return (int)cudaGetLastError();

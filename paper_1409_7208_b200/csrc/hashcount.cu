@@ -102,6 +102,10 @@ __device__ __forceinline__ void s_red_add(u32 addr, u32 v) {
 // record that did not install its slot (word by word against the record that did: two reads through the indices), and a
 // mismatch raises *overflow like everything else that does not fit, so the result stays exact. Records that are alone in
 // their slot (most of them at large k) are never read here at all.
+// Keys of TWO words are their own stand-ins: whole records (16 bytes against the 12 of a pair) go through the top passes, a.keys
+// holds them, sorted, a.vals is null, the fingerprint is made here when a record is loaded, and the check reads the record
+// that installed the slot a few hundred bytes away instead of somewhere in HBM — on reads where half of the records are
+// copies the random reads of the pair path cost more than the 4 extra bytes per pass.
 // 16 bytes of a record read at a random place: the L2 is told to fetch 64 bytes around it, not the 128 of its default
 __device__ __forceinline__ ulonglong2 ld_rec16(const u64 *p) {
     ulonglong2 v;
@@ -138,6 +142,7 @@ hash_count_kernel(HashCountArgs a) {
     static_assert(CB == 2 || CB == 4, "counts are 16-bit halves of u32 words or u32 words");
     constexpr int THREADS = WARPS * 32;
     constexpr bool MW = W > 1;
+    constexpr bool REC = W == 2;                         // a.keys holds the records themselves (W words each), no a.vals
     using rep_t = unsigned short;                                               // place of a record inside its segment
     constexpr size_t kOffCnt = (size_t)TSMAX * 8, kOffLKey = kOffCnt + (size_t)TSMAX * CB, kOffLCnt = kOffLKey + (size_t)MAXSOLID * 8;
     constexpr size_t kOffTRep = kOffLCnt + (size_t)MAXSOLID * 4, kOffLRep = kOffTRep + (MW ? (size_t)TSMAX * 2 : 0);
@@ -179,16 +184,33 @@ hash_count_kernel(HashCountArgs a) {
     auto load_group_v = [&](u64 (&k)[U][1], u32 (&v)[U], u64 first) {   // rows first + 32 u + lane of keys (and vals)
 #pragma unroll
         for (int u = 0; u < U; ++u) {
-            k[u][0] = ld_stream(a.keys + first + 32 * u + lane);
-            if constexpr (MW) v[u] = a.vals[first + 32 * u + lane]; else v[u] = 0;
+            if constexpr (REC) {
+                u64 rec[W];
+                load_key<W>(a.keys + (first + 32 * u + lane) * W, rec);
+                k[u][0] = pair_key<W>(rec, 0u, a.weak_fp);
+                v[u] = 0;
+            } else {
+                k[u][0] = ld_stream(a.keys + first + 32 * u + lane);
+                if constexpr (MW) v[u] = a.vals[first + 32 * u + lane]; else v[u] = 0;
+            }
         }
     };
+    // src = a.keys + (index of the first key): the index is what counts (records of W words in REC mode)
     auto load_group = [&](u64 (&k)[U][1], const u64 *src) { load_group_v(k, cur_v, (u64)(src - a.keys)); };
+    // the stand-in of the i-th key of the segment that starts at s0, from memory
+    auto key_at = [&](u64 s0, u32 i) -> u64 {
+        if constexpr (REC) { u64 rec[W]; load_key<W>(a.keys + (s0 + i) * W, rec); return pair_key<W>(rec, 0u, a.weak_fp); }
+        else return ld_stream(a.keys + s0 + i);
+    };
     // (W > 1) the record of the i-th key of the segment that starts at s0
-    auto rec_of = [&](u64 s0, u32 i) { return a.recs + (size_t)a.vals[s0 + i] * W; };
+    auto rec_of = [&](u64 s0, u32 i) -> const u64 * {
+        if constexpr (REC) return a.keys + (s0 + i) * W; else return a.recs + (size_t)a.vals[s0 + i] * W;
+    };
     // (W > 1) a key that met its slot taken will be compared with the record that installed it: its own record is asked
     // for now (into L2), while the rest of the segment is inserted
-    auto want_rec = [&](u32 v) { asm volatile("prefetch.global.L2 [%0];" ::"l"(a.recs + (size_t)v * W)); };
+    auto want_rec = [&](u32 v) {
+        if constexpr (!REC) asm volatile("prefetch.global.L2 [%0];" ::"l"(a.recs + (size_t)v * W));
+    };
     if (warp < groups_of(s, e)) load_group(cur, a.keys + s + (u64)warp * (32 * U));
 
     for (u32 it = 0;; ++it) {
@@ -212,11 +234,12 @@ hash_count_kernel(HashCountArgs a) {
             // loads of its insert phase, half of which are issued just before they are needed, then come from there
             const u64 pn_s = s_look[(it + 1) & 1][1], pn_e = s_look[(it + 1) & 1][2];
             if (pn_e > pn_s) {
-                const u64 p0 = (u64)(a.keys + pn_s) & ~15ull, p1 = ((u64)(a.keys + pn_e) + 15ull) & ~15ull;
+                constexpr u64 KW = REC ? W : 1;
+                const u64 p0 = (u64)(a.keys + pn_s * KW) & ~15ull, p1 = ((u64)(a.keys + pn_e * KW) + 15ull) & ~15ull;
                 asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(p0), "r"((u32)(p1 - p0)) : "memory");
             }
         }
-        if (tid == 32 % THREADS && m) { kf = a.keys[s]; kl = a.keys[e - 1]; }
+        if (tid == 32 % THREADS && m) { kf = a.keys[s * (REC ? W : 1)]; kl = a.keys[(e - 1) * (REC ? W : 1)]; }   // first words
         __syncthreads();
 
         // ---- 1: insert ---------------------------------------------------------------------------------------------------
@@ -300,8 +323,8 @@ hash_count_kernel(HashCountArgs a) {
                 const bool valid = i < m;
                 u64 key[1][1];
                 u32 kv[1];
-                key[0][0] = valid ? ld_stream(a.keys + s + i) : 0ull;
-                kv[0] = (MW && valid) ? a.vals[s + i] : 0u;
+                key[0][0] = valid ? key_at(s, i) : 0ull;
+                kv[0] = (MW && !REC && valid) ? a.vals[s + i] : 0u;
                 if (!MW && last_seg && valid && key[0][0] == kEmpty) { atomicAdd(&s_ones, 1u); insert_rows(std::integral_constant<int, 1>{}, key, kv, (row0 + x) * 32u, false); }
                 else insert_rows(std::integral_constant<int, 1>{}, key, kv, (row0 + x) * 32u, valid);
             }
@@ -333,7 +356,7 @@ hash_count_kernel(HashCountArgs a) {
                             u32 slot;
                             if (i < (u32)TSMAX) slot = s_slot[i];   // noted when the key was inserted
                             else {
-                                const u64 f = a.keys[s + i];
+                                const u64 f = key_at(s, i);
                                 u32 b8 = hash_slot(f, hshift) << 3;
                                 while (t_key[b8 >> 3] != f) b8 = (b8 + 8u) & mask8;   // it is there: the table was not full
                                 slot = b8 >> 3;
@@ -347,15 +370,22 @@ hash_count_kernel(HashCountArgs a) {
 #pragma unroll
                     for (int u = 0; u < VB; ++u) {
                         vi[u] = 0; vr[u] = 0;
-                        if ((need >> u) & 1u) { vi[u] = a.vals[s + i0 + (u32)u * THREADS]; vr[u] = a.vals[s + rep[u]]; }
+                        if constexpr (!REC) {
+                            if ((need >> u) & 1u) { vi[u] = a.vals[s + i0 + (u32)u * THREADS]; vr[u] = a.vals[s + rep[u]]; }
+                        }
                     }
                     bool same = true;
 #pragma unroll
                     for (int u = 0; u < VB; ++u) {
                         if ((need >> u) & 1u) {
                             u64 k[W], o[W];
-                            load_key<W>(a.recs + (size_t)vi[u] * W, k);
-                            load_key<W>(a.recs + (size_t)vr[u] * W, o);
+                            if constexpr (REC) {
+                                load_key<W>(a.keys + (s + i0 + (u32)u * THREADS) * W, k);
+                                load_key<W>(a.keys + (s + rep[u]) * W, o);
+                            } else {
+                                load_key<W>(a.recs + (size_t)vi[u] * W, k);
+                                load_key<W>(a.recs + (size_t)vr[u] * W, o);
+                            }
 #pragma unroll
                             for (int q = 0; q < W; ++q) same = same && o[q] == k[q];
                         }
@@ -649,7 +679,7 @@ int hash_setup() {
 
 void launch_hash_bounds(const HashCountArgs &a, cudaStream_t s) {
     const u64 warps = a.nseg + 1, blocks = (warps + 7) / 8;
-    hash_bounds_kernel<<<(unsigned)blocks, 256, 0, s>>>(a.keys, 1u, a.n, a.top_shift, a.chunk, a.window, a.nseg, a.seg_start, a.overflow);
+    hash_bounds_kernel<<<(unsigned)blocks, 256, 0, s>>>(a.keys, a.W == 2 ? 2u : 1u, a.n, a.top_shift, a.chunk, a.window, a.nseg, a.seg_start, a.overflow);
 }
 int launch_hash_count(const HashCountArgs &a, cudaStream_t s) {
     if (a.nseg == 0 || a.nseg > 0x7fffffffull || (u64)a.window + a.chunk >= 65536) return (int)cudaErrorInvalidValue;

@@ -127,7 +127,9 @@ struct HashCountArgs {
     const u64 *keys; u64 n;              // one word per record, sorted by key >> top_shift: the key itself (W = 1) or its
                                          // stand-in (ExtractArgs::pair_keys)
     u32 W;                               // words per record (0 = 1)
-    const u32 *vals; const u64 *recs;    // (W > 1) vals[i] = index of the record of keys[i] in recs (W words each, any order)
+    const u32 *vals; const u64 *recs;    // (W > 2) vals[i] = index of the record of keys[i] in recs (W words each, any order).
+                                         // W = 2: keys holds the sorted records themselves (2 words each), vals and recs are null
+    bool weak_fp;                        // (tests, W = 2) fingerprint = first word
     u32 top_shift, chunk, window;        // nominal records per segment; how far a bucket may run past a nominal border
     u32 d;                               // solid threshold, >= 2
     u64 nseg;                            // ceil(n / chunk)
