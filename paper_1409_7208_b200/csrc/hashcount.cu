@@ -20,15 +20,11 @@
 //     round trips long, and cost a quarter of the kernel's time; staging costs 24 bytes per solid edge of HBM traffic.
 // The first records of the NEXT segment are requested before step 2, so loads are in flight while a CTA sorts.
 // Nothing but the solid edges goes through any further pass. Segment borders are found by hash_bounds_kernel.
-// Whatever does not fit (a bucket longer than the search window, a full table, more solid edges than sort places)
-// raises *overflow; the caller then sorts the range the plain way (api_count.inc), so the result is the same.
+// Whatever does not fit (a bucket longer than the search window, a full table, more solid edges than sort places, two keys
+// of several words with one stand-in) raises *overflow; the caller then sorts the range the plain way (api_count.inc), so
+// the result is the same. Keys of several words: see "keys of W > 1 words" below.
 #include "kernels.cuh"
 #include <type_traits>
-#include <cstdio>
-
-#ifndef SDBG_HASH_CASFIRST
-#define SDBG_HASH_CASFIRST 0   // 1: the home slot is probed with the CAS itself; 0: with a load, CAS only into empty slots
-#endif
 
 namespace sdbg {
 

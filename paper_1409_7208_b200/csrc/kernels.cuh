@@ -52,7 +52,7 @@ struct ExtractArgs {
                                   // bits). Histogram-only call (nothing else set), k >= 8: counted in shared memory, no key is made
     int want_csum;
     PassTable passes;
-    // keys of several words on the table-count path: beside every record (same index) a sortable stand-in of one word,
+    // keys of three and four words on the table-count path: beside every record (same index) a sortable stand-in of one word,
     // pair_keys[i] = top pair_top_bits bits of the first key word | fingerprint of the whole key below them (pair_key() in
     // common.cuh), and pair_idx[i] = i. The top passes then move 12 bytes per record instead of 8 W.
     u64 *pair_keys; u32 *pair_idx; u32 pair_top_bits;
