@@ -643,11 +643,17 @@ struct HashShape {
 #ifndef SDBG_HASH_BIG_CB
 #define SDBG_HASH_BIG_CB 4
 #endif
+#ifndef SDBG_BIG_U
+#define SDBG_BIG_U 4
+#endif
+#ifndef SDBG_SMALL_U
+#define SDBG_SMALL_U 4
+#endif
 #ifndef SDBG_HASH_BIG
-#define SDBG_HASH_BIG 16, 2, 4, SDBG_HASH_BIG_TS, 1024, SDBG_HASH_BIG_CB
+#define SDBG_HASH_BIG 16, 2, SDBG_BIG_U, SDBG_HASH_BIG_TS, 1024, SDBG_HASH_BIG_CB
 #endif
 #ifndef SDBG_HASH_SMALL
-#define SDBG_HASH_SMALL 8, 4, 4, 4096, 1024, 2
+#define SDBG_HASH_SMALL 8, 4, SDBG_SMALL_U, 4096, 1024, 2
 #endif
 #ifndef SDBG_MW_WARPS
 #define SDBG_MW_WARPS 8
