@@ -152,26 +152,32 @@ hash_count_kernel(HashCountArgs a) {
     rep_t *l_rep = reinterpret_cast<rep_t *>(smem_raw + kOffLRep);              // (W > 1) rep_t[MAXSOLID]
     rep_t *s_slot = reinterpret_cast<rep_t *>(smem_raw + kOffSlot);
     __shared__ u32 s_ones, s_full, s_nsolid, s_distinct, s_clash;
-    __shared__ u64 s_sum, s_look[2][3], s_krange[2];
+    __shared__ u64 s_sum, s_look[2][4], s_krange[2];
     __shared__ u32 s_w[WARPS];
     const u32 tid = threadIdx.x, lane = tid & 31u, warp = tid >> 5;
     const u32 tkey_s = (u32)__cvta_generic_to_shared(smem_raw);
-    const u64 nseg = a.nseg;
+    // tickets run over the segments, or over the list of the non-empty ones (long buckets: a third of the nominal segments
+    // is empty there, and an iteration without records still costs its barriers and the latency of the look-ahead)
+    constexpr bool LIST = TSMAX > 4096;                  // the long-bucket shape
+    const u64 nseg = LIST ? (u64)*a.n_list : a.nseg;
 
     // Tickets are taken two segments ahead by thread 0, which also fetches the bounds of that segment while the CTA works:
     // s_look[p] = {segment, first record, end} of the iteration with parity p (nothing depends on a load it just issued).
-    auto bounds_of = [&](u64 sg, u64 &bs, u64 &be) { bs = be = 0; if (sg < nseg) { bs = a.seg_start[sg]; be = a.seg_start[sg + 1]; } };
+    auto bounds_of = [&](u64 t, u64 &id, u64 &bs, u64 &be) {   // ticket t -> segment id and its records [bs, be)
+        id = t; bs = be = 0;
+        if (t < nseg) { if constexpr (LIST) id = a.seg_list[t]; bs = a.seg_start[id]; be = a.seg_start[id + 1]; }
+    };
     if (tid == 0) {
         const u64 t0 = atomicAdd(a.ticket, 1u), t1 = atomicAdd(a.ticket, 1u);
-        u64 b0, e0, b1, e1;
-        bounds_of(t0, b0, e0); bounds_of(t1, b1, e1);
-        s_look[0][0] = t0; s_look[0][1] = b0; s_look[0][2] = e0;
-        s_look[1][0] = t1; s_look[1][1] = b1; s_look[1][2] = e1;
+        u64 i0, b0, e0, i1, b1, e1;
+        bounds_of(t0, i0, b0, e0); bounds_of(t1, i1, b1, e1);
+        s_look[0][0] = t0; s_look[0][1] = b0; s_look[0][2] = e0; s_look[0][3] = i0;
+        s_look[1][0] = t1; s_look[1][1] = b1; s_look[1][2] = e1; s_look[1][3] = i1;
     }
     __syncthreads();
-    u64 seg = s_look[0][0];
+    u64 seg = s_look[0][0];                              // the ticket; seg_id is the segment
     if (seg >= nseg) return;
-    u64 s = s_look[0][1], e = s_look[0][2];
+    u64 s = s_look[0][1], e = s_look[0][2], seg_id = s_look[0][3];
     // full groups of the segment [bs, be) (none for the segment that ends with the last record of all: it alone can hold
     // the all-ones key, which is counted beside the table by the row-by-row code)
     auto groups_of = [&](u64 bs, u64 be) { return be <= bs || be == a.n ? 0u : ((u32)(be - bs) >> 5) / (u32)U; };
@@ -221,7 +227,7 @@ hash_count_kernel(HashCountArgs a) {
             for (u32 i = tid; i < TS / 2; i += THREADS) k4[i] = ones;
             for (u32 i = tid; i < TS * CB / 16; i += THREADS) c4[i] = zero;
         }
-        u64 la_seg = 0, la_s = 0, la_e = 0;              // (thread 0) the segment of the iteration after the next one
+        u64 la_seg = 0, la_s = 0, la_e = 0, la_id = 0;   // (thread 0) the segment of the iteration after the next one
         u64 kf = 0, kl = 0;                              // (thread 32) first word of the first and of the last record
         if (tid == 0) {
             s_ones = 0; s_full = 0; s_nsolid = 0; s_distinct = 0; s_sum = 0; s_clash = 0;
@@ -326,12 +332,12 @@ hash_count_kernel(HashCountArgs a) {
             }
         }
         // the first records of my next segment are on their way while this one is finished (its bounds came an iteration ago)
-        const u64 next = s_look[(it + 1) & 1][0], ns_ = s_look[(it + 1) & 1][1], ne_ = s_look[(it + 1) & 1][2];
+        const u64 next = s_look[(it + 1) & 1][0], ns_ = s_look[(it + 1) & 1][1], ne_ = s_look[(it + 1) & 1][2], nid_ = s_look[(it + 1) & 1][3];
         if (!MW && next < nseg && warp < groups_of(ns_, ne_)) load_group(cur, a.keys + ns_ + (u64)warp * (32 * U));
         if (created) atomicAdd(&s_distinct, created);
         if (tid == 32 % THREADS) { s_krange[0] = kf >> a.top_shift; s_krange[1] = kl >> a.top_shift; }
         __syncthreads();
-        if (tid == 0) bounds_of(la_seg, la_s, la_e);     // stored at the end of the iteration
+        if (tid == 0) bounds_of(la_seg, la_id, la_s, la_e);   // stored at the end of the iteration
         const u64 kfirst = s_krange[0], klast = s_krange[1];
         const bool full = s_full != 0;
         if (full && tid == 0) atomicOr(a.overflow, 2u);
@@ -447,9 +453,9 @@ hash_count_kernel(HashCountArgs a) {
         if (full) ns = 0;
         // ---- 3a: the count of the segment, the sum of its block, statistics ---------------------------------------------------------
         if (tid == 0) {
-            a.seg_count[seg] = ns;
-            if (ns) atomicAdd(a.blk_sum + seg / kSegBlock, (u64)ns);
-            u64 *slot = a.stat_slots + (size_t)(seg & (kStatSlots - 1)) * kStatSlotWords;
+            a.seg_count[seg_id] = ns;
+            if (ns) atomicAdd(a.blk_sum + seg_id / kSegBlock, (u64)ns);
+            u64 *slot = a.stat_slots + (size_t)(seg_id & (kStatSlots - 1)) * kStatSlotWords;
             if (ns) atomicAdd(&slot[1], s_sum);
             if (s_distinct && !full) atomicAdd(&slot[0], (u64)s_distinct);
         }
@@ -541,10 +547,24 @@ hash_count_kernel(HashCountArgs a) {
             }
         }
         if (next >= nseg) break;
-        if (tid == 0) { s_look[it & 1][0] = la_seg; s_look[it & 1][1] = la_s; s_look[it & 1][2] = la_e; }
-        seg = next; s = ns_; e = ne_;
+        if (tid == 0) { s_look[it & 1][0] = la_seg; s_look[it & 1][1] = la_s; s_look[it & 1][2] = la_e; s_look[it & 1][3] = la_id; }
+        seg = next; s = ns_; e = ne_; seg_id = nid_;
         __syncthreads();   // the table is cleared next
     }
+}
+
+// seg_list[0 .. *n_list) = the segments with records (long buckets only). Nearly in order: a warp appends the non-empty ones
+// of its 32 segments at a place taken from *n_list; the order in which segments are counted is free (every segment writes
+// to its own places).
+__global__ void __launch_bounds__(256) hash_list_kernel(const u64 *__restrict__ seg_start, u64 nseg, u32 *__restrict__ seg_list, u32 *n_list) {
+    const u64 c = (u64)blockIdx.x * blockDim.x + threadIdx.x;
+    const bool has = c < nseg && seg_start[c] < seg_start[c + 1];
+    const u32 b = __ballot_sync(0xffffffffu, has);
+    if (b == 0) return;
+    u32 base = 0;
+    if (lane_id() == 0) base = atomicAdd(n_list, (u32)__popc(b));
+    base = __shfl_sync(0xffffffffu, base, 0);
+    if (has) seg_list[base + (u32)__popc(b & lanemask_lt())] = (u32)c;
 }
 
 // blk_sum[b] (solid edges of segments [64 b, 64 b + 64)) -> exclusive prefix in place, total to *total and the output
@@ -681,7 +701,9 @@ int hash_setup() {
 
 void launch_hash_bounds(const HashCountArgs &a, cudaStream_t s) {
     const u64 warps = a.nseg + 1, blocks = (warps + 7) / 8;
+    if (a.seg_list) cudaMemsetAsync(a.seg_count, 0, a.nseg * 8, s);   // the empty segments are never visited
     hash_bounds_kernel<<<(unsigned)blocks, 256, 0, s>>>(a.keys, a.W == 2 ? 2u : 1u, a.n, a.top_shift, a.chunk, a.window, a.nseg, a.seg_start, a.overflow);
+    if (a.seg_list) hash_list_kernel<<<(unsigned)((a.nseg + 255) / 256), 256, 0, s>>>(a.seg_start, a.nseg, a.seg_list, a.n_list);
 }
 int launch_hash_count(const HashCountArgs &a, cudaStream_t s) {
     if (a.nseg == 0 || a.nseg > 0x7fffffffull || (u64)a.window + a.chunk >= 65536) return (int)cudaErrorInvalidValue;

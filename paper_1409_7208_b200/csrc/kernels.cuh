@@ -135,6 +135,7 @@ struct HashCountArgs {
     u64 nseg;                            // ceil(n / chunk)
     u64 *seg_start;                      // u64[nseg + 1] scratch
     u64 *seg_count;                      // u64[nseg] scratch: solid edges per segment
+    u32 *seg_list; u32 *n_list;          // null, or u32[nseg] + one word of scratch: the non-empty segments (long buckets)
     u64 *blk_sum;                        // u64[ceil(nseg / 64)] scratch, zeroed: solid edges per block of 64 segments, then their prefix
     u64 *stage_keys;                     // u64[n W] scratch (the sorter's spare buffer, or the second record buffer)
     u32 *ticket;                         // zeroed: segments are handed out in order
