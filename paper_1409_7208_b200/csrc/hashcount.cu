@@ -132,7 +132,7 @@ __device__ __forceinline__ bool rest_less(const u64 *__restrict__ ra, const u64 
 // places, NB = 1024 bins. Counts are 16-bit halves of u32 words (a segment has at most window + chunk < 65,536 records).
 // The records of a segment are dealt to the warps in groups of U full rows (no lane is ever idle there, so the group
 // code has no predicates); the rows that do not fill a group and the partial last row go one by one.
-template <int W, int WARPS, int MINB, int U, int TSMAX, int MAXSOLID, int CB>
+template <int W, int WARPS, int MINB, int U, int TSMAX, int MAXSOLID, int CB, bool LIST = false>
 __global__ void __launch_bounds__(WARPS * 32, MINB)
 hash_count_kernel(HashCountArgs a) {
     static_assert(CB == 2 || CB == 4, "counts are 16-bit halves of u32 words or u32 words");
@@ -158,7 +158,6 @@ hash_count_kernel(HashCountArgs a) {
     const u32 tkey_s = (u32)__cvta_generic_to_shared(smem_raw);
     // tickets run over the segments, or over the list of the non-empty ones (long buckets: a third of the nominal segments
     // is empty there, and an iteration without records still costs its barriers and the latency of the look-ahead)
-    constexpr bool LIST = TSMAX > 4096;                  // the long-bucket shape
     const u64 nseg = LIST ? (u64)*a.n_list : a.nseg;
 
     // Tickets are taken two segments ahead by thread 0, which also fetches the bounds of that segment while the CTA works:
@@ -641,19 +640,19 @@ __global__ void __launch_bounds__(256) hash_copy_kernel(HashCountArgs a) {
 }
 
 // shapes: long buckets (chunk 4,096: one or two buckets per segment) and short ones (chunk 2,048: many buckets per segment)
-template <int W, int WARPS, int MINB, int U, int TSMAX, int MAXSOLID, int CB>
+template <int W, int WARPS, int MINB, int U, int TSMAX, int MAXSOLID, int CB, bool LIST = false>
 struct HashShape {
     static constexpr int THREADS = WARPS * 32;
     static constexpr size_t kSmem = (size_t)TSMAX * (8 + CB) + (size_t)MAXSOLID * 12 + (W > 1 ? (size_t)TSMAX * 4 + (size_t)MAXSOLID * 2 : 0);
     static int setup(int *blocks_per_sm) {
-        int e = (int)cudaFuncSetAttribute(hash_count_kernel<W, WARPS, MINB, U, TSMAX, MAXSOLID, CB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmem);
+        int e = (int)cudaFuncSetAttribute(hash_count_kernel<W, WARPS, MINB, U, TSMAX, MAXSOLID, CB, LIST>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmem);
         if (e) return e;
-        return (int)cudaOccupancyMaxActiveBlocksPerMultiprocessor(blocks_per_sm, hash_count_kernel<W, WARPS, MINB, U, TSMAX, MAXSOLID, CB>, THREADS, kSmem);
+        return (int)cudaOccupancyMaxActiveBlocksPerMultiprocessor(blocks_per_sm, hash_count_kernel<W, WARPS, MINB, U, TSMAX, MAXSOLID, CB, LIST>, THREADS, kSmem);
     }
     static int launch(const HashCountArgs &a, int blocks_per_sm, cudaStream_t s) {
         u64 g = (u64)num_sms() * (u64)(blocks_per_sm > 0 ? blocks_per_sm : 1);
         if (g > a.nseg) g = a.nseg;
-        hash_count_kernel<W, WARPS, MINB, U, TSMAX, MAXSOLID, CB><<<(unsigned)g, THREADS, kSmem, s>>>(a);
+        hash_count_kernel<W, WARPS, MINB, U, TSMAX, MAXSOLID, CB, LIST><<<(unsigned)g, THREADS, kSmem, s>>>(a);
         return (int)cudaGetLastError();
     }
 };
@@ -683,7 +682,7 @@ struct HashShape {
 #ifndef SDBG_HASH_MW   // keys of several words (one-word stand-ins with an index payload): short buckets only
 #define SDBG_HASH_MW SDBG_MW_WARPS, SDBG_MW_MINB, SDBG_MW_U, 4096, 1024, 2
 #endif
-using HashBig = HashShape<1, SDBG_HASH_BIG>;
+using HashBig = HashShape<1, SDBG_HASH_BIG, true>;       // always over the list of the non-empty segments
 using HashSmall = HashShape<1, SDBG_HASH_SMALL>;
 using HashMW2 = HashShape<2, SDBG_HASH_MW>;
 using HashMW3 = HashShape<3, SDBG_HASH_MW>;
@@ -716,7 +715,8 @@ int launch_hash_count(const HashCountArgs &a, cudaStream_t s) {
         }
         return (int)cudaErrorInvalidValue;
     }
-    return a.chunk >= 4096 ? HashBig::launch(a, g_occ_big, s) : HashSmall::launch(a, g_occ_small, s);
+    if (a.chunk >= 4096) return a.seg_list ? HashBig::launch(a, g_occ_big, s) : (int)cudaErrorInvalidValue;
+    return a.seg_list ? (int)cudaErrorInvalidValue : HashSmall::launch(a, g_occ_small, s);
 }
 void launch_hash_append(const HashCountArgs &a, u64 *total, cudaStream_t s) {
     const u64 nblk = (a.nseg + kSegBlock - 1) / kSegBlock;
