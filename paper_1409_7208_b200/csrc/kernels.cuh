@@ -88,6 +88,8 @@ struct RadixArgs {
     u32 *ticket;                         // zeroed
     PassDesc pass; u32 epoch;
     bool force_wide;                     // use the layout for ranges of 2^32 records and more whatever n is (tests)
+    bool maybe_unstable; u32 sorted_lo;  // a LATER pass of such a sort (same contract as `unstable`, (b) above all): the input is sorted by key
+                                         // bits [sorted_lo, pass.shift); tiles whose keys all agree in them are ranked by arrival
     bool unstable;                       // CONTRACT: set only when (a) this is pass 0 of a multi-pass sort whose input order carries no
                                          // information AND (b) the caller merges equal keys afterwards (sdbg_count_edges). The pass then
                                          // need not keep the order of equal digits (radix.cu FIRST: rank = return value of the count atomic,

@@ -292,7 +292,7 @@ __device__ __forceinline__ void stage_get(const u64 *base, u32 pos, u64 (&k)[W])
 // FIRST: the first pass of a sort. Its input order is arbitrary, so the pass need not be stable: the rank of a key
 // inside (warp, digit) is what the count atomic returned, and the match step of phase 3 is not needed (full tiles
 // only: the pads of the last tile rely on the stable order).
-template <int W, bool HAS_VAL, bool HI, bool WIDE, bool FIRST = false>
+template <int W, bool HAS_VAL, bool HI, bool WIDE, bool FIRST = false, bool MAYBE = false>
 __global__ void __launch_bounds__(RadixCfg<W, HAS_VAL>::THREADS, RadixCfg<W, HAS_VAL>::MINB)
 onesweep_kernel(RadixArgs a) {
     using L = RadixSmem<W, HAS_VAL>;
@@ -355,17 +355,31 @@ onesweep_kernel(RadixArgs a) {
     };
     auto tile_count = [&](u32 t) { return (a.n - (u64)t * TILE < (u64)TILE) ? (u32)(a.n - (u64)t * TILE) : (u32)TILE; };
     // phase 1: digits of the keys in registers -> warp-private histogram
-    u32 rkp[FIRST ? (KPT + 1) / 2 : 1];   // FIRST: arrival rank inside (warp, digit), 16 bits each
+    // MAYBE: a later pass of a sort whose equal keys are merged afterwards (RadixArgs::sorted_lo). The order of equal digits
+    // matters only where the bits sorted so far differ; a full tile whose first and last key agree in them (the input is
+    // sorted by them, so all its keys do) is ranked like FIRST, the others the stable way.
+    constexpr bool RK = FIRST || MAYBE;
+    u32 rkp[RK ? (KPT + 1) / 2 : 1];      // arrival rank inside (warp, digit), 16 bits each
+    bool uni = false;                     // the tile counted last is ranked by arrival
+    auto tile_free = [&](u32 t, u32 c) -> bool {
+        if (c != (u32)TILE) return false;                 // the pads of the last tile rely on the stable order
+        if constexpr (FIRST) return true;
+        const u64 kf = a.keys_in[(u64)t * TILE * W], kl = a.keys_in[((u64)t * TILE + TILE - 1) * W];
+        return (((kf ^ kl) >> a.sorted_lo) << (64u - (a.pass.shift - a.sorted_lo))) == 0;   // bits [sorted_lo, pass.shift) agree
+    };
     auto count_keys = [&]() {
+        if constexpr (RK) {
+            if (uni) {
 #pragma unroll
-        for (int j = 0; j < KPT; ++j) {
-            if constexpr (FIRST) {
-                const u32 r = atomicAdd(&wp[digit8<W, HI>(key[j], word, psel)], 1u);
-                if (j & 1) rkp[j / 2] |= r << 16; else rkp[j / 2] = r;
-            } else {
-                atomicAdd(&wp[digit8<W, HI>(key[j], word, psel)], 1u);
+                for (int j = 0; j < KPT; ++j) {
+                    const u32 r = atomicAdd(&wp[digit8<W, HI>(key[j], word, psel)], 1u);
+                    if (j & 1) rkp[j / 2] |= r << 16; else rkp[j / 2] = r;
+                }
+                return;
             }
         }
+#pragma unroll
+        for (int j = 0; j < KPT; ++j) atomicAdd(&wp[digit8<W, HI>(key[j], word, psel)], 1u);
     };
     // phase 2a (one thread per bin, after a block barrier): tile count, published LOCAL at once; scan over the bins
     u32 my_cnt = 0, incl = 0;
@@ -425,6 +439,7 @@ onesweep_kernel(RadixArgs a) {
     u32 cnt = tile_count(tile);
     load_tile<W, HAS_VAL, KPT>(a, (u64)tile * TILE, cnt, wbase, key, val);
     reserve_next();
+    if constexpr (RK) uni = tile_free(tile, cnt);
     count_keys();
     __syncthreads();
     if (scanner) scan_bins(tile, cnt);
@@ -437,8 +452,8 @@ onesweep_kernel(RadixArgs a) {
         const u32 next = SDBG_PERSISTENT ? s_tick[(it + 1) & 1] : ntiles;
         // ---- 3: rank within the warp (stable in tile order), scatter to shared memory in bin-sorted order ------
         bool ranked = false;
-        if constexpr (FIRST) {
-            if (cnt == (u32)TILE) {
+        if constexpr (RK) {
+            if (uni) {
                 ranked = true;
 #pragma unroll
                 for (int j = 0; j < KPT; ++j) {
@@ -489,6 +504,7 @@ onesweep_kernel(RadixArgs a) {
             cnt = tile_count(next);
             load_tile<W, HAS_VAL, KPT>(a, (u64)next * TILE, cnt, wbase, key, val);
             ++it; reserve_next(); --it;
+            if constexpr (RK) uni = tile_free(next, cnt);
             count_keys();
         }
         __syncthreads();
@@ -538,6 +554,18 @@ static int setup_one() {
         e = (int)cudaFuncSetAttribute(onesweep_kernel<1, false, false, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
         if (e) return e;
         e = (int)cudaFuncSetAttribute(onesweep_kernel<1, false, true, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
+        if (e) return e;
+        e = (int)cudaFuncSetAttribute(onesweep_kernel<1, false, false, false, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
+        if (e) return e;
+        e = (int)cudaFuncSetAttribute(onesweep_kernel<1, false, true, false, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
+        if (e) return e;
+        e = (int)cudaFuncSetAttribute(onesweep_kernel<1, false, false, true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
+        if (e) return e;
+        e = (int)cudaFuncSetAttribute(onesweep_kernel<1, false, true, true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
+        if (e) return e;
+        e = (int)cudaFuncSetAttribute(onesweep_kernel<1, false, false, true, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
+        if (e) return e;
+        e = (int)cudaFuncSetAttribute(onesweep_kernel<1, false, true, true, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
         if (e) return e;
     }
     e = (int)cudaFuncSetAttribute(onesweep_kernel<W, false, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
@@ -596,6 +624,20 @@ static int launch_one(const RadixArgs &a, cudaStream_t s) {
     const bool hi = a.pass.shift >= 32;
     if constexpr (!HAS_VAL) {
         if (wide) {
+            if constexpr (W == 1) {                      // the same two unstable variants with wide look-back words
+                if (a.unstable) {
+                    ++g_unstable_launches;
+                    if (hi) onesweep_kernel<1, false, true, true, true><<<g, t, sm, s>>>(a);
+                    else    onesweep_kernel<1, false, false, true, true><<<g, t, sm, s>>>(a);
+                    return (int)cudaGetLastError();
+                }
+                if (a.maybe_unstable && a.sorted_lo < a.pass.shift) {
+                    ++g_unstable_launches;
+                    if (hi) onesweep_kernel<1, false, true, true, false, true><<<g, t, sm, s>>>(a);
+                    else    onesweep_kernel<1, false, false, true, false, true><<<g, t, sm, s>>>(a);
+                    return (int)cudaGetLastError();
+                }
+            }
             if (hi) onesweep_kernel<W, false, true, true><<<g, t, sm, s>>>(a);
             else    onesweep_kernel<W, false, false, true><<<g, t, sm, s>>>(a);
             return (int)cudaGetLastError();
@@ -606,6 +648,12 @@ static int launch_one(const RadixArgs &a, cudaStream_t s) {
             ++g_unstable_launches;
             if (hi) onesweep_kernel<1, false, true, false, true><<<g, t, sm, s>>>(a);
             else    onesweep_kernel<1, false, false, false, true><<<g, t, sm, s>>>(a);
+            return (int)cudaGetLastError();
+        }
+        if (a.maybe_unstable && a.sorted_lo < a.pass.shift) {
+            ++g_unstable_launches;
+            if (hi) onesweep_kernel<1, false, true, false, false, true><<<g, t, sm, s>>>(a);
+            else    onesweep_kernel<1, false, false, false, false, true><<<g, t, sm, s>>>(a);
             return (int)cudaGetLastError();
         }
     }
