@@ -546,6 +546,13 @@ onesweep_kernel(RadixArgs a) {
 template <int W, bool HAS_VAL>
 static int setup_one() {
     const int bytes = (int)RadixSmem<W, HAS_VAL>::kBytes;
+    if constexpr (W == 1 || (W == 2 && !HAS_VAL)) {      // the unstable variants (narrow look-back words)
+        int e2;
+        if ((e2 = (int)cudaFuncSetAttribute(onesweep_kernel<W, HAS_VAL, false, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes))) return e2;
+        if ((e2 = (int)cudaFuncSetAttribute(onesweep_kernel<W, HAS_VAL, true, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes))) return e2;
+        if ((e2 = (int)cudaFuncSetAttribute(onesweep_kernel<W, HAS_VAL, false, false, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes))) return e2;
+        if ((e2 = (int)cudaFuncSetAttribute(onesweep_kernel<W, HAS_VAL, true, false, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes))) return e2;
+    }
     int e = (int)cudaFuncSetAttribute(onesweep_kernel<W, HAS_VAL, false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
     if (e) return e;
     e = (int)cudaFuncSetAttribute(onesweep_kernel<W, HAS_VAL, true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
@@ -643,17 +650,18 @@ static int launch_one(const RadixArgs &a, cudaStream_t s) {
             return (int)cudaGetLastError();
         }
     }
-    if constexpr (W == 1 && !HAS_VAL) {
+    // one-word keys (with or without payload: the stand-in pairs of long keys) and two-word records: the unstable variants
+    if constexpr (W == 1 || (W == 2 && !HAS_VAL)) {
         if (a.unstable) {
             ++g_unstable_launches;
-            if (hi) onesweep_kernel<1, false, true, false, true><<<g, t, sm, s>>>(a);
-            else    onesweep_kernel<1, false, false, false, true><<<g, t, sm, s>>>(a);
+            if (hi) onesweep_kernel<W, HAS_VAL, true, false, true><<<g, t, sm, s>>>(a);
+            else    onesweep_kernel<W, HAS_VAL, false, false, true><<<g, t, sm, s>>>(a);
             return (int)cudaGetLastError();
         }
-        if (a.maybe_unstable && a.sorted_lo < a.pass.shift) {
+        if (a.maybe_unstable && a.sorted_lo < a.pass.shift && a.pass.word == 0) {
             ++g_unstable_launches;
-            if (hi) onesweep_kernel<1, false, true, false, false, true><<<g, t, sm, s>>>(a);
-            else    onesweep_kernel<1, false, false, false, false, true><<<g, t, sm, s>>>(a);
+            if (hi) onesweep_kernel<W, HAS_VAL, true, false, false, true><<<g, t, sm, s>>>(a);
+            else    onesweep_kernel<W, HAS_VAL, false, false, false, true><<<g, t, sm, s>>>(a);
             return (int)cudaGetLastError();
         }
     }
